@@ -1,0 +1,350 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Wilson-Dirac matvec D*psi (eq. (2.2)) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--kernel auto|site|tile]
+                    [--recon 18|12] [--impl wd|reference]
+
+One JSON line on stdout (rank 0).  Definitions:
+  * workload   default c3_32x64_fp32 = BASELINE.json:configs[3], the configuration the metric is
+               quoted on: 32^3x64, fp32, smooth links, m=-0.42, single RHS, 18-real links.
+  * step       the Krylov-loop batch of configs[3]: APPLIES_PER_STEP (=100) wd_apply calls back to
+               back on one stream with no host sync, rotating through NBUF distinct input and
+               output fields (reading S9: not a chain D^100 psi, which overflows fp32).
+  * value      Gflop/s at 1368 flops/site/RHS (1320 hopping + 48 diagonal), all ranks together,
+               inputs resident in HBM, timed with CUDA events on the launching stream, max over ranks.
+  * L2         gauge (604 MB) + rotating spinors exceed the 126 MB L2, so no flush is needed
+               ("inputs larger than L2" in config.l2).
+  * e2e        the same metric through wd_apply_host: pinned HOST buffers in canonical layout,
+               H2D copy + pack + apply + unpack + D2H copy + sync inside the timed region.
+  * roofline   HBM: algorithmic (compulsory) bytes per launch / mean launch duration, against
+               MEASURED_PEAKS.json:hbm_gbs.
+  * cpu_baseline  the oracle (oracle/wd_oracle.c, fp64, OpenMP) on this box's host cores, on a
+               bounded sample of the same workload.
+Multi-GPU (torchrun): the path has no exchange step on one GPU per lattice; ranks run independent
+replicas of the workload (different seeds), no data-path collective; scaling "weak".
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_0912_2186_b200 import fields  # noqa: E402  (seeded generators only; no arithmetic of the method)
+
+APPLIES_PER_STEP = 100
+NBUF = 4
+FLOPS_PER_SITE = 1368
+METRIC = "wilson_dslash_gflops"
+UNIT = "Gflop/s"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def compulsory_bytes_per_site(precision, recon, nrhs):
+    """Algorithmic HBM bytes per site per launch: every spinor read once and
+    written once, every link read once."""
+    w = 4 if precision == 32 else 8
+    return nrhs * 2 * 24 * w + 4 * recon * w
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json:hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(workload, recon):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    try:
+        return json.load(open(p)).get(f"{workload}_r{recon}", {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """Samples SM clock and clock-event (throttle) reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    NAMES = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+             0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+             0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in self.NAMES.items():
+                    if mask & bit and name != "gpu_idle":
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+
+    def summary(self):
+        return {"sm_mhz": (float(np.median(self.samples)) if self.samples else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    return rank, local, world
+
+
+def oracle_rate(cfg, U, psi, budget_s=12.0):
+    """Time the oracle as it stands on a bounded sample: whole-lattice applies of RHS 0, repeated
+    until ~budget_s of CPU work (at least 1, at most 8).  Returns the cpu_baseline object."""
+    from oracle import wd_oracle
+    U64 = np.ascontiguousarray(U if cfg.recon == 18 else U[..., :2, :, :], dtype=np.float64)
+    p64 = np.ascontiguousarray(psi[0], dtype=np.float64)
+    V = fields.volume(cfg.dims)
+    # calibrate on a slab so a slow box cannot run away
+    n0 = max(1, V // 16)
+    t0 = time.perf_counter()
+    wd_oracle.apply_range(p64, U64, cfg.dims, cfg.mass, 0, n0)
+    rate = n0 / (time.perf_counter() - t0)
+    n = int(min(V, max(n0, rate * budget_s / 3)))
+    best = None
+    reps = 0
+    t_all = time.perf_counter()
+    while reps < 8 and (reps < 1 or time.perf_counter() - t_all < budget_s):
+        t0 = time.perf_counter()
+        wd_oracle.apply_range(p64, U64, cfg.dims, cfg.mass, 0, n)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+        reps += 1
+    return {"value": n * FLOPS_PER_SITE / best / 1e9, "unit": UNIT, "cores": wd_oracle.num_threads(),
+            "kind": "oracle", "sites_per_s": n / best,
+            "sample": f"fp64 oracle, first {n} of {V} sites of {cfg.name} (1 RHS), best of {reps} passes"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores (rank 0 only), same metric/config/unit."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    from oracle import wd_oracle
+    cfg = fields.CONFIGS[args.workload]
+    U, psi = fields.make_fields(cfg, nrhs=1)
+    U64 = np.ascontiguousarray(U if args.recon == 18 else U[..., :2, :, :], dtype=np.float64)
+    p64 = np.ascontiguousarray(psi[0], dtype=np.float64)
+    V = fields.volume(cfg.dims)
+    n0 = max(1, V // 32)
+    t0 = time.perf_counter()
+    wd_oracle.apply_range(p64, U64, cfg.dims, cfg.mass, 0, n0)
+    rate = n0 / (time.perf_counter() - t0)
+    # each step: a bounded sample of ~1 s so that steps+warmup end within a few minutes
+    n = int(min(V, max(1024, rate * min(1.0, 120.0 / max(1, args.steps + args.warmup)))))
+    for _ in range(args.warmup):
+        wd_oracle.apply_range(p64, U64, cfg.dims, cfg.mass, 0, n)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        wd_oracle.apply_range(p64, U64, cfg.dims, cfg.mass, 0, n)
+    dt = time.perf_counter() - t0
+    value = args.steps * n * FLOPS_PER_SITE / dt / 1e9
+    sample = f"fp64 oracle, first {n} of {V} sites of {cfg.name} (1 RHS) per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "dims": list(cfg.dims), "recon": args.recon, "nrhs": 1,
+                   "flops_per_site": FLOPS_PER_SITE, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": wd_oracle.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_wd(args):
+    import torch
+    from paper_0912_2186_b200 import binding, build
+
+    rank, local, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    build.build()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg = fields.CONFIGS[args.workload]
+    recon = args.recon
+    nrhs = cfg.nrhs
+    V = fields.volume(cfg.dims)
+    tdt = torch.float32 if cfg.precision == 32 else torch.float64
+    kernel = {"auto": binding.WD_KERNEL_AUTO, "site": binding.WD_KERNEL_SITE, "tile": binding.WD_KERNEL_TILE}[args.kernel]
+
+    # ---- synthetic inputs (each rank its own replica: seeds shifted by rank) -------------------
+    cfg_r = fields.Config(cfg.name, cfg.dims, cfg.precision, cfg.links, recon, cfg.mass, nrhs, cfg.seed + 100 * rank,
+                          cfg.eps)
+    U, psi = fields.make_fields(cfg_r)
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        u_dev = torch.from_numpy(U).to(dev)
+        op = binding.WilsonDirac(cfg.dims, u_dev, cfg.precision, recon, stream=stream.cuda_stream, kernel=kernel)
+        canon = torch.from_numpy(psi).to(dev)
+        ins = [torch.empty(nrhs * V * 24, dtype=tdt, device=dev) for _ in range(NBUF)]
+        outs = [torch.empty(nrhs * V * 24, dtype=tdt, device=dev) for _ in range(NBUF)]
+        op.pack(ins[0], canon, nrhs)
+        for b in range(1, NBUF):  # distinct inputs: scaled copies of the packed field
+            torch.mul(ins[0], 1.0 + 0.25 * b, out=ins[b])
+    stream.synchronize()
+    del u_dev, canon
+
+    aps = args.applies_per_step
+
+    def step():
+        for i in range(aps):
+            op.apply(outs[i % NBUF], ins[i % NBUF], cfg.mass, nrhs)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing ---------------------------------------------------------------
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    n0 = binding.wd_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clocks:
+        ev0.record(stream)
+        for _ in range(args.steps):
+            step()
+        ev1.record(stream)
+        barrier()
+    launches = binding.wd_launch_count() - n0
+    ms = ev0.elapsed_time(ev1)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    applies = args.steps * aps
+    flops_per_apply = FLOPS_PER_SITE * V * nrhs
+    value = world * applies * flops_per_apply / (ms * 1e-3) / 1e9
+    launch_ms = ms / applies
+    bytes_per_launch = compulsory_bytes_per_site(cfg.precision, recon, nrhs) * V
+    peak, peak_src = measured_peak()
+    achieved = bytes_per_launch / (launch_ms * 1e-3) / 1e9
+
+    # ---- end to end through wd_apply_host (pinned host buffers, copies inside the timed region) -
+    e2e_applies = max(2, min(args.steps, 5))
+    h_in = torch.from_numpy(psi).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    for _ in range(2):
+        op.apply_host(h_out, h_in, cfg.mass, nrhs)
+    barrier()
+    t0 = time.perf_counter()  # wd_apply_host synchronises its stream before returning: wall clock is exact
+    for _ in range(e2e_applies):
+        op.apply_host(h_out, h_in, cfg.mass, nrhs)
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    if world > 1:
+        t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_value = world * e2e_applies * flops_per_apply / (e2e_ms * 1e-3) / 1e9
+    field_bytes = nrhs * V * 24 * (4 if cfg.precision == 32 else 8)
+
+    line = None
+    if rank == 0:
+        cpu = oracle_rate(cfg_r, U, psi) if (world == 1 and not args.no_cpu_baseline) else None
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if cfg.precision == 32 else "f64",
+            "data": "synthetic",
+            "config": {"workload": cfg.name, "dims": list(cfg.dims), "links": cfg.links, "recon": recon, "nrhs": nrhs,
+                       "mass": cfg.mass, "kernel": args.kernel, "applies_per_step": aps,
+                       "rotating_buffers": NBUF, "flops_per_site": FLOPS_PER_SITE,
+                       "gflops_at_1320_per_site": value * 1320.0 / FLOPS_PER_SITE,
+                       "l2": "inputs larger than L2 (gauge + rotating spinor fields), no flush",
+                       "parallelism": "independent replicas, no collective" if world > 1 else "single GPU"},
+            "us_per_apply": launch_ms * 1e3,
+            "clocks": clocks.summary(),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": field_bytes * aps,
+                    "d2h_bytes_per_step": field_bytes * aps, "applies_timed": e2e_applies,
+                    "ms_per_apply": e2e_ms / e2e_applies,
+                    "note": "wd_apply_host per apply: H2D + pack + apply + unpack + D2H + sync; bytes are per "
+                            "100-apply step"},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": ncu_traffic(cfg.name, recon), "peak_source": peak_src,
+                         "bytes_per_launch": bytes_per_launch, "kernel": "wd dslash (" + args.kernel + ")"},
+        }
+        if cpu is not None:
+            line["cpu_baseline"] = cpu
+        print(json.dumps(line), flush=True)
+    op.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return line
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="c3_32x64_fp32", choices=sorted(fields.CONFIGS))
+    ap.add_argument("--kernel", default="auto", choices=["auto", "site", "tile"])
+    ap.add_argument("--recon", type=int, default=None, choices=[18, 12])
+    ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--applies-per-step", type=int, default=APPLIES_PER_STEP,
+                    help="wd_apply calls per step (default 100 = configs[3]; lower it only for profiling)")
+    args = ap.parse_args()
+    if args.recon is None:
+        args.recon = fields.CONFIGS[args.workload].recon
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_wd(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,164 @@
+/*
+ * wd.h -- C ABI of the B200-native Wilson-Dirac matvec library (libwd.so).
+ *
+ * The one operation: apply the fine Wilson-Dirac operator of eq. (2.2) of arXiv:0912.2186
+ * (section 2) to one or several spinor fields on a periodic 4-D lattice,
+ *
+ *   (D psi)(x) = (4+m) psi(x)
+ *              - 1/2 sum_{mu=1..4} [ (1 - gamma_mu) (x) U_mu(x)        psi(x+mu)     forward hop
+ *                                  + (1 + gamma_mu) (x) U_mu(x-mu)^dag psi(x-mu) ]   backward hop
+ *
+ * gamma_mu in the DeGrand-Rossi basis (reading S2), gamma on spin, U on colour,
+ * x +- mu modulo L_mu (periodic, no phase; reading S3).  The "many test vectors, same links"
+ * use of the adaptive set-up (eq. (2.6); N_v = 20) is the
+ * nrhs > 1 case: out[r] = D in[r] for r < nrhs, one link load shared by all r.
+ *
+ * Everything is plain C: opaque handles, raw pointers, ints and doubles.  No torch types.
+ * Every pointer named *_dev is a CUDA DEVICE pointer owned by the caller (e.g. the data_ptr()
+ * of a torch tensor); every pointer named *_host is HOST memory owned by the caller.  The
+ * library never frees caller memory and keeps no reference to it after the call returns,
+ * except that work enqueued on the stream still reads/writes it until the stream reaches
+ * that point: keep buffers alive until you synchronise.
+ *
+ * Error behaviour: every int-returning function returns WD_OK (0) or a negative wd_status;
+ * nothing throws, exits or prints.  wd_last_error() gives a human-readable message for the
+ * last failure on the calling thread.  wd_apply does not synchronise the host with the
+ * device: launch errors are reported, asynchronous faults surface at the caller's next sync.
+ * There is NO CPU fallback anywhere: without a CUDA device every compute entry point
+ * returns WD_ERR_CUDA.
+ *
+ * CANONICAL layouts (what callers, tests and the oracle speak; C order, last index fastest):
+ *   spinor  psi[rhs][t][z][y][x][spin 0..3][colour 0..2][re,im]      24 reals per site
+ *   links   U  [mu 0..3][t][z][y][x][row a][col b][re,im]            18 reals per link
+ *           mu = 0,1,2,3 <-> x,y,z,t; dims = {Lx, Ly, Lz, Lt}; U_mu(x) sits on the link
+ *           x -> x+mu and (U psi)_a = sum_b U[a][b] psi_b            (readings S5, S6)
+ * NATIVE layouts (what wd_apply reads and writes):
+ *   spinor  [rhs][chunk][site] of 16-byte chunks (float4 / double2), site = x + Lx*(y + Ly*(z + Lz*t))
+ *   links   private to wd_gauge.
+ *   wd_pack_spinor / wd_unpack_spinor convert between the two, so a Krylov loop (100 applies
+ *   back to back, BASELINE.json:configs[3]) never repacks.
+ */
+#ifndef WD_H
+#define WD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    WD_OK = 0,
+    WD_ERR_NULL = -1,      /* a required pointer is NULL                                   */
+    WD_ERR_DIMS = -2,      /* an extent < 1, volume overflow, or dims do not match gauge   */
+    WD_ERR_PRECISION = -3, /* precision is not WD_FP32 / WD_FP64 or differs from the gauge */
+    WD_ERR_RECON = -4,     /* recon is not WD_RECON_18 / WD_RECON_12                       */
+    WD_ERR_NRHS = -5,      /* nrhs < 1                                                     */
+    WD_ERR_ALIAS = -6,     /* out and in overlap (the stencil is not in-place safe)        */
+    WD_ERR_MISMATCH = -7,  /* handle belongs to another lattice / bad kernel selector      */
+    WD_ERR_CUDA = -8,      /* a CUDA runtime call or launch failed (see wd_last_error)     */
+    WD_ERR_ALLOC = -9      /* host or device allocation failed                             */
+} wd_status;
+
+typedef enum { WD_FP32 = 32, WD_FP64 = 64 } wd_precision; /* arithmetic AND storage type    */
+typedef enum { WD_RECON_18 = 18, WD_RECON_12 = 12 } wd_recon; /* reals stored per link       */
+
+/* Kernel selector for wd_set_kernel (measurement and tests; default WD_KERNEL_AUTO). */
+typedef enum {
+    WD_KERNEL_AUTO = 0,    /* fastest kernel valid for the lattice                         */
+    WD_KERNEL_SITE = 1,    /* one thread per site, neighbours straight from L1/L2, any dims */
+    WD_KERNEL_TILE = 2     /* shared-memory tiled kernel (needs dims it supports)          */
+} wd_kernel;
+
+typedef struct wd_lattice wd_lattice; /* opaque: extents, volume                           */
+typedef struct wd_gauge wd_gauge;     /* opaque: native device copy of the links + stream  */
+
+/*
+ * wd_create_lattice -- describe a periodic Lx x Ly x Lz x Lt lattice ("a
+ * hypercubic lattice", vector space of dimension 12 L^3 T).  Host-only, needs no GPU.
+ * dims[mu] >= 1 (extent 1 and 2 follow reading S4: coincident neighbours both count).
+ * On success *lat is a new handle to be released with wd_destroy.
+ */
+int wd_create_lattice(const int dims[4], wd_lattice **lat);
+
+/* Extents / volume of a lattice handle (host-only helpers). */
+int wd_lattice_dims(const wd_lattice *lat, int dims_out[4]);
+long long wd_lattice_volume(const wd_lattice *lat);
+
+/*
+ * wd_load_gauge -- take the links U_mu(x) of eq. (2.2) ("3x3 (dense) SU(3) color
+ * matrices") in CANONICAL 18-real layout from DEVICE memory `links_canonical_dev`
+ * (4*V*18 reals of the given precision) and build the library's native copy:
+ * reordered to structure-of-arrays and, for recon == WD_RECON_12, compressed to rows 0 and 1
+ * of each link, the third row being rebuilt in the kernel as conj(row0 x row1)
+ * ("Gauge field stored as 12 ... floats"; reading S7).
+ * The conversion is enqueued on `stream` (a cudaStream_t cast to void*, NULL = default
+ * stream), which also becomes the stream wd_apply launches on.  The caller may free
+ * `links_canonical_dev` once that stream work has completed.  *gauge is owned by the
+ * library (device memory from cudaMalloc) until wd_destroy_gauge.
+ */
+int wd_load_gauge(const wd_lattice *lat, const void *links_canonical_dev, int precision, int recon,
+                  void *stream, wd_gauge **gauge);
+
+/* Stream (cudaStream_t as void*) on which wd_apply / pack / unpack for this gauge launch. */
+int wd_set_stream(wd_gauge *gauge, void *stream);
+
+/* Force a kernel variant (wd_kernel).  WD_ERR_MISMATCH if it cannot handle the lattice. */
+int wd_set_kernel(wd_gauge *gauge, int kernel);
+
+/* Bytes of a NATIVE spinor buffer holding nrhs fields: nrhs * V * 24 * sizeof(real). */
+size_t wd_spinor_bytes(const wd_lattice *lat, int nrhs, int precision);
+
+/*
+ * wd_pack_spinor / wd_unpack_spinor -- CANONICAL <-> NATIVE spinor layout on the device
+ * (pure data movement, no arithmetic), enqueued on `stream`.  Both buffers hold nrhs fields
+ * of V*24 reals of the given precision and must not overlap.
+ */
+int wd_pack_spinor(const wd_lattice *lat, void *native_dev, const void *canonical_dev, int nrhs,
+                   int precision, void *stream);
+int wd_unpack_spinor(const wd_lattice *lat, void *canonical_dev, const void *native_dev, int nrhs,
+                     int precision, void *stream);
+
+/*
+ * wd_apply -- out[r] = D(U; mass) in[r], r = 0..nrhs-1: eq. (2.2); all of
+ * SURVEY.md section 8(a) steps a1-a7 (neighbour gather with periodic wrap, 12-real link
+ * reconstruction, spin projection, SU(3) mat-vec on half spinors, reconstruct-and-accumulate,
+ * fused (4+m) diagonal, store) run inside ONE kernel launch on the gauge's stream.
+ *   out_native_dev, in_native_dev : DEVICE, NATIVE layout, nrhs fields, 16-byte aligned, no overlap
+ *   gauge     : from wd_load_gauge
+ *   mass      : m of eq. (2.2); the diagonal coefficient 4+m is formed in double, then rounded
+ *               to the working precision; the hopping coefficient is exactly 1/2 (reading S8)
+ *   dims      : must equal the lattice the gauge was loaded for (checked, not trusted)
+ *   nrhs      : number of right-hand sides (>= 1); links are loaded once per site and
+ *               direction for a group of right-hand sides
+ *   precision : WD_FP32 / WD_FP64, must equal the gauge's
+ * Signature order follows BASELINE.json:north_star.
+ */
+int wd_apply(void *out_native_dev, const void *in_native_dev, const wd_gauge *gauge, double mass,
+             const int dims[4], int nrhs, int precision);
+
+/*
+ * wd_apply_host -- the same operation for callers whose data lives in HOST memory, in
+ * CANONICAL layout: copies in_canonical_host to the device, packs, applies D, unpacks, copies
+ * the result to out_canonical_host and synchronises the gauge's stream before returning.
+ * Device staging buffers are owned by the gauge handle (allocated on first use, reused).
+ * Pinned host memory gives asynchronous copies; pageable memory works but is slower.
+ */
+int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_gauge *gauge,
+                  double mass, const int dims[4], int nrhs, int precision);
+
+/* Number of CUDA kernels the library has launched in this process (all handles). */
+long long wd_launch_count(void);
+
+/* Message for the last error on this thread ("" if none); static storage, never NULL. */
+const char *wd_last_error(void);
+
+/* Release handles.  NULL is a no-op.  A gauge must be destroyed before its lattice is
+ * only in the sense that it keeps its own copy of the extents: order does not matter. */
+void wd_destroy_gauge(wd_gauge *gauge);
+void wd_destroy(wd_lattice *lat);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WD_H */

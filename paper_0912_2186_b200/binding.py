@@ -1,1 +1,222 @@
-"""placeholder"""
+"""Thin ctypes binding of libwd.so -- same names as include/wd.h, argument marshalling only.
+
+Every step of the Wilson-Dirac hot path (eq. (2.2)) runs in the CUDA kernels
+behind the C ABI; nothing here computes.  PyTorch appears only as the owner of device memory and
+streams: a "device pointer" argument may be a torch tensor (its data_ptr() is passed) or an int.
+
+There is NO CPU fallback: if libwd.so has not been built (python -m paper_0912_2186_b200.build)
+the first call raises WdError, loudly.
+"""
+import ctypes
+import os
+
+WD_OK = 0
+WD_FP32, WD_FP64 = 32, 64
+WD_RECON_18, WD_RECON_12 = 18, 12
+WD_KERNEL_AUTO, WD_KERNEL_SITE, WD_KERNEL_TILE = 0, 1, 2
+
+STATUS_NAMES = {
+    0: "WD_OK", -1: "WD_ERR_NULL", -2: "WD_ERR_DIMS", -3: "WD_ERR_PRECISION", -4: "WD_ERR_RECON",
+    -5: "WD_ERR_NRHS", -6: "WD_ERR_ALIAS", -7: "WD_ERR_MISMATCH", -8: "WD_ERR_CUDA", -9: "WD_ERR_ALLOC",
+}
+
+# every symbol include/wd.h declares (tests check that the library exports all of them)
+SYMBOLS = (
+    "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
+    "wd_set_kernel", "wd_spinor_bytes", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
+    "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
+)
+
+LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libwd.so")
+_lib = None
+
+
+class WdError(RuntimeError):
+    def __init__(self, code, where, msg=""):
+        self.code = int(code)
+        super().__init__(f"{where}: {STATUS_NAMES.get(self.code, self.code)} {msg}".rstrip())
+
+
+def lib():
+    """Load libwd.so once.  Raises WdError if it is missing -- there is no other code path."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise WdError(-8, "binding.lib", f"{LIB_PATH} not built; run `python -m paper_0912_2186_b200.build`")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, ip, i, d = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.c_int, ctypes.c_double
+    L.wd_create_lattice.argtypes = [ip, ctypes.POINTER(vp)]
+    L.wd_lattice_dims.argtypes = [vp, ip]
+    L.wd_lattice_volume.argtypes = [vp]
+    L.wd_lattice_volume.restype = ctypes.c_longlong
+    L.wd_load_gauge.argtypes = [vp, vp, i, i, vp, ctypes.POINTER(vp)]
+    L.wd_set_stream.argtypes = [vp, vp]
+    L.wd_set_kernel.argtypes = [vp, i]
+    L.wd_spinor_bytes.argtypes = [vp, i, i]
+    L.wd_spinor_bytes.restype = ctypes.c_size_t
+    L.wd_pack_spinor.argtypes = [vp, vp, vp, i, i, vp]
+    L.wd_unpack_spinor.argtypes = [vp, vp, vp, i, i, vp]
+    L.wd_apply.argtypes = [vp, vp, vp, d, ip, i, i]
+    L.wd_apply_host.argtypes = [vp, vp, vp, d, ip, i, i]
+    L.wd_launch_count.argtypes = []
+    L.wd_launch_count.restype = ctypes.c_longlong
+    L.wd_last_error.argtypes = []
+    L.wd_last_error.restype = ctypes.c_char_p
+    L.wd_destroy_gauge.argtypes = [vp]
+    L.wd_destroy_gauge.restype = None
+    L.wd_destroy.argtypes = [vp]
+    L.wd_destroy.restype = None
+    for name in ("wd_create_lattice", "wd_lattice_dims", "wd_load_gauge", "wd_set_stream", "wd_set_kernel",
+                 "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host"):
+        getattr(L, name).restype = i
+    _lib = L
+    return L
+
+
+def _ptr(x):
+    """torch tensor / numpy array / int / None -> integer address (no copies, no checks on content)."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):
+        return x.ctypes.data
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _dims(dims):
+    if dims is None:
+        return None
+    return (ctypes.c_int * 4)(*[int(v) for v in dims])
+
+
+def _check(rc, where):
+    if rc != WD_OK:
+        raise WdError(rc, where, wd_last_error())
+
+
+def wd_last_error():
+    return lib().wd_last_error().decode()
+
+
+def wd_launch_count():
+    return int(lib().wd_launch_count())
+
+
+def wd_create_lattice(dims):
+    h = ctypes.c_void_p()
+    _check(lib().wd_create_lattice(_dims(dims), ctypes.byref(h)), "wd_create_lattice")
+    return h
+
+
+def wd_lattice_dims(lat):
+    out = (ctypes.c_int * 4)()
+    _check(lib().wd_lattice_dims(lat, out), "wd_lattice_dims")
+    return tuple(out)
+
+
+def wd_lattice_volume(lat):
+    return int(lib().wd_lattice_volume(lat))
+
+
+def wd_load_gauge(lat, links_canonical_dev, precision, recon, stream=None):
+    h = ctypes.c_void_p()
+    _check(lib().wd_load_gauge(lat, _ptr(links_canonical_dev), int(precision), int(recon), _ptr(stream),
+                               ctypes.byref(h)), "wd_load_gauge")
+    return h
+
+
+def wd_set_stream(gauge, stream):
+    _check(lib().wd_set_stream(gauge, _ptr(stream)), "wd_set_stream")
+
+
+def wd_set_kernel(gauge, kernel):
+    _check(lib().wd_set_kernel(gauge, int(kernel)), "wd_set_kernel")
+
+
+def wd_spinor_bytes(lat, nrhs, precision):
+    return int(lib().wd_spinor_bytes(lat, int(nrhs), int(precision)))
+
+
+def wd_pack_spinor(lat, native_dev, canonical_dev, nrhs, precision, stream=None):
+    _check(lib().wd_pack_spinor(lat, _ptr(native_dev), _ptr(canonical_dev), int(nrhs), int(precision),
+                                _ptr(stream)), "wd_pack_spinor")
+
+
+def wd_unpack_spinor(lat, canonical_dev, native_dev, nrhs, precision, stream=None):
+    _check(lib().wd_unpack_spinor(lat, _ptr(canonical_dev), _ptr(native_dev), int(nrhs), int(precision),
+                                  _ptr(stream)), "wd_unpack_spinor")
+
+
+def wd_apply(out_native_dev, in_native_dev, gauge, mass, dims, nrhs, precision):
+    _check(lib().wd_apply(_ptr(out_native_dev), _ptr(in_native_dev), gauge, float(mass), _dims(dims), int(nrhs),
+                          int(precision)), "wd_apply")
+
+
+def wd_apply_host(out_canonical_host, in_canonical_host, gauge, mass, dims, nrhs, precision):
+    _check(lib().wd_apply_host(_ptr(out_canonical_host), _ptr(in_canonical_host), gauge, float(mass), _dims(dims),
+                               int(nrhs), int(precision)), "wd_apply_host")
+
+
+def wd_destroy_gauge(gauge):
+    lib().wd_destroy_gauge(gauge)
+
+
+def wd_destroy(lat):
+    lib().wd_destroy(lat)
+
+
+class WilsonDirac:
+    """Handle bundle for one gauge field: lattice + native links (+ the stream to launch on).
+
+    Marshalling only.  `links_canonical_dev` is a torch CUDA tensor [4,Lt,Lz,Ly,Lx,3,3,2] of
+    float32/float64; spinors passed to apply() are NATIVE-layout torch CUDA tensors (use pack()).
+    """
+
+    def __init__(self, dims, links_canonical_dev, precision, recon=WD_RECON_18, stream=None, kernel=WD_KERNEL_AUTO):
+        self.dims = tuple(int(v) for v in dims)
+        self.precision = int(precision)
+        self.recon = int(recon)
+        self.stream = stream
+        self.lat = wd_create_lattice(self.dims)
+        self.gauge = None
+        self.gauge = wd_load_gauge(self.lat, links_canonical_dev, self.precision, self.recon, stream)
+        self.volume = wd_lattice_volume(self.lat)
+        if kernel != WD_KERNEL_AUTO:
+            wd_set_kernel(self.gauge, kernel)
+
+    def set_stream(self, stream):
+        wd_set_stream(self.gauge, stream)
+        self.stream = stream
+
+    def set_kernel(self, kernel):
+        wd_set_kernel(self.gauge, kernel)
+
+    def pack(self, native_dev, canonical_dev, nrhs, stream=None):
+        wd_pack_spinor(self.lat, native_dev, canonical_dev, nrhs, self.precision, stream or self.stream)
+
+    def unpack(self, canonical_dev, native_dev, nrhs, stream=None):
+        wd_unpack_spinor(self.lat, canonical_dev, native_dev, nrhs, self.precision, stream or self.stream)
+
+    def apply(self, out_native_dev, in_native_dev, mass, nrhs=1):
+        wd_apply(out_native_dev, in_native_dev, self.gauge, mass, self.dims, nrhs, self.precision)
+
+    def apply_host(self, out_canonical_host, in_canonical_host, mass, nrhs=1):
+        wd_apply_host(out_canonical_host, in_canonical_host, self.gauge, mass, self.dims, nrhs, self.precision)
+
+    def close(self):
+        if self.gauge is not None:
+            wd_destroy_gauge(self.gauge)
+            self.gauge = None
+        if self.lat is not None:
+            wd_destroy(self.lat)
+            self.lat = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

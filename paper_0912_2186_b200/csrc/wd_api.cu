@@ -1,0 +1,305 @@
+// wd_api.cu -- the extern "C" boundary declared in include/wd.h: argument validation, handle
+// management and kernel dispatch.  No arithmetic of the method lives here.
+#include <atomic>
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/wd.h"
+#include "wd_internal.h"
+
+namespace {
+
+constexpr unsigned LATTICE_MAGIC = 0x57444c41u; // "WDLA"
+constexpr unsigned GAUGE_MAGIC = 0x57444741u;   // "WDGA"
+
+thread_local char g_err[512] = "";
+std::atomic<long long> g_launches{0};
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    return fail(WD_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+bool valid_precision(int p) { return p == WD_FP32 || p == WD_FP64; }
+bool valid_recon(int r) { return r == WD_RECON_18 || r == WD_RECON_12; }
+
+// volume with overflow guard; returns -1 on bad extents
+long long checked_volume(const int dims[4])
+{
+    long long v = 1;
+    for (int d = 0; d < 4; ++d) {
+        if (dims[d] < 1) return -1;
+        v *= dims[d];
+        if (v > (1LL << 40)) return -1;
+    }
+    return v;
+}
+
+bool overlap(const void *a, const void *b, size_t bytes)
+{
+    const uintptr_t pa = (uintptr_t)a, pb = (uintptr_t)b;
+    return pa < pb + bytes && pb < pa + bytes;
+}
+
+int check_apply_args(const void *out, const void *in, const wd_gauge *g, const int dims[4], int nrhs, int precision)
+{
+    if (!out || !in || !g || !dims) return fail(WD_ERR_NULL, "wd_apply: NULL argument");
+    if (g->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_apply: not a live wd_gauge handle");
+    if (!valid_precision(precision)) return fail(WD_ERR_PRECISION, "wd_apply: precision %d is not 32 or 64", precision);
+    if (precision != g->precision)
+        return fail(WD_ERR_PRECISION, "wd_apply: precision %d but gauge was loaded in %d", precision, g->precision);
+    for (int d = 0; d < 4; ++d)
+        if (dims[d] != g->dims[d])
+            return fail(WD_ERR_DIMS, "wd_apply: dims[%d]=%d but gauge lattice has %d", d, dims[d], g->dims[d]);
+    if (nrhs < 1) return fail(WD_ERR_NRHS, "wd_apply: nrhs=%d", nrhs);
+    return WD_OK;
+}
+
+} // namespace
+
+namespace wd {
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+} // namespace wd
+
+extern "C" {
+
+int wd_create_lattice(const int dims[4], wd_lattice **lat)
+{
+    if (!dims || !lat) return fail(WD_ERR_NULL, "wd_create_lattice: NULL argument");
+    *lat = nullptr;
+    const long long V = checked_volume(dims);
+    if (V < 0) return fail(WD_ERR_DIMS, "wd_create_lattice: bad extents %d %d %d %d", dims[0], dims[1], dims[2], dims[3]);
+    wd_lattice *l = new (std::nothrow) wd_lattice;
+    if (!l) return fail(WD_ERR_ALLOC, "wd_create_lattice: out of host memory");
+    l->magic = LATTICE_MAGIC;
+    for (int d = 0; d < 4; ++d) l->dims[d] = dims[d];
+    l->V = V;
+    *lat = l;
+    return WD_OK;
+}
+
+int wd_lattice_dims(const wd_lattice *lat, int dims_out[4])
+{
+    if (!lat || !dims_out) return fail(WD_ERR_NULL, "wd_lattice_dims: NULL argument");
+    if (lat->magic != LATTICE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_lattice_dims: not a live wd_lattice handle");
+    for (int d = 0; d < 4; ++d) dims_out[d] = lat->dims[d];
+    return WD_OK;
+}
+
+long long wd_lattice_volume(const wd_lattice *lat)
+{
+    if (!lat || lat->magic != LATTICE_MAGIC) return -1;
+    return lat->V;
+}
+
+size_t wd_spinor_bytes(const wd_lattice *lat, int nrhs, int precision)
+{
+    if (!lat || lat->magic != LATTICE_MAGIC || nrhs < 1 || !valid_precision(precision)) return 0;
+    return (size_t)nrhs * (size_t)lat->V * 24 * (precision == WD_FP32 ? 4 : 8);
+}
+
+int wd_load_gauge(const wd_lattice *lat, const void *links_canonical_dev, int precision, int recon, void *stream,
+                  wd_gauge **gauge)
+{
+    if (!lat || !links_canonical_dev || !gauge) return fail(WD_ERR_NULL, "wd_load_gauge: NULL argument");
+    *gauge = nullptr;
+    if (lat->magic != LATTICE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_load_gauge: not a live wd_lattice handle");
+    if (!valid_precision(precision)) return fail(WD_ERR_PRECISION, "wd_load_gauge: precision %d is not 32 or 64", precision);
+    if (!valid_recon(recon)) return fail(WD_ERR_RECON, "wd_load_gauge: recon %d is not 18 or 12", recon);
+    wd_gauge *g = new (std::nothrow) wd_gauge;
+    if (!g) return fail(WD_ERR_ALLOC, "wd_load_gauge: out of host memory");
+    memset(g, 0, sizeof(*g));
+    g->magic = GAUGE_MAGIC;
+    for (int d = 0; d < 4; ++d) g->dims[d] = lat->dims[d];
+    g->V = lat->V;
+    g->precision = precision;
+    g->recon = recon;
+    g->kernel = WD_KERNEL_AUTO;
+    g->stream = (cudaStream_t)stream;
+    g->links_bytes = wd::native_link_bytes(g->V, precision, recon);
+    cudaError_t e = cudaMalloc(&g->links, g->links_bytes);
+    if (e != cudaSuccess) {
+        delete g;
+        return e == cudaErrorMemoryAllocation ? fail(WD_ERR_ALLOC, "wd_load_gauge: cudaMalloc failed")
+                                              : cuda_fail(e, "wd_load_gauge: cudaMalloc");
+    }
+    e = wd::launch_pack_links(g->links, links_canonical_dev, g->V, precision, recon, g->stream);
+    if (e != cudaSuccess) {
+        cudaFree(g->links);
+        delete g;
+        return cuda_fail(e, "wd_load_gauge: pack kernel");
+    }
+    *gauge = g;
+    return WD_OK;
+}
+
+int wd_set_stream(wd_gauge *gauge, void *stream)
+{
+    if (!gauge) return fail(WD_ERR_NULL, "wd_set_stream: NULL gauge");
+    if (gauge->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_set_stream: not a live wd_gauge handle");
+    gauge->stream = (cudaStream_t)stream;
+    return WD_OK;
+}
+
+int wd_set_kernel(wd_gauge *gauge, int kernel)
+{
+    if (!gauge) return fail(WD_ERR_NULL, "wd_set_kernel: NULL gauge");
+    if (gauge->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_set_kernel: not a live wd_gauge handle");
+    if (kernel != WD_KERNEL_AUTO && kernel != WD_KERNEL_SITE && kernel != WD_KERNEL_TILE)
+        return fail(WD_ERR_MISMATCH, "wd_set_kernel: unknown kernel %d", kernel);
+    if (kernel == WD_KERNEL_TILE) {
+        wd::ApplyArgs a{};
+        for (int d = 0; d < 4; ++d) a.dims[d] = gauge->dims[d];
+        a.V = gauge->V;
+        a.nrhs = 1;
+        a.precision = gauge->precision;
+        a.recon = gauge->recon;
+        if (!wd::tile_supported(a))
+            return fail(WD_ERR_MISMATCH, "wd_set_kernel: tiled kernel does not support lattice %d %d %d %d", a.dims[0],
+                        a.dims[1], a.dims[2], a.dims[3]);
+    }
+    gauge->kernel = kernel;
+    return WD_OK;
+}
+
+static int check_pack_args(const char *who, const wd_lattice *lat, const void *a, const void *b, int nrhs, int precision)
+{
+    if (!lat || !a || !b) return fail(WD_ERR_NULL, "%s: NULL argument", who);
+    if (lat->magic != LATTICE_MAGIC) return fail(WD_ERR_MISMATCH, "%s: not a live wd_lattice handle", who);
+    if (!valid_precision(precision)) return fail(WD_ERR_PRECISION, "%s: precision %d is not 32 or 64", who, precision);
+    if (nrhs < 1) return fail(WD_ERR_NRHS, "%s: nrhs=%d", who, nrhs);
+    if (overlap(a, b, wd_spinor_bytes(lat, nrhs, precision))) return fail(WD_ERR_ALIAS, "%s: buffers overlap", who);
+    return WD_OK;
+}
+
+int wd_pack_spinor(const wd_lattice *lat, void *native_dev, const void *canonical_dev, int nrhs, int precision,
+                   void *stream)
+{
+    int rc = check_pack_args("wd_pack_spinor", lat, native_dev, canonical_dev, nrhs, precision);
+    if (rc) return rc;
+    cudaError_t e = wd::launch_pack_spinor(native_dev, canonical_dev, lat->V, nrhs, precision, (cudaStream_t)stream);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_pack_spinor");
+}
+
+int wd_unpack_spinor(const wd_lattice *lat, void *canonical_dev, const void *native_dev, int nrhs, int precision,
+                     void *stream)
+{
+    int rc = check_pack_args("wd_unpack_spinor", lat, canonical_dev, native_dev, nrhs, precision);
+    if (rc) return rc;
+    cudaError_t e = wd::launch_unpack_spinor(canonical_dev, native_dev, lat->V, nrhs, precision, (cudaStream_t)stream);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_unpack_spinor");
+}
+
+static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double mass, int nrhs)
+{
+    wd::ApplyArgs a{};
+    a.out = out;
+    a.in = in;
+    a.links = g->links;
+    for (int d = 0; d < 4; ++d) a.dims[d] = g->dims[d];
+    a.V = g->V;
+    a.mass = mass;
+    a.nrhs = nrhs;
+    a.precision = g->precision;
+    a.recon = g->recon;
+    a.stream = g->stream;
+    cudaError_t e;
+    if (g->kernel == WD_KERNEL_SITE)
+        e = wd::launch_site(a);
+    else if (g->kernel == WD_KERNEL_TILE) {
+        if (!wd::tile_supported(a)) return fail(WD_ERR_MISMATCH, "wd_apply: tiled kernel cannot take this call");
+        e = wd::launch_tile(a);
+    } else
+        e = wd::tile_supported(a) ? wd::launch_tile(a) : wd::launch_site(a);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply: kernel launch");
+}
+
+int wd_apply(void *out_native_dev, const void *in_native_dev, const wd_gauge *gauge, double mass, const int dims[4],
+             int nrhs, int precision)
+{
+    int rc = check_apply_args(out_native_dev, in_native_dev, gauge, dims, nrhs, precision);
+    if (rc) return rc;
+    const size_t bytes = (size_t)nrhs * (size_t)gauge->V * 24 * (precision == WD_FP32 ? 4 : 8);
+    if (overlap(out_native_dev, in_native_dev, bytes)) return fail(WD_ERR_ALIAS, "wd_apply: out and in overlap");
+    if (((uintptr_t)out_native_dev | (uintptr_t)in_native_dev) & 15)
+        return fail(WD_ERR_MISMATCH, "wd_apply: buffers must be 16-byte aligned");
+    return dispatch_apply(out_native_dev, in_native_dev, gauge, mass, nrhs);
+}
+
+int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_gauge *gauge, double mass,
+                  const int dims[4], int nrhs, int precision)
+{
+    int rc = check_apply_args(out_canonical_host, in_canonical_host, gauge, dims, nrhs, precision);
+    if (rc) return rc;
+    wd_gauge *g = gauge;
+    const size_t bytes = (size_t)nrhs * (size_t)g->V * 24 * (precision == WD_FP32 ? 4 : 8);
+    if (g->stage_bytes < bytes) {
+        cudaFree(g->stage_canon);
+        cudaFree(g->stage_in);
+        cudaFree(g->stage_out);
+        g->stage_canon = g->stage_in = g->stage_out = nullptr;
+        g->stage_bytes = 0;
+        cudaError_t e = cudaMalloc(&g->stage_canon, bytes);
+        if (e == cudaSuccess) e = cudaMalloc(&g->stage_in, bytes);
+        if (e == cudaSuccess) e = cudaMalloc(&g->stage_out, bytes);
+        if (e != cudaSuccess) {
+            cudaFree(g->stage_canon);
+            cudaFree(g->stage_in);
+            cudaFree(g->stage_out);
+            g->stage_canon = g->stage_in = g->stage_out = nullptr;
+            cudaGetLastError();
+            return fail(WD_ERR_ALLOC, "wd_apply_host: cudaMalloc of %zu staging bytes failed", 3 * bytes);
+        }
+        g->stage_bytes = bytes;
+    }
+    cudaStream_t s = g->stream;
+    cudaError_t e = cudaMemcpyAsync(g->stage_canon, in_canonical_host, bytes, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: H2D copy");
+    e = wd::launch_pack_spinor(g->stage_in, g->stage_canon, g->V, nrhs, precision, s);
+    if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: pack");
+    rc = dispatch_apply(g->stage_out, g->stage_in, g, mass, nrhs);
+    if (rc) return rc;
+    e = wd::launch_unpack_spinor(g->stage_canon, g->stage_out, g->V, nrhs, precision, s);
+    if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: unpack");
+    e = cudaMemcpyAsync(out_canonical_host, g->stage_canon, bytes, cudaMemcpyDeviceToHost, s);
+    if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: D2H copy");
+    e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: stream synchronize");
+    return WD_OK;
+}
+
+long long wd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+const char *wd_last_error(void) { return g_err; }
+
+void wd_destroy_gauge(wd_gauge *gauge)
+{
+    if (!gauge || gauge->magic != GAUGE_MAGIC) return;
+    gauge->magic = 0;
+    cudaFree(gauge->links);
+    cudaFree(gauge->stage_canon);
+    cudaFree(gauge->stage_in);
+    cudaFree(gauge->stage_out);
+    delete gauge;
+}
+
+void wd_destroy(wd_lattice *lat)
+{
+    if (!lat || lat->magic != LATTICE_MAGIC) return;
+    lat->magic = 0;
+    delete lat;
+}
+
+} // extern "C"

@@ -1,0 +1,121 @@
+// wd_dslash_site.cu -- WD_KERNEL_SITE: one thread per lattice site, neighbours fetched straight
+// from global memory (L1/L2 provide the reuse).  Works for ANY extents >= 1, including the
+// degenerate L = 1, 2 cases of reading S4 (coincident neighbours are simply fetched twice and
+// both hops accumulate).  It is the general-purpose kernel and the fallback for lattices the
+// tiled kernel does not take; eq. (2.2); SURVEY.md 8(a) steps a1-a7.
+//
+// A thread handles NR right-hand sides of its site: each link is loaded (and, for recon 12,
+// rebuilt) once per direction and reused for the NR spinors (step a').
+#include "wd_internal.h"
+#include "wd_layout.cuh"
+#include "wd_math.cuh"
+
+namespace wd {
+
+constexpr int SITE_THREADS = 128;
+
+template <typename T, int RECON>
+__device__ __forceinline__ void load_link(const T *__restrict__ links, long long V, int mu, long long site, T (&u)[18])
+{
+    using L = LinkLayout<T, RECON>;
+    const typename L::Vec *q = reinterpret_cast<const typename L::Vec *>(links) + (long long)mu * L::NCH * V + site;
+#pragma unroll
+    for (int c = 0; c < L::NCH; ++c) {
+        const typename L::Vec v = __ldg(q + (long long)c * V);
+        unpack(v, &u[c * L::CR]);
+    }
+    if (RECON == 12) reconstruct_row2(u);
+}
+
+template <int MU, typename T, int RECON, int NR>
+__device__ __forceinline__ void hop_pair(T (&acc)[NR][24], const T *__restrict__ in, const T *__restrict__ links,
+                                         long long V, long long site, long long sf, long long sb, int rhs0, int nrhs)
+{
+    T u[18];
+    load_link<T, RECON>(links, V, MU, site, u); // U_mu(x)
+#pragma unroll
+    for (int r = 0; r < NR; ++r)
+        if (rhs0 + r < nrhs) {
+            T p[24];
+            load_spinor(in + (long long)(rhs0 + r) * 24 * V, V, sf, p); // psi(x+mu)
+            hop_forward<MU>(acc[r], u, p);
+        }
+    load_link<T, RECON>(links, V, MU, sb, u); // U_mu(x-mu)
+#pragma unroll
+    for (int r = 0; r < NR; ++r)
+        if (rhs0 + r < nrhs) {
+            T p[24];
+            load_spinor(in + (long long)(rhs0 + r) * 24 * V, V, sb, p); // psi(x-mu)
+            hop_backward<MU>(acc[r], u, p);
+        }
+}
+
+template <typename T, int RECON, int NR>
+__global__ void __launch_bounds__(SITE_THREADS)
+dslash_site_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ links, int Lx, int Ly, int Lz,
+                   int Lt, long long V, T cdiag, int nrhs)
+{
+    const long long site = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (site >= V) return;
+    const int rhs0 = blockIdx.y * NR;
+
+    // periodic neighbours (step a1): coordinates from the lexicographic index, wrap by compare
+    long long rem = site;
+    const int x = (int)(rem % Lx); rem /= Lx;
+    const int y = (int)(rem % Ly); rem /= Ly;
+    const int z = (int)(rem % Lz);
+    const int t = (int)(rem / Lz);
+    const long long sx = 1, sy = Lx, sz = (long long)Lx * Ly, st = (long long)Lx * Ly * Lz;
+    const long long xf = site + (x + 1 == Lx ? -(Lx - 1) * sx : sx), xb = site + (x == 0 ? (Lx - 1) * sx : -sx);
+    const long long yf = site + (y + 1 == Ly ? -(Ly - 1) * sy : sy), yb = site + (y == 0 ? (Ly - 1) * sy : -sy);
+    const long long zf = site + (z + 1 == Lz ? -(Lz - 1) * sz : sz), zb = site + (z == 0 ? (Lz - 1) * sz : -sz);
+    const long long tf = site + (t + 1 == Lt ? -(Lt - 1) * st : st), tb = site + (t == 0 ? (Lt - 1) * st : -st);
+
+    T acc[NR][24];
+#pragma unroll
+    for (int r = 0; r < NR; ++r)
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[r][i] = (T)0;
+
+    hop_pair<0, T, RECON, NR>(acc, in, links, V, site, xf, xb, rhs0, nrhs);
+    hop_pair<1, T, RECON, NR>(acc, in, links, V, site, yf, yb, rhs0, nrhs);
+    hop_pair<2, T, RECON, NR>(acc, in, links, V, site, zf, zb, rhs0, nrhs);
+    hop_pair<3, T, RECON, NR>(acc, in, links, V, site, tf, tb, rhs0, nrhs);
+
+    // fused diagonal (step a6): out = (4+m) psi(x) - 1/2 acc
+#pragma unroll
+    for (int r = 0; r < NR; ++r)
+        if (rhs0 + r < nrhs) {
+            T p[24];
+            load_spinor(in + (long long)(rhs0 + r) * 24 * V, V, site, p);
+#pragma unroll
+            for (int i = 0; i < 24; ++i) p[i] = fma(cdiag, p[i], (T)-0.5 * acc[r][i]);
+            store_spinor(out + (long long)(rhs0 + r) * 24 * V, V, site, p);
+        }
+}
+
+template <typename T, int RECON, int NR>
+static cudaError_t launch_site_t(const ApplyArgs &a)
+{
+    dim3 grid((unsigned)((a.V + SITE_THREADS - 1) / SITE_THREADS), (unsigned)((a.nrhs + NR - 1) / NR));
+    const T cdiag = (T)(4.0 + a.mass); // formed in double, rounded once (reading S8)
+    dslash_site_kernel<T, RECON, NR><<<grid, SITE_THREADS, 0, a.stream>>>(
+        (T *)a.out, (const T *)a.in, (const T *)a.links, a.dims[0], a.dims[1], a.dims[2], a.dims[3], a.V, cdiag, a.nrhs);
+    count_launch();
+    return cudaGetLastError();
+}
+
+template <typename T, int RECON>
+static cudaError_t launch_site_r(const ApplyArgs &a)
+{
+    if (a.nrhs >= 2 && sizeof(T) == 4) return launch_site_t<T, RECON, 2>(a);
+    return launch_site_t<T, RECON, 1>(a);
+}
+
+cudaError_t launch_site(const ApplyArgs &a)
+{
+    if (a.precision == 32) return a.recon == 18 ? launch_site_r<float, 18>(a) : launch_site_r<float, 12>(a);
+    return a.recon == 18 ? launch_site_r<double, 18>(a) : launch_site_r<double, 12>(a);
+}
+
+} // namespace wd

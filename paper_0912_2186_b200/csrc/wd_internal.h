@@ -1,0 +1,60 @@
+// wd_internal.h -- host-side structures shared by the translation units of libwd.so.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+struct wd_lattice {
+    unsigned magic;
+    int dims[4];      // Lx, Ly, Lz, Lt
+    long long V;
+};
+
+struct wd_gauge {
+    unsigned magic;
+    int dims[4];
+    long long V;
+    int precision;    // 32 / 64
+    int recon;        // 18 / 12
+    int kernel;       // wd_kernel selector
+    void *links;      // native links, device (cudaMalloc)
+    size_t links_bytes;
+    cudaStream_t stream;
+    // staging for wd_apply_host (allocated on first use)
+    void *stage_canon;   // canonical spinor buffer, device
+    void *stage_in;      // native in
+    void *stage_out;     // native out
+    size_t stage_bytes;
+};
+
+namespace wd {
+
+struct ApplyArgs {
+    void *out;
+    const void *in;
+    const void *links;
+    int dims[4];
+    long long V;
+    double mass;
+    int nrhs;
+    int precision;
+    int recon;
+    cudaStream_t stream;
+};
+
+void count_launch(int n = 1);
+
+// one thread per site, any extents >= 1
+cudaError_t launch_site(const ApplyArgs &a);
+// shared-memory tiled kernel; supported() is a pure host-side predicate
+bool tile_supported(const ApplyArgs &a);
+cudaError_t launch_tile(const ApplyArgs &a);
+
+cudaError_t launch_pack_spinor(void *native, const void *canonical, long long V, int nrhs, int precision,
+                               cudaStream_t s);
+cudaError_t launch_unpack_spinor(void *canonical, const void *native, long long V, int nrhs, int precision,
+                                 cudaStream_t s);
+cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon,
+                              cudaStream_t s);
+size_t native_link_bytes(long long V, int precision, int recon);
+
+} // namespace wd

@@ -1,0 +1,164 @@
+// wd_math.cuh -- per-site arithmetic of the Wilson-Dirac hopping term (device only).
+//
+// Implements SURVEY.md section 8(a) steps a2-a6 for eq. (2.2) of arXiv:0912.2186
+// (PAPER.md:69-73): 12-real link reconstruction, spin projection with (1 +- gamma_mu),
+// SU(3) mat-vec on the two independent spin rows, reconstruction of rows 2,3 and
+// accumulation.  Everything is written out for the DeGrand-Rossi basis (S2):
+//
+//   gamma_x = [[0,0,0,i],[0,0,i,0],[0,-i,0,0],[-i,0,0,0]]   gamma_y = [[0,0,0,-1],[0,0,1,0],[0,1,0,0],[-1,0,0,0]]
+//   gamma_z = [[0,0,i,0],[0,0,0,-i],[-i,0,0,0],[0,i,0,0]]   gamma_t = [[0,0,1,0],[0,0,0,1],[1,0,0,0],[0,1,0,0]]
+//
+// Each projector (1 + S gamma_mu), S = +-1, has rank 2: rows 2,3 of (1 + S gamma_mu) psi are
+// unit multiples of rows 0,1 ("h0", "h1"), so the colour matrix only multiplies h0 and h1:
+//
+//   mu   h0                 h1                 row 2        row 3
+//   x    psi0 + S i psi3    psi1 + S i psi2    -S i h1      -S i h0
+//   y    psi0 - S   psi3    psi1 + S   psi2     S   h1      -S   h0
+//   z    psi0 + S i psi2    psi1 - S i psi3    -S i h0       S i h1
+//   t    psi0 + S   psi2    psi1 + S   psi3     S   h0       S   h1
+//
+// Register layouts: spinor  p[24], index (spin*3 + colour)*2 + {0:re, 1:im}
+//                   half    h[12], index (row*3  + colour)*2 + {0:re, 1:im}
+//                   link    u[18], index (a*3 + b)*2 + {0:re, 1:im},  (U v)_a = sum_b U[a][b] v_b
+#pragma once
+
+namespace wd {
+
+// h = rows 0,1 of (1 + S gamma_MU) p
+template <int MU, int S, typename T>
+__device__ __forceinline__ void project(const T (&p)[24], T (&h)[12])
+{
+    constexpr T s = (T)S;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const T p0r = p[(0 * 3 + c) * 2], p0i = p[(0 * 3 + c) * 2 + 1];
+        const T p1r = p[(1 * 3 + c) * 2], p1i = p[(1 * 3 + c) * 2 + 1];
+        const T p2r = p[(2 * 3 + c) * 2], p2i = p[(2 * 3 + c) * 2 + 1];
+        const T p3r = p[(3 * 3 + c) * 2], p3i = p[(3 * 3 + c) * 2 + 1];
+        T h0r, h0i, h1r, h1i;
+        if (MU == 0) {        // h0 = p0 + S i p3 ; h1 = p1 + S i p2
+            h0r = p0r - s * p3i; h0i = p0i + s * p3r;
+            h1r = p1r - s * p2i; h1i = p1i + s * p2r;
+        } else if (MU == 1) { // h0 = p0 - S p3 ; h1 = p1 + S p2
+            h0r = p0r - s * p3r; h0i = p0i - s * p3i;
+            h1r = p1r + s * p2r; h1i = p1i + s * p2i;
+        } else if (MU == 2) { // h0 = p0 + S i p2 ; h1 = p1 - S i p3
+            h0r = p0r - s * p2i; h0i = p0i + s * p2r;
+            h1r = p1r + s * p3i; h1i = p1i - s * p3r;
+        } else {              // h0 = p0 + S p2 ; h1 = p1 + S p3
+            h0r = p0r + s * p2r; h0i = p0i + s * p2i;
+            h1r = p1r + s * p3r; h1i = p1i + s * p3i;
+        }
+        h[(0 * 3 + c) * 2] = h0r; h[(0 * 3 + c) * 2 + 1] = h0i;
+        h[(1 * 3 + c) * 2] = h1r; h[(1 * 3 + c) * 2 + 1] = h1i;
+    }
+}
+
+// chi_row = U h_row  (forward hop: the un-daggered link)
+template <typename T>
+__device__ __forceinline__ void su3_mul(const T (&u)[18], const T (&h)[12], T (&chi)[12])
+{
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            T re = (T)0, im = (T)0;
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const T ur = u[(a * 3 + b) * 2], ui = u[(a * 3 + b) * 2 + 1];
+                const T hr = h[(r * 3 + b) * 2], hi = h[(r * 3 + b) * 2 + 1];
+                re = fma(ur, hr, re); re = fma(-ui, hi, re);
+                im = fma(ur, hi, im); im = fma(ui, hr, im);
+            }
+            chi[(r * 3 + a) * 2] = re; chi[(r * 3 + a) * 2 + 1] = im;
+        }
+}
+
+// chi_row = U^dagger h_row  (backward hop):  (U^dag)[a][b] = conj(U[b][a])
+template <typename T>
+__device__ __forceinline__ void su3_dag_mul(const T (&u)[18], const T (&h)[12], T (&chi)[12])
+{
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            T re = (T)0, im = (T)0;
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const T ur = u[(b * 3 + a) * 2], ui = u[(b * 3 + a) * 2 + 1];
+                const T hr = h[(r * 3 + b) * 2], hi = h[(r * 3 + b) * 2 + 1];
+                re = fma(ur, hr, re); re = fma(ui, hi, re);
+                im = fma(ur, hi, im); im = fma(-ui, hr, im);
+            }
+            chi[(r * 3 + a) * 2] = re; chi[(r * 3 + a) * 2 + 1] = im;
+        }
+}
+
+// acc += (1 + S gamma_MU)-reconstruction of chi (rows 0,1 = chi; rows 2,3 per the table above)
+template <int MU, int S, typename T>
+__device__ __forceinline__ void reconstruct_add(T (&acc)[24], const T (&chi)[12])
+{
+    constexpr T s = (T)S;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const T c0r = chi[(0 * 3 + c) * 2], c0i = chi[(0 * 3 + c) * 2 + 1];
+        const T c1r = chi[(1 * 3 + c) * 2], c1i = chi[(1 * 3 + c) * 2 + 1];
+        acc[(0 * 3 + c) * 2] += c0r; acc[(0 * 3 + c) * 2 + 1] += c0i;
+        acc[(1 * 3 + c) * 2] += c1r; acc[(1 * 3 + c) * 2 + 1] += c1i;
+        if (MU == 0) {        // row2 = -S i chi1 ; row3 = -S i chi0      (-S i)(a+ib) = S b - S i a
+            acc[(2 * 3 + c) * 2] += s * c1i; acc[(2 * 3 + c) * 2 + 1] -= s * c1r;
+            acc[(3 * 3 + c) * 2] += s * c0i; acc[(3 * 3 + c) * 2 + 1] -= s * c0r;
+        } else if (MU == 1) { // row2 = S chi1 ; row3 = -S chi0
+            acc[(2 * 3 + c) * 2] += s * c1r; acc[(2 * 3 + c) * 2 + 1] += s * c1i;
+            acc[(3 * 3 + c) * 2] -= s * c0r; acc[(3 * 3 + c) * 2 + 1] -= s * c0i;
+        } else if (MU == 2) { // row2 = -S i chi0 ; row3 = S i chi1        (S i)(a+ib) = -S b + S i a
+            acc[(2 * 3 + c) * 2] += s * c0i; acc[(2 * 3 + c) * 2 + 1] -= s * c0r;
+            acc[(3 * 3 + c) * 2] -= s * c1i; acc[(3 * 3 + c) * 2 + 1] += s * c1r;
+        } else {              // row2 = S chi0 ; row3 = S chi1
+            acc[(2 * 3 + c) * 2] += s * c0r; acc[(2 * 3 + c) * 2 + 1] += s * c0i;
+            acc[(3 * 3 + c) * 2] += s * c1r; acc[(3 * 3 + c) * 2 + 1] += s * c1i;
+        }
+    }
+}
+
+// Third row of a special-unitary matrix from the first two: row2 = conj(row0 x row1)
+// ("stored as 12 ... floats").
+template <typename T>
+__device__ __forceinline__ void reconstruct_row2(T (&u)[18])
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int j = (c + 1) % 3, k = (c + 2) % 3;
+        const T ajr = u[(0 * 3 + j) * 2], aji = u[(0 * 3 + j) * 2 + 1];
+        const T akr = u[(0 * 3 + k) * 2], aki = u[(0 * 3 + k) * 2 + 1];
+        const T bjr = u[(1 * 3 + j) * 2], bji = u[(1 * 3 + j) * 2 + 1];
+        const T bkr = u[(1 * 3 + k) * 2], bki = u[(1 * 3 + k) * 2 + 1];
+        // z = a_j b_k - a_k b_j ;  row2[c] = conj(z)
+        const T zr = ajr * bkr - aji * bki - (akr * bjr - aki * bji);
+        const T zi = ajr * bki + aji * bkr - (akr * bji + aki * bjr);
+        u[(2 * 3 + c) * 2] = zr;
+        u[(2 * 3 + c) * 2 + 1] = -zi;
+    }
+}
+
+// One forward + one backward hop in direction MU accumulated into acc:
+//   acc += (1 - gamma_MU) U_f p_f  +  (1 + gamma_MU) U_b^dag p_b
+template <int MU, typename T>
+__device__ __forceinline__ void hop_forward(T (&acc)[24], const T (&u)[18], const T (&p)[24])
+{
+    T h[12], chi[12];
+    project<MU, -1>(p, h);
+    su3_mul(u, h, chi);
+    reconstruct_add<MU, -1>(acc, chi);
+}
+
+template <int MU, typename T>
+__device__ __forceinline__ void hop_backward(T (&acc)[24], const T (&u)[18], const T (&p)[24])
+{
+    T h[12], chi[12];
+    project<MU, +1>(p, h);
+    su3_dag_mul(u, h, chi);
+    reconstruct_add<MU, +1>(acc, chi);
+}
+
+} // namespace wd

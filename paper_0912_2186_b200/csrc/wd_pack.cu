@@ -1,0 +1,114 @@
+// wd_pack.cu -- canonical <-> native layout conversion (pure data movement, no arithmetic).
+// SURVEY.md section 8(a) step a0; canonical layouts are DESIGN.md readings S5/S6.
+#include "wd_internal.h"
+#include "wd_layout.cuh"
+
+namespace wd {
+
+constexpr int PACK_SITES = 128; // sites per CTA; also the CTA size
+
+// canonical [rhs][site][NCH chunks]  <->  native [rhs][chunk][site]; transposed through shared
+// memory so that both the global reads and the global writes are contiguous 16-byte-per-lane.
+template <typename Vec, int NCH, bool TO_NATIVE>
+__global__ void __launch_bounds__(PACK_SITES) spinor_transpose_kernel(Vec *__restrict__ dst, const Vec *__restrict__ src,
+                                                                     long long V)
+{
+    __shared__ Vec tile[NCH][PACK_SITES + 1];
+    const long long site0 = (long long)blockIdx.x * PACK_SITES;
+    const int rhs = blockIdx.y;
+    const int tid = threadIdx.x;
+    const long long nsite = min((long long)PACK_SITES, V - site0);
+    const Vec *canon_src = src + ((long long)rhs * V + site0) * NCH;
+    Vec *canon_dst = dst + ((long long)rhs * V + site0) * NCH;
+    if (TO_NATIVE) {
+#pragma unroll
+        for (int i = 0; i < NCH; ++i) {
+            const int idx = i * PACK_SITES + tid;
+            if (idx < nsite * NCH) tile[idx % NCH][idx / NCH] = canon_src[idx];
+        }
+        __syncthreads();
+        if (tid < nsite) {
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) dst[((long long)rhs * NCH + c) * V + site0 + tid] = tile[c][tid];
+        }
+    } else {
+        if (tid < nsite) {
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) tile[c][tid] = src[((long long)rhs * NCH + c) * V + site0 + tid];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < NCH; ++i) {
+            const int idx = i * PACK_SITES + tid;
+            if (idx < nsite * NCH) canon_dst[idx] = tile[idx % NCH][idx / NCH];
+        }
+    }
+}
+
+template <bool TO_NATIVE>
+static cudaError_t transpose_spinor(void *dst, const void *src, long long V, int nrhs, int precision, cudaStream_t s)
+{
+    if (V <= 0 || nrhs <= 0) return cudaSuccess;
+    dim3 grid((unsigned)((V + PACK_SITES - 1) / PACK_SITES), (unsigned)nrhs);
+    if (precision == 32)
+        spinor_transpose_kernel<float4, 6, TO_NATIVE><<<grid, PACK_SITES, 0, s>>>((float4 *)dst, (const float4 *)src, V);
+    else
+        spinor_transpose_kernel<double2, 12, TO_NATIVE><<<grid, PACK_SITES, 0, s>>>((double2 *)dst, (const double2 *)src, V);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pack_spinor(void *native, const void *canonical, long long V, int nrhs, int precision, cudaStream_t s)
+{
+    return transpose_spinor<true>(native, canonical, V, nrhs, precision, s);
+}
+
+cudaError_t launch_unpack_spinor(void *canonical, const void *native, long long V, int nrhs, int precision,
+                                 cudaStream_t s)
+{
+    return transpose_spinor<false>(canonical, native, V, nrhs, precision, s);
+}
+
+// canonical U[mu][site][a][b][re,im] -> native [mu][chunk][site]; recon 12 keeps rows a = 0,1.
+template <typename T, int RECON>
+__global__ void pack_links_kernel(T *__restrict__ dst, const T *__restrict__ src, long long V)
+{
+    using L = LinkLayout<T, RECON>;
+    const long long site = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int mu = blockIdx.y;
+    if (site >= V) return;
+    const T *p = src + ((long long)mu * V + site) * 18;
+    typename L::Vec *q = reinterpret_cast<typename L::Vec *>(dst) + (long long)mu * L::NCH * V + site;
+#pragma unroll
+    for (int c = 0; c < L::NCH; ++c) {
+        T r[L::CR];
+#pragma unroll
+        for (int k = 0; k < L::CR; ++k) r[k] = p[c * L::CR + k];
+        typename L::Vec v;
+        pack(v, r);
+        q[(long long)c * V] = v;
+    }
+}
+
+size_t native_link_bytes(long long V, int precision, int recon)
+{
+    return (size_t)4 * (size_t)V * (size_t)recon * (precision == 32 ? 4 : 8);
+}
+
+cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon, cudaStream_t s)
+{
+    if (V <= 0) return cudaSuccess;
+    dim3 grid((unsigned)((V + 127) / 128), 4);
+    if (precision == 32 && recon == 18)
+        pack_links_kernel<float, 18><<<grid, 128, 0, s>>>((float *)native, (const float *)canonical, V);
+    else if (precision == 32)
+        pack_links_kernel<float, 12><<<grid, 128, 0, s>>>((float *)native, (const float *)canonical, V);
+    else if (recon == 18)
+        pack_links_kernel<double, 18><<<grid, 128, 0, s>>>((double *)native, (const double *)canonical, V);
+    else
+        pack_links_kernel<double, 12><<<grid, 128, 0, s>>>((double *)native, (const double *)canonical, V);
+    count_launch();
+    return cudaGetLastError();
+}
+
+} // namespace wd

@@ -176,10 +176,18 @@ def unit_links(dims):
     return u
 
 
-def gaussian_spinor(dims, seed, nrhs=1):
-    """Complex Gaussian spinors (Re, Im ~ N(0,1)), float64 [nrhs, Lt, Lz, Ly, Lx, 4, 3, 2]."""
+def gaussian_spinor(dims, seed, nrhs=1, precision=64):
+    """Complex Gaussian spinors (Re, Im ~ N(0,1)), [nrhs, Lt, Lz, Ly, Lx, 4, 3, 2].
+
+    Drawn in canonical order from one generator, one right-hand side per standard_normal call
+    (the stream is the same as a single call); each is rounded once to `precision` as it is drawn
+    so that 24 right-hand sides of 32^3x64 never exist in float64 at the same time."""
     rng = np.random.default_rng(seed)
-    return rng.standard_normal((int(nrhs),) + _site_shape(dims) + (4, 3, 2))
+    shape = _site_shape(dims) + (4, 3, 2)
+    out = np.empty((int(nrhs),) + shape, dtype=np.float32 if int(precision) == 32 else np.float64)
+    for r in range(int(nrhs)):
+        out[r] = rng.standard_normal(shape)
+    return out
 
 
 def round_to(a, precision):
@@ -198,5 +206,5 @@ def make_fields(cfg, nrhs=None, dims=None):
         u = smooth_links(d, cfg.seed, cfg.eps)
     else:
         raise ValueError(cfg.links)
-    psi = gaussian_spinor(d, cfg.seed + 1000, n)
-    return round_to(u, cfg.precision), round_to(psi, cfg.precision)
+    psi = gaussian_spinor(d, cfg.seed + 1000, n, cfg.precision)
+    return round_to(u, cfg.precision), psi

@@ -1,0 +1,198 @@
+"""-m gpu parity tests: the CUDA path, called through the C ABI (libwd.so), against the CPU oracle
+on the same seeded inputs, element by element (relative L2 over the whole field, per RHS).
+
+Tolerances (BASELINE.json:north_star): <= 1e-13 in fp64, <= 2e-6 in fp32.  The inputs are rounded
+once to the working precision and the oracle consumes those same bits widened to fp64 (S12).
+For recon 12 the oracle consumes the same 12 stored reals per link (rows 0,1; S7).
+"""
+import numpy as np
+import pytest
+
+from paper_0912_2186_b200 import fields
+from gpu_util import TOL, GpuOp, np_dtype, oracle_apply, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = {"auto": 0, "site": 1, "tile": 2}
+
+
+def oracle_links(U, recon):
+    return U if recon == 18 else np.ascontiguousarray(U[..., :2, :, :])
+
+
+def check_config(oracle, cfg, kernel="auto", nrhs=None, dims=None):
+    U, psi = fields.make_fields(cfg, nrhs=nrhs, dims=dims)
+    d = tuple(dims) if dims is not None else cfg.dims
+    op = GpuOp(U, d, cfg.precision, cfg.recon, KERNELS[kernel])
+    try:
+        got = op.apply(psi, cfg.mass)
+    finally:
+        op.close()
+    assert np.isfinite(got).all()
+    Uo = oracle_links(U, cfg.recon)
+    worst = 0.0
+    for r in range(psi.shape[0]):
+        want = oracle.apply(psi[r].astype(np.float64), Uo.astype(np.float64), d, cfg.mass)
+        worst = max(worst, rel_l2(got[r], want))
+    assert worst <= TOL[cfg.precision], (cfg.name, kernel, worst)
+    return worst
+
+
+# ---------------------------------------------------------------- the five BASELINE configs
+@pytest.mark.parametrize("name", ["c0_4x4_fp64", "c1_16x32_fp32", "c2_24x64_fp32_r12"])
+@pytest.mark.parametrize("kernel", ["auto", "site"])
+def test_baseline_configs_small(oracle, name, kernel):
+    check_config(oracle, fields.CONFIGS[name], kernel)
+
+
+@pytest.mark.parametrize("name", ["c3_32x64_fp32", "c3_32x64_fp64"])
+def test_baseline_config3_full_size(oracle, name):
+    check_config(oracle, fields.CONFIGS[name], "auto")
+
+
+def test_baseline_config4_24rhs_full_size(oracle):
+    check_config(oracle, fields.CONFIGS["c4_32x64_fp32_24rhs"], "auto")
+
+
+def test_paper_nv20_rhs(oracle):
+    """N_v = 20 test vectors on a smaller lattice: nrhs is a runtime value."""
+    check_config(oracle, fields.CONFIGS["c4_32x64_fp32_24rhs"], "auto", nrhs=20, dims=(16, 16, 16, 16))
+
+
+# ---------------------------------------------------------------- shapes, tails, degenerate extents
+SHAPES = [(4, 8, 12, 16), (8, 4, 4, 12), (6, 10, 4, 8), (3, 5, 2, 7), (2, 2, 2, 2), (1, 1, 1, 1), (1, 4, 1, 3),
+          (5, 1, 2, 9), (32, 4, 4, 4), (16, 8, 8, 6), (24, 12, 4, 5), (12, 12, 12, 12), (32, 8, 8, 3)]
+
+
+@pytest.mark.parametrize("dims", SHAPES)
+@pytest.mark.parametrize("precision,recon", [(64, 18), (32, 18), (32, 12), (64, 12)])
+def test_shapes(oracle, dims, precision, recon):
+    cfg = fields.Config("shape", dims, precision, "haar", recon, -0.3, 1, 11)
+    for nrhs in (1, 3):
+        check_config(oracle, cfg, "auto", nrhs=nrhs)
+    check_config(oracle, cfg, "site", nrhs=2)
+
+
+@pytest.mark.parametrize("nrhs", [1, 2, 3, 4, 5, 7, 8, 12, 20, 24])
+def test_nrhs_sweep(oracle, nrhs):
+    cfg = fields.Config("nrhs", (8, 8, 8, 8), 32, "smooth", 18, -0.42, nrhs, 21)
+    check_config(oracle, cfg, "auto")
+
+
+# ---------------------------------------------------------------- invariants of the CUDA path itself
+def test_deterministic_and_repeatable():
+    """No atomics: launch #100 on input A is bit-identical to launch #1 on input A (S9)."""
+    import torch
+    cfg = fields.CONFIGS["c1_16x32_fp32"]
+    U, psi = fields.make_fields(cfg)
+    op = GpuOp(U, cfg.dims, cfg.precision, cfg.recon)
+    canon = torch.from_numpy(psi).cuda()
+    a = torch.empty_like(canon)
+    op.op.pack(a, canon, 1)
+    outs = [torch.empty_like(canon) for _ in range(3)]
+    op.op.apply(outs[0], a, cfg.mass, 1)
+    first = outs[0].clone()
+    for i in range(1, 100):
+        op.op.apply(outs[i % 3], a, cfg.mass, 1)
+    torch.cuda.synchronize()
+    assert torch.equal(outs[99 % 3], first)
+    op.close()
+
+
+def test_batched_matches_single(oracle):
+    """out[r] of one 6-RHS apply agrees with six single applies (S10) to fp32 rounding."""
+    cfg = fields.Config("b", (8, 8, 8, 16), 32, "smooth", 18, -0.42, 6, 31)
+    U, psi = fields.make_fields(cfg)
+    op = GpuOp(U, cfg.dims, 32, 18)
+    batched = op.apply(psi, cfg.mass)
+    for r in range(6):
+        single = op.apply(psi[r:r + 1], cfg.mass)
+        assert rel_l2(batched[r], single[0]) <= 1e-6
+    op.close()
+
+
+def test_translation_covariance_through_native_layout():
+    """P6 on the CUDA path: shifting U and psi by one site in direction mu shifts the output."""
+    dims = (8, 4, 12, 6)
+    cfg = fields.Config("t", dims, 64, "haar", 18, 0.05, 1, 41)
+    U, psi = fields.make_fields(cfg)
+    op = GpuOp(U, dims, 64, 18)
+    base = op.apply(psi, cfg.mass)
+    op.close()
+    for mu in range(4):
+        ax = 3 - mu  # site axes are [t, z, y, x]
+        Us = np.roll(U, 1, axis=1 + ax)
+        ps = np.roll(psi, 1, axis=1 + ax)
+        op = GpuOp(Us, dims, 64, 18)
+        got = op.apply(ps, cfg.mass)
+        op.close()
+        assert rel_l2(got, np.roll(base, 1, axis=1 + ax)) <= 1e-14
+
+
+def test_pack_unpack_roundtrip_and_native_layout():
+    """Native layout is [rhs][chunk][site] of 16-byte chunks (include/wd.h); pure data movement."""
+    import torch
+    from paper_0912_2186_b200 import binding
+    dims = (6, 4, 2, 5)
+    V = 6 * 4 * 2 * 5
+    for precision, cr in ((32, 4), (64, 2)):
+        psi = fields.gaussian_spinor(dims, 5, 3, precision)
+        lat = binding.wd_create_lattice(dims)
+        canon = torch.from_numpy(psi).cuda()
+        native = torch.empty_like(canon)
+        back = torch.empty_like(canon)
+        binding.wd_pack_spinor(lat, native, canon, 3, precision)
+        binding.wd_unpack_spinor(lat, back, native, 3, precision)
+        torch.cuda.synchronize()
+        assert torch.equal(back, canon)
+        want = psi.reshape(3, V, 24 // cr, cr).transpose(0, 2, 1, 3)
+        assert np.array_equal(native.cpu().numpy().reshape(3, 24 // cr, V, cr), want)
+        binding.wd_destroy(lat)
+
+
+def test_apply_host_matches_device_path(oracle):
+    cfg = fields.Config("h", (8, 8, 4, 6), 32, "haar", 18, -0.4, 2, 51)
+    U, psi = fields.make_fields(cfg)
+    op = GpuOp(U, cfg.dims, 32, 18)
+    dev = op.apply(psi, cfg.mass)
+    out = np.full_like(psi, np.nan)
+    op.op.apply_host(out, psi, cfg.mass, 2)
+    assert np.array_equal(out, dev)
+    want = oracle_apply(oracle, psi, U, cfg.dims, cfg.mass)
+    assert rel_l2(out, want) <= TOL[32]
+    op.close()
+
+
+def test_argument_errors_on_device():
+    import torch
+    from paper_0912_2186_b200 import binding
+    cfg = fields.Config("e", (4, 4, 4, 4), 32, "haar", 18, 0.1, 1, 61)
+    U, psi = fields.make_fields(cfg)
+    op = GpuOp(U, cfg.dims, 32, 18)
+    a = torch.from_numpy(psi).cuda()
+    b = torch.empty_like(a)
+    c = torch.empty(a.numel() + 64, dtype=a.dtype, device=a.device)
+    cases = [
+        (lambda: binding.wd_apply(a, a, op.op.gauge, 0.1, cfg.dims, 1, 32), -6),
+        (lambda: binding.wd_apply(b, a, op.op.gauge, 0.1, (4, 4, 4, 8), 1, 32), -2),
+        (lambda: binding.wd_apply(b, a, op.op.gauge, 0.1, cfg.dims, 1, 64), -3),
+        (lambda: binding.wd_apply(b, a, op.op.gauge, 0.1, cfg.dims, 0, 32), -5),
+        (lambda: binding.wd_apply(c.data_ptr() + 4, a, op.op.gauge, 0.1, cfg.dims, 1, 32), -7),
+        (lambda: binding.wd_set_kernel(op.op.gauge, 99), -7),
+    ]
+    for fn, code in cases:
+        with pytest.raises(binding.WdError) as e:
+            fn()
+        assert e.value.code == code
+    op.close()
+
+
+def test_launch_counter_counts_kernels():
+    from paper_0912_2186_b200 import binding
+    cfg = fields.Config("l", (4, 4, 4, 4), 32, "haar", 18, 0.1, 1, 71)
+    U, psi = fields.make_fields(cfg)
+    op = GpuOp(U, cfg.dims, 32, 18)
+    n0 = binding.wd_launch_count()
+    op.apply(psi, cfg.mass)  # pack + apply + unpack
+    assert binding.wd_launch_count() - n0 == 3
+    op.close()
