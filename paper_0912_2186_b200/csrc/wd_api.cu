@@ -222,7 +222,7 @@ static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double m
         if (!wd::tile_supported(a)) return fail(WD_ERR_MISMATCH, "wd_apply: tiled kernel cannot take this call");
         e = wd::launch_tile(a);
     } else
-        e = wd::tile_supported(a) ? wd::launch_tile(a) : wd::launch_site(a);
+        e = wd::tile_preferred(a) ? wd::launch_tile(a) : wd::launch_site(a);
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply: kernel launch");
 }
 

@@ -9,23 +9,11 @@
 #include "wd_internal.h"
 #include "wd_layout.cuh"
 #include "wd_math.cuh"
+#include "wd_link.cuh"
 
 namespace wd {
 
 constexpr int SITE_THREADS = 128;
-
-template <typename T, int RECON>
-__device__ __forceinline__ void load_link(const T *__restrict__ links, long long V, int mu, long long site, T (&u)[18])
-{
-    using L = LinkLayout<T, RECON>;
-    const typename L::Vec *q = reinterpret_cast<const typename L::Vec *>(links) + (long long)mu * L::NCH * V + site;
-#pragma unroll
-    for (int c = 0; c < L::NCH; ++c) {
-        const typename L::Vec v = __ldg(q + (long long)c * V);
-        unpack(v, &u[c * L::CR]);
-    }
-    if (RECON == 12) reconstruct_row2(u);
-}
 
 template <int MU, typename T, int RECON, int NR>
 __device__ __forceinline__ void hop_pair(T (&acc)[NR][24], const T *__restrict__ in, const T *__restrict__ links,
@@ -55,6 +43,9 @@ __global__ void __launch_bounds__(SITE_THREADS)
 dslash_site_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ links, int Lx, int Ly, int Lz,
                    int Lt, long long V, T cdiag, int nrhs)
 {
+    // grid = (site blocks, RHS groups), site blocks fastest: one sweep over the lattice per group.
+    // (Measured on B200: making the RHS group the fastest index keeps the links in L2 but pushes
+    // the t-neighbour reuse distance of the spinors past L2 and is 30 % slower.)
     const long long site = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
     if (site >= V) return;
     const int rhs0 = blockIdx.y * NR;

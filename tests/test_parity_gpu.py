@@ -79,6 +79,57 @@ def test_nrhs_sweep(oracle, nrhs):
     check_config(oracle, cfg, "auto")
 
 
+# ---------------------------------------------------------------- the shared-memory t-marching kernel
+TILE_SHAPES = [(32, 4, 4, 4), (16, 8, 8, 6), (8, 4, 4, 12), (4, 8, 16, 5), (32, 8, 8, 3), (32, 2, 2, 2), (16, 2, 4, 1),
+               (32, 1, 1, 1), (8, 12, 4, 7)]
+
+
+@pytest.mark.parametrize("dims", TILE_SHAPES)
+@pytest.mark.parametrize("precision,recon", [(32, 18), (32, 12), (64, 18), (64, 12)])
+def test_tile_kernel_shapes(oracle, dims, precision, recon):
+    cfg = fields.Config("tile", dims, precision, "haar", recon, -0.3, 1, 13)
+    check_config(oracle, cfg, "tile", nrhs=1)
+    check_config(oracle, cfg, "tile", nrhs=3)
+
+
+@pytest.mark.parametrize("shape", ["1,1", "2,1", "2,2", "4,1", "4,2", "8,1", "1,2", "2,4"])
+@pytest.mark.parametrize("precision", [32, 64])
+def test_tile_kernel_forced_tile_shapes(oracle, monkeypatch, shape, precision):
+    """Every tile shape (WD_TILE_SHAPE=ty,tz) gives the same operator; shapes the precision cannot
+    hold fall back to the automatic choice, which must still be right."""
+    monkeypatch.setenv("WD_TILE_SHAPE", shape)
+    cfg = fields.Config("tileshape", (32, 8, 8, 5), precision, "smooth", 18, -0.42, 1, 17)
+    check_config(oracle, cfg, "tile")
+
+
+@pytest.mark.parametrize("name", ["c1_16x32_fp32", "c3_32x64_fp32", "c3_32x64_fp64"])
+def test_tile_kernel_baseline_configs(oracle, name):
+    check_config(oracle, fields.CONFIGS[name], "tile")
+
+
+def test_tile_kernel_rejects_unsupported_lattice():
+    from paper_0912_2186_b200 import binding
+    cfg = fields.Config("bad", (24, 4, 4, 4), 32, "haar", 18, 0.1, 1, 3)
+    U, _ = fields.make_fields(cfg)
+    op = GpuOp(U, cfg.dims, 32, 18)
+    with pytest.raises(binding.WdError) as e:
+        binding.wd_set_kernel(op.op.gauge, KERNELS["tile"])
+    assert e.value.code == -7
+    op.close()
+
+
+def test_tile_kernel_deterministic():
+    import torch
+    cfg = fields.Config("det", (32, 8, 8, 16), 32, "smooth", 18, -0.42, 1, 19)
+    U, psi = fields.make_fields(cfg)
+    op = GpuOp(U, cfg.dims, 32, 18, KERNELS["tile"])
+    a = op.apply(psi, cfg.mass, return_native=True).clone()
+    for _ in range(20):
+        b = op.apply(psi, cfg.mass, return_native=True)
+    assert torch.equal(a, b)
+    op.close()
+
+
 # ---------------------------------------------------------------- invariants of the CUDA path itself
 def test_deterministic_and_repeatable():
     """No atomics: launch #100 on input A is bit-identical to launch #1 on input A (S9)."""
