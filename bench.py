@@ -225,8 +225,8 @@ def run_wd(args):
         u_dev = torch.from_numpy(U).to(dev)
         op = binding.WilsonDirac(cfg.dims, u_dev, cfg.precision, recon, stream=stream.cuda_stream, kernel=kernel)
         canon = torch.from_numpy(psi).to(dev)
-        ins = [torch.empty(nrhs * V * 24, dtype=tdt, device=dev) for _ in range(NBUF)]
-        outs = [torch.empty(nrhs * V * 24, dtype=tdt, device=dev) for _ in range(NBUF)]
+        ins = [torch.empty(op.native_numel(nrhs), dtype=tdt, device=dev) for _ in range(NBUF)]
+        outs = [torch.empty(op.native_numel(nrhs), dtype=tdt, device=dev) for _ in range(NBUF)]
         op.pack(ins[0], canon, nrhs)
         for b in range(1, NBUF):  # distinct inputs: scaled copies of the packed field
             torch.mul(ins[0], 1.0 + 0.25 * b, out=ins[b])

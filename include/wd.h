@@ -33,7 +33,9 @@
  *           mu = 0,1,2,3 <-> x,y,z,t; dims = {Lx, Ly, Lz, Lt}; U_mu(x) sits on the link
  *           x -> x+mu and (U psi)_a = sum_b U[a][b] psi_b            (readings S5, S6)
  * NATIVE layouts (what wd_apply reads and writes):
- *   spinor  [rhs][chunk][site] of 16-byte chunks (float4 / double2), site = x + Lx*(y + Ly*(z + Lz*t))
+ *   spinor  [rhs][block of 32 sites][16-byte vector (float4 / double2)][lane], site = 32*block + lane
+ *           = x + Lx*(y + Ly*(z + Lz*t)); the volume is padded to a multiple of 32 sites, so a native
+ *           buffer holds wd_spinor_bytes() bytes (>= nrhs*V*24*sizeof(real)); pad sites are never read.
  *   links   private to wd_gauge.
  *   wd_pack_spinor / wd_unpack_spinor convert between the two, so a Krylov loop (100 applies
  *   back to back, BASELINE.json:configs[3]) never repacks.
@@ -106,13 +108,14 @@ int wd_set_stream(wd_gauge *gauge, void *stream);
 /* Force a kernel variant (wd_kernel).  WD_ERR_MISMATCH if it cannot handle the lattice. */
 int wd_set_kernel(wd_gauge *gauge, int kernel);
 
-/* Bytes of a NATIVE spinor buffer holding nrhs fields: nrhs * V * 24 * sizeof(real). */
+/* Bytes of a NATIVE spinor buffer holding nrhs fields: nrhs * Vpad * 24 * sizeof(real), where
+ * Vpad = V rounded up to a multiple of 32 sites.  0 on bad arguments. */
 size_t wd_spinor_bytes(const wd_lattice *lat, int nrhs, int precision);
 
 /*
  * wd_pack_spinor / wd_unpack_spinor -- CANONICAL <-> NATIVE spinor layout on the device
- * (pure data movement, no arithmetic), enqueued on `stream`.  Both buffers hold nrhs fields
- * of V*24 reals of the given precision and must not overlap.
+ * (pure data movement, no arithmetic), enqueued on `stream`.  The canonical buffer holds nrhs
+ * fields of V*24 reals, the native buffer wd_spinor_bytes() bytes; they must not overlap.
  */
 int wd_pack_spinor(const wd_lattice *lat, void *native_dev, const void *canonical_dev, int nrhs,
                    int precision, void *stream);

@@ -201,6 +201,10 @@ class WilsonDirac:
     def unpack(self, canonical_dev, native_dev, nrhs, stream=None):
         wd_unpack_spinor(self.lat, canonical_dev, native_dev, nrhs, self.precision, stream or self.stream)
 
+    def native_numel(self, nrhs=1):
+        """Reals in a NATIVE spinor buffer of nrhs fields (the volume is padded to 32-site blocks)."""
+        return wd_spinor_bytes(self.lat, nrhs, self.precision) // (4 if self.precision == 32 else 8)
+
     def apply(self, out_native_dev, in_native_dev, mass, nrhs=1):
         wd_apply(out_native_dev, in_native_dev, self.gauge, mass, self.dims, nrhs, self.precision)
 

@@ -9,6 +9,7 @@
 
 #include "../../include/wd.h"
 #include "wd_internal.h"
+#include "wd_layout.cuh"
 
 namespace {
 
@@ -47,10 +48,10 @@ long long checked_volume(const int dims[4])
     return v;
 }
 
-bool overlap(const void *a, const void *b, size_t bytes)
+bool overlap(const void *a, size_t abytes, const void *b, size_t bbytes)
 {
     const uintptr_t pa = (uintptr_t)a, pb = (uintptr_t)b;
-    return pa < pb + bytes && pb < pa + bytes;
+    return pa < pb + bbytes && pb < pa + abytes;
 }
 
 int check_apply_args(const void *out, const void *in, const wd_gauge *g, const int dims[4], int nrhs, int precision)
@@ -107,7 +108,7 @@ long long wd_lattice_volume(const wd_lattice *lat)
 size_t wd_spinor_bytes(const wd_lattice *lat, int nrhs, int precision)
 {
     if (!lat || lat->magic != LATTICE_MAGIC || nrhs < 1 || !valid_precision(precision)) return 0;
-    return (size_t)nrhs * (size_t)lat->V * 24 * (precision == WD_FP32 ? 4 : 8);
+    return (size_t)nrhs * (size_t)wd::padded_volume(lat->V) * 24 * (precision == WD_FP32 ? 4 : 8);
 }
 
 int wd_load_gauge(const wd_lattice *lat, const void *links_canonical_dev, int precision, int recon, void *stream,
@@ -174,13 +175,18 @@ int wd_set_kernel(wd_gauge *gauge, int kernel)
     return WD_OK;
 }
 
-static int check_pack_args(const char *who, const wd_lattice *lat, const void *a, const void *b, int nrhs, int precision)
+// native: wd_spinor_bytes() bytes (padded volume); canonical: nrhs * V * 24 reals
+static int check_pack_args(const char *who, const wd_lattice *lat, const void *native, const void *canonical, int nrhs,
+                           int precision)
 {
+    const void *a = native, *b = canonical;
     if (!lat || !a || !b) return fail(WD_ERR_NULL, "%s: NULL argument", who);
     if (lat->magic != LATTICE_MAGIC) return fail(WD_ERR_MISMATCH, "%s: not a live wd_lattice handle", who);
     if (!valid_precision(precision)) return fail(WD_ERR_PRECISION, "%s: precision %d is not 32 or 64", who, precision);
     if (nrhs < 1) return fail(WD_ERR_NRHS, "%s: nrhs=%d", who, nrhs);
-    if (overlap(a, b, wd_spinor_bytes(lat, nrhs, precision))) return fail(WD_ERR_ALIAS, "%s: buffers overlap", who);
+    const size_t cbytes = (size_t)nrhs * (size_t)lat->V * 24 * (precision == WD_FP32 ? 4 : 8);
+    if (overlap(native, wd_spinor_bytes(lat, nrhs, precision), canonical, cbytes))
+        return fail(WD_ERR_ALIAS, "%s: buffers overlap", who);
     return WD_OK;
 }
 
@@ -196,7 +202,7 @@ int wd_pack_spinor(const wd_lattice *lat, void *native_dev, const void *canonica
 int wd_unpack_spinor(const wd_lattice *lat, void *canonical_dev, const void *native_dev, int nrhs, int precision,
                      void *stream)
 {
-    int rc = check_pack_args("wd_unpack_spinor", lat, canonical_dev, native_dev, nrhs, precision);
+    int rc = check_pack_args("wd_unpack_spinor", lat, native_dev, canonical_dev, nrhs, precision);
     if (rc) return rc;
     cudaError_t e = wd::launch_unpack_spinor(canonical_dev, native_dev, lat->V, nrhs, precision, (cudaStream_t)stream);
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_unpack_spinor");
@@ -231,8 +237,8 @@ int wd_apply(void *out_native_dev, const void *in_native_dev, const wd_gauge *ga
 {
     int rc = check_apply_args(out_native_dev, in_native_dev, gauge, dims, nrhs, precision);
     if (rc) return rc;
-    const size_t bytes = (size_t)nrhs * (size_t)gauge->V * 24 * (precision == WD_FP32 ? 4 : 8);
-    if (overlap(out_native_dev, in_native_dev, bytes)) return fail(WD_ERR_ALIAS, "wd_apply: out and in overlap");
+    const size_t bytes = (size_t)nrhs * (size_t)wd::padded_volume(gauge->V) * 24 * (precision == WD_FP32 ? 4 : 8);
+    if (overlap(out_native_dev, bytes, in_native_dev, bytes)) return fail(WD_ERR_ALIAS, "wd_apply: out and in overlap");
     if (((uintptr_t)out_native_dev | (uintptr_t)in_native_dev) & 15)
         return fail(WD_ERR_MISMATCH, "wd_apply: buffers must be 16-byte aligned");
     return dispatch_apply(out_native_dev, in_native_dev, gauge, mass, nrhs);
@@ -244,25 +250,26 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
     int rc = check_apply_args(out_canonical_host, in_canonical_host, gauge, dims, nrhs, precision);
     if (rc) return rc;
     wd_gauge *g = gauge;
-    const size_t bytes = (size_t)nrhs * (size_t)g->V * 24 * (precision == WD_FP32 ? 4 : 8);
-    if (g->stage_bytes < bytes) {
+    const size_t bytes = (size_t)nrhs * (size_t)g->V * 24 * (precision == WD_FP32 ? 4 : 8); // canonical
+    const size_t nbytes = (size_t)nrhs * (size_t)wd::padded_volume(g->V) * 24 * (precision == WD_FP32 ? 4 : 8); // native
+    if (g->stage_bytes < nbytes) {
         cudaFree(g->stage_canon);
         cudaFree(g->stage_in);
         cudaFree(g->stage_out);
         g->stage_canon = g->stage_in = g->stage_out = nullptr;
         g->stage_bytes = 0;
-        cudaError_t e = cudaMalloc(&g->stage_canon, bytes);
-        if (e == cudaSuccess) e = cudaMalloc(&g->stage_in, bytes);
-        if (e == cudaSuccess) e = cudaMalloc(&g->stage_out, bytes);
+        cudaError_t e = cudaMalloc(&g->stage_canon, nbytes);
+        if (e == cudaSuccess) e = cudaMalloc(&g->stage_in, nbytes);
+        if (e == cudaSuccess) e = cudaMalloc(&g->stage_out, nbytes);
         if (e != cudaSuccess) {
             cudaFree(g->stage_canon);
             cudaFree(g->stage_in);
             cudaFree(g->stage_out);
             g->stage_canon = g->stage_in = g->stage_out = nullptr;
             cudaGetLastError();
-            return fail(WD_ERR_ALLOC, "wd_apply_host: cudaMalloc of %zu staging bytes failed", 3 * bytes);
+            return fail(WD_ERR_ALLOC, "wd_apply_host: cudaMalloc of %zu staging bytes failed", 3 * nbytes);
         }
-        g->stage_bytes = bytes;
+        g->stage_bytes = nbytes;
     }
     cudaStream_t s = g->stream;
     cudaError_t e = cudaMemcpyAsync(g->stage_canon, in_canonical_host, bytes, cudaMemcpyHostToDevice, s);

@@ -6,6 +6,7 @@
 //
 // A thread handles NR right-hand sides of its site: each link is loaded (and, for recon 12,
 // rebuilt) once per direction and reused for the NR spinors (step a').
+#include <cstdlib>
 #include "wd_internal.h"
 #include "wd_layout.cuh"
 #include "wd_math.cuh"
@@ -17,23 +18,23 @@ constexpr int SITE_THREADS = 128;
 
 template <int MU, typename T, int RECON, int NR>
 __device__ __forceinline__ void hop_pair(T (&acc)[NR][24], const T *__restrict__ in, const T *__restrict__ links,
-                                         long long V, long long site, long long sf, long long sb, int rhs0, int nrhs)
+                                         long long Vp, long long site, long long sf, long long sb, int rhs0, int nrhs)
 {
     T u[18];
-    load_link<T, RECON>(links, V, MU, site, u); // U_mu(x)
+    load_link<MU, T, RECON>(links, site, u); // U_mu(x)
 #pragma unroll
     for (int r = 0; r < NR; ++r)
         if (rhs0 + r < nrhs) {
             T p[24];
-            load_spinor(in + (long long)(rhs0 + r) * 24 * V, V, sf, p); // psi(x+mu)
+            load_spinor(in + (long long)(rhs0 + r) * 24 * Vp, sf, p); // psi(x+mu)
             hop_forward<MU>(acc[r], u, p);
         }
-    load_link<T, RECON>(links, V, MU, sb, u); // U_mu(x-mu)
+    load_link<MU, T, RECON>(links, sb, u); // U_mu(x-mu)
 #pragma unroll
     for (int r = 0; r < NR; ++r)
         if (rhs0 + r < nrhs) {
             T p[24];
-            load_spinor(in + (long long)(rhs0 + r) * 24 * V, V, sb, p); // psi(x-mu)
+            load_spinor(in + (long long)(rhs0 + r) * 24 * Vp, sb, p); // psi(x-mu)
             hop_backward<MU>(acc[r], u, p);
         }
 }
@@ -41,14 +42,24 @@ __device__ __forceinline__ void hop_pair(T (&acc)[NR][24], const T *__restrict__
 template <typename T, int RECON, int NR>
 __global__ void __launch_bounds__(SITE_THREADS)
 dslash_site_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ links, int Lx, int Ly, int Lz,
-                   int Lt, long long V, T cdiag, int nrhs)
+                   int Lt, long long V, T cdiag, int nrhs, int bps)
 {
-    // grid = (site blocks, RHS groups), site blocks fastest: one sweep over the lattice per group.
-    // (Measured on B200: making the RHS group the fastest index keeps the links in L2 but pushes
-    // the t-neighbour reuse distance of the spinors past L2 and is 30 % slower.)
-    const long long site = (long long)blockIdx.x * SITE_THREADS + threadIdx.x;
+    // Block order (step a'): the lattice is cut into SLABS of bps consecutive site blocks (a few time
+    // slices); within a slab all RHS groups are swept one after the other, then the next slab.  The
+    // links of a slab (sized to stay in L2) come from HBM once and serve every group; the spinors of
+    // a group keep their short t-neighbour reuse distance.  (Measured on B200: one sweep of the whole
+    // lattice per group re-reads the 604 MB gauge field 12 x from HBM; RHS group fastest loses the
+    // spinors' t reuse instead and is slower still.)
+    const int ngroups = (nrhs + NR - 1) / NR;
+    const long long nb = (V + SITE_THREADS - 1) / SITE_THREADS;
+    const long long bid = blockIdx.x;
+    const long long slab = bid / ((long long)bps * ngroups);
+    const long long nbl = min((long long)bps, nb - slab * bps); // site blocks in this slab
+    const long long r = bid - slab * bps * ngroups;
+    const long long site = (slab * bps + r % nbl) * SITE_THREADS + threadIdx.x;
     if (site >= V) return;
-    const int rhs0 = blockIdx.y * NR;
+    const int rhs0 = (int)(r / nbl) * NR;
+    const long long Vp = padded_volume(V); // sites per right-hand side in the native layout
 
     // periodic neighbours (step a1): coordinates from the lexicographic index, wrap by compare
     long long rem = site;
@@ -68,30 +79,44 @@ dslash_site_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
 #pragma unroll
         for (int i = 0; i < 24; ++i) acc[r][i] = (T)0;
 
-    hop_pair<0, T, RECON, NR>(acc, in, links, V, site, xf, xb, rhs0, nrhs);
-    hop_pair<1, T, RECON, NR>(acc, in, links, V, site, yf, yb, rhs0, nrhs);
-    hop_pair<2, T, RECON, NR>(acc, in, links, V, site, zf, zb, rhs0, nrhs);
-    hop_pair<3, T, RECON, NR>(acc, in, links, V, site, tf, tb, rhs0, nrhs);
+    hop_pair<0, T, RECON, NR>(acc, in, links, Vp, site, xf, xb, rhs0, nrhs);
+    hop_pair<1, T, RECON, NR>(acc, in, links, Vp, site, yf, yb, rhs0, nrhs);
+    hop_pair<2, T, RECON, NR>(acc, in, links, Vp, site, zf, zb, rhs0, nrhs);
+    hop_pair<3, T, RECON, NR>(acc, in, links, Vp, site, tf, tb, rhs0, nrhs);
 
     // fused diagonal (step a6): out = (4+m) psi(x) - 1/2 acc
 #pragma unroll
     for (int r = 0; r < NR; ++r)
         if (rhs0 + r < nrhs) {
             T p[24];
-            load_spinor(in + (long long)(rhs0 + r) * 24 * V, V, site, p);
+            load_spinor(in + (long long)(rhs0 + r) * 24 * Vp, site, p);
 #pragma unroll
             for (int i = 0; i < 24; ++i) p[i] = fma(cdiag, p[i], (T)-0.5 * acc[r][i]);
-            store_spinor(out + (long long)(rhs0 + r) * 24 * V, V, site, p);
+            store_spinor(out + (long long)(rhs0 + r) * 24 * Vp, site, p);
         }
 }
 
 template <typename T, int RECON, int NR>
 static cudaError_t launch_site_t(const ApplyArgs &a)
 {
-    dim3 grid((unsigned)((a.V + SITE_THREADS - 1) / SITE_THREADS), (unsigned)((a.nrhs + NR - 1) / NR));
+    const long long nb = (a.V + SITE_THREADS - 1) / SITE_THREADS;
+    const long long ngroups = (a.nrhs + NR - 1) / NR;
+    if (nb * ngroups > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    // slab: ~32 MB of links (WD_SITE_SLAB_MB overrides) -- a fraction of the 126 MB L2, leaving room
+    // for the spinor streams of the groups passing through
+    double slab_mb = 32.0;
+    if (const char *ev = getenv("WD_SITE_SLAB_MB")) {
+        const double v = atof(ev);
+        if (v > 0) slab_mb = v;
+    }
+    long long bps = (long long)(slab_mb * 1e6 / ((double)SITE_THREADS * 4 * RECON * sizeof(T)));
+    if (ngroups == 1 || bps > nb) bps = nb;
+    if (bps < 1) bps = 1;
+    dim3 grid((unsigned)(nb * ngroups));
     const T cdiag = (T)(4.0 + a.mass); // formed in double, rounded once (reading S8)
     dslash_site_kernel<T, RECON, NR><<<grid, SITE_THREADS, 0, a.stream>>>(
-        (T *)a.out, (const T *)a.in, (const T *)a.links, a.dims[0], a.dims[1], a.dims[2], a.dims[3], a.V, cdiag, a.nrhs);
+        (T *)a.out, (const T *)a.in, (const T *)a.links, a.dims[0], a.dims[1], a.dims[2], a.dims[3], a.V, cdiag, a.nrhs,
+        (int)bps);
     count_launch();
     return cudaGetLastError();
 }

@@ -72,22 +72,6 @@ __device__ __forceinline__ void lds_half(const typename SpinorLayout<T>::Vec *bu
     for (int c = 0; c < L::NCH / 2; ++c) unpack(buf[c * nt + slot], &h[c * L::CR]);
 }
 
-// Pull the four links of `site` (the slice this thread handles NEXT) from HBM into L2 while the
-// current slice is being computed: each link is used by exactly one thread exactly once, so
-// without this every link load pays the full HBM latency inside the dependent chain.
-template <typename T, int RECON>
-__device__ __forceinline__ void prefetch_links_l2(const T *__restrict__ links, long long V, long long site)
-{
-    using L = LinkLayout<T, RECON>;
-    const typename L::Vec *q = reinterpret_cast<const typename L::Vec *>(links) + site;
-#pragma unroll
-    // one request per 128-byte line: only the lane whose chunk starts a line asks for it
-    if (((threadIdx.x & 31) * sizeof(typename L::Vec)) % 128 == 0) {
-#pragma unroll
-        for (int c = 0; c < 4 * L::NCH; ++c) asm volatile("prefetch.global.L2 [%0];\n" ::"l"(q + (long long)c * V));
-    }
-}
-
 template <typename T>
 __device__ __forceinline__ void shfl_half(T (&dst)[12], const T (&src)[12], int src_lane)
 {
@@ -102,7 +86,7 @@ template <typename T> constexpr size_t tile_smem_bytes(int nt) { return (size_t)
 
 // One launch = out = D in for one right-hand side (rhs = blockIdx.y).
 //   dims Lx (power of two, 4..32), Ly % ty == 0, Lz % tz == 0, blockDim.x = Lx*ty*tz (multiple of 32)
-template <typename T, int RECON, int MAXT, int MINB, bool PF>
+template <typename T, int RECON, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB)
 dslash_tile_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ links, int Lx, int Ly, int Lz,
                    int Lt, int ty, int tz, long long V, T cdiag)
@@ -117,9 +101,8 @@ dslash_tile_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
     Vec *xchg_y = plane0 + 2 * plane_sz;     // U_y^dag P+_y psi of every tile site, for the site at y+1
     Vec *xchg_z = xchg_y + (NCH / 2) * nt;   // same for z
 
-    in += (long long)blockIdx.y * 24 * V;
-    out += (long long)blockIdx.y * 24 * V;
-    const Vec *in_v = reinterpret_cast<const Vec *>(in);
+    in += (long long)blockIdx.y * 24 * padded_volume(V);
+    out += (long long)blockIdx.y * 24 * padded_volume(V);
 
     // thread <-> site of the tile: x fastest, then y, then z (x-rows are (parts of) warps)
     const int x = tid & (Lx - 1);
@@ -156,12 +139,12 @@ dslash_tile_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
     {   // ---- start the march at slice t_begin ----
         const long long site = s3 + (long long)t_begin * S3;
 #pragma unroll
-        for (int c = 0; c < NCH; ++c) cp_async16(&plane0[cur * plane_sz + c * nt + tid], in_v + (long long)c * V + site);
+        for (int c = 0; c < NCH; ++c) cp_async16(&plane0[cur * plane_sz + c * nt + tid], spinor_ptr(in, site) + c * BLK);
         cp_async_commit();
         const long long site_tb = s3 + (long long)(t_begin == 0 ? Lt - 1 : t_begin - 1) * S3;
         T u[18], p[24], h[12];
-        load_link<T, RECON>(links, V, 3, site_tb, u);
-        load_spinor(in, V, site_tb, p);
+        load_link<3, T, RECON>(links, site_tb, u);
+        load_spinor(in, site_tb, p);
         project<3, +1>(p, h);
         su3_dag_mul(u, h, chi_t);
     }
@@ -172,10 +155,9 @@ dslash_tile_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
         {   // slice t+1 of this tile -> the other buffer (its previous content, slice t-1, is no longer read)
             const long long site_tf = s3 + (long long)(t + 1 == Lt ? 0 : t + 1) * S3;
 #pragma unroll
-            for (int c = 0; c < NCH; ++c) cp_async16(&plane0[(cur ^ 1) * plane_sz + c * nt + tid], in_v + (long long)c * V + site_tf);
+            for (int c = 0; c < NCH; ++c) cp_async16(&plane0[(cur ^ 1) * plane_sz + c * nt + tid], spinor_ptr(in, site_tf) + c * BLK);
             cp_async_commit();
         }
-        if (PF) prefetch_links_l2<T, RECON>(links, V, s3 + (long long)(t + 1 == Lt ? 0 : t + 1) * S3);
         asm volatile("cp.async.wait_group 1;\n" ::: "memory"); // slice t has landed (own part)
         __syncthreads();                                        // (A) ... and everybody else's
 
@@ -187,7 +169,7 @@ dslash_tile_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
         reconstruct_add<3, +1>(acc, chi_t); // backward t hop, product carried from the previous slice
 
         // ---- x: both hops through warp shuffles ----
-        load_link<T, RECON>(links, V, 0, site, u);
+        load_link<0, T, RECON>(links, site, u);
         {
             T h[12], g[12], chi[12];
             project<0, -1>(psi, h);
@@ -200,39 +182,39 @@ dslash_tile_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
             reconstruct_add<0, +1>(acc, g);
         }
         // ---- y ----
-        load_link<T, RECON>(links, V, 1, site, u);
+        load_link<1, T, RECON>(links, site, u);
         {
             T pn[24], h[12], chi[12];
-            if (face_yf) load_spinor(in, V, s3_yf + toff, pn);
+            if (face_yf) load_spinor(in, s3_yf + toff, pn);
             else lds_spinor<T>(pl, nt, slot_yf, pn);
             hop_forward<1>(acc, u, pn);
             project<1, +1>(psi, h);
             su3_dag_mul(u, h, chi);
             sts_half<T>(xchg_y, nt, tid, chi);
             if (face_yb) { // the site below is outside the tile: do its backward hop here
-                load_link<T, RECON>(links, V, 1, s3_yb + toff, u);
-                load_spinor(in, V, s3_yb + toff, pn);
+                load_link<1, T, RECON>(links, s3_yb + toff, u);
+                load_spinor(in, s3_yb + toff, pn);
                 hop_backward<1>(acc, u, pn);
             }
         }
         // ---- z ----
-        load_link<T, RECON>(links, V, 2, site, u);
+        load_link<2, T, RECON>(links, site, u);
         {
             T pn[24], h[12], chi[12];
-            if (face_zf) load_spinor(in, V, s3_zf + toff, pn);
+            if (face_zf) load_spinor(in, s3_zf + toff, pn);
             else lds_spinor<T>(pl, nt, slot_zf, pn);
             hop_forward<2>(acc, u, pn);
             project<2, +1>(psi, h);
             su3_dag_mul(u, h, chi);
             sts_half<T>(xchg_z, nt, tid, chi);
             if (face_zb) {
-                load_link<T, RECON>(links, V, 2, s3_zb + toff, u);
-                load_spinor(in, V, s3_zb + toff, pn);
+                load_link<2, T, RECON>(links, s3_zb + toff, u);
+                load_spinor(in, s3_zb + toff, pn);
                 hop_backward<2>(acc, u, pn);
             }
         }
         // ---- t: forward hop now, backward product for the next slice ----
-        load_link<T, RECON>(links, V, 3, site, u);
+        load_link<3, T, RECON>(links, site, u);
         cp_async_wait_all(); // own spinor of slice t+1 has landed in the other buffer
         {
             T pn[24], h[12];
@@ -255,7 +237,7 @@ dslash_tile_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
         // fused diagonal (step a6) and store (a7)
 #pragma unroll
         for (int i = 0; i < 24; ++i) psi[i] = fma(cdiag, psi[i], (T)-0.5 * acc[i]);
-        store_spinor(out, V, site, psi);
+        store_spinor(out, site, psi);
         cur ^= 1;
     }
     cp_async_wait_all();
@@ -311,8 +293,7 @@ cudaError_t launch_tile_t(const ApplyArgs &a)
 {
     constexpr int MAXT = tile_max_threads<T>();
     constexpr int MINB = 2;
-    static const bool pf = !(getenv("WD_TILE_PF") && atoi(getenv("WD_TILE_PF")) == 0);
-    auto kern = pf ? dslash_tile_kernel<T, RECON, MAXT, MINB, true> : dslash_tile_kernel<T, RECON, MAXT, MINB, false>;
+    auto kern = dslash_tile_kernel<T, RECON, MAXT, MINB>;
     TileShape s;
     if (!choose_shape(a, MAXT, s)) return cudaErrorInvalidConfiguration;
     const size_t smem = tile_smem_bytes<T>(s.nt);

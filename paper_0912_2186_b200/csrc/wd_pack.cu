@@ -7,8 +7,9 @@ namespace wd {
 
 constexpr int PACK_SITES = 128; // sites per CTA; also the CTA size
 
-// canonical [rhs][site][NCH chunks]  <->  native [rhs][chunk][site]; transposed through shared
-// memory so that both the global reads and the global writes are contiguous 16-byte-per-lane.
+// canonical [rhs][site][NCH vectors]  <->  native [rhs][block][vector][lane] (wd_layout.cuh);
+// transposed through shared memory so that both the global reads and the global writes are
+// contiguous 16-byte-per-lane.  Pad sites of the last native block are left untouched.
 template <typename Vec, int NCH, bool TO_NATIVE>
 __global__ void __launch_bounds__(PACK_SITES) spinor_transpose_kernel(Vec *__restrict__ dst, const Vec *__restrict__ src,
                                                                      long long V)
@@ -20,6 +21,8 @@ __global__ void __launch_bounds__(PACK_SITES) spinor_transpose_kernel(Vec *__res
     const long long nsite = min((long long)PACK_SITES, V - site0);
     const Vec *canon_src = src + ((long long)rhs * V + site0) * NCH;
     Vec *canon_dst = dst + ((long long)rhs * V + site0) * NCH;
+    // native vector 0 of site site0 + tid (site0 is a multiple of 32)
+    const long long nat = (long long)rhs * padded_volume(V) * NCH + ((site0 + tid) >> 5) * (NCH * BLK) + (tid & (BLK - 1));
     if (TO_NATIVE) {
 #pragma unroll
         for (int i = 0; i < NCH; ++i) {
@@ -29,12 +32,12 @@ __global__ void __launch_bounds__(PACK_SITES) spinor_transpose_kernel(Vec *__res
         __syncthreads();
         if (tid < nsite) {
 #pragma unroll
-            for (int c = 0; c < NCH; ++c) dst[((long long)rhs * NCH + c) * V + site0 + tid] = tile[c][tid];
+            for (int c = 0; c < NCH; ++c) dst[nat + c * BLK] = tile[c][tid];
         }
     } else {
         if (tid < nsite) {
 #pragma unroll
-            for (int c = 0; c < NCH; ++c) tile[c][tid] = src[((long long)rhs * NCH + c) * V + site0 + tid];
+            for (int c = 0; c < NCH; ++c) tile[c][tid] = src[nat + c * BLK];
         }
         __syncthreads();
 #pragma unroll
@@ -69,36 +72,39 @@ cudaError_t launch_unpack_spinor(void *canonical, const void *native, long long 
     return transpose_spinor<false>(canonical, native, V, nrhs, precision, s);
 }
 
-// canonical U[mu][site][a][b][re,im] -> native [mu][chunk][site]; recon 12 keeps rows a = 0,1.
+// canonical U[mu][site][a][b][re,im] -> native [block][vector][lane], the four links of a site
+// together (wd_layout.cuh); recon 12 keeps rows a = 0,1 of every link.
 template <typename T, int RECON>
 __global__ void pack_links_kernel(T *__restrict__ dst, const T *__restrict__ src, long long V)
 {
     using L = LinkLayout<T, RECON>;
     const long long site = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int mu = blockIdx.y;
     if (site >= V) return;
-    const T *p = src + ((long long)mu * V + site) * 18;
-    typename L::Vec *q = reinterpret_cast<typename L::Vec *>(dst) + (long long)mu * L::NCH * V + site;
+    typename L::Vec *q = reinterpret_cast<typename L::Vec *>(dst) + (site >> 5) * (L::NVEC * BLK) + (site & (BLK - 1));
+    T r[4 * RECON];
 #pragma unroll
-    for (int c = 0; c < L::NCH; ++c) {
-        T r[L::CR];
+    for (int mu = 0; mu < 4; ++mu) {
+        const T *p = src + ((long long)mu * V + site) * 18;
 #pragma unroll
-        for (int k = 0; k < L::CR; ++k) r[k] = p[c * L::CR + k];
+        for (int i = 0; i < RECON; ++i) r[mu * RECON + i] = p[i];
+    }
+#pragma unroll
+    for (int j = 0; j < L::NVEC; ++j) {
         typename L::Vec v;
-        pack(v, r);
-        q[(long long)c * V] = v;
+        pack(v, &r[j * L::CR]);
+        q[j * BLK] = v;
     }
 }
 
 size_t native_link_bytes(long long V, int precision, int recon)
 {
-    return (size_t)4 * (size_t)V * (size_t)recon * (precision == 32 ? 4 : 8);
+    return (size_t)4 * (size_t)padded_volume(V) * (size_t)recon * (precision == 32 ? 4 : 8);
 }
 
 cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon, cudaStream_t s)
 {
     if (V <= 0) return cudaSuccess;
-    dim3 grid((unsigned)((V + 127) / 128), 4);
+    dim3 grid((unsigned)((V + 127) / 128));
     if (precision == 32 && recon == 18)
         pack_links_kernel<float, 18><<<grid, 128, 0, s>>>((float *)native, (const float *)canonical, V);
     else if (precision == 32)

@@ -39,8 +39,9 @@ class GpuOp:
         psi = np.ascontiguousarray(psi, dtype=np_dtype(self.precision))
         nrhs = psi.shape[0]
         canon = torch.from_numpy(psi).cuda()
-        native_in = torch.empty_like(canon)
-        native_out = torch.full_like(canon, float("nan"))
+        n = self.op.native_numel(nrhs)  # >= canon.numel(): the native volume is padded to 32-site blocks
+        native_in = torch.full((n,), float("nan"), dtype=canon.dtype, device=canon.device)
+        native_out = torch.full((n,), float("nan"), dtype=canon.dtype, device=canon.device)
         self.op.pack(native_in, canon, nrhs)
         self.op.apply(native_out, native_in, mass, nrhs)
         if return_native:

@@ -181,24 +181,30 @@ def test_translation_covariance_through_native_layout():
 
 
 def test_pack_unpack_roundtrip_and_native_layout():
-    """Native layout is [rhs][chunk][site] of 16-byte chunks (include/wd.h); pure data movement."""
+    """Native layout is [rhs][block of 32 sites][16-byte vector][lane] (include/wd.h), the volume
+    padded to a multiple of 32 sites; pure data movement, pad sites untouched."""
     import torch
     from paper_0912_2186_b200 import binding
-    dims = (6, 4, 2, 5)
-    V = 6 * 4 * 2 * 5
-    for precision, cr in ((32, 4), (64, 2)):
-        psi = fields.gaussian_spinor(dims, 5, 3, precision)
-        lat = binding.wd_create_lattice(dims)
-        canon = torch.from_numpy(psi).cuda()
-        native = torch.empty_like(canon)
-        back = torch.empty_like(canon)
-        binding.wd_pack_spinor(lat, native, canon, 3, precision)
-        binding.wd_unpack_spinor(lat, back, native, 3, precision)
-        torch.cuda.synchronize()
-        assert torch.equal(back, canon)
-        want = psi.reshape(3, V, 24 // cr, cr).transpose(0, 2, 1, 3)
-        assert np.array_equal(native.cpu().numpy().reshape(3, 24 // cr, V, cr), want)
-        binding.wd_destroy(lat)
+    for dims in ((6, 4, 2, 5), (3, 5, 2, 7), (8, 4, 4, 4)):
+        V = int(np.prod(dims))
+        Vp = (V + 31) // 32 * 32
+        for precision, cr in ((32, 4), (64, 2)):
+            psi = fields.gaussian_spinor(dims, 5, 3, precision)
+            lat = binding.wd_create_lattice(dims)
+            assert binding.wd_spinor_bytes(lat, 3, precision) == 3 * Vp * 24 * (precision // 8)
+            canon = torch.from_numpy(psi).cuda()
+            native = torch.full((3 * Vp * 24,), -7.0, dtype=canon.dtype, device="cuda")
+            back = torch.empty_like(canon)
+            binding.wd_pack_spinor(lat, native, canon, 3, precision)
+            binding.wd_unpack_spinor(lat, back, native, 3, precision)
+            torch.cuda.synchronize()
+            assert torch.equal(back, canon)
+            nvec = 24 // cr
+            padded = np.full((3, Vp, nvec, cr), -7.0, dtype=psi.dtype)
+            padded[:, :V] = psi.reshape(3, V, nvec, cr)
+            want = padded.reshape(3, Vp // 32, 32, nvec, cr).transpose(0, 1, 3, 2, 4)
+            assert np.array_equal(native.cpu().numpy().reshape(3, Vp // 32, nvec, 32, cr), want)
+            binding.wd_destroy(lat)
 
 
 def test_apply_host_matches_device_path(oracle):
