@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the Wilson-Dirac matvec D*psi (eq. (2.2)) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--kernel auto|site|tile]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--kernel auto|site|tile|stage]
                     [--recon 18|12] [--impl wd|reference]
 
 One JSON line on stdout (rank 0).  Definitions:
@@ -214,7 +214,8 @@ def run_wd(args):
     nrhs = cfg.nrhs
     V = fields.volume(cfg.dims)
     tdt = torch.float32 if cfg.precision == 32 else torch.float64
-    kernel = {"auto": binding.WD_KERNEL_AUTO, "site": binding.WD_KERNEL_SITE, "tile": binding.WD_KERNEL_TILE}[args.kernel]
+    kernel = {"auto": binding.WD_KERNEL_AUTO, "site": binding.WD_KERNEL_SITE, "tile": binding.WD_KERNEL_TILE,
+              "stage": binding.WD_KERNEL_STAGE}[args.kernel]
 
     # ---- synthetic inputs (each rank its own replica: seeds shifted by rank) -------------------
     cfg_r = fields.Config(cfg.name, cfg.dims, cfg.precision, cfg.links, recon, cfg.mass, nrhs, cfg.seed + 100 * rank,
@@ -331,7 +332,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="c3_32x64_fp32", choices=sorted(fields.CONFIGS))
-    ap.add_argument("--kernel", default="auto", choices=["auto", "site", "tile"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "site", "tile", "stage"])
     ap.add_argument("--recon", type=int, default=None, choices=[18, 12])
     ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")

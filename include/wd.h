@@ -69,7 +69,8 @@ typedef enum { WD_RECON_18 = 18, WD_RECON_12 = 12 } wd_recon; /* reals stored pe
 typedef enum {
     WD_KERNEL_AUTO = 0,    /* fastest kernel valid for the lattice                         */
     WD_KERNEL_SITE = 1,    /* one thread per site, neighbours straight from L1/L2, any dims */
-    WD_KERNEL_TILE = 2     /* shared-memory tiled kernel (needs dims it supports)          */
+    WD_KERNEL_TILE = 2,    /* shared-memory tiled kernel (needs dims it supports)          */
+    WD_KERNEL_STAGE = 3    /* tiled kernel, all global reads staged by cp.async (fp32)     */
 } wd_kernel;
 
 typedef struct wd_lattice wd_lattice; /* opaque: extents, volume                           */

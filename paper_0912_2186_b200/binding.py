@@ -13,7 +13,7 @@ import os
 WD_OK = 0
 WD_FP32, WD_FP64 = 32, 64
 WD_RECON_18, WD_RECON_12 = 18, 12
-WD_KERNEL_AUTO, WD_KERNEL_SITE, WD_KERNEL_TILE = 0, 1, 2
+WD_KERNEL_AUTO, WD_KERNEL_SITE, WD_KERNEL_TILE, WD_KERNEL_STAGE = 0, 1, 2, 3
 
 STATUS_NAMES = {
     0: "WD_OK", -1: "WD_ERR_NULL", -2: "WD_ERR_DIMS", -3: "WD_ERR_PRECISION", -4: "WD_ERR_RECON",

@@ -158,16 +158,16 @@ int wd_set_kernel(wd_gauge *gauge, int kernel)
 {
     if (!gauge) return fail(WD_ERR_NULL, "wd_set_kernel: NULL gauge");
     if (gauge->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_set_kernel: not a live wd_gauge handle");
-    if (kernel != WD_KERNEL_AUTO && kernel != WD_KERNEL_SITE && kernel != WD_KERNEL_TILE)
+    if (kernel != WD_KERNEL_AUTO && kernel != WD_KERNEL_SITE && kernel != WD_KERNEL_TILE && kernel != WD_KERNEL_STAGE)
         return fail(WD_ERR_MISMATCH, "wd_set_kernel: unknown kernel %d", kernel);
-    if (kernel == WD_KERNEL_TILE) {
+    if (kernel == WD_KERNEL_TILE || kernel == WD_KERNEL_STAGE) {
         wd::ApplyArgs a{};
         for (int d = 0; d < 4; ++d) a.dims[d] = gauge->dims[d];
         a.V = gauge->V;
         a.nrhs = 1;
         a.precision = gauge->precision;
         a.recon = gauge->recon;
-        if (!wd::tile_supported(a))
+        if (!(kernel == WD_KERNEL_TILE ? wd::tile_supported(a) : wd::stage_supported(a)))
             return fail(WD_ERR_MISMATCH, "wd_set_kernel: tiled kernel does not support lattice %d %d %d %d", a.dims[0],
                         a.dims[1], a.dims[2], a.dims[3]);
     }
@@ -227,6 +227,9 @@ static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double m
     else if (g->kernel == WD_KERNEL_TILE) {
         if (!wd::tile_supported(a)) return fail(WD_ERR_MISMATCH, "wd_apply: tiled kernel cannot take this call");
         e = wd::launch_tile(a);
+    } else if (g->kernel == WD_KERNEL_STAGE) {
+        if (!wd::stage_supported(a)) return fail(WD_ERR_MISMATCH, "wd_apply: staged kernel cannot take this call");
+        e = wd::launch_stage(a);
     } else
         e = wd::tile_preferred(a) ? wd::launch_tile(a) : wd::launch_site(a);
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply: kernel launch");

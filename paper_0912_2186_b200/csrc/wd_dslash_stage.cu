@@ -1,0 +1,384 @@
+// wd_dslash_stage.cu -- WD_KERNEL_STAGE: the t-marching tile kernel with EVERY global read staged
+// through shared memory by cp.async one step ahead (fp32).
+//
+// eq. (2.2); SURVEY.md 8(a) steps a1-a7 in one launch.  Same decomposition as
+// wd_dslash_tile.cu (tile Lx x ty x tz of one time slice per CTA, marching along t; x hops by warp
+// shuffles, y/z hops through a shared-memory slice, backward hops computed at the source site and
+// handed over through shared memory, t hops in registers).  What differs: ncu showed the tile
+// kernel latency bound (profiles/r01_tile_ncu.md: ~60 % of the stall samples are the first use of a
+// link / face load, 4-5 dependent L2/HBM round trips per slice with 16 warps per SM).  Here no
+// arithmetic ever waits for HBM or L2:
+//
+//   * the four links of the thread's site, its out-of-tile face neighbours (spinor, plus the link for
+//     a backward face) and its own spinor of the next slice are all copied global -> shared by
+//     16-byte cp.async into slots PRIVATE to the thread, issued half a step to a full step before
+//     they are read back with LDS; a slot is refilled for slice t+1 right after slice t consumed it;
+//   * cp.async group bookkeeping per slice (commit order):  P = own spinor of t+1 (top of slice),
+//     A = links x,y + y face of t+1 (after the y hops), B = links z,t + z face of t+1 (after the t
+//     hops);  waits: wait_group 2 at the top (P(t), A(t-1 issued) done), 2 before z, 1 before t.
+//
+// Registers are no longer held across memory latency, shared memory is: 840 B/site, two CTAs of
+// 128 sites per SM.  Requires ty, tz >= 2 (a thread has at most one face per direction), Lx a power
+// of two <= 32, Lx*Ly*Lz a multiple of 32.
+#include <cstdio>
+#include <cstdlib>
+#include "wd_internal.h"
+#include "wd_layout.cuh"
+#include "wd_math.cuh"
+#include "wd_link.cuh"
+
+namespace wd {
+
+namespace {
+
+__device__ __forceinline__ void cpa16(float4 *smem_dst, const float4 *gsrc)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cpa_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cpa_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+// NV vectors [vec][slot stride] -> registers
+template <int NV>
+__device__ __forceinline__ void lds_vecs(const float4 *buf, int stride, int slot, float *r)
+{
+#pragma unroll
+    for (int c = 0; c < NV; ++c) unpack(buf[c * stride + slot], &r[c * 4]);
+}
+
+// link MU out of the staged link record (vectors [first, last] of the site's NVEC)
+template <int MU, int RECON>
+__device__ __forceinline__ void lds_link(const float4 *lnk, int nt, int tid, float (&u)[18])
+{
+    constexpr int first = (MU * RECON) / 4, last = (MU * RECON + RECON - 1) / 4, skip = MU * RECON - first * 4;
+    float tmp[(last - first + 1) * 4];
+    lds_vecs<last - first + 1>(lnk + first * nt, nt, tid, tmp);
+#pragma unroll
+    for (int i = 0; i < RECON; ++i) u[i] = tmp[skip + i];
+    if (RECON == 12) reconstruct_row2(u);
+}
+
+// face link MU staged alone: vectors [first, last] of the neighbour's record, stored from vector 0
+template <int MU, int RECON>
+__device__ __forceinline__ void lds_face_link(const float4 *buf, int stride, int slot, float (&u)[18])
+{
+    constexpr int first = (MU * RECON) / 4, last = (MU * RECON + RECON - 1) / 4, skip = MU * RECON - first * 4;
+    float tmp[(last - first + 1) * 4];
+    lds_vecs<last - first + 1>(buf, stride, slot, tmp);
+#pragma unroll
+    for (int i = 0; i < RECON; ++i) u[i] = tmp[skip + i];
+    if (RECON == 12) reconstruct_row2(u);
+}
+
+template <int MU, int RECON> struct FaceLinkVecs {
+    static constexpr int first = (MU * RECON) / 4, last = (MU * RECON + RECON - 1) / 4, n = last - first + 1;
+};
+
+__device__ __forceinline__ void shfl12(float (&dst)[12], const float (&src)[12], int src_lane)
+{
+#pragma unroll
+    for (int i = 0; i < 12; ++i) dst[i] = __shfl_sync(0xffffffffu, src[i], src_lane);
+}
+
+} // namespace
+
+// shared-memory float4 vectors of one CTA (see the kernel for the carve-up)
+template <int RECON> constexpr int stage_smem_vecs(int nt, int nyb, int nzb)
+{
+    return nt * (2 * 6 + 3 + 3 + LinkLayout<float, RECON>::NVEC + 6 + 6) + nyb * FaceLinkVecs<1, RECON>::n +
+           nzb * FaceLinkVecs<2, RECON>::n;
+}
+
+// gridDim.x = nchunk * nrhs * ncol, ordered (t-chunk, right-hand side, tile column): all right-hand
+// sides of a t-chunk run back to back, so the chunk's links come from HBM once and then from L2.
+template <int RECON>
+__global__ void __launch_bounds__(256, 1)
+dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const float *__restrict__ links, int Lx, int Ly,
+                    int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk)
+{
+    using LL = LinkLayout<float, RECON>;
+    constexpr int NVEC = LL::NVEC;
+    constexpr int A_END = FaceLinkVecs<1, RECON>::last + 1; // links x,y = vectors [0, A_END), z,t = [A_END, NVEC)
+    using FY = FaceLinkVecs<1, RECON>;
+    using FZ = FaceLinkVecs<2, RECON>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int nt = blockDim.x, tid = threadIdx.x;
+    const int nyb = Lx * tz, nzb = Lx * ty;
+    float4 *plane0 = reinterpret_cast<float4 *>(smem_raw); // two slice buffers [6][nt]
+    const int plane_sz = 6 * nt;
+    float4 *xchg_y = plane0 + 2 * plane_sz; // [3][nt]  U_y^dag P+_y psi, for the site at y+1
+    float4 *xchg_z = xchg_y + 3 * nt;       // [3][nt]
+    float4 *lnk = xchg_z + 3 * nt;          // [NVEC][nt] the four links of the thread's site
+    float4 *fy = lnk + NVEC * nt;           // [6][nt]   out-of-tile y neighbour spinor (face threads)
+    float4 *fz = fy + 6 * nt;               // [6][nt]   out-of-tile z neighbour spinor
+    float4 *fly = fz + 6 * nt;              // [FY::n][nyb]  U_y of the -y neighbour (yy == 0 threads)
+    float4 *flz = fly + FY::n * nyb;        // [FZ::n][nzb]  U_z of the -z neighbour (zz == 0 threads)
+
+    const int ncy = Ly / ty;
+    const int ncol = ncy * (Lz / tz);
+    const int col = blockIdx.x % ncol;
+    const int kg = blockIdx.x / ncol;
+    const int rhs = kg % nrhs, k = kg / nrhs;
+    in += (long long)rhs * 24 * padded_volume(V);
+    out += (long long)rhs * 24 * padded_volume(V);
+
+    const int x = tid & (Lx - 1);
+    const int row = tid / Lx;
+    const int yy = row % ty, zz = row / ty;
+    const int lane = tid & 31;
+    const int lane_r = (lane & ~(Lx - 1)) | ((lane + 1) & (Lx - 1));
+    const int lane_l = (lane & ~(Lx - 1)) | ((lane - 1) & (Lx - 1));
+    const int slot_yb = tid - Lx, slot_yf = tid + Lx;
+    const int slot_zb = tid - Lx * ty, slot_zf = tid + Lx * ty;
+    const bool face_yb = (yy == 0), face_yf = (yy == ty - 1), face_zb = (zz == 0), face_zf = (zz == tz - 1);
+    const int rank_y = zz * Lx + x, rank_z = yy * Lx + x;
+
+    const long long S3 = (long long)Lx * Ly * Lz;
+    const int t_begin = (int)((long long)Lt * k / nchunk), t_end = (int)((long long)Lt * (k + 1) / nchunk);
+    const int cy = col % ncy, cz = col / ncy;
+    const int y = cy * ty + yy, z = cz * tz + zz;
+    const long long s3 = x + (long long)Lx * (y + (long long)Ly * z);
+    // out-of-tile neighbour of a face thread (at most one per direction since ty, tz >= 2)
+    const long long s3_y = face_yf ? s3 + (y + 1 == Ly ? -(long long)(Ly - 1) * Lx : (long long)Lx)
+                                   : s3 + (y == 0 ? (long long)(Ly - 1) * Lx : -(long long)Lx);
+    const long long s3_z = face_zf ? s3 + (z + 1 == Lz ? -(long long)(Lz - 1) * Lx * Ly : (long long)Lx * Ly)
+                                   : s3 + (z == 0 ? (long long)(Lz - 1) * Lx * Ly : -(long long)Lx * Ly);
+
+    // ---- staging helpers (slots private to the thread) ----
+    auto stage_spinor = [&](float4 *dst, long long site) {
+        const float4 *q = spinor_ptr(in, site);
+#pragma unroll
+        for (int c = 0; c < 6; ++c) cpa16(dst + c * nt + tid, q + c * BLK);
+    };
+    auto stage_A = [&](long long toff) { // links x,y of the own site + y face, slice offset toff
+        const float4 *q = link_ptr<float, RECON>(links, s3 + toff);
+#pragma unroll
+        for (int j = 0; j < A_END; ++j) cpa16(lnk + j * nt + tid, q + j * BLK);
+        if (face_yf | face_yb) stage_spinor(fy, s3_y + toff);
+        if (face_yb) {
+            const float4 *f = link_ptr<float, RECON>(links, s3_y + toff);
+#pragma unroll
+            for (int j = 0; j < FY::n; ++j) cpa16(fly + j * nyb + rank_y, f + (FY::first + j) * BLK);
+        }
+    };
+    auto stage_B = [&](long long toff) { // links z,t of the own site + z face
+        const float4 *q = link_ptr<float, RECON>(links, s3 + toff);
+#pragma unroll
+        for (int j = A_END; j < NVEC; ++j) cpa16(lnk + j * nt + tid, q + j * BLK);
+        if (face_zf | face_zb) stage_spinor(fz, s3_z + toff);
+        if (face_zb) {
+            const float4 *f = link_ptr<float, RECON>(links, s3_z + toff);
+#pragma unroll
+            for (int j = 0; j < FZ::n; ++j) cpa16(flz + j * nzb + rank_z, f + (FZ::first + j) * BLK);
+        }
+    };
+
+    float chi_t[12]; // U_t(t-1)^dag P+_t psi(t-1) of this site
+    int cur = 0;
+    if (t_begin < t_end) { // ---- start the march at slice t_begin ----
+        const long long toff = (long long)t_begin * S3;
+        stage_spinor(plane0 + cur * plane_sz, s3 + toff);
+        cpa_commit(); // P'
+        stage_A(toff);
+        cpa_commit(); // A'
+        stage_B(toff);
+        cpa_commit(); // B'
+        const long long site_tb = s3 + (long long)(t_begin == 0 ? Lt - 1 : t_begin - 1) * S3;
+        float u[18], p[24], h[12];
+        load_link<3, float, RECON>(links, site_tb, u);
+        load_spinor(in, site_tb, p);
+        project<3, +1>(p, h);
+        su3_dag_mul(u, h, chi_t);
+    }
+
+    for (int t = t_begin; t < t_end; ++t) {
+        const long long toff = (long long)t * S3;
+        const long long toff_n = (long long)(t + 1 == Lt ? 0 : t + 1) * S3;
+        const bool more = (t + 1 < t_end); // the next slice is still ours: keep its links and faces coming
+        // P: own spinor of slice t+1 -> the other slice buffer (its old content, slice t-1, is dead)
+        stage_spinor(plane0 + (cur ^ 1) * plane_sz, s3 + toff_n);
+        cpa_commit();
+        cpa_wait<2>();   // own spinor of slice t (earlier P) and group A of slice t have landed
+        __syncthreads(); // (A) slice t complete for every thread
+
+        const float4 *pl = plane0 + cur * plane_sz;
+        float acc[24], psi[24], u[18];
+        lds_vecs<6>(pl, nt, tid, psi);
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] = 0.f;
+        reconstruct_add<3, +1>(acc, chi_t); // backward t hop, product carried from the previous slice
+
+        // ---- x: both hops through warp shuffles ----
+        lds_link<0, RECON>(lnk, nt, tid, u);
+        {
+            float h[12], g[12], chi[12];
+            project<0, -1>(psi, h);
+            shfl12(g, h, lane_r); // P-_x psi(x+1)
+            su3_mul(u, g, chi);
+            reconstruct_add<0, -1>(acc, chi);
+            project<0, +1>(psi, h);
+            su3_dag_mul(u, h, chi); // U_x(x)^dag P+_x psi(x): belongs to x+1
+            shfl12(g, chi, lane_l);
+            reconstruct_add<0, +1>(acc, g);
+        }
+        // ---- y ----
+        lds_link<1, RECON>(lnk, nt, tid, u);
+        {
+            float pn[24], h[12], chi[12];
+            if (face_yf) lds_vecs<6>(fy, nt, tid, pn);
+            else lds_vecs<6>(pl, nt, slot_yf, pn);
+            hop_forward<1>(acc, u, pn);
+            project<1, +1>(psi, h);
+            su3_dag_mul(u, h, chi);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) xchg_y[c * nt + tid] = make_float4(chi[4 * c], chi[4 * c + 1], chi[4 * c + 2], chi[4 * c + 3]);
+            if (face_yb) { // the site below is outside the tile: do its backward hop here
+                lds_face_link<1, RECON>(fly, nyb, rank_y, u);
+                lds_vecs<6>(fy, nt, tid, pn);
+                hop_backward<1>(acc, u, pn);
+            }
+        }
+        if (more) stage_A(toff_n); // slots of links x,y and the y face are free again
+        cpa_commit();
+        cpa_wait<2>(); // group B of slice t (links z,t, z face) has landed
+        // ---- z ----
+        lds_link<2, RECON>(lnk, nt, tid, u);
+        {
+            float pn[24], h[12], chi[12];
+            if (face_zf) lds_vecs<6>(fz, nt, tid, pn);
+            else lds_vecs<6>(pl, nt, slot_zf, pn);
+            hop_forward<2>(acc, u, pn);
+            project<2, +1>(psi, h);
+            su3_dag_mul(u, h, chi);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) xchg_z[c * nt + tid] = make_float4(chi[4 * c], chi[4 * c + 1], chi[4 * c + 2], chi[4 * c + 3]);
+            if (face_zb) {
+                lds_face_link<2, RECON>(flz, nzb, rank_z, u);
+                lds_vecs<6>(fz, nt, tid, pn);
+                hop_backward<2>(acc, u, pn);
+            }
+        }
+        // ---- t: forward hop now, backward product for the next slice ----
+        lds_link<3, RECON>(lnk, nt, tid, u);
+        cpa_wait<1>(); // own spinor of slice t+1 (this slice's P) has landed
+        {
+            float pn[24], h[12];
+            lds_vecs<6>(plane0 + (cur ^ 1) * plane_sz, nt, tid, pn);
+            hop_forward<3>(acc, u, pn);
+            project<3, +1>(psi, h);
+            su3_dag_mul(u, h, chi_t);
+        }
+        if (more) stage_B(toff_n); // slots of links z,t and the z face are free again
+        cpa_commit();
+        __syncthreads(); // (B) exchange buffers complete
+        if (!face_yb) {
+            float chi[12];
+            lds_vecs<3>(xchg_y, nt, slot_yb, chi);
+            reconstruct_add<1, +1>(acc, chi);
+        }
+        if (!face_zb) {
+            float chi[12];
+            lds_vecs<3>(xchg_z, nt, slot_zb, chi);
+            reconstruct_add<2, +1>(acc, chi);
+        }
+        // fused diagonal (step a6) and store (a7)
+#pragma unroll
+        for (int i = 0; i < 24; ++i) psi[i] = fmaf(cdiag, psi[i], -0.5f * acc[i]);
+        store_spinor(out, s3 + toff, psi);
+        cur ^= 1;
+    }
+    cpa_wait<0>();
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+struct StageShape {
+    int ty, tz, nt;
+};
+
+bool stage_shape(const ApplyArgs &a, StageShape &s)
+{
+    const int Lx = a.dims[0], Ly = a.dims[1], Lz = a.dims[2];
+    if (a.precision != 32) return false;
+    if (Lx < 4 || Lx > 32 || (Lx & (Lx - 1))) return false;
+    if (((long long)Lx * Ly * Lz) % BLK) return false;
+    if (const char *e = getenv("WD_TILE_SHAPE")) {
+        int ty = 0, tz = 0;
+        if (sscanf(e, "%d,%d", &ty, &tz) == 2 && ty >= 2 && tz >= 2 && Ly % ty == 0 && Lz % tz == 0 &&
+            (Lx * ty * tz) % 32 == 0 && Lx * ty * tz <= 256) {
+            s = {ty, tz, Lx * ty * tz};
+            return true;
+        }
+    }
+    int best = 0;
+    for (int ty = 2; ty <= Ly && ty <= 16; ++ty) {
+        if (Ly % ty) continue;
+        for (int tz = 2; tz <= ty && tz <= Lz; ++tz) {
+            if (Lz % tz) continue;
+            const int nt = Lx * ty * tz;
+            if (nt % 32 || nt > 128) continue; // 128 sites per tile: two CTAs per SM
+            const int score = nt * 64 - (ty - tz);
+            if (score > best) {
+                best = score;
+                s = {ty, tz, nt};
+            }
+        }
+    }
+    return best > 0;
+}
+
+template <int RECON>
+cudaError_t launch_stage_t(const ApplyArgs &a)
+{
+    auto kern = dslash_stage_kernel<RECON>;
+    StageShape s;
+    if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
+    const size_t smem = (size_t)stage_smem_vecs<RECON>(s.nt, a.dims[0] * s.tz, a.dims[0] * s.ty) * sizeof(float4);
+    if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
+    static size_t smem_set = 0;
+    cudaError_t e;
+    if (smem > smem_set) {
+        if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        smem_set = smem;
+    }
+    // t-chunks of 8 slices (WD_TILE_TC / WD_TILE_NCHUNK override): the start of a march is the one place
+    // where this kernel waits for memory, so chunks are longer than in the tile kernel
+    int tc = 8;
+    if (const char *ev = getenv("WD_TILE_TC")) {
+        const int v = atoi(ev);
+        if (v >= 1) tc = v;
+    }
+    int nchunk = (a.dims[3] + tc - 1) / tc;
+    if (const char *ev = getenv("WD_TILE_NCHUNK")) {
+        const int v = atoi(ev);
+        if (v >= 1 && v <= a.dims[3]) nchunk = v;
+    }
+    if (nchunk < 1) nchunk = 1;
+    const long long ncol = (long long)(a.dims[1] / s.ty) * (a.dims[2] / s.tz);
+    if (ncol * nchunk * a.nrhs > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)(ncol * nchunk * a.nrhs));
+    const float cdiag = (float)(4.0 + a.mass); // formed in double, rounded once (reading S8)
+    kern<<<grid, s.nt, smem, a.stream>>>((float *)a.out, (const float *)a.in, (const float *)a.links, a.dims[0], a.dims[1],
+                                          a.dims[2], a.dims[3], s.ty, s.tz, a.V, cdiag, a.nrhs, nchunk);
+    count_launch();
+    return cudaGetLastError();
+}
+
+} // namespace
+
+bool stage_supported(const ApplyArgs &a)
+{
+    StageShape s;
+    return a.nrhs >= 1 && stage_shape(a, s);
+}
+
+cudaError_t launch_stage(const ApplyArgs &a)
+{
+    return a.recon == 18 ? launch_stage_t<18>(a) : launch_stage_t<12>(a);
+}
+
+} // namespace wd

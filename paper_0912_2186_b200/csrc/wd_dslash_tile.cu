@@ -84,12 +84,16 @@ __device__ __forceinline__ void shfl_half(T (&dst)[12], const T (&src)[12], int 
 // smem bytes of one CTA: two slice buffers (24 reals/site) + two exchange buffers (12 reals/site)
 template <typename T> constexpr size_t tile_smem_bytes(int nt) { return (size_t)nt * (2 * 24 + 2 * 12) * sizeof(T); }
 
-// One launch = out = D in for one right-hand side (rhs = blockIdx.y).
-//   dims Lx (power of two, 4..32), Ly % ty == 0, Lz % tz == 0, blockDim.x = Lx*ty*tz (multiple of 32)
+// One launch = out[r] = D in[r] for all right-hand sides.
+//   dims Lx (power of two, 4..32), Ly % ty == 0, Lz % tz == 0,
+//   blockDim.x = Lx*ty*tz*nrb: the tile's sites times nrb right-hand sides (step a'): the nrb
+//   threads of a site load the same links, one from L2, the others from L1.
+//   gridDim.x = nchunk * ngroups * ncol, ordered (t-chunk, RHS group, tile column): all RHS groups
+//   of a t-chunk run back to back, so the chunk's links come from HBM once and then from L2.
 template <typename T, int RECON, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB)
 dslash_tile_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ links, int Lx, int Ly, int Lz,
-                   int Lt, int ty, int tz, long long V, T cdiag)
+                   int Lt, int ty, int tz, long long V, T cdiag, int nrhs, int nrb, int nchunk)
 {
     using SL = SpinorLayout<T>;
     using Vec = typename SL::Vec;
@@ -101,13 +105,27 @@ dslash_tile_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
     Vec *xchg_y = plane0 + 2 * plane_sz;     // U_y^dag P+_y psi of every tile site, for the site at y+1
     Vec *xchg_z = xchg_y + (NCH / 2) * nt;   // same for z
 
-    in += (long long)blockIdx.y * 24 * padded_volume(V);
-    out += (long long)blockIdx.y * 24 * padded_volume(V);
+    const int ncy = Ly / ty;
+    const int ncol = ncy * (Lz / tz);
+    const int ngroups = (nrhs + nrb - 1) / nrb;
+    // Work item = (t-chunk k, RHS group g, tile column col), k-major in blockIdx.x: the block
+    // scheduler hands out CTAs in index order, so at any time the resident CTAs cover ALL columns of
+    // a few consecutive (chunk, group) pairs and march through the same slices together -- a face
+    // site's out-of-tile neighbour has just been (or is about to be) loaded by the neighbouring CTA
+    // and is served from L2, not HBM.
+    const int col = blockIdx.x % ncol;
+    const int kg = blockIdx.x / ncol;
+    const int g = kg % ngroups, k = kg / ngroups;
 
-    // thread <-> site of the tile: x fastest, then y, then z (x-rows are (parts of) warps)
+    // thread <-> (site of the tile, RHS of the group): x fastest, then y, z, RHS (x-rows are
+    // (parts of) warps; shared-memory slots are indexed by tid, so neighbours stay within one RHS)
     const int x = tid & (Lx - 1);
     const int row = tid / Lx;
-    const int yy = row % ty, zz = row / ty;
+    const int yy = row % ty, zz = (row / ty) % tz;
+    const int rhs = g * nrb + row / (ty * tz);
+    const bool live = rhs < nrhs; // a partial last group computes a duplicate and does not store it
+    in += (long long)(live ? rhs : nrhs - 1) * 24 * padded_volume(V);
+    out += (long long)(live ? rhs : nrhs - 1) * 24 * padded_volume(V);
     const int lane = tid & 31;
     const int lane_r = (lane & ~(Lx - 1)) | ((lane + 1) & (Lx - 1)); // x+1, periodic
     const int lane_l = (lane & ~(Lx - 1)) | ((lane - 1) & (Lx - 1)); // x-1, periodic
@@ -116,14 +134,6 @@ dslash_tile_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
     const bool face_yb = (yy == 0), face_yf = (yy == ty - 1), face_zb = (zz == 0), face_zf = (zz == tz - 1);
 
     const long long S3 = (long long)Lx * Ly * Lz;
-    const int ncy = Ly / ty;
-    const int ncol = ncy * (Lz / tz);
-    // Work item = (t-chunk k, tile column col), k-major in blockIdx.x: the block scheduler hands out
-    // CTAs in index order, so at any time the resident CTAs cover ALL columns of a few consecutive
-    // chunks and march through the same slices together -- a face site's out-of-tile neighbour has
-    // just been (or is about to be) loaded by the neighbouring CTA and is served from L2, not HBM.
-    const int k = blockIdx.x / ncol, col = blockIdx.x - k * ncol;
-    const int nchunk = gridDim.x / ncol;
     const int t_begin = (int)((long long)Lt * k / nchunk), t_end = (int)((long long)Lt * (k + 1) / nchunk);
 
     const int cy = col % ncy, cz = col / ncy;
@@ -237,7 +247,7 @@ dslash_tile_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
         // fused diagonal (step a6) and store (a7)
 #pragma unroll
         for (int i = 0; i < 24; ++i) psi[i] = fma(cdiag, psi[i], (T)-0.5 * acc[i]);
-        store_spinor(out, site, psi);
+        if (live) store_spinor(out, site, psi);
         cur ^= 1;
     }
     cp_async_wait_all();
@@ -255,8 +265,8 @@ struct TileShape {
 bool pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 
 // Tile shape: Lx x ty x tz threads, ty | Ly, tz | Lz, a multiple of 32 and at most max_threads.
-// WD_TILE_SHAPE="ty,tz" overrides the choice (tuning / tests); otherwise the largest tile wins,
-// squarer tiles first (less face traffic).
+// WD_TILE_SHAPE="ty,tz" overrides the choice (tuning / tests); otherwise the largest tile of at
+// most 128 sites wins, squarer tiles first (less face traffic).
 bool choose_shape(const ApplyArgs &a, int max_threads, TileShape &s)
 {
     const int Lx = a.dims[0], Ly = a.dims[1], Lz = a.dims[2];
@@ -275,7 +285,7 @@ bool choose_shape(const ApplyArgs &a, int max_threads, TileShape &s)
         for (int tz = 1; tz <= ty && tz <= Lz; ++tz) {
             if (Lz % tz) continue;
             const int nt = Lx * ty * tz;
-            if (nt % 32 || nt > max_threads) continue;
+            if (nt % 32 || nt > 128) continue; // 128 sites per tile measured best (profiles/)
             const int score = nt * 64 - (ty - tz); // bigger first, then squarer
             if (score > best) {
                 best = score;
@@ -296,7 +306,17 @@ cudaError_t launch_tile_t(const ApplyArgs &a)
     auto kern = dslash_tile_kernel<T, RECON, MAXT, MINB>;
     TileShape s;
     if (!choose_shape(a, MAXT, s)) return cudaErrorInvalidConfiguration;
-    const size_t smem = tile_smem_bytes<T>(s.nt);
+    // right-hand sides per CTA: fill the CTA up to MAXT threads (WD_TILE_NRB overrides)
+    int nrb = MAXT / s.nt;
+    if (const char *ev = getenv("WD_TILE_NRB")) {
+        const int v = atoi(ev);
+        if (v >= 1 && v * s.nt <= MAXT) nrb = v;
+    }
+    if (nrb > a.nrhs) nrb = a.nrhs;
+    if (nrb < 1) nrb = 1;
+    const int ngroups = (a.nrhs + nrb - 1) / nrb;
+    const int nthreads = s.nt * nrb;
+    const size_t smem = tile_smem_bytes<T>(nthreads);
 
     static size_t smem_set = 0;
     cudaError_t e;
@@ -304,9 +324,10 @@ cudaError_t launch_tile_t(const ApplyArgs &a)
         if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
         smem_set = smem;
     }
-    // t is cut into chunks of ~8 slices (WD_TILE_TC overrides): long enough to amortise the start of a
-    // march (one extra spinor + link per site), short enough for many CTAs per SM-slot (load balance).
-    int tc = 8;
+    // t is cut into chunks of 4 slices (WD_TILE_TC / WD_TILE_NCHUNK override; measured best on B200 for
+    // 32^3 x 64): the start of a march costs one extra spinor + link per site (served from L2, the
+    // previous chunk has just used them), short chunks give many CTAs per SM slot (load balance).
+    int tc = 4;
     if (const char *ev = getenv("WD_TILE_TC")) {
         const int v = atoi(ev);
         if (v >= 1) tc = v;
@@ -318,11 +339,11 @@ cudaError_t launch_tile_t(const ApplyArgs &a)
     }
     if (nchunk < 1) nchunk = 1;
     const long long ncol = (long long)(a.dims[1] / s.ty) * (a.dims[2] / s.tz);
-    if (ncol * nchunk > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    dim3 grid((unsigned)(ncol * nchunk), (unsigned)a.nrhs);
+    if (ncol * nchunk * ngroups > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)(ncol * nchunk * ngroups));
     const T cdiag = (T)(4.0 + a.mass); // formed in double, rounded once (reading S8)
-    kern<<<grid, s.nt, smem, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)a.links, a.dims[0], a.dims[1], a.dims[2],
-                                          a.dims[3], s.ty, s.tz, a.V, cdiag);
+    kern<<<grid, nthreads, smem, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)a.links, a.dims[0], a.dims[1],
+                                              a.dims[2], a.dims[3], s.ty, s.tz, a.V, cdiag, a.nrhs, nrb, nchunk);
     count_launch();
     return cudaGetLastError();
 }
@@ -331,15 +352,15 @@ cudaError_t launch_tile_t(const ApplyArgs &a)
 
 bool tile_supported(const ApplyArgs &a)
 {
-    if (a.nrhs < 1 || a.nrhs > 65535) return false;
+    if (a.nrhs < 1) return false;
     TileShape s;
     return choose_shape(a, a.precision == 32 ? tile_max_threads<float>() : tile_max_threads<double>(), s);
 }
 
 bool tile_preferred(const ApplyArgs &a)
 {
-    // measured (profiles/): single right-hand side fp32 on lattices of at least a few waves of tiles
-    return a.nrhs == 1 && a.precision == 32 && a.V >= (1LL << 18) && tile_supported(a);
+    // measured (profiles/): single right-hand side, lattices of at least a few waves of tiles
+    return a.nrhs == 1 && a.V >= (1LL << 18) && tile_supported(a);
 }
 
 cudaError_t launch_tile(const ApplyArgs &a)

@@ -50,6 +50,9 @@ bool tile_supported(const ApplyArgs &a);
 // WD_KERNEL_AUTO picks the tiled kernel when this holds (measured faster), else the site kernel
 bool tile_preferred(const ApplyArgs &a);
 cudaError_t launch_tile(const ApplyArgs &a);
+// tile kernel with every global read staged through shared memory by cp.async (fp32)
+bool stage_supported(const ApplyArgs &a);
+cudaError_t launch_stage(const ApplyArgs &a);
 
 cudaError_t launch_pack_spinor(void *native, const void *canonical, long long V, int nrhs, int precision,
                                cudaStream_t s);

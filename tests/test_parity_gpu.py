@@ -13,7 +13,7 @@ from gpu_util import TOL, GpuOp, np_dtype, oracle_apply, rel_l2
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = {"auto": 0, "site": 1, "tile": 2}
+KERNELS = {"auto": 0, "site": 1, "tile": 2, "stage": 3}
 
 
 def oracle_links(U, recon):
@@ -105,6 +105,57 @@ def test_tile_kernel_forced_tile_shapes(oracle, monkeypatch, shape, precision):
 @pytest.mark.parametrize("name", ["c1_16x32_fp32", "c3_32x64_fp32", "c3_32x64_fp64"])
 def test_tile_kernel_baseline_configs(oracle, name):
     check_config(oracle, fields.CONFIGS[name], "tile")
+
+
+# ---------------------------------------------------------------- the cp.async-staged tile kernel (fp32)
+STAGE_SHAPES = [(32, 4, 4, 4), (16, 8, 8, 6), (8, 4, 4, 12), (4, 8, 16, 5), (32, 8, 8, 3), (32, 2, 2, 2), (16, 2, 4, 1),
+                (32, 6, 10, 4), (8, 12, 4, 7)]
+
+
+@pytest.mark.parametrize("dims", STAGE_SHAPES)
+@pytest.mark.parametrize("recon", [18, 12])
+def test_stage_kernel_shapes(oracle, dims, recon):
+    cfg = fields.Config("stage", dims, 32, "haar", recon, -0.3, 1, 15)
+    check_config(oracle, cfg, "stage", nrhs=1)
+    check_config(oracle, cfg, "stage", nrhs=3)
+
+
+@pytest.mark.parametrize("shape", ["2,2", "4,2", "2,4", "4,4", "8,1"])
+@pytest.mark.parametrize("tc", ["1", "2", "5", "100"])
+def test_stage_kernel_forced_tile_shapes_and_chunks(oracle, monkeypatch, shape, tc):
+    monkeypatch.setenv("WD_TILE_SHAPE", shape)
+    monkeypatch.setenv("WD_TILE_TC", tc)
+    cfg = fields.Config("stageshape", (32, 8, 8, 5), 32, "smooth", 18, -0.42, 2, 23)
+    check_config(oracle, cfg, "stage")
+
+
+@pytest.mark.parametrize("name", ["c1_16x32_fp32", "c3_32x64_fp32"])
+def test_stage_kernel_baseline_configs(oracle, name):
+    check_config(oracle, fields.CONFIGS[name], "stage")
+
+
+def test_stage_kernel_rejects_fp64_and_odd_lattices():
+    from paper_0912_2186_b200 import binding
+    for dims, precision in (((8, 4, 4, 4), 64), ((24, 4, 4, 4), 32), ((32, 3, 4, 4), 32)):
+        cfg = fields.Config("bad", dims, precision, "haar", 18, 0.1, 1, 3)
+        U, _ = fields.make_fields(cfg)
+        op = GpuOp(U, cfg.dims, precision, 18)
+        with pytest.raises(binding.WdError) as e:
+            binding.wd_set_kernel(op.op.gauge, KERNELS["stage"])
+        assert e.value.code == -7
+        op.close()
+
+
+def test_stage_kernel_deterministic():
+    import torch
+    cfg = fields.Config("det", (32, 8, 8, 16), 32, "smooth", 18, -0.42, 1, 19)
+    U, psi = fields.make_fields(cfg)
+    op = GpuOp(U, cfg.dims, 32, 18, KERNELS["stage"])
+    a = op.apply(psi, cfg.mass, return_native=True).clone()
+    for _ in range(20):
+        b = op.apply(psi, cfg.mass, return_native=True)
+    assert torch.equal(a, b)
+    op.close()
 
 
 def test_tile_kernel_rejects_unsupported_lattice():
