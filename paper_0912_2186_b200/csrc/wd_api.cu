@@ -230,8 +230,17 @@ static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double m
     } else if (g->kernel == WD_KERNEL_STAGE) {
         if (!wd::stage_supported(a)) return fail(WD_ERR_MISMATCH, "wd_apply: staged kernel cannot take this call");
         e = wd::launch_stage(a);
-    } else
-        e = wd::tile_preferred(a) ? wd::launch_tile(a) : wd::launch_site(a);
+    } else {
+        // WD_KERNEL_AUTO, by measurement (profiles/): single right-hand side on a lattice of at least a
+        // few waves of tiles -> staged kernel (fp32) or tile kernel (fp64); everything else -> site kernel
+        const bool big1 = a.nrhs == 1 && a.V >= (1LL << 18);
+        if (big1 && wd::stage_supported(a))
+            e = wd::launch_stage(a);
+        else if (big1 && wd::tile_supported(a))
+            e = wd::launch_tile(a);
+        else
+            e = wd::launch_site(a);
+    }
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply: kernel launch");
 }
 

@@ -22,6 +22,7 @@
 // of two <= 32, Lx*Ly*Lz a multiple of 32.
 #include <cstdio>
 #include <cstdlib>
+#define WD_USE_F32X2 // packed FFMA2 SU(3) products (wd_math.cuh)
 #include "wd_internal.h"
 #include "wd_layout.cuh"
 #include "wd_math.cuh"

@@ -357,12 +357,6 @@ bool tile_supported(const ApplyArgs &a)
     return choose_shape(a, a.precision == 32 ? tile_max_threads<float>() : tile_max_threads<double>(), s);
 }
 
-bool tile_preferred(const ApplyArgs &a)
-{
-    // measured (profiles/): single right-hand side, lattices of at least a few waves of tiles
-    return a.nrhs == 1 && a.V >= (1LL << 18) && tile_supported(a);
-}
-
 cudaError_t launch_tile(const ApplyArgs &a)
 {
     if (a.precision == 32) return a.recon == 18 ? launch_tile_t<float, 18>(a) : launch_tile_t<float, 12>(a);

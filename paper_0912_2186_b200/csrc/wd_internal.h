@@ -47,8 +47,6 @@ void count_launch(int n = 1);
 cudaError_t launch_site(const ApplyArgs &a);
 // shared-memory tiled kernel; supported() is a pure host-side predicate
 bool tile_supported(const ApplyArgs &a);
-// WD_KERNEL_AUTO picks the tiled kernel when this holds (measured faster), else the site kernel
-bool tile_preferred(const ApplyArgs &a);
 cudaError_t launch_tile(const ApplyArgs &a);
 // tile kernel with every global read staged through shared memory by cp.async (fp32)
 bool stage_supported(const ApplyArgs &a);

@@ -94,6 +94,80 @@ __device__ __forceinline__ void su3_dag_mul(const T (&u)[18], const T (&h)[12], 
         }
 }
 
+// ---- fp32: packed two-lane FMA (Blackwell fma.rn.f32x2 -> SASS FFMA2) ------------------------
+// The two independent spin rows h0, h1 of a half spinor are multiplied by the SAME link, so they
+// ride in the two lanes of one f32x2 operand while the link element is the scalar (broadcast)
+// operand: 36 FFMA2 instead of 72 FFMA per SU(3) x half-spinor product, i.e. half the issue slots
+// for 60 % of the kernel's floating-point instructions.  Same products, same summation order per
+// lane as the scalar code above.  Opt-in per translation unit (#define WD_USE_F32X2 before this
+// header): measured on B200 it helps the cp.async-staged kernel, whose limit is issue slots, and
+// slows the latency-bound site and tile kernels (profiles/r01_stage_ncu.md).
+#ifdef WD_USE_F32X2
+__device__ __forceinline__ unsigned long long f2_pack(float lo, float hi)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void f2_unpack(unsigned long long v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ unsigned long long f2_mul(unsigned long long a, unsigned long long b)
+{
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+
+template <bool DAG>
+__device__ __forceinline__ void su3_mul_f2(const float (&u)[18], const float (&h)[12], float (&chi)[12])
+{
+    unsigned long long hre[3], him[3];
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        hre[b] = f2_pack(h[(0 * 3 + b) * 2], h[(1 * 3 + b) * 2]);
+        him[b] = f2_pack(h[(0 * 3 + b) * 2 + 1], h[(1 * 3 + b) * 2 + 1]);
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        unsigned long long re, im;
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            // element (a,b) of U, or of U^dagger = conj(U[b][a])
+            const float ur = DAG ? u[(b * 3 + a) * 2] : u[(a * 3 + b) * 2];
+            const float ui = DAG ? -u[(b * 3 + a) * 2 + 1] : u[(a * 3 + b) * 2 + 1];
+            const unsigned long long urr = f2_pack(ur, ur), uii = f2_pack(ui, ui), umi = f2_pack(-ui, -ui);
+            if (b == 0) {
+                re = f2_mul(urr, hre[b]);
+                im = f2_mul(urr, him[b]);
+            } else {
+                re = f2_fma(urr, hre[b], re);
+                im = f2_fma(urr, him[b], im);
+            }
+            re = f2_fma(umi, him[b], re);
+            im = f2_fma(uii, hre[b], im);
+        }
+        f2_unpack(re, chi[(0 * 3 + a) * 2], chi[(1 * 3 + a) * 2]);
+        f2_unpack(im, chi[(0 * 3 + a) * 2 + 1], chi[(1 * 3 + a) * 2 + 1]);
+    }
+}
+__device__ __forceinline__ void su3_mul(const float (&u)[18], const float (&h)[12], float (&chi)[12])
+{
+    su3_mul_f2<false>(u, h, chi);
+}
+__device__ __forceinline__ void su3_dag_mul(const float (&u)[18], const float (&h)[12], float (&chi)[12])
+{
+    su3_mul_f2<true>(u, h, chi);
+}
+#endif
+
 // acc += (1 + S gamma_MU)-reconstruction of chi (rows 0,1 = chi; rows 2,3 per the table above)
 template <int MU, int S, typename T>
 __device__ __forceinline__ void reconstruct_add(T (&acc)[24], const T (&chi)[12])
