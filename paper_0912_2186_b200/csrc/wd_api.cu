@@ -231,10 +231,12 @@ static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double m
         if (!wd::stage_supported(a)) return fail(WD_ERR_MISMATCH, "wd_apply: staged kernel cannot take this call");
         e = wd::launch_stage(a);
     } else {
-        // WD_KERNEL_AUTO, by measurement (profiles/): single right-hand side on a lattice of at least a
-        // few waves of tiles -> staged kernel (fp32) or tile kernel (fp64); everything else -> site kernel
-        const bool big1 = a.nrhs == 1 && a.V >= (1LL << 18);
-        if (big1 && wd::stage_supported(a))
+        // WD_KERNEL_AUTO, by measurement (profiles/): on a lattice of at least a few waves of tiles the
+        // staged kernels (fp32; single- and multi-RHS members) or, for one fp64 right-hand side, the tile
+        // kernel; everything else -> site kernel
+        const bool big = a.V >= (1LL << 18);
+        const bool big1 = big && a.nrhs == 1;
+        if (big && wd::stage_supported(a))
             e = wd::launch_stage(a);
         else if (big1 && wd::tile_supported(a))
             e = wd::launch_tile(a);

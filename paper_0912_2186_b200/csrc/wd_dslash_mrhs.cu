@@ -1,0 +1,335 @@
+// wd_dslash_mrhs.cu -- the multi-right-hand-side member of WD_KERNEL_STAGE (fp32): D applied to the
+// N_v test vectors of the adaptive set-up with ONE link load per site shared by the vectors
+// (SURVEY.md 8(a) step a'; BASELINE.json:configs[4]).
+//
+// Same t-marching tile decomposition and cp.async staging as wd_dslash_stage.cu, with a
+// right-hand-side dimension in the CTA: blockDim.x = (Lx*ty*tz sites) x (nrb right-hand sides).
+//   * The links of the tile's sites (and the backward-face links) sit in shared memory ONCE and are
+//     read by the nrb threads of a site; their cp.async copies are spread over those threads.
+//     They are single buffered in two halves: links z,t of slice t are (re)filled right after the
+//     barrier at the top of step t (the previous slice's z,t hops are over) and used half a step
+//     later; links x,y of slice t+1 right after the mid-step barrier (this slice's x,y hops are
+//     over) and used at the top of the next step.
+//   * With the links of in-tile neighbours in shared memory, a backward hop in y or z is computed by
+//     the receiving site itself (neighbour's link + neighbour's spinor from the slice buffer): no
+//     exchange buffers, every thread does exactly eight hops.  x hops use warp shuffles, t hops
+//     registers, as in the single-RHS kernels.
+//   * Spinor data stay private per (site, rhs) thread: two slice buffers + two face slots = 384 B.
+//   * Blocks are ordered (t-chunk, RHS group, tile column): all groups of a chunk run back to back, so
+//     the chunk's links come from HBM once and from L2 for the other groups.
+// cp.async groups per step t (commit order):  c1 = {links z,t + z-face link of t, own spinor of t+1}
+// after barrier A;  c2 = {y-face spinor of t+1} after the y hops;  c3 = {links x,y + y-face link of
+// t+1} after barrier M;  c4 = {z-face spinor of t+1} after the z hops.  Waits: wait_group 1 before A
+// (c2, c3 of the previous step done) and wait_group 1 before M (c4 of the previous step, c1 done).
+#include <cstdio>
+#include <cstdlib>
+#include <type_traits>
+#define WD_USE_F32X2 // packed FFMA2 SU(3) products (wd_math.cuh)
+#include "wd_internal.h"
+#include "wd_layout.cuh"
+#include "wd_math.cuh"
+#include "wd_link.cuh"
+
+namespace wd {
+
+namespace {
+
+__device__ __forceinline__ void cpa16(float4 *smem_dst, const float4 *gsrc)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cpa_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cpa_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+template <int NV>
+__device__ __forceinline__ void lds_vecs(const float4 *buf, int stride, int slot, float *r)
+{
+#pragma unroll
+    for (int c = 0; c < NV; ++c) unpack(buf[c * stride + slot], &r[c * 4]);
+}
+
+template <int MU, int RECON> struct LinkVecs {
+    static constexpr int first = (MU * RECON) / 4, last = (MU * RECON + RECON - 1) / 4, n = last - first + 1;
+    static constexpr int skip = MU * RECON - first * 4;
+};
+
+// link MU of site slot `slot` out of a staged record [vec][stride]; `base` is vector `first0` of the record
+template <int MU, int RECON>
+__device__ __forceinline__ void lds_link(const float4 *base, int first0, int stride, int slot, float (&u)[18])
+{
+    using LV = LinkVecs<MU, RECON>;
+    float tmp[LV::n * 4];
+    lds_vecs<LV::n>(base + (LV::first - first0) * stride, stride, slot, tmp);
+#pragma unroll
+    for (int i = 0; i < RECON; ++i) u[i] = tmp[LV::skip + i];
+    if (RECON == 12) reconstruct_row2(u);
+}
+
+__device__ __forceinline__ void shfl12(float (&dst)[12], const float (&src)[12], int src_lane)
+{
+#pragma unroll
+    for (int i = 0; i < 12; ++i) dst[i] = __shfl_sync(0xffffffffu, src[i], src_lane);
+}
+
+} // namespace
+
+// shared-memory float4 vectors of one CTA
+template <int RECON> constexpr int mrhs_smem_vecs(int nts, int nrb, int nyb, int nzb)
+{
+    return nts * nrb * (2 * 6 + 6 + 6) + nts * LinkLayout<float, RECON>::NVEC + nyb * LinkVecs<1, RECON>::n +
+           nzb * LinkVecs<2, RECON>::n;
+}
+
+// gridDim.x = nchunk * ngroups * ncol, ordered (t-chunk, RHS group, tile column).
+// blockDim.x = nts * NRB, nts = Lx*ty*tz sites of the tile (a multiple of 32, at most 128).
+template <int RECON, int NRB>
+__global__ void __launch_bounds__(128 * NRB, 1)
+dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const float *__restrict__ links, int Lx, int Ly,
+                   int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk)
+{
+    constexpr int NVEC = LinkLayout<float, RECON>::NVEC;
+    using FY = LinkVecs<1, RECON>;
+    using FZ = LinkVecs<2, RECON>;
+    constexpr int A_END = FY::last + 1; // links x,y = vectors [0, A_END), links z,t = [A_END, NVEC)
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int nt = blockDim.x, tid = threadIdx.x;
+    const int nts = nt / NRB;
+    const int st = tid % nts, rr = tid / nts; // site slot of the tile, right-hand side of the group
+    const int nyb = Lx * tz, nzb = Lx * ty;
+    float4 *plane0 = reinterpret_cast<float4 *>(smem_raw); // two slice buffers [6][nt], private slots
+    const int plane_sz = 6 * nt;
+    float4 *fy = plane0 + 2 * plane_sz; // [6][nt] out-of-tile y neighbour spinor (face threads)
+    float4 *fz = fy + 6 * nt;           // [6][nt] out-of-tile z neighbour spinor
+    float4 *lnk = fz + 6 * nt;          // [NVEC][nts] the four links of every tile site (shared by the RHS)
+    float4 *fly = lnk + NVEC * nts;     // [FY::n][nyb] U_y of the -y neighbour of the yy == 0 sites
+    float4 *flz = fly + FY::n * nyb;    // [FZ::n][nzb] U_z of the -z neighbour of the zz == 0 sites
+
+    const int ncy = Ly / ty;
+    const int ncol = ncy * (Lz / tz);
+    const int ngroups = (nrhs + NRB - 1) / NRB;
+    const int col = blockIdx.x % ncol;
+    const int kg = blockIdx.x / ncol;
+    const int g = kg % ngroups, k = kg / ngroups;
+    const int rhs = g * NRB + rr;
+    const bool live = rhs < nrhs; // a partial last group computes a duplicate and does not store it
+    in += (long long)(live ? rhs : nrhs - 1) * 24 * padded_volume(V);
+    out += (long long)(live ? rhs : nrhs - 1) * 24 * padded_volume(V);
+
+    const int x = st & (Lx - 1);
+    const int row = st / Lx;
+    const int yy = row % ty, zz = row / ty;
+    const int lane = tid & 31;
+    const int lane_r = (lane & ~(Lx - 1)) | ((lane + 1) & (Lx - 1));
+    const int lane_l = (lane & ~(Lx - 1)) | ((lane - 1) & (Lx - 1));
+    const bool face_yb = (yy == 0), face_yf = (yy == ty - 1), face_zb = (zz == 0), face_zf = (zz == tz - 1);
+    const int rank_y = zz * Lx + x, rank_z = yy * Lx + x;
+
+    const long long S3 = (long long)Lx * Ly * Lz;
+    const int t_begin = (int)((long long)Lt * k / nchunk), t_end = (int)((long long)Lt * (k + 1) / nchunk);
+    const int cy = col % ncy, cz = col / ncy;
+    const int y = cy * ty + yy, z = cz * tz + zz;
+    const long long s3 = x + (long long)Lx * (y + (long long)Ly * z);
+    // out-of-tile neighbour of a face thread (at most one per direction since ty, tz >= 2)
+    const long long s3_y = face_yf ? s3 + (y + 1 == Ly ? -(long long)(Ly - 1) * Lx : (long long)Lx)
+                                   : s3 + (y == 0 ? (long long)(Ly - 1) * Lx : -(long long)Lx);
+    const long long s3_z = face_zf ? s3 + (z + 1 == Lz ? -(long long)(Lz - 1) * Lx * Ly : (long long)Lx * Ly)
+                                   : s3 + (z == 0 ? (long long)(Lz - 1) * Lx * Ly : -(long long)Lx * Ly);
+
+    // ---- staging helpers ----
+    auto stage_spinor = [&](float4 *dst, long long site) { // private slot
+        const float4 *q = spinor_ptr(in, site);
+#pragma unroll
+        for (int c = 0; c < 6; ++c) cpa16(dst + c * nt + tid, q + c * BLK);
+    };
+    // link copies of a site are dealt out to its NRB threads: vector j goes to rr == j % NRB.  rr is
+    // warp uniform; the dispatch below makes `j % NRB == RR` a compile-time test, so the cp.async
+    // instructions sit in plain (unpredicated) branches.
+    // (Tried and dropped: createpolicy evict_last hints on the link copies to keep a chunk's links in
+    // L2 across RHS groups -- within noise on B200, and one launch shape faulted.)
+    auto copy_links = [&](auto rr_tag, int j0, int j1, float4 *dst, int stride, int slot, const float4 *src, int src0) {
+        constexpr int RR = decltype(rr_tag)::value;
+#pragma unroll
+        for (int j = 0; j < NVEC; ++j)
+            if (j >= j0 && j < j1 && (j - j0) % NRB == RR) cpa16(dst + (j - j0) * stride + slot, src + (src0 + j - j0) * BLK);
+    };
+    auto deal_links = [&](int j0, int j1, float4 *dst, int stride, int slot, const float4 *src, int src0) {
+        if (NRB == 1 || rr == 0) copy_links(std::integral_constant<int, 0>{}, j0, j1, dst, stride, slot, src, src0);
+        else if (NRB == 2 || rr == 1) copy_links(std::integral_constant<int, 1 % NRB>{}, j0, j1, dst, stride, slot, src, src0);
+        else copy_links(std::integral_constant<int, 2 % NRB>{}, j0, j1, dst, stride, slot, src, src0);
+    };
+    auto stage_XY = [&](long long toff) { // links x,y of the site + the y-face link
+        deal_links(0, A_END, lnk, nts, st, link_ptr<float, RECON>(links, s3 + toff), 0);
+        if (face_yb) deal_links(0, FY::n, fly, nyb, rank_y, link_ptr<float, RECON>(links, s3_y + toff), FY::first);
+    };
+    auto stage_ZT = [&](long long toff) { // links z,t of the site + the z-face link
+        deal_links(A_END, NVEC, lnk + A_END * nts, nts, st, link_ptr<float, RECON>(links, s3 + toff), A_END);
+        if (face_zb) deal_links(0, FZ::n, flz, nzb, rank_z, link_ptr<float, RECON>(links, s3_z + toff), FZ::first);
+    };
+
+    float chi_t[12]; // U_t(t-1)^dag P+_t psi(t-1) of this (site, rhs)
+    int cur = 0;
+    if (t_begin < t_end) { // ---- start the march at slice t_begin ----
+        const long long toff = (long long)t_begin * S3;
+        stage_spinor(plane0 + cur * plane_sz, s3 + toff);
+        cpa_commit(); // c0
+        if (face_yf | face_yb) stage_spinor(fy, s3_y + toff);
+        cpa_commit(); // c2'
+        stage_XY(toff);
+        cpa_commit(); // c3'
+        if (face_zf | face_zb) stage_spinor(fz, s3_z + toff);
+        cpa_commit(); // c4'
+        const long long site_tb = s3 + (long long)(t_begin == 0 ? Lt - 1 : t_begin - 1) * S3;
+        float u[18], p[24], h[12];
+        load_link<3, float, RECON>(links, site_tb, u);
+        load_spinor(in, site_tb, p);
+        project<3, +1>(p, h);
+        su3_dag_mul(u, h, chi_t);
+    }
+
+    for (int t = t_begin; t < t_end; ++t) {
+        const long long toff = (long long)t * S3;
+        const long long toff_n = (long long)(t + 1 == Lt ? 0 : t + 1) * S3;
+        const bool more = (t + 1 < t_end);
+        cpa_wait<1>();   // links x,y and the y-face spinor of slice t have landed (own copies)
+        __syncthreads(); // (A) ... everybody's; the z,t hops of slice t-1 are over
+        stage_ZT(toff);
+        stage_spinor(plane0 + (cur ^ 1) * plane_sz, s3 + toff_n);
+        cpa_commit(); // c1
+
+        const float4 *pl = plane0 + cur * plane_sz;
+        float acc[24], psi[24], u[18], pn[24];
+        lds_vecs<6>(pl, nt, tid, psi);
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] = 0.f;
+        reconstruct_add<3, +1>(acc, chi_t); // backward t hop, product carried from the previous slice
+
+        // ---- x: both hops through warp shuffles ----
+        lds_link<0, RECON>(lnk, 0, nts, st, u);
+        {
+            float h[12], gg[12], chi[12];
+            project<0, -1>(psi, h);
+            shfl12(gg, h, lane_r); // P-_x psi(x+1)
+            su3_mul(u, gg, chi);
+            reconstruct_add<0, -1>(acc, chi);
+            project<0, +1>(psi, h);
+            su3_dag_mul(u, h, chi); // U_x(x)^dag P+_x psi(x): belongs to x+1
+            shfl12(gg, chi, lane_l);
+            reconstruct_add<0, +1>(acc, gg);
+        }
+        // ---- y: forward with the own link, backward with the link of the site below ----
+        lds_link<1, RECON>(lnk, 0, nts, st, u);
+        if (face_yf) lds_vecs<6>(fy, nt, tid, pn);
+        else lds_vecs<6>(pl, nt, tid + Lx, pn);
+        hop_forward<1>(acc, u, pn);
+        if (face_yb) {
+            lds_link<1, RECON>(fly, FY::first, nyb, rank_y, u);
+            lds_vecs<6>(fy, nt, tid, pn);
+        } else {
+            lds_link<1, RECON>(lnk, 0, nts, st - Lx, u);
+            lds_vecs<6>(pl, nt, tid - Lx, pn);
+        }
+        hop_backward<1>(acc, u, pn);
+        if (more && (face_yf | face_yb)) stage_spinor(fy, s3_y + toff_n);
+        cpa_commit(); // c2
+        cpa_wait<1>();   // links z,t of slice t, own spinor of slice t+1, z-face spinor of slice t have landed
+        __syncthreads(); // (M) ... everybody's; the x,y hops of slice t are over
+        if (more) stage_XY(toff_n);
+        cpa_commit(); // c3
+        // ---- z ----
+        lds_link<2, RECON>(lnk, 0, nts, st, u);
+        if (face_zf) lds_vecs<6>(fz, nt, tid, pn);
+        else lds_vecs<6>(pl, nt, tid + Lx * ty, pn);
+        hop_forward<2>(acc, u, pn);
+        if (face_zb) {
+            lds_link<2, RECON>(flz, FZ::first, nzb, rank_z, u);
+            lds_vecs<6>(fz, nt, tid, pn);
+        } else {
+            lds_link<2, RECON>(lnk, 0, nts, st - Lx * ty, u);
+            lds_vecs<6>(pl, nt, tid - Lx * ty, pn);
+        }
+        hop_backward<2>(acc, u, pn);
+        if (more && (face_zf | face_zb)) stage_spinor(fz, s3_z + toff_n);
+        cpa_commit(); // c4
+        // ---- t: forward hop now, backward product for the next slice ----
+        lds_link<3, RECON>(lnk, 0, nts, st, u);
+        {
+            float h[12];
+            lds_vecs<6>(plane0 + (cur ^ 1) * plane_sz, nt, tid, pn);
+            hop_forward<3>(acc, u, pn);
+            project<3, +1>(psi, h);
+            su3_dag_mul(u, h, chi_t);
+        }
+        // fused diagonal (step a6) and store (a7)
+#pragma unroll
+        for (int i = 0; i < 24; ++i) psi[i] = fmaf(cdiag, psi[i], -0.5f * acc[i]);
+        if (live) store_spinor(out, s3 + toff, psi);
+        cur ^= 1;
+    }
+    cpa_wait<0>();
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+template <int RECON, int NRB>
+cudaError_t launch_mrhs_t(const ApplyArgs &a, int ty, int tz)
+{
+    auto kern = dslash_mrhs_kernel<RECON, NRB>;
+    const int Lx = a.dims[0];
+    const int nts = Lx * ty * tz;
+    const size_t smem = (size_t)mrhs_smem_vecs<RECON>(nts, NRB, Lx * tz, Lx * ty) * sizeof(float4);
+    if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
+    static size_t smem_set = 0;
+    cudaError_t e;
+    if (smem > smem_set) {
+        if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        smem_set = smem;
+    }
+    int tc = 16; // slices per t-chunk (WD_TILE_TC / WD_TILE_NCHUNK override); measured best for 24 RHS on 32^3 x 64
+    if (const char *ev = getenv("WD_TILE_TC")) {
+        const int v = atoi(ev);
+        if (v >= 1) tc = v;
+    }
+    int nchunk = (a.dims[3] + tc - 1) / tc;
+    if (const char *ev = getenv("WD_TILE_NCHUNK")) {
+        const int v = atoi(ev);
+        if (v >= 1 && v <= a.dims[3]) nchunk = v;
+    }
+    if (nchunk < 1) nchunk = 1;
+    const long long ncol = (long long)(a.dims[1] / ty) * (a.dims[2] / tz);
+    const long long ngroups = (a.nrhs + NRB - 1) / NRB;
+    if (ncol * nchunk * ngroups > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)(ncol * nchunk * ngroups));
+    const float cdiag = (float)(4.0 + a.mass); // formed in double, rounded once (reading S8)
+    kern<<<grid, nts * NRB, smem, a.stream>>>((float *)a.out, (const float *)a.in, (const float *)a.links, a.dims[0],
+                                               a.dims[1], a.dims[2], a.dims[3], ty, tz, a.V, cdiag, a.nrhs, nchunk);
+    count_launch();
+    return cudaGetLastError();
+}
+
+template <int RECON>
+cudaError_t launch_mrhs_r(const ApplyArgs &a, int ty, int tz)
+{
+    // right-hand sides per CTA: 3 (12 warps per SM; 24 = 8 x 3) unless WD_TILE_NRB says otherwise
+    int nrb = a.nrhs >= 3 ? 3 : a.nrhs;
+    if (const char *ev = getenv("WD_TILE_NRB")) {
+        const int v = atoi(ev);
+        if (v >= 1 && v <= 3) nrb = v;
+    }
+    if (nrb >= 3) return launch_mrhs_t<RECON, 3>(a, ty, tz);
+    if (nrb == 2) return launch_mrhs_t<RECON, 2>(a, ty, tz);
+    return launch_mrhs_t<RECON, 1>(a, ty, tz);
+}
+
+} // namespace
+
+// shape: chosen by the caller (wd_dslash_stage.cu: same rule as the single-RHS staged kernel)
+cudaError_t launch_mrhs(const ApplyArgs &a, int ty, int tz)
+{
+    return a.recon == 18 ? launch_mrhs_r<18>(a, ty, tz) : launch_mrhs_r<12>(a, ty, tz);
+}
+
+} // namespace wd

@@ -377,8 +377,15 @@ bool stage_supported(const ApplyArgs &a)
     return a.nrhs >= 1 && stage_shape(a, s);
 }
 
+cudaError_t launch_mrhs(const ApplyArgs &a, int ty, int tz); // wd_dslash_mrhs.cu
+
 cudaError_t launch_stage(const ApplyArgs &a)
 {
+    if (a.nrhs > 1 && !(getenv("WD_STAGE_NO_MRHS") && atoi(getenv("WD_STAGE_NO_MRHS")))) {
+        StageShape s; // several right-hand sides: the kernel that shares the staged links between them
+        if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
+        if (s.nt <= 128) return launch_mrhs(a, s.ty, s.tz); // (a forced bigger tile runs RHS by RHS below)
+    }
     return a.recon == 18 ? launch_stage_t<18>(a) : launch_stage_t<12>(a);
 }
 

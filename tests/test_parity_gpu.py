@@ -134,6 +134,33 @@ def test_stage_kernel_baseline_configs(oracle, name):
     check_config(oracle, fields.CONFIGS[name], "stage")
 
 
+@pytest.mark.parametrize("nrb", ["1", "2", "3"])
+@pytest.mark.parametrize("nrhs", [2, 3, 4, 5, 7, 24])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_stage_kernel_multi_rhs_groups(oracle, monkeypatch, nrb, nrhs, recon):
+    """The multi-RHS staged kernel (links shared in smem by WD_TILE_NRB right-hand sides per CTA),
+    including partial last groups."""
+    monkeypatch.setenv("WD_TILE_NRB", nrb)
+    cfg = fields.Config("mrhs", (16, 4, 8, 6), 32, "haar", recon, -0.42, nrhs, 29)
+    check_config(oracle, cfg, "stage")
+
+
+def test_stage_kernel_nv20_and_batched_consistency(oracle):
+    """N_v = 20 through the multi-RHS kernel; each RHS equals its single-RHS apply bit for bit
+    is not required (S10), 1e-6 is."""
+    cfg = fields.Config("nv20", (32, 4, 4, 8), 32, "smooth", 18, -0.42, 20, 33)
+    U, psi = fields.make_fields(cfg)
+    op = GpuOp(U, cfg.dims, 32, 18, KERNELS["stage"])
+    batched = op.apply(psi, cfg.mass)
+    for r in (0, 7, 19):
+        single = op.apply(psi[r:r + 1], cfg.mass)
+        assert rel_l2(batched[r], single[0]) <= 1e-6
+    want = oracle_apply(oracle, psi, U, cfg.dims, cfg.mass)
+    for r in range(20):
+        assert rel_l2(batched[r], want[r]) <= TOL[32]
+    op.close()
+
+
 def test_stage_kernel_rejects_fp64_and_odd_lattices():
     from paper_0912_2186_b200 import binding
     for dims, precision in (((8, 4, 4, 4), 64), ((24, 4, 4, 4), 32), ((32, 3, 4, 4), 32)):
