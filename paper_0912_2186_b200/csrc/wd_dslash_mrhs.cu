@@ -86,7 +86,7 @@ template <int RECON> constexpr int mrhs_smem_vecs(int nts, int nrb, int nyb, int
 template <int RECON, int NRB>
 __global__ void __launch_bounds__(128 * NRB, 1)
 dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const float *__restrict__ links, int Lx, int Ly,
-                   int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk)
+                   int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk, int patch)
 {
     constexpr int NVEC = LinkLayout<float, RECON>::NVEC;
     using FY = LinkVecs<1, RECON>;
@@ -108,9 +108,28 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
     const int ncy = Ly / ty;
     const int ncol = ncy * (Lz / tz);
     const int ngroups = (nrhs + NRB - 1) / NRB;
-    const int col = blockIdx.x % ncol;
-    const int kg = blockIdx.x / ncol;
-    const int g = kg % ngroups, k = kg / ngroups;
+    int col, g, k;
+    if (patch > 0) {
+        // (t-chunk, patch of patch x patch tile columns, column in patch, RHS group), group FASTEST: the
+        // ~#SM resident CTAs are all RHS groups of one compact patch of columns marching through the
+        // same slices, so a slice's links are read from HBM by one group and from L2 by the others,
+        // and only faces on the patch boundary leave the patch.
+        const int per_chunk = ncol * ngroups;
+        k = blockIdx.x / per_chunk;
+        const int r = blockIdx.x - k * per_chunk;
+        const int per_patch = patch * patch * ngroups;
+        const int p = r / per_patch, w = r - p * per_patch;
+        g = w % ngroups;
+        const int c = w / ngroups;                 // column within the patch
+        const int npy = ncy / patch;               // patches along y
+        const int cyy = (p % npy) * patch + c % patch, czz = (p / npy) * patch + c / patch;
+        col = cyy + ncy * czz;
+    } else { // (t-chunk, RHS group, tile column)
+        col = blockIdx.x % ncol;
+        const int kg = blockIdx.x / ncol;
+        g = kg % ngroups;
+        k = kg / ngroups;
+    }
     const int rhs = g * NRB + rr;
     const bool live = rhs < nrhs; // a partial last group computes a duplicate and does not store it
     in += (long long)(live ? rhs : nrhs - 1) * 24 * padded_volume(V);
@@ -288,7 +307,9 @@ cudaError_t launch_mrhs_t(const ApplyArgs &a, int ty, int tz)
         if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
         smem_set = smem;
     }
-    int tc = 16; // slices per t-chunk (WD_TILE_TC / WD_TILE_NCHUNK override); measured best for 24 RHS on 32^3 x 64
+    // slices per t-chunk (WD_TILE_TC / WD_TILE_NCHUNK override): with (columns x RHS groups) already many
+    // times the SM count, long marches win (measured for 24 RHS on 32^3 x 64: 64 > 32 > 16 > 8)
+    int tc = 64;
     if (const char *ev = getenv("WD_TILE_TC")) {
         const int v = atoi(ev);
         if (v >= 1) tc = v;
@@ -303,9 +324,15 @@ cudaError_t launch_mrhs_t(const ApplyArgs &a, int ty, int tz)
     const long long ngroups = (a.nrhs + NRB - 1) / NRB;
     if (ncol * nchunk * ngroups > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     dim3 grid((unsigned)(ncol * nchunk * ngroups));
+    // block order: patches of 4 x 4 tile columns with the RHS group fastest when the column grid allows
+    // it (WD_MRHS_PATCH=0 / n overrides), else (t-chunk, RHS group, column)
+    int patch = 4;
+    if (const char *ev = getenv("WD_MRHS_PATCH")) patch = atoi(ev);
+    const int ncyh = a.dims[1] / ty, nczh = a.dims[2] / tz;
+    if (patch < 1 || ncyh % patch || nczh % patch) patch = 0;
     const float cdiag = (float)(4.0 + a.mass); // formed in double, rounded once (reading S8)
     kern<<<grid, nts * NRB, smem, a.stream>>>((float *)a.out, (const float *)a.in, (const float *)a.links, a.dims[0],
-                                               a.dims[1], a.dims[2], a.dims[3], ty, tz, a.V, cdiag, a.nrhs, nchunk);
+                                               a.dims[1], a.dims[2], a.dims[3], ty, tz, a.V, cdiag, a.nrhs, nchunk, patch);
     count_launch();
     return cudaGetLastError();
 }
