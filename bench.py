@@ -129,6 +129,27 @@ def dist_env():
     return rank, local, world
 
 
+def rank_config(cfg, recon, nrhs, rank):
+    """Replica of the workload for one rank: same shape, seeds shifted by rank (no data-path collective)."""
+    return fields.Config(cfg.name, cfg.dims, cfg.precision, cfg.links, recon, cfg.mass, nrhs, cfg.seed + 100 * rank, cfg.eps)
+
+
+def max_over_ranks(value, world, device=None):
+    """Slowest rank decides: all-reduce MAX of a host float over the default process group."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gflops(world, applies, flops_per_apply, ms):
+    """Aggregate throughput of `world` replicas that each did `applies` applies in `ms` (max over ranks)."""
+    return world * applies * flops_per_apply / (ms * 1e-3) / 1e9
+
+
 def oracle_rate(cfg, U, psi, budget_s=12.0):
     """Time the oracle as it stands on a bounded sample: whole-lattice applies of RHS 0, repeated
     until ~budget_s of CPU work (at least 1, at most 8).  Returns the cpu_baseline object."""
@@ -218,8 +239,7 @@ def run_wd(args):
               "stage": binding.WD_KERNEL_STAGE}[args.kernel]
 
     # ---- synthetic inputs (each rank its own replica: seeds shifted by rank) -------------------
-    cfg_r = fields.Config(cfg.name, cfg.dims, cfg.precision, cfg.links, recon, cfg.mass, nrhs, cfg.seed + 100 * rank,
-                          cfg.eps)
+    cfg_r = rank_config(cfg, recon, nrhs, rank)
     U, psi = fields.make_fields(cfg_r)
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
@@ -258,14 +278,10 @@ def run_wd(args):
         ev1.record(stream)
         barrier()
     launches = binding.wd_launch_count() - n0
-    ms = ev0.elapsed_time(ev1)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ev0.elapsed_time(ev1), world, dev)
     applies = args.steps * aps
     flops_per_apply = FLOPS_PER_SITE * V * nrhs
-    value = world * applies * flops_per_apply / (ms * 1e-3) / 1e9
+    value = whole_job_gflops(world, applies, flops_per_apply, ms)
     launch_ms = ms / applies
     bytes_per_launch = compulsory_bytes_per_site(cfg.precision, recon, nrhs) * V
     peak, peak_src = measured_peak()
@@ -283,11 +299,8 @@ def run_wd(args):
         op.apply_host(h_out, h_in, cfg.mass, nrhs)
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3
-    if world > 1:
-        t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    e2e_value = world * e2e_applies * flops_per_apply / (e2e_ms * 1e-3) / 1e9
+    e2e_ms = max_over_ranks(e2e_ms, world, dev)
+    e2e_value = whole_job_gflops(world, e2e_applies, flops_per_apply, e2e_ms)
     field_bytes = nrhs * V * 24 * (4 if cfg.precision == 32 else 8)
 
     line = None
