@@ -327,7 +327,8 @@ def run_wd(args):
             "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": ncu_traffic(cfg.name, recon), "peak_source": peak_src,
-                         "bytes_per_launch": bytes_per_launch, "kernel": "wd dslash (" + args.kernel + ")"},
+                         "bytes_per_launch": bytes_per_launch,
+                         "kernel": "wd dslash, " + op.selected_kernel(nrhs) + " kernel" + (" (multi-RHS member)" if nrhs > 1 and op.selected_kernel(nrhs) == "stage" else "")},
         }
         if cpu is not None:
             line["cpu_baseline"] = cpu

@@ -109,6 +109,10 @@ int wd_set_stream(wd_gauge *gauge, void *stream);
 /* Force a kernel variant (wd_kernel).  WD_ERR_MISMATCH if it cannot handle the lattice. */
 int wd_set_kernel(wd_gauge *gauge, int kernel);
 
+/* The kernel (wd_kernel, > 0) that wd_apply will launch for this gauge and nrhs right-hand sides:
+ * the forced one, or what WD_KERNEL_AUTO resolves to.  Host-only query; negative wd_status on error. */
+int wd_selected_kernel(const wd_gauge *gauge, int nrhs);
+
 /* Bytes of a NATIVE spinor buffer holding nrhs fields: nrhs * Vpad * 24 * sizeof(real), where
  * Vpad = V rounded up to a multiple of 32 sites.  0 on bad arguments. */
 size_t wd_spinor_bytes(const wd_lattice *lat, int nrhs, int precision);

@@ -23,7 +23,7 @@ STATUS_NAMES = {
 # every symbol include/wd.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
-    "wd_set_kernel", "wd_spinor_bytes", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
+    "wd_set_kernel", "wd_selected_kernel", "wd_spinor_bytes", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
     "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
 )
 
@@ -53,6 +53,7 @@ def lib():
     L.wd_load_gauge.argtypes = [vp, vp, i, i, vp, ctypes.POINTER(vp)]
     L.wd_set_stream.argtypes = [vp, vp]
     L.wd_set_kernel.argtypes = [vp, i]
+    L.wd_selected_kernel.argtypes = [vp, i]
     L.wd_spinor_bytes.argtypes = [vp, i, i]
     L.wd_spinor_bytes.restype = ctypes.c_size_t
     L.wd_pack_spinor.argtypes = [vp, vp, vp, i, i, vp]
@@ -68,7 +69,7 @@ def lib():
     L.wd_destroy.argtypes = [vp]
     L.wd_destroy.restype = None
     for name in ("wd_create_lattice", "wd_lattice_dims", "wd_load_gauge", "wd_set_stream", "wd_set_kernel",
-                 "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host"):
+                 "wd_selected_kernel", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host"):
         getattr(L, name).restype = i
     _lib = L
     return L
@@ -137,6 +138,16 @@ def wd_set_kernel(gauge, kernel):
     _check(lib().wd_set_kernel(gauge, int(kernel)), "wd_set_kernel")
 
 
+def wd_selected_kernel(gauge, nrhs=1):
+    k = int(lib().wd_selected_kernel(gauge, int(nrhs)))
+    if k < 0:
+        _check(k, "wd_selected_kernel")
+    return k
+
+
+KERNEL_NAMES = {WD_KERNEL_SITE: "site", WD_KERNEL_TILE: "tile", WD_KERNEL_STAGE: "stage"}
+
+
 def wd_spinor_bytes(lat, nrhs, precision):
     return int(lib().wd_spinor_bytes(lat, int(nrhs), int(precision)))
 
@@ -200,6 +211,10 @@ class WilsonDirac:
 
     def unpack(self, canonical_dev, native_dev, nrhs, stream=None):
         wd_unpack_spinor(self.lat, canonical_dev, native_dev, nrhs, self.precision, stream or self.stream)
+
+    def selected_kernel(self, nrhs=1):
+        """Name of the kernel wd_apply will launch for nrhs right-hand sides ("site", "tile", "stage")."""
+        return KERNEL_NAMES[wd_selected_kernel(self.gauge, nrhs)]
 
     def native_numel(self, nrhs=1):
         """Reals in a NATIVE spinor buffer of nrhs fields (the volume is padded to 32-site blocks)."""

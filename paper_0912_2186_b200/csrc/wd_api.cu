@@ -208,6 +208,28 @@ int wd_unpack_spinor(const wd_lattice *lat, void *canonical_dev, const void *nat
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_unpack_spinor");
 }
 
+// which kernel WD_KERNEL_AUTO resolves to, by measurement (profiles/): on a lattice of at least a few
+// waves of tiles the staged kernels (fp32; single- and multi-RHS members) or, for one fp64 right-hand
+// side, the tile kernel; everything else -> site kernel
+static int auto_kernel(const wd::ApplyArgs &a)
+{
+    const bool big = a.V >= (1LL << 18);
+    if (big && wd::stage_supported(a)) return WD_KERNEL_STAGE;
+    if (big && a.nrhs == 1 && wd::tile_supported(a)) return WD_KERNEL_TILE;
+    return WD_KERNEL_SITE;
+}
+
+static wd::ApplyArgs shape_args(const wd_gauge *g, int nrhs)
+{
+    wd::ApplyArgs a{};
+    for (int d = 0; d < 4; ++d) a.dims[d] = g->dims[d];
+    a.V = g->V;
+    a.nrhs = nrhs;
+    a.precision = g->precision;
+    a.recon = g->recon;
+    return a;
+}
+
 static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double mass, int nrhs)
 {
     wd::ApplyArgs a{};
@@ -231,17 +253,8 @@ static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double m
         if (!wd::stage_supported(a)) return fail(WD_ERR_MISMATCH, "wd_apply: staged kernel cannot take this call");
         e = wd::launch_stage(a);
     } else {
-        // WD_KERNEL_AUTO, by measurement (profiles/): on a lattice of at least a few waves of tiles the
-        // staged kernels (fp32; single- and multi-RHS members) or, for one fp64 right-hand side, the tile
-        // kernel; everything else -> site kernel
-        const bool big = a.V >= (1LL << 18);
-        const bool big1 = big && a.nrhs == 1;
-        if (big && wd::stage_supported(a))
-            e = wd::launch_stage(a);
-        else if (big1 && wd::tile_supported(a))
-            e = wd::launch_tile(a);
-        else
-            e = wd::launch_site(a);
+        const int k = auto_kernel(a);
+        e = k == WD_KERNEL_STAGE ? wd::launch_stage(a) : k == WD_KERNEL_TILE ? wd::launch_tile(a) : wd::launch_site(a);
     }
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply: kernel launch");
 }
@@ -299,6 +312,15 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
     e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: stream synchronize");
     return WD_OK;
+}
+
+int wd_selected_kernel(const wd_gauge *gauge, int nrhs)
+{
+    if (!gauge) return fail(WD_ERR_NULL, "wd_selected_kernel: NULL gauge");
+    if (gauge->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_selected_kernel: not a live wd_gauge handle");
+    if (nrhs < 1) return fail(WD_ERR_NRHS, "wd_selected_kernel: nrhs=%d", nrhs);
+    if (gauge->kernel != WD_KERNEL_AUTO) return gauge->kernel;
+    return auto_kernel(shape_args(gauge, nrhs));
 }
 
 long long wd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }

@@ -155,9 +155,17 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
     const long long s3_z = face_zf ? s3 + (z + 1 == Lz ? -(long long)(Lz - 1) * Lx * Ly : (long long)Lx * Ly)
                                    : s3 + (z == 0 ? (long long)(Lz - 1) * Lx * Ly : -(long long)Lx * Ly);
 
+    // Native addresses: Lx*Ly*Lz is a multiple of the 32-site layout block, so moving a site by `toff`
+    // (a whole number of slices) moves its record by toff * (vectors per site): one base pointer per
+    // stream, computed once, plus a per-slice offset.
+    const float4 *sp_own = spinor_ptr(in, s3), *sp_y = spinor_ptr(in, s3_y), *sp_z = spinor_ptr(in, s3_z);
+    const float4 *lk_own = link_ptr<float, RECON>(links, s3), *lk_y = link_ptr<float, RECON>(links, s3_y),
+                 *lk_z = link_ptr<float, RECON>(links, s3_z);
+    float4 *out_own = const_cast<float4 *>(spinor_ptr(out, s3));
+
     // ---- staging helpers ----
-    auto stage_spinor = [&](float4 *dst, long long site) { // private slot
-        const float4 *q = spinor_ptr(in, site);
+    auto stage_spinor = [&](float4 *dst, const float4 *base, long long toff) { // private slot
+        const float4 *q = base + toff * 6;
 #pragma unroll
         for (int c = 0; c < 6; ++c) cpa16(dst + c * nt + tid, q + c * BLK);
     };
@@ -178,25 +186,25 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         else copy_links(std::integral_constant<int, 2 % NRB>{}, j0, j1, dst, stride, slot, src, src0);
     };
     auto stage_XY = [&](long long toff) { // links x,y of the site + the y-face link
-        deal_links(0, A_END, lnk, nts, st, link_ptr<float, RECON>(links, s3 + toff), 0);
-        if (face_yb) deal_links(0, FY::n, fly, nyb, rank_y, link_ptr<float, RECON>(links, s3_y + toff), FY::first);
+        deal_links(0, A_END, lnk, nts, st, lk_own + toff * NVEC, 0);
+        if (face_yb) deal_links(0, FY::n, fly, nyb, rank_y, lk_y + toff * NVEC, FY::first);
     };
     auto stage_ZT = [&](long long toff) { // links z,t of the site + the z-face link
-        deal_links(A_END, NVEC, lnk + A_END * nts, nts, st, link_ptr<float, RECON>(links, s3 + toff), A_END);
-        if (face_zb) deal_links(0, FZ::n, flz, nzb, rank_z, link_ptr<float, RECON>(links, s3_z + toff), FZ::first);
+        deal_links(A_END, NVEC, lnk + A_END * nts, nts, st, lk_own + toff * NVEC, A_END);
+        if (face_zb) deal_links(0, FZ::n, flz, nzb, rank_z, lk_z + toff * NVEC, FZ::first);
     };
 
     float chi_t[12]; // U_t(t-1)^dag P+_t psi(t-1) of this (site, rhs)
     int cur = 0;
     if (t_begin < t_end) { // ---- start the march at slice t_begin ----
         const long long toff = (long long)t_begin * S3;
-        stage_spinor(plane0 + cur * plane_sz, s3 + toff);
+        stage_spinor(plane0 + cur * plane_sz, sp_own, toff);
         cpa_commit(); // c0
-        if (face_yf | face_yb) stage_spinor(fy, s3_y + toff);
+        if (face_yf | face_yb) stage_spinor(fy, sp_y, toff);
         cpa_commit(); // c2'
         stage_XY(toff);
         cpa_commit(); // c3'
-        if (face_zf | face_zb) stage_spinor(fz, s3_z + toff);
+        if (face_zf | face_zb) stage_spinor(fz, sp_z, toff);
         cpa_commit(); // c4'
         const long long site_tb = s3 + (long long)(t_begin == 0 ? Lt - 1 : t_begin - 1) * S3;
         float u[18], p[24], h[12];
@@ -213,7 +221,7 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         cpa_wait<1>();   // links x,y and the y-face spinor of slice t have landed (own copies)
         __syncthreads(); // (A) ... everybody's; the z,t hops of slice t-1 are over
         stage_ZT(toff);
-        stage_spinor(plane0 + (cur ^ 1) * plane_sz, s3 + toff_n);
+        stage_spinor(plane0 + (cur ^ 1) * plane_sz, sp_own, toff_n);
         cpa_commit(); // c1
 
         const float4 *pl = plane0 + cur * plane_sz;
@@ -249,7 +257,7 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
             lds_vecs<6>(pl, nt, tid - Lx, pn);
         }
         hop_backward<1>(acc, u, pn);
-        if (more && (face_yf | face_yb)) stage_spinor(fy, s3_y + toff_n);
+        if (more && (face_yf | face_yb)) stage_spinor(fy, sp_y, toff_n);
         cpa_commit(); // c2
         cpa_wait<1>();   // links z,t of slice t, own spinor of slice t+1, z-face spinor of slice t have landed
         __syncthreads(); // (M) ... everybody's; the x,y hops of slice t are over
@@ -268,7 +276,7 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
             lds_vecs<6>(pl, nt, tid - Lx * ty, pn);
         }
         hop_backward<2>(acc, u, pn);
-        if (more && (face_zf | face_zb)) stage_spinor(fz, s3_z + toff_n);
+        if (more && (face_zf | face_zb)) stage_spinor(fz, sp_z, toff_n);
         cpa_commit(); // c4
         // ---- t: forward hop now, backward product for the next slice ----
         lds_link<3, RECON>(lnk, 0, nts, st, u);
@@ -282,7 +290,11 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         // fused diagonal (step a6) and store (a7)
 #pragma unroll
         for (int i = 0; i < 24; ++i) psi[i] = fmaf(cdiag, psi[i], -0.5f * acc[i]);
-        if (live) store_spinor(out, s3 + toff, psi);
+        if (live) {
+            float4 *q = out_own + toff * 6;
+#pragma unroll
+            for (int c = 0; c < 6; ++c) q[c * BLK] = make_float4(psi[4 * c], psi[4 * c + 1], psi[4 * c + 2], psi[4 * c + 3]);
+        }
         cur ^= 1;
     }
     cpa_wait<0>();

@@ -146,30 +146,38 @@ dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const
     const long long s3_z = face_zf ? s3 + (z + 1 == Lz ? -(long long)(Lz - 1) * Lx * Ly : (long long)Lx * Ly)
                                    : s3 + (z == 0 ? (long long)(Lz - 1) * Lx * Ly : -(long long)Lx * Ly);
 
+    // Native addresses: Lx*Ly*Lz is a multiple of the 32-site layout block, so moving a site by `toff`
+    // (a whole number of slices) moves its record by toff * (vectors per site): one base pointer per
+    // stream, computed once, plus a per-slice offset -- no per-copy index arithmetic.
+    const float4 *sp_own = spinor_ptr(in, s3), *sp_y = spinor_ptr(in, s3_y), *sp_z = spinor_ptr(in, s3_z);
+    const float4 *lk_own = link_ptr<float, RECON>(links, s3), *lk_y = link_ptr<float, RECON>(links, s3_y),
+                 *lk_z = link_ptr<float, RECON>(links, s3_z);
+    float4 *out_own = const_cast<float4 *>(spinor_ptr(out, s3));
+
     // ---- staging helpers (slots private to the thread) ----
-    auto stage_spinor = [&](float4 *dst, long long site) {
-        const float4 *q = spinor_ptr(in, site);
+    auto stage_spinor = [&](float4 *dst, const float4 *base, long long toff) {
+        const float4 *q = base + toff * 6;
 #pragma unroll
         for (int c = 0; c < 6; ++c) cpa16(dst + c * nt + tid, q + c * BLK);
     };
     auto stage_A = [&](long long toff) { // links x,y of the own site + y face, slice offset toff
-        const float4 *q = link_ptr<float, RECON>(links, s3 + toff);
+        const float4 *q = lk_own + toff * NVEC;
 #pragma unroll
         for (int j = 0; j < A_END; ++j) cpa16(lnk + j * nt + tid, q + j * BLK);
-        if (face_yf | face_yb) stage_spinor(fy, s3_y + toff);
+        if (face_yf | face_yb) stage_spinor(fy, sp_y, toff);
         if (face_yb) {
-            const float4 *f = link_ptr<float, RECON>(links, s3_y + toff);
+            const float4 *f = lk_y + toff * NVEC;
 #pragma unroll
             for (int j = 0; j < FY::n; ++j) cpa16(fly + j * nyb + rank_y, f + (FY::first + j) * BLK);
         }
     };
     auto stage_B = [&](long long toff) { // links z,t of the own site + z face
-        const float4 *q = link_ptr<float, RECON>(links, s3 + toff);
+        const float4 *q = lk_own + toff * NVEC;
 #pragma unroll
         for (int j = A_END; j < NVEC; ++j) cpa16(lnk + j * nt + tid, q + j * BLK);
-        if (face_zf | face_zb) stage_spinor(fz, s3_z + toff);
+        if (face_zf | face_zb) stage_spinor(fz, sp_z, toff);
         if (face_zb) {
-            const float4 *f = link_ptr<float, RECON>(links, s3_z + toff);
+            const float4 *f = lk_z + toff * NVEC;
 #pragma unroll
             for (int j = 0; j < FZ::n; ++j) cpa16(flz + j * nzb + rank_z, f + (FZ::first + j) * BLK);
         }
@@ -179,7 +187,7 @@ dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const
     int cur = 0;
     if (t_begin < t_end) { // ---- start the march at slice t_begin ----
         const long long toff = (long long)t_begin * S3;
-        stage_spinor(plane0 + cur * plane_sz, s3 + toff);
+        stage_spinor(plane0 + cur * plane_sz, sp_own, toff);
         cpa_commit(); // P'
         stage_A(toff);
         cpa_commit(); // A'
@@ -198,7 +206,7 @@ dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const
         const long long toff_n = (long long)(t + 1 == Lt ? 0 : t + 1) * S3;
         const bool more = (t + 1 < t_end); // the next slice is still ours: keep its links and faces coming
         // P: own spinor of slice t+1 -> the other slice buffer (its old content, slice t-1, is dead)
-        stage_spinor(plane0 + (cur ^ 1) * plane_sz, s3 + toff_n);
+        stage_spinor(plane0 + (cur ^ 1) * plane_sz, sp_own, toff_n);
         cpa_commit();
         cpa_wait<2>();   // own spinor of slice t (earlier P) and group A of slice t have landed
         __syncthreads(); // (A) slice t complete for every thread
@@ -286,7 +294,11 @@ dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const
         // fused diagonal (step a6) and store (a7)
 #pragma unroll
         for (int i = 0; i < 24; ++i) psi[i] = fmaf(cdiag, psi[i], -0.5f * acc[i]);
-        store_spinor(out, s3 + toff, psi);
+        {
+            float4 *q = out_own + toff * 6;
+#pragma unroll
+            for (int c = 0; c < 6; ++c) q[c * BLK] = make_float4(psi[4 * c], psi[4 * c + 1], psi[4 * c + 2], psi[4 * c + 3]);
+        }
         cur ^= 1;
     }
     cpa_wait<0>();

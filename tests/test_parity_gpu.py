@@ -322,6 +322,21 @@ def test_argument_errors_on_device():
     op.close()
 
 
+def test_auto_kernel_selection():
+    """WD_KERNEL_AUTO resolves by lattice, precision and nrhs; a forced kernel is reported."""
+    from paper_0912_2186_b200 import binding
+    cases = [((32, 16, 16, 32), 32, 1, "stage"), ((32, 16, 16, 32), 32, 24, "stage"), ((32, 16, 16, 32), 64, 1, "tile"),
+             ((32, 16, 16, 32), 64, 4, "site"), ((24, 24, 24, 32), 32, 1, "site"), ((8, 8, 8, 8), 32, 1, "site")]
+    for dims, precision, nrhs, want in cases:
+        cfg = fields.Config("sel", dims, precision, "haar", 18, 0.1, 1, 5)
+        U, _ = fields.make_fields(cfg)
+        op = GpuOp(U, dims, precision, 18)
+        assert op.op.selected_kernel(nrhs) == want, (dims, precision, nrhs)
+        op.op.set_kernel(KERNELS["site"])
+        assert op.op.selected_kernel(nrhs) == "site"
+        op.close()
+
+
 def test_launch_counter_counts_kernels():
     from paper_0912_2186_b200 import binding
     cfg = fields.Config("l", (4, 4, 4, 4), 32, "haar", 18, 0.1, 1, 71)
