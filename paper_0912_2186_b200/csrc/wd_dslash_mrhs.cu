@@ -83,7 +83,8 @@ template <int RECON> constexpr int mrhs_smem_vecs(int nts, int nrb, int nyb, int
 
 // gridDim.x = nchunk * ngroups * ncol, ordered (t-chunk, RHS group, tile column).
 // blockDim.x = nts * NRB, nts = Lx*ty*tz sites of the tile (a multiple of 32, at most 128).
-template <int RECON, int NRB>
+// NTS: sites per tile known at compile time (128, the default tile) or 0 = blockDim.x / NRB
+template <int RECON, int NRB, int NTS>
 __global__ void __launch_bounds__(128 * NRB, 1)
 dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const float *__restrict__ links, int Lx, int Ly,
                    int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk, int patch)
@@ -93,8 +94,8 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
     using FZ = LinkVecs<2, RECON>;
     constexpr int A_END = FY::last + 1; // links x,y = vectors [0, A_END), links z,t = [A_END, NVEC)
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int nt = blockDim.x, tid = threadIdx.x;
-    const int nts = nt / NRB;
+    const int nts = NTS ? NTS : (int)blockDim.x / NRB, tid = threadIdx.x;
+    const int nt = nts * NRB;
     const int st = tid % nts, rr = tid / nts; // site slot of the tile, right-hand side of the group
     const int nyb = Lx * tz, nzb = Lx * ty;
     float4 *plane0 = reinterpret_cast<float4 *>(smem_raw); // two slice buffers [6][nt], private slots
@@ -305,10 +306,10 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
 // ---------------------------------------------------------------------------------------------
 namespace {
 
-template <int RECON, int NRB>
-cudaError_t launch_mrhs_t(const ApplyArgs &a, int ty, int tz)
+template <int RECON, int NRB, int NTS>
+cudaError_t launch_mrhs_n(const ApplyArgs &a, int ty, int tz)
 {
-    auto kern = dslash_mrhs_kernel<RECON, NRB>;
+    auto kern = dslash_mrhs_kernel<RECON, NRB, NTS>;
     const int Lx = a.dims[0];
     const int nts = Lx * ty * tz;
     const size_t smem = (size_t)mrhs_smem_vecs<RECON>(nts, NRB, Lx * tz, Lx * ty) * sizeof(float4);
@@ -347,6 +348,12 @@ cudaError_t launch_mrhs_t(const ApplyArgs &a, int ty, int tz)
                                                a.dims[1], a.dims[2], a.dims[3], ty, tz, a.V, cdiag, a.nrhs, nchunk, patch);
     count_launch();
     return cudaGetLastError();
+}
+
+template <int RECON, int NRB>
+cudaError_t launch_mrhs_t(const ApplyArgs &a, int ty, int tz)
+{
+    return a.dims[0] * ty * tz == 128 ? launch_mrhs_n<RECON, NRB, 128>(a, ty, tz) : launch_mrhs_n<RECON, NRB, 0>(a, ty, tz);
 }
 
 template <int RECON>

@@ -93,8 +93,10 @@ template <int RECON> constexpr int stage_smem_vecs(int nt, int nyb, int nzb)
 
 // gridDim.x = nchunk * nrhs * ncol, ordered (t-chunk, right-hand side, tile column): all right-hand
 // sides of a t-chunk run back to back, so the chunk's links come from HBM once and then from L2.
-template <int RECON>
-__global__ void __launch_bounds__(256, 1)
+// NT: threads per CTA known at compile time (128, the default tile) or 0 = read blockDim.x; with a
+// constant NT every shared-memory slot is an immediate offset from one base register.
+template <int RECON, int NT>
+__global__ void __launch_bounds__(NT ? NT : 256, 1)
 dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const float *__restrict__ links, int Lx, int Ly,
                     int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk)
 {
@@ -104,7 +106,7 @@ dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const
     using FY = FaceLinkVecs<1, RECON>;
     using FZ = FaceLinkVecs<2, RECON>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int nt = blockDim.x, tid = threadIdx.x;
+    const int nt = NT ? NT : (int)blockDim.x, tid = threadIdx.x;
     const int nyb = Lx * tz, nzb = Lx * ty;
     float4 *plane0 = reinterpret_cast<float4 *>(smem_raw); // two slice buffers [6][nt]
     const int plane_sz = 6 * nt;
@@ -344,12 +346,10 @@ bool stage_shape(const ApplyArgs &a, StageShape &s)
     return best > 0;
 }
 
-template <int RECON>
-cudaError_t launch_stage_t(const ApplyArgs &a)
+template <int RECON, int NT>
+cudaError_t launch_stage_nt(const ApplyArgs &a, const StageShape &s)
 {
-    auto kern = dslash_stage_kernel<RECON>;
-    StageShape s;
-    if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
+    auto kern = dslash_stage_kernel<RECON, NT>;
     const size_t smem = (size_t)stage_smem_vecs<RECON>(s.nt, a.dims[0] * s.tz, a.dims[0] * s.ty) * sizeof(float4);
     if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
     static size_t smem_set = 0;
@@ -379,6 +379,14 @@ cudaError_t launch_stage_t(const ApplyArgs &a)
                                           a.dims[2], a.dims[3], s.ty, s.tz, a.V, cdiag, a.nrhs, nchunk);
     count_launch();
     return cudaGetLastError();
+}
+
+template <int RECON>
+cudaError_t launch_stage_t(const ApplyArgs &a)
+{
+    StageShape s;
+    if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
+    return s.nt == 128 ? launch_stage_nt<RECON, 128>(a, s) : launch_stage_nt<RECON, 0>(a, s);
 }
 
 } // namespace
