@@ -4,6 +4,7 @@
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -280,34 +281,104 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
     const size_t bytes = (size_t)nrhs * (size_t)g->V * 24 * (precision == WD_FP32 ? 4 : 8); // canonical
     const size_t nbytes = (size_t)nrhs * (size_t)wd::padded_volume(g->V) * 24 * (precision == WD_FP32 ? 4 : 8); // native
     if (g->stage_bytes < nbytes) {
-        cudaFree(g->stage_canon);
-        cudaFree(g->stage_in);
-        cudaFree(g->stage_out);
-        g->stage_canon = g->stage_in = g->stage_out = nullptr;
+        void **bufs[4] = {&g->stage_canon, &g->stage_canon_out, &g->stage_in, &g->stage_out};
+        for (void **b : bufs) {
+            cudaFree(*b);
+            *b = nullptr;
+        }
         g->stage_bytes = 0;
-        cudaError_t e = cudaMalloc(&g->stage_canon, nbytes);
-        if (e == cudaSuccess) e = cudaMalloc(&g->stage_in, nbytes);
-        if (e == cudaSuccess) e = cudaMalloc(&g->stage_out, nbytes);
+        cudaError_t e = cudaSuccess;
+        for (void **b : bufs)
+            if (e == cudaSuccess) e = cudaMalloc(b, nbytes);
         if (e != cudaSuccess) {
-            cudaFree(g->stage_canon);
-            cudaFree(g->stage_in);
-            cudaFree(g->stage_out);
-            g->stage_canon = g->stage_in = g->stage_out = nullptr;
+            for (void **b : bufs) {
+                cudaFree(*b);
+                *b = nullptr;
+            }
             cudaGetLastError();
-            return fail(WD_ERR_ALLOC, "wd_apply_host: cudaMalloc of %zu staging bytes failed", 3 * nbytes);
+            return fail(WD_ERR_ALLOC, "wd_apply_host: cudaMalloc of %zu staging bytes failed", 4 * nbytes);
         }
         g->stage_bytes = nbytes;
     }
     cudaStream_t s = g->stream;
-    cudaError_t e = cudaMemcpyAsync(g->stage_canon, in_canonical_host, bytes, cudaMemcpyHostToDevice, s);
+    const size_t w = precision == WD_FP32 ? 4 : 8;
+    const long long S3 = (long long)g->dims[0] * g->dims[1] * g->dims[2];
+    const int Lt = g->dims[3];
+    cudaError_t e;
+
+    // ---- pipelined path: the lattice is cut into up to 16 slabs of whole time slices; slab k is copied in
+    // and packed on one stream, D is applied to it (site kernel on the slab's site range) on a second
+    // stream as soon as slabs k-1, k, k+1 have arrived, and its result is unpacked and copied out on a
+    // third stream, so the host->device and device->host transfers overlap (PCIe is full duplex) ----
+    const int nslab = Lt >= 16 ? 16 : Lt; // (the event arrays of wd_gauge hold 16)
+    const bool pipelined = nslab >= 3 && S3 % 128 == 0 && bytes >= (8u << 20) &&
+                           !(getenv("WD_HOST_NO_PIPELINE") && atoi(getenv("WD_HOST_NO_PIPELINE")));
+    if (pipelined) {
+        if (!g->pipe_stream[0]) {
+            for (int i = 0; i < 3; ++i)
+                if ((e = cudaStreamCreateWithFlags(&g->pipe_stream[i], cudaStreamNonBlocking)) != cudaSuccess)
+                    return cuda_fail(e, "wd_apply_host: stream create");
+            for (auto &ev : g->pipe_event)
+                if ((e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess)
+                    return cuda_fail(e, "wd_apply_host: event create");
+        }
+        cudaStream_t s_in = g->pipe_stream[0], s_cmp = g->pipe_stream[1], s_out = g->pipe_stream[2];
+        cudaEvent_t *ev_in = g->pipe_event, *ev_cmp = g->pipe_event + 16, ev_start = g->pipe_event[32], ev_end = g->pipe_event[33];
+        // everything enqueued on the gauge's stream so far (e.g. the link conversion) comes first
+        if ((e = cudaEventRecord(ev_start, s)) != cudaSuccess) return cuda_fail(e, "wd_apply_host: event record");
+        for (int i = 0; i < 3; ++i) cudaStreamWaitEvent(g->pipe_stream[i], ev_start, 0);
+        auto t0 = [&](int k) { return (long long)Lt * k / nslab; };
+        const size_t row = (size_t)g->V * 24 * w; // bytes of one right-hand side, canonical
+        for (int k = 0; k < nslab; ++k) {
+            const long long s0 = t0(k) * S3, ns = (t0(k + 1) - t0(k)) * S3;
+            e = cudaMemcpy2DAsync((char *)g->stage_canon + (size_t)s0 * 24 * w, row,
+                                  (const char *)in_canonical_host + (size_t)s0 * 24 * w, row, (size_t)ns * 24 * w, nrhs,
+                                  cudaMemcpyHostToDevice, s_in);
+            if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: H2D copy");
+            e = wd::launch_pack_spinor(g->stage_in, g->stage_canon, g->V, nrhs, precision, s_in, s0, ns);
+            if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: pack");
+            cudaEventRecord(ev_in[k], s_in);
+        }
+        // interior slabs in arrival order, then the two that need the wrap-around neighbour
+        for (int i = 0; i < nslab; ++i) {
+            const int k = i < nslab - 2 ? i + 1 : (i == nslab - 2 ? 0 : nslab - 1);
+            const int need[3] = {(k + nslab - 1) % nslab, k, (k + 1) % nslab};
+            for (int n : need) cudaStreamWaitEvent(s_cmp, ev_in[n], 0);
+            wd::ApplyArgs a = shape_args(g, nrhs);
+            a.out = g->stage_out;
+            a.in = g->stage_in;
+            a.links = g->links;
+            a.mass = mass;
+            a.stream = s_cmp;
+            a.site_begin = t0(k) * S3;
+            a.site_end = t0(k + 1) * S3;
+            if ((e = wd::launch_site(a)) != cudaSuccess) return cuda_fail(e, "wd_apply_host: kernel launch");
+            cudaEventRecord(ev_cmp[k], s_cmp);
+            cudaStreamWaitEvent(s_out, ev_cmp[k], 0);
+            e = wd::launch_unpack_spinor(g->stage_canon_out, g->stage_out, g->V, nrhs, precision, s_out, a.site_begin,
+                                         a.site_end - a.site_begin);
+            if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: unpack");
+            e = cudaMemcpy2DAsync((char *)out_canonical_host + (size_t)a.site_begin * 24 * w, row,
+                                  (const char *)g->stage_canon_out + (size_t)a.site_begin * 24 * w, row,
+                                  (size_t)(a.site_end - a.site_begin) * 24 * w, nrhs, cudaMemcpyDeviceToHost, s_out);
+            if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: D2H copy");
+        }
+        if ((e = cudaEventRecord(ev_end, s_out)) != cudaSuccess) return cuda_fail(e, "wd_apply_host: event record");
+        cudaStreamWaitEvent(s, ev_end, 0);
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(e, "wd_apply_host: stream synchronize");
+        return WD_OK;
+    }
+
+    // ---- small or oddly shaped lattices: one stream, whole field at a time ----
+    e = cudaMemcpyAsync(g->stage_canon, in_canonical_host, bytes, cudaMemcpyHostToDevice, s);
     if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: H2D copy");
     e = wd::launch_pack_spinor(g->stage_in, g->stage_canon, g->V, nrhs, precision, s);
     if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: pack");
     rc = dispatch_apply(g->stage_out, g->stage_in, g, mass, nrhs);
     if (rc) return rc;
-    e = wd::launch_unpack_spinor(g->stage_canon, g->stage_out, g->V, nrhs, precision, s);
+    e = wd::launch_unpack_spinor(g->stage_canon_out, g->stage_out, g->V, nrhs, precision, s);
     if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: unpack");
-    e = cudaMemcpyAsync(out_canonical_host, g->stage_canon, bytes, cudaMemcpyDeviceToHost, s);
+    e = cudaMemcpyAsync(out_canonical_host, g->stage_canon_out, bytes, cudaMemcpyDeviceToHost, s);
     if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: D2H copy");
     e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: stream synchronize");
@@ -333,8 +404,13 @@ void wd_destroy_gauge(wd_gauge *gauge)
     gauge->magic = 0;
     cudaFree(gauge->links);
     cudaFree(gauge->stage_canon);
+    cudaFree(gauge->stage_canon_out);
     cudaFree(gauge->stage_in);
     cudaFree(gauge->stage_out);
+    if (gauge->pipe_stream[0]) {
+        for (auto &st : gauge->pipe_stream) cudaStreamDestroy(st);
+        for (auto &ev : gauge->pipe_event) cudaEventDestroy(ev);
+    }
     delete gauge;
 }
 

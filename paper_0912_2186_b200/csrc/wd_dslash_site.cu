@@ -42,7 +42,7 @@ __device__ __forceinline__ void hop_pair(T (&acc)[NR][24], const T *__restrict__
 template <typename T, int RECON, int NR>
 __global__ void __launch_bounds__(SITE_THREADS)
 dslash_site_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ links, int Lx, int Ly, int Lz,
-                   int Lt, long long V, T cdiag, int nrhs, int bps)
+                   int Lt, long long V, T cdiag, int nrhs, int bps, long long site0, long long nsites)
 {
     // Block order (step a'): the lattice is cut into SLABS of bps consecutive site blocks (a few time
     // slices); within a slab all RHS groups are swept one after the other, then the next slab.  The
@@ -51,13 +51,13 @@ dslash_site_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
     // lattice per group re-reads the 604 MB gauge field 12 x from HBM; RHS group fastest loses the
     // spinors' t reuse instead and is slower still.)
     const int ngroups = (nrhs + NR - 1) / NR;
-    const long long nb = (V + SITE_THREADS - 1) / SITE_THREADS;
+    const long long nb = (nsites + SITE_THREADS - 1) / SITE_THREADS; // the launch covers sites [site0, site0 + nsites)
     const long long bid = blockIdx.x;
     const long long slab = bid / ((long long)bps * ngroups);
     const long long nbl = min((long long)bps, nb - slab * bps); // site blocks in this slab
     const long long r = bid - slab * bps * ngroups;
-    const long long site = (slab * bps + r % nbl) * SITE_THREADS + threadIdx.x;
-    if (site >= V) return;
+    const long long site = site0 + (slab * bps + r % nbl) * SITE_THREADS + threadIdx.x;
+    if (site >= site0 + nsites) return;
     const int rhs0 = (int)(r / nbl) * NR;
     const long long Vp = padded_volume(V); // sites per right-hand side in the native layout
 
@@ -99,7 +99,9 @@ dslash_site_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
 template <typename T, int RECON, int NR>
 static cudaError_t launch_site_t(const ApplyArgs &a)
 {
-    const long long nb = (a.V + SITE_THREADS - 1) / SITE_THREADS;
+    const long long site0 = a.site_end > a.site_begin ? a.site_begin : 0;
+    const long long nsites = a.site_end > a.site_begin ? a.site_end - a.site_begin : a.V;
+    const long long nb = (nsites + SITE_THREADS - 1) / SITE_THREADS;
     const long long ngroups = (a.nrhs + NR - 1) / NR;
     if (nb * ngroups > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     // slab: ~32 MB of links (WD_SITE_SLAB_MB overrides) -- a fraction of the 126 MB L2, leaving room
@@ -116,7 +118,7 @@ static cudaError_t launch_site_t(const ApplyArgs &a)
     const T cdiag = (T)(4.0 + a.mass); // formed in double, rounded once (reading S8)
     dslash_site_kernel<T, RECON, NR><<<grid, SITE_THREADS, 0, a.stream>>>(
         (T *)a.out, (const T *)a.in, (const T *)a.links, a.dims[0], a.dims[1], a.dims[2], a.dims[3], a.V, cdiag, a.nrhs,
-        (int)bps);
+        (int)bps, site0, nsites);
     count_launch();
     return cudaGetLastError();
 }

@@ -20,10 +20,13 @@ struct wd_gauge {
     size_t links_bytes;
     cudaStream_t stream;
     // staging for wd_apply_host (allocated on first use)
-    void *stage_canon;   // canonical spinor buffer, device
+    void *stage_canon;   // canonical spinor buffer (input), device
+    void *stage_canon_out; // canonical spinor buffer (result), device
     void *stage_in;      // native in
     void *stage_out;     // native out
     size_t stage_bytes;
+    cudaStream_t pipe_stream[3]; // copy-in, compute, copy-out streams of the pipelined host path
+    cudaEvent_t pipe_event[2 * 16 + 2];
 };
 
 namespace wd {
@@ -39,6 +42,7 @@ struct ApplyArgs {
     int precision;
     int recon;
     cudaStream_t stream;
+    long long site_begin, site_end; // site kernel only: apply on [site_begin, site_end); 0,0 = whole lattice
 };
 
 void count_launch(int n = 1);
@@ -52,10 +56,11 @@ cudaError_t launch_tile(const ApplyArgs &a);
 bool stage_supported(const ApplyArgs &a);
 cudaError_t launch_stage(const ApplyArgs &a);
 
+// site range [site0, site0 + nsites) of every right-hand side; site0 a multiple of 128; nsites < 0 = all
 cudaError_t launch_pack_spinor(void *native, const void *canonical, long long V, int nrhs, int precision,
-                               cudaStream_t s);
+                               cudaStream_t s, long long site0 = 0, long long nsites = -1);
 cudaError_t launch_unpack_spinor(void *canonical, const void *native, long long V, int nrhs, int precision,
-                                 cudaStream_t s);
+                                 cudaStream_t s, long long site0 = 0, long long nsites = -1);
 cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon,
                               cudaStream_t s);
 size_t native_link_bytes(long long V, int precision, int recon);

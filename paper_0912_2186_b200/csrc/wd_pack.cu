@@ -12,13 +12,13 @@ constexpr int PACK_SITES = 128; // sites per CTA; also the CTA size
 // contiguous 16-byte-per-lane.  Pad sites of the last native block are left untouched.
 template <typename Vec, int NCH, bool TO_NATIVE>
 __global__ void __launch_bounds__(PACK_SITES) spinor_transpose_kernel(Vec *__restrict__ dst, const Vec *__restrict__ src,
-                                                                     long long V)
+                                                                     long long V, long long first, long long end)
 {
     __shared__ Vec tile[NCH][PACK_SITES + 1];
-    const long long site0 = (long long)blockIdx.x * PACK_SITES;
+    const long long site0 = first + (long long)blockIdx.x * PACK_SITES; // first is a multiple of PACK_SITES
     const int rhs = blockIdx.y;
     const int tid = threadIdx.x;
-    const long long nsite = min((long long)PACK_SITES, V - site0);
+    const long long nsite = min((long long)PACK_SITES, end - site0);
     const Vec *canon_src = src + ((long long)rhs * V + site0) * NCH;
     Vec *canon_dst = dst + ((long long)rhs * V + site0) * NCH;
     // native vector 0 of site site0 + tid (site0 is a multiple of 32)
@@ -49,27 +49,32 @@ __global__ void __launch_bounds__(PACK_SITES) spinor_transpose_kernel(Vec *__res
 }
 
 template <bool TO_NATIVE>
-static cudaError_t transpose_spinor(void *dst, const void *src, long long V, int nrhs, int precision, cudaStream_t s)
+static cudaError_t transpose_spinor(void *dst, const void *src, long long V, int nrhs, int precision, cudaStream_t s,
+                                    long long site0, long long nsites)
 {
-    if (V <= 0 || nrhs <= 0) return cudaSuccess;
-    dim3 grid((unsigned)((V + PACK_SITES - 1) / PACK_SITES), (unsigned)nrhs);
+    if (nsites < 0) nsites = V - site0;
+    if (V <= 0 || nrhs <= 0 || nsites <= 0) return cudaSuccess;
+    if (site0 % PACK_SITES || site0 + nsites > V) return cudaErrorInvalidValue;
+    const long long end = site0 + nsites;
+    dim3 grid((unsigned)((nsites + PACK_SITES - 1) / PACK_SITES), (unsigned)nrhs);
     if (precision == 32)
-        spinor_transpose_kernel<float4, 6, TO_NATIVE><<<grid, PACK_SITES, 0, s>>>((float4 *)dst, (const float4 *)src, V);
+        spinor_transpose_kernel<float4, 6, TO_NATIVE><<<grid, PACK_SITES, 0, s>>>((float4 *)dst, (const float4 *)src, V, site0, end);
     else
-        spinor_transpose_kernel<double2, 12, TO_NATIVE><<<grid, PACK_SITES, 0, s>>>((double2 *)dst, (const double2 *)src, V);
+        spinor_transpose_kernel<double2, 12, TO_NATIVE><<<grid, PACK_SITES, 0, s>>>((double2 *)dst, (const double2 *)src, V, site0, end);
     count_launch();
     return cudaGetLastError();
 }
 
-cudaError_t launch_pack_spinor(void *native, const void *canonical, long long V, int nrhs, int precision, cudaStream_t s)
+cudaError_t launch_pack_spinor(void *native, const void *canonical, long long V, int nrhs, int precision, cudaStream_t s,
+                               long long site0, long long nsites)
 {
-    return transpose_spinor<true>(native, canonical, V, nrhs, precision, s);
+    return transpose_spinor<true>(native, canonical, V, nrhs, precision, s, site0, nsites);
 }
 
 cudaError_t launch_unpack_spinor(void *canonical, const void *native, long long V, int nrhs, int precision,
-                                 cudaStream_t s)
+                                 cudaStream_t s, long long site0, long long nsites)
 {
-    return transpose_spinor<false>(canonical, native, V, nrhs, precision, s);
+    return transpose_spinor<false>(canonical, native, V, nrhs, precision, s, site0, nsites);
 }
 
 // canonical U[mu][site][a][b][re,im] -> native [block][vector][lane], the four links of a site

@@ -322,6 +322,31 @@ def test_argument_errors_on_device():
     op.close()
 
 
+@pytest.mark.parametrize("dims,precision,recon,nrhs", [((16, 16, 16, 16), 32, 18, 2), ((32, 16, 16, 5), 64, 12, 2),
+                                                     ((32, 8, 16, 3), 32, 18, 8), ((16, 16, 8, 24), 32, 12, 3)])
+def test_apply_host_pipelined_path(oracle, monkeypatch, dims, precision, recon, nrhs):
+    """wd_apply_host on fields large enough for its slab pipeline (H2D / apply / D2H overlapped on three
+    streams): same bits as the one-stream host path, and the oracle's result."""
+    cfg = fields.Config("hp", dims, precision, "haar", recon, -0.4, nrhs, 53)
+    U, psi = fields.make_fields(cfg)
+    assert psi.nbytes >= 8 << 20
+    op = GpuOp(U, dims, precision, recon, KERNELS["site"])
+    out = np.full_like(psi, np.nan)
+    op.op.apply_host(out, psi, cfg.mass, nrhs)
+    again = np.full_like(psi, np.nan)
+    op.op.apply_host(again, psi, cfg.mass, nrhs)
+    assert np.array_equal(out, again)
+    monkeypatch.setenv("WD_HOST_NO_PIPELINE", "1")
+    plain = np.full_like(psi, np.nan)
+    op.op.apply_host(plain, psi, cfg.mass, nrhs)
+    op.close()
+    assert np.array_equal(out, plain)
+    Uo = oracle_links(U, recon)
+    want = oracle_apply(oracle, psi, Uo, dims, cfg.mass)
+    for r in range(nrhs):
+        assert rel_l2(out[r], want[r]) <= TOL[precision]
+
+
 def test_auto_kernel_selection():
     """WD_KERNEL_AUTO resolves by lattice, precision and nrhs; a forced kernel is reported."""
     from paper_0912_2186_b200 import binding
