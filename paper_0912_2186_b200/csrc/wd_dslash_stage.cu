@@ -1,5 +1,5 @@
 // wd_dslash_stage.cu -- WD_KERNEL_STAGE: the t-marching tile kernel with EVERY global read staged
-// through shared memory by cp.async one step ahead (fp32).
+// through shared memory by cp.async one step ahead (fp32 and fp64).
 //
 // eq. (2.2); SURVEY.md 8(a) steps a1-a7 in one launch.  Same decomposition as
 // wd_dslash_tile.cu (tile Lx x ty x tz of one time slice per CTA, marching along t; x hops by warp
@@ -17,8 +17,8 @@
 //     A = links x,y + y face of t+1 (after the y hops), B = links z,t + z face of t+1 (after the t
 //     hops);  waits: wait_group 2 at the top (P(t), A(t-1 issued) done), 2 before z, 1 before t.
 //
-// Registers are no longer held across memory latency, shared memory is: 840 B/site, two CTAs of
-// 128 sites per SM.  Requires ty, tz >= 2 (a thread has at most one face per direction), Lx a power
+// Registers are no longer held across memory latency, shared memory is: 840 B/site in fp32 (two CTAs
+// of 128 sites per SM), twice that in fp64 (one CTA of 128 sites per SM).  Requires ty, tz >= 2 (a thread has at most one face per direction), Lx a power
 // of two <= 32, Lx*Ly*Lz a multiple of 32.
 #include <cstdio>
 #include <cstdlib>
@@ -32,7 +32,7 @@ namespace wd {
 
 namespace {
 
-__device__ __forceinline__ void cpa16(float4 *smem_dst, const float4 *gsrc)
+__device__ __forceinline__ void cpa16(void *smem_dst, const void *gsrc)
 {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gsrc) : "memory");
@@ -40,43 +40,36 @@ __device__ __forceinline__ void cpa16(float4 *smem_dst, const float4 *gsrc)
 __device__ __forceinline__ void cpa_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cpa_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
-// NV vectors [vec][slot stride] -> registers
-template <int NV>
-__device__ __forceinline__ void lds_vecs(const float4 *buf, int stride, int slot, float *r)
+// NV 16-byte vectors [vec][slot stride] -> registers
+template <int NV, typename Vec, typename T>
+__device__ __forceinline__ void lds_vecs(const Vec *buf, int stride, int slot, T *r)
 {
+    constexpr int CR = 16 / sizeof(T);
 #pragma unroll
-    for (int c = 0; c < NV; ++c) unpack(buf[c * stride + slot], &r[c * 4]);
+    for (int c = 0; c < NV; ++c) unpack(buf[c * stride + slot], &r[c * CR]);
 }
 
-// link MU out of the staged link record (vectors [first, last] of the site's NVEC)
-template <int MU, int RECON>
-__device__ __forceinline__ void lds_link(const float4 *lnk, int nt, int tid, float (&u)[18])
-{
-    constexpr int first = (MU * RECON) / 4, last = (MU * RECON + RECON - 1) / 4, skip = MU * RECON - first * 4;
-    float tmp[(last - first + 1) * 4];
-    lds_vecs<last - first + 1>(lnk + first * nt, nt, tid, tmp);
-#pragma unroll
-    for (int i = 0; i < RECON; ++i) u[i] = tmp[skip + i];
-    if (RECON == 12) reconstruct_row2(u);
-}
-
-// face link MU staged alone: vectors [first, last] of the neighbour's record, stored from vector 0
-template <int MU, int RECON>
-__device__ __forceinline__ void lds_face_link(const float4 *buf, int stride, int slot, float (&u)[18])
-{
-    constexpr int first = (MU * RECON) / 4, last = (MU * RECON + RECON - 1) / 4, skip = MU * RECON - first * 4;
-    float tmp[(last - first + 1) * 4];
-    lds_vecs<last - first + 1>(buf, stride, slot, tmp);
-#pragma unroll
-    for (int i = 0; i < RECON; ++i) u[i] = tmp[skip + i];
-    if (RECON == 12) reconstruct_row2(u);
-}
-
-template <int MU, int RECON> struct FaceLinkVecs {
-    static constexpr int first = (MU * RECON) / 4, last = (MU * RECON + RECON - 1) / 4, n = last - first + 1;
+// vectors of a site's link record that hold link MU
+template <int MU, int RECON, typename T> struct FaceLinkVecs {
+    static constexpr int CR = 16 / sizeof(T);
+    static constexpr int first = (MU * RECON) / CR, last = (MU * RECON + RECON - 1) / CR, n = last - first + 1;
+    static constexpr int skip = MU * RECON - first * CR;
 };
 
-__device__ __forceinline__ void shfl12(float (&dst)[12], const float (&src)[12], int src_lane)
+// link MU out of a staged record: `base` points at vector `first0` of the record, slots `stride` apart
+template <int MU, int RECON, typename Vec, typename T>
+__device__ __forceinline__ void lds_link_at(const Vec *base, int first0, int stride, int slot, T (&u)[18])
+{
+    using LV = FaceLinkVecs<MU, RECON, T>;
+    T tmp[LV::n * LV::CR];
+    lds_vecs<LV::n>(base + (LV::first - first0) * stride, stride, slot, tmp);
+#pragma unroll
+    for (int i = 0; i < RECON; ++i) u[i] = tmp[LV::skip + i];
+    if (RECON == 12) reconstruct_row2(u);
+}
+
+template <typename T>
+__device__ __forceinline__ void shfl12(T (&dst)[12], const T (&src)[12], int src_lane)
 {
 #pragma unroll
     for (int i = 0; i < 12; ++i) dst[i] = __shfl_sync(0xffffffffu, src[i], src_lane);
@@ -84,39 +77,43 @@ __device__ __forceinline__ void shfl12(float (&dst)[12], const float (&src)[12],
 
 } // namespace
 
-// shared-memory float4 vectors of one CTA (see the kernel for the carve-up)
-template <int RECON> constexpr int stage_smem_vecs(int nt, int nyb, int nzb)
+// shared-memory 16-byte vectors of one CTA (see the kernel for the carve-up)
+template <typename T, int RECON> constexpr int stage_smem_vecs(int nt, int nyb, int nzb)
 {
-    return nt * (2 * 6 + 3 + 3 + LinkLayout<float, RECON>::NVEC + 6 + 6) + nyb * FaceLinkVecs<1, RECON>::n +
-           nzb * FaceLinkVecs<2, RECON>::n;
+    return nt * (2 * SpinorLayout<T>::NCH + 2 * (SpinorLayout<T>::NCH / 2) + LinkLayout<T, RECON>::NVEC +
+                 2 * SpinorLayout<T>::NCH) +
+           nyb * FaceLinkVecs<1, RECON, T>::n + nzb * FaceLinkVecs<2, RECON, T>::n;
 }
 
 // gridDim.x = nchunk * nrhs * ncol, ordered (t-chunk, right-hand side, tile column): all right-hand
 // sides of a t-chunk run back to back, so the chunk's links come from HBM once and then from L2.
 // NT: threads per CTA known at compile time (128, the default tile) or 0 = read blockDim.x; with a
 // constant NT every shared-memory slot is an immediate offset from one base register.
-template <int RECON, int NT>
+template <typename T, int RECON, int NT>
 __global__ void __launch_bounds__(NT ? NT : 256, 1)
-dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const float *__restrict__ links, int Lx, int Ly,
-                    int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk)
+dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ links, int Lx, int Ly,
+                    int Lz, int Lt, int ty, int tz, long long V, T cdiag, int nrhs, int nchunk)
 {
-    using LL = LinkLayout<float, RECON>;
+    using SL = SpinorLayout<T>;
+    using Vec = typename SL::Vec;
+    constexpr int NCH = SL::NCH, CR = SL::CR, HCH = NCH / 2; // vectors per spinor / reals per vector / per half spinor
+    using LL = LinkLayout<T, RECON>;
     constexpr int NVEC = LL::NVEC;
-    constexpr int A_END = FaceLinkVecs<1, RECON>::last + 1; // links x,y = vectors [0, A_END), z,t = [A_END, NVEC)
-    using FY = FaceLinkVecs<1, RECON>;
-    using FZ = FaceLinkVecs<2, RECON>;
+    using FY = FaceLinkVecs<1, RECON, T>;
+    using FZ = FaceLinkVecs<2, RECON, T>;
+    constexpr int A_END = FY::last + 1; // links x,y = vectors [0, A_END), z,t = [A_END, NVEC)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nt = NT ? NT : (int)blockDim.x, tid = threadIdx.x;
     const int nyb = Lx * tz, nzb = Lx * ty;
-    float4 *plane0 = reinterpret_cast<float4 *>(smem_raw); // two slice buffers [6][nt]
-    const int plane_sz = 6 * nt;
-    float4 *xchg_y = plane0 + 2 * plane_sz; // [3][nt]  U_y^dag P+_y psi, for the site at y+1
-    float4 *xchg_z = xchg_y + 3 * nt;       // [3][nt]
-    float4 *lnk = xchg_z + 3 * nt;          // [NVEC][nt] the four links of the thread's site
-    float4 *fy = lnk + NVEC * nt;           // [6][nt]   out-of-tile y neighbour spinor (face threads)
-    float4 *fz = fy + 6 * nt;               // [6][nt]   out-of-tile z neighbour spinor
-    float4 *fly = fz + 6 * nt;              // [FY::n][nyb]  U_y of the -y neighbour (yy == 0 threads)
-    float4 *flz = fly + FY::n * nyb;        // [FZ::n][nzb]  U_z of the -z neighbour (zz == 0 threads)
+    Vec *plane0 = reinterpret_cast<Vec *>(smem_raw); // two slice buffers [NCH][nt]
+    const int plane_sz = NCH * nt;
+    Vec *xchg_y = plane0 + 2 * plane_sz; // [HCH][nt]  U_y^dag P+_y psi, for the site at y+1
+    Vec *xchg_z = xchg_y + HCH * nt;     // [HCH][nt]
+    Vec *lnk = xchg_z + HCH * nt;        // [NVEC][nt] the four links of the thread's site
+    Vec *fy = lnk + NVEC * nt;           // [NCH][nt]  out-of-tile y neighbour spinor (face threads)
+    Vec *fz = fy + NCH * nt;             // [NCH][nt]  out-of-tile z neighbour spinor
+    Vec *fly = fz + NCH * nt;            // [FY::n][nyb]  U_y of the -y neighbour (yy == 0 threads)
+    Vec *flz = fly + FY::n * nyb;        // [FZ::n][nzb]  U_z of the -z neighbour (zz == 0 threads)
 
     const int ncy = Ly / ty;
     const int ncol = ncy * (Lz / tz);
@@ -151,41 +148,41 @@ dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const
     // Native addresses: Lx*Ly*Lz is a multiple of the 32-site layout block, so moving a site by `toff`
     // (a whole number of slices) moves its record by toff * (vectors per site): one base pointer per
     // stream, computed once, plus a per-slice offset -- no per-copy index arithmetic.
-    const float4 *sp_own = spinor_ptr(in, s3), *sp_y = spinor_ptr(in, s3_y), *sp_z = spinor_ptr(in, s3_z);
-    const float4 *lk_own = link_ptr<float, RECON>(links, s3), *lk_y = link_ptr<float, RECON>(links, s3_y),
-                 *lk_z = link_ptr<float, RECON>(links, s3_z);
-    float4 *out_own = const_cast<float4 *>(spinor_ptr(out, s3));
+    const Vec *sp_own = spinor_ptr(in, s3), *sp_y = spinor_ptr(in, s3_y), *sp_z = spinor_ptr(in, s3_z);
+    const Vec *lk_own = link_ptr<T, RECON>(links, s3), *lk_y = link_ptr<T, RECON>(links, s3_y),
+              *lk_z = link_ptr<T, RECON>(links, s3_z);
+    Vec *out_own = const_cast<Vec *>(spinor_ptr(static_cast<const T *>(out), s3));
 
     // ---- staging helpers (slots private to the thread) ----
-    auto stage_spinor = [&](float4 *dst, const float4 *base, long long toff) {
-        const float4 *q = base + toff * 6;
+    auto stage_spinor = [&](Vec *dst, const Vec *base, long long toff) {
+        const Vec *q = base + toff * NCH;
 #pragma unroll
-        for (int c = 0; c < 6; ++c) cpa16(dst + c * nt + tid, q + c * BLK);
+        for (int c = 0; c < NCH; ++c) cpa16(dst + c * nt + tid, q + c * BLK);
     };
     auto stage_A = [&](long long toff) { // links x,y of the own site + y face, slice offset toff
-        const float4 *q = lk_own + toff * NVEC;
+        const Vec *q = lk_own + toff * NVEC;
 #pragma unroll
         for (int j = 0; j < A_END; ++j) cpa16(lnk + j * nt + tid, q + j * BLK);
         if (face_yf | face_yb) stage_spinor(fy, sp_y, toff);
         if (face_yb) {
-            const float4 *f = lk_y + toff * NVEC;
+            const Vec *f = lk_y + toff * NVEC;
 #pragma unroll
             for (int j = 0; j < FY::n; ++j) cpa16(fly + j * nyb + rank_y, f + (FY::first + j) * BLK);
         }
     };
     auto stage_B = [&](long long toff) { // links z,t of the own site + z face
-        const float4 *q = lk_own + toff * NVEC;
+        const Vec *q = lk_own + toff * NVEC;
 #pragma unroll
         for (int j = A_END; j < NVEC; ++j) cpa16(lnk + j * nt + tid, q + j * BLK);
         if (face_zf | face_zb) stage_spinor(fz, sp_z, toff);
         if (face_zb) {
-            const float4 *f = lk_z + toff * NVEC;
+            const Vec *f = lk_z + toff * NVEC;
 #pragma unroll
             for (int j = 0; j < FZ::n; ++j) cpa16(flz + j * nzb + rank_z, f + (FZ::first + j) * BLK);
         }
     };
 
-    float chi_t[12]; // U_t(t-1)^dag P+_t psi(t-1) of this site
+    T chi_t[12]; // U_t(t-1)^dag P+_t psi(t-1) of this site
     int cur = 0;
     if (t_begin < t_end) { // ---- start the march at slice t_begin ----
         const long long toff = (long long)t_begin * S3;
@@ -196,8 +193,8 @@ dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const
         stage_B(toff);
         cpa_commit(); // B'
         const long long site_tb = s3 + (long long)(t_begin == 0 ? Lt - 1 : t_begin - 1) * S3;
-        float u[18], p[24], h[12];
-        load_link<3, float, RECON>(links, site_tb, u);
+        T u[18], p[24], h[12];
+        load_link<3, T, RECON>(links, site_tb, u);
         load_spinor(in, site_tb, p);
         project<3, +1>(p, h);
         su3_dag_mul(u, h, chi_t);
@@ -213,17 +210,17 @@ dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const
         cpa_wait<2>();   // own spinor of slice t (earlier P) and group A of slice t have landed
         __syncthreads(); // (A) slice t complete for every thread
 
-        const float4 *pl = plane0 + cur * plane_sz;
-        float acc[24], psi[24], u[18];
-        lds_vecs<6>(pl, nt, tid, psi);
+        const Vec *pl = plane0 + cur * plane_sz;
+        T acc[24], psi[24], u[18];
+        lds_vecs<NCH>(pl, nt, tid, psi);
 #pragma unroll
-        for (int i = 0; i < 24; ++i) acc[i] = 0.f;
+        for (int i = 0; i < 24; ++i) acc[i] = (T)0;
         reconstruct_add<3, +1>(acc, chi_t); // backward t hop, product carried from the previous slice
 
         // ---- x: both hops through warp shuffles ----
-        lds_link<0, RECON>(lnk, nt, tid, u);
+        lds_link_at<0, RECON>(lnk, 0, nt, tid, u);
         {
-            float h[12], g[12], chi[12];
+            T h[12], g[12], chi[12];
             project<0, -1>(psi, h);
             shfl12(g, h, lane_r); // P-_x psi(x+1)
             su3_mul(u, g, chi);
@@ -234,19 +231,19 @@ dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const
             reconstruct_add<0, +1>(acc, g);
         }
         // ---- y ----
-        lds_link<1, RECON>(lnk, nt, tid, u);
+        lds_link_at<1, RECON>(lnk, 0, nt, tid, u);
         {
-            float pn[24], h[12], chi[12];
-            if (face_yf) lds_vecs<6>(fy, nt, tid, pn);
-            else lds_vecs<6>(pl, nt, slot_yf, pn);
+            T pn[24], h[12], chi[12];
+            if (face_yf) lds_vecs<NCH>(fy, nt, tid, pn);
+            else lds_vecs<NCH>(pl, nt, slot_yf, pn);
             hop_forward<1>(acc, u, pn);
             project<1, +1>(psi, h);
             su3_dag_mul(u, h, chi);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) xchg_y[c * nt + tid] = make_float4(chi[4 * c], chi[4 * c + 1], chi[4 * c + 2], chi[4 * c + 3]);
+            for (int c = 0; c < HCH; ++c) pack(xchg_y[c * nt + tid], &chi[c * CR]);
             if (face_yb) { // the site below is outside the tile: do its backward hop here
-                lds_face_link<1, RECON>(fly, nyb, rank_y, u);
-                lds_vecs<6>(fy, nt, tid, pn);
+                lds_link_at<1, RECON>(fly, FY::first, nyb, rank_y, u);
+                lds_vecs<NCH>(fy, nt, tid, pn);
                 hop_backward<1>(acc, u, pn);
             }
         }
@@ -254,28 +251,28 @@ dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const
         cpa_commit();
         cpa_wait<2>(); // group B of slice t (links z,t, z face) has landed
         // ---- z ----
-        lds_link<2, RECON>(lnk, nt, tid, u);
+        lds_link_at<2, RECON>(lnk, 0, nt, tid, u);
         {
-            float pn[24], h[12], chi[12];
-            if (face_zf) lds_vecs<6>(fz, nt, tid, pn);
-            else lds_vecs<6>(pl, nt, slot_zf, pn);
+            T pn[24], h[12], chi[12];
+            if (face_zf) lds_vecs<NCH>(fz, nt, tid, pn);
+            else lds_vecs<NCH>(pl, nt, slot_zf, pn);
             hop_forward<2>(acc, u, pn);
             project<2, +1>(psi, h);
             su3_dag_mul(u, h, chi);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) xchg_z[c * nt + tid] = make_float4(chi[4 * c], chi[4 * c + 1], chi[4 * c + 2], chi[4 * c + 3]);
+            for (int c = 0; c < HCH; ++c) pack(xchg_z[c * nt + tid], &chi[c * CR]);
             if (face_zb) {
-                lds_face_link<2, RECON>(flz, nzb, rank_z, u);
-                lds_vecs<6>(fz, nt, tid, pn);
+                lds_link_at<2, RECON>(flz, FZ::first, nzb, rank_z, u);
+                lds_vecs<NCH>(fz, nt, tid, pn);
                 hop_backward<2>(acc, u, pn);
             }
         }
         // ---- t: forward hop now, backward product for the next slice ----
-        lds_link<3, RECON>(lnk, nt, tid, u);
+        lds_link_at<3, RECON>(lnk, 0, nt, tid, u);
         cpa_wait<1>(); // own spinor of slice t+1 (this slice's P) has landed
         {
-            float pn[24], h[12];
-            lds_vecs<6>(plane0 + (cur ^ 1) * plane_sz, nt, tid, pn);
+            T pn[24], h[12];
+            lds_vecs<NCH>(plane0 + (cur ^ 1) * plane_sz, nt, tid, pn);
             hop_forward<3>(acc, u, pn);
             project<3, +1>(psi, h);
             su3_dag_mul(u, h, chi_t);
@@ -284,22 +281,22 @@ dslash_stage_kernel(float *__restrict__ out, const float *__restrict__ in, const
         cpa_commit();
         __syncthreads(); // (B) exchange buffers complete
         if (!face_yb) {
-            float chi[12];
-            lds_vecs<3>(xchg_y, nt, slot_yb, chi);
+            T chi[12];
+            lds_vecs<HCH>(xchg_y, nt, slot_yb, chi);
             reconstruct_add<1, +1>(acc, chi);
         }
         if (!face_zb) {
-            float chi[12];
-            lds_vecs<3>(xchg_z, nt, slot_zb, chi);
+            T chi[12];
+            lds_vecs<HCH>(xchg_z, nt, slot_zb, chi);
             reconstruct_add<2, +1>(acc, chi);
         }
         // fused diagonal (step a6) and store (a7)
 #pragma unroll
-        for (int i = 0; i < 24; ++i) psi[i] = fmaf(cdiag, psi[i], -0.5f * acc[i]);
+        for (int i = 0; i < 24; ++i) psi[i] = fma(cdiag, psi[i], (T)-0.5 * acc[i]);
         {
-            float4 *q = out_own + toff * 6;
+            Vec *q = out_own + toff * NCH;
 #pragma unroll
-            for (int c = 0; c < 6; ++c) q[c * BLK] = make_float4(psi[4 * c], psi[4 * c + 1], psi[4 * c + 2], psi[4 * c + 3]);
+            for (int c = 0; c < NCH; ++c) pack(q[c * BLK], &psi[c * CR]);
         }
         cur ^= 1;
     }
@@ -318,7 +315,6 @@ struct StageShape {
 bool stage_shape(const ApplyArgs &a, StageShape &s)
 {
     const int Lx = a.dims[0], Ly = a.dims[1], Lz = a.dims[2];
-    if (a.precision != 32) return false;
     if (Lx < 4 || Lx > 32 || (Lx & (Lx - 1))) return false;
     if (((long long)Lx * Ly * Lz) % BLK) return false;
     if (const char *e = getenv("WD_TILE_SHAPE")) {
@@ -346,11 +342,16 @@ bool stage_shape(const ApplyArgs &a, StageShape &s)
     return best > 0;
 }
 
-template <int RECON, int NT>
+template <typename T, int RECON> size_t stage_smem_bytes(const ApplyArgs &a, const StageShape &s)
+{
+    return (size_t)stage_smem_vecs<T, RECON>(s.nt, a.dims[0] * s.tz, a.dims[0] * s.ty) * 16;
+}
+
+template <typename T, int RECON, int NT>
 cudaError_t launch_stage_nt(const ApplyArgs &a, const StageShape &s)
 {
-    auto kern = dslash_stage_kernel<RECON, NT>;
-    const size_t smem = (size_t)stage_smem_vecs<RECON>(s.nt, a.dims[0] * s.tz, a.dims[0] * s.ty) * sizeof(float4);
+    auto kern = dslash_stage_kernel<T, RECON, NT>;
+    const size_t smem = stage_smem_bytes<T, RECON>(a, s);
     if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
     static size_t smem_set = 0;
     cudaError_t e;
@@ -358,9 +359,10 @@ cudaError_t launch_stage_nt(const ApplyArgs &a, const StageShape &s)
         if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
         smem_set = smem;
     }
-    // t-chunks of 8 slices (WD_TILE_TC / WD_TILE_NCHUNK override): the start of a march is the one place
-    // where this kernel waits for memory, so chunks are longer than in the tile kernel
-    int tc = 8;
+    // t-chunks of 16 slices (WD_TILE_TC / WD_TILE_NCHUNK override; measured 16 > 8 > 32 on 32^3 x 64 in both
+    // precisions): the start of a march is the one place where this kernel waits for memory, so chunks
+    // are longer than in the tile kernel
+    int tc = 16;
     if (const char *ev = getenv("WD_TILE_TC")) {
         const int v = atoi(ev);
         if (v >= 1) tc = v;
@@ -374,19 +376,19 @@ cudaError_t launch_stage_nt(const ApplyArgs &a, const StageShape &s)
     const long long ncol = (long long)(a.dims[1] / s.ty) * (a.dims[2] / s.tz);
     if (ncol * nchunk * a.nrhs > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     dim3 grid((unsigned)(ncol * nchunk * a.nrhs));
-    const float cdiag = (float)(4.0 + a.mass); // formed in double, rounded once (reading S8)
-    kern<<<grid, s.nt, smem, a.stream>>>((float *)a.out, (const float *)a.in, (const float *)a.links, a.dims[0], a.dims[1],
-                                          a.dims[2], a.dims[3], s.ty, s.tz, a.V, cdiag, a.nrhs, nchunk);
+    const T cdiag = (T)(4.0 + a.mass); // formed in double, rounded once (reading S8)
+    kern<<<grid, s.nt, smem, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)a.links, a.dims[0], a.dims[1], a.dims[2],
+                                          a.dims[3], s.ty, s.tz, a.V, cdiag, a.nrhs, nchunk);
     count_launch();
     return cudaGetLastError();
 }
 
-template <int RECON>
+template <typename T, int RECON>
 cudaError_t launch_stage_t(const ApplyArgs &a)
 {
     StageShape s;
     if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
-    return s.nt == 128 ? launch_stage_nt<RECON, 128>(a, s) : launch_stage_nt<RECON, 0>(a, s);
+    return s.nt == 128 ? launch_stage_nt<T, RECON, 128>(a, s) : launch_stage_nt<T, RECON, 0>(a, s);
 }
 
 } // namespace
@@ -394,19 +396,24 @@ cudaError_t launch_stage_t(const ApplyArgs &a)
 bool stage_supported(const ApplyArgs &a)
 {
     StageShape s;
-    return a.nrhs >= 1 && stage_shape(a, s);
+    if (a.nrhs < 1 || !stage_shape(a, s)) return false;
+    // the tile's staging area must fit the 227 KB of shared memory a CTA can have (fp64 needs twice fp32's)
+    const size_t smem = a.precision == 32 ? (a.recon == 18 ? stage_smem_bytes<float, 18>(a, s) : stage_smem_bytes<float, 12>(a, s))
+                                          : (a.recon == 18 ? stage_smem_bytes<double, 18>(a, s) : stage_smem_bytes<double, 12>(a, s));
+    return smem <= 227 * 1024;
 }
 
 cudaError_t launch_mrhs(const ApplyArgs &a, int ty, int tz); // wd_dslash_mrhs.cu
 
 cudaError_t launch_stage(const ApplyArgs &a)
 {
-    if (a.nrhs > 1 && !(getenv("WD_STAGE_NO_MRHS") && atoi(getenv("WD_STAGE_NO_MRHS")))) {
+    if (a.precision == 32 && a.nrhs > 1 && !(getenv("WD_STAGE_NO_MRHS") && atoi(getenv("WD_STAGE_NO_MRHS")))) {
         StageShape s; // several right-hand sides: the kernel that shares the staged links between them
         if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
         if (s.nt <= 128) return launch_mrhs(a, s.ty, s.tz); // (a forced bigger tile runs RHS by RHS below)
     }
-    return a.recon == 18 ? launch_stage_t<18>(a) : launch_stage_t<12>(a);
+    if (a.precision == 32) return a.recon == 18 ? launch_stage_t<float, 18>(a) : launch_stage_t<float, 12>(a);
+    return a.recon == 18 ? launch_stage_t<double, 18>(a) : launch_stage_t<double, 12>(a);
 }
 
 } // namespace wd

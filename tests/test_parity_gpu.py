@@ -113,9 +113,9 @@ STAGE_SHAPES = [(32, 4, 4, 4), (16, 8, 8, 6), (8, 4, 4, 12), (4, 8, 16, 5), (32,
 
 
 @pytest.mark.parametrize("dims", STAGE_SHAPES)
-@pytest.mark.parametrize("recon", [18, 12])
-def test_stage_kernel_shapes(oracle, dims, recon):
-    cfg = fields.Config("stage", dims, 32, "haar", recon, -0.3, 1, 15)
+@pytest.mark.parametrize("precision,recon", [(32, 18), (32, 12), (64, 18), (64, 12)])
+def test_stage_kernel_shapes(oracle, dims, precision, recon):
+    cfg = fields.Config("stage", dims, precision, "haar", recon, -0.3, 1, 15)
     check_config(oracle, cfg, "stage", nrhs=1)
     check_config(oracle, cfg, "stage", nrhs=3)
 
@@ -129,7 +129,7 @@ def test_stage_kernel_forced_tile_shapes_and_chunks(oracle, monkeypatch, shape, 
     check_config(oracle, cfg, "stage")
 
 
-@pytest.mark.parametrize("name", ["c1_16x32_fp32", "c3_32x64_fp32"])
+@pytest.mark.parametrize("name", ["c1_16x32_fp32", "c3_32x64_fp32", "c3_32x64_fp64"])
 def test_stage_kernel_baseline_configs(oracle, name):
     check_config(oracle, fields.CONFIGS[name], "stage")
 
@@ -161,9 +161,9 @@ def test_stage_kernel_nv20_and_batched_consistency(oracle):
     op.close()
 
 
-def test_stage_kernel_rejects_fp64_and_odd_lattices():
+def test_stage_kernel_rejects_lattices_it_cannot_tile():
     from paper_0912_2186_b200 import binding
-    for dims, precision in (((8, 4, 4, 4), 64), ((24, 4, 4, 4), 32), ((32, 3, 4, 4), 32)):
+    for dims, precision in (((24, 4, 4, 4), 64), ((24, 4, 4, 4), 32), ((32, 3, 4, 4), 32), ((4, 2, 2, 4), 32)):
         cfg = fields.Config("bad", dims, precision, "haar", 18, 0.1, 1, 3)
         U, _ = fields.make_fields(cfg)
         op = GpuOp(U, cfg.dims, precision, 18)
@@ -350,8 +350,8 @@ def test_apply_host_pipelined_path(oracle, monkeypatch, dims, precision, recon, 
 def test_auto_kernel_selection():
     """WD_KERNEL_AUTO resolves by lattice, precision and nrhs; a forced kernel is reported."""
     from paper_0912_2186_b200 import binding
-    cases = [((32, 16, 16, 32), 32, 1, "stage"), ((32, 16, 16, 32), 32, 24, "stage"), ((32, 16, 16, 32), 64, 1, "tile"),
-             ((32, 16, 16, 32), 64, 4, "site"), ((24, 24, 24, 32), 32, 1, "site"), ((8, 8, 8, 8), 32, 1, "site")]
+    cases = [((32, 16, 16, 32), 32, 1, "stage"), ((32, 16, 16, 32), 32, 24, "stage"), ((32, 16, 16, 32), 64, 1, "stage"),
+             ((32, 16, 16, 32), 64, 4, "stage"), ((24, 24, 24, 32), 32, 1, "site"), ((8, 8, 8, 8), 32, 1, "site")]
     for dims, precision, nrhs, want in cases:
         cfg = fields.Config("sel", dims, precision, "haar", 18, 0.1, 1, 5)
         U, _ = fields.make_fields(cfg)
