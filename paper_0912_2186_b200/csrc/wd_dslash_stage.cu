@@ -18,8 +18,10 @@
 //     hops);  waits: wait_group 2 at the top (P(t), A(t-1 issued) done), 2 before z, 1 before t.
 //
 // Registers are no longer held across memory latency, shared memory is: 840 B/site in fp32 (two CTAs
-// of 128 sites per SM), twice that in fp64 (one CTA of 128 sites per SM).  Requires ty, tz >= 2 (a thread has at most one face per direction), Lx a power
-// of two <= 32, Lx*Ly*Lz a multiple of 32.
+// of 128 sites per SM), twice that in fp64 (one CTA of 128 sites per SM).  Requires ty, tz >= 2 (a thread
+// has at most one face per direction), 4 <= Lx <= 32 (a tile spans the whole x extent; a power-of-two Lx
+// exchanges x neighbours by warp shuffles, any other Lx through shared memory), Lx*ty*tz and Lx*Ly*Lz
+// multiples of 32.
 #include <cstdio>
 #include <cstdlib>
 #define WD_USE_F32X2 // packed FFMA2 SU(3) products (wd_math.cuh)
@@ -78,9 +80,9 @@ __device__ __forceinline__ void shfl12(T (&dst)[12], const T (&src)[12], int src
 } // namespace
 
 // shared-memory 16-byte vectors of one CTA (see the kernel for the carve-up)
-template <typename T, int RECON> constexpr int stage_smem_vecs(int nt, int nyb, int nzb)
+template <typename T, int RECON> constexpr int stage_smem_vecs(int nt, int nyb, int nzb, bool xs)
 {
-    return nt * (2 * SpinorLayout<T>::NCH + 2 * (SpinorLayout<T>::NCH / 2) + LinkLayout<T, RECON>::NVEC +
+    return nt * (2 * SpinorLayout<T>::NCH + (xs ? 2 : 3) * (SpinorLayout<T>::NCH / 2) + LinkLayout<T, RECON>::NVEC +
                  2 * SpinorLayout<T>::NCH) +
            nyb * FaceLinkVecs<1, RECON, T>::n + nzb * FaceLinkVecs<2, RECON, T>::n;
 }
@@ -89,7 +91,10 @@ template <typename T, int RECON> constexpr int stage_smem_vecs(int nt, int nyb, 
 // sides of a t-chunk run back to back, so the chunk's links come from HBM once and then from L2.
 // NT: threads per CTA known at compile time (128, the default tile) or 0 = read blockDim.x; with a
 // constant NT every shared-memory slot is an immediate offset from one base register.
-template <typename T, int RECON, int NT>
+// XS: x hops by warp shuffles (Lx a power of two); otherwise (e.g. Lx = 24) x is handled like y and z
+// inside the tile -- forward hop from the slice buffer, backward product through an exchange buffer --
+// with the periodic wrap in the slot arithmetic (the tile always spans the whole x extent).
+template <typename T, int RECON, int NT, bool XS>
 __global__ void __launch_bounds__(NT ? NT : 256, 1)
 dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ links, int Lx, int Ly,
                     int Lz, int Lt, int ty, int tz, long long V, T cdiag, int nrhs, int nchunk)
@@ -114,6 +119,7 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
     Vec *fz = fy + NCH * nt;             // [NCH][nt]  out-of-tile z neighbour spinor
     Vec *fly = fz + NCH * nt;            // [FY::n][nyb]  U_y of the -y neighbour (yy == 0 threads)
     Vec *flz = fly + FY::n * nyb;        // [FZ::n][nzb]  U_z of the -z neighbour (zz == 0 threads)
+    Vec *xchg_x = flz + FZ::n * nzb;     // [HCH][nt]  U_x^dag P+_x psi, for the site at x+1 (only if !XS)
 
     const int ncy = Ly / ty;
     const int ncol = ncy * (Lz / tz);
@@ -123,12 +129,13 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
     in += (long long)rhs * 24 * padded_volume(V);
     out += (long long)rhs * 24 * padded_volume(V);
 
-    const int x = tid & (Lx - 1);
     const int row = tid / Lx;
+    const int x = tid - row * Lx;
     const int yy = row % ty, zz = row / ty;
     const int lane = tid & 31;
-    const int lane_r = (lane & ~(Lx - 1)) | ((lane + 1) & (Lx - 1));
+    const int lane_r = (lane & ~(Lx - 1)) | ((lane + 1) & (Lx - 1)); // XS only
     const int lane_l = (lane & ~(Lx - 1)) | ((lane - 1) & (Lx - 1));
+    const int slot_xf = tid + (x + 1 == Lx ? 1 - Lx : 1), slot_xb = tid + (x == 0 ? Lx - 1 : -1); // !XS only
     const int slot_yb = tid - Lx, slot_yf = tid + Lx;
     const int slot_zb = tid - Lx * ty, slot_zf = tid + Lx * ty;
     const bool face_yb = (yy == 0), face_yf = (yy == ty - 1), face_zb = (zz == 0), face_zf = (zz == tz - 1);
@@ -219,7 +226,7 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
 
         // ---- x: both hops through warp shuffles ----
         lds_link_at<0, RECON>(lnk, 0, nt, tid, u);
-        {
+        if (XS) {
             T h[12], g[12], chi[12];
             project<0, -1>(psi, h);
             shfl12(g, h, lane_r); // P-_x psi(x+1)
@@ -229,6 +236,14 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
             su3_dag_mul(u, h, chi); // U_x(x)^dag P+_x psi(x): belongs to x+1
             shfl12(g, chi, lane_l);
             reconstruct_add<0, +1>(acc, g);
+        } else {
+            T pn[24], h[12], chi[12];
+            lds_vecs<NCH>(pl, nt, slot_xf, pn);
+            hop_forward<0>(acc, u, pn);
+            project<0, +1>(psi, h);
+            su3_dag_mul(u, h, chi);
+#pragma unroll
+            for (int c = 0; c < HCH; ++c) pack(xchg_x[c * nt + tid], &chi[c * CR]);
         }
         // ---- y ----
         lds_link_at<1, RECON>(lnk, 0, nt, tid, u);
@@ -280,6 +295,11 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
         if (more) stage_B(toff_n); // slots of links z,t and the z face are free again
         cpa_commit();
         __syncthreads(); // (B) exchange buffers complete
+        if (!XS) {
+            T chi[12];
+            lds_vecs<HCH>(xchg_x, nt, slot_xb, chi);
+            reconstruct_add<0, +1>(acc, chi);
+        }
         if (!face_yb) {
             T chi[12];
             lds_vecs<HCH>(xchg_y, nt, slot_yb, chi);
@@ -315,7 +335,7 @@ struct StageShape {
 bool stage_shape(const ApplyArgs &a, StageShape &s)
 {
     const int Lx = a.dims[0], Ly = a.dims[1], Lz = a.dims[2];
-    if (Lx < 4 || Lx > 32 || (Lx & (Lx - 1))) return false;
+    if (Lx < 4 || Lx > 32) return false; // a tile spans the whole x extent; power-of-two Lx uses warp shuffles in x
     if (((long long)Lx * Ly * Lz) % BLK) return false;
     if (const char *e = getenv("WD_TILE_SHAPE")) {
         int ty = 0, tz = 0;
@@ -344,13 +364,14 @@ bool stage_shape(const ApplyArgs &a, StageShape &s)
 
 template <typename T, int RECON> size_t stage_smem_bytes(const ApplyArgs &a, const StageShape &s)
 {
-    return (size_t)stage_smem_vecs<T, RECON>(s.nt, a.dims[0] * s.tz, a.dims[0] * s.ty) * 16;
+    const bool xs = (a.dims[0] & (a.dims[0] - 1)) == 0;
+    return (size_t)stage_smem_vecs<T, RECON>(s.nt, a.dims[0] * s.tz, a.dims[0] * s.ty, xs) * 16;
 }
 
-template <typename T, int RECON, int NT>
+template <typename T, int RECON, int NT, bool XS>
 cudaError_t launch_stage_nt(const ApplyArgs &a, const StageShape &s)
 {
-    auto kern = dslash_stage_kernel<T, RECON, NT>;
+    auto kern = dslash_stage_kernel<T, RECON, NT, XS>;
     const size_t smem = stage_smem_bytes<T, RECON>(a, s);
     if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
     static size_t smem_set = 0;
@@ -388,7 +409,8 @@ cudaError_t launch_stage_t(const ApplyArgs &a)
 {
     StageShape s;
     if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
-    return s.nt == 128 ? launch_stage_nt<T, RECON, 128>(a, s) : launch_stage_nt<T, RECON, 0>(a, s);
+    if (a.dims[0] & (a.dims[0] - 1)) return launch_stage_nt<T, RECON, 0, false>(a, s);
+    return s.nt == 128 ? launch_stage_nt<T, RECON, 128, true>(a, s) : launch_stage_nt<T, RECON, 0, true>(a, s);
 }
 
 } // namespace
@@ -410,7 +432,8 @@ cudaError_t launch_stage(const ApplyArgs &a)
     if (a.precision == 32 && a.nrhs > 1 && !(getenv("WD_STAGE_NO_MRHS") && atoi(getenv("WD_STAGE_NO_MRHS")))) {
         StageShape s; // several right-hand sides: the kernel that shares the staged links between them
         if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
-        if (s.nt <= 128) return launch_mrhs(a, s.ty, s.tz); // (a forced bigger tile runs RHS by RHS below)
+        if (s.nt <= 128 && !(a.dims[0] & (a.dims[0] - 1)))
+            return launch_mrhs(a, s.ty, s.tz); // (a forced bigger tile or a non-power-of-two Lx runs RHS by RHS below)
     }
     if (a.precision == 32) return a.recon == 18 ? launch_stage_t<float, 18>(a) : launch_stage_t<float, 12>(a);
     return a.recon == 18 ? launch_stage_t<double, 18>(a) : launch_stage_t<double, 12>(a);

@@ -109,7 +109,9 @@ def test_tile_kernel_baseline_configs(oracle, name):
 
 # ---------------------------------------------------------------- the cp.async-staged tile kernel (fp32)
 STAGE_SHAPES = [(32, 4, 4, 4), (16, 8, 8, 6), (8, 4, 4, 12), (4, 8, 16, 5), (32, 8, 8, 3), (32, 2, 2, 2), (16, 2, 4, 1),
-                (32, 6, 10, 4), (8, 12, 4, 7)]
+                (32, 6, 10, 4), (8, 12, 4, 7),
+                # Lx not a power of two: x hops through shared memory instead of warp shuffles
+                (24, 4, 4, 6), (24, 6, 2, 3), (12, 8, 4, 5), (6, 8, 8, 4), (24, 2, 2, 2)]
 
 
 @pytest.mark.parametrize("dims", STAGE_SHAPES)
@@ -129,7 +131,7 @@ def test_stage_kernel_forced_tile_shapes_and_chunks(oracle, monkeypatch, shape, 
     check_config(oracle, cfg, "stage")
 
 
-@pytest.mark.parametrize("name", ["c1_16x32_fp32", "c3_32x64_fp32", "c3_32x64_fp64"])
+@pytest.mark.parametrize("name", ["c1_16x32_fp32", "c2_24x64_fp32_r12", "c3_32x64_fp32", "c3_32x64_fp64"])
 def test_stage_kernel_baseline_configs(oracle, name):
     check_config(oracle, fields.CONFIGS[name], "stage")
 
@@ -163,7 +165,7 @@ def test_stage_kernel_nv20_and_batched_consistency(oracle):
 
 def test_stage_kernel_rejects_lattices_it_cannot_tile():
     from paper_0912_2186_b200 import binding
-    for dims, precision in (((24, 4, 4, 4), 64), ((24, 4, 4, 4), 32), ((32, 3, 4, 4), 32), ((4, 2, 2, 4), 32)):
+    for dims, precision in (((20, 4, 4, 4), 64), ((36, 4, 4, 4), 32), ((32, 3, 4, 4), 32), ((4, 2, 2, 4), 32)):
         cfg = fields.Config("bad", dims, precision, "haar", 18, 0.1, 1, 3)
         U, _ = fields.make_fields(cfg)
         op = GpuOp(U, cfg.dims, precision, 18)
@@ -351,7 +353,7 @@ def test_auto_kernel_selection():
     """WD_KERNEL_AUTO resolves by lattice, precision and nrhs; a forced kernel is reported."""
     from paper_0912_2186_b200 import binding
     cases = [((32, 16, 16, 32), 32, 1, "stage"), ((32, 16, 16, 32), 32, 24, "stage"), ((32, 16, 16, 32), 64, 1, "stage"),
-             ((32, 16, 16, 32), 64, 4, "stage"), ((24, 24, 24, 32), 32, 1, "site"), ((8, 8, 8, 8), 32, 1, "site")]
+             ((32, 16, 16, 32), 64, 4, "stage"), ((24, 24, 24, 32), 32, 1, "stage"), ((24, 24, 24, 32), 32, 3, "stage"), ((20, 20, 20, 40), 32, 1, "site"), ((8, 8, 8, 8), 32, 1, "site")]
     for dims, precision, nrhs, want in cases:
         cfg = fields.Config("sel", dims, precision, "haar", 18, 0.1, 1, 5)
         U, _ = fields.make_fields(cfg)
