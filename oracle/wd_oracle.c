@@ -34,7 +34,9 @@
  * BOTH hops are accumulated; for L_mu = 1 both are self-hops.  Any L_mu >= 1 is accepted.
  *
  * Parity pins live in tests/test_oracle_pins.py (free-field closed form, gamma5-hermiticity,
- * gauge covariance, brute-force dense matrix, point source, translation covariance).
+ * gauge covariance, brute-force dense matrix, point source, translation covariance) and, for the
+ * red/black pieces at the end of this file, in tests/test_oracle_pins_evenodd.py (block
+ * decomposition of the pinned full operator, dense Schur complement, solve identity).
  * The paper prints no worked numeric example of D*psi, so the S1 choice (which projector
  * sits on the forward hop) is pinned only by BASELINE.json's convention + the point-source
  * test written from the displayed formula: "parity unpinned" for S1 alone.
@@ -215,4 +217,150 @@ int wdo_apply_range(double *out, const double *psi, const double *U, const int d
         }
     }
     return 0;
+}
+
+/*
+ * ---- red/black (even-odd) pieces: SURVEY.md 8(f) row f1; PAPER.md:126 ("red/black
+ * preconditioning"), PAPER.md:157 (the paper's GPU kernel is the even-odd matvec) ----
+ *
+ * Site parity p(x) = (x1+x2+x3+x4) mod 2.  With every extent even, all eight neighbours of a
+ * site have the opposite parity, so in the ordering (even sites, odd sites)
+ *
+ *        D = [ (4+m) 1     H_eo   ]        H_pq = hopping term of eq. (2.2) from parity q to parity p
+ *            [  H_oe     (4+m) 1  ]        (including its factor -1/2)
+ *
+ * wdo_hop_parity:  out(x) = (H psi)(x) = -1/2 sum_mu [ (1+sign*gamma_mu) U_mu(x) psi(x+mu)
+ *                                                    + (1-sign*gamma_mu) U_mu(x-mu)^dag psi(x-mu) ]
+ *                  for the sites x of parity `parity`; out(x) = 0 on the other sites.  psi is a
+ *                  full-lattice field; only its values on the opposite parity are read.
+ * wdo_schur:       the even-odd preconditioned operator on parity p (Schur complement of the
+ *                  opposite-parity block, whose diagonal block (4+m) 1 is a scalar for Wilson):
+ *                      Mhat psi_p = (4+m) psi_p - H_pq (4+m)^-1 H_qp psi_p ,   q = 1 - p
+ *                  psi's values on parity q are ignored; out is 0 there.
+ * Both are the definitions written out: same gamma tables, link loader and periodic indexing as
+ * wdo_apply above.  Extents must be even (return -2 otherwise: the block form above needs it).
+ */
+static int site_parity(const int x[4]) { return (x[0] + x[1] + x[2] + x[3]) & 1; }
+
+int wdo_hop_parity(double *out, const double *psi, const double *U, const int dims[4], int nrhs,
+                   int recon, int sign, int parity)
+{
+    if (!out || !psi || !U || !dims) return -1;
+    if (recon != 18 && recon != 12) return -1;
+    if (sign != 1 && sign != -1) return -1;
+    if (parity != 0 && parity != 1) return -1;
+    if (nrhs < 1) return -1;
+    for (int d = 0; d < 4; ++d) {
+        if (dims[d] < 1) return -1;
+        if (dims[d] % 2) return -2;
+    }
+    const int L[4] = {dims[0], dims[1], dims[2], dims[3]};
+    const size_t V = (size_t)L[0] * L[1] * L[2] * L[3];
+    cplx PF[4][4][4], PB[4][4][4];
+    for (int mu = 0; mu < 4; ++mu)
+        for (int i = 0; i < 4; ++i)
+            for (int j = 0; j < 4; ++j) {
+                cplx one = (i == j) ? 1.0 : 0.0;
+                PF[mu][i][j] = one + (double)sign * GAMMA[mu][i][j];
+                PB[mu][i][j] = one - (double)sign * GAMMA[mu][i][j];
+            }
+    for (int r = 0; r < nrhs; ++r) {
+        const double *psi_r = psi + (size_t)r * V * 24;
+        double *out_r = out + (size_t)r * V * 24;
+#pragma omp parallel for schedule(static)
+        for (long site = 0; site < (long)V; ++site) {
+            int x[4];
+            size_t rem = (size_t)site;
+            for (int d = 0; d < 4; ++d) {
+                x[d] = (int)(rem % (size_t)L[d]);
+                rem /= (size_t)L[d];
+            }
+            double *o = out_r + (size_t)site * 24;
+            if (site_parity(x) != parity) {
+                for (int i = 0; i < 24; ++i) o[i] = 0.0;
+                continue;
+            }
+            cplx acc[4][3];
+            for (int s = 0; s < 4; ++s)
+                for (int a = 0; a < 3; ++a) acc[s][a] = 0.0;
+            for (int mu = 0; mu < 4; ++mu) {
+                int xf[4] = {x[0], x[1], x[2], x[3]};
+                int xb[4] = {x[0], x[1], x[2], x[3]};
+                xf[mu] = (x[mu] + 1) % L[mu];
+                xb[mu] = (x[mu] - 1 + L[mu]) % L[mu];
+                size_t sf = (size_t)xf[0] + (size_t)L[0] * (xf[1] + (size_t)L[1] * (xf[2] + (size_t)L[2] * xf[3]));
+                size_t sb = (size_t)xb[0] + (size_t)L[0] * (xb[1] + (size_t)L[1] * (xb[2] + (size_t)L[2] * xb[3]));
+                cplx Uf[3][3], Ub[3][3], pf[4][3], pb[4][3], tf[4][3], tb[4][3];
+                load_link(Uf, U, recon, V, mu, (size_t)site); /* U_mu(x)      */
+                load_link(Ub, U, recon, V, mu, sb);           /* U_mu(x - mu) */
+                load_spinor(pf, psi_r, sf);                   /* psi(x + mu): opposite parity */
+                load_spinor(pb, psi_r, sb);                   /* psi(x - mu): opposite parity */
+                for (int s = 0; s < 4; ++s)
+                    for (int a = 0; a < 3; ++a) {
+                        cplx f = 0.0, b = 0.0;
+                        for (int c = 0; c < 3; ++c) {
+                            f += Uf[a][c] * pf[s][c];
+                            b += conj(Ub[c][a]) * pb[s][c];
+                        }
+                        tf[s][a] = f;
+                        tb[s][a] = b;
+                    }
+                for (int s = 0; s < 4; ++s)
+                    for (int a = 0; a < 3; ++a) {
+                        cplx v = 0.0;
+                        for (int s2 = 0; s2 < 4; ++s2)
+                            v += PF[mu][s][s2] * tf[s2][a] + PB[mu][s][s2] * tb[s2][a];
+                        acc[s][a] += v;
+                    }
+            }
+            for (int s = 0; s < 4; ++s)
+                for (int a = 0; a < 3; ++a) {
+                    cplx v = -0.5 * acc[s][a];
+                    o[(s * 3 + a) * 2] = creal(v);
+                    o[(s * 3 + a) * 2 + 1] = cimag(v);
+                }
+        }
+    }
+    return 0;
+}
+
+int wdo_schur(double *out, const double *psi, const double *U, const int dims[4], double mass,
+              int nrhs, int recon, int sign, int parity)
+{
+    if (!out || !psi || !U || !dims) return -1;
+    if (parity != 0 && parity != 1) return -1;
+    if (nrhs < 1) return -1;
+    for (int d = 0; d < 4; ++d)
+        if (dims[d] < 1) return -1;
+    if (4.0 + mass == 0.0) return -3; /* the diagonal block is not invertible */
+    const size_t n = (size_t)nrhs * dims[0] * dims[1] * dims[2] * dims[3] * 24;
+    double *t1 = (double *)malloc(n * sizeof(double)); /* H_qp psi_p          (parity q) */
+    double *t2 = (double *)malloc(n * sizeof(double)); /* H_pq (H_qp psi_p)   (parity p) */
+    if (!t1 || !t2) {
+        free(t1);
+        free(t2);
+        return -4;
+    }
+    int rc = wdo_hop_parity(t1, psi, U, dims, nrhs, recon, sign, 1 - parity);
+    if (rc == 0) rc = wdo_hop_parity(t2, t1, U, dims, nrhs, recon, sign, parity);
+    if (rc == 0) {
+        const int L[4] = {dims[0], dims[1], dims[2], dims[3]};
+        const size_t V = (size_t)L[0] * L[1] * L[2] * L[3];
+        const double a = 4.0 + mass;
+        for (int r = 0; r < nrhs; ++r)
+            for (size_t site = 0; site < V; ++site) {
+                int x[4];
+                size_t rem = site;
+                for (int d = 0; d < 4; ++d) {
+                    x[d] = (int)(rem % (size_t)L[d]);
+                    rem /= (size_t)L[d];
+                }
+                const size_t o = ((size_t)r * V + site) * 24;
+                for (int i = 0; i < 24; ++i)
+                    out[o + i] = site_parity(x) == parity ? a * psi[o + i] - t2[o + i] / a : 0.0;
+            }
+    }
+    free(t1);
+    free(t2);
+    return rc;
 }

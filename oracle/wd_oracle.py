@@ -43,6 +43,10 @@ def _load():
         lib.wdo_apply_range.argtypes = [dp, dp, dp, ip, ctypes.c_double, ctypes.c_int, ctypes.c_int,
                                         ctypes.c_int, ctypes.c_long, ctypes.c_long]
         lib.wdo_apply_range.restype = ctypes.c_int
+        lib.wdo_hop_parity.argtypes = [dp, dp, dp, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]
+        lib.wdo_hop_parity.restype = ctypes.c_int
+        lib.wdo_schur.argtypes = [dp, dp, dp, ip, ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]
+        lib.wdo_schur.restype = ctypes.c_int
         lib.wdo_gamma.argtypes = [ctypes.c_int, dp]
         lib.wdo_gamma.restype = None
         lib.wdo_num_threads.restype = ctypes.c_int
@@ -115,3 +119,28 @@ def apply_range(psi, U, dims, mass, site_begin, site_end, sign=-1):
         raise RuntimeError(f"wdo_apply_range failed rc={rc}")
     res = out.reshape(psi.shape[0], -1, 4, 3, 2)[:, site_begin:site_end].copy()
     return res[0] if squeeze else res
+
+
+def hop_parity(psi, U, dims, parity, sign=-1):
+    """Red/black hopping block: on the sites of `parity`,
+    out = -1/2 sum_mu [(1+sign g_mu) U psi(x+mu) + (1-sign g_mu) U^dag psi(x-mu)] read from the
+    opposite parity; 0 on the other sites.  Full-lattice canonical arrays; extents must be even."""
+    psi, U, recon, squeeze, d = _check(psi, U, dims)
+    out = np.empty_like(psi)
+    cd = (ctypes.c_int * 4)(*d)
+    rc = _load().wdo_hop_parity(_dptr(out), _dptr(psi), _dptr(U), cd, psi.shape[0], recon, int(sign), int(parity))
+    if rc != 0:
+        raise RuntimeError(f"wdo_hop_parity failed rc={rc}")
+    return out[0] if squeeze else out
+
+
+def schur(psi, U, dims, mass, parity, sign=-1):
+    """Even-odd preconditioned operator on `parity`: (4+m) psi_p - H_pq H_qp psi_p / (4+m); 0 elsewhere."""
+    psi, U, recon, squeeze, d = _check(psi, U, dims)
+    out = np.empty_like(psi)
+    cd = (ctypes.c_int * 4)(*d)
+    rc = _load().wdo_schur(_dptr(out), _dptr(psi), _dptr(U), cd, float(mass), psi.shape[0], recon, int(sign),
+                           int(parity))
+    if rc != 0:
+        raise RuntimeError(f"wdo_schur failed rc={rc}")
+    return out[0] if squeeze else out

@@ -6,8 +6,8 @@
 // spinor and every link enters an SM (almost) once:
 //
 //   * A CTA owns a tile  Lx x TY x TZ  of one time slice (one thread per site, a warp = x-rows)
-//     and MARCHES along t over a contiguous range of slices.  The grid is persistent: the
-//     ncol*Lt (tile, t) work items are split evenly over  #SM x occupancy  CTAs.
+//     and MARCHES along t over a chunk of slices.  Blocks are ordered (t-chunk, RHS group, tile
+//     column), so the resident CTAs march through the same slices together (face neighbours in L2).
 //   * t direction lives in registers: the thread that owns (x,y,z) at slice t loads U_t(x,t)
 //     once, uses it for the forward hop  U_t(t) P- psi(t+1)  and, one step later, for the backward
 //     hop into slice t+1,  U_t(t)^dag P+ psi(t)  (12 registers carried across the step).
