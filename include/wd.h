@@ -160,6 +160,32 @@ int wd_apply(void *out_native_dev, const void *in_native_dev, const wd_gauge *ga
 int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_gauge *gauge,
                   double mass, const int dims[4], int nrhs, int precision);
 
+/*
+ * ---- red/black (even-odd) blocks: PAPER.md:126 ("red/black preconditioning"), PAPER.md:157 (the paper's GPU
+ * kernel is the even-odd matvec); SURVEY.md 8(f) row f1.  Every extent must be even (WD_ERR_DIMS otherwise).
+ * Site parity p(x) = (x+y+z+t) mod 2; D = [ (4+m) 1, H_eo ; H_oe, (4+m) 1 ] with H_pq the hopping term of
+ * eq. (2.2) from parity q to parity p (factor -1/2 included).  A HALF FIELD holds the V/2 sites of one parity in
+ * the blocked native layout over the checkerboard index lex/2; wd_spinor_bytes_parity() is its size.
+ */
+size_t wd_spinor_bytes_parity(const wd_lattice *lat, int nrhs, int precision);
+
+/* CANONICAL full-lattice field (nrhs * V * 24 reals, DEVICE) -> native half field of `parity`, and back
+ * (unpack writes only the sites of `parity`; the other sites of the canonical buffer are left untouched). */
+int wd_pack_spinor_parity(const wd_lattice *lat, void *native_half_dev, const void *canonical_dev, int nrhs,
+                          int precision, int parity, void *stream);
+int wd_unpack_spinor_parity(const wd_lattice *lat, void *canonical_dev, const void *native_half_dev, int nrhs,
+                            int precision, int parity, void *stream);
+
+/* out_p = H_pq in_q : `out_half_dev` is a half field of parity `parity_out`, `in_half_dev` of the opposite
+ * parity; one kernel launch on the gauge's stream.  Buffers 16-byte aligned, no overlap. */
+int wd_apply_hop(void *out_half_dev, const void *in_half_dev, const wd_gauge *gauge, const int dims[4], int nrhs,
+                 int precision, int parity_out);
+
+/* Even-odd preconditioned operator on `parity`:  out = (4+mass) in - H_pq (4+mass)^-1 H_qp in  (two launches;
+ * `tmp_half_dev` is a caller-owned half field that receives H_qp in).  mass != -4. */
+int wd_apply_schur(void *out_half_dev, const void *in_half_dev, void *tmp_half_dev, const wd_gauge *gauge, double mass,
+                   const int dims[4], int nrhs, int precision, int parity);
+
 /* Number of CUDA kernels the library has launched in this process (all handles). */
 long long wd_launch_count(void);
 

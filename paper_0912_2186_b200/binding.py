@@ -23,7 +23,8 @@ STATUS_NAMES = {
 # every symbol include/wd.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
-    "wd_set_kernel", "wd_selected_kernel", "wd_spinor_bytes", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
+    "wd_set_kernel", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
+    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
     "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
 )
 
@@ -60,6 +61,12 @@ def lib():
     L.wd_unpack_spinor.argtypes = [vp, vp, vp, i, i, vp]
     L.wd_apply.argtypes = [vp, vp, vp, d, ip, i, i]
     L.wd_apply_host.argtypes = [vp, vp, vp, d, ip, i, i]
+    L.wd_spinor_bytes_parity.argtypes = [vp, i, i]
+    L.wd_spinor_bytes_parity.restype = ctypes.c_size_t
+    L.wd_pack_spinor_parity.argtypes = [vp, vp, vp, i, i, i, vp]
+    L.wd_unpack_spinor_parity.argtypes = [vp, vp, vp, i, i, i, vp]
+    L.wd_apply_hop.argtypes = [vp, vp, vp, ip, i, i, i]
+    L.wd_apply_schur.argtypes = [vp, vp, vp, vp, d, ip, i, i, i]
     L.wd_launch_count.argtypes = []
     L.wd_launch_count.restype = ctypes.c_longlong
     L.wd_last_error.argtypes = []
@@ -69,7 +76,8 @@ def lib():
     L.wd_destroy.argtypes = [vp]
     L.wd_destroy.restype = None
     for name in ("wd_create_lattice", "wd_lattice_dims", "wd_load_gauge", "wd_set_stream", "wd_set_kernel",
-                 "wd_selected_kernel", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host"):
+                 "wd_selected_kernel", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
+                 "wd_pack_spinor_parity", "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur"):
         getattr(L, name).restype = i
     _lib = L
     return L
@@ -172,6 +180,30 @@ def wd_apply_host(out_canonical_host, in_canonical_host, gauge, mass, dims, nrhs
                                int(nrhs), int(precision)), "wd_apply_host")
 
 
+def wd_spinor_bytes_parity(lat, nrhs, precision):
+    return int(lib().wd_spinor_bytes_parity(lat, int(nrhs), int(precision)))
+
+
+def wd_pack_spinor_parity(lat, native_half_dev, canonical_dev, nrhs, precision, parity, stream=None):
+    _check(lib().wd_pack_spinor_parity(lat, _ptr(native_half_dev), _ptr(canonical_dev), int(nrhs), int(precision),
+                                       int(parity), _ptr(stream)), "wd_pack_spinor_parity")
+
+
+def wd_unpack_spinor_parity(lat, canonical_dev, native_half_dev, nrhs, precision, parity, stream=None):
+    _check(lib().wd_unpack_spinor_parity(lat, _ptr(canonical_dev), _ptr(native_half_dev), int(nrhs), int(precision),
+                                         int(parity), _ptr(stream)), "wd_unpack_spinor_parity")
+
+
+def wd_apply_hop(out_half_dev, in_half_dev, gauge, dims, nrhs, precision, parity_out):
+    _check(lib().wd_apply_hop(_ptr(out_half_dev), _ptr(in_half_dev), gauge, _dims(dims), int(nrhs), int(precision),
+                              int(parity_out)), "wd_apply_hop")
+
+
+def wd_apply_schur(out_half_dev, in_half_dev, tmp_half_dev, gauge, mass, dims, nrhs, precision, parity):
+    _check(lib().wd_apply_schur(_ptr(out_half_dev), _ptr(in_half_dev), _ptr(tmp_half_dev), gauge, float(mass),
+                                _dims(dims), int(nrhs), int(precision), int(parity)), "wd_apply_schur")
+
+
 def wd_destroy_gauge(gauge):
     lib().wd_destroy_gauge(gauge)
 
@@ -222,6 +254,24 @@ class WilsonDirac:
 
     def apply(self, out_native_dev, in_native_dev, mass, nrhs=1):
         wd_apply(out_native_dev, in_native_dev, self.gauge, mass, self.dims, nrhs, self.precision)
+
+    # ---- red/black (even-odd) blocks: half fields of one parity ----
+    def half_numel(self, nrhs=1):
+        """Reals in a native HALF field (one parity) of nrhs right-hand sides; 0 if an extent is odd."""
+        return wd_spinor_bytes_parity(self.lat, nrhs, self.precision) // (4 if self.precision == 32 else 8)
+
+    def pack_parity(self, native_half_dev, canonical_dev, nrhs, parity, stream=None):
+        wd_pack_spinor_parity(self.lat, native_half_dev, canonical_dev, nrhs, self.precision, parity, stream or self.stream)
+
+    def unpack_parity(self, canonical_dev, native_half_dev, nrhs, parity, stream=None):
+        wd_unpack_spinor_parity(self.lat, canonical_dev, native_half_dev, nrhs, self.precision, parity,
+                                stream or self.stream)
+
+    def apply_hop(self, out_half_dev, in_half_dev, parity_out, nrhs=1):
+        wd_apply_hop(out_half_dev, in_half_dev, self.gauge, self.dims, nrhs, self.precision, parity_out)
+
+    def apply_schur(self, out_half_dev, in_half_dev, tmp_half_dev, mass, parity, nrhs=1):
+        wd_apply_schur(out_half_dev, in_half_dev, tmp_half_dev, self.gauge, mass, self.dims, nrhs, self.precision, parity)
 
     def apply_host(self, out_canonical_host, in_canonical_host, mass, nrhs=1):
         wd_apply_host(out_canonical_host, in_canonical_host, self.gauge, mass, self.dims, nrhs, self.precision)

@@ -394,6 +394,106 @@ int wd_selected_kernel(const wd_gauge *gauge, int nrhs)
     return auto_kernel(shape_args(gauge, nrhs));
 }
 
+// ---- red/black blocks ----------------------------------------------------------------------------
+static bool all_even(const int dims[4])
+{
+    for (int d = 0; d < 4; ++d)
+        if (dims[d] % 2) return false;
+    return true;
+}
+
+static size_t half_bytes(long long V, int nrhs, int precision)
+{
+    return (size_t)nrhs * (size_t)wd::padded_volume(V / 2) * 24 * (precision == WD_FP32 ? 4 : 8);
+}
+
+size_t wd_spinor_bytes_parity(const wd_lattice *lat, int nrhs, int precision)
+{
+    if (!lat || lat->magic != LATTICE_MAGIC || nrhs < 1 || !valid_precision(precision) || !all_even(lat->dims)) return 0;
+    return half_bytes(lat->V, nrhs, precision);
+}
+
+static int parity_copy(const char *who, const wd_lattice *lat, void *native, void *canon, int nrhs, int precision,
+                       int parity, bool to_native, void *stream)
+{
+    if (!lat || !native || !canon) return fail(WD_ERR_NULL, "%s: NULL argument", who);
+    if (lat->magic != LATTICE_MAGIC) return fail(WD_ERR_MISMATCH, "%s: not a live wd_lattice handle", who);
+    if (!valid_precision(precision)) return fail(WD_ERR_PRECISION, "%s: precision %d is not 32 or 64", who, precision);
+    if (nrhs < 1) return fail(WD_ERR_NRHS, "%s: nrhs=%d", who, nrhs);
+    if (!all_even(lat->dims)) return fail(WD_ERR_DIMS, "%s: red/black fields need even extents", who);
+    if (parity != 0 && parity != 1) return fail(WD_ERR_MISMATCH, "%s: parity %d is not 0 or 1", who, parity);
+    const size_t cbytes = (size_t)nrhs * (size_t)lat->V * 24 * (precision == WD_FP32 ? 4 : 8);
+    if (overlap(native, half_bytes(lat->V, nrhs, precision), canon, cbytes)) return fail(WD_ERR_ALIAS, "%s: buffers overlap", who);
+    cudaError_t e = wd::launch_parity_copy(native, canon, lat->dims, lat->V, nrhs, precision, parity, to_native,
+                                           (cudaStream_t)stream);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, who);
+}
+
+int wd_pack_spinor_parity(const wd_lattice *lat, void *native_half_dev, const void *canonical_dev, int nrhs, int precision,
+                          int parity, void *stream)
+{
+    return parity_copy("wd_pack_spinor_parity", lat, native_half_dev, const_cast<void *>(canonical_dev), nrhs, precision,
+                       parity, true, stream);
+}
+
+int wd_unpack_spinor_parity(const wd_lattice *lat, void *canonical_dev, const void *native_half_dev, int nrhs,
+                            int precision, int parity, void *stream)
+{
+    return parity_copy("wd_unpack_spinor_parity", lat, const_cast<void *>(native_half_dev), canonical_dev, nrhs, precision,
+                       parity, false, stream);
+}
+
+static int check_eo_args(const char *who, const void *out, const void *in, const wd_gauge *g, const int dims[4], int nrhs,
+                         int precision, int parity)
+{
+    int rc = check_apply_args(out, in, g, dims, nrhs, precision);
+    if (rc) return rc;
+    if (!all_even(g->dims)) return fail(WD_ERR_DIMS, "%s: red/black blocks need even extents", who);
+    if (parity != 0 && parity != 1) return fail(WD_ERR_MISMATCH, "%s: parity %d is not 0 or 1", who, parity);
+    const size_t hb = half_bytes(g->V, nrhs, precision);
+    if (overlap(out, hb, in, hb)) return fail(WD_ERR_ALIAS, "%s: out and in overlap", who);
+    if (((uintptr_t)out | (uintptr_t)in) & 15) return fail(WD_ERR_MISMATCH, "%s: buffers must be 16-byte aligned", who);
+    return WD_OK;
+}
+
+int wd_apply_hop(void *out_half_dev, const void *in_half_dev, const wd_gauge *gauge, const int dims[4], int nrhs,
+                 int precision, int parity_out)
+{
+    int rc = check_eo_args("wd_apply_hop", out_half_dev, in_half_dev, gauge, dims, nrhs, precision, parity_out);
+    if (rc) return rc;
+    wd::ApplyArgs a = shape_args(gauge, nrhs);
+    a.out = out_half_dev;
+    a.in = in_half_dev;
+    a.links = gauge->links;
+    a.stream = gauge->stream;
+    cudaError_t e = wd::launch_eo(a, nullptr, 0.0, -0.5, parity_out);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply_hop: kernel launch");
+}
+
+int wd_apply_schur(void *out_half_dev, const void *in_half_dev, void *tmp_half_dev, const wd_gauge *gauge, double mass,
+                   const int dims[4], int nrhs, int precision, int parity)
+{
+    int rc = check_eo_args("wd_apply_schur", out_half_dev, in_half_dev, gauge, dims, nrhs, precision, parity);
+    if (rc) return rc;
+    if (!tmp_half_dev) return fail(WD_ERR_NULL, "wd_apply_schur: NULL tmp");
+    const size_t hb = half_bytes(gauge->V, nrhs, precision);
+    if (overlap(tmp_half_dev, hb, in_half_dev, hb) || overlap(tmp_half_dev, hb, out_half_dev, hb) || ((uintptr_t)tmp_half_dev & 15))
+        return fail(WD_ERR_ALIAS, "wd_apply_schur: tmp overlaps out or in, or is not 16-byte aligned");
+    const double a0 = 4.0 + mass;
+    if (a0 == 0.0) return fail(WD_ERR_MISMATCH, "wd_apply_schur: 4 + mass = 0, the diagonal block is not invertible");
+    wd::ApplyArgs a = shape_args(gauge, nrhs);
+    a.links = gauge->links;
+    a.stream = gauge->stream;
+    a.out = tmp_half_dev; // tmp_q = H_qp in_p
+    a.in = in_half_dev;
+    cudaError_t e = wd::launch_eo(a, nullptr, 0.0, -0.5, 1 - parity);
+    if (e != cudaSuccess) return cuda_fail(e, "wd_apply_schur: kernel launch");
+    a.out = out_half_dev; // out_p = (4+m) in_p - H_pq tmp_q / (4+m) = (4+m) in_p + hops(tmp_q) / (2 (4+m))
+    a.in = tmp_half_dev;
+    e = wd::launch_eo(a, in_half_dev, a0, 0.5 / a0, parity);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply_schur: kernel launch");
+}
+
 long long wd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 const char *wd_last_error(void) { return g_err; }

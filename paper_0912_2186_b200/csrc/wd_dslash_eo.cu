@@ -1,0 +1,146 @@
+// wd_dslash_eo.cu -- red/black (even-odd) hopping blocks of the Wilson-Dirac operator (first cut).
+//
+// SURVEY.md 8(f) row f1; PAPER.md:126 ("red/black preconditioning"), PAPER.md:157 (the paper's own GPU
+// kernel is the even-odd matvec).  Site parity p(x) = (x+y+z+t) mod 2; with every extent even
+//     D = [ (4+m) 1    H_eo   ]     H_pq = hopping term of eq. (2.2) from parity q to parity p, factor -1/2 included
+//         [  H_oe    (4+m) 1  ]
+// One kernel:   out_p = alpha * x_p + beta * sum_mu [ (1-g_mu) U_mu(x) in_q(x+mu) + (1+g_mu) U_mu(x-mu)^dag in_q(x-mu) ]
+// which gives H_pq (alpha = 0, beta = -1/2) and, in two launches, the even-odd preconditioned operator
+//     Mhat psi_p = (4+m) psi_p - H_pq (4+m)^-1 H_qp psi_p          (second launch: alpha = 4+m, beta = 1/(2(4+m))).
+//
+// Fields of one parity ("half fields") use the blocked native spinor layout of wd_layout.cuh over the
+// checkerboard index  cb = lex / 2  (lex = x + Lx*(y + Ly*(z + Lz*t)), Lx even), Vh = V/2 sites.  The links
+// are the gauge handle's ordinary full-lattice native links, indexed by lex.  One thread per output site,
+// neighbours straight from global memory (the structure of WD_KERNEL_SITE): every link of the lattice is
+// used exactly once per launch (forward at parity p, daggered at parity q), every input spinor eight times.
+#include "wd_internal.h"
+#include "wd_layout.cuh"
+#include "wd_math.cuh"
+#include "wd_link.cuh"
+
+namespace wd {
+
+constexpr int EO_THREADS = 128;
+
+template <typename T, int RECON>
+__global__ void __launch_bounds__(EO_THREADS)
+dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ xin, const T *__restrict__ links,
+                 int Lx, int Ly, int Lz, int Lt, long long Vh, T alpha, T beta, int parity)
+{
+    const long long cb = (long long)blockIdx.x * EO_THREADS + threadIdx.x;
+    if (cb >= Vh) return;
+    const long long Vhp = padded_volume(Vh); // sites per right-hand side of a half field
+    in += (long long)blockIdx.y * 24 * Vhp;
+    out += (long long)blockIdx.y * 24 * Vhp;
+
+    const int Lxh = Lx / 2;
+    long long rem = cb;
+    const int xh = (int)(rem % Lxh); rem /= Lxh;
+    const int y = (int)(rem % Ly); rem /= Ly;
+    const int z = (int)(rem % Lz);
+    const int t = (int)(rem / Lz);
+    const int x = 2 * xh + ((y + z + t + parity) & 1);
+    const long long sy = Lx, sz = (long long)Lx * Ly, st = (long long)Lx * Ly * Lz;
+    const long long site = x + sy * y + sz * z + st * t; // full-lattice index (links)
+    const long long xf = site + (x + 1 == Lx ? -(long long)(Lx - 1) : 1), xb = site + (x == 0 ? (long long)(Lx - 1) : -1);
+    const long long yf = site + (y + 1 == Ly ? -(Ly - 1) * sy : sy), yb = site + (y == 0 ? (Ly - 1) * sy : -sy);
+    const long long zf = site + (z + 1 == Lz ? -(Lz - 1) * sz : sz), zb = site + (z == 0 ? (Lz - 1) * sz : -sz);
+    const long long tf = site + (t + 1 == Lt ? -(Lt - 1) * st : st), tb = site + (t == 0 ? (Lt - 1) * st : -st);
+
+    T acc[24];
+#pragma unroll
+    for (int i = 0; i < 24; ++i) acc[i] = (T)0;
+    T u[18], p[24];
+    // neighbours have the opposite parity; their half-field index is lex / 2
+    load_link<0, T, RECON>(links, site, u); load_spinor(in, xf >> 1, p); hop_forward<0>(acc, u, p);
+    load_link<0, T, RECON>(links, xb, u);   load_spinor(in, xb >> 1, p); hop_backward<0>(acc, u, p);
+    load_link<1, T, RECON>(links, site, u); load_spinor(in, yf >> 1, p); hop_forward<1>(acc, u, p);
+    load_link<1, T, RECON>(links, yb, u);   load_spinor(in, yb >> 1, p); hop_backward<1>(acc, u, p);
+    load_link<2, T, RECON>(links, site, u); load_spinor(in, zf >> 1, p); hop_forward<2>(acc, u, p);
+    load_link<2, T, RECON>(links, zb, u);   load_spinor(in, zb >> 1, p); hop_backward<2>(acc, u, p);
+    load_link<3, T, RECON>(links, site, u); load_spinor(in, tf >> 1, p); hop_forward<3>(acc, u, p);
+    load_link<3, T, RECON>(links, tb, u);   load_spinor(in, tb >> 1, p); hop_backward<3>(acc, u, p);
+
+    if (xin) {
+        load_spinor(xin + (long long)blockIdx.y * 24 * Vhp, cb, p);
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] = fma(alpha, p[i], beta * acc[i]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] = beta * acc[i];
+    }
+    store_spinor(out, cb, acc);
+}
+
+template <typename T, int RECON>
+static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity)
+{
+    const long long Vh = a.V / 2;
+    const long long nb = (Vh + EO_THREADS - 1) / EO_THREADS;
+    if (nb > 0x7fffffffLL || a.nrhs > 65535) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)nb, (unsigned)a.nrhs);
+    dslash_eo_kernel<T, RECON><<<grid, EO_THREADS, 0, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)xin,
+                                                                   (const T *)a.links, a.dims[0], a.dims[1], a.dims[2],
+                                                                   a.dims[3], Vh, (T)alpha, (T)beta, parity);
+    count_launch();
+    return cudaGetLastError();
+}
+
+// out_p = alpha * xin_p + beta * (sum of the eight projected, link-multiplied hops from parity 1-p); xin may be NULL
+cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity)
+{
+    if (a.precision == 32)
+        return a.recon == 18 ? launch_eo_t<float, 18>(a, xin, alpha, beta, parity) : launch_eo_t<float, 12>(a, xin, alpha, beta, parity);
+    return a.recon == 18 ? launch_eo_t<double, 18>(a, xin, alpha, beta, parity) : launch_eo_t<double, 12>(a, xin, alpha, beta, parity);
+}
+
+// canonical full-lattice field <-> native half field of one parity (pure data movement)
+template <typename T, bool TO_NATIVE>
+__global__ void parity_copy_kernel(T *__restrict__ native, T *__restrict__ canon, int Lx, int Ly, int Lz, long long V,
+                                   int parity)
+{
+    using L = SpinorLayout<T>;
+    const long long Vh = V / 2, Vhp = padded_volume(Vh);
+    const long long cb = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= Vh) return;
+    const int Lxh = Lx / 2;
+    long long rem = cb;
+    const int xh = (int)(rem % Lxh); rem /= Lxh;
+    const int y = (int)(rem % Ly); rem /= Ly;
+    const int z = (int)(rem % Lz);
+    const long long t = rem / Lz;
+    const int x = 2 * xh + (int)((y + z + t + parity) & 1);
+    const long long site = x + (long long)Lx * (y + (long long)Ly * (z + (long long)Lz * t));
+    T *c = canon + ((long long)blockIdx.y * V + site) * 24;
+    typename L::Vec *q = reinterpret_cast<typename L::Vec *>(native + (long long)blockIdx.y * 24 * Vhp) +
+                         (cb >> 5) * (L::NCH * BLK) + (cb & (BLK - 1));
+#pragma unroll
+    for (int v = 0; v < L::NCH; ++v) {
+        if (TO_NATIVE) {
+            typename L::Vec w;
+            pack(w, c + v * L::CR);
+            q[v * BLK] = w;
+        } else {
+            unpack(q[v * BLK], c + v * L::CR);
+        }
+    }
+}
+
+cudaError_t launch_parity_copy(void *native, void *canon, const int dims[4], long long V, int nrhs, int precision,
+                               int parity, bool to_native, cudaStream_t s)
+{
+    const long long Vh = V / 2;
+    if (Vh <= 0 || nrhs <= 0) return cudaSuccess;
+    dim3 grid((unsigned)((Vh + 127) / 128), (unsigned)nrhs);
+    if (precision == 32) {
+        if (to_native) parity_copy_kernel<float, true><<<grid, 128, 0, s>>>((float *)native, (float *)canon, dims[0], dims[1], dims[2], V, parity);
+        else parity_copy_kernel<float, false><<<grid, 128, 0, s>>>((float *)native, (float *)canon, dims[0], dims[1], dims[2], V, parity);
+    } else {
+        if (to_native) parity_copy_kernel<double, true><<<grid, 128, 0, s>>>((double *)native, (double *)canon, dims[0], dims[1], dims[2], V, parity);
+        else parity_copy_kernel<double, false><<<grid, 128, 0, s>>>((double *)native, (double *)canon, dims[0], dims[1], dims[2], V, parity);
+    }
+    count_launch();
+    return cudaGetLastError();
+}
+
+} // namespace wd
