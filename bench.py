@@ -340,6 +340,79 @@ def run_wd(args):
     return line
 
 
+def run_schur(args):
+    """--op schur: the even-odd preconditioned operator on the same
+    lattice: a step = APPLIES wd_apply_schur calls (two kernel launches each) on half fields resident in HBM.
+    Flops per even site: 2 x 1320 (two hopping blocks) + 48; algorithmic bytes per even site: both launches
+    read every link once (2 x 4*recon*w x 2 sites); spinors: in, tmp written, tmp read, in again, out = 5 x 24*w."""
+    import torch
+    from paper_0912_2186_b200 import binding, build
+    rank, local, world = dist_env()
+    if world > 1:
+        raise SystemExit("bench.py --op schur: single GPU only")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    build.build()
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(local)
+    cfg = fields.CONFIGS[args.workload]
+    recon, nrhs = args.recon, cfg.nrhs
+    V = fields.volume(cfg.dims)
+    w = 4 if cfg.precision == 32 else 8
+    tdt = torch.float32 if cfg.precision == 32 else torch.float64
+    U, psi = fields.make_fields(rank_config(cfg, recon, nrhs, rank))
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        u_dev = torch.from_numpy(U).to(dev)
+        op = binding.WilsonDirac(cfg.dims, u_dev, cfg.precision, recon, stream=stream.cuda_stream)
+        canon = torch.from_numpy(psi).to(dev)
+        n = op.half_numel(nrhs)
+        ins = [torch.empty(n, dtype=tdt, device=dev) for _ in range(NBUF)]
+        outs = [torch.empty(n, dtype=tdt, device=dev) for _ in range(NBUF)]
+        tmp = torch.empty(n, dtype=tdt, device=dev)
+        op.pack_parity(ins[0], canon, nrhs, 0)
+        for b in range(1, NBUF):
+            torch.mul(ins[0], 1.0 + 0.25 * b, out=ins[b])
+    stream.synchronize()
+    aps = args.applies_per_step
+
+    def step():
+        for i in range(aps):
+            op.apply_schur(outs[i % NBUF], ins[i % NBUF], tmp, cfg.mass, 0, nrhs)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    n0 = binding.wd_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clocks:
+        ev0.record(stream)
+        for _ in range(args.steps):
+            step()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1)
+    applies = args.steps * aps
+    flops = (2 * 1320 + 48) * (V // 2) * nrhs
+    bytes_per_apply = (V // 2) * (2 * 2 * 4 * recon * w + nrhs * 5 * 24 * w)
+    peak, peak_src = measured_peak()
+    achieved = bytes_per_apply * applies / (ms * 1e-3) / 1e9
+    line = {"metric": "wilson_schur_gflops", "value": applies * flops / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if cfg.precision == 32 else "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "op": "even-odd preconditioned operator (2 launches per apply)",
+                       "dims": list(cfg.dims), "recon": recon, "nrhs": nrhs, "mass": cfg.mass, "applies_per_step": aps,
+                       "flops_per_even_site": 2 * 1320 + 48,
+                       "l2": "inputs larger than L2 (gauge + rotating half fields), no flush"},
+            "us_per_apply": ms / applies * 1e3, "clocks": clocks.summary(),
+            "gpu_launches": int(binding.wd_launch_count() - n0),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src, "bytes_per_launch": bytes_per_apply // 2,
+                         "kernel": "wd dslash_eo (site-style half-lattice kernel)"}}
+    print(json.dumps(line), flush=True)
+    op.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -349,6 +422,8 @@ def main():
     ap.add_argument("--kernel", default="auto", choices=["auto", "site", "tile", "stage"])
     ap.add_argument("--recon", type=int, default=None, choices=[18, 12])
     ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
+    ap.add_argument("--op", default="full", choices=["full", "schur"],
+                    help="full = D of eq. (2.2) (the headline); schur = even-odd preconditioned operator (row f1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--applies-per-step", type=int, default=APPLIES_PER_STEP,
                     help="wd_apply calls per step (default 100 = configs[3]; lower it only for profiling)")
@@ -357,6 +432,8 @@ def main():
         args.recon = fields.CONFIGS[args.workload].recon
     if args.impl == "reference":
         run_reference(args)
+    elif args.op == "schur":
+        run_schur(args)
     else:
         run_wd(args)
 
