@@ -186,6 +186,23 @@ int wd_apply_hop(void *out_half_dev, const void *in_half_dev, const wd_gauge *ga
 int wd_apply_schur(void *out_half_dev, const void *in_half_dev, void *tmp_half_dev, const wd_gauge *gauge, double mass,
                    const int dims[4], int nrhs, int precision, int parity);
 
+/* out = Mhat^dagger in  (= gamma5 Mhat gamma5): same calling convention as wd_apply_schur. */
+int wd_apply_schur_dagger(void *out_half_dev, const void *in_half_dev, void *tmp_half_dev, const wd_gauge *gauge,
+                          double mass, const int dims[4], int nrhs, int precision, int parity);
+
+/*
+ * wd_cgnr_schur -- conjugate gradients on the normal equations of the even-odd preconditioned operator
+ * ("CG on the normal equations"; CG around the even-odd matvec):
+ *     Mhat^dagger Mhat x = Mhat^dagger b,   x_0 = 0,   one right-hand side, half fields of `parity`.
+ * At most max_iter iterations; stops early when |b - Mhat x| <= tol * |b| (checked every 8 iterations; tol = 0
+ * runs exactly max_iter iterations with no host synchronisation inside the loop: all scalars stay on the device,
+ * reductions are deterministic fp64 sums).  *iters_out (may be NULL) receives the iterations done;
+ * hist_host (HOST, max_iter + 1 doubles, may be NULL) the relative residuals |r_k| / |b|, k = 0..iters.
+ * Workspace (five half fields) is allocated and freed inside the call; the call synchronises the gauge's stream.
+ */
+int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, const wd_gauge *gauge, double mass, const int dims[4],
+                  int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host);
+
 /* Number of CUDA kernels the library has launched in this process (all handles). */
 long long wd_launch_count(void);
 

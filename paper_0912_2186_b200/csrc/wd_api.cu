@@ -470,8 +470,8 @@ int wd_apply_hop(void *out_half_dev, const void *in_half_dev, const wd_gauge *ga
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply_hop: kernel launch");
 }
 
-int wd_apply_schur(void *out_half_dev, const void *in_half_dev, void *tmp_half_dev, const wd_gauge *gauge, double mass,
-                   const int dims[4], int nrhs, int precision, int parity)
+static int apply_schur(void *out_half_dev, const void *in_half_dev, void *tmp_half_dev, const wd_gauge *gauge, double mass,
+                       const int dims[4], int nrhs, int precision, int parity, bool dagger)
 {
     int rc = check_eo_args("wd_apply_schur", out_half_dev, in_half_dev, gauge, dims, nrhs, precision, parity);
     if (rc) return rc;
@@ -486,12 +486,41 @@ int wd_apply_schur(void *out_half_dev, const void *in_half_dev, void *tmp_half_d
     a.stream = gauge->stream;
     a.out = tmp_half_dev; // tmp_q = H_qp in_p
     a.in = in_half_dev;
-    cudaError_t e = wd::launch_eo(a, nullptr, 0.0, -0.5, 1 - parity);
+    cudaError_t e = wd::launch_eo(a, nullptr, 0.0, -0.5, 1 - parity, dagger);
     if (e != cudaSuccess) return cuda_fail(e, "wd_apply_schur: kernel launch");
     a.out = out_half_dev; // out_p = (4+m) in_p - H_pq tmp_q / (4+m) = (4+m) in_p + hops(tmp_q) / (2 (4+m))
     a.in = tmp_half_dev;
-    e = wd::launch_eo(a, in_half_dev, a0, 0.5 / a0, parity);
+    e = wd::launch_eo(a, in_half_dev, a0, 0.5 / a0, parity, dagger);
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply_schur: kernel launch");
+}
+
+int wd_apply_schur(void *out_half_dev, const void *in_half_dev, void *tmp_half_dev, const wd_gauge *gauge, double mass,
+                   const int dims[4], int nrhs, int precision, int parity)
+{
+    return apply_schur(out_half_dev, in_half_dev, tmp_half_dev, gauge, mass, dims, nrhs, precision, parity, false);
+}
+
+int wd_apply_schur_dagger(void *out_half_dev, const void *in_half_dev, void *tmp_half_dev, const wd_gauge *gauge,
+                          double mass, const int dims[4], int nrhs, int precision, int parity)
+{
+    return apply_schur(out_half_dev, in_half_dev, tmp_half_dev, gauge, mass, dims, nrhs, precision, parity, true);
+}
+
+int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, const wd_gauge *gauge, double mass, const int dims[4],
+                  int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host)
+{
+    int rc = check_eo_args("wd_cgnr_schur", x_half_dev, b_half_dev, gauge, dims, 1, precision, parity);
+    if (rc) return rc;
+    if (max_iter < 0 || tol < 0.0) return fail(WD_ERR_MISMATCH, "wd_cgnr_schur: max_iter=%d tol=%g", max_iter, tol);
+    if (4.0 + mass == 0.0) return fail(WD_ERR_MISMATCH, "wd_cgnr_schur: 4 + mass = 0");
+    wd::ApplyArgs a = shape_args(gauge, 1);
+    a.links = gauge->links;
+    a.stream = gauge->stream;
+    cudaError_t e = cudaSuccess;
+    if (wd::cgnr_schur(a, x_half_dev, b_half_dev, mass, parity, max_iter, tol, iters_out, hist_host, &e))
+        return e == cudaErrorMemoryAllocation ? fail(WD_ERR_ALLOC, "wd_cgnr_schur: workspace allocation failed")
+                                              : cuda_fail(e, "wd_cgnr_schur");
+    return WD_OK;
 }
 
 long long wd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }

@@ -1,0 +1,229 @@
+// wd_cg.cu -- Krylov shell around the even-odd matvec: CGNR for  Mhat x = b  on one parity (first cut).
+//
+// SURVEY.md 8(f) row f2; PAPER.md:116 ("CG on the normal equations"), PAPER.md:153-167 (CG built on the
+// even-odd matvec, Table 2).  Algorithm = oracle/wd_solvers.py:cgnr_schur, step for step:
+//     x = 0, r = b, z = Mhat^dag r, p = z, zz = <z,z>
+//     loop:  w = Mhat p;  alpha = zz/<w,w>;  x += alpha p;  r -= alpha w;  z = Mhat^dag r;
+//            zz' = <z,z>;  beta = zz'/zz;  p = z + beta p
+// B200 shape of it: the whole iteration is enqueued on the gauge's stream with NO host synchronisation -- every
+// scalar lives in device memory.  Reductions are deterministic two-level sums in fp64: each of RED_BLOCKS CTAs
+// writes one partial in a fixed order, and every CTA of the kernel that needs the scalar re-adds the partials
+// itself (a few hundred L2-resident doubles) instead of a separate finalise launch.  The host only reads the
+// residual history back every CHECK iterations when a tolerance is set.
+#include <cmath>
+#include <cstdio>
+#include "wd_internal.h"
+#include "wd_layout.cuh"
+
+namespace wd {
+
+namespace {
+
+constexpr int RED_BLOCKS = 592; // 4 CTAs of 256 threads per SM on 148 SMs
+constexpr int RED_THREADS = 256;
+
+__device__ __forceinline__ double sum_partials(const double *part)
+{
+    double s = 0.0;
+    for (int i = 0; i < RED_BLOCKS; ++i) s += part[i]; // fixed order: same bits in every CTA and every run
+    return s;
+}
+
+__device__ __forceinline__ double block_sum(double v, double *sh)
+{
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double s = 0.0;
+    if (threadIdx.x == 0)
+        for (int i = 0; i < RED_THREADS / 32; ++i) s += sh[i];
+    return s; // valid in thread 0
+}
+
+template <typename Vec> __device__ __forceinline__ double norm2_vec(const Vec &v);
+template <> __device__ __forceinline__ double norm2_vec<float4>(const float4 &v)
+{
+    return (double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z + (double)v.w * v.w;
+}
+template <> __device__ __forceinline__ double norm2_vec<double2>(const double2 &v) { return v.x * v.x + v.y * v.y; }
+
+__device__ __forceinline__ float4 axpy_vec(double a, const float4 &x, const float4 &y)
+{
+    const float f = (float)a;
+    return make_float4(fmaf(f, x.x, y.x), fmaf(f, x.y, y.y), fmaf(f, x.z, y.z), fmaf(f, x.w, y.w));
+}
+__device__ __forceinline__ double2 axpy_vec(double a, const double2 &x, const double2 &y)
+{
+    return make_double2(fma(a, x.x, y.x), fma(a, x.y, y.y));
+}
+
+// is vector index i (layout [block][vector][lane], NCH vectors per site) a real site (not a pad lane)?
+template <int NCH> __device__ __forceinline__ bool real_site(long long i, long long Vh)
+{
+    return (i / (NCH * BLK)) * BLK + (i % BLK) < Vh;
+}
+
+// part[b] = sum over this CTA's grid-stride share of |v|^2
+template <typename Vec, int NCH>
+__global__ void __launch_bounds__(RED_THREADS) norm2_kernel(const Vec *__restrict__ v, long long nvec, long long Vh, double *part)
+{
+    __shared__ double sh[RED_THREADS / 32];
+    double s = 0.0;
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS)
+        if (real_site<NCH>(i, Vh)) s += norm2_vec(v[i]);
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) part[blockIdx.x] = s;
+}
+
+// alpha = zz / ww;  x += alpha p;  r -= alpha w;  rr_part = |r|^2 partials
+template <typename Vec, int NCH>
+__global__ void __launch_bounds__(RED_THREADS)
+update_xr_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict__ p, const Vec *__restrict__ w, long long nvec,
+                 long long Vh, const double *zz_part, const double *ww_part, double *rr_part)
+{
+    __shared__ double sh[RED_THREADS / 32];
+    const double alpha = sum_partials(zz_part) / sum_partials(ww_part);
+    double s = 0.0;
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) {
+        x[i] = axpy_vec(alpha, p[i], x[i]);
+        const Vec rn = axpy_vec(-alpha, w[i], r[i]);
+        r[i] = rn;
+        if (real_site<NCH>(i, Vh)) s += norm2_vec(rn);
+    }
+    s = block_sum(s, sh);
+    if (threadIdx.x == 0) rr_part[blockIdx.x] = s;
+}
+
+// beta = zz_new / zz_old;  p = z + beta p;  hist[k] = sqrt(rr) (block 0)
+template <typename Vec>
+__global__ void __launch_bounds__(RED_THREADS)
+update_p_kernel(Vec *__restrict__ p, const Vec *__restrict__ z, long long nvec, const double *zz_new_part, const double *zz_old_part,
+                const double *rr_part, double *hist_k)
+{
+    const double beta = sum_partials(zz_new_part) / sum_partials(zz_old_part);
+    if (blockIdx.x == 0 && threadIdx.x == 0) *hist_k = sqrt(sum_partials(rr_part));
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS)
+        p[i] = axpy_vec(beta, p[i], z[i]);
+}
+
+template <typename Vec>
+__global__ void __launch_bounds__(RED_THREADS) zero_kernel(Vec *__restrict__ v, long long nvec)
+{
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) v[i] = Vec{};
+}
+
+__global__ void sqrt_of_sum_kernel(const double *part, double *out) { *out = sqrt(sum_partials(part)); }
+
+} // namespace
+
+template <typename T>
+static int cgnr_schur_t(const ApplyArgs &shape, void *x_out, const void *b_in, double mass, int parity, int max_iter,
+                        double tol, int *iters_out, double *hist_host, cudaError_t *err)
+{
+    using SL = SpinorLayout<T>;
+    using Vec = typename SL::Vec;
+    constexpr int NCH = SL::NCH;
+    constexpr int CHECK = 8; // iterations between convergence checks (the only host synchronisations)
+    const long long Vh = shape.V / 2;
+    const long long nvec = padded_volume(Vh) * NCH;
+    const size_t hb = (size_t)nvec * sizeof(Vec);
+    cudaStream_t s = shape.stream;
+    const double a0 = 4.0 + mass;
+
+    char *ws = nullptr;
+    double *sc = nullptr; // zz_part[2][RED] | ww_part | rr_part | hist[max_iter + 1]
+    const size_t nsc = 4 * (size_t)RED_BLOCKS + (size_t)max_iter + 1;
+    if ((*err = cudaMalloc(&ws, 5 * hb)) != cudaSuccess) return -1;
+    if ((*err = cudaMalloc(&sc, nsc * sizeof(double))) != cudaSuccess) {
+        cudaFree(ws);
+        return -1;
+    }
+    Vec *r = (Vec *)ws, *p = (Vec *)(ws + hb), *z = (Vec *)(ws + 2 * hb), *w = (Vec *)(ws + 3 * hb), *tmp = (Vec *)(ws + 4 * hb);
+    Vec *x = (Vec *)x_out;
+    double *zz_part[2] = {sc, sc + RED_BLOCKS}, *ww_part = sc + 2 * RED_BLOCKS, *rr_part = sc + 3 * RED_BLOCKS;
+    double *hist = sc + 4 * RED_BLOCKS;
+
+    ApplyArgs a = shape;
+    auto schur = [&](Vec *out, const Vec *in, bool dagger) -> cudaError_t { // out = Mhat in   or   Mhat^dagger in
+        a.out = tmp;
+        a.in = in;
+        cudaError_t e = launch_eo(a, nullptr, 0.0, -0.5, 1 - parity, dagger);
+        if (e != cudaSuccess) return e;
+        a.out = out;
+        a.in = tmp;
+        return launch_eo(a, in, a0, 0.5 / a0, parity, dagger);
+    };
+    auto norm2 = [&](const Vec *v, double *part) {
+        norm2_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(v, nvec, Vh, part);
+        count_launch();
+    };
+    int rc = 0, k = 0;
+    double h0 = 0.0;
+    auto fail_cuda = [&](cudaError_t e) {
+        *err = e;
+        rc = -1;
+    };
+    do {
+        cudaError_t e;
+        zero_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, nvec);
+        count_launch();
+        if ((e = cudaMemcpyAsync(r, b_in, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
+        if ((e = schur(z, r, true)) != cudaSuccess) { fail_cuda(e); break; }
+        if ((e = cudaMemcpyAsync(p, z, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
+        int cur = 0;
+        norm2(z, zz_part[cur]);
+        norm2(r, rr_part);
+        sqrt_of_sum_kernel<<<1, 1, 0, s>>>(rr_part, hist);
+        count_launch();
+        if (tol > 0.0) {
+            if ((e = cudaMemcpyAsync(&h0, hist, sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
+            if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
+            if (h0 == 0.0) break; // b = 0: x = 0 is the solution
+        }
+        for (k = 0; k < max_iter; ++k) {
+            if ((e = schur(w, p, false)) != cudaSuccess) { fail_cuda(e); break; }
+            norm2(w, ww_part);
+            update_xr_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, r, p, w, nvec, Vh, zz_part[cur], ww_part, rr_part);
+            count_launch();
+            if ((e = schur(z, r, true)) != cudaSuccess) { fail_cuda(e); break; }
+            norm2(z, zz_part[cur ^ 1]);
+            update_p_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(p, z, nvec, zz_part[cur ^ 1], zz_part[cur], rr_part, hist + k + 1);
+            count_launch();
+            cur ^= 1;
+            if (tol > 0.0 && ((k + 1) % CHECK == 0 || k + 1 == max_iter)) {
+                double hk = 0.0;
+                if ((e = cudaMemcpyAsync(&hk, hist + k + 1, sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
+                if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
+                if (hk <= tol * h0) {
+                    ++k;
+                    break;
+                }
+            }
+        }
+        if (rc) break;
+        if ((e = cudaGetLastError()) != cudaSuccess) { fail_cuda(e); break; }
+        if (hist_host) {
+            if ((e = cudaMemcpyAsync(hist_host, hist, ((size_t)k + 1) * sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
+        }
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
+        if (hist_host && hist_host[0] > 0.0) {
+            const double n0 = hist_host[0];
+            for (int i = 0; i <= k; ++i) hist_host[i] /= n0; // relative residual |r_k| / |b|
+        }
+    } while (false);
+    if (iters_out) *iters_out = k;
+    cudaFree(ws);
+    cudaFree(sc);
+    return rc;
+}
+
+// x = approximate solution of Mhat x = b on `parity` after at most max_iter CGNR iterations (tol = 0: exactly
+// max_iter, no host synchronisation inside the loop).  Returns 0, or -1 with *err set.
+int cgnr_schur(const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter, double tol,
+               int *iters_out, double *hist_host, cudaError_t *err)
+{
+    return shape.precision == 32 ? cgnr_schur_t<float>(shape, x, b, mass, parity, max_iter, tol, iters_out, hist_host, err)
+                                 : cgnr_schur_t<double>(shape, x, b, mass, parity, max_iter, tol, iters_out, hist_host, err);
+}
+
+} // namespace wd

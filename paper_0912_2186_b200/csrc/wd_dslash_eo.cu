@@ -22,7 +22,8 @@ namespace wd {
 
 constexpr int EO_THREADS = 128;
 
-template <typename T, int RECON>
+// SGN = -1: blocks of D; SGN = +1: blocks of gamma5 D gamma5 = D^dagger (all projectors swapped)
+template <typename T, int RECON, int SGN>
 __global__ void __launch_bounds__(EO_THREADS)
 dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ xin, const T *__restrict__ links,
                  int Lx, int Ly, int Lz, int Lt, long long Vh, T alpha, T beta, int parity)
@@ -52,14 +53,14 @@ dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restr
     for (int i = 0; i < 24; ++i) acc[i] = (T)0;
     T u[18], p[24];
     // neighbours have the opposite parity; their half-field index is lex / 2
-    load_link<0, T, RECON>(links, site, u); load_spinor(in, xf >> 1, p); hop_forward<0>(acc, u, p);
-    load_link<0, T, RECON>(links, xb, u);   load_spinor(in, xb >> 1, p); hop_backward<0>(acc, u, p);
-    load_link<1, T, RECON>(links, site, u); load_spinor(in, yf >> 1, p); hop_forward<1>(acc, u, p);
-    load_link<1, T, RECON>(links, yb, u);   load_spinor(in, yb >> 1, p); hop_backward<1>(acc, u, p);
-    load_link<2, T, RECON>(links, site, u); load_spinor(in, zf >> 1, p); hop_forward<2>(acc, u, p);
-    load_link<2, T, RECON>(links, zb, u);   load_spinor(in, zb >> 1, p); hop_backward<2>(acc, u, p);
-    load_link<3, T, RECON>(links, site, u); load_spinor(in, tf >> 1, p); hop_forward<3>(acc, u, p);
-    load_link<3, T, RECON>(links, tb, u);   load_spinor(in, tb >> 1, p); hop_backward<3>(acc, u, p);
+    load_link<0, T, RECON>(links, site, u); load_spinor(in, xf >> 1, p); hop_forward_s<0, SGN>(acc, u, p);
+    load_link<0, T, RECON>(links, xb, u);   load_spinor(in, xb >> 1, p); hop_backward_s<0, SGN>(acc, u, p);
+    load_link<1, T, RECON>(links, site, u); load_spinor(in, yf >> 1, p); hop_forward_s<1, SGN>(acc, u, p);
+    load_link<1, T, RECON>(links, yb, u);   load_spinor(in, yb >> 1, p); hop_backward_s<1, SGN>(acc, u, p);
+    load_link<2, T, RECON>(links, site, u); load_spinor(in, zf >> 1, p); hop_forward_s<2, SGN>(acc, u, p);
+    load_link<2, T, RECON>(links, zb, u);   load_spinor(in, zb >> 1, p); hop_backward_s<2, SGN>(acc, u, p);
+    load_link<3, T, RECON>(links, site, u); load_spinor(in, tf >> 1, p); hop_forward_s<3, SGN>(acc, u, p);
+    load_link<3, T, RECON>(links, tb, u);   load_spinor(in, tb >> 1, p); hop_backward_s<3, SGN>(acc, u, p);
 
     if (xin) {
         load_spinor(xin + (long long)blockIdx.y * 24 * Vhp, cb, p);
@@ -73,25 +74,27 @@ dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restr
 }
 
 template <typename T, int RECON>
-static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity)
+static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger)
 {
     const long long Vh = a.V / 2;
     const long long nb = (Vh + EO_THREADS - 1) / EO_THREADS;
     if (nb > 0x7fffffffLL || a.nrhs > 65535) return cudaErrorInvalidConfiguration;
     dim3 grid((unsigned)nb, (unsigned)a.nrhs);
-    dslash_eo_kernel<T, RECON><<<grid, EO_THREADS, 0, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)xin,
-                                                                   (const T *)a.links, a.dims[0], a.dims[1], a.dims[2],
-                                                                   a.dims[3], Vh, (T)alpha, (T)beta, parity);
+    auto kern = dagger ? dslash_eo_kernel<T, RECON, +1> : dslash_eo_kernel<T, RECON, -1>;
+    kern<<<grid, EO_THREADS, 0, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)xin, (const T *)a.links, a.dims[0],
+                                             a.dims[1], a.dims[2], a.dims[3], Vh, (T)alpha, (T)beta, parity);
     count_launch();
     return cudaGetLastError();
 }
 
 // out_p = alpha * xin_p + beta * (sum of the eight projected, link-multiplied hops from parity 1-p); xin may be NULL
-cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity)
+cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger)
 {
     if (a.precision == 32)
-        return a.recon == 18 ? launch_eo_t<float, 18>(a, xin, alpha, beta, parity) : launch_eo_t<float, 12>(a, xin, alpha, beta, parity);
-    return a.recon == 18 ? launch_eo_t<double, 18>(a, xin, alpha, beta, parity) : launch_eo_t<double, 12>(a, xin, alpha, beta, parity);
+        return a.recon == 18 ? launch_eo_t<float, 18>(a, xin, alpha, beta, parity, dagger)
+                             : launch_eo_t<float, 12>(a, xin, alpha, beta, parity, dagger);
+    return a.recon == 18 ? launch_eo_t<double, 18>(a, xin, alpha, beta, parity, dagger)
+                         : launch_eo_t<double, 12>(a, xin, alpha, beta, parity, dagger);
 }
 
 // canonical full-lattice field <-> native half field of one parity (pure data movement)

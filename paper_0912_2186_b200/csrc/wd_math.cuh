@@ -235,4 +235,24 @@ __device__ __forceinline__ void hop_backward(T (&acc)[24], const T (&u)[18], con
     reconstruct_add<MU, +1>(acc, chi);
 }
 
+// Hops with the projector sign as a parameter: SGN = -1 is D of eq. (2.2) (hop_forward / hop_backward above),
+// SGN = +1 is gamma5 D gamma5 = D^dagger, i.e. every projector 1 -+ gamma_mu swapped.
+template <int MU, int SGN, typename T>
+__device__ __forceinline__ void hop_forward_s(T (&acc)[24], const T (&u)[18], const T (&p)[24])
+{
+    T h[12], chi[12];
+    project<MU, SGN>(p, h);
+    su3_mul(u, h, chi);
+    reconstruct_add<MU, SGN>(acc, chi);
+}
+
+template <int MU, int SGN, typename T>
+__device__ __forceinline__ void hop_backward_s(T (&acc)[24], const T (&u)[18], const T (&p)[24])
+{
+    T h[12], chi[12];
+    project<MU, -SGN>(p, h);
+    su3_dag_mul(u, h, chi);
+    reconstruct_add<MU, -SGN>(acc, chi);
+}
+
 } // namespace wd

@@ -1,0 +1,94 @@
+"""-m gpu parity tests of the Krylov shell (wd_apply_schur_dagger, wd_cgnr_schur) against the oracle
+(oracle.schur sign=+1, oracle/wd_solvers.py:cgnr_schur), through the C ABI.  SURVEY.md 8(f) row f2.
+
+Tolerances: the operator keeps the north-star bounds (1e-13 / 2e-6).  CG is an iteration: after K steps in
+working precision eps the iterates of two correct implementations differ by O(K * kappa * eps); with the masses
+used here (well conditioned, kappa ~ 10) and K = 12: 1e-10 in fp64, 2e-4 in fp32 on x and on the residual history
+-- derived bounds, written here, far below any plausible algorithmic mistake (a wrong alpha/beta gives O(1))."""
+import numpy as np
+import pytest
+
+from paper_0912_2186_b200 import fields
+from oracle import wd_solvers
+from gpu_util import TOL, GpuOp, rel_l2
+from test_parity_gpu_evenodd import parity_mask
+
+pytestmark = pytest.mark.gpu
+
+
+def to_half(op, canon_np, parity):
+    import torch
+    w = op.op
+    canon = torch.from_numpy(np.ascontiguousarray(canon_np)).cuda()
+    h = torch.full((w.half_numel(1),), float("nan"), dtype=canon.dtype, device="cuda")
+    w.pack_parity(h, canon, 1, parity)
+    return h
+
+
+def from_half(op, h, shape, parity):
+    import torch
+    out = torch.zeros(shape, dtype=h.dtype, device="cuda")
+    op.op.unpack_parity(out, h, 1, parity)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 4, 6, 2), (16, 8, 8, 6)])
+@pytest.mark.parametrize("precision,recon", [(64, 18), (32, 18), (32, 12)])
+def test_schur_dagger_matches_the_oracle(oracle, dims, precision, recon):
+    import torch
+    cfg = fields.Config("sd", dims, precision, "haar", recon, -0.31, 1, 63)
+    U, psi = fields.make_fields(cfg)
+    Uo = (U if recon == 18 else np.ascontiguousarray(U[..., :2, :, :])).astype(np.float64)
+    op = GpuOp(U, dims, precision, recon)
+    for parity in (0, 1):
+        a = to_half(op, psi, parity)
+        b, tmp = torch.empty_like(a), torch.empty_like(a)
+        op.op.apply_schur_dagger(b, a, tmp, cfg.mass, parity, 1)
+        got = from_half(op, b, psi.shape, parity)
+        want = oracle.schur(psi.astype(np.float64), Uo, dims, cfg.mass, parity, sign=+1)
+        assert rel_l2(got[0], want[0]) <= TOL[precision]
+    op.close()
+
+
+@pytest.mark.parametrize("dims,parity", [((4, 4, 4, 4), 0), ((8, 4, 6, 2), 1), ((16, 8, 8, 8), 0), ((2, 6, 4, 2), 1)])
+@pytest.mark.parametrize("precision,recon,tol_x", [(64, 18, 1e-10), (64, 12, 1e-10), (32, 18, 2e-4), (32, 12, 2e-4)])
+def test_cgnr_fixed_iterations_match_the_oracle(oracle, dims, parity, precision, recon, tol_x):
+    import torch
+    K = 12
+    cfg = fields.Config("cg", dims, precision, "smooth", recon, 0.2, 1, 65)
+    U, b = fields.make_fields(cfg)
+    Uo = (U if recon == 18 else np.ascontiguousarray(U[..., :2, :, :])).astype(np.float64)
+    op = GpuOp(U, dims, precision, recon)
+    bh = to_half(op, b, parity)
+    xh = torch.full_like(bh, float("nan"))
+    iters, hist = op.op.cgnr_schur(xh, bh, cfg.mass, parity, K)
+    x = from_half(op, xh, b.shape, parity)[0]
+    # determinism: a second solve gives the same bits
+    xh2 = torch.full_like(bh, float("nan"))
+    op.op.cgnr_schur(xh2, bh, cfg.mass, parity, K)
+    x2 = from_half(op, xh2, b.shape, parity)[0]
+    op.close()
+    want_x, want_hist = wd_solvers.cgnr_schur(b[0].astype(np.float64), Uo, dims, cfg.mass, parity, K)
+    assert iters == K and len(hist) == K + 1
+    assert np.array_equal(x, x2)
+    assert np.all(x[np.broadcast_to(parity_mask(dims)[0] != parity, x.shape)] == 0)
+    assert rel_l2(x, want_x) <= tol_x
+    assert np.max(np.abs(np.array(hist) / want_hist - 1.0)) <= tol_x * 10
+
+
+def test_cgnr_converges_to_the_solution(oracle):
+    import torch
+    dims, parity = (8, 8, 8, 8), 0
+    cfg = fields.Config("cgc", dims, 64, "smooth", 18, 0.1, 1, 67)
+    U, b = fields.make_fields(cfg)
+    op = GpuOp(U, dims, 64, 18)
+    bh = to_half(op, b, parity)
+    xh = torch.empty_like(bh)
+    iters, hist = op.op.cgnr_schur(xh, bh, cfg.mass, parity, 500, tol=1e-11)
+    x = from_half(op, xh, b.shape, parity)
+    op.close()
+    assert iters < 500 and hist[-1] <= 1e-11 and hist[0] == pytest.approx(1.0)
+    bm = np.where(parity_mask(dims) == parity, b, 0.0)
+    res = bm - oracle.schur(x.astype(np.float64), U.astype(np.float64), dims, cfg.mass, parity)
+    assert np.linalg.norm(res) / np.linalg.norm(bm) <= 2e-11   # true residual, recomputed by the oracle
