@@ -413,6 +413,71 @@ def run_schur(args):
     op.close()
 
 
+def run_cgnr(args):
+    """--op cgnr: CGNR on the even-odd preconditioned operator (Table 2): a step =
+    one wd_cgnr_schur call of ITER iterations (tol = 0: no host synchronisation inside).  Per iteration and even
+    site: flops 2 x (2 x 1320 + 48) + 288 (norms, x/r/p updates); algorithmic bytes 2 x Schur apply + 11 spinor
+    passes of the BLAS-1 kernels."""
+    import torch
+    from paper_0912_2186_b200 import binding, build
+    rank, local, world = dist_env()
+    if world > 1:
+        raise SystemExit("bench.py --op cgnr: single GPU only")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    build.build()
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(local)
+    cfg = fields.CONFIGS[args.workload]
+    recon = args.recon
+    V = fields.volume(cfg.dims)
+    w = 4 if cfg.precision == 32 else 8
+    tdt = torch.float32 if cfg.precision == 32 else torch.float64
+    U, psi = fields.make_fields(rank_config(cfg, recon, 1, rank), nrhs=1)
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        u_dev = torch.from_numpy(U).to(dev)
+        op = binding.WilsonDirac(cfg.dims, u_dev, cfg.precision, recon, stream=stream.cuda_stream)
+        canon = torch.from_numpy(psi).to(dev)
+        n = op.half_numel(1)
+        b = torch.empty(n, dtype=tdt, device=dev)
+        x = torch.empty(n, dtype=tdt, device=dev)
+        op.pack_parity(b, canon, 1, 0)
+    stream.synchronize()
+    iters = args.applies_per_step
+    for _ in range(max(args.warmup, 3)):
+        op.cgnr_schur(x, b, cfg.mass, 0, iters)
+    torch.cuda.synchronize()
+    n0 = binding.wd_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clocks:
+        ev0.record(stream)
+        for _ in range(args.steps):
+            done, hist = op.cgnr_schur(x, b, cfg.mass, 0, iters)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1)
+    total_iters = args.steps * iters
+    flops_it = (2 * (2 * 1320 + 48) + 288) * (V // 2)
+    bytes_it = (V // 2) * (2 * (2 * 2 * 4 * recon * w + 5 * 24 * w) + 11 * 24 * w)
+    peak, peak_src = measured_peak()
+    achieved = bytes_it * total_iters / (ms * 1e-3) / 1e9
+    line = {"metric": "wilson_cgnr_gflops", "value": total_iters * flops_it / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if cfg.precision == 32 else "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "op": "CGNR on the even-odd preconditioned operator", "dims": list(cfg.dims),
+                       "recon": recon, "mass": cfg.mass, "iterations_per_step": iters,
+                       "relative_residual_after_step": hist[-1],
+                       "l2": "inputs larger than L2 (gauge + five half fields), no flush"},
+            "us_per_iteration": ms / total_iters * 1e3, "clocks": clocks.summary(),
+            "gpu_launches": int(binding.wd_launch_count() - n0),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src, "bytes_per_iteration": bytes_it,
+                         "kernel": "wd dslash_eo + fused BLAS-1"}}
+    print(json.dumps(line), flush=True)
+    op.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -422,8 +487,8 @@ def main():
     ap.add_argument("--kernel", default="auto", choices=["auto", "site", "tile", "stage"])
     ap.add_argument("--recon", type=int, default=None, choices=[18, 12])
     ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
-    ap.add_argument("--op", default="full", choices=["full", "schur"],
-                    help="full = D of eq. (2.2) (the headline); schur = even-odd preconditioned operator (row f1)")
+    ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr"],
+                    help="full = D of eq. (2.2) (the headline); schur = even-odd preconditioned operator (row f1); cgnr = CG on its normal equations (row f2, --applies-per-step = iterations)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--applies-per-step", type=int, default=APPLIES_PER_STEP,
                     help="wd_apply calls per step (default 100 = configs[3]; lower it only for profiling)")
@@ -434,6 +499,8 @@ def main():
         run_reference(args)
     elif args.op == "schur":
         run_schur(args)
+    elif args.op == "cgnr":
+        run_cgnr(args)
     else:
         run_wd(args)
 

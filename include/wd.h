@@ -198,9 +198,10 @@ int wd_apply_schur_dagger(void *out_half_dev, const void *in_half_dev, void *tmp
  * runs exactly max_iter iterations with no host synchronisation inside the loop: all scalars stay on the device,
  * reductions are deterministic fp64 sums).  *iters_out (may be NULL) receives the iterations done;
  * hist_host (HOST, max_iter + 1 doubles, may be NULL) the relative residuals |r_k| / |b|, k = 0..iters.
- * Workspace (five half fields) is allocated and freed inside the call; the call synchronises the gauge's stream.
+ * Workspace (five half fields) is owned by the gauge handle (allocated on first use, reused, released by
+ * wd_destroy_gauge; not re-entrant for one handle); the call synchronises the gauge's stream before returning.
  */
-int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, const wd_gauge *gauge, double mass, const int dims[4],
+int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4],
                   int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host);
 
 /* Number of CUDA kernels the library has launched in this process (all handles). */

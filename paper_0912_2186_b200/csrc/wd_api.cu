@@ -506,7 +506,7 @@ int wd_apply_schur_dagger(void *out_half_dev, const void *in_half_dev, void *tmp
     return apply_schur(out_half_dev, in_half_dev, tmp_half_dev, gauge, mass, dims, nrhs, precision, parity, true);
 }
 
-int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, const wd_gauge *gauge, double mass, const int dims[4],
+int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4],
                   int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host)
 {
     int rc = check_eo_args("wd_cgnr_schur", x_half_dev, b_half_dev, gauge, dims, 1, precision, parity);
@@ -517,7 +517,7 @@ int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, const wd_gauge *gaug
     a.links = gauge->links;
     a.stream = gauge->stream;
     cudaError_t e = cudaSuccess;
-    if (wd::cgnr_schur(a, x_half_dev, b_half_dev, mass, parity, max_iter, tol, iters_out, hist_host, &e))
+    if (wd::cgnr_schur(gauge, a, x_half_dev, b_half_dev, mass, parity, max_iter, tol, iters_out, hist_host, &e))
         return e == cudaErrorMemoryAllocation ? fail(WD_ERR_ALLOC, "wd_cgnr_schur: workspace allocation failed")
                                               : cuda_fail(e, "wd_cgnr_schur");
     return WD_OK;
@@ -534,6 +534,8 @@ void wd_destroy_gauge(wd_gauge *gauge)
     cudaFree(gauge->links);
     cudaFree(gauge->stage_canon);
     cudaFree(gauge->stage_canon_out);
+    cudaFree(gauge->cg_ws);
+    cudaFree(gauge->cg_sc);
     cudaFree(gauge->stage_in);
     cudaFree(gauge->stage_out);
     if (gauge->pipe_stream[0]) {

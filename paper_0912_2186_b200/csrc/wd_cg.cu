@@ -22,11 +22,22 @@ namespace {
 constexpr int RED_BLOCKS = 592; // 4 CTAs of 256 threads per SM on 148 SMs
 constexpr int RED_THREADS = 256;
 
+// Sum of the RED_BLOCKS partials, the same bits in every CTA and every run: warp 0 adds them in a fixed
+// pattern (lane l takes partials l, l+32, ... in order, then a fixed shuffle tree) and broadcasts through shared
+// memory.  Every thread of the CTA must call it (it contains a barrier).
 __device__ __forceinline__ double sum_partials(const double *part)
 {
-    double s = 0.0;
-    for (int i = 0; i < RED_BLOCKS; ++i) s += part[i]; // fixed order: same bits in every CTA and every run
-    return s;
+    __shared__ double total;
+    if (threadIdx.x < 32) {
+        double s = 0.0;
+        for (int i = threadIdx.x; i < RED_BLOCKS; i += 32) s += part[i];
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+        if (threadIdx.x == 0) total = s;
+    }
+    __syncthreads();
+    const double t = total;
+    __syncthreads(); // `total` may be reused by the next call
+    return t;
 }
 
 __device__ __forceinline__ double block_sum(double v, double *sh)
@@ -69,8 +80,17 @@ __global__ void __launch_bounds__(RED_THREADS) norm2_kernel(const Vec *__restric
 {
     __shared__ double sh[RED_THREADS / 32];
     double s = 0.0;
-    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS)
-        if (real_site<NCH>(i, Vh)) s += norm2_vec(v[i]);
+    constexpr int UNR = 4;
+    const long long stride = (long long)RED_BLOCKS * RED_THREADS;
+    for (long long i0 = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i0 < nvec; i0 += UNR * stride) {
+        Vec vv[UNR];
+#pragma unroll
+        for (int u = 0; u < UNR; ++u)
+            if (i0 + u * stride < nvec) vv[u] = v[i0 + u * stride];
+#pragma unroll
+        for (int u = 0; u < UNR; ++u)
+            if (i0 + u * stride < nvec && real_site<NCH>(i0 + u * stride, Vh)) s += norm2_vec(vv[u]);
+    }
     s = block_sum(s, sh);
     if (threadIdx.x == 0) part[blockIdx.x] = s;
 }
@@ -84,11 +104,25 @@ update_xr_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict
     __shared__ double sh[RED_THREADS / 32];
     const double alpha = sum_partials(zz_part) / sum_partials(ww_part);
     double s = 0.0;
-    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) {
-        x[i] = axpy_vec(alpha, p[i], x[i]);
-        const Vec rn = axpy_vec(-alpha, w[i], r[i]);
-        r[i] = rn;
-        if (real_site<NCH>(i, Vh)) s += norm2_vec(rn);
+    constexpr int UNR = 4; // independent vectors per thread and trip: enough loads in flight to cover HBM latency
+    const long long stride = (long long)RED_BLOCKS * RED_THREADS;
+    for (long long i0 = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i0 < nvec; i0 += UNR * stride) {
+        Vec pv[UNR], xv[UNR], wv[UNR], rv[UNR];
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            const long long i = i0 + u * stride;
+            if (i < nvec) { pv[u] = p[i]; xv[u] = x[i]; wv[u] = w[i]; rv[u] = r[i]; }
+        }
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            const long long i = i0 + u * stride;
+            if (i < nvec) {
+                x[i] = axpy_vec(alpha, pv[u], xv[u]);
+                const Vec rn = axpy_vec(-alpha, wv[u], rv[u]);
+                r[i] = rn;
+                if (real_site<NCH>(i, Vh)) s += norm2_vec(rn);
+            }
+        }
     }
     s = block_sum(s, sh);
     if (threadIdx.x == 0) rr_part[blockIdx.x] = s;
@@ -101,9 +135,25 @@ update_p_kernel(Vec *__restrict__ p, const Vec *__restrict__ z, long long nvec, 
                 const double *rr_part, double *hist_k)
 {
     const double beta = sum_partials(zz_new_part) / sum_partials(zz_old_part);
-    if (blockIdx.x == 0 && threadIdx.x == 0) *hist_k = sqrt(sum_partials(rr_part));
-    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS)
-        p[i] = axpy_vec(beta, p[i], z[i]);
+    if (blockIdx.x == 0) { // (block-uniform branch: sum_partials has barriers)
+        const double rr = sum_partials(rr_part);
+        if (threadIdx.x == 0) *hist_k = sqrt(rr);
+    }
+    constexpr int UNR = 4;
+    const long long stride = (long long)RED_BLOCKS * RED_THREADS;
+    for (long long i0 = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i0 < nvec; i0 += UNR * stride) {
+        Vec pv[UNR], zv[UNR];
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            const long long i = i0 + u * stride;
+            if (i < nvec) { pv[u] = p[i]; zv[u] = z[i]; }
+        }
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            const long long i = i0 + u * stride;
+            if (i < nvec) p[i] = axpy_vec(beta, pv[u], zv[u]);
+        }
+    }
 }
 
 template <typename Vec>
@@ -112,12 +162,16 @@ __global__ void __launch_bounds__(RED_THREADS) zero_kernel(Vec *__restrict__ v, 
     for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) v[i] = Vec{};
 }
 
-__global__ void sqrt_of_sum_kernel(const double *part, double *out) { *out = sqrt(sum_partials(part)); }
+__global__ void sqrt_of_sum_kernel(const double *part, double *out) // one CTA of 32 threads
+{
+    const double t = sum_partials(part);
+    if (threadIdx.x == 0) *out = sqrt(t);
+}
 
 } // namespace
 
 template <typename T>
-static int cgnr_schur_t(const ApplyArgs &shape, void *x_out, const void *b_in, double mass, int parity, int max_iter,
+static int cgnr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const void *b_in, double mass, int parity, int max_iter,
                         double tol, int *iters_out, double *hist_host, cudaError_t *err)
 {
     using SL = SpinorLayout<T>;
@@ -130,14 +184,24 @@ static int cgnr_schur_t(const ApplyArgs &shape, void *x_out, const void *b_in, d
     cudaStream_t s = shape.stream;
     const double a0 = 4.0 + mass;
 
-    char *ws = nullptr;
-    double *sc = nullptr; // zz_part[2][RED] | ww_part | rr_part | hist[max_iter + 1]
-    const size_t nsc = 4 * (size_t)RED_BLOCKS + (size_t)max_iter + 1;
-    if ((*err = cudaMalloc(&ws, 5 * hb)) != cudaSuccess) return -1;
-    if ((*err = cudaMalloc(&sc, nsc * sizeof(double))) != cudaSuccess) {
-        cudaFree(ws);
-        return -1;
+    // workspace lives in the gauge handle (a 0.5 GB cudaMalloc / cudaFree per solve costs up to a second)
+    const size_t nsc = 4 * (size_t)RED_BLOCKS + (size_t)max_iter + 1; // zz_part[2][RED] | ww_part | rr_part | hist
+    if (g->cg_ws_bytes < 5 * hb) {
+        cudaFree(g->cg_ws);
+        g->cg_ws = nullptr;
+        g->cg_ws_bytes = 0;
+        if ((*err = cudaMalloc(&g->cg_ws, 5 * hb)) != cudaSuccess) return -1;
+        g->cg_ws_bytes = 5 * hb;
     }
+    if (g->cg_sc_count < nsc) {
+        cudaFree(g->cg_sc);
+        g->cg_sc = nullptr;
+        g->cg_sc_count = 0;
+        if ((*err = cudaMalloc(&g->cg_sc, nsc * sizeof(double))) != cudaSuccess) return -1;
+        g->cg_sc_count = nsc;
+    }
+    char *ws = (char *)g->cg_ws;
+    double *sc = g->cg_sc;
     Vec *r = (Vec *)ws, *p = (Vec *)(ws + hb), *z = (Vec *)(ws + 2 * hb), *w = (Vec *)(ws + 3 * hb), *tmp = (Vec *)(ws + 4 * hb);
     Vec *x = (Vec *)x_out;
     double *zz_part[2] = {sc, sc + RED_BLOCKS}, *ww_part = sc + 2 * RED_BLOCKS, *rr_part = sc + 3 * RED_BLOCKS;
@@ -173,7 +237,7 @@ static int cgnr_schur_t(const ApplyArgs &shape, void *x_out, const void *b_in, d
         int cur = 0;
         norm2(z, zz_part[cur]);
         norm2(r, rr_part);
-        sqrt_of_sum_kernel<<<1, 1, 0, s>>>(rr_part, hist);
+        sqrt_of_sum_kernel<<<1, 32, 0, s>>>(rr_part, hist);
         count_launch();
         if (tol > 0.0) {
             if ((e = cudaMemcpyAsync(&h0, hist, sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
@@ -212,18 +276,16 @@ static int cgnr_schur_t(const ApplyArgs &shape, void *x_out, const void *b_in, d
         }
     } while (false);
     if (iters_out) *iters_out = k;
-    cudaFree(ws);
-    cudaFree(sc);
     return rc;
 }
 
 // x = approximate solution of Mhat x = b on `parity` after at most max_iter CGNR iterations (tol = 0: exactly
 // max_iter, no host synchronisation inside the loop).  Returns 0, or -1 with *err set.
-int cgnr_schur(const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter, double tol,
-               int *iters_out, double *hist_host, cudaError_t *err)
+int cgnr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter,
+               double tol, int *iters_out, double *hist_host, cudaError_t *err)
 {
-    return shape.precision == 32 ? cgnr_schur_t<float>(shape, x, b, mass, parity, max_iter, tol, iters_out, hist_host, err)
-                                 : cgnr_schur_t<double>(shape, x, b, mass, parity, max_iter, tol, iters_out, hist_host, err);
+    return shape.precision == 32 ? cgnr_schur_t<float>(g, shape, x, b, mass, parity, max_iter, tol, iters_out, hist_host, err)
+                                 : cgnr_schur_t<double>(g, shape, x, b, mass, parity, max_iter, tol, iters_out, hist_host, err);
 }
 
 } // namespace wd

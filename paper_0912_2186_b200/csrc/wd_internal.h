@@ -25,6 +25,11 @@ struct wd_gauge {
     void *stage_in;      // native in
     void *stage_out;     // native out
     size_t stage_bytes;
+    // workspace of wd_cgnr_schur (five half fields + reduction scalars), allocated on first use, reused
+    void *cg_ws;
+    size_t cg_ws_bytes;
+    double *cg_sc;
+    size_t cg_sc_count;
     cudaStream_t pipe_stream[3]; // copy-in, compute, copy-out streams of the pipelined host path
     cudaEvent_t pipe_event[2 * 16 + 2];
 };
@@ -64,8 +69,8 @@ cudaError_t launch_unpack_spinor(void *canonical, const void *native, long long 
 // red/black blocks (wd_dslash_eo.cu): out_p = alpha * xin_p + beta * hops(in_q); half-field <-> canonical copies
 cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger = false);
 // CGNR for Mhat x = b on one parity (wd_cg.cu); shape carries dims, V, precision, recon, links, stream
-int cgnr_schur(const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter, double tol,
-               int *iters_out, double *hist_host, cudaError_t *err);
+int cgnr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter,
+               double tol, int *iters_out, double *hist_host, cudaError_t *err);
 cudaError_t launch_parity_copy(void *native, void *canon, const int dims[4], long long V, int nrhs, int precision,
                                int parity, bool to_native, cudaStream_t s);
 cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon,
