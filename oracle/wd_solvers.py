@@ -61,3 +61,45 @@ def cgnr_schur(b, U, dims, mass, parity, niter, tol=0.0):
         zz = zz_new
         hist.append(float(np.sqrt(np.vdot(r, r))) / bnorm)
     return x, np.array(hist)
+
+
+def bicgstab_schur(b, U, dims, mass, parity, niter, tol=0.0):
+    """niter iterations (or until |r|/|b| <= tol) of BiCGstab (van der Vorst 1992, unpreconditioned) for
+    Mhat x = b on `parity`, x_0 = 0 (the paper's other solver around the even-odd matvec):
+
+        r = b, rhat = r, rho = alpha = omega = 1, v = p = 0
+        loop:  rho' = <rhat, r>;  beta = (rho'/rho)(alpha/omega);  p = r + beta (p - omega v);  v = Mhat p
+               alpha = rho' / <rhat, v>;  s = r - alpha v;  t = Mhat s;  omega = <t, s> / <t, t>
+               x += alpha p + omega s;  r = s - omega t;  rho = rho'
+
+    Complex inner products <a, b> = sum conj(a) b over (site, spin, colour).  Returns x (real-pair layout) and the
+    history of |r_k| / |b|."""
+    b = _mask(np.ascontiguousarray(b, dtype=np.float64), dims, parity)
+    U = np.ascontiguousarray(U, dtype=np.float64)
+    c = lambda v: v[..., 0] + 1j * v[..., 1]
+    rp = lambda v: np.stack([v.real, v.imag], axis=-1)
+    M = lambda v: c(wd_oracle.schur(np.ascontiguousarray(rp(v)), U, dims, mass, parity))
+    r = c(b)
+    rhat = r.copy()
+    x = np.zeros_like(r)
+    v = np.zeros_like(r)
+    p = np.zeros_like(r)
+    rho = alpha = omega = 1.0 + 0.0j
+    bnorm = float(np.sqrt(np.vdot(r, r).real))
+    hist = [1.0]
+    for _ in range(niter):
+        if hist[-1] <= tol:
+            break
+        rho_new = np.vdot(rhat, r)
+        beta = (rho_new / rho) * (alpha / omega)
+        p = r + beta * (p - omega * v)
+        v = M(p)
+        alpha = rho_new / np.vdot(rhat, v)
+        s = r - alpha * v
+        t = M(s)
+        omega = np.vdot(t, s) / np.vdot(t, t)
+        x = x + alpha * p + omega * s
+        r = s - omega * t
+        rho = rho_new
+        hist.append(float(np.sqrt(np.vdot(r, r).real)) / bnorm)
+    return rp(x), np.array(hist)

@@ -41,3 +41,33 @@ def test_k2_k3_residual_history(oracle):
     bm = np.where((parity_mask(dims) == 0)[..., None, None, None], c2r(b[0]), 0.0)
     true_r = bm - oracle.schur(x, c2r(U), dims, mass, 0)
     assert np.linalg.norm(true_r) / np.linalg.norm(bm) == pytest.approx(hist[-1], rel=1e-9)   # K3
+
+
+@pytest.mark.parametrize("parity", [0, 1])
+def test_k4_bicgstab_converged_solution_matches_dense_solve(oracle, parity):
+    dims = (2, 2, 2, 2)
+    U, b = random_fields(dims, 211)
+    mass = 0.25
+    V = fields.volume(dims)
+    M = dense_matrix(U, dims, mass)
+    par = np.repeat(parity_mask(dims).reshape(V), 12)
+    ip, iq = np.where(par == parity)[0], np.where(par != parity)[0]
+    S = M[np.ix_(ip, ip)] - M[np.ix_(ip, iq)] @ np.linalg.solve(M[np.ix_(iq, iq)], M[np.ix_(iq, ip)])
+    x, hist = wd_solvers.bicgstab_schur(c2r(b[0]), c2r(U), dims, mass, parity, niter=200, tol=1e-13)
+    want = np.linalg.solve(S, b[0].reshape(12 * V)[ip])
+    got = r2c(x).reshape(12 * V)
+    assert hist[-1] <= 1e-13
+    assert np.max(np.abs(got[ip] - want)) < 1e-11
+    assert np.all(got[iq] == 0)
+
+
+def test_k5_bicgstab_history_is_the_true_residual(oracle):
+    dims = (4, 2, 2, 4)
+    U, b = random_fields(dims, 213)
+    mass = -0.1
+    x, hist = wd_solvers.bicgstab_schur(c2r(b[0]), c2r(U), dims, mass, 0, niter=12)
+    bm = np.where((parity_mask(dims) == 0)[..., None, None, None], c2r(b[0]), 0.0)
+    true_r = bm - oracle.schur(np.ascontiguousarray(x), c2r(U), dims, mass, 0)
+    assert len(hist) == 13
+    assert np.linalg.norm(true_r) / np.linalg.norm(bm) == pytest.approx(hist[-1], rel=1e-8)
+    assert hist[-1] < 1e-2 * hist[0]   # it does converge on this well-conditioned system
