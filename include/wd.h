@@ -204,6 +204,12 @@ int wd_apply_schur_dagger(void *out_half_dev, const void *in_half_dev, void *tmp
 int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4],
                   int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host);
 
+/* wd_bicgstab_schur -- BiCGstab (van der Vorst) for Mhat x = b, x_0 = 0: the paper's other solver around the
+ * even-odd matvec (Table 2).  Same arguments, execution model and workspace as wd_cgnr_schur;
+ * one iteration = two Mhat applications; complex inner products summed deterministically in fp64. */
+int wd_bicgstab_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4],
+                      int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host);
+
 /* Number of CUDA kernels the library has launched in this process (all handles). */
 long long wd_launch_count(void);
 

@@ -168,7 +168,142 @@ __global__ void sqrt_of_sum_kernel(const double *part, double *out) // one CTA o
     if (threadIdx.x == 0) *out = sqrt(t);
 }
 
+// ---- BiCGstab pieces: complex inner products on the (re, im) pair layout, scalars as double2 in device memory ----
+struct cplxd {
+    double re, im;
+};
+__device__ __forceinline__ cplxd cmul(cplxd a, cplxd b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+__device__ __forceinline__ cplxd cdiv(cplxd a, cplxd b)
+{
+    const double d = b.re * b.re + b.im * b.im;
+    return {(a.re * b.re + a.im * b.im) / d, (a.im * b.re - a.re * b.im) / d};
+}
+__device__ __forceinline__ cplxd sum_partials_c(const double *part) // part[0..RED) = re, part[RED..2 RED) = im
+{
+    cplxd r;
+    r.re = sum_partials(part);
+    r.im = sum_partials(part + RED_BLOCKS);
+    return r;
+}
+
+// conj(a) * b summed over the complex numbers of one vector
+__device__ __forceinline__ void cdot_vec(const float4 &a, const float4 &b, double &re, double &im)
+{
+    re += (double)a.x * b.x + (double)a.y * b.y + (double)a.z * b.z + (double)a.w * b.w;
+    im += (double)a.x * b.y - (double)a.y * b.x + (double)a.z * b.w - (double)a.w * b.z;
+}
+__device__ __forceinline__ void cdot_vec(const double2 &a, const double2 &b, double &re, double &im)
+{
+    re += a.x * b.x + a.y * b.y;
+    im += a.x * b.y - a.y * b.x;
+}
+// y + c * x for complex c
+__device__ __forceinline__ float4 caxpy_vec(cplxd c, const float4 &x, const float4 &y)
+{
+    const float cr = (float)c.re, ci = (float)c.im;
+    return make_float4(y.x + cr * x.x - ci * x.y, y.y + cr * x.y + ci * x.x, y.z + cr * x.z - ci * x.w, y.w + cr * x.w + ci * x.z);
+}
+__device__ __forceinline__ double2 caxpy_vec(cplxd c, const double2 &x, const double2 &y)
+{
+    return make_double2(y.x + c.re * x.x - c.im * x.y, y.y + c.re * x.y + c.im * x.x);
+}
+
+// part = <a, b> (and, if TT, part2 = <a, a>) partials
+template <typename Vec, int NCH, bool TT>
+__global__ void __launch_bounds__(RED_THREADS)
+cdot_kernel(const Vec *__restrict__ a, const Vec *__restrict__ b, long long nvec, long long Vh, double *part, double *part2)
+{
+    __shared__ double sh[RED_THREADS / 32];
+    double re = 0.0, im = 0.0, aa = 0.0;
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS)
+        if (real_site<NCH>(i, Vh)) {
+            const Vec av = a[i], bv = b[i];
+            cdot_vec(av, bv, re, im);
+            if (TT) aa += norm2_vec(av);
+        }
+    re = block_sum(re, sh);
+    __syncthreads();
+    im = block_sum(im, sh);
+    __syncthreads();
+    if (TT) aa = block_sum(aa, sh);
+    if (threadIdx.x == 0) {
+        part[blockIdx.x] = re;
+        part[RED_BLOCKS + blockIdx.x] = im;
+        if (TT) part2[blockIdx.x] = aa;
+    }
+}
+
+// scal = {rho, alpha, omega} (device).  rho' = sum(rho_part); beta = (rho'/rho)(alpha/omega); p = r + beta (p - omega v);
+// block 0 stores rho <- rho' and the residual norm of the previous iteration into *hist_k
+template <typename Vec>
+__global__ void __launch_bounds__(RED_THREADS)
+bicg_p_kernel(Vec *__restrict__ p, const Vec *__restrict__ r, const Vec *__restrict__ v, long long nvec, const double *rho_part,
+              cplxd *scal, const double *rr_part, double *hist_k)
+{
+    const cplxd rho_new = sum_partials_c(rho_part);
+    const cplxd rho = scal[0], alpha = scal[1], omega = scal[2];
+    const cplxd beta = cmul(cdiv(rho_new, rho), cdiv(alpha, omega));
+    const cplxd mbo = {-(beta.re * omega.re - beta.im * omega.im), -(beta.re * omega.im + beta.im * omega.re)};
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS)
+        p[i] = caxpy_vec(mbo, v[i], caxpy_vec(beta, p[i], r[i])); // r + beta p - beta omega v
+    if (blockIdx.x == 0) {
+        const double rr = sum_partials(rr_part);
+        __syncthreads(); // every thread has read scal[0] before it is overwritten
+        if (threadIdx.x == 0) {
+            scal[3] = rho_new; // becomes rho after the alpha kernel (other CTAs may still be reading scal[0])
+            *hist_k = sqrt(rr);
+        }
+    }
+}
+
+// alpha = rho' / <rhat, v>;  s = r - alpha v  (s overwrites r);  block 0 stores alpha and rho <- rho'
+template <typename Vec>
+__global__ void __launch_bounds__(RED_THREADS)
+bicg_s_kernel(Vec *__restrict__ r, const Vec *__restrict__ v, long long nvec, const double *rv_part, cplxd *scal)
+{
+    const cplxd alpha = cdiv(scal[3], sum_partials_c(rv_part));
+    const cplxd ma = {-alpha.re, -alpha.im};
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS)
+        r[i] = caxpy_vec(ma, v[i], r[i]);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        scal[1] = alpha;
+        scal[0] = scal[3];
+    }
+}
+
+// omega = <t, s> / <t, t>;  x += alpha p + omega s;  r = s - omega t (s lives in r);  |r|^2 partials; block 0 stores omega
+template <typename Vec, int NCH>
+__global__ void __launch_bounds__(RED_THREADS)
+bicg_x_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict__ p, const Vec *__restrict__ t, long long nvec,
+              long long Vh, const double *ts_part, const double *tt_part, cplxd *scal, double *rr_part)
+{
+    __shared__ double sh[RED_THREADS / 32];
+    const cplxd ts = sum_partials_c(ts_part);
+    const double tt = sum_partials(tt_part);
+    const cplxd omega = {ts.re / tt, ts.im / tt};
+    const cplxd alpha = scal[1];
+    const cplxd mo = {-omega.re, -omega.im};
+    double s2 = 0.0;
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) {
+        const Vec sv = r[i];
+        x[i] = caxpy_vec(omega, sv, caxpy_vec(alpha, p[i], x[i]));
+        const Vec rn = caxpy_vec(mo, t[i], sv);
+        r[i] = rn;
+        if (real_site<NCH>(i, Vh)) s2 += norm2_vec(rn);
+    }
+    s2 = block_sum(s2, sh);
+    if (threadIdx.x == 0) rr_part[blockIdx.x] = s2;
+    if (blockIdx.x == 0 && threadIdx.x == 0) scal[2] = omega;
+}
+
+__global__ void bicg_init_kernel(cplxd *scal)
+{
+    for (int i = 0; i < 4; ++i) scal[i] = {1.0, 0.0};
+}
+
 } // namespace
+
+static cudaError_t ensure_workspace(wd_gauge *g, size_t ws_bytes, size_t nsc);
 
 template <typename T>
 static int cgnr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const void *b_in, double mass, int parity, int max_iter,
@@ -186,20 +321,7 @@ static int cgnr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const 
 
     // workspace lives in the gauge handle (a 0.5 GB cudaMalloc / cudaFree per solve costs up to a second)
     const size_t nsc = 4 * (size_t)RED_BLOCKS + (size_t)max_iter + 1; // zz_part[2][RED] | ww_part | rr_part | hist
-    if (g->cg_ws_bytes < 5 * hb) {
-        cudaFree(g->cg_ws);
-        g->cg_ws = nullptr;
-        g->cg_ws_bytes = 0;
-        if ((*err = cudaMalloc(&g->cg_ws, 5 * hb)) != cudaSuccess) return -1;
-        g->cg_ws_bytes = 5 * hb;
-    }
-    if (g->cg_sc_count < nsc) {
-        cudaFree(g->cg_sc);
-        g->cg_sc = nullptr;
-        g->cg_sc_count = 0;
-        if ((*err = cudaMalloc(&g->cg_sc, nsc * sizeof(double))) != cudaSuccess) return -1;
-        g->cg_sc_count = nsc;
-    }
+    if ((*err = ensure_workspace(g, 5 * hb, nsc)) != cudaSuccess) return -1;
     char *ws = (char *)g->cg_ws;
     double *sc = g->cg_sc;
     Vec *r = (Vec *)ws, *p = (Vec *)(ws + hb), *z = (Vec *)(ws + 2 * hb), *w = (Vec *)(ws + 3 * hb), *tmp = (Vec *)(ws + 4 * hb);
@@ -277,6 +399,134 @@ static int cgnr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const 
     } while (false);
     if (iters_out) *iters_out = k;
     return rc;
+}
+
+static cudaError_t ensure_workspace(wd_gauge *g, size_t ws_bytes, size_t nsc)
+{
+    cudaError_t e;
+    if (g->cg_ws_bytes < ws_bytes) {
+        cudaFree(g->cg_ws);
+        g->cg_ws = nullptr;
+        g->cg_ws_bytes = 0;
+        if ((e = cudaMalloc(&g->cg_ws, ws_bytes)) != cudaSuccess) return e;
+        g->cg_ws_bytes = ws_bytes;
+    }
+    if (g->cg_sc_count < nsc) {
+        cudaFree(g->cg_sc);
+        g->cg_sc = nullptr;
+        g->cg_sc_count = 0;
+        if ((e = cudaMalloc(&g->cg_sc, nsc * sizeof(double))) != cudaSuccess) return e;
+        g->cg_sc_count = nsc;
+    }
+    return cudaSuccess;
+}
+
+// BiCGstab for Mhat x = b, x_0 = 0: oracle/wd_solvers.py:bicgstab_schur step for step; same execution model as CGNR
+template <typename T>
+static int bicgstab_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const void *b_in, double mass, int parity,
+                            int max_iter, double tol, int *iters_out, double *hist_host, cudaError_t *err)
+{
+    using SL = SpinorLayout<T>;
+    using Vec = typename SL::Vec;
+    constexpr int NCH = SL::NCH;
+    constexpr int CHECK = 8;
+    const long long Vh = shape.V / 2;
+    const long long nvec = padded_volume(Vh) * NCH;
+    const size_t hb = (size_t)nvec * sizeof(Vec);
+    cudaStream_t s = shape.stream;
+    const double a0 = 4.0 + mass;
+    const size_t nsc = 8 * (size_t)RED_BLOCKS + 8 + (size_t)max_iter + 1;
+    if ((*err = ensure_workspace(g, 6 * hb, nsc)) != cudaSuccess) return -1;
+    char *ws = (char *)g->cg_ws;
+    Vec *r = (Vec *)ws, *rhat = (Vec *)(ws + hb), *p = (Vec *)(ws + 2 * hb), *v = (Vec *)(ws + 3 * hb), *t = (Vec *)(ws + 4 * hb),
+        *tmp = (Vec *)(ws + 5 * hb);
+    Vec *x = (Vec *)x_out;
+    double *sc = g->cg_sc;
+    double *rho_part = sc, *rv_part = sc + 2 * RED_BLOCKS, *ts_part = sc + 4 * RED_BLOCKS, *tt_part = sc + 6 * RED_BLOCKS,
+           *rr_part = sc + 7 * RED_BLOCKS;
+    cplxd *scal = (cplxd *)(sc + 8 * RED_BLOCKS);
+    double *hist = sc + 8 * RED_BLOCKS + 8;
+
+    ApplyArgs a = shape;
+    auto schur = [&](Vec *out, const Vec *in) -> cudaError_t {
+        a.out = tmp;
+        a.in = in;
+        cudaError_t e = launch_eo(a, nullptr, 0.0, -0.5, 1 - parity, false);
+        if (e != cudaSuccess) return e;
+        a.out = out;
+        a.in = tmp;
+        return launch_eo(a, in, a0, 0.5 / a0, parity, false);
+    };
+    int rc = 0, k = 0;
+    double h0 = 0.0;
+    auto fail_cuda = [&](cudaError_t e) {
+        *err = e;
+        rc = -1;
+    };
+    do {
+        cudaError_t e;
+        zero_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, nvec);
+        zero_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(p, nvec);
+        zero_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(v, nvec);
+        bicg_init_kernel<<<1, 1, 0, s>>>(scal);
+        count_launch(4);
+        if ((e = cudaMemcpyAsync(r, b_in, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
+        if ((e = cudaMemcpyAsync(rhat, b_in, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
+        norm2_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(r, nvec, Vh, rr_part);
+        sqrt_of_sum_kernel<<<1, 32, 0, s>>>(rr_part, hist);
+        count_launch(2);
+        if (tol > 0.0) {
+            if ((e = cudaMemcpyAsync(&h0, hist, sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
+            if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
+            if (h0 == 0.0) break;
+        }
+        for (k = 0; k < max_iter; ++k) {
+            cdot_kernel<Vec, NCH, false><<<RED_BLOCKS, RED_THREADS, 0, s>>>(rhat, r, nvec, Vh, rho_part, nullptr);
+            bicg_p_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(p, r, v, nvec, rho_part, scal, rr_part, hist + k);
+            count_launch(2);
+            if ((e = schur(v, p)) != cudaSuccess) { fail_cuda(e); break; }
+            cdot_kernel<Vec, NCH, false><<<RED_BLOCKS, RED_THREADS, 0, s>>>(rhat, v, nvec, Vh, rv_part, nullptr);
+            bicg_s_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(r, v, nvec, rv_part, scal);
+            count_launch(2);
+            if ((e = schur(t, r)) != cudaSuccess) { fail_cuda(e); break; }
+            cdot_kernel<Vec, NCH, true><<<RED_BLOCKS, RED_THREADS, 0, s>>>(t, r, nvec, Vh, ts_part, tt_part);
+            bicg_x_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, r, p, t, nvec, Vh, ts_part, tt_part, scal, rr_part);
+            count_launch(2);
+            if (tol > 0.0 && ((k + 1) % CHECK == 0 || k + 1 == max_iter)) {
+                double hk = 0.0;
+                sqrt_of_sum_kernel<<<1, 32, 0, s>>>(rr_part, hist + k + 1);
+                count_launch();
+                if ((e = cudaMemcpyAsync(&hk, hist + k + 1, sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
+                if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
+                if (hk <= tol * h0) {
+                    ++k;
+                    break;
+                }
+            }
+        }
+        if (rc) break;
+        sqrt_of_sum_kernel<<<1, 32, 0, s>>>(rr_part, hist + k); // |r_k| of the last iterate
+        count_launch();
+        if ((e = cudaGetLastError()) != cudaSuccess) { fail_cuda(e); break; }
+        if (hist_host) {
+            if ((e = cudaMemcpyAsync(hist_host, hist, ((size_t)k + 1) * sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
+        }
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
+        if (hist_host && hist_host[0] > 0.0) {
+            const double n0 = hist_host[0];
+            for (int i = 0; i <= k; ++i) hist_host[i] /= n0;
+        }
+    } while (false);
+    if (iters_out) *iters_out = k;
+    return rc;
+}
+
+int bicgstab_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter,
+                   double tol, int *iters_out, double *hist_host, cudaError_t *err)
+{
+    return shape.precision == 32
+               ? bicgstab_schur_t<float>(g, shape, x, b, mass, parity, max_iter, tol, iters_out, hist_host, err)
+               : bicgstab_schur_t<double>(g, shape, x, b, mass, parity, max_iter, tol, iters_out, hist_host, err);
 }
 
 // x = approximate solution of Mhat x = b on `parity` after at most max_iter CGNR iterations (tol = 0: exactly

@@ -71,6 +71,8 @@ cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double 
 // CGNR for Mhat x = b on one parity (wd_cg.cu); shape carries dims, V, precision, recon, links, stream
 int cgnr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter,
                double tol, int *iters_out, double *hist_host, cudaError_t *err);
+int bicgstab_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter,
+                   double tol, int *iters_out, double *hist_host, cudaError_t *err);
 cudaError_t launch_parity_copy(void *native, void *canon, const int dims[4], long long V, int nrhs, int precision,
                                int parity, bool to_native, cudaStream_t s);
 cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon,

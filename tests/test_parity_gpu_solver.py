@@ -92,3 +92,47 @@ def test_cgnr_converges_to_the_solution(oracle):
     bm = np.where(parity_mask(dims) == parity, b, 0.0)
     res = bm - oracle.schur(x.astype(np.float64), U.astype(np.float64), dims, cfg.mass, parity)
     assert np.linalg.norm(res) / np.linalg.norm(bm) <= 2e-11   # true residual, recomputed by the oracle
+
+
+@pytest.mark.parametrize("dims,parity", [((4, 4, 4, 4), 0), ((8, 4, 6, 2), 1), ((16, 8, 8, 8), 0), ((2, 6, 4, 2), 1)])
+@pytest.mark.parametrize("precision,recon,tol_x", [(64, 18, 1e-9), (64, 12, 1e-9), (32, 18, 1e-3), (32, 12, 1e-3)])
+def test_bicgstab_fixed_iterations_match_the_oracle(oracle, dims, parity, precision, recon, tol_x):
+    """K = 8 BiCGstab iterations (16 matvecs).  BiCGstab's scalars are ratios of inner products that shrink with the
+    residual, so rounding differences grow faster than in CG: 1e-9 (fp64) / 1e-3 (fp32) on x, ten times that on the
+    residual history -- derived bounds; a wrong alpha, omega or beta changes x at O(1)."""
+    import torch
+    K = 8
+    cfg = fields.Config("bi", dims, precision, "smooth", recon, 0.2, 1, 69)
+    U, b = fields.make_fields(cfg)
+    Uo = (U if recon == 18 else np.ascontiguousarray(U[..., :2, :, :])).astype(np.float64)
+    op = GpuOp(U, dims, precision, recon)
+    bh = to_half(op, b, parity)
+    xh = torch.full_like(bh, float("nan"))
+    iters, hist = op.op.bicgstab_schur(xh, bh, cfg.mass, parity, K)
+    x = from_half(op, xh, b.shape, parity)[0]
+    xh2 = torch.full_like(bh, float("nan"))
+    op.op.bicgstab_schur(xh2, bh, cfg.mass, parity, K)
+    x2 = from_half(op, xh2, b.shape, parity)[0]
+    op.close()
+    want_x, want_hist = wd_solvers.bicgstab_schur(b[0].astype(np.float64), Uo, dims, cfg.mass, parity, K)
+    assert iters == K and len(hist) == K + 1
+    assert np.array_equal(x, x2)                                   # deterministic reductions
+    assert rel_l2(x, want_x) <= tol_x
+    assert np.max(np.abs(np.array(hist) / want_hist - 1.0)) <= tol_x * 10
+
+
+def test_bicgstab_converges_to_the_solution(oracle):
+    import torch
+    dims, parity = (8, 8, 8, 8), 1
+    cfg = fields.Config("bic", dims, 64, "smooth", 18, 0.1, 1, 71)
+    U, b = fields.make_fields(cfg)
+    op = GpuOp(U, dims, 64, 18)
+    bh = to_half(op, b, parity)
+    xh = torch.empty_like(bh)
+    iters, hist = op.op.bicgstab_schur(xh, bh, cfg.mass, parity, 300, tol=1e-11)
+    x = from_half(op, xh, b.shape, parity)
+    op.close()
+    assert iters < 300 and hist[-1] <= 1e-11
+    bm = np.where(parity_mask(dims) == parity, b, 0.0)
+    res = bm - oracle.schur(x.astype(np.float64), U.astype(np.float64), dims, cfg.mass, parity)
+    assert np.linalg.norm(res) / np.linalg.norm(bm) <= 5e-11
