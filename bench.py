@@ -414,10 +414,10 @@ def run_schur(args):
 
 
 def run_cgnr(args):
-    """--op cgnr: CGNR on the even-odd preconditioned operator (Table 2): a step =
-    one wd_cgnr_schur call of ITER iterations (tol = 0: no host synchronisation inside).  Per iteration and even
-    site: flops 2 x (2 x 1320 + 48) + 288 (norms, x/r/p updates); algorithmic bytes 2 x Schur apply + 11 spinor
-    passes of the BLAS-1 kernels."""
+    """--op cgnr | bicgstab: the Krylov solvers on the even-odd preconditioned operator (SURVEY.md 8(f) f2;
+    PAPER.md:116, Table 2): a step = one solver call of ITER iterations (tol = 0: no host synchronisation inside).
+    Per iteration and even site: two operator applications (2 x (2 x 1320 + 48) flops, 2 x Schur-apply bytes) plus
+    the BLAS-1 kernels: CGNR 288 flops / 11 spinor passes, BiCGstab 672 flops / 19 spinor passes."""
     import torch
     from paper_0912_2186_b200 import binding, build
     rank, local, world = dist_env()
@@ -445,27 +445,29 @@ def run_cgnr(args):
         op.pack_parity(b, canon, 1, 0)
     stream.synchronize()
     iters = args.applies_per_step
+    solve = op.cgnr_schur if args.op == "cgnr" else op.bicgstab_schur
+    blas_flops, blas_passes = (288, 11) if args.op == "cgnr" else (672, 19)
     for _ in range(max(args.warmup, 3)):
-        op.cgnr_schur(x, b, cfg.mass, 0, iters)
+        solve(x, b, cfg.mass, 0, iters)
     torch.cuda.synchronize()
     n0 = binding.wd_launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local) as clocks:
         ev0.record(stream)
         for _ in range(args.steps):
-            done, hist = op.cgnr_schur(x, b, cfg.mass, 0, iters)
+            done, hist = solve(x, b, cfg.mass, 0, iters)
         ev1.record(stream)
         torch.cuda.synchronize()
     ms = ev0.elapsed_time(ev1)
     total_iters = args.steps * iters
-    flops_it = (2 * (2 * 1320 + 48) + 288) * (V // 2)
-    bytes_it = (V // 2) * (2 * (2 * 2 * 4 * recon * w + 5 * 24 * w) + 11 * 24 * w)
+    flops_it = (2 * (2 * 1320 + 48) + blas_flops) * (V // 2)
+    bytes_it = (V // 2) * (2 * (2 * 2 * 4 * recon * w + 5 * 24 * w) + blas_passes * 24 * w)
     peak, peak_src = measured_peak()
     achieved = bytes_it * total_iters / (ms * 1e-3) / 1e9
-    line = {"metric": "wilson_cgnr_gflops", "value": total_iters * flops_it / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
+    line = {"metric": "wilson_%s_gflops" % args.op, "value": total_iters * flops_it / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32" if cfg.precision == 32 else "f64", "data": "synthetic",
-            "config": {"workload": cfg.name, "op": "CGNR on the even-odd preconditioned operator", "dims": list(cfg.dims),
+            "config": {"workload": cfg.name, "op": ("CGNR" if args.op == "cgnr" else "BiCGstab") + " on the even-odd preconditioned operator", "dims": list(cfg.dims),
                        "recon": recon, "mass": cfg.mass, "iterations_per_step": iters,
                        "relative_residual_after_step": hist[-1],
                        "l2": "inputs larger than L2 (gauge + five half fields), no flush"},
@@ -487,7 +489,7 @@ def main():
     ap.add_argument("--kernel", default="auto", choices=["auto", "site", "tile", "stage"])
     ap.add_argument("--recon", type=int, default=None, choices=[18, 12])
     ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
-    ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr"],
+    ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr", "bicgstab"],
                     help="full = D of eq. (2.2) (the headline); schur = even-odd preconditioned operator (row f1); cgnr = CG on its normal equations (row f2, --applies-per-step = iterations)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--applies-per-step", type=int, default=APPLIES_PER_STEP,
@@ -499,7 +501,7 @@ def main():
         run_reference(args)
     elif args.op == "schur":
         run_schur(args)
-    elif args.op == "cgnr":
+    elif args.op in ("cgnr", "bicgstab"):
         run_cgnr(args)
     else:
         run_wd(args)
