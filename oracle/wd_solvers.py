@@ -103,3 +103,46 @@ def bicgstab_schur(b, U, dims, mass, parity, niter, tol=0.0):
         rho = rho_new
         hist.append(float(np.sqrt(np.vdot(r, r).real)) / bnorm)
     return rp(x), np.array(hist)
+
+
+def gcr_schur(b, U, dims, mass, parity, niter, restart=8, tol=0.0):
+    """niter iterations of restarted GCR(restart) (Eisenstat-Elman-Schultz 1983; "GCR(8) outer Krylov
+    solver"), here without a preconditioner, for Mhat x = b on `parity`, x_0 = 0:
+
+        r = b
+        loop k = 0, 1, ...   (j = k mod restart is the position inside the current cycle; a new cycle forgets all p's)
+            p_j = r;  q_j = Mhat p_j
+            for i < j:  beta = <q_i, q_j> / <q_i, q_i>;  p_j -= beta p_i;  q_j -= beta q_i        (modified Gram-Schmidt)
+            alpha = <q_j, r> / <q_j, q_j>;  x += alpha p_j;  r -= alpha q_j
+
+    One operator application per iteration.  Returns x (real-pair layout) and the history of |r_k| / |b|."""
+    b = _mask(np.ascontiguousarray(b, dtype=np.float64), dims, parity)
+    U = np.ascontiguousarray(U, dtype=np.float64)
+    c = lambda v: v[..., 0] + 1j * v[..., 1]
+    rp = lambda v: np.stack([v.real, v.imag], axis=-1)
+    M = lambda v: c(wd_oracle.schur(np.ascontiguousarray(rp(v)), U, dims, mass, parity))
+    r = c(b)
+    x = np.zeros_like(r)
+    bnorm = float(np.sqrt(np.vdot(r, r).real))
+    hist = [1.0]
+    P, Q, QQ = [], [], []
+    for k in range(niter):
+        if hist[-1] <= tol:
+            break
+        if k % restart == 0:
+            P, Q, QQ = [], [], []
+        p = r.copy()
+        q = M(p)
+        for pi, qi, qqi in zip(P, Q, QQ):
+            beta = np.vdot(qi, q) / qqi
+            p = p - beta * pi
+            q = q - beta * qi
+        qq = np.vdot(q, q).real
+        alpha = np.vdot(q, r) / qq
+        x = x + alpha * p
+        r = r - alpha * q
+        P.append(p)
+        Q.append(q)
+        QQ.append(qq)
+        hist.append(float(np.sqrt(np.vdot(r, r).real)) / bnorm)
+    return rp(x), np.array(hist)
