@@ -445,8 +445,10 @@ def run_cgnr(args):
         op.pack_parity(b, canon, 1, 0)
     stream.synchronize()
     iters = args.applies_per_step
-    solve = op.cgnr_schur if args.op == "cgnr" else op.bicgstab_schur
-    blas_flops, blas_passes = (288, 11) if args.op == "cgnr" else (672, 19)
+    solve = {"cgnr": op.cgnr_schur, "bicgstab": op.bicgstab_schur, "gcr": op.gcr_schur}[args.op]
+    # BLAS-1 flops / spinor passes per iteration and even site; matvecs per iteration.  GCR(8): averages over a cycle
+    # (3.5 Gram-Schmidt steps of 2 + 6 passes each, plus the copy, the <q,r> dot and the x/r update)
+    blas_flops, blas_passes, nmv = {"cgnr": (288, 11, 2), "bicgstab": (672, 19, 2), "gcr": (1150, 38, 1)}[args.op]
     for _ in range(max(args.warmup, 3)):
         solve(x, b, cfg.mass, 0, iters)
     torch.cuda.synchronize()
@@ -460,14 +462,14 @@ def run_cgnr(args):
         torch.cuda.synchronize()
     ms = ev0.elapsed_time(ev1)
     total_iters = args.steps * iters
-    flops_it = (2 * (2 * 1320 + 48) + blas_flops) * (V // 2)
-    bytes_it = (V // 2) * (2 * (2 * 2 * 4 * recon * w + 5 * 24 * w) + blas_passes * 24 * w)
+    flops_it = (nmv * (2 * 1320 + 48) + blas_flops) * (V // 2)
+    bytes_it = (V // 2) * (nmv * (2 * 2 * 4 * recon * w + 5 * 24 * w) + blas_passes * 24 * w)
     peak, peak_src = measured_peak()
     achieved = bytes_it * total_iters / (ms * 1e-3) / 1e9
     line = {"metric": "wilson_%s_gflops" % args.op, "value": total_iters * flops_it / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32" if cfg.precision == 32 else "f64", "data": "synthetic",
-            "config": {"workload": cfg.name, "op": ("CGNR" if args.op == "cgnr" else "BiCGstab") + " on the even-odd preconditioned operator", "dims": list(cfg.dims),
+            "config": {"workload": cfg.name, "op": {"cgnr": "CGNR", "bicgstab": "BiCGstab", "gcr": "GCR(8)"}[args.op] + " on the even-odd preconditioned operator", "dims": list(cfg.dims),
                        "recon": recon, "mass": cfg.mass, "iterations_per_step": iters,
                        "relative_residual_after_step": hist[-1],
                        "l2": "inputs larger than L2 (gauge + five half fields), no flush"},
@@ -489,7 +491,7 @@ def main():
     ap.add_argument("--kernel", default="auto", choices=["auto", "site", "tile", "stage"])
     ap.add_argument("--recon", type=int, default=None, choices=[18, 12])
     ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
-    ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr", "bicgstab"],
+    ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr", "bicgstab", "gcr"],
                     help="full = D of eq. (2.2) (the headline); schur = even-odd preconditioned operator (row f1); cgnr = CG on its normal equations (row f2, --applies-per-step = iterations)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--applies-per-step", type=int, default=APPLIES_PER_STEP,
@@ -501,7 +503,7 @@ def main():
         run_reference(args)
     elif args.op == "schur":
         run_schur(args)
-    elif args.op in ("cgnr", "bicgstab"):
+    elif args.op in ("cgnr", "bicgstab", "gcr"):
         run_cgnr(args)
     else:
         run_wd(args)

@@ -210,6 +210,12 @@ int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, dou
 int wd_bicgstab_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4],
                       int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host);
 
+/* wd_gcr_schur -- restarted GCR(restart) for Mhat x = b, x_0 = 0, no preconditioner: the paper's outer Krylov solver
+ * ("GCR(8)"), one Mhat application per iteration, modified Gram-Schmidt against the directions of the
+ * current cycle.  1 <= restart <= 32.  Otherwise as wd_cgnr_schur (workspace: 2*restart + 2 half fields). */
+int wd_gcr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4], int precision,
+                 int parity, int max_iter, int restart, double tol, int *iters_out, double *hist_host);
+
 /* Number of CUDA kernels the library has launched in this process (all handles). */
 long long wd_launch_count(void);
 

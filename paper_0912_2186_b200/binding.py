@@ -24,7 +24,7 @@ STATUS_NAMES = {
 SYMBOLS = (
     "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
     "wd_set_kernel", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
-    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
+    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
     "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
 )
 
@@ -70,6 +70,7 @@ def lib():
     L.wd_apply_schur_dagger.argtypes = [vp, vp, vp, vp, d, ip, i, i, i]
     L.wd_cgnr_schur.argtypes = [vp, vp, vp, d, ip, i, i, i, d, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]
     L.wd_bicgstab_schur.argtypes = L.wd_cgnr_schur.argtypes
+    L.wd_gcr_schur.argtypes = [vp, vp, vp, d, ip, i, i, i, i, d, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]
     L.wd_launch_count.argtypes = []
     L.wd_launch_count.restype = ctypes.c_longlong
     L.wd_last_error.argtypes = []
@@ -81,7 +82,7 @@ def lib():
     for name in ("wd_create_lattice", "wd_lattice_dims", "wd_load_gauge", "wd_set_stream", "wd_set_kernel",
                  "wd_selected_kernel", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
                  "wd_pack_spinor_parity", "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur",
-                 "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur"):
+                 "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur"):
         getattr(L, name).restype = i
     _lib = L
     return L
@@ -231,6 +232,15 @@ def wd_bicgstab_schur(x_half_dev, b_half_dev, gauge, mass, dims, precision, pari
     return _solve("wd_bicgstab_schur", x_half_dev, b_half_dev, gauge, mass, dims, precision, parity, max_iter, tol)
 
 
+def wd_gcr_schur(x_half_dev, b_half_dev, gauge, mass, dims, precision, parity, max_iter, restart=8, tol=0.0):
+    """Returns (iterations done, relative residual history as a list of floats)."""
+    it = ctypes.c_int(0)
+    hist = (ctypes.c_double * (int(max_iter) + 1))()
+    _check(lib().wd_gcr_schur(_ptr(x_half_dev), _ptr(b_half_dev), gauge, float(mass), _dims(dims), int(precision),
+                              int(parity), int(max_iter), int(restart), float(tol), ctypes.byref(it), hist), "wd_gcr_schur")
+    return it.value, [hist[i] for i in range(it.value + 1)]
+
+
 def wd_destroy_gauge(gauge):
     lib().wd_destroy_gauge(gauge)
 
@@ -309,6 +319,10 @@ class WilsonDirac:
 
     def bicgstab_schur(self, x_half_dev, b_half_dev, mass, parity, max_iter, tol=0.0):
         return wd_bicgstab_schur(x_half_dev, b_half_dev, self.gauge, mass, self.dims, self.precision, parity, max_iter, tol)
+
+    def gcr_schur(self, x_half_dev, b_half_dev, mass, parity, max_iter, restart=8, tol=0.0):
+        return wd_gcr_schur(x_half_dev, b_half_dev, self.gauge, mass, self.dims, self.precision, parity, max_iter, restart,
+                            tol)
 
     def apply_host(self, out_canonical_host, in_canonical_host, mass, nrhs=1):
         wd_apply_host(out_canonical_host, in_canonical_host, self.gauge, mass, self.dims, nrhs, self.precision)

@@ -540,6 +540,24 @@ int wd_bicgstab_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge,
     return WD_OK;
 }
 
+int wd_gcr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4], int precision,
+                 int parity, int max_iter, int restart, double tol, int *iters_out, double *hist_host)
+{
+    int rc = check_eo_args("wd_gcr_schur", x_half_dev, b_half_dev, gauge, dims, 1, precision, parity);
+    if (rc) return rc;
+    if (max_iter < 0 || tol < 0.0 || restart < 1 || restart > 32)
+        return fail(WD_ERR_MISMATCH, "wd_gcr_schur: max_iter=%d restart=%d tol=%g", max_iter, restart, tol);
+    if (4.0 + mass == 0.0) return fail(WD_ERR_MISMATCH, "wd_gcr_schur: 4 + mass = 0");
+    wd::ApplyArgs a = shape_args(gauge, 1);
+    a.links = gauge->links;
+    a.stream = gauge->stream;
+    cudaError_t e = cudaSuccess;
+    if (wd::gcr_schur(gauge, a, x_half_dev, b_half_dev, mass, parity, max_iter, restart, tol, iters_out, hist_host, &e))
+        return e == cudaErrorMemoryAllocation ? fail(WD_ERR_ALLOC, "wd_gcr_schur: workspace allocation failed")
+                                              : cuda_fail(e, "wd_gcr_schur");
+    return WD_OK;
+}
+
 long long wd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 const char *wd_last_error(void) { return g_err; }

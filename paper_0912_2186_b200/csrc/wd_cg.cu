@@ -529,6 +529,144 @@ int bicgstab_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, 
                : bicgstab_schur_t<double>(g, shape, x, b, mass, parity, max_iter, tol, iters_out, hist_host, err);
 }
 
+// ---- GCR(m) pieces ----
+// beta = <q_i, q_j> / qq_i;  p_j -= beta p_i;  q_j -= beta q_i
+template <typename Vec>
+__global__ void __launch_bounds__(RED_THREADS)
+gcr_orth_kernel(Vec *__restrict__ pj, Vec *__restrict__ qj, const Vec *__restrict__ pi, const Vec *__restrict__ qi, long long nvec,
+                const double *dot_part, const double *qq_i)
+{
+    const cplxd d = sum_partials_c(dot_part);
+    const double qq = *qq_i;
+    const cplxd mb = {-d.re / qq, -d.im / qq};
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) {
+        pj[i] = caxpy_vec(mb, pi[i], pj[i]);
+        qj[i] = caxpy_vec(mb, qi[i], qj[i]);
+    }
+}
+
+// alpha = <q, r> / <q, q>;  x += alpha p;  r -= alpha q;  |r|^2 partials;  block 0 stores <q, q>
+template <typename Vec, int NCH>
+__global__ void __launch_bounds__(RED_THREADS)
+gcr_update_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict__ p, const Vec *__restrict__ q, long long nvec,
+                  long long Vh, const double *qr_part, const double *qq_part, double *qq_out, double *rr_part)
+{
+    __shared__ double sh[RED_THREADS / 32];
+    const cplxd qr = sum_partials_c(qr_part);
+    const double qq = sum_partials(qq_part);
+    const cplxd alpha = {qr.re / qq, qr.im / qq};
+    const cplxd ma = {-alpha.re, -alpha.im};
+    double s2 = 0.0;
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) {
+        x[i] = caxpy_vec(alpha, p[i], x[i]);
+        const Vec rn = caxpy_vec(ma, q[i], r[i]);
+        r[i] = rn;
+        if (real_site<NCH>(i, Vh)) s2 += norm2_vec(rn);
+    }
+    s2 = block_sum(s2, sh);
+    if (threadIdx.x == 0) rr_part[blockIdx.x] = s2;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *qq_out = qq;
+}
+
+// restarted GCR(m) for Mhat x = b, x_0 = 0, no preconditioner: oracle/wd_solvers.py:gcr_schur step for step
+template <typename T>
+static int gcr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const void *b_in, double mass, int parity, int max_iter,
+                       int restart, double tol, int *iters_out, double *hist_host, cudaError_t *err)
+{
+    using SL = SpinorLayout<T>;
+    using Vec = typename SL::Vec;
+    constexpr int NCH = SL::NCH;
+    constexpr int CHECK = 8;
+    const long long Vh = shape.V / 2;
+    const long long nvec = padded_volume(Vh) * NCH;
+    const size_t hb = (size_t)nvec * sizeof(Vec);
+    cudaStream_t s = shape.stream;
+    const double a0 = 4.0 + mass;
+    const size_t nsc = 6 * (size_t)RED_BLOCKS + (size_t)restart + (size_t)max_iter + 1;
+    if ((*err = ensure_workspace(g, (size_t)(2 * restart + 2) * hb, nsc)) != cudaSuccess) return -1;
+    char *ws = (char *)g->cg_ws;
+    Vec *r = (Vec *)ws, *tmp = (Vec *)(ws + hb);
+    auto P = [&](int j) { return (Vec *)(ws + (size_t)(2 + j) * hb); };
+    auto Q = [&](int j) { return (Vec *)(ws + (size_t)(2 + restart + j) * hb); };
+    Vec *x = (Vec *)x_out;
+    double *sc = g->cg_sc;
+    double *dot_part = sc, *qr_part = sc + 2 * RED_BLOCKS, *qq_part = sc + 4 * RED_BLOCKS, *rr_part = sc + 5 * RED_BLOCKS;
+    double *qq = sc + 6 * RED_BLOCKS, *hist = qq + restart;
+
+    ApplyArgs a = shape;
+    auto schur = [&](Vec *out, const Vec *in) -> cudaError_t {
+        a.out = tmp;
+        a.in = in;
+        cudaError_t e = launch_eo(a, nullptr, 0.0, -0.5, 1 - parity, false);
+        if (e != cudaSuccess) return e;
+        a.out = out;
+        a.in = tmp;
+        return launch_eo(a, in, a0, 0.5 / a0, parity, false);
+    };
+    int rc = 0, k = 0;
+    double h0 = 0.0;
+    auto fail_cuda = [&](cudaError_t e) {
+        *err = e;
+        rc = -1;
+    };
+    do {
+        cudaError_t e;
+        zero_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, nvec);
+        if ((e = cudaMemcpyAsync(r, b_in, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
+        norm2_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(r, nvec, Vh, rr_part);
+        sqrt_of_sum_kernel<<<1, 32, 0, s>>>(rr_part, hist);
+        count_launch(3);
+        if (tol > 0.0) {
+            if ((e = cudaMemcpyAsync(&h0, hist, sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
+            if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
+            if (h0 == 0.0) break;
+        }
+        for (k = 0; k < max_iter; ++k) {
+            const int j = k % restart;
+            if ((e = cudaMemcpyAsync(P(j), r, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
+            if ((e = schur(Q(j), P(j))) != cudaSuccess) { fail_cuda(e); break; }
+            for (int i = 0; i < j; ++i) { // modified Gram-Schmidt against the cycle's earlier directions
+                cdot_kernel<Vec, NCH, false><<<RED_BLOCKS, RED_THREADS, 0, s>>>(Q(i), Q(j), nvec, Vh, dot_part, nullptr);
+                gcr_orth_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(P(j), Q(j), P(i), Q(i), nvec, dot_part, qq + i);
+                count_launch(2);
+            }
+            cdot_kernel<Vec, NCH, true><<<RED_BLOCKS, RED_THREADS, 0, s>>>(Q(j), r, nvec, Vh, qr_part, qq_part);
+            gcr_update_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, r, P(j), Q(j), nvec, Vh, qr_part, qq_part, qq + j, rr_part);
+            sqrt_of_sum_kernel<<<1, 32, 0, s>>>(rr_part, hist + k + 1);
+            count_launch(3);
+            if (tol > 0.0 && ((k + 1) % CHECK == 0 || k + 1 == max_iter)) {
+                double hk = 0.0;
+                if ((e = cudaMemcpyAsync(&hk, hist + k + 1, sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
+                if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
+                if (hk <= tol * h0) {
+                    ++k;
+                    break;
+                }
+            }
+        }
+        if (rc) break;
+        if ((e = cudaGetLastError()) != cudaSuccess) { fail_cuda(e); break; }
+        if (hist_host) {
+            if ((e = cudaMemcpyAsync(hist_host, hist, ((size_t)k + 1) * sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
+        }
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
+        if (hist_host && hist_host[0] > 0.0) {
+            const double n0 = hist_host[0];
+            for (int i = 0; i <= k; ++i) hist_host[i] /= n0;
+        }
+    } while (false);
+    if (iters_out) *iters_out = k;
+    return rc;
+}
+
+int gcr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter, int restart,
+              double tol, int *iters_out, double *hist_host, cudaError_t *err)
+{
+    return shape.precision == 32
+               ? gcr_schur_t<float>(g, shape, x, b, mass, parity, max_iter, restart, tol, iters_out, hist_host, err)
+               : gcr_schur_t<double>(g, shape, x, b, mass, parity, max_iter, restart, tol, iters_out, hist_host, err);
+}
+
 // x = approximate solution of Mhat x = b on `parity` after at most max_iter CGNR iterations (tol = 0: exactly
 // max_iter, no host synchronisation inside the loop).  Returns 0, or -1 with *err set.
 int cgnr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter,

@@ -73,6 +73,8 @@ int cgnr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, doub
                double tol, int *iters_out, double *hist_host, cudaError_t *err);
 int bicgstab_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter,
                    double tol, int *iters_out, double *hist_host, cudaError_t *err);
+int gcr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter, int restart,
+              double tol, int *iters_out, double *hist_host, cudaError_t *err);
 cudaError_t launch_parity_copy(void *native, void *canon, const int dims[4], long long V, int nrhs, int precision,
                                int parity, bool to_native, cudaStream_t s);
 cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon,

@@ -136,3 +136,47 @@ def test_bicgstab_converges_to_the_solution(oracle):
     bm = np.where(parity_mask(dims) == parity, b, 0.0)
     res = bm - oracle.schur(x.astype(np.float64), U.astype(np.float64), dims, cfg.mass, parity)
     assert np.linalg.norm(res) / np.linalg.norm(bm) <= 5e-11
+
+
+@pytest.mark.parametrize("dims,parity", [((4, 4, 4, 4), 0), ((8, 4, 6, 2), 1), ((16, 8, 8, 8), 0)])
+@pytest.mark.parametrize("precision,recon,tol_x", [(64, 18, 1e-10), (64, 12, 1e-10), (32, 18, 2e-4), (32, 12, 2e-4)])
+@pytest.mark.parametrize("restart", [8, 3])
+def test_gcr_fixed_iterations_match_the_oracle(oracle, dims, parity, precision, recon, tol_x, restart):
+    """K = 13 iterations of GCR(restart): more than one restart cycle.  Same derived bounds as CGNR (orthogonal
+    projections, well-conditioned system)."""
+    import torch
+    K = 13
+    cfg = fields.Config("gcr", dims, precision, "smooth", recon, 0.2, 1, 73)
+    U, b = fields.make_fields(cfg)
+    Uo = (U if recon == 18 else np.ascontiguousarray(U[..., :2, :, :])).astype(np.float64)
+    op = GpuOp(U, dims, precision, recon)
+    bh = to_half(op, b, parity)
+    xh = torch.full_like(bh, float("nan"))
+    iters, hist = op.op.gcr_schur(xh, bh, cfg.mass, parity, K, restart)
+    x = from_half(op, xh, b.shape, parity)[0]
+    xh2 = torch.full_like(bh, float("nan"))
+    op.op.gcr_schur(xh2, bh, cfg.mass, parity, K, restart)
+    x2 = from_half(op, xh2, b.shape, parity)[0]
+    op.close()
+    want_x, want_hist = wd_solvers.gcr_schur(b[0].astype(np.float64), Uo, dims, cfg.mass, parity, K, restart=restart)
+    assert iters == K and len(hist) == K + 1
+    assert np.array_equal(x, x2)
+    assert rel_l2(x, want_x) <= tol_x
+    assert np.max(np.abs(np.array(hist) / want_hist - 1.0)) <= tol_x * 10
+
+
+def test_gcr8_converges_to_the_solution(oracle):
+    import torch
+    dims, parity = (8, 8, 8, 8), 0
+    cfg = fields.Config("gcrc", dims, 64, "smooth", 18, 0.1, 1, 75)
+    U, b = fields.make_fields(cfg)
+    op = GpuOp(U, dims, 64, 18)
+    bh = to_half(op, b, parity)
+    xh = torch.empty_like(bh)
+    iters, hist = op.op.gcr_schur(xh, bh, cfg.mass, parity, 400, 8, tol=1e-11)
+    x = from_half(op, xh, b.shape, parity)
+    op.close()
+    assert iters < 400 and hist[-1] <= 1e-11
+    bm = np.where(parity_mask(dims) == parity, b, 0.0)
+    res = bm - oracle.schur(x.astype(np.float64), U.astype(np.float64), dims, cfg.mass, parity)
+    assert np.linalg.norm(res) / np.linalg.norm(bm) <= 5e-11
