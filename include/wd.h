@@ -216,6 +216,23 @@ int wd_bicgstab_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge,
 int wd_gcr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4], int precision,
                  int parity, int max_iter, int restart, double tol, int *iters_out, double *hist_host);
 
+/*
+ * ---- transfer operators of the adaptive multigrid set-up: eq. (2.7), on 4^4 space-time blocks with
+ * the gamma5 = +-1 (sigma3) split of PAPER.md:116; SURVEY.md 8(f) row f3.  Every extent must be a multiple of 4.
+ * The nv vectors are nv right-hand sides of ONE native buffer (wd_spinor_bytes(lat, nv, precision)).  Coarse vectors:
+ * [bt][bz][by][bx][sigma 0..1][alpha 0..nv-1][re, im] reals of the working precision, wd_coarse_reals(lat, nv) of them.
+ */
+long long wd_coarse_reals(const wd_lattice *lat, int nv);
+/* In place: vecs_native_dev <- orthonormal basis of its restrictions to every (block, chirality), modified
+ * Gram-Schmidt in the order alpha = 0..nv-1 (the columns P_{x; xhat, alpha} of eq. (2.7)). */
+int wd_block_orthonormalise(const wd_lattice *lat, void *vecs_native_dev, int nv, int precision, void *stream);
+/* coarse = P^dagger psi   (psi: one native field). */
+int wd_restrict(const wd_lattice *lat, void *coarse_dev, const void *basis_native_dev, const void *psi_native_dev, int nv,
+                int precision, void *stream);
+/* psi = P coarse. */
+int wd_prolong(const wd_lattice *lat, void *psi_native_dev, const void *basis_native_dev, const void *coarse_dev, int nv,
+               int precision, void *stream);
+
 /* Number of CUDA kernels the library has launched in this process (all handles). */
 long long wd_launch_count(void);
 

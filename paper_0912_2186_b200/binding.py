@@ -24,7 +24,8 @@ STATUS_NAMES = {
 SYMBOLS = (
     "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
     "wd_set_kernel", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
-    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
+    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_coarse_reals",
+    "wd_block_orthonormalise", "wd_restrict", "wd_prolong", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
     "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
 )
 
@@ -71,6 +72,11 @@ def lib():
     L.wd_cgnr_schur.argtypes = [vp, vp, vp, d, ip, i, i, i, d, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]
     L.wd_bicgstab_schur.argtypes = L.wd_cgnr_schur.argtypes
     L.wd_gcr_schur.argtypes = [vp, vp, vp, d, ip, i, i, i, i, d, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]
+    L.wd_coarse_reals.argtypes = [vp, i]
+    L.wd_coarse_reals.restype = ctypes.c_longlong
+    L.wd_block_orthonormalise.argtypes = [vp, vp, i, i, vp]
+    L.wd_restrict.argtypes = [vp, vp, vp, vp, i, i, vp]
+    L.wd_prolong.argtypes = [vp, vp, vp, vp, i, i, vp]
     L.wd_launch_count.argtypes = []
     L.wd_launch_count.restype = ctypes.c_longlong
     L.wd_last_error.argtypes = []
@@ -82,7 +88,8 @@ def lib():
     for name in ("wd_create_lattice", "wd_lattice_dims", "wd_load_gauge", "wd_set_stream", "wd_set_kernel",
                  "wd_selected_kernel", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
                  "wd_pack_spinor_parity", "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur",
-                 "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur"):
+                 "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur",
+                 "wd_block_orthonormalise", "wd_restrict", "wd_prolong"):
         getattr(L, name).restype = i
     _lib = L
     return L
@@ -239,6 +246,25 @@ def wd_gcr_schur(x_half_dev, b_half_dev, gauge, mass, dims, precision, parity, m
     _check(lib().wd_gcr_schur(_ptr(x_half_dev), _ptr(b_half_dev), gauge, float(mass), _dims(dims), int(precision),
                               int(parity), int(max_iter), int(restart), float(tol), ctypes.byref(it), hist), "wd_gcr_schur")
     return it.value, [hist[i] for i in range(it.value + 1)]
+
+
+def wd_coarse_reals(lat, nv):
+    return int(lib().wd_coarse_reals(lat, int(nv)))
+
+
+def wd_block_orthonormalise(lat, vecs_native_dev, nv, precision, stream=None):
+    _check(lib().wd_block_orthonormalise(lat, _ptr(vecs_native_dev), int(nv), int(precision), _ptr(stream)),
+           "wd_block_orthonormalise")
+
+
+def wd_restrict(lat, coarse_dev, basis_native_dev, psi_native_dev, nv, precision, stream=None):
+    _check(lib().wd_restrict(lat, _ptr(coarse_dev), _ptr(basis_native_dev), _ptr(psi_native_dev), int(nv), int(precision),
+                             _ptr(stream)), "wd_restrict")
+
+
+def wd_prolong(lat, psi_native_dev, basis_native_dev, coarse_dev, nv, precision, stream=None):
+    _check(lib().wd_prolong(lat, _ptr(psi_native_dev), _ptr(basis_native_dev), _ptr(coarse_dev), int(nv), int(precision),
+                            _ptr(stream)), "wd_prolong")
 
 
 def wd_destroy_gauge(gauge):

@@ -558,6 +558,55 @@ int wd_gcr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, doub
     return WD_OK;
 }
 
+// ---- transfer operators ------------------------------------------------------------------------------
+static int check_transfer(const char *who, const wd_lattice *lat, int nv, int precision)
+{
+    if (!lat) return fail(WD_ERR_NULL, "%s: NULL lattice", who);
+    if (lat->magic != LATTICE_MAGIC) return fail(WD_ERR_MISMATCH, "%s: not a live wd_lattice handle", who);
+    if (!valid_precision(precision)) return fail(WD_ERR_PRECISION, "%s: precision %d is not 32 or 64", who, precision);
+    if (nv < 1) return fail(WD_ERR_NRHS, "%s: nv=%d", who, nv);
+    for (int d = 0; d < 4; ++d)
+        if (lat->dims[d] % 4) return fail(WD_ERR_DIMS, "%s: extents must be multiples of the 4^4 block", who);
+    return WD_OK;
+}
+
+long long wd_coarse_reals(const wd_lattice *lat, int nv)
+{
+    if (check_transfer("wd_coarse_reals", lat, nv, WD_FP32)) return -1;
+    return lat->V / 256 * 2 * nv * 2;
+}
+
+int wd_block_orthonormalise(const wd_lattice *lat, void *vecs_native_dev, int nv, int precision, void *stream)
+{
+    int rc = check_transfer("wd_block_orthonormalise", lat, nv, precision);
+    if (rc) return rc;
+    if (!vecs_native_dev) return fail(WD_ERR_NULL, "wd_block_orthonormalise: NULL argument");
+    cudaError_t e = wd::launch_transfer(0, vecs_native_dev, nullptr, nullptr, lat->dims, lat->V, nv, precision, (cudaStream_t)stream);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_block_orthonormalise");
+}
+
+int wd_restrict(const wd_lattice *lat, void *coarse_dev, const void *basis_native_dev, const void *psi_native_dev, int nv,
+                int precision, void *stream)
+{
+    int rc = check_transfer("wd_restrict", lat, nv, precision);
+    if (rc) return rc;
+    if (!coarse_dev || !basis_native_dev || !psi_native_dev) return fail(WD_ERR_NULL, "wd_restrict: NULL argument");
+    cudaError_t e = wd::launch_transfer(1, coarse_dev, basis_native_dev, psi_native_dev, lat->dims, lat->V, nv, precision, (cudaStream_t)stream);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_restrict");
+}
+
+int wd_prolong(const wd_lattice *lat, void *psi_native_dev, const void *basis_native_dev, const void *coarse_dev, int nv,
+               int precision, void *stream)
+{
+    int rc = check_transfer("wd_prolong", lat, nv, precision);
+    if (rc) return rc;
+    if (!psi_native_dev || !basis_native_dev || !coarse_dev) return fail(WD_ERR_NULL, "wd_prolong: NULL argument");
+    if (overlap(psi_native_dev, wd_spinor_bytes(lat, 1, precision), basis_native_dev, wd_spinor_bytes(lat, nv, precision)))
+        return fail(WD_ERR_ALIAS, "wd_prolong: psi overlaps the basis");
+    cudaError_t e = wd::launch_transfer(2, psi_native_dev, basis_native_dev, coarse_dev, lat->dims, lat->V, nv, precision, (cudaStream_t)stream);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_prolong");
+}
+
 long long wd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 const char *wd_last_error(void) { return g_err; }

@@ -75,6 +75,9 @@ int bicgstab_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, 
                    double tol, int *iters_out, double *hist_host, cudaError_t *err);
 int gcr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter, int restart,
               double tol, int *iters_out, double *hist_host, cudaError_t *err);
+// transfer operators of the multigrid set-up (wd_transfer.cu)
+cudaError_t launch_transfer(int what, void *a, const void *b, const void *c, const int dims[4], long long V, int nv,
+                            int precision, cudaStream_t s);
 cudaError_t launch_parity_copy(void *native, void *canon, const int dims[4], long long V, int nrhs, int precision,
                                int parity, bool to_native, cudaStream_t s);
 cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon,
