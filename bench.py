@@ -482,6 +482,62 @@ def run_cgnr(args):
     op.close()
 
 
+def run_transfer(args):
+    """--op transfer: the multigrid transfer operators (eq. (2.7)) with N_v = 20 vectors
+     on the workload's lattice: a step = one wd_restrict + one wd_prolong; the block Gram-Schmidt is
+    timed once.  Algorithmic bytes: restrict reads N_v + 1 fields, prolong reads N_v and writes 1."""
+    import torch
+    from paper_0912_2186_b200 import binding, build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    build.build()
+    cfg = fields.CONFIGS[args.workload]
+    nv = 20
+    V = fields.volume(cfg.dims)
+    w = 4 if cfg.precision == 32 else 8
+    tdt = torch.float32 if cfg.precision == 32 else torch.float64
+    lat = binding.wd_create_lattice(cfg.dims)
+    n = binding.wd_spinor_bytes(lat, 1, cfg.precision) // w
+    g = torch.Generator(device="cuda").manual_seed(cfg.seed)
+    basis = torch.randn(nv * n, dtype=tdt, device="cuda", generator=g)   # native layout: any values are valid vectors
+    psi = torch.randn(n, dtype=tdt, device="cuda", generator=g)
+    out = torch.empty_like(psi)
+    coarse = torch.empty(binding.wd_coarse_reals(lat, nv), dtype=tdt, device="cuda")
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    ev[0].record()
+    binding.wd_block_orthonormalise(lat, basis, nv, cfg.precision)
+    ev[1].record()
+    for _ in range(max(args.warmup, 3)):
+        binding.wd_restrict(lat, coarse, basis, psi, nv, cfg.precision)
+        binding.wd_prolong(lat, out, basis, coarse, nv, cfg.precision)
+    torch.cuda.synchronize()
+    n0 = binding.wd_launch_count()
+    with ClockSampler(0) as clocks:
+        ev[2].record()
+        for _ in range(args.steps):
+            binding.wd_restrict(lat, coarse, basis, psi, nv, cfg.precision)
+            binding.wd_prolong(lat, out, basis, coarse, nv, cfg.precision)
+        ev[3].record()
+        torch.cuda.synchronize()
+    ms = ev[2].elapsed_time(ev[3]) / args.steps
+    bytes_step = (2 * nv + 2) * V * 24 * w
+    flops_step = 2 * nv * V * 12 * 8   # one complex multiply-add per component, vector and direction
+    peak, peak_src = measured_peak()
+    achieved = bytes_step / (ms * 1e-3) / 1e9
+    line = {"metric": "mg_transfer_gflops", "value": flops_step / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32" if cfg.precision == 32 else "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "op": "restrict + prolong, N_v = 20, 4^4 blocks x 2 chiralities",
+                       "dims": list(cfg.dims), "block_gram_schmidt_ms": ev[0].elapsed_time(ev[1]),
+                       "l2": "basis (20 fields) larger than L2, no flush"},
+            "clocks": clocks.summary(), "gpu_launches": int(binding.wd_launch_count() - n0),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src, "bytes_per_step": bytes_step,
+                         "kernel": "wd restrict_kernel + prolong_kernel"}}
+    print(json.dumps(line), flush=True)
+    binding.wd_destroy(lat)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -491,7 +547,7 @@ def main():
     ap.add_argument("--kernel", default="auto", choices=["auto", "site", "tile", "stage"])
     ap.add_argument("--recon", type=int, default=None, choices=[18, 12])
     ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
-    ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr", "bicgstab", "gcr"],
+    ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr", "bicgstab", "gcr", "transfer"],
                     help="full = D of eq. (2.2) (the headline); schur = even-odd preconditioned operator (row f1); cgnr = CG on its normal equations (row f2, --applies-per-step = iterations)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--applies-per-step", type=int, default=APPLIES_PER_STEP,
@@ -503,6 +559,8 @@ def main():
         run_reference(args)
     elif args.op == "schur":
         run_schur(args)
+    elif args.op == "transfer":
+        run_transfer(args)
     elif args.op in ("cgnr", "bicgstab", "gcr"):
         run_cgnr(args)
     else:

@@ -99,3 +99,37 @@ def test_transfer_rejects_bad_extents():
         binding.wd_block_orthonormalise(lat, buf, 4, 32)
     assert e.value.code == -2
     binding.wd_destroy(lat)
+
+
+@pytest.mark.parametrize("precision,tol", [(64, 1e-12), (32, 5e-6)])
+def test_galerkin_coarse_operator_by_composition(oracle, precision, tol):
+    """Dhat c = P^dagger D P c with every factor on the GPU (wd_prolong -> wd_apply -> wd_restrict)
+    against oracle/wd_coarsen.py:coarse_apply with the same basis."""
+    import torch
+    from gpu_util import GpuOp
+    dims, nv = (8, 8, 4, 8), 6
+    cfg = fields.Config("gal", dims, precision, "smooth", 18, -0.3, nv, 405)
+    U, psis = fields.make_fields(cfg)
+    x = Xfer(dims, precision)
+    basis = x.native(psis, nv)
+    binding.wd_block_orthonormalise(x.lat, basis, nv, precision)
+    Wc = to_c(x.canonical(basis, nv))
+    rng = np.random.default_rng(407)
+    shape = (dims[3] // 4, dims[2] // 4, dims[1] // 4, dims[0] // 4, 2, nv)
+    c = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+    c_dev = torch.from_numpy(np.ascontiguousarray(np.stack([c.real, c.imag], axis=-1)).astype(np_dtype(precision))).cuda()
+    op = GpuOp(U, dims, precision, 18)
+    n1 = op.op.native_numel(1)
+    fine = torch.full((n1,), float("nan"), dtype=x.tdt, device="cuda")
+    dfine = torch.full_like(fine, float("nan"))
+    out = torch.full_like(c_dev, float("nan"))
+    binding.wd_prolong(x.lat, fine, basis, c_dev, nv, precision)
+    op.op.apply(dfine, fine, cfg.mass, 1)
+    binding.wd_restrict(x.lat, out, basis, dfine, nv, precision)
+    torch.cuda.synchronize()
+    got = to_c(out.cpu().numpy().astype(np.float64))
+    cq = to_c(c_dev.cpu().numpy().astype(np.float64))       # the coarse vector as rounded to the working precision
+    want = wc.coarse_apply(Wc, cq, U.astype(np.float64), dims, cfg.mass)
+    op.close()
+    x.close()
+    assert rel_l2(rv(got), rv(want)) <= tol
