@@ -241,10 +241,14 @@ def run_wd(args):
     # ---- synthetic inputs (each rank its own replica: seeds shifted by rank) -------------------
     cfg_r = rank_config(cfg, recon, nrhs, rank)
     U, psi = fields.make_fields(cfg_r)
+    if args.temporal_gauge:
+        U, _ = fields.temporal_gauge(U, cfg.precision)
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
         u_dev = torch.from_numpy(U).to(dev)
         op = binding.WilsonDirac(cfg.dims, u_dev, cfg.precision, recon, stream=stream.cuda_stream, kernel=kernel)
+        if args.temporal_gauge:
+            op.set_temporal_gauge(True)
         canon = torch.from_numpy(psi).to(dev)
         ins = [torch.empty(op.native_numel(nrhs), dtype=tdt, device=dev) for _ in range(NBUF)]
         outs = [torch.empty(op.native_numel(nrhs), dtype=tdt, device=dev) for _ in range(NBUF)]
@@ -284,6 +288,8 @@ def run_wd(args):
     value = whole_job_gflops(world, applies, flops_per_apply, ms)
     launch_ms = ms / applies
     bytes_per_launch = compulsory_bytes_per_site(cfg.precision, recon, nrhs) * V
+    if args.temporal_gauge:  # unit t-links are not read except on the last time slice
+        bytes_per_launch -= recon * (4 if cfg.precision == 32 else 8) * (V - V // cfg.dims[3])
     peak, peak_src = measured_peak()
     achieved = bytes_per_launch / (launch_ms * 1e-3) / 1e9
 
@@ -312,7 +318,7 @@ def run_wd(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f32" if cfg.precision == 32 else "f64",
             "data": "synthetic",
             "config": {"workload": cfg.name, "dims": list(cfg.dims), "links": cfg.links, "recon": recon, "nrhs": nrhs,
-                       "mass": cfg.mass, "kernel": args.kernel, "applies_per_step": aps,
+                       "mass": cfg.mass, "kernel": args.kernel, "temporal_gauge": bool(args.temporal_gauge), "applies_per_step": aps,
                        "rotating_buffers": NBUF, "flops_per_site": FLOPS_PER_SITE,
                        "gflops_at_1320_per_site": value * 1320.0 / FLOPS_PER_SITE,
                        "l2": "inputs larger than L2 (gauge + rotating spinor fields), no flush",
@@ -549,6 +555,9 @@ def main():
     ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
     ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr", "bicgstab", "gcr", "transfer"],
                     help="full = D of eq. (2.2) (the headline); schur = even-odd preconditioned operator (row f1); cgnr = CG on its normal equations (row f2, --applies-per-step = iterations)")
+    ap.add_argument("--temporal-gauge", action="store_true",
+                    help="gauge-fix the synthetic links to temporal gauge and let the kernel skip the unit t-links "
+                         "(PAPER.md:157; row f4); algorithmic bytes then count 3 links + the last slice's t-links")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--applies-per-step", type=int, default=APPLIES_PER_STEP,
                     help="wd_apply calls per step (default 100 = configs[3]; lower it only for profiling)")

@@ -106,6 +106,13 @@ int wd_load_gauge(const wd_lattice *lat, const void *links_canonical_dev, int pr
 /* Stream (cudaStream_t as void*) on which wd_apply / pack / unpack for this gauge launch. */
 int wd_set_stream(wd_gauge *gauge, void *stream);
 
+/* Temporal gauge ("temporal gauge fixing", Fig. 4 / Table 2 "GF"): on != 0 declares that the loaded links
+ * satisfy U_t(x,t) = 1 for every t < Lt-1 (the last slice carries the Polyakov lines).  The library verifies it
+ * (WD_ERR_MISMATCH if some such link differs from 1 by more than 1e-6 / 1e-12; synchronises the stream) and the staged
+ * kernel then neither loads those links nor multiplies by them; the other kernels ignore the flag (same result).
+ * The operator is unchanged: D(U^g)(g psi) = g D(U) psi. */
+int wd_set_temporal_gauge(wd_gauge *gauge, int on);
+
 /* Force a kernel variant (wd_kernel).  WD_ERR_MISMATCH if it cannot handle the lattice. */
 int wd_set_kernel(wd_gauge *gauge, int kernel);
 

@@ -23,7 +23,7 @@ STATUS_NAMES = {
 # every symbol include/wd.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
-    "wd_set_kernel", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
+    "wd_set_kernel", "wd_set_temporal_gauge", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
     "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_coarse_reals",
     "wd_block_orthonormalise", "wd_restrict", "wd_prolong", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
     "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
@@ -55,6 +55,7 @@ def lib():
     L.wd_load_gauge.argtypes = [vp, vp, i, i, vp, ctypes.POINTER(vp)]
     L.wd_set_stream.argtypes = [vp, vp]
     L.wd_set_kernel.argtypes = [vp, i]
+    L.wd_set_temporal_gauge.argtypes = [vp, i]
     L.wd_selected_kernel.argtypes = [vp, i]
     L.wd_spinor_bytes.argtypes = [vp, i, i]
     L.wd_spinor_bytes.restype = ctypes.c_size_t
@@ -86,6 +87,7 @@ def lib():
     L.wd_destroy.argtypes = [vp]
     L.wd_destroy.restype = None
     for name in ("wd_create_lattice", "wd_lattice_dims", "wd_load_gauge", "wd_set_stream", "wd_set_kernel",
+                 "wd_set_temporal_gauge",
                  "wd_selected_kernel", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
                  "wd_pack_spinor_parity", "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur",
                  "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur",
@@ -166,6 +168,10 @@ def wd_selected_kernel(gauge, nrhs=1):
 
 
 KERNEL_NAMES = {WD_KERNEL_SITE: "site", WD_KERNEL_TILE: "tile", WD_KERNEL_STAGE: "stage"}
+
+
+def wd_set_temporal_gauge(gauge, on=True):
+    _check(lib().wd_set_temporal_gauge(gauge, int(bool(on))), "wd_set_temporal_gauge")
 
 
 def wd_spinor_bytes(lat, nrhs, precision):
@@ -306,6 +312,9 @@ class WilsonDirac:
 
     def unpack(self, canonical_dev, native_dev, nrhs, stream=None):
         wd_unpack_spinor(self.lat, canonical_dev, native_dev, nrhs, self.precision, stream or self.stream)
+
+    def set_temporal_gauge(self, on=True):
+        wd_set_temporal_gauge(self.gauge, on)
 
     def selected_kernel(self, nrhs=1):
         """Name of the kernel wd_apply will launch for nrhs right-hand sides ("site", "tile", "stage")."""

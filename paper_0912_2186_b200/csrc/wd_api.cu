@@ -155,6 +155,28 @@ int wd_set_stream(wd_gauge *gauge, void *stream)
     return WD_OK;
 }
 
+int wd_set_temporal_gauge(wd_gauge *gauge, int on)
+{
+    if (!gauge) return fail(WD_ERR_NULL, "wd_set_temporal_gauge: NULL gauge");
+    if (gauge->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_set_temporal_gauge: not a live wd_gauge handle");
+    if (!on) {
+        gauge->tgauge = 0;
+        return WD_OK;
+    }
+    int *flag = nullptr, h = 0;
+    cudaError_t e = cudaMalloc(&flag, sizeof(int));
+    if (e != cudaSuccess) return cuda_fail(e, "wd_set_temporal_gauge: cudaMalloc");
+    e = cudaMemsetAsync(flag, 0, sizeof(int), gauge->stream);
+    if (e == cudaSuccess) e = wd::launch_check_temporal_gauge(gauge->links, gauge->dims, gauge->V, gauge->precision, gauge->recon, flag, gauge->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, gauge->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(gauge->stream);
+    cudaFree(flag);
+    if (e != cudaSuccess) return cuda_fail(e, "wd_set_temporal_gauge");
+    if (h) return fail(WD_ERR_MISMATCH, "wd_set_temporal_gauge: some U_t(x,t), t < Lt-1, is not the unit matrix");
+    gauge->tgauge = 1;
+    return WD_OK;
+}
+
 int wd_set_kernel(wd_gauge *gauge, int kernel)
 {
     if (!gauge) return fail(WD_ERR_NULL, "wd_set_kernel: NULL gauge");
@@ -228,6 +250,7 @@ static wd::ApplyArgs shape_args(const wd_gauge *g, int nrhs)
     a.nrhs = nrhs;
     a.precision = g->precision;
     a.recon = g->recon;
+    a.tgauge = g->tgauge;
     return a;
 }
 
@@ -243,6 +266,7 @@ static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double m
     a.nrhs = nrhs;
     a.precision = g->precision;
     a.recon = g->recon;
+    a.tgauge = g->tgauge;
     a.stream = g->stream;
     cudaError_t e;
     if (g->kernel == WD_KERNEL_SITE)

@@ -97,7 +97,7 @@ template <typename T, int RECON> constexpr int stage_smem_vecs(int nt, int nyb, 
 template <typename T, int RECON, int NT, bool XS>
 __global__ void __launch_bounds__(NT ? NT : 256, 1)
 dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ links, int Lx, int Ly,
-                    int Lz, int Lt, int ty, int tz, long long V, T cdiag, int nrhs, int nchunk)
+                    int Lz, int Lt, int ty, int tz, long long V, T cdiag, int nrhs, int nchunk, int tgauge)
 {
     using SL = SpinorLayout<T>;
     using Vec = typename SL::Vec;
@@ -177,10 +177,16 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
             for (int j = 0; j < FY::n; ++j) cpa16(fly + j * nyb + rank_y, f + (FY::first + j) * BLK);
         }
     };
-    auto stage_B = [&](long long toff) { // links z,t of the own site + z face
+    // tgauge: the caller's links are in temporal gauge (U_t(x,t) = 1 for t < Lt-1; "temporal gauge
+    // fixing"): on those slices the vectors that hold only U_t are neither copied nor read and the t hops skip
+    // the colour multiplication.
+    auto unit_t = [&](int t) { return tgauge && t != Lt - 1; };
+    auto stage_B = [&](long long toff, int t) { // links z,t of the own site + z face
         const Vec *q = lk_own + toff * NVEC;
+        const int jend = unit_t(t) ? FZ::last + 1 : NVEC;
 #pragma unroll
-        for (int j = A_END; j < NVEC; ++j) cpa16(lnk + j * nt + tid, q + j * BLK);
+        for (int j = A_END; j < NVEC; ++j)
+            if (j < jend) cpa16(lnk + j * nt + tid, q + j * BLK);
         if (face_zf | face_zb) stage_spinor(fz, sp_z, toff);
         if (face_zb) {
             const Vec *f = lk_z + toff * NVEC;
@@ -197,14 +203,20 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
         cpa_commit(); // P'
         stage_A(toff);
         cpa_commit(); // A'
-        stage_B(toff);
+        stage_B(toff, t_begin);
         cpa_commit(); // B'
-        const long long site_tb = s3 + (long long)(t_begin == 0 ? Lt - 1 : t_begin - 1) * S3;
+        const int tb = t_begin == 0 ? Lt - 1 : t_begin - 1;
+        const long long site_tb = s3 + (long long)tb * S3;
         T u[18], p[24], h[12];
-        load_link<3, T, RECON>(links, site_tb, u);
         load_spinor(in, site_tb, p);
         project<3, +1>(p, h);
-        su3_dag_mul(u, h, chi_t);
+        if (unit_t(tb)) {
+#pragma unroll
+            for (int i = 0; i < 12; ++i) chi_t[i] = h[i];
+        } else {
+            load_link<3, T, RECON>(links, site_tb, u);
+            su3_dag_mul(u, h, chi_t);
+        }
     }
 
     for (int t = t_begin; t < t_end; ++t) {
@@ -283,16 +295,23 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
             }
         }
         // ---- t: forward hop now, backward product for the next slice ----
-        lds_link_at<3, RECON>(lnk, 0, nt, tid, u);
+        const bool ut = unit_t(t);
+        if (!ut) lds_link_at<3, RECON>(lnk, 0, nt, tid, u);
         cpa_wait<1>(); // own spinor of slice t+1 (this slice's P) has landed
         {
             T pn[24], h[12];
             lds_vecs<NCH>(plane0 + (cur ^ 1) * plane_sz, nt, tid, pn);
-            hop_forward<3>(acc, u, pn);
-            project<3, +1>(psi, h);
-            su3_dag_mul(u, h, chi_t);
+            if (ut) { // U_t(x,t) = 1: the hops are projection and reconstruction only
+                project<3, -1>(pn, h);
+                reconstruct_add<3, -1>(acc, h);
+                project<3, +1>(psi, chi_t);
+            } else {
+                hop_forward<3>(acc, u, pn);
+                project<3, +1>(psi, h);
+                su3_dag_mul(u, h, chi_t);
+            }
         }
-        if (more) stage_B(toff_n); // slots of links z,t and the z face are free again
+        if (more) stage_B(toff_n, t + 1 == Lt ? 0 : t + 1); // slots of links z,t and the z face are free again
         cpa_commit();
         __syncthreads(); // (B) exchange buffers complete
         if (!XS) {
@@ -399,7 +418,7 @@ cudaError_t launch_stage_nt(const ApplyArgs &a, const StageShape &s)
     dim3 grid((unsigned)(ncol * nchunk * a.nrhs));
     const T cdiag = (T)(4.0 + a.mass); // formed in double, rounded once (reading S8)
     kern<<<grid, s.nt, smem, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)a.links, a.dims[0], a.dims[1], a.dims[2],
-                                          a.dims[3], s.ty, s.tz, a.V, cdiag, a.nrhs, nchunk);
+                                          a.dims[3], s.ty, s.tz, a.V, cdiag, a.nrhs, nchunk, a.tgauge);
     count_launch();
     return cudaGetLastError();
 }

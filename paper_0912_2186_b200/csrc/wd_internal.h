@@ -16,6 +16,7 @@ struct wd_gauge {
     int precision;    // 32 / 64
     int recon;        // 18 / 12
     int kernel;       // wd_kernel selector
+    int tgauge;       // wd_set_temporal_gauge: U_t(x,t) = 1 for t < Lt-1 (verified when set)
     void *links;      // native links, device (cudaMalloc)
     size_t links_bytes;
     cudaStream_t stream;
@@ -47,6 +48,7 @@ struct ApplyArgs {
     int precision;
     int recon;
     cudaStream_t stream;
+    int tgauge;                     // links are in temporal gauge (U_t = 1 for t < Lt-1): kernels may skip them
     long long site_begin, site_end; // site kernel only: apply on [site_begin, site_end); 0,0 = whole lattice
 };
 
@@ -82,6 +84,8 @@ cudaError_t launch_parity_copy(void *native, void *canon, const int dims[4], lon
                                int parity, bool to_native, cudaStream_t s);
 cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon,
                               cudaStream_t s);
+cudaError_t launch_check_temporal_gauge(const void *links, const int dims[4], long long V, int precision, int recon,
+                                        int *flag_dev, cudaStream_t s);
 size_t native_link_bytes(long long V, int precision, int recon);
 
 } // namespace wd

@@ -122,4 +122,39 @@ cudaError_t launch_pack_links(void *native, const void *canonical, long long V, 
     return cudaGetLastError();
 }
 
+// flag |= 1 if some U_t(x, t) with t < Lt-1 differs from the unit matrix by more than tol (native links)
+template <typename T, int RECON>
+__global__ void check_temporal_gauge_kernel(const T *__restrict__ links, long long S3, long long V, double tol, int *flag)
+{
+    using L = LinkLayout<T, RECON>;
+    const long long site = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (site >= V - S3) return; // the last slice may hold anything
+    const typename L::Vec *q = reinterpret_cast<const typename L::Vec *>(links) + (site >> 5) * (L::NVEC * BLK) + (site & (BLK - 1));
+    bool bad = false;
+    for (int i = 0; i < RECON; ++i) { // reals of link 3: [3*RECON, 4*RECON)
+        const int r = 3 * RECON + i;
+        T v[L::CR];
+        unpack(q[(r / L::CR) * BLK], v);
+        const int elem = i / 2, a = elem / 3, b = elem % 3;
+        const double want = (i % 2 == 0 && a == b) ? 1.0 : 0.0;
+        if (fabs((double)v[r % L::CR] - want) > tol) bad = true;
+    }
+    if (bad) atomicOr(flag, 1);
+}
+
+cudaError_t launch_check_temporal_gauge(const void *links, const int dims[4], long long V, int precision, int recon, int *flag_dev,
+                                        cudaStream_t s)
+{
+    const long long S3 = (long long)dims[0] * dims[1] * dims[2];
+    if (V <= S3) return cudaSuccess;
+    const unsigned grid = (unsigned)((V - S3 + 127) / 128);
+    const double tol = precision == 32 ? 1e-6 : 1e-12;
+    if (precision == 32 && recon == 18) check_temporal_gauge_kernel<float, 18><<<grid, 128, 0, s>>>((const float *)links, S3, V, tol, flag_dev);
+    else if (precision == 32) check_temporal_gauge_kernel<float, 12><<<grid, 128, 0, s>>>((const float *)links, S3, V, tol, flag_dev);
+    else if (recon == 18) check_temporal_gauge_kernel<double, 18><<<grid, 128, 0, s>>>((const double *)links, S3, V, tol, flag_dev);
+    else check_temporal_gauge_kernel<double, 12><<<grid, 128, 0, s>>>((const double *)links, S3, V, tol, flag_dev);
+    count_launch();
+    return cudaGetLastError();
+}
+
 } // namespace wd

@@ -208,3 +208,22 @@ def make_fields(cfg, nrhs=None, dims=None):
         raise ValueError(cfg.links)
     psi = gaussian_spinor(d, cfg.seed + 1000, n, cfg.precision)
     return round_to(u, cfg.precision), psi
+
+
+def temporal_gauge(U, precision=64):
+    """Gauge-transform canonical links U [4,Lt,Lz,Ly,Lx,3,3,2] to temporal gauge ("temporal gauge fixing"):
+    g(x,0) = 1, g(x,t+1) = g(x,t) U_t(x,t), U'_mu(x) = g(x) U_mu(x) g(x+mu)^dagger, so that U'_t(x,t) = 1 (set exactly)
+    for t < Lt-1 and the last slice carries the Polyakov lines.  Input preparation only: D(U')(g psi) = g D(U) psi is
+    the same operator.  Returns (U' rounded to `precision`, g as complex [Lt,Lz,Ly,Lx,3,3])."""
+    Uc = U[..., 0].astype(np.float64) + 1j * U[..., 1].astype(np.float64)        # [4,Lt,Lz,Ly,Lx,3,3]
+    Lt = Uc.shape[1]
+    g = np.empty(Uc.shape[1:], dtype=np.complex128)
+    g[0] = np.eye(3)
+    for t in range(Lt - 1):
+        g[t + 1] = g[t] @ Uc[3, t]
+    out = np.empty_like(Uc)
+    for mu in range(4):
+        g_fwd = np.roll(g, -1, axis=3 - mu)                                      # g(x + mu), site axes are [t,z,y,x]
+        out[mu] = g @ Uc[mu] @ np.conj(np.swapaxes(g_fwd, -1, -2))
+    out[3, :Lt - 1] = np.eye(3)
+    return round_to(_to_real_pairs(out), precision), g
