@@ -109,7 +109,7 @@ int wd_set_stream(wd_gauge *gauge, void *stream);
 /* Temporal gauge ("temporal gauge fixing", Fig. 4 / Table 2 "GF"): on != 0 declares that the loaded links
  * satisfy U_t(x,t) = 1 for every t < Lt-1 (the last slice carries the Polyakov lines).  The library verifies it
  * (WD_ERR_MISMATCH if some such link differs from 1 by more than 1e-6 / 1e-12; synchronises the stream) and the staged
- * kernel then neither loads those links nor multiplies by them; the other kernels ignore the flag (same result).
+ * kernels then neither load those links nor multiply by them; the other kernels ignore the flag (same result).
  * The operator is unchanged: D(U^g)(g psi) = g D(U) psi. */
 int wd_set_temporal_gauge(wd_gauge *gauge, int on);
 

@@ -87,7 +87,7 @@ template <int RECON> constexpr int mrhs_smem_vecs(int nts, int nrb, int nyb, int
 template <int RECON, int NRB, int NTS>
 __global__ void __launch_bounds__(128 * NRB, 1)
 dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const float *__restrict__ links, int Lx, int Ly,
-                   int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk, int patch)
+                   int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk, int patch, int tgauge)
 {
     constexpr int NVEC = LinkLayout<float, RECON>::NVEC;
     using FY = LinkVecs<1, RECON>;
@@ -190,8 +190,10 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         deal_links(0, A_END, lnk, nts, st, lk_own + toff * NVEC, 0);
         if (face_yb) deal_links(0, FY::n, fly, nyb, rank_y, lk_y + toff * NVEC, FY::first);
     };
-    auto stage_ZT = [&](long long toff) { // links z,t of the site + the z-face link
-        deal_links(A_END, NVEC, lnk + A_END * nts, nts, st, lk_own + toff * NVEC, A_END);
+    // temporal gauge (wd_set_temporal_gauge): U_t(x,t) = 1 for t < Lt-1 -- those links are neither copied nor read
+    auto unit_t = [&](int t) { return tgauge && t != Lt - 1; };
+    auto stage_ZT = [&](long long toff, int t) { // links z,t of the site + the z-face link
+        deal_links(A_END, unit_t(t) ? FZ::last + 1 : NVEC, lnk + A_END * nts, nts, st, lk_own + toff * NVEC, A_END);
         if (face_zb) deal_links(0, FZ::n, flz, nzb, rank_z, lk_z + toff * NVEC, FZ::first);
     };
 
@@ -207,12 +209,18 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         cpa_commit(); // c3'
         if (face_zf | face_zb) stage_spinor(fz, sp_z, toff);
         cpa_commit(); // c4'
-        const long long site_tb = s3 + (long long)(t_begin == 0 ? Lt - 1 : t_begin - 1) * S3;
+        const int tb = t_begin == 0 ? Lt - 1 : t_begin - 1;
+        const long long site_tb = s3 + (long long)tb * S3;
         float u[18], p[24], h[12];
-        load_link<3, float, RECON>(links, site_tb, u);
         load_spinor(in, site_tb, p);
         project<3, +1>(p, h);
-        su3_dag_mul(u, h, chi_t);
+        if (unit_t(tb)) {
+#pragma unroll
+            for (int i = 0; i < 12; ++i) chi_t[i] = h[i];
+        } else {
+            load_link<3, float, RECON>(links, site_tb, u);
+            su3_dag_mul(u, h, chi_t);
+        }
     }
 
     for (int t = t_begin; t < t_end; ++t) {
@@ -221,7 +229,7 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         const bool more = (t + 1 < t_end);
         cpa_wait<1>();   // links x,y and the y-face spinor of slice t have landed (own copies)
         __syncthreads(); // (A) ... everybody's; the z,t hops of slice t-1 are over
-        stage_ZT(toff);
+        stage_ZT(toff, t);
         stage_spinor(plane0 + (cur ^ 1) * plane_sz, sp_own, toff_n);
         cpa_commit(); // c1
 
@@ -280,13 +288,19 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         if (more && (face_zf | face_zb)) stage_spinor(fz, sp_z, toff_n);
         cpa_commit(); // c4
         // ---- t: forward hop now, backward product for the next slice ----
-        lds_link<3, RECON>(lnk, 0, nts, st, u);
         {
             float h[12];
             lds_vecs<6>(plane0 + (cur ^ 1) * plane_sz, nt, tid, pn);
-            hop_forward<3>(acc, u, pn);
-            project<3, +1>(psi, h);
-            su3_dag_mul(u, h, chi_t);
+            if (unit_t(t)) { // U_t(x,t) = 1: projection and reconstruction only
+                project<3, -1>(pn, h);
+                reconstruct_add<3, -1>(acc, h);
+                project<3, +1>(psi, chi_t);
+            } else {
+                lds_link<3, RECON>(lnk, 0, nts, st, u);
+                hop_forward<3>(acc, u, pn);
+                project<3, +1>(psi, h);
+                su3_dag_mul(u, h, chi_t);
+            }
         }
         // fused diagonal (step a6) and store (a7)
 #pragma unroll
@@ -345,7 +359,7 @@ cudaError_t launch_mrhs_n(const ApplyArgs &a, int ty, int tz)
     if (patch < 1 || ncyh % patch || nczh % patch) patch = 0;
     const float cdiag = (float)(4.0 + a.mass); // formed in double, rounded once (reading S8)
     kern<<<grid, nts * NRB, smem, a.stream>>>((float *)a.out, (const float *)a.in, (const float *)a.links, a.dims[0],
-                                               a.dims[1], a.dims[2], a.dims[3], ty, tz, a.V, cdiag, a.nrhs, nchunk, patch);
+                                               a.dims[1], a.dims[2], a.dims[3], ty, tz, a.V, cdiag, a.nrhs, nchunk, patch, a.tgauge);
     count_launch();
     return cudaGetLastError();
 }
