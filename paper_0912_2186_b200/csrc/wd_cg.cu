@@ -104,7 +104,7 @@ update_xr_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict
     __shared__ double sh[RED_THREADS / 32];
     const double alpha = sum_partials(zz_part) / sum_partials(ww_part);
     double s = 0.0;
-    constexpr int UNR = 4; // independent vectors per thread and trip: enough loads in flight to cover HBM latency
+    constexpr int UNR = 2; // independent vectors per thread and trip (4 streams x 2 loads in flight; 4 costs occupancy)
     const long long stride = (long long)RED_BLOCKS * RED_THREADS;
     for (long long i0 = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i0 < nvec; i0 += UNR * stride) {
         Vec pv[UNR], xv[UNR], wv[UNR], rv[UNR];

@@ -99,28 +99,53 @@ __global__ void __launch_bounds__(TB) block_orthonormalise_kernel(T *__restrict_
     }
 }
 
+// restrict: the N_v inner products are taken CH at a time -- CH independent vector loads in flight, 4*CH partial
+// sums reduced by warp shuffles, one shared-memory hand-off (two barriers) per chunk instead of per vector
 template <typename T>
 __global__ void __launch_bounds__(TB)
 restrict_kernel(T *__restrict__ coarse, const T *__restrict__ W, const T *__restrict__ psi, int Lx, int Ly, int Lz, long long V, int nv)
 {
-    __shared__ double sh[TB / 32];
+    constexpr int CH = 4;
+    __shared__ double sh[TB / 32][4 * CH];
     const long long site = block_site(threadIdx.x, blockIdx.x, Lx, Ly, Lz);
     const long long stride = 24 * padded_volume(V);
     T p[24];
     load_spinor(psi, site, p);
-    for (int a = 0; a < nv; ++a) {
-        T w[24];
-        load_spinor(W + a * stride, site, w);
-        double d[4];
-        chiral_dots(w, p, d);
+    T *c = coarse + ((long long)blockIdx.x * 2 * nv) * 2;
+    for (int a0 = 0; a0 < nv; a0 += CH) {
+        double d[CH][4];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) d[i] = cta_sum(d[i], sh);
-        if (threadIdx.x == 0) {
-            T *c = coarse + ((long long)blockIdx.x * 2 * nv) * 2;
-            c[(0 * nv + a) * 2] = (T)d[0];
-            c[(0 * nv + a) * 2 + 1] = (T)d[1];
-            c[(1 * nv + a) * 2] = (T)d[2];
-            c[(1 * nv + a) * 2 + 1] = (T)d[3];
+        for (int k = 0; k < CH; ++k) {
+            if (a0 + k < nv) { // block-uniform
+                T w[24];
+                load_spinor(W + (a0 + k) * stride, site, w);
+                chiral_dots(w, p, d[k]);
+            } else {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) d[k][i] = 0.0;
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < CH; ++k)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                double v = d[k][i];
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+                d[k][i] = v;
+            }
+        __syncthreads(); // sh free again
+        if ((threadIdx.x & 31) == 0)
+#pragma unroll
+            for (int k = 0; k < CH; ++k)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) sh[threadIdx.x >> 5][4 * k + i] = d[k][i];
+        __syncthreads();
+        if (threadIdx.x < 4 * CH) { // thread j finishes sum j = 4*k + i in a fixed order
+            double sum = 0.0;
+#pragma unroll
+            for (int wp = 0; wp < TB / 32; ++wp) sum += sh[wp][threadIdx.x];
+            const int k = threadIdx.x >> 2, i = threadIdx.x & 3, a = a0 + k;
+            if (a < nv) c[((i >> 1) * nv + a) * 2 + (i & 1)] = (T)sum;
         }
     }
 }
