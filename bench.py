@@ -232,7 +232,7 @@ def run_wd(args):
 
     cfg = fields.CONFIGS[args.workload]
     recon = args.recon
-    nrhs = cfg.nrhs
+    nrhs = args.nrhs if args.nrhs else cfg.nrhs
     V = fields.volume(cfg.dims)
     tdt = torch.float32 if cfg.precision == 32 else torch.float64
     kernel = {"auto": binding.WD_KERNEL_AUTO, "site": binding.WD_KERNEL_SITE, "tile": binding.WD_KERNEL_TILE,
@@ -555,6 +555,8 @@ def main():
     ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
     ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr", "bicgstab", "gcr", "transfer"],
                     help="full = D of eq. (2.2) (the headline); schur = even-odd preconditioned operator (row f1); cgnr = CG on its normal equations (row f2, --applies-per-step = iterations)")
+    ap.add_argument("--nrhs", type=int, default=None,
+                    help="override the workload's number of right-hand sides (e.g. 20 = the paper's N_v, PAPER.md:124)")
     ap.add_argument("--temporal-gauge", action="store_true",
                     help="gauge-fix the synthetic links to temporal gauge and let the kernel skip the unit t-links "
                          "(PAPER.md:157; row f4); algorithmic bytes then count 3 links + the last slice's t-links")
