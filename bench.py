@@ -423,7 +423,8 @@ def run_cgnr(args):
     """--op cgnr | bicgstab: the Krylov solvers on the even-odd preconditioned operator (SURVEY.md 8(f) f2;
     PAPER.md:116, Table 2): a step = one solver call of ITER iterations (tol = 0: no host synchronisation inside).
     Per iteration and even site: two operator applications (2 x (2 x 1320 + 48) flops, 2 x Schur-apply bytes) plus
-    the BLAS-1 kernels: CGNR 288 flops / 11 spinor passes, BiCGstab 672 flops / 19 spinor passes."""
+    the BLAS-1 kernels: CGNR 288 flops / 9 spinor passes (the two norms come out of the matvec epilogue), BiCGstab
+    672 flops / 19 spinor passes, GCR(8) ~1150 flops / 38 passes averaged over a cycle."""
     import torch
     from paper_0912_2186_b200 import binding, build
     rank, local, world = dist_env()
@@ -454,7 +455,7 @@ def run_cgnr(args):
     solve = {"cgnr": op.cgnr_schur, "bicgstab": op.bicgstab_schur, "gcr": op.gcr_schur}[args.op]
     # BLAS-1 flops / spinor passes per iteration and even site; matvecs per iteration.  GCR(8): averages over a cycle
     # (3.5 Gram-Schmidt steps of 2 + 6 passes each, plus the copy, the <q,r> dot and the x/r update)
-    blas_flops, blas_passes, nmv = {"cgnr": (288, 11, 2), "bicgstab": (672, 19, 2), "gcr": (1150, 38, 1)}[args.op]
+    blas_flops, blas_passes, nmv = {"cgnr": (288, 9, 2), "bicgstab": (672, 19, 2), "gcr": (1150, 38, 1)}[args.op]
     for _ in range(max(args.warmup, 3)):
         solve(x, b, cfg.mass, 0, iters)
     torch.cuda.synchronize()

@@ -5,6 +5,7 @@
 //     x = 0, r = b, z = Mhat^dag r, p = z, zz = <z,z>
 //     loop:  w = Mhat p;  alpha = zz/<w,w>;  x += alpha p;  r -= alpha w;  z = Mhat^dag r;
 //            zz' = <z,z>;  beta = zz'/zz;  p = z + beta p
+// (<w,w> and <z,z> are produced by the epilogue of the matvec kernel itself: no extra pass over w and z)
 // B200 shape of it: the whole iteration is enqueued on the gauge's stream with NO host synchronisation -- every
 // scalar lives in device memory.  Reductions are deterministic two-level sums in fp64: each of RED_BLOCKS CTAs
 // writes one partial in a fixed order, and every CTA of the kernel that needs the scalar re-adds the partials
@@ -25,12 +26,12 @@ constexpr int RED_THREADS = 256;
 // Sum of the RED_BLOCKS partials, the same bits in every CTA and every run: warp 0 adds them in a fixed
 // pattern (lane l takes partials l, l+32, ... in order, then a fixed shuffle tree) and broadcasts through shared
 // memory.  Every thread of the CTA must call it (it contains a barrier).
-__device__ __forceinline__ double sum_partials(const double *part)
+__device__ __forceinline__ double sum_partials(const double *part, int n = RED_BLOCKS)
 {
     __shared__ double total;
     if (threadIdx.x < 32) {
         double s = 0.0;
-        for (int i = threadIdx.x; i < RED_BLOCKS; i += 32) s += part[i];
+        for (int i = threadIdx.x; i < n; i += 32) s += part[i];
         for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
         if (threadIdx.x == 0) total = s;
     }
@@ -99,10 +100,10 @@ __global__ void __launch_bounds__(RED_THREADS) norm2_kernel(const Vec *__restric
 template <typename Vec, int NCH>
 __global__ void __launch_bounds__(RED_THREADS)
 update_xr_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict__ p, const Vec *__restrict__ w, long long nvec,
-                 long long Vh, const double *zz_part, const double *ww_part, double *rr_part)
+                 long long Vh, const double *zz_part, const double *ww_part, int npart, double *rr_part)
 {
     __shared__ double sh[RED_THREADS / 32];
-    const double alpha = sum_partials(zz_part) / sum_partials(ww_part);
+    const double alpha = sum_partials(zz_part, npart) / sum_partials(ww_part, npart);
     double s = 0.0;
     constexpr int UNR = 2; // independent vectors per thread and trip (4 streams x 2 loads in flight; 4 costs occupancy)
     const long long stride = (long long)RED_BLOCKS * RED_THREADS;
@@ -132,9 +133,9 @@ update_xr_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict
 template <typename Vec>
 __global__ void __launch_bounds__(RED_THREADS)
 update_p_kernel(Vec *__restrict__ p, const Vec *__restrict__ z, long long nvec, const double *zz_new_part, const double *zz_old_part,
-                const double *rr_part, double *hist_k)
+                int npart, const double *rr_part, double *hist_k)
 {
-    const double beta = sum_partials(zz_new_part) / sum_partials(zz_old_part);
+    const double beta = sum_partials(zz_new_part, npart) / sum_partials(zz_old_part, npart);
     if (blockIdx.x == 0) { // (block-uniform branch: sum_partials has barriers)
         const double rr = sum_partials(rr_part);
         if (threadIdx.x == 0) *hist_k = sqrt(rr);
@@ -320,24 +321,27 @@ static int cgnr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const 
     const double a0 = 4.0 + mass;
 
     // workspace lives in the gauge handle (a 0.5 GB cudaMalloc / cudaFree per solve costs up to a second)
-    const size_t nsc = 4 * (size_t)RED_BLOCKS + (size_t)max_iter + 1; // zz_part[2][RED] | ww_part | rr_part | hist
+    // |Mhat p|^2 and |Mhat^dag r|^2 come out of the matvec's epilogue as one partial per CTA of that kernel
+    const int npart = (int)((Vh + 127) / 128);
+    const size_t nsc = 3 * (size_t)npart + RED_BLOCKS + (size_t)max_iter + 1; // zz_part[2][npart] | ww_part | rr_part | hist
     if ((*err = ensure_workspace(g, 5 * hb, nsc)) != cudaSuccess) return -1;
     char *ws = (char *)g->cg_ws;
     double *sc = g->cg_sc;
     Vec *r = (Vec *)ws, *p = (Vec *)(ws + hb), *z = (Vec *)(ws + 2 * hb), *w = (Vec *)(ws + 3 * hb), *tmp = (Vec *)(ws + 4 * hb);
     Vec *x = (Vec *)x_out;
-    double *zz_part[2] = {sc, sc + RED_BLOCKS}, *ww_part = sc + 2 * RED_BLOCKS, *rr_part = sc + 3 * RED_BLOCKS;
-    double *hist = sc + 4 * RED_BLOCKS;
+    double *zz_part[2] = {sc, sc + npart}, *ww_part = sc + 2 * (size_t)npart, *rr_part = sc + 3 * (size_t)npart;
+    double *hist = rr_part + RED_BLOCKS;
 
     ApplyArgs a = shape;
-    auto schur = [&](Vec *out, const Vec *in, bool dagger) -> cudaError_t { // out = Mhat in   or   Mhat^dagger in
+    // out = Mhat in  or  Mhat^dagger in;  norm_part receives the per-CTA partials of |out|^2
+    auto schur = [&](Vec *out, const Vec *in, bool dagger, double *norm_part) -> cudaError_t {
         a.out = tmp;
         a.in = in;
         cudaError_t e = launch_eo(a, nullptr, 0.0, -0.5, 1 - parity, dagger);
         if (e != cudaSuccess) return e;
         a.out = out;
         a.in = tmp;
-        return launch_eo(a, in, a0, 0.5 / a0, parity, dagger);
+        return launch_eo(a, in, a0, 0.5 / a0, parity, dagger, norm_part);
     };
     auto norm2 = [&](const Vec *v, double *part) {
         norm2_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(v, nvec, Vh, part);
@@ -354,10 +358,9 @@ static int cgnr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const 
         zero_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, nvec);
         count_launch();
         if ((e = cudaMemcpyAsync(r, b_in, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
-        if ((e = schur(z, r, true)) != cudaSuccess) { fail_cuda(e); break; }
-        if ((e = cudaMemcpyAsync(p, z, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
         int cur = 0;
-        norm2(z, zz_part[cur]);
+        if ((e = schur(z, r, true, zz_part[cur])) != cudaSuccess) { fail_cuda(e); break; }
+        if ((e = cudaMemcpyAsync(p, z, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
         norm2(r, rr_part);
         sqrt_of_sum_kernel<<<1, 32, 0, s>>>(rr_part, hist);
         count_launch();
@@ -367,13 +370,11 @@ static int cgnr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const 
             if (h0 == 0.0) break; // b = 0: x = 0 is the solution
         }
         for (k = 0; k < max_iter; ++k) {
-            if ((e = schur(w, p, false)) != cudaSuccess) { fail_cuda(e); break; }
-            norm2(w, ww_part);
-            update_xr_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, r, p, w, nvec, Vh, zz_part[cur], ww_part, rr_part);
+            if ((e = schur(w, p, false, ww_part)) != cudaSuccess) { fail_cuda(e); break; }
+            update_xr_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, r, p, w, nvec, Vh, zz_part[cur], ww_part, npart, rr_part);
             count_launch();
-            if ((e = schur(z, r, true)) != cudaSuccess) { fail_cuda(e); break; }
-            norm2(z, zz_part[cur ^ 1]);
-            update_p_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(p, z, nvec, zz_part[cur ^ 1], zz_part[cur], rr_part, hist + k + 1);
+            if ((e = schur(z, r, true, zz_part[cur ^ 1])) != cudaSuccess) { fail_cuda(e); break; }
+            update_p_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(p, z, nvec, zz_part[cur ^ 1], zz_part[cur], npart, rr_part, hist + k + 1);
             count_launch();
             cur ^= 1;
             if (tol > 0.0 && ((k + 1) % CHECK == 0 || k + 1 == max_iter)) {

@@ -26,10 +26,14 @@ constexpr int EO_THREADS = 128;
 template <typename T, int RECON, int SGN>
 __global__ void __launch_bounds__(EO_THREADS)
 dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ xin, const T *__restrict__ links,
-                 int Lx, int Ly, int Lz, int Lt, long long Vh, T alpha, T beta, int parity)
+                 int Lx, int Ly, int Lz, int Lt, long long Vh, T alpha, T beta, int parity, double *__restrict__ norm_part)
 {
-    const long long cb = (long long)blockIdx.x * EO_THREADS + threadIdx.x;
-    if (cb >= Vh) return;
+    // norm_part (may be NULL): per-CTA partial sums of |out|^2 in fp64, fixed order -- lets a solver take the norm of
+    // the result without another pass over it (wd_cg.cu)
+    const long long cb_raw = (long long)blockIdx.x * EO_THREADS + threadIdx.x;
+    const bool valid = cb_raw < Vh;
+    if (!valid && !norm_part) return;
+    const long long cb = valid ? cb_raw : Vh - 1; // (only the last CTA has such threads; they redo a site and drop it)
     const long long Vhp = padded_volume(Vh); // sites per right-hand side of a half field
     in += (long long)blockIdx.y * 24 * Vhp;
     out += (long long)blockIdx.y * 24 * Vhp;
@@ -70,11 +74,28 @@ dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restr
 #pragma unroll
         for (int i = 0; i < 24; ++i) acc[i] = beta * acc[i];
     }
-    store_spinor(out, cb, acc);
+    if (valid) store_spinor(out, cb, acc);
+    if (norm_part) {
+        __shared__ double sh[EO_THREADS / 32];
+        double s2 = 0.0;
+        if (valid)
+#pragma unroll
+            for (int i = 0; i < 24; ++i) s2 += (double)acc[i] * acc[i];
+        for (int o = 16; o > 0; o >>= 1) s2 += __shfl_down_sync(0xffffffffu, s2, o);
+        if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s2;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = 0.0;
+#pragma unroll
+            for (int i = 0; i < EO_THREADS / 32; ++i) t += sh[i];
+            norm_part[(long long)blockIdx.y * gridDim.x + blockIdx.x] = t;
+        }
+    }
 }
 
 template <typename T, int RECON>
-static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger)
+static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger,
+                               double *norm_part)
 {
     const long long Vh = a.V / 2;
     const long long nb = (Vh + EO_THREADS - 1) / EO_THREADS;
@@ -82,19 +103,21 @@ static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha
     dim3 grid((unsigned)nb, (unsigned)a.nrhs);
     auto kern = dagger ? dslash_eo_kernel<T, RECON, +1> : dslash_eo_kernel<T, RECON, -1>;
     kern<<<grid, EO_THREADS, 0, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)xin, (const T *)a.links, a.dims[0],
-                                             a.dims[1], a.dims[2], a.dims[3], Vh, (T)alpha, (T)beta, parity);
+                                             a.dims[1], a.dims[2], a.dims[3], Vh, (T)alpha, (T)beta, parity, norm_part);
     count_launch();
     return cudaGetLastError();
 }
 
 // out_p = alpha * xin_p + beta * (sum of the eight projected, link-multiplied hops from parity 1-p); xin may be NULL
-cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger)
+// norm_part: NULL, or ceil(Vh / 128) * nrhs doubles that receive per-CTA partial sums of |out|^2
+cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger,
+                      double *norm_part)
 {
     if (a.precision == 32)
-        return a.recon == 18 ? launch_eo_t<float, 18>(a, xin, alpha, beta, parity, dagger)
-                             : launch_eo_t<float, 12>(a, xin, alpha, beta, parity, dagger);
-    return a.recon == 18 ? launch_eo_t<double, 18>(a, xin, alpha, beta, parity, dagger)
-                         : launch_eo_t<double, 12>(a, xin, alpha, beta, parity, dagger);
+        return a.recon == 18 ? launch_eo_t<float, 18>(a, xin, alpha, beta, parity, dagger, norm_part)
+                             : launch_eo_t<float, 12>(a, xin, alpha, beta, parity, dagger, norm_part);
+    return a.recon == 18 ? launch_eo_t<double, 18>(a, xin, alpha, beta, parity, dagger, norm_part)
+                         : launch_eo_t<double, 12>(a, xin, alpha, beta, parity, dagger, norm_part);
 }
 
 // canonical full-lattice field <-> native half field of one parity (pure data movement)

@@ -69,7 +69,8 @@ cudaError_t launch_pack_spinor(void *native, const void *canonical, long long V,
 cudaError_t launch_unpack_spinor(void *canonical, const void *native, long long V, int nrhs, int precision,
                                  cudaStream_t s, long long site0 = 0, long long nsites = -1);
 // red/black blocks (wd_dslash_eo.cu): out_p = alpha * xin_p + beta * hops(in_q); half-field <-> canonical copies
-cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger = false);
+cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger = false,
+                      double *norm_part = nullptr);
 // CGNR for Mhat x = b on one parity (wd_cg.cu); shape carries dims, V, precision, recon, links, stream
 int cgnr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter,
                double tol, int *iters_out, double *hist_host, cudaError_t *err);
