@@ -152,6 +152,11 @@ int wd_unpack_spinor(const wd_lattice *lat, void *canonical_dev, const void *nat
 int wd_apply(void *out_native_dev, const void *in_native_dev, const wd_gauge *gauge, double mass,
              const int dims[4], int nrhs, int precision);
 
+/* wd_apply_dagger -- out[r] = D^dagger in[r] = gamma5 D gamma5 in[r] ("gamma5-Hermiticity"): every
+ * projector 1 -+ gamma_mu swapped; same arguments and checks as wd_apply; always the one-thread-per-site kernel. */
+int wd_apply_dagger(void *out_native_dev, const void *in_native_dev, const wd_gauge *gauge, double mass,
+                    const int dims[4], int nrhs, int precision);
+
 /*
  * wd_apply_host -- the same operation for callers whose data lives in HOST memory, in
  * CANONICAL layout: copies in_canonical_host to the device, packs, applies D, unpacks, copies

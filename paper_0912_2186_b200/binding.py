@@ -25,7 +25,7 @@ SYMBOLS = (
     "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
     "wd_set_kernel", "wd_set_temporal_gauge", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
     "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_coarse_reals",
-    "wd_block_orthonormalise", "wd_restrict", "wd_prolong", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
+    "wd_block_orthonormalise", "wd_restrict", "wd_prolong", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_dagger", "wd_apply_host",
     "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
 )
 
@@ -62,6 +62,7 @@ def lib():
     L.wd_pack_spinor.argtypes = [vp, vp, vp, i, i, vp]
     L.wd_unpack_spinor.argtypes = [vp, vp, vp, i, i, vp]
     L.wd_apply.argtypes = [vp, vp, vp, d, ip, i, i]
+    L.wd_apply_dagger.argtypes = [vp, vp, vp, d, ip, i, i]
     L.wd_apply_host.argtypes = [vp, vp, vp, d, ip, i, i]
     L.wd_spinor_bytes_parity.argtypes = [vp, i, i]
     L.wd_spinor_bytes_parity.restype = ctypes.c_size_t
@@ -88,7 +89,7 @@ def lib():
     L.wd_destroy.restype = None
     for name in ("wd_create_lattice", "wd_lattice_dims", "wd_load_gauge", "wd_set_stream", "wd_set_kernel",
                  "wd_set_temporal_gauge",
-                 "wd_selected_kernel", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_host",
+                 "wd_selected_kernel", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_dagger", "wd_apply_host",
                  "wd_pack_spinor_parity", "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur",
                  "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur",
                  "wd_block_orthonormalise", "wd_restrict", "wd_prolong"):
@@ -191,6 +192,11 @@ def wd_unpack_spinor(lat, canonical_dev, native_dev, nrhs, precision, stream=Non
 def wd_apply(out_native_dev, in_native_dev, gauge, mass, dims, nrhs, precision):
     _check(lib().wd_apply(_ptr(out_native_dev), _ptr(in_native_dev), gauge, float(mass), _dims(dims), int(nrhs),
                           int(precision)), "wd_apply")
+
+
+def wd_apply_dagger(out_native_dev, in_native_dev, gauge, mass, dims, nrhs, precision):
+    _check(lib().wd_apply_dagger(_ptr(out_native_dev), _ptr(in_native_dev), gauge, float(mass), _dims(dims), int(nrhs),
+                                 int(precision)), "wd_apply_dagger")
 
 
 def wd_apply_host(out_canonical_host, in_canonical_host, gauge, mass, dims, nrhs, precision):
@@ -319,6 +325,9 @@ class WilsonDirac:
     def selected_kernel(self, nrhs=1):
         """Name of the kernel wd_apply will launch for nrhs right-hand sides ("site", "tile", "stage")."""
         return KERNEL_NAMES[wd_selected_kernel(self.gauge, nrhs)]
+
+    def apply_dagger(self, out_native_dev, in_native_dev, mass, nrhs=1):
+        wd_apply_dagger(out_native_dev, in_native_dev, self.gauge, mass, self.dims, nrhs, self.precision)
 
     def native_numel(self, nrhs=1):
         """Reals in a NATIVE spinor buffer of nrhs fields (the volume is padded to 32-site blocks)."""

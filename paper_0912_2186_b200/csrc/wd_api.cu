@@ -296,6 +296,26 @@ int wd_apply(void *out_native_dev, const void *in_native_dev, const wd_gauge *ga
     return dispatch_apply(out_native_dev, in_native_dev, gauge, mass, nrhs);
 }
 
+int wd_apply_dagger(void *out_native_dev, const void *in_native_dev, const wd_gauge *gauge, double mass, const int dims[4],
+                    int nrhs, int precision)
+{
+    int rc = check_apply_args(out_native_dev, in_native_dev, gauge, dims, nrhs, precision);
+    if (rc) return rc;
+    const size_t bytes = (size_t)nrhs * (size_t)wd::padded_volume(gauge->V) * 24 * (precision == WD_FP32 ? 4 : 8);
+    if (overlap(out_native_dev, bytes, in_native_dev, bytes)) return fail(WD_ERR_ALIAS, "wd_apply_dagger: out and in overlap");
+    if (((uintptr_t)out_native_dev | (uintptr_t)in_native_dev) & 15)
+        return fail(WD_ERR_MISMATCH, "wd_apply_dagger: buffers must be 16-byte aligned");
+    wd::ApplyArgs a = shape_args(gauge, nrhs);
+    a.out = out_native_dev;
+    a.in = in_native_dev;
+    a.links = gauge->links;
+    a.mass = mass;
+    a.stream = gauge->stream;
+    a.dagger = 1;
+    cudaError_t e = wd::launch_site(a);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply_dagger: kernel launch");
+}
+
 int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_gauge *gauge, double mass,
                   const int dims[4], int nrhs, int precision)
 {

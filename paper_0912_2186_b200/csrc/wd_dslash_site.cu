@@ -16,7 +16,7 @@ namespace wd {
 
 constexpr int SITE_THREADS = 128;
 
-template <int MU, typename T, int RECON, int NR>
+template <int MU, int SGN, typename T, int RECON, int NR>
 __device__ __forceinline__ void hop_pair(T (&acc)[NR][24], const T *__restrict__ in, const T *__restrict__ links,
                                          long long Vp, long long site, long long sf, long long sb, int rhs0, int nrhs)
 {
@@ -27,7 +27,7 @@ __device__ __forceinline__ void hop_pair(T (&acc)[NR][24], const T *__restrict__
         if (rhs0 + r < nrhs) {
             T p[24];
             load_spinor(in + (long long)(rhs0 + r) * 24 * Vp, sf, p); // psi(x+mu)
-            hop_forward<MU>(acc[r], u, p);
+            hop_forward_s<MU, SGN>(acc[r], u, p);
         }
     load_link<MU, T, RECON>(links, sb, u); // U_mu(x-mu)
 #pragma unroll
@@ -35,11 +35,12 @@ __device__ __forceinline__ void hop_pair(T (&acc)[NR][24], const T *__restrict__
         if (rhs0 + r < nrhs) {
             T p[24];
             load_spinor(in + (long long)(rhs0 + r) * 24 * Vp, sb, p); // psi(x-mu)
-            hop_backward<MU>(acc[r], u, p);
+            hop_backward_s<MU, SGN>(acc[r], u, p);
         }
 }
 
-template <typename T, int RECON, int NR>
+// SGN = -1: D of eq. (2.2); SGN = +1: gamma5 D gamma5 = D^dagger, every projector swapped
+template <typename T, int RECON, int NR, int SGN>
 __global__ void __launch_bounds__(SITE_THREADS)
 dslash_site_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ links, int Lx, int Ly, int Lz,
                    int Lt, long long V, T cdiag, int nrhs, int bps, long long site0, long long nsites)
@@ -79,10 +80,10 @@ dslash_site_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__res
 #pragma unroll
         for (int i = 0; i < 24; ++i) acc[r][i] = (T)0;
 
-    hop_pair<0, T, RECON, NR>(acc, in, links, Vp, site, xf, xb, rhs0, nrhs);
-    hop_pair<1, T, RECON, NR>(acc, in, links, Vp, site, yf, yb, rhs0, nrhs);
-    hop_pair<2, T, RECON, NR>(acc, in, links, Vp, site, zf, zb, rhs0, nrhs);
-    hop_pair<3, T, RECON, NR>(acc, in, links, Vp, site, tf, tb, rhs0, nrhs);
+    hop_pair<0, SGN, T, RECON, NR>(acc, in, links, Vp, site, xf, xb, rhs0, nrhs);
+    hop_pair<1, SGN, T, RECON, NR>(acc, in, links, Vp, site, yf, yb, rhs0, nrhs);
+    hop_pair<2, SGN, T, RECON, NR>(acc, in, links, Vp, site, zf, zb, rhs0, nrhs);
+    hop_pair<3, SGN, T, RECON, NR>(acc, in, links, Vp, site, tf, tb, rhs0, nrhs);
 
     // fused diagonal (step a6): out = (4+m) psi(x) - 1/2 acc
 #pragma unroll
@@ -116,7 +117,8 @@ static cudaError_t launch_site_t(const ApplyArgs &a)
     if (bps < 1) bps = 1;
     dim3 grid((unsigned)(nb * ngroups));
     const T cdiag = (T)(4.0 + a.mass); // formed in double, rounded once (reading S8)
-    dslash_site_kernel<T, RECON, NR><<<grid, SITE_THREADS, 0, a.stream>>>(
+    auto kern = a.dagger ? dslash_site_kernel<T, RECON, NR, +1> : dslash_site_kernel<T, RECON, NR, -1>;
+    kern<<<grid, SITE_THREADS, 0, a.stream>>>(
         (T *)a.out, (const T *)a.in, (const T *)a.links, a.dims[0], a.dims[1], a.dims[2], a.dims[3], a.V, cdiag, a.nrhs,
         (int)bps, site0, nsites);
     count_launch();

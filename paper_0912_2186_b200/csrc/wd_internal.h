@@ -48,6 +48,7 @@ struct ApplyArgs {
     int precision;
     int recon;
     cudaStream_t stream;
+    int dagger;                     // site kernel only: apply D^dagger = gamma5 D gamma5 instead of D
     int tgauge;                     // links are in temporal gauge (U_t = 1 for t < Lt-1): kernels may skip them
     long long site_begin, site_end; // site kernel only: apply on [site_begin, site_end); 0,0 = whole lattice
 };

@@ -349,6 +349,44 @@ def test_apply_host_pipelined_path(oracle, monkeypatch, dims, precision, recon, 
         assert rel_l2(out[r], want[r]) <= TOL[precision]
 
 
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 4, 12, 6), (3, 5, 2, 7), (2, 2, 2, 2), (16, 8, 8, 6)])
+@pytest.mark.parametrize("precision,recon", [(64, 18), (32, 18), (32, 12), (64, 12)])
+def test_apply_dagger_matches_the_oracle_and_gamma5_hermiticity(oracle, dims, precision, recon):
+    """wd_apply_dagger = D^dagger = gamma5 D gamma5: against the oracle's sign=+1 operator, and
+    <phi, D^dagger psi> = <D phi, psi> with both sides from the CUDA path."""
+    import torch
+    cfg = fields.Config("dag", dims, precision, "haar", recon, -0.3, 2, 91)
+    U, psi = fields.make_fields(cfg)
+    Uo = oracle_links(U, recon).astype(np.float64)
+    op = GpuOp(U, dims, precision, recon)
+    w = op.op
+    canon = torch.from_numpy(psi).cuda()
+    n = w.native_numel(2)
+    a = torch.empty(n, dtype=canon.dtype, device="cuda")
+    b = torch.empty_like(a)
+    c = torch.empty_like(a)
+    out = torch.empty_like(canon)
+    w.pack(a, canon, 2)
+    w.apply_dagger(b, a, cfg.mass, 2)
+    w.unpack(out, b, 2)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    for r in range(2):
+        want = oracle.apply(psi[r].astype(np.float64), Uo, dims, cfg.mass, sign=+1)
+        assert rel_l2(got[r], want) <= TOL[precision]
+    w.apply(c, a, cfg.mass, 2)                      # D psi_0, D psi_1
+    dout = torch.empty_like(canon)
+    w.unpack(dout, c, 2)
+    torch.cuda.synchronize()
+    d = dout.cpu().numpy().astype(np.float64)
+    cplx = lambda v: v[..., 0] + 1j * v[..., 1]
+    phi, ps = cplx(psi[0].astype(np.float64)), cplx(psi[1].astype(np.float64))
+    lhs = np.vdot(phi, cplx(got[1].astype(np.float64)))        # <phi, D^dagger psi>
+    rhs = np.vdot(cplx(d[0]), ps)                              # <D phi, psi>
+    assert abs(lhs - rhs) <= (1e-11 if precision == 64 else 2e-4) * abs(rhs) + (1e-9 if precision == 64 else 1e-2)
+    op.close()
+
+
 def test_auto_kernel_selection():
     """WD_KERNEL_AUTO resolves by lattice, precision and nrhs; a forced kernel is reported."""
     from paper_0912_2186_b200 import binding
