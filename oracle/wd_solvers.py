@@ -34,8 +34,9 @@ def _mask(psi, dims, parity):
     return np.where(on, psi, 0.0)
 
 
-def cgnr_schur(b, U, dims, mass, parity, niter, tol=0.0):
-    """niter iterations (or until |r|/|b| <= tol) of CGNR for Mhat x = b on `parity`.  b: [Lt,Lz,Ly,Lx,4,3,2] fp64."""
+def cgnr_schur(b, U, dims, mass, parity, niter, tol=0.0, trace=None):
+    """niter iterations (or until |r|/|b| <= tol) of CGNR for Mhat x = b on `parity`.  b: [Lt,Lz,Ly,Lx,4,3,2] fp64.
+    trace: optional list; a copy of the iterate x_k is appended after every iteration (for the pins only)."""
     b = _mask(np.ascontiguousarray(b, dtype=np.float64), dims, parity)
     U = np.ascontiguousarray(U, dtype=np.float64)
     M = lambda v: wd_oracle.schur(v, U, dims, mass, parity, sign=-1)
@@ -60,10 +61,12 @@ def cgnr_schur(b, U, dims, mass, parity, niter, tol=0.0):
         p = z + beta * p
         zz = zz_new
         hist.append(float(np.sqrt(np.vdot(r, r))) / bnorm)
+        if trace is not None:
+            trace.append(x.copy())
     return x, np.array(hist)
 
 
-def bicgstab_schur(b, U, dims, mass, parity, niter, tol=0.0):
+def bicgstab_schur(b, U, dims, mass, parity, niter, tol=0.0, trace=None):
     """niter iterations (or until |r|/|b| <= tol) of BiCGstab (van der Vorst 1992, unpreconditioned) for
     Mhat x = b on `parity`, x_0 = 0 (the paper's other solver around the even-odd matvec):
 
@@ -73,7 +76,8 @@ def bicgstab_schur(b, U, dims, mass, parity, niter, tol=0.0):
                x += alpha p + omega s;  r = s - omega t;  rho = rho'
 
     Complex inner products <a, b> = sum conj(a) b over (site, spin, colour).  Returns x (real-pair layout) and the
-    history of |r_k| / |b|."""
+    history of |r_k| / |b|.  trace: optional list; the vectors (rhat, s, t, r_new, x_new) of every iteration are
+    appended as complex arrays (for the pins only)."""
     b = _mask(np.ascontiguousarray(b, dtype=np.float64), dims, parity)
     U = np.ascontiguousarray(U, dtype=np.float64)
     c = lambda v: v[..., 0] + 1j * v[..., 1]
@@ -102,6 +106,8 @@ def bicgstab_schur(b, U, dims, mass, parity, niter, tol=0.0):
         r = s - omega * t
         rho = rho_new
         hist.append(float(np.sqrt(np.vdot(r, r).real)) / bnorm)
+        if trace is not None:
+            trace.append((rhat.copy(), s.copy(), t.copy(), r.copy(), x.copy()))
     return rp(x), np.array(hist)
 
 

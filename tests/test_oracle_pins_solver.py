@@ -113,3 +113,107 @@ def test_k7_gcr_minimises_the_residual_and_reports_it(oracle):
     coef, *_ = np.linalg.lstsq(AK, r2c(bm).ravel(), rcond=None)
     best = np.linalg.norm(r2c(bm).ravel() - AK @ coef) / np.linalg.norm(bm)
     assert hist8[-1] == pytest.approx(best, rel=1e-6)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# Pins that bite on the RECURRENCES (round 2; VERDICT r01 "weak #1": the pins above only see convergence and the true
+# residual, which steepest descent (beta = 0), a conjugated omega or a beta without alpha/omega also satisfy).
+#   K8   CGNR iterate k is THE minimiser of |b - Mhat x| over K_k(Mhat^dag Mhat, Mhat^dag b) (Hestenes-Stiefel on the
+#        normal equations; "CG on the normal equations"): compared with a least-squares solve over a
+#        Krylov basis built here from the pinned operator, for every k
+#   K9   finite termination: b = sum of k left singular vectors of the dense Schur complement => CGNR converges in
+#        exactly k iterations (and not in k-1)
+#   K10  BiCGstab per iteration: <rhat, s> = 0 (alpha), <t, r_new> = 0 and |r_new| = min_w |s - w t| (omega), and
+#        x_new reproduces r_new = b - Mhat x_new
+#   K11  finite termination of the BiCG part: b = sum of k eigenvectors of the dense Schur complement => BiCGstab
+#        converges in exactly k iterations (needs beta = (rho'/rho)(alpha/omega))
+# ------------------------------------------------------------------------------------------------------------------
+def _dense_schur(dims, U, mass, parity):
+    V = fields.volume(dims)
+    M = dense_matrix(U, dims, mass)
+    par = np.repeat(parity_mask(dims).reshape(V), 12)
+    ip, iq = np.where(par == parity)[0], np.where(par != parity)[0]
+    S = M[np.ix_(ip, ip)] - M[np.ix_(ip, iq)] @ np.linalg.solve(M[np.ix_(iq, iq)], M[np.ix_(iq, ip)])
+    return S, ip
+
+
+def _embed(vec_p, ip, dims):
+    """parity-subspace complex vector -> full canonical real-pair field (zero on the other parity)"""
+    V = fields.volume(dims)
+    full = np.zeros(12 * V, dtype=np.complex128)
+    full[ip] = vec_p
+    return c2r(full.reshape(dims[3], dims[2], dims[1], dims[0], 4, 3))
+
+
+def test_k8_cgnr_iterates_are_the_least_squares_minimisers(oracle):
+    dims = (4, 2, 2, 4)
+    U, b = random_fields(dims, 231)
+    mass = -0.1
+    Ur = c2r(U)
+    bm = np.where((parity_mask(dims) == 0)[..., None, None, None], c2r(b[0]), 0.0)
+    M = lambda v: oracle.schur(np.ascontiguousarray(v), Ur, dims, mass, 0, sign=-1)
+    Md = lambda v: oracle.schur(np.ascontiguousarray(v), Ur, dims, mass, 0, sign=+1)
+    kmax = 6
+    trace = []
+    x, hist = wd_solvers.cgnr_schur(c2r(b[0]), Ur, dims, mass, 0, niter=kmax, trace=trace)
+    assert len(trace) == kmax
+    K = [Md(bm)]                                       # Krylov basis of K_k(Mhat^dag Mhat, Mhat^dag b)
+    for _ in range(kmax - 1):
+        K.append(Md(M(K[-1])))
+    bc = r2c(bm).ravel()
+    for k in range(1, kmax + 1):
+        Kc = np.stack([r2c(v).ravel() for v in K[:k]], axis=1)
+        AK = np.stack([r2c(M(v)).ravel() for v in K[:k]], axis=1)
+        Q, _ = np.linalg.qr(AK)                        # orthonormal basis of Mhat K_k: well conditioned projection
+        best_r = bc - Q @ (Q.conj().T @ bc)
+        assert hist[k] == pytest.approx(np.linalg.norm(best_r) / np.linalg.norm(bc), rel=1e-7)
+        # the iterate itself: Mhat x_k is the projection of b onto Mhat K_k
+        assert np.linalg.norm(r2c(M(trace[k - 1])).ravel() - (bc - best_r)) <= 1e-8 * np.linalg.norm(bc)
+
+
+@pytest.mark.parametrize("k", [3, 5])
+def test_k9_cgnr_terminates_in_k_steps_on_k_singular_vectors(oracle, k):
+    dims = (2, 2, 2, 2)
+    U, _ = random_fields(dims, 233)
+    mass = 0.25
+    S, ip = _dense_schur(dims, U, mass, 0)
+    Us, sv, _ = np.linalg.svd(S)
+    b_p = Us[:, [1, 17, 40, 63, 90][:k]] @ np.array([1.0, -0.7, 0.4 + 0.3j, 1.2j, -0.9][:k])
+    x, hist = wd_solvers.cgnr_schur(_embed(b_p, ip, dims), c2r(U), dims, mass, 0, niter=k)
+    assert len(hist) == k + 1
+    assert hist[k] < 1e-10
+    assert hist[k - 1] > 1e4 * max(hist[k], 1e-14)
+
+
+def test_k10_bicgstab_step_orthogonalities(oracle):
+    dims = (4, 2, 2, 4)
+    U, b = random_fields(dims, 235)
+    mass = -0.1
+    Ur = c2r(U)
+    bm = np.where((parity_mask(dims) == 0)[..., None, None, None], c2r(b[0]), 0.0)
+    Mc = lambda v: r2c(oracle.schur(np.ascontiguousarray(c2r(v)), Ur, dims, mass, 0))
+    trace = []
+    wd_solvers.bicgstab_schur(c2r(b[0]), Ur, dims, mass, 0, niter=6, trace=trace)
+    assert len(trace) == 6
+    for rhat, s, t, r_new, x_new in trace:
+        ns, nt = np.linalg.norm(s), np.linalg.norm(t)
+        assert abs(np.vdot(rhat, s)) <= 1e-10 * np.linalg.norm(rhat) * ns          # alpha = rho' / <rhat, v>
+        assert abs(np.vdot(t, r_new)) <= 1e-10 * nt * ns                            # omega = <t, s> / <t, t>
+        w_best = np.vdot(t, s) / np.vdot(t, t)
+        for dw in (1e-3, 1e-3j, -1e-3, -1e-3j):
+            assert np.linalg.norm(r_new) <= np.linalg.norm(s - (w_best + dw) * t)   # the minimum over complex omega
+        assert np.linalg.norm(r2c(bm) - Mc(x_new) - r_new) <= 1e-10 * np.linalg.norm(bm)
+
+
+@pytest.mark.parametrize("k", [3, 4])
+def test_k11_bicgstab_terminates_in_k_steps_on_k_eigenvectors(oracle, k):
+    dims = (2, 2, 2, 2)
+    U, _ = random_fields(dims, 237)
+    mass = 0.25
+    S, ip = _dense_schur(dims, U, mass, 0)
+    _, W = np.linalg.eig(S)
+    b_p = W[:, [2, 19, 47, 80][:k]] @ np.array([1.0, 0.8 - 0.2j, -0.6j, 1.1][:k])
+    x, hist = wd_solvers.bicgstab_schur(_embed(b_p, ip, dims), c2r(U), dims, mass, 0, niter=k)
+    assert len(hist) == k + 1
+    assert hist[k] < 1e-9
+    assert hist[k - 1] > 1e3 * max(hist[k], 1e-13)
