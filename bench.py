@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the Wilson-Dirac matvec D*psi (eq. (2.2)) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--kernel auto|site|tile|stage]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--kernel auto|site|stage]
                     [--recon 18|12] [--impl wd|reference]
 
 One JSON line on stdout (rank 0).  Definitions:
@@ -18,6 +18,10 @@ One JSON line on stdout (rank 0).  Definitions:
                H2D copy + pack + apply + unpack + D2H copy + sync inside the timed region.
   * roofline   HBM: algorithmic (compulsory) bytes per launch / mean launch duration, against
                MEASURED_PEAKS.json:hbm_gbs.
+  * secondary  (default run only) two short legs after the headline timing, same launch path, own clocks record:
+               configs[4] = 24 right-hand sides (2 steps x 10 applies; roofline.frac against the HBM peak, plus
+               frac_of_own_peak against min(HBM bound, FMA-pipe bound at the observed clock)) and configs[3] in fp64
+               (2 steps x 25 applies).  The headline's metric, config and value are unchanged.
   * cpu_baseline  the oracle (oracle/wd_oracle.c, fp64, OpenMP) on this box's host cores, on a
                bounded sample of the same workload.
 Multi-GPU (torchrun): the path has no exchange step on one GPU per lattice; ranks run independent
@@ -216,6 +220,117 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def issue_bound_gbs(precision, recon, nrhs, sm_mhz):
+    """FP32/FP64-pipe ceiling of a multi-RHS apply expressed in the roofline's unit (algorithmic GB/s): the SASS of
+    the staged kernels spends ~912 FMA-pipe cycles per 32 (site, rhs) (profiles/r02_ubench.md: FFMA2 2 clk, scalar
+    FADD/FMUL 1 clk per warp instruction and SMSP), i.e. 148 SMs x 4 SMSPs x 32 / 912 (site, rhs) per clock."""
+    if sm_mhz is None:
+        return None
+    per_clk = 148 * 4 * 32 / (912.0 if precision == 32 else 2 * 912.0)
+    site_rhs_per_s = per_clk * sm_mhz * 1e6
+    return site_rhs_per_s / nrhs * compulsory_bytes_per_site(precision, recon, nrhs) / 1e9
+
+
+def secondary_leg(binding, torch, dev, stream, local, name, U, recon, nrhs, steps, aps):
+    """One short timed leg of another BASELINE workload (north_star: "the batched 24-RHS apply reported in Gflop/s
+    and as a fraction of its own roofline"; configs[3] is "fp64 and fp32").  Links: the array handed in (same recipe
+    and shape as the workload's); spinors: complex Gaussian drawn on the device (seeded torch generator) straight into
+    the native buffers -- the native layout is a permutation of the canonical one, so the distribution is the same."""
+    cfg = fields.CONFIGS[name]
+    V = fields.volume(cfg.dims)
+    tdt = torch.float32 if cfg.precision == 32 else torch.float64
+    nbuf = 2 if nrhs > 1 else NBUF
+    with torch.cuda.stream(stream):
+        u_dev = torch.from_numpy(fields.round_to(U, cfg.precision)).to(dev)
+        op = binding.WilsonDirac(cfg.dims, u_dev, cfg.precision, recon, stream=stream.cuda_stream)
+        g = torch.Generator(device=dev).manual_seed(cfg.seed + 1000)
+        ins = [torch.randn(op.native_numel(nrhs), dtype=tdt, device=dev, generator=g) for _ in range(nbuf)]
+        outs = [torch.empty(op.native_numel(nrhs), dtype=tdt, device=dev) for _ in range(nbuf)]
+    stream.synchronize()
+    del u_dev
+
+    def step():
+        for i in range(aps):
+            op.apply(outs[i % nbuf], ins[i % nbuf], cfg.mass, nrhs)
+
+    for _ in range(3):
+        step()
+    torch.cuda.synchronize()
+    n0 = binding.wd_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clocks:
+        ev0.record(stream)
+        for _ in range(steps):
+            step()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / (steps * aps)
+    launches = binding.wd_launch_count() - n0
+    kern = op.selected_kernel(nrhs)
+    op.close()
+    del ins, outs
+    torch.cuda.empty_cache()
+    bytes_per_launch = compulsory_bytes_per_site(cfg.precision, recon, nrhs) * V
+    peak, peak_src = measured_peak()
+    achieved = bytes_per_launch / (ms * 1e-3) / 1e9
+    ck = clocks.summary()
+    roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": ncu_traffic(name, recon), "peak_source": peak_src, "bytes_per_launch": bytes_per_launch,
+            "kernel": "wd dslash, " + kern + " kernel" + (" (multi-RHS member)" if nrhs > 1 and kern == "stage" else "")}
+    if nrhs > 1:  # its own roofline = min(HBM bound, FMA-pipe bound at the observed clock); both printed
+        ib = issue_bound_gbs(cfg.precision, recon, nrhs, ck["sm_mhz"])
+        roof["fma_pipe_bound_gbs"] = ib
+        roof["own_peak"] = min(peak, ib) if ib else peak
+        roof["frac_of_own_peak"] = achieved / roof["own_peak"]
+    return {"workload": name, "value": FLOPS_PER_SITE * V * nrhs / (ms * 1e-3) / 1e9, "unit": UNIT, "nrhs": nrhs,
+            "recon": recon, "dtype": "f32" if cfg.precision == 32 else "f64", "us_per_apply": ms * 1e3,
+            "steps": steps, "applies_per_step": aps, "gpu_launches": int(launches),
+            "data": "synthetic: headline links recipe (smooth, eps=0.3), device-drawn Gaussian spinors",
+            "roofline": roof, "clocks": ck}
+
+
+def run_wd_device_inputs(args, torch, binding, cfg, recon, nrhs, dev, local, kernel):
+    """--device-inputs: a quick timing-only run for kernel work (sweeps, ncu captures): links and spinors are
+    N(0,1)/2 numbers drawn on the device (the kernels' cost is data independent), no e2e leg, no oracle leg.
+    Its line says data = "device-random (timing only)" and is never a bench record."""
+    V = fields.volume(cfg.dims)
+    tdt = torch.float32 if cfg.precision == 32 else torch.float64
+    stream = torch.cuda.Stream(device=dev)
+    nbuf = 2 if nrhs > 1 else NBUF
+    with torch.cuda.stream(stream):
+        g = torch.Generator(device=dev).manual_seed(cfg.seed)
+        Lx, Ly, Lz, Lt = cfg.dims
+        u_dev = torch.randn((4, Lt, Lz, Ly, Lx, 3, 3, 2), dtype=tdt, device=dev, generator=g) * 0.5
+        op = binding.WilsonDirac(cfg.dims, u_dev, cfg.precision, recon, stream=stream.cuda_stream, kernel=kernel)
+        ins = [torch.randn(op.native_numel(nrhs), dtype=tdt, device=dev, generator=g) for _ in range(nbuf)]
+        outs = [torch.empty(op.native_numel(nrhs), dtype=tdt, device=dev) for _ in range(nbuf)]
+    stream.synchronize()
+    del u_dev
+    aps = args.applies_per_step
+    for _ in range(max(args.warmup, 3) * aps):
+        op.apply(outs[0], ins[0], cfg.mass, nrhs)
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clocks:
+        ev0.record(stream)
+        for i in range(args.steps * aps):
+            op.apply(outs[i % nbuf], ins[i % nbuf], cfg.mass, nrhs)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / (args.steps * aps)
+    bytes_per_launch = compulsory_bytes_per_site(cfg.precision, recon, nrhs) * V
+    peak, peak_src = measured_peak()
+    achieved = bytes_per_launch / (ms * 1e-3) / 1e9
+    line = {"metric": METRIC, "value": FLOPS_PER_SITE * V * nrhs / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "data": "device-random (timing only)",
+            "config": {"workload": cfg.name, "recon": recon, "nrhs": nrhs, "kernel": args.kernel, "applies_per_step": aps},
+            "us_per_apply": ms * 1e3, "clocks": clocks.summary(),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "peak_source": peak_src, "kernel": op.selected_kernel(nrhs)}}
+    print(json.dumps(line), flush=True)
+    op.close()
+    return line
+
 def run_wd(args):
     import torch
     from paper_0912_2186_b200 import binding, build
@@ -235,12 +350,16 @@ def run_wd(args):
     nrhs = args.nrhs if args.nrhs else cfg.nrhs
     V = fields.volume(cfg.dims)
     tdt = torch.float32 if cfg.precision == 32 else torch.float64
-    kernel = {"auto": binding.WD_KERNEL_AUTO, "site": binding.WD_KERNEL_SITE, "tile": binding.WD_KERNEL_TILE,
+    kernel = {"auto": binding.WD_KERNEL_AUTO, "site": binding.WD_KERNEL_SITE,
               "stage": binding.WD_KERNEL_STAGE}[args.kernel]
 
     # ---- synthetic inputs (each rank its own replica: seeds shifted by rank) -------------------
     cfg_r = rank_config(cfg, recon, nrhs, rank)
+    if args.device_inputs:
+        return run_wd_device_inputs(args, torch, binding, cfg, recon, nrhs, dev, local, kernel)
     U, psi = fields.make_fields(cfg_r)
+    want_secondary = (world == 1 and args.workload == "c3_32x64_fp32" and not args.no_secondary and args.nrhs is None
+                      and not args.temporal_gauge and args.kernel == "auto")
     if args.temporal_gauge:
         U, _ = fields.temporal_gauge(U, cfg.precision)
     stream = torch.cuda.Stream(device=dev)
@@ -309,6 +428,16 @@ def run_wd(args):
     e2e_value = whole_job_gflops(world, e2e_applies, flops_per_apply, e2e_ms)
     field_bytes = nrhs * V * 24 * (4 if cfg.precision == 32 else 8)
 
+    secondary = None
+    if want_secondary:
+        # free the headline's device buffers first (24 RHS need 2 x 2 x 4.8 GB)
+        del ins, outs, h_in, h_out
+        torch.cuda.empty_cache()
+        secondary = [
+            secondary_leg(binding, torch, dev, stream, local, "c4_32x64_fp32_24rhs", U, 18, 24, 2, 10),
+            secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp64", U, 18, 1, 2, 25),
+        ]
+
     line = None
     if rank == 0:
         cpu = oracle_rate(cfg_r, U, psi) if (world == 1 and not args.no_cpu_baseline) else None
@@ -338,6 +467,8 @@ def run_wd(args):
         }
         if cpu is not None:
             line["cpu_baseline"] = cpu
+        if secondary is not None:
+            line["secondary"] = secondary
         print(json.dumps(line), flush=True)
     op.close()
     if world > 1:
@@ -551,7 +682,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="c3_32x64_fp32", choices=sorted(fields.CONFIGS))
-    ap.add_argument("--kernel", default="auto", choices=["auto", "site", "tile", "stage"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "site", "stage"])
     ap.add_argument("--recon", type=int, default=None, choices=[18, 12])
     ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
     ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr", "bicgstab", "gcr", "transfer"],
@@ -562,6 +693,10 @@ def main():
                     help="gauge-fix the synthetic links to temporal gauge and let the kernel skip the unit t-links "
                          "(PAPER.md:157; row f4); algorithmic bytes then count 3 links + the last slice's t-links")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--device-inputs", action="store_true",
+                    help="timing-only quick mode for kernel work: device-drawn random links and spinors, no e2e/oracle legs")
+    ap.add_argument("--no-secondary", action="store_true",
+                    help="skip the short legs for configs[4] (24 RHS) and configs[3] in fp64 that the default run adds")
     ap.add_argument("--applies-per-step", type=int, default=APPLIES_PER_STEP,
                     help="wd_apply calls per step (default 100 = configs[3]; lower it only for profiling)")
     args = ap.parse_args()

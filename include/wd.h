@@ -69,8 +69,9 @@ typedef enum { WD_RECON_18 = 18, WD_RECON_12 = 12 } wd_recon; /* reals stored pe
 typedef enum {
     WD_KERNEL_AUTO = 0,    /* fastest kernel valid for the lattice                         */
     WD_KERNEL_SITE = 1,    /* one thread per site, neighbours straight from L1/L2, any dims */
-    WD_KERNEL_TILE = 2,    /* shared-memory tiled kernel (needs dims it supports)          */
-    WD_KERNEL_STAGE = 3    /* tiled kernel, all global reads staged by cp.async (fp32)     */
+    /* 2 was the round-1 tile kernel: superseded by the staged kernel on every measured case, removed */
+    WD_KERNEL_STAGE = 3    /* t-marching tile kernel, all global reads staged by cp.async (fp32 and fp64; its multi-RHS
+                              member shares the staged links between right-hand sides in fp32) */
 } wd_kernel;
 
 typedef struct wd_lattice wd_lattice; /* opaque: extents, volume                           */
@@ -103,8 +104,21 @@ long long wd_lattice_volume(const wd_lattice *lat);
 int wd_load_gauge(const wd_lattice *lat, const void *links_canonical_dev, int precision, int recon,
                   void *stream, wd_gauge **gauge);
 
-/* Stream (cudaStream_t as void*) on which wd_apply / pack / unpack for this gauge launch. */
+/* Stream (cudaStream_t as void*) on which every entry point that takes a wd_gauge launches from now on: wd_apply,
+ * wd_apply_dagger, wd_apply_hop / _schur, the solvers, wd_set_temporal_gauge, wd_apply_host (which also uses three
+ * private streams, ordered after and before this one).  Work already queued on the previous stream (the link conversion
+ * of wd_load_gauge, earlier applies) is ordered BEFORE anything launched on the new stream (event record + wait).
+ * wd_pack_spinor / wd_unpack_spinor / the transfer operators take their own stream argument and are NOT tied to the
+ * gauge's stream: the caller orders them. */
 int wd_set_stream(wd_gauge *gauge, void *stream);
+
+/* Tuning variables of the launchers.  They are read from the environment ONCE, at wd_load_gauge
+ * (WD_TILE_SHAPE=ty,tz, WD_TILE_TC, WD_TILE_NCHUNK, WD_TILE_NRB, WD_MRHS_PATCH, WD_STAGE_NO_MRHS, WD_SITE_SLAB_MB,
+ * WD_HOST_NO_PIPELINE, WD_MRHS_NO_TAIL), and stored in the gauge handle; no launch reads the environment.
+ * wd_set_tuning changes one of them afterwards: name is the lower-case variable without the WD_ prefix ("tile_ty",
+ * "tile_tz", "tile_tc", "tile_nchunk", "tile_nrb", "mrhs_patch", "stage_no_mrhs", "site_slab_mb", "host_no_pipeline",
+ * "mrhs_no_tail"); value < 0 restores the default.  WD_ERR_MISMATCH for an unknown name.  Host-only. */
+int wd_set_tuning(wd_gauge *gauge, const char *name, int value);
 
 /* Temporal gauge ("temporal gauge fixing", Fig. 4 / Table 2 "GF"): on != 0 declares that the loaded links
  * satisfy U_t(x,t) = 1 for every t < Lt-1 (the last slice carries the Polyakov lines).  The library verifies it
@@ -153,7 +167,8 @@ int wd_apply(void *out_native_dev, const void *in_native_dev, const wd_gauge *ga
              const int dims[4], int nrhs, int precision);
 
 /* wd_apply_dagger -- out[r] = D^dagger in[r] = gamma5 D gamma5 in[r] ("gamma5-Hermiticity"): every
- * projector 1 -+ gamma_mu swapped; same arguments and checks as wd_apply; always the one-thread-per-site kernel. */
+ * projector 1 -+ gamma_mu swapped; same arguments, checks and kernel selection as wd_apply (the staged kernel is
+ * templated on the projector sign; several right-hand sides go through its single-RHS member). */
 int wd_apply_dagger(void *out_native_dev, const void *in_native_dev, const wd_gauge *gauge, double mass,
                     const int dims[4], int nrhs, int precision);
 

@@ -87,3 +87,85 @@ def coarse_apply(W, c, U, dims, mass, block=BLOCK):
     psi = prolong(W, c, dims, block)
     dpsi = wd_oracle.apply(np.ascontiguousarray(np.stack([psi.real, psi.imag], axis=-1)), U, dims, mass)
     return restrict(W, dpsi[..., 0] + 1j * dpsi[..., 1], dims, block)
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# The coarse operator as an explicit nearest-neighbour stencil (PAPER.md:82-88 Galerkin form Dhat = P^dagger D P;
+# PAPER.md:116 4^4 blocks x chirality; "N_V x N_V complex matrix operations needed for the coarse
+# operators").  D of eq. (2.2) couples nearest neighbours only, so Dhat couples a block to itself and to its 8
+# neighbouring blocks.  With the coarse index i = sigma * N_v + alpha (n = 2 N_v per block) and W^sigma_alpha the basis
+# vector restricted to chirality sigma, the definition written out is
+#
+#   S[b][0]       = A(b)     = sum_{x in b} W(x)^dag [ (4+m) W(x) + sum over the 8 hops whose source site is ALSO in b ]
+#   S[b][1 + mu]  = F_mu(b)  = sum_{x in b, x+mu in b+mu}  W(x)^dag [ -1/2 (1 - gamma_mu) U_mu(x)          W(x+mu) ]
+#   S[b][5 + mu]  = B_mu(b)  = sum_{x in b, x-mu in b-mu}  W(x)^dag [ -1/2 (1 + gamma_mu) U_mu(x-mu)^dag   W(x-mu) ]
+#
+#   (Dhat c)(b) = A(b) c(b) + sum_mu [ F_mu(b) c(b+mu) + B_mu(b) c(b-mu) ]          (periodic coarse lattice)
+#
+# "x+mu in b+mu" means the hop leaves the block through its +mu face (x_mu mod 4 == 3), whatever block it lands in: with
+# coarse extent 1 or 2 the block b+mu coincides with b or with b-mu and the terms simply add (reading S4 carried over).
+# Explicit dense gamma matrices (wd_oracle.gamma), np.roll for the periodic shifts; no blocking or fusion.
+# ----------------------------------------------------------------------------------------------------------------------
+def _site_axis(mu):
+    """axis of direction mu (0..3 = x,y,z,t) in a [Lt, Lz, Ly, Lx, ...] array"""
+    return 3 - mu
+
+
+def coarse_stencil(W, U, dims, mass, block=BLOCK):
+    """W complex [Nv, Lt,Lz,Ly,Lx, 4,3] (the columns of P, eq. (2.7)); U real-pair canonical links [4, Lt,Lz,Ly,Lx,3,3,2].
+    Returns S complex [Bt,Bz,By,Bx, 9, n, n], n = 2 Nv, row/column index sigma * Nv + alpha, matrices ordered
+    (A, F_x, F_y, F_z, F_t, B_x, B_y, B_z, B_t)."""
+    check_dims(dims, block)
+    W = np.asarray(W, dtype=np.complex128)
+    nv = W.shape[0]
+    Uc = np.asarray(U, dtype=np.float64)
+    Uc = Uc[..., 0] + 1j * Uc[..., 1]                                   # [4, Lt,Lz,Ly,Lx, 3,3]
+    Lx, Ly, Lz, Lt = dims
+    coords = np.meshgrid(np.arange(Lt), np.arange(Lz), np.arange(Ly), np.arange(Lx), indexing="ij")   # t, z, y, x
+    nb = (Lt // block[3], Lz // block[2], Ly // block[1], Lx // block[0])
+    S = np.zeros(nb + (9, 2, nv, 2, nv), dtype=np.complex128)          # [.., k, sigma, alpha, sigma', alpha']
+    Wb = _blocked(W, dims, block)                                      # [Nv, B.., sigma, sites x spin-in-chirality x colour]
+
+    def accumulate(k, H, sp, mask):
+        """S[.., k, sigma, alpha, sp, alpha'] += sum over the masked sites of conj(W_alpha) . H_alpha' (rows in sigma)"""
+        Hb = _blocked(H * mask[None, ..., None, None], dims, block)    # [Nv', B.., sigma, n]
+        S[..., k, :, :, sp, :] += np.einsum("aBCDEsn,cBCDEsn->BCDEsac", np.conj(Wb), Hb)
+
+    one = np.ones((Lt, Lz, Ly, Lx))
+    for sp in range(2):                                                # chirality sigma' of the source vectors
+        Wsp = np.zeros_like(W)
+        Wsp[..., 2 * sp:2 * sp + 2, :] = W[..., 2 * sp:2 * sp + 2, :]
+        accumulate(0, (4.0 + mass) * Wsp, sp, one)                     # diagonal term of eq. (2.2)
+        for mu in range(4):
+            ax = _site_axis(mu)
+            g = wd_oracle.gamma(mu)
+            xm = coords[ax] % block[mu]
+            # forward hop: -1/2 (1 - gamma_mu) U_mu(x) W(x + mu)
+            Wf = np.roll(Wsp, -1, axis=1 + ax)
+            H = np.einsum("...ab,n...sb->n...sa", Uc[mu], Wf)
+            H = -0.5 * np.einsum("st,n...ta->n...sa", np.eye(4) - g, H)
+            leaves = (xm == block[mu] - 1).astype(np.float64)
+            accumulate(1 + mu, H, sp, leaves)
+            accumulate(0, H, sp, 1.0 - leaves)
+            # backward hop: -1/2 (1 + gamma_mu) U_mu(x - mu)^dag W(x - mu)
+            Wbk = np.roll(Wsp, +1, axis=1 + ax)
+            Ub = np.roll(Uc[mu], +1, axis=ax)
+            H = np.einsum("...ba,n...sb->n...sa", np.conj(Ub), Wbk)
+            H = -0.5 * np.einsum("st,n...ta->n...sa", np.eye(4) + g, H)
+            leaves = (xm == 0).astype(np.float64)
+            accumulate(5 + mu, H, sp, leaves)
+            accumulate(0, H, sp, 1.0 - leaves)
+    return S.reshape(nb + (9, 2 * nv, 2 * nv))
+
+
+def coarse_apply_stencil(S, c):
+    """(Dhat c)(b) = A(b) c(b) + sum_mu [ F_mu(b) c(b+mu) + B_mu(b) c(b-mu) ];  c [Bt,Bz,By,Bx, 2, Nv] -> same shape."""
+    c = np.asarray(c, dtype=np.complex128)
+    shp = c.shape
+    v = c.reshape(shp[:4] + (-1,))
+    out = np.einsum("...ij,...j->...i", S[..., 0, :, :], v)
+    for mu in range(4):
+        ax = _site_axis(mu)
+        out += np.einsum("...ij,...j->...i", S[..., 1 + mu, :, :], np.roll(v, -1, axis=ax))
+        out += np.einsum("...ij,...j->...i", S[..., 5 + mu, :, :], np.roll(v, +1, axis=ax))
+    return out.reshape(shp)

@@ -13,7 +13,7 @@ import os
 WD_OK = 0
 WD_FP32, WD_FP64 = 32, 64
 WD_RECON_18, WD_RECON_12 = 18, 12
-WD_KERNEL_AUTO, WD_KERNEL_SITE, WD_KERNEL_TILE, WD_KERNEL_STAGE = 0, 1, 2, 3
+WD_KERNEL_AUTO, WD_KERNEL_SITE, WD_KERNEL_STAGE = 0, 1, 3
 
 STATUS_NAMES = {
     0: "WD_OK", -1: "WD_ERR_NULL", -2: "WD_ERR_DIMS", -3: "WD_ERR_PRECISION", -4: "WD_ERR_RECON",
@@ -23,7 +23,7 @@ STATUS_NAMES = {
 # every symbol include/wd.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
-    "wd_set_kernel", "wd_set_temporal_gauge", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
+    "wd_set_kernel", "wd_set_tuning", "wd_set_temporal_gauge", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
     "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_coarse_reals",
     "wd_block_orthonormalise", "wd_restrict", "wd_prolong", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_dagger", "wd_apply_host",
     "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
@@ -55,6 +55,7 @@ def lib():
     L.wd_load_gauge.argtypes = [vp, vp, i, i, vp, ctypes.POINTER(vp)]
     L.wd_set_stream.argtypes = [vp, vp]
     L.wd_set_kernel.argtypes = [vp, i]
+    L.wd_set_tuning.argtypes = [vp, ctypes.c_char_p, i]
     L.wd_set_temporal_gauge.argtypes = [vp, i]
     L.wd_selected_kernel.argtypes = [vp, i]
     L.wd_spinor_bytes.argtypes = [vp, i, i]
@@ -88,7 +89,7 @@ def lib():
     L.wd_destroy.argtypes = [vp]
     L.wd_destroy.restype = None
     for name in ("wd_create_lattice", "wd_lattice_dims", "wd_load_gauge", "wd_set_stream", "wd_set_kernel",
-                 "wd_set_temporal_gauge",
+                 "wd_set_tuning", "wd_set_temporal_gauge",
                  "wd_selected_kernel", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_dagger", "wd_apply_host",
                  "wd_pack_spinor_parity", "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur",
                  "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur",
@@ -104,6 +105,8 @@ def _ptr(x):
         return None
     if isinstance(x, int):
         return x
+    if hasattr(x, "cuda_stream"):  # torch.cuda.Stream
+        return int(x.cuda_stream)
     if hasattr(x, "data_ptr"):
         return x.data_ptr()
     if hasattr(x, "ctypes"):
@@ -161,6 +164,10 @@ def wd_set_kernel(gauge, kernel):
     _check(lib().wd_set_kernel(gauge, int(kernel)), "wd_set_kernel")
 
 
+def wd_set_tuning(gauge, name, value):
+    _check(lib().wd_set_tuning(gauge, name.encode(), int(value)), "wd_set_tuning")
+
+
 def wd_selected_kernel(gauge, nrhs=1):
     k = int(lib().wd_selected_kernel(gauge, int(nrhs)))
     if k < 0:
@@ -168,7 +175,7 @@ def wd_selected_kernel(gauge, nrhs=1):
     return k
 
 
-KERNEL_NAMES = {WD_KERNEL_SITE: "site", WD_KERNEL_TILE: "tile", WD_KERNEL_STAGE: "stage"}
+KERNEL_NAMES = {WD_KERNEL_SITE: "site", WD_KERNEL_STAGE: "stage"}
 
 
 def wd_set_temporal_gauge(gauge, on=True):
@@ -313,6 +320,9 @@ class WilsonDirac:
     def set_kernel(self, kernel):
         wd_set_kernel(self.gauge, kernel)
 
+    def set_tuning(self, name, value):
+        wd_set_tuning(self.gauge, name, value)
+
     def pack(self, native_dev, canonical_dev, nrhs, stream=None):
         wd_pack_spinor(self.lat, native_dev, canonical_dev, nrhs, self.precision, stream or self.stream)
 
@@ -323,7 +333,7 @@ class WilsonDirac:
         wd_set_temporal_gauge(self.gauge, on)
 
     def selected_kernel(self, nrhs=1):
-        """Name of the kernel wd_apply will launch for nrhs right-hand sides ("site", "tile", "stage")."""
+        """Name of the kernel wd_apply will launch for nrhs right-hand sides ("site", "stage")."""
         return KERNEL_NAMES[wd_selected_kernel(self.gauge, nrhs)]
 
     def apply_dagger(self, out_native_dev, in_native_dev, mass, nrhs=1):

@@ -73,6 +73,55 @@ int check_apply_args(const void *out, const void *in, const wd_gauge *g, const i
 
 namespace wd {
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+static int env_int(const char *name)
+{
+    const char *e = getenv(name);
+    if (!e || !*e) return -1;
+    const int v = atoi(e);
+    return v < 0 ? -1 : v;
+}
+
+void tuning_from_env(Tuning &t)
+{
+    t = Tuning();
+    if (const char *e = getenv("WD_TILE_SHAPE")) {
+        int ty = 0, tz = 0;
+        if (sscanf(e, "%d,%d", &ty, &tz) == 2 && ty >= 1 && tz >= 1) {
+            t.tile_ty = ty;
+            t.tile_tz = tz;
+        }
+    }
+    t.tile_tc = env_int("WD_TILE_TC");
+    t.tile_nchunk = env_int("WD_TILE_NCHUNK");
+    t.tile_nrb = env_int("WD_TILE_NRB");
+    t.mrhs_patch = env_int("WD_MRHS_PATCH");
+    t.stage_no_mrhs = env_int("WD_STAGE_NO_MRHS");
+    t.site_slab_mb = env_int("WD_SITE_SLAB_MB");
+    t.host_no_pipeline = env_int("WD_HOST_NO_PIPELINE");
+    t.mrhs_no_tail = env_int("WD_MRHS_NO_TAIL");
+}
+
+int tuning_set(Tuning &t, const char *name, int value)
+{
+    struct { const char *n; int Tuning::*f; } tab[] = {
+        {"tile_ty", &Tuning::tile_ty}, {"tile_tz", &Tuning::tile_tz}, {"tile_tc", &Tuning::tile_tc},
+        {"tile_nchunk", &Tuning::tile_nchunk}, {"tile_nrb", &Tuning::tile_nrb}, {"mrhs_patch", &Tuning::mrhs_patch},
+        {"stage_no_mrhs", &Tuning::stage_no_mrhs}, {"site_slab_mb", &Tuning::site_slab_mb},
+        {"host_no_pipeline", &Tuning::host_no_pipeline}, {"mrhs_no_tail", &Tuning::mrhs_no_tail}};
+    for (auto &e : tab)
+        if (!strcmp(name, e.n)) {
+            t.*(e.f) = value < 0 ? -1 : value;
+            return 0;
+        }
+    return -1;
+}
+
+const Tuning &default_tuning()
+{
+    static const Tuning t;
+    return t;
+}
 } // namespace wd
 
 extern "C" {
@@ -129,6 +178,8 @@ int wd_load_gauge(const wd_lattice *lat, const void *links_canonical_dev, int pr
     g->precision = precision;
     g->recon = recon;
     g->kernel = WD_KERNEL_AUTO;
+    g->tune = wd::Tuning();
+    wd::tuning_from_env(g->tune); // the one place the environment is read
     g->stream = (cudaStream_t)stream;
     g->links_bytes = wd::native_link_bytes(g->V, precision, recon);
     cudaError_t e = cudaMalloc(&g->links, g->links_bytes);
@@ -151,7 +202,24 @@ int wd_set_stream(wd_gauge *gauge, void *stream)
 {
     if (!gauge) return fail(WD_ERR_NULL, "wd_set_stream: NULL gauge");
     if (gauge->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_set_stream: not a live wd_gauge handle");
+    // work already queued on the old stream (the link conversion of wd_load_gauge, earlier applies) comes first
+    if ((cudaStream_t)stream != gauge->stream) {
+        cudaEvent_t ev;
+        cudaError_t e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventRecord(ev, gauge->stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent((cudaStream_t)stream, ev, 0);
+        if (e == cudaSuccess) e = cudaEventDestroy(ev);
+        if (e != cudaSuccess) return cuda_fail(e, "wd_set_stream");
+    }
     gauge->stream = (cudaStream_t)stream;
+    return WD_OK;
+}
+
+int wd_set_tuning(wd_gauge *gauge, const char *name, int value)
+{
+    if (!gauge || !name) return fail(WD_ERR_NULL, "wd_set_tuning: NULL argument");
+    if (gauge->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_set_tuning: not a live wd_gauge handle");
+    if (wd::tuning_set(gauge->tune, name, value)) return fail(WD_ERR_MISMATCH, "wd_set_tuning: unknown variable '%s'", name);
     return WD_OK;
 }
 
@@ -181,17 +249,18 @@ int wd_set_kernel(wd_gauge *gauge, int kernel)
 {
     if (!gauge) return fail(WD_ERR_NULL, "wd_set_kernel: NULL gauge");
     if (gauge->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_set_kernel: not a live wd_gauge handle");
-    if (kernel != WD_KERNEL_AUTO && kernel != WD_KERNEL_SITE && kernel != WD_KERNEL_TILE && kernel != WD_KERNEL_STAGE)
+    if (kernel != WD_KERNEL_AUTO && kernel != WD_KERNEL_SITE && kernel != WD_KERNEL_STAGE)
         return fail(WD_ERR_MISMATCH, "wd_set_kernel: unknown kernel %d", kernel);
-    if (kernel == WD_KERNEL_TILE || kernel == WD_KERNEL_STAGE) {
+    if (kernel == WD_KERNEL_STAGE) {
         wd::ApplyArgs a{};
         for (int d = 0; d < 4; ++d) a.dims[d] = gauge->dims[d];
         a.V = gauge->V;
         a.nrhs = 1;
         a.precision = gauge->precision;
         a.recon = gauge->recon;
-        if (!(kernel == WD_KERNEL_TILE ? wd::tile_supported(a) : wd::stage_supported(a)))
-            return fail(WD_ERR_MISMATCH, "wd_set_kernel: tiled kernel does not support lattice %d %d %d %d", a.dims[0],
+        a.tune = &gauge->tune;
+        if (!wd::stage_supported(a))
+            return fail(WD_ERR_MISMATCH, "wd_set_kernel: staged kernel does not support lattice %d %d %d %d", a.dims[0],
                         a.dims[1], a.dims[2], a.dims[3]);
     }
     gauge->kernel = kernel;
@@ -231,14 +300,12 @@ int wd_unpack_spinor(const wd_lattice *lat, void *canonical_dev, const void *nat
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_unpack_spinor");
 }
 
-// which kernel WD_KERNEL_AUTO resolves to, by measurement (profiles/): on a lattice of at least a few
-// waves of tiles the staged kernels (fp32; single- and multi-RHS members) or, for one fp64 right-hand
-// side, the tile kernel; everything else -> site kernel
+// which kernel WD_KERNEL_AUTO resolves to, by measurement (profiles/): the staged kernels (single- and multi-RHS
+// members) on every lattice they can tile that has at least one wave of tiles; everything else -> site kernel
 static int auto_kernel(const wd::ApplyArgs &a)
 {
     const bool big = a.V >= (1LL << 18);
     if (big && wd::stage_supported(a)) return WD_KERNEL_STAGE;
-    if (big && a.nrhs == 1 && wd::tile_supported(a)) return WD_KERNEL_TILE;
     return WD_KERNEL_SITE;
 }
 
@@ -251,10 +318,11 @@ static wd::ApplyArgs shape_args(const wd_gauge *g, int nrhs)
     a.precision = g->precision;
     a.recon = g->recon;
     a.tgauge = g->tgauge;
+    a.tune = &g->tune;
     return a;
 }
 
-static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double mass, int nrhs)
+static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double mass, int nrhs, int dagger = 0)
 {
     wd::ApplyArgs a{};
     a.out = out;
@@ -267,20 +335,17 @@ static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double m
     a.precision = g->precision;
     a.recon = g->recon;
     a.tgauge = g->tgauge;
+    a.tune = &g->tune;
     a.stream = g->stream;
+    a.dagger = dagger;
     cudaError_t e;
     if (g->kernel == WD_KERNEL_SITE)
         e = wd::launch_site(a);
-    else if (g->kernel == WD_KERNEL_TILE) {
-        if (!wd::tile_supported(a)) return fail(WD_ERR_MISMATCH, "wd_apply: tiled kernel cannot take this call");
-        e = wd::launch_tile(a);
-    } else if (g->kernel == WD_KERNEL_STAGE) {
+    else if (g->kernel == WD_KERNEL_STAGE) {
         if (!wd::stage_supported(a)) return fail(WD_ERR_MISMATCH, "wd_apply: staged kernel cannot take this call");
         e = wd::launch_stage(a);
-    } else {
-        const int k = auto_kernel(a);
-        e = k == WD_KERNEL_STAGE ? wd::launch_stage(a) : k == WD_KERNEL_TILE ? wd::launch_tile(a) : wd::launch_site(a);
-    }
+    } else
+        e = auto_kernel(a) == WD_KERNEL_STAGE ? wd::launch_stage(a) : wd::launch_site(a);
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply: kernel launch");
 }
 
@@ -305,15 +370,7 @@ int wd_apply_dagger(void *out_native_dev, const void *in_native_dev, const wd_ga
     if (overlap(out_native_dev, bytes, in_native_dev, bytes)) return fail(WD_ERR_ALIAS, "wd_apply_dagger: out and in overlap");
     if (((uintptr_t)out_native_dev | (uintptr_t)in_native_dev) & 15)
         return fail(WD_ERR_MISMATCH, "wd_apply_dagger: buffers must be 16-byte aligned");
-    wd::ApplyArgs a = shape_args(gauge, nrhs);
-    a.out = out_native_dev;
-    a.in = in_native_dev;
-    a.links = gauge->links;
-    a.mass = mass;
-    a.stream = gauge->stream;
-    a.dagger = 1;
-    cudaError_t e = wd::launch_site(a);
-    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply_dagger: kernel launch");
+    return dispatch_apply(out_native_dev, in_native_dev, gauge, mass, nrhs, 1);
 }
 
 int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_gauge *gauge, double mass,
@@ -355,21 +412,36 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
     // stream as soon as slabs k-1, k, k+1 have arrived, and its result is unpacked and copied out on a
     // third stream, so the host->device and device->host transfers overlap (PCIe is full duplex) ----
     const int nslab = Lt >= 16 ? 16 : Lt; // (the event arrays of wd_gauge hold 16)
-    const bool pipelined = nslab >= 3 && S3 % 128 == 0 && bytes >= (8u << 20) &&
-                           !(getenv("WD_HOST_NO_PIPELINE") && atoi(getenv("WD_HOST_NO_PIPELINE")));
+    const bool pipelined = nslab >= 3 && S3 % 128 == 0 && bytes >= (8u << 20) && g->tune.host_no_pipeline <= 0;
     if (pipelined) {
-        if (!g->pipe_stream[0]) {
-            for (int i = 0; i < 3; ++i)
-                if ((e = cudaStreamCreateWithFlags(&g->pipe_stream[i], cudaStreamNonBlocking)) != cudaSuccess)
-                    return cuda_fail(e, "wd_apply_host: stream create");
+        if (!g->pipe_ready) { // all 3 streams and 34 events, or none
+            e = cudaSuccess;
+            for (int i = 0; i < 3 && e == cudaSuccess; ++i) e = cudaStreamCreateWithFlags(&g->pipe_stream[i], cudaStreamNonBlocking);
             for (auto &ev : g->pipe_event)
-                if ((e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess)
-                    return cuda_fail(e, "wd_apply_host: event create");
+                if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+            if (e != cudaSuccess) {
+                for (auto &st : g->pipe_stream) {
+                    if (st) cudaStreamDestroy(st);
+                    st = nullptr;
+                }
+                for (auto &ev : g->pipe_event) {
+                    if (ev) cudaEventDestroy(ev);
+                    ev = nullptr;
+                }
+                return cuda_fail(e, "wd_apply_host: stream / event create");
+            }
+            g->pipe_ready = 1;
         }
+        // on any error below: drain the three private streams before returning, so that no copy or kernel still
+        // touches the caller's host buffers after the call has failed
+        auto bail = [&](cudaError_t err, const char *what) {
+            for (auto &st : g->pipe_stream) cudaStreamSynchronize(st);
+            return cuda_fail(err, what);
+        };
         cudaStream_t s_in = g->pipe_stream[0], s_cmp = g->pipe_stream[1], s_out = g->pipe_stream[2];
         cudaEvent_t *ev_in = g->pipe_event, *ev_cmp = g->pipe_event + 16, ev_start = g->pipe_event[32], ev_end = g->pipe_event[33];
         // everything enqueued on the gauge's stream so far (e.g. the link conversion) comes first
-        if ((e = cudaEventRecord(ev_start, s)) != cudaSuccess) return cuda_fail(e, "wd_apply_host: event record");
+        if ((e = cudaEventRecord(ev_start, s)) != cudaSuccess) return bail(e, "wd_apply_host: event record");
         for (int i = 0; i < 3; ++i) cudaStreamWaitEvent(g->pipe_stream[i], ev_start, 0);
         auto t0 = [&](int k) { return (long long)Lt * k / nslab; };
         const size_t row = (size_t)g->V * 24 * w; // bytes of one right-hand side, canonical
@@ -378,9 +450,9 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
             e = cudaMemcpy2DAsync((char *)g->stage_canon + (size_t)s0 * 24 * w, row,
                                   (const char *)in_canonical_host + (size_t)s0 * 24 * w, row, (size_t)ns * 24 * w, nrhs,
                                   cudaMemcpyHostToDevice, s_in);
-            if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: H2D copy");
+            if (e != cudaSuccess) return bail(e, "wd_apply_host: H2D copy");
             e = wd::launch_pack_spinor(g->stage_in, g->stage_canon, g->V, nrhs, precision, s_in, s0, ns);
-            if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: pack");
+            if (e != cudaSuccess) return bail(e, "wd_apply_host: pack");
             cudaEventRecord(ev_in[k], s_in);
         }
         // interior slabs in arrival order, then the two that need the wrap-around neighbour
@@ -396,20 +468,20 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
             a.stream = s_cmp;
             a.site_begin = t0(k) * S3;
             a.site_end = t0(k + 1) * S3;
-            if ((e = wd::launch_site(a)) != cudaSuccess) return cuda_fail(e, "wd_apply_host: kernel launch");
+            if ((e = wd::launch_site(a)) != cudaSuccess) return bail(e, "wd_apply_host: kernel launch");
             cudaEventRecord(ev_cmp[k], s_cmp);
             cudaStreamWaitEvent(s_out, ev_cmp[k], 0);
             e = wd::launch_unpack_spinor(g->stage_canon_out, g->stage_out, g->V, nrhs, precision, s_out, a.site_begin,
                                          a.site_end - a.site_begin);
-            if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: unpack");
+            if (e != cudaSuccess) return bail(e, "wd_apply_host: unpack");
             e = cudaMemcpy2DAsync((char *)out_canonical_host + (size_t)a.site_begin * 24 * w, row,
                                   (const char *)g->stage_canon_out + (size_t)a.site_begin * 24 * w, row,
                                   (size_t)(a.site_end - a.site_begin) * 24 * w, nrhs, cudaMemcpyDeviceToHost, s_out);
-            if (e != cudaSuccess) return cuda_fail(e, "wd_apply_host: D2H copy");
+            if (e != cudaSuccess) return bail(e, "wd_apply_host: D2H copy");
         }
-        if ((e = cudaEventRecord(ev_end, s_out)) != cudaSuccess) return cuda_fail(e, "wd_apply_host: event record");
+        if ((e = cudaEventRecord(ev_end, s_out)) != cudaSuccess) return bail(e, "wd_apply_host: event record");
         cudaStreamWaitEvent(s, ev_end, 0);
-        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(e, "wd_apply_host: stream synchronize");
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return bail(e, "wd_apply_host: stream synchronize");
         return WD_OK;
     }
 
@@ -666,7 +738,7 @@ void wd_destroy_gauge(wd_gauge *gauge)
     cudaFree(gauge->cg_sc);
     cudaFree(gauge->stage_in);
     cudaFree(gauge->stage_out);
-    if (gauge->pipe_stream[0]) {
+    if (gauge->pipe_ready) {
         for (auto &st : gauge->pipe_stream) cudaStreamDestroy(st);
         for (auto &ev : gauge->pipe_event) cudaEventDestroy(ev);
     }

@@ -81,13 +81,19 @@ template <int RECON> constexpr int mrhs_smem_vecs(int nts, int nrb, int nyb, int
            nzb * LinkVecs<2, RECON>::n;
 }
 
-// gridDim.x = nchunk * ngroups * ncol, ordered (t-chunk, RHS group, tile column).
+// Work items = (t-chunk, RHS group, tile column) in the order described below; block b < n_full runs item b over its
+// whole t-chunk, the blocks after that run the LAST (partial) wave of items cut into ksplit shorter marches each, so
+// that the tail of the launch keeps every SM busy (one CTA per SM: without the cut a launch of 3.46 waves costs 4).
 // blockDim.x = nts * NRB, nts = Lx*ty*tz sites of the tile (a multiple of 32, at most 128).
 // NTS: sites per tile known at compile time (128, the default tile) or 0 = blockDim.x / NRB
-template <int RECON, int NRB, int NTS>
+// XS: x hops by warp shuffles (Lx a power of two); otherwise (e.g. Lx = 24, the paper's 24^3 x 64 volume)
+// x is handled like y and z: neighbour spinor from the slice buffer, neighbour link from the staged links, periodic
+// wrap in the slot arithmetic (the tile always spans the whole x extent).
+template <int RECON, int NRB, int NTS, bool XS>
 __global__ void __launch_bounds__(128 * NRB, 1)
 dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const float *__restrict__ links, int Lx, int Ly,
-                   int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk, int patch, int tgauge)
+                   int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk, int patch, int tgauge,
+                   int n_full, int ksplit)
 {
     constexpr int NVEC = LinkLayout<float, RECON>::NVEC;
     using FY = LinkVecs<1, RECON>;
@@ -110,14 +116,20 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
     const int ncol = ncy * (Lz / tz);
     const int ngroups = (nrhs + NRB - 1) / NRB;
     int col, g, k;
+    int item = blockIdx.x, sub = 0;
+    if ((int)blockIdx.x >= n_full) { // last wave: ksplit blocks share one item
+        const int j = blockIdx.x - n_full;
+        item = n_full + j / ksplit;
+        sub = j - (j / ksplit) * ksplit;
+    }
     if (patch > 0) {
         // (t-chunk, patch of patch x patch tile columns, column in patch, RHS group), group FASTEST: the
         // ~#SM resident CTAs are all RHS groups of one compact patch of columns marching through the
         // same slices, so a slice's links are read from HBM by one group and from L2 by the others,
         // and only faces on the patch boundary leave the patch.
         const int per_chunk = ncol * ngroups;
-        k = blockIdx.x / per_chunk;
-        const int r = blockIdx.x - k * per_chunk;
+        k = item / per_chunk;
+        const int r = item - k * per_chunk;
         const int per_patch = patch * patch * ngroups;
         const int p = r / per_patch, w = r - p * per_patch;
         g = w % ngroups;
@@ -126,8 +138,8 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         const int cyy = (p % npy) * patch + c % patch, czz = (p / npy) * patch + c / patch;
         col = cyy + ncy * czz;
     } else { // (t-chunk, RHS group, tile column)
-        col = blockIdx.x % ncol;
-        const int kg = blockIdx.x / ncol;
+        col = item % ncol;
+        const int kg = item / ncol;
         g = kg % ngroups;
         k = kg / ngroups;
     }
@@ -136,8 +148,8 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
     in += (long long)(live ? rhs : nrhs - 1) * 24 * padded_volume(V);
     out += (long long)(live ? rhs : nrhs - 1) * 24 * padded_volume(V);
 
-    const int x = st & (Lx - 1);
     const int row = st / Lx;
+    const int x = st - row * Lx;
     const int yy = row % ty, zz = row / ty;
     const int lane = tid & 31;
     const int lane_r = (lane & ~(Lx - 1)) | ((lane + 1) & (Lx - 1));
@@ -146,7 +158,12 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
     const int rank_y = zz * Lx + x, rank_z = yy * Lx + x;
 
     const long long S3 = (long long)Lx * Ly * Lz;
-    const int t_begin = (int)((long long)Lt * k / nchunk), t_end = (int)((long long)Lt * (k + 1) / nchunk);
+    int t_begin = (int)((long long)Lt * k / nchunk), t_end = (int)((long long)Lt * (k + 1) / nchunk);
+    if ((int)blockIdx.x >= n_full) { // this block's share of the chunk
+        const int len = t_end - t_begin;
+        t_end = t_begin + (int)((long long)len * (sub + 1) / ksplit);
+        t_begin += (int)((long long)len * sub / ksplit);
+    }
     const int cy = col % ncy, cz = col / ncy;
     const int y = cy * ty + yy, z = cz * tz + zz;
     const long long s3 = x + (long long)Lx * (y + (long long)Ly * z);
@@ -240,9 +257,16 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         for (int i = 0; i < 24; ++i) acc[i] = 0.f;
         reconstruct_add<3, +1>(acc, chi_t); // backward t hop, product carried from the previous slice
 
-        // ---- x: both hops through warp shuffles ----
+        // ---- x: both hops through warp shuffles (XS), else like y and z ----
         lds_link<0, RECON>(lnk, 0, nts, st, u);
-        {
+        if (!XS) {
+            const int dxf = (x + 1 == Lx ? 1 - Lx : 1), dxb = (x == 0 ? Lx - 1 : -1);
+            lds_vecs<6>(pl, nt, tid + dxf, pn);
+            hop_forward<0>(acc, u, pn);
+            lds_link<0, RECON>(lnk, 0, nts, st + dxb, u);
+            lds_vecs<6>(pl, nt, tid + dxb, pn);
+            hop_backward<0>(acc, u, pn);
+        } else {
             float h[12], gg[12], chi[12];
             project<0, -1>(psi, h);
             shfl12(gg, h, lane_r); // P-_x psi(x+1)
@@ -320,46 +344,51 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
 // ---------------------------------------------------------------------------------------------
 namespace {
 
-template <int RECON, int NRB, int NTS>
+template <int RECON, int NRB, int NTS, bool XS>
 cudaError_t launch_mrhs_n(const ApplyArgs &a, int ty, int tz)
 {
-    auto kern = dslash_mrhs_kernel<RECON, NRB, NTS>;
+    auto kern = dslash_mrhs_kernel<RECON, NRB, NTS, XS>;
     const int Lx = a.dims[0];
     const int nts = Lx * ty * tz;
     const size_t smem = (size_t)mrhs_smem_vecs<RECON>(nts, NRB, Lx * tz, Lx * ty) * sizeof(float4);
     if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
-    static size_t smem_set = 0;
-    cudaError_t e;
-    if (smem > smem_set) {
-        if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        smem_set = smem;
-    }
-    // slices per t-chunk (WD_TILE_TC / WD_TILE_NCHUNK override): with (columns x RHS groups) already many
+    static size_t smem_set[64];
+    cudaError_t e = ensure_dynamic_smem((const void *)kern, smem, smem_set);
+    if (e != cudaSuccess) return e;
+    const Tuning &tn = a.tune ? *a.tune : default_tuning();
+    // slices per t-chunk (tile_tc / tile_nchunk override): with (columns x RHS groups) already many
     // times the SM count, long marches win (measured for 24 RHS on 32^3 x 64: 64 > 32 > 16 > 8)
-    int tc = 64;
-    if (const char *ev = getenv("WD_TILE_TC")) {
-        const int v = atoi(ev);
-        if (v >= 1) tc = v;
-    }
+    const int tc = tn.tile_tc >= 1 ? tn.tile_tc : 64;
     int nchunk = (a.dims[3] + tc - 1) / tc;
-    if (const char *ev = getenv("WD_TILE_NCHUNK")) {
-        const int v = atoi(ev);
-        if (v >= 1 && v <= a.dims[3]) nchunk = v;
-    }
+    if (tn.tile_nchunk >= 1 && tn.tile_nchunk <= a.dims[3]) nchunk = tn.tile_nchunk;
     if (nchunk < 1) nchunk = 1;
     const long long ncol = (long long)(a.dims[1] / ty) * (a.dims[2] / tz);
     const long long ngroups = (a.nrhs + NRB - 1) / NRB;
-    if (ncol * nchunk * ngroups > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    dim3 grid((unsigned)(ncol * nchunk * ngroups));
+    const long long nitems = ncol * nchunk * ngroups;
+    if (nitems > 0x3fffffffLL) return cudaErrorInvalidConfiguration;
     // block order: patches of 4 x 4 tile columns with the RHS group fastest when the column grid allows
-    // it (WD_MRHS_PATCH=0 / n overrides), else (t-chunk, RHS group, column)
-    int patch = 4;
-    if (const char *ev = getenv("WD_MRHS_PATCH")) patch = atoi(ev);
+    // it (mrhs_patch = 0 / n overrides), else (t-chunk, RHS group, column)
+    int patch = tn.mrhs_patch >= 0 ? tn.mrhs_patch : 4;
     const int ncyh = a.dims[1] / ty, nczh = a.dims[2] / tz;
     if (patch < 1 || ncyh % patch || nczh % patch) patch = 0;
+    // the last, partial wave: its items are cut into ksplit shorter marches (at least 8 slices each) so that it
+    // fills the machine and ends after 1/ksplit of a wave.  CTAs resident per SM: by shared memory.
+    const int per_sm = smem > 113 * 1024 ? 1 : 2;
+    const long long slots = (long long)sm_count() * per_sm;
+    long long n_full = nitems, ksplit = 1;
+    const long long rem = nitems % slots;
+    const int chunk_len = a.dims[3] / nchunk;
+    if (rem > 0 && nitems > slots && tn.mrhs_no_tail <= 0) {
+        ksplit = slots / rem;
+        if (ksplit > chunk_len / 8) ksplit = chunk_len / 8;
+        if (ksplit < 1) ksplit = 1;
+        if (ksplit > 1) n_full = nitems - rem;
+    }
+    dim3 grid((unsigned)(n_full + (nitems - n_full) * ksplit));
     const float cdiag = (float)(4.0 + a.mass); // formed in double, rounded once (reading S8)
     kern<<<grid, nts * NRB, smem, a.stream>>>((float *)a.out, (const float *)a.in, (const float *)a.links, a.dims[0],
-                                               a.dims[1], a.dims[2], a.dims[3], ty, tz, a.V, cdiag, a.nrhs, nchunk, patch, a.tgauge);
+                                               a.dims[1], a.dims[2], a.dims[3], ty, tz, a.V, cdiag, a.nrhs, nchunk, patch, a.tgauge,
+                                               (int)n_full, (int)ksplit);
     count_launch();
     return cudaGetLastError();
 }
@@ -367,18 +396,18 @@ cudaError_t launch_mrhs_n(const ApplyArgs &a, int ty, int tz)
 template <int RECON, int NRB>
 cudaError_t launch_mrhs_t(const ApplyArgs &a, int ty, int tz)
 {
-    return a.dims[0] * ty * tz == 128 ? launch_mrhs_n<RECON, NRB, 128>(a, ty, tz) : launch_mrhs_n<RECON, NRB, 0>(a, ty, tz);
+    const int nts = a.dims[0] * ty * tz;
+    if (a.dims[0] & (a.dims[0] - 1)) return nts == 96 ? launch_mrhs_n<RECON, NRB, 96, false>(a, ty, tz) : launch_mrhs_n<RECON, NRB, 0, false>(a, ty, tz);
+    return nts == 128 ? launch_mrhs_n<RECON, NRB, 128, true>(a, ty, tz) : launch_mrhs_n<RECON, NRB, 0, true>(a, ty, tz);
 }
 
 template <int RECON>
 cudaError_t launch_mrhs_r(const ApplyArgs &a, int ty, int tz)
 {
-    // right-hand sides per CTA: 3 (12 warps per SM; 24 = 8 x 3) unless WD_TILE_NRB says otherwise
+    // right-hand sides per CTA: 3 (12 warps per SM; 24 = 8 x 3) unless tile_nrb says otherwise
+    const Tuning &tn = a.tune ? *a.tune : default_tuning();
     int nrb = a.nrhs >= 3 ? 3 : a.nrhs;
-    if (const char *ev = getenv("WD_TILE_NRB")) {
-        const int v = atoi(ev);
-        if (v >= 1 && v <= 3) nrb = v;
-    }
+    if (tn.tile_nrb >= 1 && tn.tile_nrb <= 3) nrb = tn.tile_nrb;
     if (nrb >= 3) return launch_mrhs_t<RECON, 3>(a, ty, tz);
     if (nrb == 2) return launch_mrhs_t<RECON, 2>(a, ty, tz);
     return launch_mrhs_t<RECON, 1>(a, ty, tz);

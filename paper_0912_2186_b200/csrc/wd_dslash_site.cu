@@ -107,11 +107,8 @@ static cudaError_t launch_site_t(const ApplyArgs &a)
     if (nb * ngroups > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     // slab: ~32 MB of links (WD_SITE_SLAB_MB overrides) -- a fraction of the 126 MB L2, leaving room
     // for the spinor streams of the groups passing through
-    double slab_mb = 32.0;
-    if (const char *ev = getenv("WD_SITE_SLAB_MB")) {
-        const double v = atof(ev);
-        if (v > 0) slab_mb = v;
-    }
+    const Tuning &tn = a.tune ? *a.tune : default_tuning();
+    const double slab_mb = tn.site_slab_mb > 0 ? (double)tn.site_slab_mb : 32.0;
     long long bps = (long long)(slab_mb * 1e6 / ((double)SITE_THREADS * 4 * RECON * sizeof(T)));
     if (ngroups == 1 || bps > nb) bps = nb;
     if (bps < 1) bps = 1;

@@ -94,11 +94,16 @@ template <typename T, int RECON> constexpr int stage_smem_vecs(int nt, int nyb, 
 // XS: x hops by warp shuffles (Lx a power of two); otherwise (e.g. Lx = 24) x is handled like y and z
 // inside the tile -- forward hop from the slice buffer, backward product through an exchange buffer --
 // with the periodic wrap in the slot arithmetic (the tile always spans the whole x extent).
-template <typename T, int RECON, int NT, bool XS>
+// SGN = -1: D of eq. (2.2); SGN = +1: gamma5 D gamma5 = D^dagger, every projector 1 -+ gamma_mu swapped.
+// patch > 0 (several right-hand sides): blocks ordered (t-chunk, patch of patch x patch tile columns, column in patch,
+// right-hand side) with the right-hand side FASTEST, so the CTAs resident at any time are all right-hand sides of a few
+// neighbouring columns marching through the same slices: a slice's links come from HBM once and from L2 for the others.
+template <typename T, int RECON, int NT, bool XS, int SGN>
 __global__ void __launch_bounds__(NT ? NT : 256, 1)
 dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ links, int Lx, int Ly,
-                    int Lz, int Lt, int ty, int tz, long long V, T cdiag, int nrhs, int nchunk, int tgauge)
+                    int Lz, int Lt, int ty, int tz, long long V, T cdiag, int nrhs, int nchunk, int tgauge, int patch)
 {
+    constexpr int FS = SGN, BS = -SGN; // projector signs of the forward / backward hops
     using SL = SpinorLayout<T>;
     using Vec = typename SL::Vec;
     constexpr int NCH = SL::NCH, CR = SL::CR, HCH = NCH / 2; // vectors per spinor / reals per vector / per half spinor
@@ -123,9 +128,23 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
 
     const int ncy = Ly / ty;
     const int ncol = ncy * (Lz / tz);
-    const int col = blockIdx.x % ncol;
-    const int kg = blockIdx.x / ncol;
-    const int rhs = kg % nrhs, k = kg / nrhs;
+    int col, rhs, k;
+    if (patch > 0) {
+        const int per_chunk = ncol * nrhs;
+        k = blockIdx.x / per_chunk;
+        const int r = blockIdx.x - k * per_chunk;
+        const int per_patch = patch * patch * nrhs;
+        const int p = r / per_patch, w = r - p * per_patch;
+        rhs = w % nrhs;
+        const int c = w / nrhs;      // column within the patch
+        const int npy = ncy / patch; // patches along y
+        col = (p % npy) * patch + c % patch + ncy * ((p / npy) * patch + c / patch);
+    } else { // (t-chunk, right-hand side, tile column)
+        col = blockIdx.x % ncol;
+        const int kg = blockIdx.x / ncol;
+        rhs = kg % nrhs;
+        k = kg / nrhs;
+    }
     in += (long long)rhs * 24 * padded_volume(V);
     out += (long long)rhs * 24 * padded_volume(V);
 
@@ -209,7 +228,7 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
         const long long site_tb = s3 + (long long)tb * S3;
         T u[18], p[24], h[12];
         load_spinor(in, site_tb, p);
-        project<3, +1>(p, h);
+        project<3, BS>(p, h);
         if (unit_t(tb)) {
 #pragma unroll
             for (int i = 0; i < 12; ++i) chi_t[i] = h[i];
@@ -234,25 +253,25 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
         lds_vecs<NCH>(pl, nt, tid, psi);
 #pragma unroll
         for (int i = 0; i < 24; ++i) acc[i] = (T)0;
-        reconstruct_add<3, +1>(acc, chi_t); // backward t hop, product carried from the previous slice
+        reconstruct_add<3, BS>(acc, chi_t); // backward t hop, product carried from the previous slice
 
         // ---- x: both hops through warp shuffles ----
         lds_link_at<0, RECON>(lnk, 0, nt, tid, u);
         if (XS) {
             T h[12], g[12], chi[12];
-            project<0, -1>(psi, h);
+            project<0, FS>(psi, h);
             shfl12(g, h, lane_r); // P-_x psi(x+1)
             su3_mul(u, g, chi);
-            reconstruct_add<0, -1>(acc, chi);
-            project<0, +1>(psi, h);
+            reconstruct_add<0, FS>(acc, chi);
+            project<0, BS>(psi, h);
             su3_dag_mul(u, h, chi); // U_x(x)^dag P+_x psi(x): belongs to x+1
             shfl12(g, chi, lane_l);
-            reconstruct_add<0, +1>(acc, g);
+            reconstruct_add<0, BS>(acc, g);
         } else {
             T pn[24], h[12], chi[12];
             lds_vecs<NCH>(pl, nt, slot_xf, pn);
-            hop_forward<0>(acc, u, pn);
-            project<0, +1>(psi, h);
+            hop_forward_s<0, SGN>(acc, u, pn);
+            project<0, BS>(psi, h);
             su3_dag_mul(u, h, chi);
 #pragma unroll
             for (int c = 0; c < HCH; ++c) pack(xchg_x[c * nt + tid], &chi[c * CR]);
@@ -263,15 +282,15 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
             T pn[24], h[12], chi[12];
             if (face_yf) lds_vecs<NCH>(fy, nt, tid, pn);
             else lds_vecs<NCH>(pl, nt, slot_yf, pn);
-            hop_forward<1>(acc, u, pn);
-            project<1, +1>(psi, h);
+            hop_forward_s<1, SGN>(acc, u, pn);
+            project<1, BS>(psi, h);
             su3_dag_mul(u, h, chi);
 #pragma unroll
             for (int c = 0; c < HCH; ++c) pack(xchg_y[c * nt + tid], &chi[c * CR]);
             if (face_yb) { // the site below is outside the tile: do its backward hop here
                 lds_link_at<1, RECON>(fly, FY::first, nyb, rank_y, u);
                 lds_vecs<NCH>(fy, nt, tid, pn);
-                hop_backward<1>(acc, u, pn);
+                hop_backward_s<1, SGN>(acc, u, pn);
             }
         }
         if (more) stage_A(toff_n); // slots of links x,y and the y face are free again
@@ -283,15 +302,15 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
             T pn[24], h[12], chi[12];
             if (face_zf) lds_vecs<NCH>(fz, nt, tid, pn);
             else lds_vecs<NCH>(pl, nt, slot_zf, pn);
-            hop_forward<2>(acc, u, pn);
-            project<2, +1>(psi, h);
+            hop_forward_s<2, SGN>(acc, u, pn);
+            project<2, BS>(psi, h);
             su3_dag_mul(u, h, chi);
 #pragma unroll
             for (int c = 0; c < HCH; ++c) pack(xchg_z[c * nt + tid], &chi[c * CR]);
             if (face_zb) {
                 lds_link_at<2, RECON>(flz, FZ::first, nzb, rank_z, u);
                 lds_vecs<NCH>(fz, nt, tid, pn);
-                hop_backward<2>(acc, u, pn);
+                hop_backward_s<2, SGN>(acc, u, pn);
             }
         }
         // ---- t: forward hop now, backward product for the next slice ----
@@ -302,12 +321,12 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
             T pn[24], h[12];
             lds_vecs<NCH>(plane0 + (cur ^ 1) * plane_sz, nt, tid, pn);
             if (ut) { // U_t(x,t) = 1: the hops are projection and reconstruction only
-                project<3, -1>(pn, h);
-                reconstruct_add<3, -1>(acc, h);
-                project<3, +1>(psi, chi_t);
+                project<3, FS>(pn, h);
+                reconstruct_add<3, FS>(acc, h);
+                project<3, BS>(psi, chi_t);
             } else {
-                hop_forward<3>(acc, u, pn);
-                project<3, +1>(psi, h);
+                hop_forward_s<3, SGN>(acc, u, pn);
+                project<3, BS>(psi, h);
                 su3_dag_mul(u, h, chi_t);
             }
         }
@@ -317,17 +336,17 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
         if (!XS) {
             T chi[12];
             lds_vecs<HCH>(xchg_x, nt, slot_xb, chi);
-            reconstruct_add<0, +1>(acc, chi);
+            reconstruct_add<0, BS>(acc, chi);
         }
         if (!face_yb) {
             T chi[12];
             lds_vecs<HCH>(xchg_y, nt, slot_yb, chi);
-            reconstruct_add<1, +1>(acc, chi);
+            reconstruct_add<1, BS>(acc, chi);
         }
         if (!face_zb) {
             T chi[12];
             lds_vecs<HCH>(xchg_z, nt, slot_zb, chi);
-            reconstruct_add<2, +1>(acc, chi);
+            reconstruct_add<2, BS>(acc, chi);
         }
         // fused diagonal (step a6) and store (a7)
 #pragma unroll
@@ -345,6 +364,33 @@ dslash_stage_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__re
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
+cudaError_t ensure_dynamic_smem(const void *kernel, size_t bytes, size_t *per_device_cache)
+{
+    // the attribute is per device; the cache is an array of 64 entries (device ordinal), updated with relaxed atomics
+    // (a race sets the same attribute twice, which is harmless)
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    size_t have = __atomic_load_n(&per_device_cache[dev], __ATOMIC_RELAXED);
+    if (bytes <= have) return cudaSuccess;
+    if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes)) != cudaSuccess) return e;
+    __atomic_store_n(&per_device_cache[dev], bytes, __ATOMIC_RELAXED);
+    return cudaSuccess;
+}
+
+int sm_count()
+{
+    static int cache[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    int n = __atomic_load_n(&cache[dev], __ATOMIC_RELAXED);
+    if (n > 0) return n;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 148;
+    __atomic_store_n(&cache[dev], n, __ATOMIC_RELAXED);
+    return n;
+}
+
 namespace {
 
 struct StageShape {
@@ -356,10 +402,10 @@ bool stage_shape(const ApplyArgs &a, StageShape &s)
     const int Lx = a.dims[0], Ly = a.dims[1], Lz = a.dims[2];
     if (Lx < 4 || Lx > 32) return false; // a tile spans the whole x extent; power-of-two Lx uses warp shuffles in x
     if (((long long)Lx * Ly * Lz) % BLK) return false;
-    if (const char *e = getenv("WD_TILE_SHAPE")) {
-        int ty = 0, tz = 0;
-        if (sscanf(e, "%d,%d", &ty, &tz) == 2 && ty >= 2 && tz >= 2 && Ly % ty == 0 && Lz % tz == 0 &&
-            (Lx * ty * tz) % 32 == 0 && Lx * ty * tz <= 256) {
+    const Tuning &tn = a.tune ? *a.tune : default_tuning();
+    if (tn.tile_ty >= 2 && tn.tile_tz >= 2) {
+        const int ty = tn.tile_ty, tz = tn.tile_tz;
+        if (Ly % ty == 0 && Lz % tz == 0 && (Lx * ty * tz) % 32 == 0 && Lx * ty * tz <= 256) {
             s = {ty, tz, Lx * ty * tz};
             return true;
         }
@@ -387,40 +433,46 @@ template <typename T, int RECON> size_t stage_smem_bytes(const ApplyArgs &a, con
     return (size_t)stage_smem_vecs<T, RECON>(s.nt, a.dims[0] * s.tz, a.dims[0] * s.ty, xs) * 16;
 }
 
-template <typename T, int RECON, int NT, bool XS>
-cudaError_t launch_stage_nt(const ApplyArgs &a, const StageShape &s)
+template <typename T, int RECON, int NT, bool XS, int SGN>
+cudaError_t launch_stage_sgn(const ApplyArgs &a, const StageShape &s)
 {
-    auto kern = dslash_stage_kernel<T, RECON, NT, XS>;
+    auto kern = dslash_stage_kernel<T, RECON, NT, XS, SGN>;
     const size_t smem = stage_smem_bytes<T, RECON>(a, s);
     if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
-    static size_t smem_set = 0;
-    cudaError_t e;
-    if (smem > smem_set) {
-        if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        smem_set = smem;
-    }
-    // t-chunks of 16 slices (WD_TILE_TC / WD_TILE_NCHUNK override; measured 16 > 8 > 32 on 32^3 x 64 in both
+    static size_t smem_set[64];
+    cudaError_t e = ensure_dynamic_smem((const void *)kern, smem, smem_set);
+    if (e != cudaSuccess) return e;
+    const Tuning &tn = a.tune ? *a.tune : default_tuning();
+    // t-chunks of 16 slices (tile_tc / tile_nchunk override; measured 16 > 8 > 32 on 32^3 x 64 in both
     // precisions): the start of a march is the one place where this kernel waits for memory, so chunks
-    // are longer than in the tile kernel
-    int tc = 16;
-    if (const char *ev = getenv("WD_TILE_TC")) {
-        const int v = atoi(ev);
-        if (v >= 1) tc = v;
-    }
+    // are not shorter than that
+    const int tc = tn.tile_tc >= 1 ? tn.tile_tc : 16;
     int nchunk = (a.dims[3] + tc - 1) / tc;
-    if (const char *ev = getenv("WD_TILE_NCHUNK")) {
-        const int v = atoi(ev);
-        if (v >= 1 && v <= a.dims[3]) nchunk = v;
-    }
+    if (tn.tile_nchunk >= 1 && tn.tile_nchunk <= a.dims[3]) nchunk = tn.tile_nchunk;
     if (nchunk < 1) nchunk = 1;
-    const long long ncol = (long long)(a.dims[1] / s.ty) * (a.dims[2] / s.tz);
+    const int ncy = a.dims[1] / s.ty, ncz = a.dims[2] / s.tz;
+    const long long ncol = (long long)ncy * ncz;
     if (ncol * nchunk * a.nrhs > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    // several right-hand sides through this kernel (fp64, or tile shapes the multi-RHS kernel does not take): order
+    // the blocks so that all right-hand sides of a patch of columns are resident together and share the links in L2
+    int patch = 0;
+    if (a.nrhs > 1) {
+        patch = tn.mrhs_patch >= 0 ? tn.mrhs_patch : 4;
+        while (patch > 1 && (ncy % patch || ncz % patch)) patch >>= 1;
+        if (patch < 1 || ncy % patch || ncz % patch) patch = 0;
+    }
     dim3 grid((unsigned)(ncol * nchunk * a.nrhs));
     const T cdiag = (T)(4.0 + a.mass); // formed in double, rounded once (reading S8)
     kern<<<grid, s.nt, smem, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)a.links, a.dims[0], a.dims[1], a.dims[2],
-                                          a.dims[3], s.ty, s.tz, a.V, cdiag, a.nrhs, nchunk, a.tgauge);
+                                          a.dims[3], s.ty, s.tz, a.V, cdiag, a.nrhs, nchunk, a.tgauge, patch);
     count_launch();
     return cudaGetLastError();
+}
+
+template <typename T, int RECON, int NT, bool XS>
+cudaError_t launch_stage_nt(const ApplyArgs &a, const StageShape &s)
+{
+    return a.dagger ? launch_stage_sgn<T, RECON, NT, XS, +1>(a, s) : launch_stage_sgn<T, RECON, NT, XS, -1>(a, s);
 }
 
 template <typename T, int RECON>
@@ -428,7 +480,7 @@ cudaError_t launch_stage_t(const ApplyArgs &a)
 {
     StageShape s;
     if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
-    if (a.dims[0] & (a.dims[0] - 1)) return launch_stage_nt<T, RECON, 0, false>(a, s);
+    if (a.dims[0] & (a.dims[0] - 1)) return s.nt == 96 ? launch_stage_nt<T, RECON, 96, false>(a, s) : launch_stage_nt<T, RECON, 0, false>(a, s);
     return s.nt == 128 ? launch_stage_nt<T, RECON, 128, true>(a, s) : launch_stage_nt<T, RECON, 0, true>(a, s);
 }
 
@@ -448,11 +500,11 @@ cudaError_t launch_mrhs(const ApplyArgs &a, int ty, int tz); // wd_dslash_mrhs.c
 
 cudaError_t launch_stage(const ApplyArgs &a)
 {
-    if (a.precision == 32 && a.nrhs > 1 && !(getenv("WD_STAGE_NO_MRHS") && atoi(getenv("WD_STAGE_NO_MRHS")))) {
+    const Tuning &tn = a.tune ? *a.tune : default_tuning();
+    if (a.precision == 32 && a.nrhs > 1 && !a.dagger && tn.stage_no_mrhs <= 0) {
         StageShape s; // several right-hand sides: the kernel that shares the staged links between them
         if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
-        if (s.nt <= 128 && !(a.dims[0] & (a.dims[0] - 1)))
-            return launch_mrhs(a, s.ty, s.tz); // (a forced bigger tile or a non-power-of-two Lx runs RHS by RHS below)
+        if (s.nt <= 128) return launch_mrhs(a, s.ty, s.tz); // (a forced bigger tile runs through the single-RHS kernel below)
     }
     if (a.precision == 32) return a.recon == 18 ? launch_stage_t<float, 18>(a) : launch_stage_t<float, 12>(a);
     return a.recon == 18 ? launch_stage_t<double, 18>(a) : launch_stage_t<double, 12>(a);

@@ -3,6 +3,25 @@
 #include <cuda_runtime.h>
 #include <stddef.h>
 
+namespace wd {
+// Tuning variables: read from the environment ONCE, at wd_load_gauge, into the gauge handle;
+// wd_set_tuning changes one of them later.  A negative value means "not set: use the launcher's default".
+struct Tuning {
+    int tile_ty = -1, tile_tz = -1; // WD_TILE_SHAPE=ty,tz
+    int tile_tc = -1;               // WD_TILE_TC      slices per t-chunk
+    int tile_nchunk = -1;           // WD_TILE_NCHUNK  t-chunks (overrides tile_tc)
+    int tile_nrb = -1;              // WD_TILE_NRB     right-hand sides per CTA of the multi-RHS kernel
+    int mrhs_patch = -1;            // WD_MRHS_PATCH   side of the tile-column patch of the multi-RHS block order (0 = off)
+    int stage_no_mrhs = -1;         // WD_STAGE_NO_MRHS  1 = run several right-hand sides through the single-RHS staged kernel
+    int site_slab_mb = -1;          // WD_SITE_SLAB_MB  link slab of the site kernel's multi-RHS block order
+    int host_no_pipeline = -1;      // WD_HOST_NO_PIPELINE  1 = one-stream wd_apply_host
+    int mrhs_no_tail = -1;          // WD_MRHS_NO_TAIL  1 = no shortened t-chunks in the last wave of the multi-RHS kernel
+};
+void tuning_from_env(Tuning &t);
+int tuning_set(Tuning &t, const char *name, int value); // 0 = ok, -1 = unknown name
+const Tuning &default_tuning();
+} // namespace wd
+
 struct wd_lattice {
     unsigned magic;
     int dims[4];      // Lx, Ly, Lz, Lt
@@ -17,6 +36,8 @@ struct wd_gauge {
     int recon;        // 18 / 12
     int kernel;       // wd_kernel selector
     int tgauge;       // wd_set_temporal_gauge: U_t(x,t) = 1 for t < Lt-1 (verified when set)
+    wd::Tuning tune;  // tuning variables, read once at wd_load_gauge
+    int pipe_ready;   // the three streams and 34 events of the pipelined host path all exist
     void *links;      // native links, device (cudaMalloc)
     size_t links_bytes;
     cudaStream_t stream;
@@ -48,7 +69,8 @@ struct ApplyArgs {
     int precision;
     int recon;
     cudaStream_t stream;
-    int dagger;                     // site kernel only: apply D^dagger = gamma5 D gamma5 instead of D
+    const Tuning *tune;             // never null inside the launchers (default_tuning() when the caller has none)
+    int dagger;                     // apply D^dagger = gamma5 D gamma5 instead of D (site and single-RHS staged kernels)
     int tgauge;                     // links are in temporal gauge (U_t = 1 for t < Lt-1): kernels may skip them
     long long site_begin, site_end; // site kernel only: apply on [site_begin, site_end); 0,0 = whole lattice
 };
@@ -57,12 +79,13 @@ void count_launch(int n = 1);
 
 // one thread per site, any extents >= 1
 cudaError_t launch_site(const ApplyArgs &a);
-// shared-memory tiled kernel; supported() is a pure host-side predicate
-bool tile_supported(const ApplyArgs &a);
-cudaError_t launch_tile(const ApplyArgs &a);
-// tile kernel with every global read staged through shared memory by cp.async (fp32)
+// t-marching tile kernel with every global read staged through shared memory by cp.async (fp32 and fp64);
+// stage_supported() is a pure host-side predicate
 bool stage_supported(const ApplyArgs &a);
 cudaError_t launch_stage(const ApplyArgs &a);
+// cudaFuncAttributeMaxDynamicSharedMemorySize is per device: set it once per (kernel, device), thread-safe
+cudaError_t ensure_dynamic_smem(const void *kernel, size_t bytes, size_t *per_device_cache);
+int sm_count(); // multiprocessors of the current device (cached per device)
 
 // site range [site0, site0 + nsites) of every right-hand side; site0 a multiple of 128; nsites < 0 = all
 cudaError_t launch_pack_spinor(void *native, const void *canonical, long long V, int nrhs, int precision,

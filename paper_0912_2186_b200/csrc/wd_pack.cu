@@ -137,7 +137,7 @@ __global__ void check_temporal_gauge_kernel(const T *__restrict__ links, long lo
         unpack(q[(r / L::CR) * BLK], v);
         const int elem = i / 2, a = elem / 3, b = elem % 3;
         const double want = (i % 2 == 0 && a == b) ? 1.0 : 0.0;
-        if (fabs((double)v[r % L::CR] - want) > tol) bad = true;
+        if (!(fabs((double)v[r % L::CR] - want) <= tol)) bad = true; // (NaN fails too)
     }
     if (bad) atomicOr(flag, 1);
 }

@@ -6,7 +6,13 @@
   C5  the paper's own example eq. (2.4): one vector, constant in a single spin-colour component on 4^4 blocks, gives
       P = theta / 2^d with d = 4, i.e. entries 1/16 inside the block
   C6  span: the first k columns span the same space as the first k input vectors on every block (Gram-Schmidt order)
+  C7  the explicit 9-point stencil (coarse_stencil / coarse_apply_stencil) equals the composition P^dagger D P c of the
+      pinned pieces (C1-C4 and the pinned D), on coarse lattices with extents 1, 2 and 3 (coincident neighbour blocks)
+  C8  gamma5-hermiticity block by block: A = s3 A^dag s3 and B_mu(b) = s3 F_mu(b - mu)^dag s3
+  C9  free field, the paper's piecewise-constant example: closed-form entries in tests/golden/coarse_free_field.txt
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -89,3 +95,51 @@ def test_c6_nested_spans():
 def test_bad_dims_are_refused():
     with pytest.raises(ValueError):
         wc.block_orthonormalise(vectors(1, dims=(6, 4, 4, 8)), (6, 4, 4, 8))
+
+
+@pytest.mark.parametrize("dims", [(8, 4, 4, 8), (12, 4, 8, 4), (4, 4, 4, 4)])
+def test_c7_stencil_equals_the_galerkin_composition(dims):
+    nv = 3
+    W = wc.block_orthonormalise(vectors(nv, 321, dims), dims)
+    U, _ = random_fields(dims, 323)
+    mass = -0.2
+    S = wc.coarse_stencil(W, c2r(U), dims, mass)
+    assert S.shape == (dims[3] // 4, dims[2] // 4, dims[1] // 4, dims[0] // 4, 9, 2 * nv, 2 * nv)
+    for seed in (325, 327):
+        c = rand_coarse(nv, seed, dims)
+        assert np.max(np.abs(wc.coarse_apply_stencil(S, c) - wc.coarse_apply(W, c, c2r(U), dims, mass))) < 1e-12
+
+
+def test_c8_stencil_gamma5_hermiticity_block_by_block():
+    dims, nv = (12, 4, 8, 8), 2
+    W = wc.block_orthonormalise(vectors(nv, 331, dims), dims)
+    U, _ = random_fields(dims, 333)
+    S = wc.coarse_stencil(W, c2r(U), dims, 0.1)
+    s3 = np.diag(np.repeat([1.0, -1.0], nv))
+    dag = lambda M: np.conj(np.swapaxes(M, -1, -2))
+    assert np.max(np.abs(S[..., 0, :, :] - s3 @ dag(S[..., 0, :, :]) @ s3)) < 1e-13
+    for mu in range(4):
+        F_shifted = np.roll(S[..., 1 + mu, :, :], +1, axis=3 - mu)       # F_mu(b - mu) at position b
+        assert np.max(np.abs(S[..., 5 + mu, :, :] - s3 @ dag(F_shifted) @ s3)) < 1e-13
+    assert np.max(np.abs(S[..., 1:, :, :])) > 1e-3                       # (not trivially zero)
+
+
+def test_c9_free_field_golden_stencil():
+    dims = (8, 4, 8, 4)
+    psi = np.zeros((1, dims[3], dims[2], dims[1], dims[0], 4, 3), dtype=np.complex128)
+    psi[0, ..., 0, 0] = 2.5
+    psi[0, ..., 2, 0] = -1.5
+    W = wc.block_orthonormalise(psi, dims)
+    U = np.zeros((4, dims[3], dims[2], dims[1], dims[0], 3, 3, 2))
+    for i in range(3):
+        U[..., i, i, 0] = 1.0
+    S = wc.coarse_stencil(W, U, dims, -0.25)
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "coarse_free_field.txt"))
+            if l.strip() and not l.startswith("#")]
+    assert len(rows) == 9
+    sgn = np.sign(2.5) * np.sign(-1.5)                                  # relative sign of the two normalised columns
+    for r in rows:
+        k = int(r[0])
+        v = [float(x) for x in r[1:]]
+        want = np.array([[v[0] + 1j * v[1], sgn * (v[2] + 1j * v[3])], [sgn * (v[4] + 1j * v[5]), v[6] + 1j * v[7]]])
+        assert np.max(np.abs(S[..., k, :, :] - want)) < 1e-14, k

@@ -13,7 +13,7 @@ from gpu_util import TOL, GpuOp, np_dtype, oracle_apply, rel_l2
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = {"auto": 0, "site": 1, "tile": 2, "stage": 3}
+KERNELS = {"auto": 0, "site": 1, "stage": 3}
 
 
 def oracle_links(U, recon):
@@ -79,35 +79,7 @@ def test_nrhs_sweep(oracle, nrhs):
     check_config(oracle, cfg, "auto")
 
 
-# ---------------------------------------------------------------- the shared-memory t-marching kernel
-TILE_SHAPES = [(32, 4, 4, 4), (16, 8, 8, 6), (8, 4, 4, 12), (4, 8, 16, 5), (32, 8, 8, 3), (32, 2, 2, 2), (16, 2, 4, 1),
-               (32, 1, 1, 1), (8, 12, 4, 7)]
-
-
-@pytest.mark.parametrize("dims", TILE_SHAPES)
-@pytest.mark.parametrize("precision,recon", [(32, 18), (32, 12), (64, 18), (64, 12)])
-def test_tile_kernel_shapes(oracle, dims, precision, recon):
-    cfg = fields.Config("tile", dims, precision, "haar", recon, -0.3, 1, 13)
-    check_config(oracle, cfg, "tile", nrhs=1)
-    check_config(oracle, cfg, "tile", nrhs=3)
-
-
-@pytest.mark.parametrize("shape", ["1,1", "2,1", "2,2", "4,1", "4,2", "8,1", "1,2", "2,4"])
-@pytest.mark.parametrize("precision", [32, 64])
-def test_tile_kernel_forced_tile_shapes(oracle, monkeypatch, shape, precision):
-    """Every tile shape (WD_TILE_SHAPE=ty,tz) gives the same operator; shapes the precision cannot
-    hold fall back to the automatic choice, which must still be right."""
-    monkeypatch.setenv("WD_TILE_SHAPE", shape)
-    cfg = fields.Config("tileshape", (32, 8, 8, 5), precision, "smooth", 18, -0.42, 1, 17)
-    check_config(oracle, cfg, "tile")
-
-
-@pytest.mark.parametrize("name", ["c1_16x32_fp32", "c3_32x64_fp32", "c3_32x64_fp64"])
-def test_tile_kernel_baseline_configs(oracle, name):
-    check_config(oracle, fields.CONFIGS[name], "tile")
-
-
-# ---------------------------------------------------------------- the cp.async-staged tile kernel (fp32)
+# ---------------------------------------------------------------- the cp.async-staged t-marching kernels (fp32, fp64)
 STAGE_SHAPES = [(32, 4, 4, 4), (16, 8, 8, 6), (8, 4, 4, 12), (4, 8, 16, 5), (32, 8, 8, 3), (32, 2, 2, 2), (16, 2, 4, 1),
                 (32, 6, 10, 4), (8, 12, 4, 7),
                 # Lx not a power of two: x hops through shared memory instead of warp shuffles
@@ -180,29 +152,6 @@ def test_stage_kernel_deterministic():
     cfg = fields.Config("det", (32, 8, 8, 16), 32, "smooth", 18, -0.42, 1, 19)
     U, psi = fields.make_fields(cfg)
     op = GpuOp(U, cfg.dims, 32, 18, KERNELS["stage"])
-    a = op.apply(psi, cfg.mass, return_native=True).clone()
-    for _ in range(20):
-        b = op.apply(psi, cfg.mass, return_native=True)
-    assert torch.equal(a, b)
-    op.close()
-
-
-def test_tile_kernel_rejects_unsupported_lattice():
-    from paper_0912_2186_b200 import binding
-    cfg = fields.Config("bad", (24, 4, 4, 4), 32, "haar", 18, 0.1, 1, 3)
-    U, _ = fields.make_fields(cfg)
-    op = GpuOp(U, cfg.dims, 32, 18)
-    with pytest.raises(binding.WdError) as e:
-        binding.wd_set_kernel(op.op.gauge, KERNELS["tile"])
-    assert e.value.code == -7
-    op.close()
-
-
-def test_tile_kernel_deterministic():
-    import torch
-    cfg = fields.Config("det", (32, 8, 8, 16), 32, "smooth", 18, -0.42, 1, 19)
-    U, psi = fields.make_fields(cfg)
-    op = GpuOp(U, cfg.dims, 32, 18, KERNELS["tile"])
     a = op.apply(psi, cfg.mass, return_native=True).clone()
     for _ in range(20):
         b = op.apply(psi, cfg.mass, return_native=True)
@@ -338,7 +287,7 @@ def test_apply_host_pipelined_path(oracle, monkeypatch, dims, precision, recon, 
     again = np.full_like(psi, np.nan)
     op.op.apply_host(again, psi, cfg.mass, nrhs)
     assert np.array_equal(out, again)
-    monkeypatch.setenv("WD_HOST_NO_PIPELINE", "1")
+    op.op.set_tuning("host_no_pipeline", 1)
     plain = np.full_like(psi, np.nan)
     op.op.apply_host(plain, psi, cfg.mass, nrhs)
     op.close()
@@ -385,6 +334,72 @@ def test_apply_dagger_matches_the_oracle_and_gamma5_hermiticity(oracle, dims, pr
     rhs = np.vdot(cplx(d[0]), ps)                              # <D phi, psi>
     assert abs(lhs - rhs) <= (1e-11 if precision == 64 else 2e-4) * abs(rhs) + (1e-9 if precision == 64 else 1e-2)
     op.close()
+
+
+# ---------------------------------------------------------------- round 2: dagger / Lx = 24 / fp64 members of the staged family
+@pytest.mark.parametrize("dims", [(32, 4, 4, 5), (16, 8, 8, 6), (8, 4, 12, 6), (4, 4, 4, 4), (24, 4, 4, 6), (12, 8, 4, 3)])
+@pytest.mark.parametrize("precision,recon", [(64, 18), (32, 18), (32, 12), (64, 12)])
+@pytest.mark.parametrize("nrhs", [1, 3])
+def test_staged_dagger_matches_the_oracle(oracle, dims, precision, recon, nrhs):
+    """wd_apply_dagger through the STAGED kernel (templated on the projector sign): D^dagger = gamma5 D gamma5
+     against the oracle's sign=+1 operator; several right-hand sides go through the single-RHS member in
+    the (patch, column, right-hand side) block order."""
+    import torch
+    cfg = fields.Config("sdag", dims, precision, "haar", recon, -0.3, nrhs, 93)
+    U, psi = fields.make_fields(cfg)
+    Uo = oracle_links(U, recon).astype(np.float64)
+    op = GpuOp(U, dims, precision, recon, KERNELS["stage"])
+    w = op.op
+    canon = torch.from_numpy(psi).cuda()
+    a = torch.empty(w.native_numel(nrhs), dtype=canon.dtype, device="cuda")
+    b = torch.full_like(a, float("nan"))
+    out = torch.empty_like(canon)
+    w.pack(a, canon, nrhs)
+    w.apply_dagger(b, a, cfg.mass, nrhs)
+    w.unpack(out, b, nrhs)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    op.close()
+    for r in range(nrhs):
+        want = oracle.apply(psi[r].astype(np.float64), Uo, dims, cfg.mass, sign=+1)
+        assert rel_l2(got[r], want) <= TOL[precision]
+
+
+@pytest.mark.parametrize("dims,nrhs", [((24, 8, 4, 6), 20), ((24, 4, 4, 5), 7), ((12, 8, 8, 4), 4), ((24, 2, 2, 3), 3)])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_multi_rhs_kernel_when_lx_is_not_a_power_of_two(oracle, dims, nrhs, recon):
+    """The paper's volumes have Lx = 24 and N_v = 20: the multi-RHS kernel shares the
+    staged links there too (x hops through the slice buffer instead of warp shuffles)."""
+    cfg = fields.Config("mrhs24", dims, 32, "haar", recon, -0.41, nrhs, 95)
+    check_config(oracle, cfg, "stage")
+
+
+@pytest.mark.parametrize("dims,nrhs", [((32, 8, 8, 4), 5), ((16, 4, 8, 6), 24), ((24, 4, 4, 3), 4)])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_fp64_multi_rhs_shares_links_through_l2(oracle, dims, nrhs, recon):
+    """fp64, several right-hand sides: the single-RHS staged kernel in the (patch of columns, right-hand side fastest)
+    block order; every right-hand side against the oracle at the fp64 bound."""
+    cfg = fields.Config("mrhs64", dims, 64, "haar", recon, -0.41, nrhs, 97)
+    check_config(oracle, cfg, "stage")
+
+
+def test_multi_rhs_tail_wave_split_is_bit_identical(oracle):
+    """A launch of more work items than SMs whose last wave is partial cuts that wave's items into shorter marches
+    (wd_dslash_mrhs.cu); the result is bit-identical to the uncut launch and matches the oracle."""
+    import torch
+    cfg = fields.Config("tail", (32, 16, 16, 16), 32, "smooth", 18, -0.42, 24, 99)   # 64 columns x 8 groups = 512 items
+    U, psi = fields.make_fields(cfg)
+    op = GpuOp(U, cfg.dims, 32, 18, KERNELS["stage"])
+    a = op.apply(psi, cfg.mass, return_native=True).clone()
+    op.op.set_tuning("mrhs_no_tail", 1)
+    b = op.apply(psi, cfg.mass, return_native=True).clone()
+    op.op.set_tuning("mrhs_no_tail", -1)
+    got = op.apply(psi, cfg.mass)
+    op.close()
+    assert torch.equal(a, b)
+    want = oracle_apply(oracle, psi[:3], U, cfg.dims, cfg.mass)
+    for r in range(3):
+        assert rel_l2(got[r], want[r]) <= TOL[32]
 
 
 def test_auto_kernel_selection():

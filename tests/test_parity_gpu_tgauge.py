@@ -8,7 +8,7 @@ from paper_0912_2186_b200 import binding, fields
 from gpu_util import TOL, GpuOp, rel_l2
 
 pytestmark = pytest.mark.gpu
-KERNELS = {"auto": 0, "site": 1, "tile": 2, "stage": 3}
+KERNELS = {"auto": 0, "site": 1, "stage": 3}
 
 
 def test_generator_fixes_the_gauge_and_keeps_the_operator(oracle):
