@@ -676,6 +676,75 @@ def run_transfer(args):
     binding.wd_destroy(lat)
 
 
+def run_coarse(args):
+    """--op coarse: the explicit coarse operator Dhat = P^dagger D P (row f3) with N_v = 20 on the
+    workload's lattice: wd_build_coarse timed once, then a step = APPLIES wd_apply_coarse calls.  Per coarse site the apply
+    streams nine (2 N_v)^2 complex matrices once: algorithmic bytes = 9 n^2 2w + (nrhs) (1 + 1) n 2w, flops = 9 n^2 8 nrhs."""
+    import torch
+    from paper_0912_2186_b200 import binding, build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    build.build()
+    cfg = fields.CONFIGS[args.workload]
+    nv, nrhs = 20, (args.nrhs or 1)
+    n = 2 * nv
+    V = fields.volume(cfg.dims)
+    nb = V // 256
+    w = 4 if cfg.precision == 32 else 8
+    tdt = torch.float32 if cfg.precision == 32 else torch.float64
+    g = torch.Generator(device="cuda").manual_seed(cfg.seed)
+    Lx, Ly, Lz, Lt = cfg.dims
+    stream = torch.cuda.current_stream()
+    u_dev = torch.randn((4, Lt, Lz, Ly, Lx, 3, 3, 2), dtype=tdt, device="cuda", generator=g) * 0.5   # cost is data independent
+    op = binding.WilsonDirac(cfg.dims, u_dev, cfg.precision, 18, stream=stream.cuda_stream)
+    del u_dev
+    basis = torch.randn(op.native_numel(nv), dtype=tdt, device="cuda", generator=g)
+    binding.wd_block_orthonormalise(op.lat, basis, nv, cfg.precision, stream.cuda_stream)
+    ns = binding.wd_coarse_stencil_reals(op.lat, nv)
+    S = torch.empty(ns, dtype=tdt, device="cuda")
+    scratch = torch.empty(ns, dtype=tdt, device="cuda")
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    binding.wd_build_coarse(op.gauge, S, scratch, basis, cfg.mass, cfg.dims, nv, cfg.precision)   # warm-up
+    ev[0].record()
+    binding.wd_build_coarse(op.gauge, S, scratch, basis, cfg.mass, cfg.dims, nv, cfg.precision)
+    ev[1].record()
+    del scratch
+    cin = [torch.randn(nrhs * nb * n * 2, dtype=tdt, device="cuda", generator=g) for _ in range(2)]
+    cout = [torch.empty_like(cin[0]) for _ in range(2)]
+    aps = args.applies_per_step
+    for i in range(max(args.warmup, 3) * 3):
+        binding.wd_apply_coarse(op.lat, cout[i % 2], cin[i % 2], S, nv, nrhs, cfg.precision, stream.cuda_stream)
+    torch.cuda.synchronize()
+    n0 = binding.wd_launch_count()
+    with ClockSampler(0) as clocks:
+        ev[2].record()
+        for i in range(args.steps * aps):
+            binding.wd_apply_coarse(op.lat, cout[i % 2], cin[i % 2], S, nv, nrhs, cfg.precision, stream.cuda_stream)
+        ev[3].record()
+        torch.cuda.synchronize()
+    ms = ev[2].elapsed_time(ev[3]) / (args.steps * aps)
+    bytes_apply = nb * (9 * n * n * 2 * w + nrhs * 2 * n * 2 * w)
+    flops_apply = nb * 9 * n * n * 8 * nrhs
+    peak, peak_src = measured_peak()
+    achieved = bytes_apply / (ms * 1e-3) / 1e9
+    build_ms = ev[0].elapsed_time(ev[1])
+    build_flops = V * 9 * nv * nv * 4 * 6 * 8   # the W^dag H contractions only (96 complex multiply-adds per site, pair, term)
+    line = {"metric": "mg_coarse_apply_gflops", "value": flops_apply / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms * aps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if cfg.precision == 32 else "f64",
+            "data": "device-random links and vectors (cost is data independent)",
+            "config": {"workload": cfg.name, "op": "coarse operator apply, 9-point stencil of (2 N_v)^2 complex blocks",
+                       "dims": list(cfg.dims), "coarse_dims": [d // 4 for d in cfg.dims], "nv": nv, "nrhs": nrhs,
+                       "applies_per_step": aps, "build_ms": build_ms, "build_gflops": build_flops / (build_ms * 1e-3) / 1e9,
+                       "stencil_MB": ns * w / 1e6, "l2": "stencil larger than L2, no flush"},
+            "us_per_apply": ms * 1e3, "clocks": clocks.summary(), "gpu_launches": int(binding.wd_launch_count() - n0),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src, "bytes_per_launch": bytes_apply,
+                         "kernel": "wd coarse_apply_kernel"}}
+    print(json.dumps(line), flush=True)
+    op.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -685,7 +754,7 @@ def main():
     ap.add_argument("--kernel", default="auto", choices=["auto", "site", "stage"])
     ap.add_argument("--recon", type=int, default=None, choices=[18, 12])
     ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
-    ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr", "bicgstab", "gcr", "transfer"],
+    ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr", "bicgstab", "gcr", "transfer", "coarse"],
                     help="full = D of eq. (2.2) (the headline); schur = even-odd preconditioned operator (row f1); cgnr = CG on its normal equations (row f2, --applies-per-step = iterations)")
     ap.add_argument("--nrhs", type=int, default=None,
                     help="override the workload's number of right-hand sides (e.g. 20 = the paper's N_v, PAPER.md:124)")
@@ -708,6 +777,8 @@ def main():
         run_schur(args)
     elif args.op == "transfer":
         run_transfer(args)
+    elif args.op == "coarse":
+        run_coarse(args)
     elif args.op in ("cgnr", "bicgstab", "gcr"):
         run_cgnr(args)
     else:

@@ -260,6 +260,30 @@ int wd_restrict(const wd_lattice *lat, void *coarse_dev, const void *basis_nativ
 int wd_prolong(const wd_lattice *lat, void *psi_native_dev, const void *basis_native_dev, const void *coarse_dev, int nv,
                int precision, void *stream);
 
+/*
+ * The coarse operator as an explicit stencil (PAPER.md:82-88 Galerkin form Dhat = P^dagger D P; PAPER.md:116 4^4 blocks
+ * x chirality; "the N_V x N_V complex matrix operations needed for the coarse operators").  D couples
+ * nearest neighbours, so Dhat couples a block b to itself and its 8 neighbour blocks; with the coarse index
+ * i = sigma * nv + alpha (n = 2 nv per block, as in wd_restrict's output) there are nine n x n complex matrices per block
+ *   k = 0: A(b);  k = 1 + mu: F_mu(b) (acts on c(b + mu));  k = 5 + mu: B_mu(b) (acts on c(b - mu)),  mu = 0..3 = x,y,z,t
+ *   (Dhat c)(b) = A(b) c(b) + sum_mu [ F_mu(b) c(b+mu) + B_mu(b) c(b-mu) ]        periodic coarse lattice of L/4 blocks
+ * A hop belongs to F_mu / B_mu when it leaves the block through its +mu / -mu face, whatever block it lands in (coarse
+ * extent 1 or 2: coincident neighbour blocks simply add; reading S4).  Device layout of the stencil:
+ *   S[block][k][column j][row i][re, im]   (column major) in the working precision; wd_coarse_stencil_reals() reals.
+ *
+ * wd_build_coarse: stencil from the columns of P (`basis_native_dev`: nv vectors as nv right-hand sides of one native
+ * buffer, orthonormalised per block and chirality by wd_block_orthonormalise) and the gauge's links and mass.  The
+ * Galerkin products are formed as written (the diagonal term as (4+m) W^dag W, not assumed to be (4+m) 1).  `scratch_dev`:
+ * caller-owned, same size as the stencil, overwritten.  Launches on the gauge's stream; deterministic (no atomics).
+ * nv <= 32, at most 65535 blocks.  wd_apply_coarse: out[r] = Dhat in[r] for nrhs coarse vectors
+ * [rhs][block][sigma][alpha][re, im] (wd_coarse_reals() reals each); out must not overlap in; nv <= 56.
+ */
+long long wd_coarse_stencil_reals(const wd_lattice *lat, int nv);
+int wd_build_coarse(const wd_gauge *gauge, void *stencil_dev, void *scratch_dev, const void *basis_native_dev, double mass,
+                    const int dims[4], int nv, int precision);
+int wd_apply_coarse(const wd_lattice *lat, void *out_coarse_dev, const void *in_coarse_dev, const void *stencil_dev, int nv,
+                    int nrhs, int precision, void *stream);
+
 /* Number of CUDA kernels the library has launched in this process (all handles). */
 long long wd_launch_count(void);
 

@@ -24,7 +24,7 @@ STATUS_NAMES = {
 SYMBOLS = (
     "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
     "wd_set_kernel", "wd_set_tuning", "wd_set_temporal_gauge", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
-    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_coarse_reals",
+    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_coarse_reals", "wd_coarse_stencil_reals", "wd_build_coarse", "wd_apply_coarse",
     "wd_block_orthonormalise", "wd_restrict", "wd_prolong", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_dagger", "wd_apply_host",
     "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
 )
@@ -77,6 +77,12 @@ def lib():
     L.wd_gcr_schur.argtypes = [vp, vp, vp, d, ip, i, i, i, i, d, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]
     L.wd_coarse_reals.argtypes = [vp, i]
     L.wd_coarse_reals.restype = ctypes.c_longlong
+    L.wd_coarse_stencil_reals.argtypes = [vp, i]
+    L.wd_coarse_stencil_reals.restype = ctypes.c_longlong
+    L.wd_build_coarse.argtypes = [vp, vp, vp, vp, d, ip, i, i]
+    L.wd_build_coarse.restype = i
+    L.wd_apply_coarse.argtypes = [vp, vp, vp, vp, i, i, i, vp]
+    L.wd_apply_coarse.restype = i
     L.wd_block_orthonormalise.argtypes = [vp, vp, i, i, vp]
     L.wd_restrict.argtypes = [vp, vp, vp, vp, i, i, vp]
     L.wd_prolong.argtypes = [vp, vp, vp, vp, i, i, vp]
@@ -284,6 +290,20 @@ def wd_restrict(lat, coarse_dev, basis_native_dev, psi_native_dev, nv, precision
 def wd_prolong(lat, psi_native_dev, basis_native_dev, coarse_dev, nv, precision, stream=None):
     _check(lib().wd_prolong(lat, _ptr(psi_native_dev), _ptr(basis_native_dev), _ptr(coarse_dev), int(nv), int(precision),
                             _ptr(stream)), "wd_prolong")
+
+
+def wd_coarse_stencil_reals(lat, nv):
+    return int(lib().wd_coarse_stencil_reals(lat, int(nv)))
+
+
+def wd_build_coarse(gauge, stencil_dev, scratch_dev, basis_native_dev, mass, dims, nv, precision):
+    _check(lib().wd_build_coarse(gauge, _ptr(stencil_dev), _ptr(scratch_dev), _ptr(basis_native_dev), float(mass), _dims(dims),
+                                 int(nv), int(precision)), "wd_build_coarse")
+
+
+def wd_apply_coarse(lat, out_coarse_dev, in_coarse_dev, stencil_dev, nv, nrhs, precision, stream=None):
+    _check(lib().wd_apply_coarse(lat, _ptr(out_coarse_dev), _ptr(in_coarse_dev), _ptr(stencil_dev), int(nv), int(nrhs),
+                                 int(precision), _ptr(stream)), "wd_apply_coarse")
 
 
 def wd_destroy_gauge(gauge):

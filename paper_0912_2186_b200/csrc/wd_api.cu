@@ -723,6 +723,46 @@ int wd_prolong(const wd_lattice *lat, void *psi_native_dev, const void *basis_na
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_prolong");
 }
 
+long long wd_coarse_stencil_reals(const wd_lattice *lat, int nv)
+{
+    if (check_transfer("wd_coarse_stencil_reals", lat, nv, WD_FP32)) return -1;
+    return lat->V / 256 * 9 * (2LL * nv) * (2LL * nv) * 2;
+}
+
+int wd_build_coarse(const wd_gauge *gauge, void *stencil_dev, void *scratch_dev, const void *basis_native_dev, double mass,
+                    const int dims[4], int nv, int precision)
+{
+    if (!gauge || !stencil_dev || !scratch_dev || !basis_native_dev || !dims) return fail(WD_ERR_NULL, "wd_build_coarse: NULL argument");
+    if (gauge->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_build_coarse: not a live wd_gauge handle");
+    if (!valid_precision(precision) || precision != gauge->precision)
+        return fail(WD_ERR_PRECISION, "wd_build_coarse: precision %d, gauge was loaded in %d", precision, gauge->precision);
+    for (int d = 0; d < 4; ++d) {
+        if (dims[d] != gauge->dims[d]) return fail(WD_ERR_DIMS, "wd_build_coarse: dims[%d]=%d but gauge lattice has %d", d, dims[d], gauge->dims[d]);
+        if (dims[d] % 4) return fail(WD_ERR_DIMS, "wd_build_coarse: extents must be multiples of the 4^4 block");
+    }
+    if (nv < 1 || nv > 32) return fail(WD_ERR_NRHS, "wd_build_coarse: nv=%d (1..32)", nv);
+    if (gauge->V / 256 > 65535) return fail(WD_ERR_DIMS, "wd_build_coarse: more than 65535 blocks");
+    const size_t sb = (size_t)(gauge->V / 256) * 9 * (2 * nv) * (2 * nv) * 2 * (precision == WD_FP32 ? 4 : 8);
+    if (overlap(stencil_dev, sb, scratch_dev, sb)) return fail(WD_ERR_ALIAS, "wd_build_coarse: stencil and scratch overlap");
+    cudaError_t e = wd::launch_coarse_build(stencil_dev, scratch_dev, basis_native_dev, gauge->links, gauge->dims, gauge->V, nv,
+                                            mass, precision, gauge->recon, gauge->stream);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_build_coarse");
+}
+
+int wd_apply_coarse(const wd_lattice *lat, void *out_coarse_dev, const void *in_coarse_dev, const void *stencil_dev, int nv,
+                    int nrhs, int precision, void *stream)
+{
+    int rc = check_transfer("wd_apply_coarse", lat, nv, precision);
+    if (rc) return rc;
+    if (!out_coarse_dev || !in_coarse_dev || !stencil_dev) return fail(WD_ERR_NULL, "wd_apply_coarse: NULL argument");
+    if (nrhs < 1) return fail(WD_ERR_NRHS, "wd_apply_coarse: nrhs=%d", nrhs);
+    if (nv > 56) return fail(WD_ERR_NRHS, "wd_apply_coarse: nv=%d (9 * 2 nv threads must fit one CTA)", nv);
+    const size_t cb = (size_t)nrhs * (size_t)(lat->V / 256) * 2 * nv * 2 * (precision == WD_FP32 ? 4 : 8);
+    if (overlap(out_coarse_dev, cb, in_coarse_dev, cb)) return fail(WD_ERR_ALIAS, "wd_apply_coarse: out and in overlap");
+    cudaError_t e = wd::launch_coarse_apply(out_coarse_dev, in_coarse_dev, stencil_dev, lat->dims, nv, nrhs, precision, (cudaStream_t)stream);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply_coarse");
+}
+
 long long wd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 const char *wd_last_error(void) { return g_err; }

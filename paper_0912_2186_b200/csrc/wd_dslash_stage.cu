@@ -1,13 +1,12 @@
 // wd_dslash_stage.cu -- WD_KERNEL_STAGE: the t-marching tile kernel with EVERY global read staged
 // through shared memory by cp.async one step ahead (fp32 and fp64).
 //
-// eq. (2.2); SURVEY.md 8(a) steps a1-a7 in one launch.  Same decomposition as
-// wd_dslash_tile.cu (tile Lx x ty x tz of one time slice per CTA, marching along t; x hops by warp
-// shuffles, y/z hops through a shared-memory slice, backward hops computed at the source site and
-// handed over through shared memory, t hops in registers).  What differs: ncu showed the tile
-// kernel latency bound (profiles/r01_tile_ncu.md: ~60 % of the stall samples are the first use of a
-// link / face load, 4-5 dependent L2/HBM round trips per slice with 16 warps per SM).  Here no
-// arithmetic ever waits for HBM or L2:
+// eq. (2.2); SURVEY.md 8(a) steps a1-a7 in one launch.  Decomposition: a CTA owns a tile
+// Lx x ty x tz of one time slice and marches along t over a chunk of slices; x hops by warp
+// shuffles, y/z hops through a shared-memory slice, backward hops computed at the source site (which
+// holds the link) and handed over through shared memory, t hops in registers.  The round-1 tile kernel
+// with this decomposition but plain global loads was latency bound (profiles/r01_tile_stage_ncu.md: ~60 % of
+// the stall samples were the first use of a link / face load); here no arithmetic ever waits for HBM or L2:
 //
 //   * the four links of the thread's site, its out-of-tile face neighbours (spinor, plus the link for
 //     a backward face) and its own spinor of the next slice are all copied global -> shared by
@@ -501,8 +500,14 @@ cudaError_t launch_mrhs(const ApplyArgs &a, int ty, int tz); // wd_dslash_mrhs.c
 cudaError_t launch_stage(const ApplyArgs &a)
 {
     const Tuning &tn = a.tune ? *a.tune : default_tuning();
-    if (a.precision == 32 && a.nrhs > 1 && !a.dagger && tn.stage_no_mrhs <= 0) {
-        StageShape s; // several right-hand sides: the kernel that shares the staged links between them
+    // several fp32 right-hand sides: the kernel that shares the staged links between them in shared memory when Lx is
+    // a power of two (measured, profiles/r02_mrhs.md: 24 RHS on 32^3 x 64 3.0 ms against 3.6 ms for the single-RHS member
+    // in the patch order); for other Lx (x hops through shared memory) the single-RHS member in the (patch, column,
+    // right-hand side) order, which shares the links through L2, is the faster one (20 RHS on 24^3 x 64: 1.30 against
+    // 1.39 ms).  stage_no_mrhs = 0 / 1 forces the choice.
+    const bool pow2 = !(a.dims[0] & (a.dims[0] - 1));
+    if (a.precision == 32 && a.nrhs > 1 && !a.dagger && (tn.stage_no_mrhs < 0 ? pow2 : tn.stage_no_mrhs == 0)) {
+        StageShape s;
         if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
         if (s.nt <= 128) return launch_mrhs(a, s.ty, s.tz); // (a forced bigger tile runs through the single-RHS kernel below)
     }

@@ -105,6 +105,11 @@ int gcr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, doubl
 // transfer operators of the multigrid set-up (wd_transfer.cu)
 cudaError_t launch_transfer(int what, void *a, const void *b, const void *c, const int dims[4], long long V, int nv,
                             int precision, cudaStream_t s);
+// explicit coarse operator (wd_coarse.cu): build the 9-point stencil from the basis and the links; apply it
+cudaError_t launch_coarse_build(void *S, void *part, const void *W, const void *links, const int dims[4], long long V, int nv,
+                                double mass, int precision, int recon, cudaStream_t s);
+cudaError_t launch_coarse_apply(void *out, const void *in, const void *S, const int dims[4], int nv, int nrhs, int precision,
+                                cudaStream_t s);
 cudaError_t launch_parity_copy(void *native, void *canon, const int dims[4], long long V, int nrhs, int precision,
                                int parity, bool to_native, cudaStream_t s);
 cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon,

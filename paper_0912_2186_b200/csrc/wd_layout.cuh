@@ -74,6 +74,20 @@ __device__ __forceinline__ void load_spinor(const T *__restrict__ field, long lo
     }
 }
 
+// same, through ordinary coherent loads: for fields the SAME launch also writes (ld.global.nc / __ldg is only valid
+// for data that stays read-only for the whole kernel)
+template <typename T>
+__device__ __forceinline__ void load_spinor_rw(const T *field, long long site, T (&p)[24])
+{
+    using L = SpinorLayout<T>;
+    const typename L::Vec *q = reinterpret_cast<const typename L::Vec *>(field) + (site >> 5) * (L::NCH * BLK) + (site & (BLK - 1));
+#pragma unroll
+    for (int c = 0; c < L::NCH; ++c) {
+        const typename L::Vec v = q[c * BLK];
+        unpack(v, &p[c * L::CR]);
+    }
+}
+
 template <typename T>
 __device__ __forceinline__ void store_spinor(T *__restrict__ field, long long site, const T (&p)[24])
 {

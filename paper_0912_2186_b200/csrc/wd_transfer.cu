@@ -62,17 +62,17 @@ template <typename T> __device__ __forceinline__ void chiral_dots(const T (&a)[2
 }
 
 template <typename T>
-__global__ void __launch_bounds__(TB) block_orthonormalise_kernel(T *__restrict__ vecs, int Lx, int Ly, int Lz, long long V, int nv)
+__global__ void __launch_bounds__(TB) block_orthonormalise_kernel(T *vecs, int Lx, int Ly, int Lz, long long V, int nv)
 {
     __shared__ double sh[TB / 32];
     const long long site = block_site(threadIdx.x, blockIdx.x, Lx, Ly, Lz);
     const long long stride = 24 * padded_volume(V);
     for (int a = 0; a < nv; ++a) {
         T v[24];
-        load_spinor(vecs + a * stride, site, v);
+        load_spinor_rw(vecs + a * stride, site, v); // coherent loads: this launch rewrites `vecs`
         for (int b = 0; b < a; ++b) { // modified Gram-Schmidt: v -= <w_b, v> w_b with the CURRENT v
             T w[24];
-            load_spinor(vecs + b * stride, site, w);
+            load_spinor_rw(vecs + b * stride, site, w);
             double d[4];
             chiral_dots(w, v, d);
 #pragma unroll

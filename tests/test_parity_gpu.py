@@ -367,9 +367,13 @@ def test_staged_dagger_matches_the_oracle(oracle, dims, precision, recon, nrhs):
 
 @pytest.mark.parametrize("dims,nrhs", [((24, 8, 4, 6), 20), ((24, 4, 4, 5), 7), ((12, 8, 8, 4), 4), ((24, 2, 2, 3), 3)])
 @pytest.mark.parametrize("recon", [18, 12])
-def test_multi_rhs_kernel_when_lx_is_not_a_power_of_two(oracle, dims, nrhs, recon):
-    """The paper's volumes have Lx = 24 and N_v = 20: the multi-RHS kernel shares the
-    staged links there too (x hops through the slice buffer instead of warp shuffles)."""
+@pytest.mark.parametrize("force_mrhs", [False, True])
+def test_multi_rhs_when_lx_is_not_a_power_of_two(oracle, monkeypatch, dims, nrhs, recon, force_mrhs):
+    """The paper's volumes have Lx = 24 and N_v = 20.  Default: the single-RHS staged member
+    in the (patch, column, right-hand side) order (links shared through L2, the faster choice there); WD_STAGE_NO_MRHS=0
+    forces the multi-RHS member (links shared in shared memory, x hops through the slice buffer)."""
+    if force_mrhs:
+        monkeypatch.setenv("WD_STAGE_NO_MRHS", "0")
     cfg = fields.Config("mrhs24", dims, 32, "haar", recon, -0.41, nrhs, 95)
     check_config(oracle, cfg, "stage")
 
