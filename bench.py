@@ -53,6 +53,8 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 def compulsory_bytes_per_site(precision, recon, nrhs):
     """Algorithmic HBM bytes per site per launch: every spinor read once and
     written once, every link read once."""
+    if precision == 16:  # half-precision storage: 24 binary16 ratios + one float32 scale per site; links binary16
+        return nrhs * 2 * 52 + 4 * recon * 2
     w = 4 if precision == 32 else 8
     return nrhs * 2 * 24 * w + 4 * recon * w
 
@@ -231,20 +233,29 @@ def issue_bound_gbs(precision, recon, nrhs, sm_mhz):
     return site_rhs_per_s / nrhs * compulsory_bytes_per_site(precision, recon, nrhs) / 1e9
 
 
-def secondary_leg(binding, torch, dev, stream, local, name, U, recon, nrhs, steps, aps):
+def secondary_leg(binding, torch, dev, stream, local, name, U, recon, nrhs, steps, aps, storage=None):
     """One short timed leg of another BASELINE workload (north_star: "the batched 24-RHS apply reported in Gflop/s
     and as a fraction of its own roofline"; configs[3] is "fp64 and fp32").  Links: the array handed in (same recipe
     and shape as the workload's); spinors: complex Gaussian drawn on the device (seeded torch generator) straight into
     the native buffers -- the native layout is a permutation of the canonical one, so the distribution is the same."""
     cfg = fields.CONFIGS[name]
     V = fields.volume(cfg.dims)
-    tdt = torch.float32 if cfg.precision == 32 else torch.float64
+    prec = storage or cfg.precision        # storage = 16: half-precision storage, float32 canonical side
+    tdt = {16: torch.float16, 32: torch.float32, 64: torch.float64}[prec]
     nbuf = 2 if nrhs > 1 else NBUF
     with torch.cuda.stream(stream):
-        u_dev = torch.from_numpy(fields.round_to(U, cfg.precision)).to(dev)
-        op = binding.WilsonDirac(cfg.dims, u_dev, cfg.precision, recon, stream=stream.cuda_stream)
+        u_dev = torch.from_numpy(fields.round_to(U, 32 if prec == 16 else prec)).to(dev)
+        op = binding.WilsonDirac(cfg.dims, u_dev, prec, recon, stream=stream.cuda_stream)
         g = torch.Generator(device=dev).manual_seed(cfg.seed + 1000)
-        ins = [torch.randn(op.native_numel(nrhs), dtype=tdt, device=dev, generator=g) for _ in range(nbuf)]
+        if prec == 16:   # pack float32 Gaussian fields (the native half field is ratios + scales, not plain numbers)
+            ins = [torch.empty(op.native_numel(nrhs), dtype=tdt, device=dev) for _ in range(nbuf)]
+            Lx, Ly, Lz, Lt = cfg.dims
+            for b in ins:
+                c = torch.randn((nrhs, Lt, Lz, Ly, Lx, 4, 3, 2), dtype=torch.float32, device=dev, generator=g)
+                op.pack(b, c, nrhs)
+            del c
+        else:
+            ins = [torch.randn(op.native_numel(nrhs), dtype=tdt, device=dev, generator=g) for _ in range(nbuf)]
         outs = [torch.empty(op.native_numel(nrhs), dtype=tdt, device=dev) for _ in range(nbuf)]
     stream.synchronize()
     del u_dev
@@ -270,12 +281,12 @@ def secondary_leg(binding, torch, dev, stream, local, name, U, recon, nrhs, step
     op.close()
     del ins, outs
     torch.cuda.empty_cache()
-    bytes_per_launch = compulsory_bytes_per_site(cfg.precision, recon, nrhs) * V
+    bytes_per_launch = compulsory_bytes_per_site(prec, recon, nrhs) * V
     peak, peak_src = measured_peak()
     achieved = bytes_per_launch / (ms * 1e-3) / 1e9
     ck = clocks.summary()
     roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "traffic": ncu_traffic(name, recon), "peak_source": peak_src, "bytes_per_launch": bytes_per_launch,
+            "traffic": None if storage else ncu_traffic(name, recon), "peak_source": peak_src, "bytes_per_launch": bytes_per_launch,
             "kernel": "wd dslash, " + kern + " kernel" + (" (multi-RHS member)" if nrhs > 1 and kern == "stage" else "")}
     if nrhs > 1:  # its own roofline = min(HBM bound, FMA-pipe bound at the observed clock); both printed
         ib = issue_bound_gbs(cfg.precision, recon, nrhs, ck["sm_mhz"])
@@ -283,10 +294,57 @@ def secondary_leg(binding, torch, dev, stream, local, name, U, recon, nrhs, step
         roof["own_peak"] = min(peak, ib) if ib else peak
         roof["frac_of_own_peak"] = achieved / roof["own_peak"]
     return {"workload": name, "value": FLOPS_PER_SITE * V * nrhs / (ms * 1e-3) / 1e9, "unit": UNIT, "nrhs": nrhs,
-            "recon": recon, "dtype": "f32" if cfg.precision == 32 else "f64", "us_per_apply": ms * 1e3,
+            "recon": recon, "dtype": {16: "f32 arithmetic on f16 storage", 32: "f32", 64: "f64"}[prec],
+            "bytes_per_site": compulsory_bytes_per_site(prec, recon, nrhs), "us_per_apply": ms * 1e3,
             "steps": steps, "applies_per_step": aps, "gpu_launches": int(launches),
             "data": "synthetic: headline links recipe (smooth, eps=0.3), device-drawn Gaussian spinors",
             "roofline": roof, "clocks": ck}
+
+
+def pcie_peaks(torch, dev, h_in, h_out):
+    """Measured copy rates of THIS box for the e2e roofline: one large cudaMemcpyAsync per direction from / to the pinned
+    buffers the e2e leg uses, alone (h2d, d2h) and both at once on two streams (duplex, rate per direction), best of 3,
+    CUDA events.  GB/s."""
+    nbytes = h_in.numel() * h_in.element_size()
+    d_a = torch.empty_like(h_in, device=dev)
+    d_b = torch.empty_like(h_in, device=dev)
+    s1, s2 = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+
+    def timed(fn):
+        best = None
+        for _ in range(3):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(s1)
+            s2.wait_event(e0)
+            fn()
+            e2 = torch.cuda.Event()
+            e2.record(s2)
+            s1.wait_event(e2)
+            e1.record(s1)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            best = ms if best is None else min(best, ms)
+        return nbytes / (best * 1e-3) / 1e9
+
+    def h2d():
+        with torch.cuda.stream(s1):
+            d_a.copy_(h_in, non_blocking=True)
+
+    def d2h():
+        with torch.cuda.stream(s1):
+            h_out.copy_(d_b, non_blocking=True)
+
+    def both():
+        with torch.cuda.stream(s1):
+            d_a.copy_(h_in, non_blocking=True)
+        with torch.cuda.stream(s2):
+            h_out.copy_(d_b, non_blocking=True)
+
+    d_b.zero_()
+    out = {"h2d_gbs": timed(h2d), "d2h_gbs": timed(d2h), "duplex_gbs_per_direction": timed(both)}
+    del d_a, d_b
+    return out
 
 
 def run_wd_device_inputs(args, torch, binding, cfg, recon, nrhs, dev, local, kernel):
@@ -294,15 +352,26 @@ def run_wd_device_inputs(args, torch, binding, cfg, recon, nrhs, dev, local, ker
     N(0,1)/2 numbers drawn on the device (the kernels' cost is data independent), no e2e leg, no oracle leg.
     Its line says data = "device-random (timing only)" and is never a bench record."""
     V = fields.volume(cfg.dims)
-    tdt = torch.float32 if cfg.precision == 32 else torch.float64
+    prec = 16 if args.half else cfg.precision
+    tdt = {16: torch.float16, 32: torch.float32, 64: torch.float64}[prec]
+    cdt = torch.float64 if prec == 64 else torch.float32
     stream = torch.cuda.Stream(device=dev)
     nbuf = 2 if nrhs > 1 else NBUF
     with torch.cuda.stream(stream):
         g = torch.Generator(device=dev).manual_seed(cfg.seed)
         Lx, Ly, Lz, Lt = cfg.dims
-        u_dev = torch.randn((4, Lt, Lz, Ly, Lx, 3, 3, 2), dtype=tdt, device=dev, generator=g) * 0.5
-        op = binding.WilsonDirac(cfg.dims, u_dev, cfg.precision, recon, stream=stream.cuda_stream, kernel=kernel)
-        ins = [torch.randn(op.native_numel(nrhs), dtype=tdt, device=dev, generator=g) for _ in range(nbuf)]
+        u_dev = torch.randn((4, Lt, Lz, Ly, Lx, 3, 3, 2), dtype=cdt, device=dev, generator=g) * 0.5
+        if recon == 8:  # the 8-real format needs |a2|^2 + |a3|^2 <= 1: scale the random numbers down
+            u_dev *= 0.5
+        op = binding.WilsonDirac(cfg.dims, u_dev, prec, recon, stream=stream.cuda_stream, kernel=kernel)
+        if prec == 16:
+            ins = [torch.empty(op.native_numel(nrhs), dtype=tdt, device=dev) for _ in range(nbuf)]
+            for b in ins:
+                c = torch.randn((nrhs, Lt, Lz, Ly, Lx, 4, 3, 2), dtype=torch.float32, device=dev, generator=g)
+                op.pack(b, c, nrhs)
+            del c
+        else:
+            ins = [torch.randn(op.native_numel(nrhs), dtype=tdt, device=dev, generator=g) for _ in range(nbuf)]
         outs = [torch.empty(op.native_numel(nrhs), dtype=tdt, device=dev) for _ in range(nbuf)]
     stream.synchronize()
     del u_dev
@@ -318,7 +387,7 @@ def run_wd_device_inputs(args, torch, binding, cfg, recon, nrhs, dev, local, ker
         ev1.record(stream)
         torch.cuda.synchronize()
     ms = ev0.elapsed_time(ev1) / (args.steps * aps)
-    bytes_per_launch = compulsory_bytes_per_site(cfg.precision, recon, nrhs) * V
+    bytes_per_launch = compulsory_bytes_per_site(prec, recon, nrhs) * V
     peak, peak_src = measured_peak()
     achieved = bytes_per_launch / (ms * 1e-3) / 1e9
     line = {"metric": METRIC, "value": FLOPS_PER_SITE * V * nrhs / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
@@ -427,6 +496,9 @@ def run_wd(args):
     e2e_ms = max_over_ranks(e2e_ms, world, dev)
     e2e_value = whole_job_gflops(world, e2e_applies, flops_per_apply, e2e_ms)
     field_bytes = nrhs * V * 24 * (4 if cfg.precision == 32 else 8)
+    # the e2e roofline: the field must cross PCIe once in each direction; with both directions busy the bound is
+    # field_bytes / (duplex rate per direction), measured here with plain copies of the same pinned buffers
+    pcie = pcie_peaks(torch, dev, h_in, h_out) if world == 1 else None
 
     secondary = None
     if want_secondary:
@@ -436,6 +508,10 @@ def run_wd(args):
         secondary = [
             secondary_leg(binding, torch, dev, stream, local, "c4_32x64_fp32_24rhs", U, 18, 24, 2, 10),
             secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp64", U, 18, 1, 2, 25),
+            # storage variants of the paper's Table 2: 12 and 8 reals per link, half-precision storage
+            secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp32", U, 12, 1, 2, 50),
+            secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp32", U, 8, 1, 2, 50),
+            secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp32", U, 12, 1, 2, 50, storage=16),
         ]
 
     line = None
@@ -457,6 +533,12 @@ def run_wd(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": field_bytes * aps,
                     "d2h_bytes_per_step": field_bytes * aps, "applies_timed": e2e_applies,
                     "ms_per_apply": e2e_ms / e2e_applies,
+                    "pcie": pcie,
+                    "roofline": None if pcie is None else {
+                        "bound": "pcie", "unit": "GB/s per direction", "peak": pcie["duplex_gbs_per_direction"],
+                        "achieved": field_bytes / (e2e_ms / e2e_applies * 1e-3) / 1e9,
+                        "frac": field_bytes / (e2e_ms / e2e_applies * 1e-3) / 1e9 / pcie["duplex_gbs_per_direction"],
+                        "frac_of_one_direction_alone": field_bytes / (e2e_ms / e2e_applies * 1e-3) / 1e9 / min(pcie["h2d_gbs"], pcie["d2h_gbs"])},
                     "note": "wd_apply_host per apply: H2D + pack + apply + unpack + D2H + sync; bytes are per "
                             "100-apply step"},
             "gpu_launches": int(launches),
@@ -752,7 +834,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="c3_32x64_fp32", choices=sorted(fields.CONFIGS))
     ap.add_argument("--kernel", default="auto", choices=["auto", "site", "stage"])
-    ap.add_argument("--recon", type=int, default=None, choices=[18, 12])
+    ap.add_argument("--recon", type=int, default=None, choices=[18, 12, 8])
     ap.add_argument("--impl", default="wd", choices=["wd", "reference"])
     ap.add_argument("--op", default="full", choices=["full", "schur", "cgnr", "bicgstab", "gcr", "transfer", "coarse"],
                     help="full = D of eq. (2.2) (the headline); schur = even-odd preconditioned operator (row f1); cgnr = CG on its normal equations (row f2, --applies-per-step = iterations)")
@@ -764,6 +846,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--device-inputs", action="store_true",
                     help="timing-only quick mode for kernel work: device-drawn random links and spinors, no e2e/oracle legs")
+    ap.add_argument("--half", action="store_true", help="(with --device-inputs) half-precision storage, fp32 arithmetic")
     ap.add_argument("--no-secondary", action="store_true",
                     help="skip the short legs for configs[4] (24 RHS) and configs[3] in fp64 that the default run adds")
     ap.add_argument("--applies-per-step", type=int, default=APPLIES_PER_STEP,

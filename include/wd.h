@@ -54,7 +54,7 @@ typedef enum {
     WD_ERR_NULL = -1,      /* a required pointer is NULL                                   */
     WD_ERR_DIMS = -2,      /* an extent < 1, volume overflow, or dims do not match gauge   */
     WD_ERR_PRECISION = -3, /* precision is not WD_FP32 / WD_FP64 or differs from the gauge */
-    WD_ERR_RECON = -4,     /* recon is not WD_RECON_18 / WD_RECON_12                       */
+    WD_ERR_RECON = -4,     /* recon is not WD_RECON_18 / _12 / _8, or the links cannot be stored that way */
     WD_ERR_NRHS = -5,      /* nrhs < 1                                                     */
     WD_ERR_ALIAS = -6,     /* out and in overlap (the stencil is not in-place safe)        */
     WD_ERR_MISMATCH = -7,  /* handle belongs to another lattice / bad kernel selector      */
@@ -62,8 +62,14 @@ typedef enum {
     WD_ERR_ALLOC = -9      /* host or device allocation failed                             */
 } wd_status;
 
-typedef enum { WD_FP32 = 32, WD_FP64 = 64 } wd_precision; /* arithmetic AND storage type    */
-typedef enum { WD_RECON_18 = 18, WD_RECON_12 = 12 } wd_recon; /* reals stored per link       */
+/* WD_FP32 / WD_FP64: arithmetic AND storage type.  WD_FP16: half-precision STORAGE with float32 arithmetic (PAPER.md:159-167,
+ * Table 2 row "Half"; reading RH): links as IEEE binary16 reals; spinors as, per site, a float32 scale s = max |component|
+ * and the 24 ratios component / s as binary16 (value = s * ratio) -- 52 bytes per site and right-hand side.  With
+ * WD_FP16 the CANONICAL buffers of wd_load_gauge / wd_pack_spinor / wd_unpack_spinor are float32; it is accepted by
+ * wd_create_lattice .. wd_spinor_bytes, wd_load_gauge, wd_pack_spinor, wd_unpack_spinor, wd_apply and wd_apply_dagger
+ * (one-thread-per-site kernel, any extents, any nrhs); every other entry point answers WD_ERR_PRECISION. */
+typedef enum { WD_FP16 = 16, WD_FP32 = 32, WD_FP64 = 64 } wd_precision;
+typedef enum { WD_RECON_18 = 18, WD_RECON_12 = 12, WD_RECON_8 = 8 } wd_recon; /* reals stored per link */
 
 /* Kernel selector for wd_set_kernel (measurement and tests; default WD_KERNEL_AUTO). */
 typedef enum {
@@ -95,7 +101,12 @@ long long wd_lattice_volume(const wd_lattice *lat);
  * (4*V*18 reals of the given precision) and build the library's native copy:
  * reordered to structure-of-arrays and, for recon == WD_RECON_12, compressed to rows 0 and 1
  * of each link, the third row being rebuilt in the kernel as conj(row0 x row1)
- * ("Gauge field stored as 12 ... floats"; reading S7).
+ * ("Gauge field stored as 12 ... floats"; reading S7).  recon == WD_RECON_8 ("or 8
+ * floats"; reading R8): per link the eight reals (Re a2, Im a2, Re a3, Im a3, Re b1, Im b1, arg(a1)/pi, arg(c1)/pi) of
+ * its rows a, b, c -- phases formed in double, rounded once to the working precision; the kernels rebuild the link from
+ * |a1|^2 = 1 - |a2|^2 - |a3|^2, |c1|^2 = 1 - |a1|^2 - |b1|^2 and unitarity.  A link with a2 = a3 = 0 (e.g. the unit
+ * matrix, hence temporal-gauge links) has no such representation: WD_ERR_RECON (checked; synchronises the stream).
+ * Rounding in the rebuilt rows is amplified by 1 / (|a2|^2 + |a3|^2): tolerance in DESIGN.md section 2.
  * The conversion is enqueued on `stream` (a cudaStream_t cast to void*, NULL = default
  * stream), which also becomes the stream wd_apply launches on.  The caller may free
  * `links_canonical_dev` once that stream work has completed.  *gauge is owned by the
@@ -114,10 +125,10 @@ int wd_set_stream(wd_gauge *gauge, void *stream);
 
 /* Tuning variables of the launchers.  They are read from the environment ONCE, at wd_load_gauge
  * (WD_TILE_SHAPE=ty,tz, WD_TILE_TC, WD_TILE_NCHUNK, WD_TILE_NRB, WD_MRHS_PATCH, WD_STAGE_NO_MRHS, WD_SITE_SLAB_MB,
- * WD_HOST_NO_PIPELINE, WD_MRHS_NO_TAIL), and stored in the gauge handle; no launch reads the environment.
+ * WD_HOST_NO_PIPELINE, WD_MRHS_NO_TAIL, WD_HOST_NSLAB), and stored in the gauge handle; no launch reads the environment.
  * wd_set_tuning changes one of them afterwards: name is the lower-case variable without the WD_ prefix ("tile_ty",
  * "tile_tz", "tile_tc", "tile_nchunk", "tile_nrb", "mrhs_patch", "stage_no_mrhs", "site_slab_mb", "host_no_pipeline",
- * "mrhs_no_tail"); value < 0 restores the default.  WD_ERR_MISMATCH for an unknown name.  Host-only. */
+ * "mrhs_no_tail", "host_nslab"); value < 0 restores the default.  WD_ERR_MISMATCH for an unknown name.  Host-only. */
 int wd_set_tuning(wd_gauge *gauge, const char *name, int value);
 
 /* Temporal gauge ("temporal gauge fixing", Fig. 4 / Table 2 "GF"): on != 0 declares that the loaded links
@@ -221,10 +232,15 @@ int wd_apply_schur_dagger(void *out_half_dev, const void *in_half_dev, void *tmp
  * wd_cgnr_schur -- conjugate gradients on the normal equations of the even-odd preconditioned operator
  * ("CG on the normal equations"; CG around the even-odd matvec):
  *     Mhat^dagger Mhat x = Mhat^dagger b,   x_0 = 0,   one right-hand side, half fields of `parity`.
- * At most max_iter iterations; stops early when |b - Mhat x| <= tol * |b| (checked every 8 iterations; tol = 0
- * runs exactly max_iter iterations with no host synchronisation inside the loop: all scalars stay on the device,
- * reductions are deterministic fp64 sums).  *iters_out (may be NULL) receives the iterations done;
- * hist_host (HOST, max_iter + 1 doubles, may be NULL) the relative residuals |r_k| / |b|, k = 0..iters.
+ * tol = 0 runs exactly max_iter iterations with no host synchronisation inside the loop (all scalars stay on the
+ * device, reductions are deterministic fp64 sums); hist_host then holds the RECURSIVELY updated residual norms.
+ * tol > 0: the iteration stops when the recursive residual (read back every 8 iterations) is <= tol * |b|; the TRUE
+ * residual b - Mhat x is then recomputed with one more operator application and put into the history, and while it is
+ * still above tol * |b| and iterations are left the solver is restarted on Mhat e = b - Mhat x and x += e (defect
+ * correction), until a round no longer halves the true residual (the working precision's limit, ~1e-6 in fp32):
+ * the last history entry is always the true |b - Mhat x| / |b|, so a reported convergence is real.  Exact zeros in a
+ * denominator of the recurrence (b = 0, breakdown) give a zero step, never NaN.  *iters_out (may be NULL) receives
+ * the iterations done; hist_host (HOST, max_iter + 1 doubles, may be NULL) the relative residuals, k = 0..iters.
  * Workspace (five half fields) is owned by the gauge handle (allocated on first use, reused, released by
  * wd_destroy_gauge; not re-entrant for one handle); the call synchronises the gauge's stream before returning.
  */
@@ -242,6 +258,17 @@ int wd_bicgstab_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge,
  * current cycle.  1 <= restart <= 32.  Otherwise as wd_cgnr_schur (workspace: 2*restart + 2 half fields). */
 int wd_gcr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4], int precision,
                  int parity, int max_iter, int restart, double tol, int *iters_out, double *hist_host);
+
+/* The preconditioner slot of GCR (the multigrid cycle "is used as a preconditioner for a GCR(8) outer
+ * Krylov solver").  precond(ctx, z, r, stream) must enqueue z = K r on `stream` (the gauge's stream, a cudaStream_t as
+ * void*) for native half fields z, r of `parity` and return 0; K may differ from call to call (GCR is flexible: the
+ * search direction is p_j = K r_j, then q_j = Mhat p_j is orthogonalised as before).  It may call wd_apply_*,
+ * wd_restrict / wd_prolong / wd_apply_coarse, but not the wd_*_schur solvers of this gauge (shared workspace).
+ * precond == NULL is wd_gcr_schur.  A non-zero return aborts the solve with WD_ERR_CUDA. */
+typedef int (*wd_precond_fn)(void *ctx, void *z_half_dev, const void *r_half_dev, void *stream);
+int wd_gcr_schur_precond(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4], int precision,
+                         int parity, int max_iter, int restart, double tol, int *iters_out, double *hist_host,
+                         wd_precond_fn precond, void *precond_ctx);
 
 /*
  * ---- transfer operators of the adaptive multigrid set-up: eq. (2.7), on 4^4 space-time blocks with

@@ -111,13 +111,14 @@ def bicgstab_schur(b, U, dims, mass, parity, niter, tol=0.0, trace=None):
     return rp(x), np.array(hist)
 
 
-def gcr_schur(b, U, dims, mass, parity, niter, restart=8, tol=0.0):
+def gcr_schur(b, U, dims, mass, parity, niter, restart=8, tol=0.0, precond=None):
     """niter iterations of restarted GCR(restart) (Eisenstat-Elman-Schultz 1983; "GCR(8) outer Krylov
-    solver"), here without a preconditioner, for Mhat x = b on `parity`, x_0 = 0:
+    solver") for Mhat x = b on `parity`, x_0 = 0.  precond: None, or a callable K on complex fields [Lt,Lz,Ly,Lx,4,3]
+    (the multigrid cycle "is used as a preconditioner" for this solver): the search direction is K r.
 
         r = b
         loop k = 0, 1, ...   (j = k mod restart is the position inside the current cycle; a new cycle forgets all p's)
-            p_j = r;  q_j = Mhat p_j
+            p_j = K r  (K = 1 without a preconditioner);  q_j = Mhat p_j
             for i < j:  beta = <q_i, q_j> / <q_i, q_i>;  p_j -= beta p_i;  q_j -= beta q_i        (modified Gram-Schmidt)
             alpha = <q_j, r> / <q_j, q_j>;  x += alpha p_j;  r -= alpha q_j
 
@@ -137,7 +138,7 @@ def gcr_schur(b, U, dims, mass, parity, niter, restart=8, tol=0.0):
             break
         if k % restart == 0:
             P, Q, QQ = [], [], []
-        p = r.copy()
+        p = r.copy() if precond is None else precond(r)
         q = M(p)
         for pi, qi, qqi in zip(P, Q, QQ):
             beta = np.vdot(qi, q) / qqi

@@ -11,8 +11,8 @@ import ctypes
 import os
 
 WD_OK = 0
-WD_FP32, WD_FP64 = 32, 64
-WD_RECON_18, WD_RECON_12 = 18, 12
+WD_FP16, WD_FP32, WD_FP64 = 16, 32, 64
+WD_RECON_18, WD_RECON_12, WD_RECON_8 = 18, 12, 8
 WD_KERNEL_AUTO, WD_KERNEL_SITE, WD_KERNEL_STAGE = 0, 1, 3
 
 STATUS_NAMES = {
@@ -24,7 +24,7 @@ STATUS_NAMES = {
 SYMBOLS = (
     "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
     "wd_set_kernel", "wd_set_tuning", "wd_set_temporal_gauge", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
-    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_coarse_reals", "wd_coarse_stencil_reals", "wd_build_coarse", "wd_apply_coarse",
+    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_gcr_schur_precond", "wd_coarse_reals", "wd_coarse_stencil_reals", "wd_build_coarse", "wd_apply_coarse",
     "wd_block_orthonormalise", "wd_restrict", "wd_prolong", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_dagger", "wd_apply_host",
     "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
 )
@@ -273,6 +273,25 @@ def wd_gcr_schur(x_half_dev, b_half_dev, gauge, mass, dims, precision, parity, m
     return it.value, [hist[i] for i in range(it.value + 1)]
 
 
+PRECOND_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p)
+
+
+def wd_gcr_schur_precond(x_half_dev, b_half_dev, gauge, mass, dims, precision, parity, max_iter, restart, tol, precond):
+    """GCR with the preconditioner slot: precond(z_ptr, r_ptr, stream_ptr) is a Python callable that enqueues z = K r on the
+    given stream for the two device addresses (native half fields) and returns 0.  Marshalling only."""
+    it = ctypes.c_int(0)
+    hist = (ctypes.c_double * (int(max_iter) + 1))()
+    cb = PRECOND_FN(lambda ctx, z, r, s: int(precond(z, r, s) or 0))
+    fn = lib().wd_gcr_schur_precond
+    fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_double, ctypes.POINTER(ctypes.c_int), ctypes.c_int,
+                   ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.POINTER(ctypes.c_int),
+                   ctypes.POINTER(ctypes.c_double), PRECOND_FN, ctypes.c_void_p]
+    fn.restype = ctypes.c_int
+    _check(fn(_ptr(x_half_dev), _ptr(b_half_dev), gauge, float(mass), _dims(dims), int(precision), int(parity), int(max_iter),
+              int(restart), float(tol), ctypes.byref(it), hist, cb, None), "wd_gcr_schur_precond")
+    return it.value, [hist[i] for i in range(it.value + 1)]
+
+
 def wd_coarse_reals(lat, nv):
     return int(lib().wd_coarse_reals(lat, int(nv)))
 
@@ -360,8 +379,9 @@ class WilsonDirac:
         wd_apply_dagger(out_native_dev, in_native_dev, self.gauge, mass, self.dims, nrhs, self.precision)
 
     def native_numel(self, nrhs=1):
-        """Reals in a NATIVE spinor buffer of nrhs fields (the volume is padded to 32-site blocks)."""
-        return wd_spinor_bytes(self.lat, nrhs, self.precision) // (4 if self.precision == 32 else 8)
+        """Elements (float16 / float32 / float64 by precision) of a NATIVE spinor buffer of nrhs fields (the volume is
+        padded to 32-site blocks; half-precision storage: 26 two-byte elements per site = 24 ratios + a float32 scale)."""
+        return wd_spinor_bytes(self.lat, nrhs, self.precision) // {16: 2, 32: 4, 64: 8}[self.precision]
 
     def apply(self, out_native_dev, in_native_dev, mass, nrhs=1):
         wd_apply(out_native_dev, in_native_dev, self.gauge, mass, self.dims, nrhs, self.precision)
@@ -397,6 +417,10 @@ class WilsonDirac:
     def gcr_schur(self, x_half_dev, b_half_dev, mass, parity, max_iter, restart=8, tol=0.0):
         return wd_gcr_schur(x_half_dev, b_half_dev, self.gauge, mass, self.dims, self.precision, parity, max_iter, restart,
                             tol)
+
+    def gcr_schur_precond(self, x_half_dev, b_half_dev, mass, parity, max_iter, restart, tol, precond):
+        return wd_gcr_schur_precond(x_half_dev, b_half_dev, self.gauge, mass, self.dims, self.precision, parity, max_iter,
+                                    restart, tol, precond)
 
     def apply_host(self, out_canonical_host, in_canonical_host, mass, nrhs=1):
         wd_apply_host(out_canonical_host, in_canonical_host, self.gauge, mass, self.dims, nrhs, self.precision)

@@ -34,8 +34,13 @@ int cuda_fail(cudaError_t e, const char *what)
     return fail(WD_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
-bool valid_precision(int p) { return p == WD_FP32 || p == WD_FP64; }
-bool valid_recon(int r) { return r == WD_RECON_18 || r == WD_RECON_12; }
+bool valid_precision(int p) { return p == WD_FP32 || p == WD_FP64; }                  // arithmetic precisions
+bool valid_storage(int p) { return p == WD_FP16 || p == WD_FP32 || p == WD_FP64; }    // + half-precision storage
+// bytes of one real of the CANONICAL arrays (half-precision storage exchanges float32 canonical fields)
+size_t canon_real_bytes(int p) { return p == WD_FP64 ? 8 : 4; }
+// bytes per site and right-hand side of a NATIVE spinor field (half: 24 binary16 ratios + one float32 scale)
+size_t native_site_bytes(int p) { return p == WD_FP16 ? 52 : p == WD_FP32 ? 96 : 192; }
+bool valid_recon(int r) { return r == WD_RECON_18 || r == WD_RECON_12 || r == WD_RECON_8; }
 
 // volume with overflow guard; returns -1 on bad extents
 long long checked_volume(const int dims[4])
@@ -55,11 +60,14 @@ bool overlap(const void *a, size_t abytes, const void *b, size_t bbytes)
     return pa < pb + bbytes && pb < pa + abytes;
 }
 
-int check_apply_args(const void *out, const void *in, const wd_gauge *g, const int dims[4], int nrhs, int precision)
+int check_apply_args(const void *out, const void *in, const wd_gauge *g, const int dims[4], int nrhs, int precision,
+                     bool allow_half = false)
 {
     if (!out || !in || !g || !dims) return fail(WD_ERR_NULL, "wd_apply: NULL argument");
     if (g->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_apply: not a live wd_gauge handle");
-    if (!valid_precision(precision)) return fail(WD_ERR_PRECISION, "wd_apply: precision %d is not 32 or 64", precision);
+    if (!valid_storage(precision)) return fail(WD_ERR_PRECISION, "wd_apply: precision %d is not 16, 32 or 64", precision);
+    if (precision == WD_FP16 && !allow_half)
+        return fail(WD_ERR_PRECISION, "half-precision storage is taken by wd_apply / wd_apply_dagger only");
     if (precision != g->precision)
         return fail(WD_ERR_PRECISION, "wd_apply: precision %d but gauge was loaded in %d", precision, g->precision);
     for (int d = 0; d < 4; ++d)
@@ -100,6 +108,7 @@ void tuning_from_env(Tuning &t)
     t.site_slab_mb = env_int("WD_SITE_SLAB_MB");
     t.host_no_pipeline = env_int("WD_HOST_NO_PIPELINE");
     t.mrhs_no_tail = env_int("WD_MRHS_NO_TAIL");
+    t.host_nslab = env_int("WD_HOST_NSLAB");
 }
 
 int tuning_set(Tuning &t, const char *name, int value)
@@ -108,7 +117,8 @@ int tuning_set(Tuning &t, const char *name, int value)
         {"tile_ty", &Tuning::tile_ty}, {"tile_tz", &Tuning::tile_tz}, {"tile_tc", &Tuning::tile_tc},
         {"tile_nchunk", &Tuning::tile_nchunk}, {"tile_nrb", &Tuning::tile_nrb}, {"mrhs_patch", &Tuning::mrhs_patch},
         {"stage_no_mrhs", &Tuning::stage_no_mrhs}, {"site_slab_mb", &Tuning::site_slab_mb},
-        {"host_no_pipeline", &Tuning::host_no_pipeline}, {"mrhs_no_tail", &Tuning::mrhs_no_tail}};
+        {"host_no_pipeline", &Tuning::host_no_pipeline}, {"mrhs_no_tail", &Tuning::mrhs_no_tail},
+        {"host_nslab", &Tuning::host_nslab}};
     for (auto &e : tab)
         if (!strcmp(name, e.n)) {
             t.*(e.f) = value < 0 ? -1 : value;
@@ -157,8 +167,8 @@ long long wd_lattice_volume(const wd_lattice *lat)
 
 size_t wd_spinor_bytes(const wd_lattice *lat, int nrhs, int precision)
 {
-    if (!lat || lat->magic != LATTICE_MAGIC || nrhs < 1 || !valid_precision(precision)) return 0;
-    return (size_t)nrhs * (size_t)wd::padded_volume(lat->V) * 24 * (precision == WD_FP32 ? 4 : 8);
+    if (!lat || lat->magic != LATTICE_MAGIC || nrhs < 1 || !valid_storage(precision)) return 0;
+    return (size_t)nrhs * (size_t)wd::padded_volume(lat->V) * native_site_bytes(precision);
 }
 
 int wd_load_gauge(const wd_lattice *lat, const void *links_canonical_dev, int precision, int recon, void *stream,
@@ -167,8 +177,8 @@ int wd_load_gauge(const wd_lattice *lat, const void *links_canonical_dev, int pr
     if (!lat || !links_canonical_dev || !gauge) return fail(WD_ERR_NULL, "wd_load_gauge: NULL argument");
     *gauge = nullptr;
     if (lat->magic != LATTICE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_load_gauge: not a live wd_lattice handle");
-    if (!valid_precision(precision)) return fail(WD_ERR_PRECISION, "wd_load_gauge: precision %d is not 32 or 64", precision);
-    if (!valid_recon(recon)) return fail(WD_ERR_RECON, "wd_load_gauge: recon %d is not 18 or 12", recon);
+    if (!valid_storage(precision)) return fail(WD_ERR_PRECISION, "wd_load_gauge: precision %d is not 16, 32 or 64", precision);
+    if (!valid_recon(recon)) return fail(WD_ERR_RECON, "wd_load_gauge: recon %d is not 18, 12 or 8", recon);
     wd_gauge *g = new (std::nothrow) wd_gauge;
     if (!g) return fail(WD_ERR_ALLOC, "wd_load_gauge: out of host memory");
     memset(g, 0, sizeof(*g));
@@ -188,10 +198,23 @@ int wd_load_gauge(const wd_lattice *lat, const void *links_canonical_dev, int pr
         return e == cudaErrorMemoryAllocation ? fail(WD_ERR_ALLOC, "wd_load_gauge: cudaMalloc failed")
                                               : cuda_fail(e, "wd_load_gauge: cudaMalloc");
     }
-    e = wd::launch_pack_links(g->links, links_canonical_dev, g->V, precision, recon, g->stream);
-    if (e != cudaSuccess) {
+    int *bad = nullptr, hbad = 0;
+    if (recon == WD_RECON_8) { // the 8-real parametrisation cannot hold a link with U01 = U02 = 0: checked (one sync)
+        e = cudaMalloc(&bad, sizeof(int));
+        if (e == cudaSuccess) e = cudaMemsetAsync(bad, 0, sizeof(int), g->stream);
+    }
+    if (e == cudaSuccess)
+        e = precision == WD_FP16 ? wd::launch_pack_links_half(g->links, links_canonical_dev, g->V, recon, g->stream, bad)
+                                 : wd::launch_pack_links(g->links, links_canonical_dev, g->V, precision, recon, g->stream, bad);
+    if (e == cudaSuccess && bad) {
+        e = cudaMemcpyAsync(&hbad, bad, sizeof(int), cudaMemcpyDeviceToHost, g->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(g->stream);
+    }
+    cudaFree(bad);
+    if (e != cudaSuccess || hbad) {
         cudaFree(g->links);
         delete g;
+        if (hbad) return fail(WD_ERR_RECON, "wd_load_gauge: a link with U[0][1] = U[0][2] = 0 cannot be stored in 8 reals");
         return cuda_fail(e, "wd_load_gauge: pack kernel");
     }
     *gauge = g;
@@ -231,6 +254,9 @@ int wd_set_temporal_gauge(wd_gauge *gauge, int on)
         gauge->tgauge = 0;
         return WD_OK;
     }
+    if (gauge->precision == WD_FP16) return fail(WD_ERR_PRECISION, "wd_set_temporal_gauge: not for half-precision storage");
+    if (gauge->recon == WD_RECON_8)
+        return fail(WD_ERR_RECON, "wd_set_temporal_gauge: unit links cannot be stored in 8 reals (load the gauge with recon 18 or 12)");
     int *flag = nullptr, h = 0;
     cudaError_t e = cudaMalloc(&flag, sizeof(int));
     if (e != cudaSuccess) return cuda_fail(e, "wd_set_temporal_gauge: cudaMalloc");
@@ -251,6 +277,8 @@ int wd_set_kernel(wd_gauge *gauge, int kernel)
     if (gauge->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_set_kernel: not a live wd_gauge handle");
     if (kernel != WD_KERNEL_AUTO && kernel != WD_KERNEL_SITE && kernel != WD_KERNEL_STAGE)
         return fail(WD_ERR_MISMATCH, "wd_set_kernel: unknown kernel %d", kernel);
+    if (kernel == WD_KERNEL_STAGE && gauge->precision == WD_FP16)
+        return fail(WD_ERR_MISMATCH, "wd_set_kernel: half-precision storage runs through the site-style kernel only");
     if (kernel == WD_KERNEL_STAGE) {
         wd::ApplyArgs a{};
         for (int d = 0; d < 4; ++d) a.dims[d] = gauge->dims[d];
@@ -274,9 +302,9 @@ static int check_pack_args(const char *who, const wd_lattice *lat, const void *n
     const void *a = native, *b = canonical;
     if (!lat || !a || !b) return fail(WD_ERR_NULL, "%s: NULL argument", who);
     if (lat->magic != LATTICE_MAGIC) return fail(WD_ERR_MISMATCH, "%s: not a live wd_lattice handle", who);
-    if (!valid_precision(precision)) return fail(WD_ERR_PRECISION, "%s: precision %d is not 32 or 64", who, precision);
+    if (!valid_storage(precision)) return fail(WD_ERR_PRECISION, "%s: precision %d is not 16, 32 or 64", who, precision);
     if (nrhs < 1) return fail(WD_ERR_NRHS, "%s: nrhs=%d", who, nrhs);
-    const size_t cbytes = (size_t)nrhs * (size_t)lat->V * 24 * (precision == WD_FP32 ? 4 : 8);
+    const size_t cbytes = (size_t)nrhs * (size_t)lat->V * 24 * canon_real_bytes(precision);
     if (overlap(native, wd_spinor_bytes(lat, nrhs, precision), canonical, cbytes))
         return fail(WD_ERR_ALIAS, "%s: buffers overlap", who);
     return WD_OK;
@@ -287,7 +315,9 @@ int wd_pack_spinor(const wd_lattice *lat, void *native_dev, const void *canonica
 {
     int rc = check_pack_args("wd_pack_spinor", lat, native_dev, canonical_dev, nrhs, precision);
     if (rc) return rc;
-    cudaError_t e = wd::launch_pack_spinor(native_dev, canonical_dev, lat->V, nrhs, precision, (cudaStream_t)stream);
+    cudaError_t e = precision == WD_FP16
+                        ? wd::launch_spinor_half(native_dev, const_cast<void *>(canonical_dev), lat->V, nrhs, true, (cudaStream_t)stream)
+                        : wd::launch_pack_spinor(native_dev, canonical_dev, lat->V, nrhs, precision, (cudaStream_t)stream);
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_pack_spinor");
 }
 
@@ -296,7 +326,9 @@ int wd_unpack_spinor(const wd_lattice *lat, void *canonical_dev, const void *nat
 {
     int rc = check_pack_args("wd_unpack_spinor", lat, native_dev, canonical_dev, nrhs, precision);
     if (rc) return rc;
-    cudaError_t e = wd::launch_unpack_spinor(canonical_dev, native_dev, lat->V, nrhs, precision, (cudaStream_t)stream);
+    cudaError_t e = precision == WD_FP16
+                        ? wd::launch_spinor_half(const_cast<void *>(native_dev), canonical_dev, lat->V, nrhs, false, (cudaStream_t)stream)
+                        : wd::launch_unpack_spinor(canonical_dev, native_dev, lat->V, nrhs, precision, (cudaStream_t)stream);
     return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_unpack_spinor");
 }
 
@@ -304,6 +336,7 @@ int wd_unpack_spinor(const wd_lattice *lat, void *canonical_dev, const void *nat
 // members) on every lattice they can tile that has at least one wave of tiles; everything else -> site kernel
 static int auto_kernel(const wd::ApplyArgs &a)
 {
+    if (a.precision == WD_FP16) return WD_KERNEL_SITE; // half-precision storage: the site-style kernel of wd_half.cu
     const bool big = a.V >= (1LL << 18);
     if (big && wd::stage_supported(a)) return WD_KERNEL_STAGE;
     return WD_KERNEL_SITE;
@@ -339,7 +372,9 @@ static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double m
     a.stream = g->stream;
     a.dagger = dagger;
     cudaError_t e;
-    if (g->kernel == WD_KERNEL_SITE)
+    if (g->precision == WD_FP16)
+        e = wd::launch_half(a);
+    else if (g->kernel == WD_KERNEL_SITE)
         e = wd::launch_site(a);
     else if (g->kernel == WD_KERNEL_STAGE) {
         if (!wd::stage_supported(a)) return fail(WD_ERR_MISMATCH, "wd_apply: staged kernel cannot take this call");
@@ -352,9 +387,9 @@ static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double m
 int wd_apply(void *out_native_dev, const void *in_native_dev, const wd_gauge *gauge, double mass, const int dims[4],
              int nrhs, int precision)
 {
-    int rc = check_apply_args(out_native_dev, in_native_dev, gauge, dims, nrhs, precision);
+    int rc = check_apply_args(out_native_dev, in_native_dev, gauge, dims, nrhs, precision, true);
     if (rc) return rc;
-    const size_t bytes = (size_t)nrhs * (size_t)wd::padded_volume(gauge->V) * 24 * (precision == WD_FP32 ? 4 : 8);
+    const size_t bytes = (size_t)nrhs * (size_t)wd::padded_volume(gauge->V) * native_site_bytes(precision);
     if (overlap(out_native_dev, bytes, in_native_dev, bytes)) return fail(WD_ERR_ALIAS, "wd_apply: out and in overlap");
     if (((uintptr_t)out_native_dev | (uintptr_t)in_native_dev) & 15)
         return fail(WD_ERR_MISMATCH, "wd_apply: buffers must be 16-byte aligned");
@@ -364,9 +399,9 @@ int wd_apply(void *out_native_dev, const void *in_native_dev, const wd_gauge *ga
 int wd_apply_dagger(void *out_native_dev, const void *in_native_dev, const wd_gauge *gauge, double mass, const int dims[4],
                     int nrhs, int precision)
 {
-    int rc = check_apply_args(out_native_dev, in_native_dev, gauge, dims, nrhs, precision);
+    int rc = check_apply_args(out_native_dev, in_native_dev, gauge, dims, nrhs, precision, true);
     if (rc) return rc;
-    const size_t bytes = (size_t)nrhs * (size_t)wd::padded_volume(gauge->V) * 24 * (precision == WD_FP32 ? 4 : 8);
+    const size_t bytes = (size_t)nrhs * (size_t)wd::padded_volume(gauge->V) * native_site_bytes(precision);
     if (overlap(out_native_dev, bytes, in_native_dev, bytes)) return fail(WD_ERR_ALIAS, "wd_apply_dagger: out and in overlap");
     if (((uintptr_t)out_native_dev | (uintptr_t)in_native_dev) & 15)
         return fail(WD_ERR_MISMATCH, "wd_apply_dagger: buffers must be 16-byte aligned");
@@ -407,11 +442,14 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
     const int Lt = g->dims[3];
     cudaError_t e;
 
-    // ---- pipelined path: the lattice is cut into up to 16 slabs of whole time slices; slab k is copied in
+    // ---- pipelined path: the lattice is cut into up to 32 slabs of whole time slices; slab k is copied in
     // and packed on one stream, D is applied to it (site kernel on the slab's site range) on a second
     // stream as soon as slabs k-1, k, k+1 have arrived, and its result is unpacked and copied out on a
     // third stream, so the host->device and device->host transfers overlap (PCIe is full duplex) ----
-    const int nslab = Lt >= 16 ? 16 : Lt; // (the event arrays of wd_gauge hold 16)
+    // (the event arrays of wd_gauge hold 32; more slabs = shorter pipeline fill and drain: measured 32 > 16 > 8)
+    int nslab = g->tune.host_nslab >= 3 ? g->tune.host_nslab : 32;
+    if (nslab > 32) nslab = 32;
+    if (nslab > Lt) nslab = Lt;
     const bool pipelined = nslab >= 3 && S3 % 128 == 0 && bytes >= (8u << 20) && g->tune.host_no_pipeline <= 0;
     if (pipelined) {
         if (!g->pipe_ready) { // all 3 streams and 34 events, or none
@@ -439,7 +477,7 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
             return cuda_fail(err, what);
         };
         cudaStream_t s_in = g->pipe_stream[0], s_cmp = g->pipe_stream[1], s_out = g->pipe_stream[2];
-        cudaEvent_t *ev_in = g->pipe_event, *ev_cmp = g->pipe_event + 16, ev_start = g->pipe_event[32], ev_end = g->pipe_event[33];
+        cudaEvent_t *ev_in = g->pipe_event, *ev_cmp = g->pipe_event + 32, ev_start = g->pipe_event[64], ev_end = g->pipe_event[65];
         // everything enqueued on the gauge's stream so far (e.g. the link conversion) comes first
         if ((e = cudaEventRecord(ev_start, s)) != cudaSuccess) return bail(e, "wd_apply_host: event record");
         for (int i = 0; i < 3; ++i) cudaStreamWaitEvent(g->pipe_stream[i], ev_start, 0);
@@ -633,7 +671,7 @@ int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, dou
     a.links = gauge->links;
     a.stream = gauge->stream;
     cudaError_t e = cudaSuccess;
-    if (wd::cgnr_schur(gauge, a, x_half_dev, b_half_dev, mass, parity, max_iter, tol, iters_out, hist_host, &e))
+    if (wd::solve_schur(gauge, a, 0, x_half_dev, b_half_dev, mass, parity, max_iter, 0, tol, iters_out, hist_host, &e))
         return e == cudaErrorMemoryAllocation ? fail(WD_ERR_ALLOC, "wd_cgnr_schur: workspace allocation failed")
                                               : cuda_fail(e, "wd_cgnr_schur");
     return WD_OK;
@@ -650,7 +688,7 @@ int wd_bicgstab_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge,
     a.links = gauge->links;
     a.stream = gauge->stream;
     cudaError_t e = cudaSuccess;
-    if (wd::bicgstab_schur(gauge, a, x_half_dev, b_half_dev, mass, parity, max_iter, tol, iters_out, hist_host, &e))
+    if (wd::solve_schur(gauge, a, 1, x_half_dev, b_half_dev, mass, parity, max_iter, 0, tol, iters_out, hist_host, &e))
         return e == cudaErrorMemoryAllocation ? fail(WD_ERR_ALLOC, "wd_bicgstab_schur: workspace allocation failed")
                                               : cuda_fail(e, "wd_bicgstab_schur");
     return WD_OK;
@@ -658,6 +696,14 @@ int wd_bicgstab_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge,
 
 int wd_gcr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4], int precision,
                  int parity, int max_iter, int restart, double tol, int *iters_out, double *hist_host)
+{
+    return wd_gcr_schur_precond(x_half_dev, b_half_dev, gauge, mass, dims, precision, parity, max_iter, restart, tol, iters_out,
+                                hist_host, nullptr, nullptr);
+}
+
+int wd_gcr_schur_precond(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4], int precision,
+                         int parity, int max_iter, int restart, double tol, int *iters_out, double *hist_host,
+                         wd_precond_fn precond, void *precond_ctx)
 {
     int rc = check_eo_args("wd_gcr_schur", x_half_dev, b_half_dev, gauge, dims, 1, precision, parity);
     if (rc) return rc;
@@ -668,7 +714,8 @@ int wd_gcr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, doub
     a.links = gauge->links;
     a.stream = gauge->stream;
     cudaError_t e = cudaSuccess;
-    if (wd::gcr_schur(gauge, a, x_half_dev, b_half_dev, mass, parity, max_iter, restart, tol, iters_out, hist_host, &e))
+    if (wd::solve_schur(gauge, a, 2, x_half_dev, b_half_dev, mass, parity, max_iter, restart, tol, iters_out, hist_host, &e, precond,
+                        precond_ctx))
         return e == cudaErrorMemoryAllocation ? fail(WD_ERR_ALLOC, "wd_gcr_schur: workspace allocation failed")
                                               : cuda_fail(e, "wd_gcr_schur");
     return WD_OK;
@@ -775,6 +822,7 @@ void wd_destroy_gauge(wd_gauge *gauge)
     cudaFree(gauge->stage_canon);
     cudaFree(gauge->stage_canon_out);
     cudaFree(gauge->cg_ws);
+    cudaFree(gauge->rf_ws);
     cudaFree(gauge->cg_sc);
     cudaFree(gauge->stage_in);
     cudaFree(gauge->stage_out);

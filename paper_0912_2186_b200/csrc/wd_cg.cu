@@ -41,6 +41,10 @@ __device__ __forceinline__ double sum_partials(const double *part, int n = RED_B
     return t;
 }
 
+// a / b with the breakdown guard of the solvers: an exact zero denominator (b = 0 right-hand side, a converged or
+// broken-down recurrence) gives a zero step instead of 0/0 = NaN in x
+__device__ __forceinline__ double safe_div(double a, double b) { return b != 0.0 ? a / b : 0.0; }
+
 __device__ __forceinline__ double block_sum(double v, double *sh)
 {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
@@ -103,7 +107,7 @@ update_xr_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict
                  long long Vh, const double *zz_part, const double *ww_part, int npart, double *rr_part)
 {
     __shared__ double sh[RED_THREADS / 32];
-    const double alpha = sum_partials(zz_part, npart) / sum_partials(ww_part, npart);
+    const double alpha = safe_div(sum_partials(zz_part, npart), sum_partials(ww_part, npart));
     double s = 0.0;
     constexpr int UNR = 2; // independent vectors per thread and trip (4 streams x 2 loads in flight; 4 costs occupancy)
     const long long stride = (long long)RED_BLOCKS * RED_THREADS;
@@ -135,7 +139,7 @@ __global__ void __launch_bounds__(RED_THREADS)
 update_p_kernel(Vec *__restrict__ p, const Vec *__restrict__ z, long long nvec, const double *zz_new_part, const double *zz_old_part,
                 int npart, const double *rr_part, double *hist_k)
 {
-    const double beta = sum_partials(zz_new_part, npart) / sum_partials(zz_old_part, npart);
+    const double beta = safe_div(sum_partials(zz_new_part, npart), sum_partials(zz_old_part, npart));
     if (blockIdx.x == 0) { // (block-uniform branch: sum_partials has barriers)
         const double rr = sum_partials(rr_part);
         if (threadIdx.x == 0) *hist_k = sqrt(rr);
@@ -177,6 +181,7 @@ __device__ __forceinline__ cplxd cmul(cplxd a, cplxd b) { return {a.re * b.re - 
 __device__ __forceinline__ cplxd cdiv(cplxd a, cplxd b)
 {
     const double d = b.re * b.re + b.im * b.im;
+    if (d == 0.0) return {0.0, 0.0}; // breakdown guard (see safe_div)
     return {(a.re * b.re + a.im * b.im) / d, (a.im * b.re - a.re * b.im) / d};
 }
 __device__ __forceinline__ cplxd sum_partials_c(const double *part) // part[0..RED) = re, part[RED..2 RED) = im
@@ -281,7 +286,7 @@ bicg_x_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict__ 
     __shared__ double sh[RED_THREADS / 32];
     const cplxd ts = sum_partials_c(ts_part);
     const double tt = sum_partials(tt_part);
-    const cplxd omega = {ts.re / tt, ts.im / tt};
+    const cplxd omega = {safe_div(ts.re, tt), safe_div(ts.im, tt)};
     const cplxd alpha = scal[1];
     const cplxd mo = {-omega.re, -omega.im};
     double s2 = 0.0;
@@ -539,7 +544,7 @@ gcr_orth_kernel(Vec *__restrict__ pj, Vec *__restrict__ qj, const Vec *__restric
 {
     const cplxd d = sum_partials_c(dot_part);
     const double qq = *qq_i;
-    const cplxd mb = {-d.re / qq, -d.im / qq};
+    const cplxd mb = {-safe_div(d.re, qq), -safe_div(d.im, qq)};
     for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) {
         pj[i] = caxpy_vec(mb, pi[i], pj[i]);
         qj[i] = caxpy_vec(mb, qi[i], qj[i]);
@@ -555,7 +560,7 @@ gcr_update_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restric
     __shared__ double sh[RED_THREADS / 32];
     const cplxd qr = sum_partials_c(qr_part);
     const double qq = sum_partials(qq_part);
-    const cplxd alpha = {qr.re / qq, qr.im / qq};
+    const cplxd alpha = {safe_div(qr.re, qq), safe_div(qr.im, qq)};
     const cplxd ma = {-alpha.re, -alpha.im};
     double s2 = 0.0;
     for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) {
@@ -569,10 +574,13 @@ gcr_update_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restric
     if (blockIdx.x == 0 && threadIdx.x == 0) *qq_out = qq;
 }
 
-// restarted GCR(m) for Mhat x = b, x_0 = 0, no preconditioner: oracle/wd_solvers.py:gcr_schur step for step
+// restarted GCR(m) for Mhat x = b, x_0 = 0: oracle/wd_solvers.py:gcr_schur step for step.  precond != NULL: the search
+// direction is p_j = K r with K applied by the caller's function (the multigrid cycle is "a preconditioner
+// for a GCR(8) outer Krylov solver"; K may change from call to call -- GCR is flexible); it must enqueue its work on the
+// stream it is given and must not call the wd_*_schur solvers of this gauge (they share its workspace).
 template <typename T>
 static int gcr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const void *b_in, double mass, int parity, int max_iter,
-                       int restart, double tol, int *iters_out, double *hist_host, cudaError_t *err)
+                       int restart, double tol, int *iters_out, double *hist_host, cudaError_t *err, precond_fn precond, void *ctx)
 {
     using SL = SpinorLayout<T>;
     using Vec = typename SL::Vec;
@@ -624,7 +632,9 @@ static int gcr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const v
         }
         for (k = 0; k < max_iter; ++k) {
             const int j = k % restart;
-            if ((e = cudaMemcpyAsync(P(j), r, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
+            if (precond) {
+                if (precond(ctx, P(j), r, (void *)s) != 0) { fail_cuda(cudaErrorUnknown); break; }
+            } else if ((e = cudaMemcpyAsync(P(j), r, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
             if ((e = schur(Q(j), P(j))) != cudaSuccess) { fail_cuda(e); break; }
             for (int i = 0; i < j; ++i) { // modified Gram-Schmidt against the cycle's earlier directions
                 cdot_kernel<Vec, NCH, false><<<RED_BLOCKS, RED_THREADS, 0, s>>>(Q(i), Q(j), nvec, Vh, dot_part, nullptr);
@@ -661,11 +671,139 @@ static int gcr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const v
 }
 
 int gcr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter, int restart,
-              double tol, int *iters_out, double *hist_host, cudaError_t *err)
+              double tol, int *iters_out, double *hist_host, cudaError_t *err, precond_fn precond, void *ctx)
 {
     return shape.precision == 32
-               ? gcr_schur_t<float>(g, shape, x, b, mass, parity, max_iter, restart, tol, iters_out, hist_host, err)
-               : gcr_schur_t<double>(g, shape, x, b, mass, parity, max_iter, restart, tol, iters_out, hist_host, err);
+               ? gcr_schur_t<float>(g, shape, x, b, mass, parity, max_iter, restart, tol, iters_out, hist_host, err, precond, ctx)
+               : gcr_schur_t<double>(g, shape, x, b, mass, parity, max_iter, restart, tol, iters_out, hist_host, err, precond, ctx);
+}
+
+// ---- true-residual control (tol > 0) ----------------------------------------------------------------------------
+// The solvers above iterate on the RECURSIVELY updated residual; in fp32 it keeps falling below what |b - Mhat x| can
+// reach.  With a tolerance the public entry points therefore (1) run the solver, (2) recompute r = b - Mhat x with one
+// extra operator application, (3) put that true value into the history, and (4) while it is still above tol * |b| and
+// iterations are left, solve Mhat e = r for a correction and add it (defect correction), stopping when a round no
+// longer halves the true residual.  What is reported as converged is converged.
+namespace {
+__device__ __forceinline__ void sub_vec(float4 &a, const float4 &b) { a.x -= b.x; a.y -= b.y; a.z -= b.z; a.w -= b.w; }
+__device__ __forceinline__ void sub_vec(double2 &a, const double2 &b) { a.x -= b.x; a.y -= b.y; }
+__device__ __forceinline__ void add_vec(float4 &a, const float4 &b) { a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w; }
+__device__ __forceinline__ void add_vec(double2 &a, const double2 &b) { a.x += b.x; a.y += b.y; }
+template <typename Vec, int NCH>
+__global__ void __launch_bounds__(RED_THREADS)
+true_residual_kernel(Vec *__restrict__ r, const Vec *__restrict__ b, const Vec *__restrict__ w, long long nvec, long long Vh, double *part)
+{
+    __shared__ double sh[RED_THREADS / 32];
+    double s2 = 0.0;
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) {
+        Vec v = b[i];
+        const Vec wv = w[i];
+        sub_vec(v, wv);
+        r[i] = v;
+        if (real_site<NCH>(i, Vh)) s2 += norm2_vec(v);
+    }
+    s2 = block_sum(s2, sh);
+    if (threadIdx.x == 0) part[blockIdx.x] = s2;
+}
+template <typename Vec>
+__global__ void __launch_bounds__(RED_THREADS) add_kernel(Vec *__restrict__ x, const Vec *__restrict__ e, long long nvec)
+{
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) {
+        Vec v = x[i];
+        add_vec(v, e[i]);
+        x[i] = v;
+    }
+}
+} // namespace
+
+template <typename T>
+static int refined_t(wd_gauge *g, const ApplyArgs &shape, int kind, void *x_out, const void *b_in, double mass, int parity,
+                     int max_iter, int restart, double tol, int *iters_out, double *hist_host, cudaError_t *err, precond_fn precond,
+                     void *ctx)
+{
+    using SL = SpinorLayout<T>;
+    using Vec = typename SL::Vec;
+    constexpr int NCH = SL::NCH;
+    auto inner = [&](void *x, const void *b, int iters, double t, int *done, double *hist) {
+        return kind == 0   ? cgnr_schur(g, shape, x, b, mass, parity, iters, t, done, hist, err)
+               : kind == 1 ? bicgstab_schur(g, shape, x, b, mass, parity, iters, t, done, hist, err)
+                           : gcr_schur(g, shape, x, b, mass, parity, iters, restart, t, done, hist, err, precond, ctx);
+    };
+    if (!(tol > 0.0)) return inner(x_out, b_in, max_iter, tol, iters_out, hist_host);
+    const long long Vh = shape.V / 2;
+    const long long nvec = padded_volume(Vh) * NCH;
+    const size_t hb = (size_t)nvec * sizeof(Vec);
+    cudaStream_t s = shape.stream;
+    if (g->rf_ws_bytes < 3 * hb + RED_BLOCKS * sizeof(double)) {
+        cudaFree(g->rf_ws);
+        g->rf_ws = nullptr;
+        g->rf_ws_bytes = 0;
+        if ((*err = cudaMalloc(&g->rf_ws, 3 * hb + RED_BLOCKS * sizeof(double))) != cudaSuccess) return -1;
+        g->rf_ws_bytes = 3 * hb + RED_BLOCKS * sizeof(double);
+    }
+    Vec *r = (Vec *)g->rf_ws, *e = (Vec *)((char *)g->rf_ws + hb), *tmp = (Vec *)((char *)g->rf_ws + 2 * hb);
+    double *part = (double *)((char *)g->rf_ws + 3 * hb);
+    const double a0 = 4.0 + mass;
+    ApplyArgs a = shape;
+    // |v|: partials on the device, summed on the host in a fixed order (this path synchronises anyway)
+    auto host_norm = [&](double &out) -> cudaError_t {
+        static thread_local double h[RED_BLOCKS];
+        cudaError_t ce = cudaMemcpyAsync(h, part, sizeof(h), cudaMemcpyDeviceToHost, s);
+        if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
+        double sum = 0.0;
+        for (int i = 0; i < RED_BLOCKS; ++i) sum += h[i];
+        out = sqrt(sum);
+        return ce;
+    };
+    auto true_residual = [&](const Vec *x, double &nrm) -> cudaError_t { // r = b - Mhat x
+        a.out = tmp;
+        a.in = x;
+        cudaError_t ce = launch_eo(a, nullptr, 0.0, -0.5, 1 - parity, false);
+        if (ce != cudaSuccess) return ce;
+        a.out = e; // (e is free here)
+        a.in = tmp;
+        if ((ce = launch_eo(a, x, a0, 0.5 / a0, parity, false)) != cudaSuccess) return ce;
+        true_residual_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(r, (const Vec *)b_in, e, nvec, Vh, part);
+        count_launch();
+        return host_norm(nrm);
+    };
+    double bnorm = 0.0;
+    norm2_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>((const Vec *)b_in, nvec, Vh, part);
+    count_launch();
+    if ((*err = host_norm(bnorm)) != cudaSuccess) return -1;
+    int total = 0, done = 0;
+    if (inner(x_out, b_in, max_iter, tol, &done, hist_host)) return -1;
+    total = done;
+    if (bnorm == 0.0) { // b = 0: x = 0
+        if (iters_out) *iters_out = total;
+        return 0;
+    }
+    double rn = 0.0;
+    if ((*err = true_residual((const Vec *)x_out, rn)) != cudaSuccess) return -1;
+    if (hist_host) hist_host[total] = rn / bnorm;
+    while (rn > tol * bnorm && total < max_iter) {
+        const double before = rn;
+        const int off = total;
+        if (inner(e, r, max_iter - total, tol * bnorm / rn, &done, hist_host ? hist_host + off : nullptr)) return -1;
+        if (hist_host)
+            for (int i = 0; i <= done; ++i) hist_host[off + i] *= before / bnorm; // the inner history is relative to |r|
+        total += done;
+        add_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>((Vec *)x_out, e, nvec);
+        count_launch();
+        if ((*err = true_residual((const Vec *)x_out, rn)) != cudaSuccess) return -1;
+        if (hist_host) hist_host[total] = rn / bnorm;
+        if (done == 0 || rn > 0.5 * before) break; // stagnation at the working precision: report the true value
+    }
+    if (iters_out) *iters_out = total;
+    return 0;
+}
+
+int solve_schur(wd_gauge *g, const ApplyArgs &shape, int kind, void *x, const void *b, double mass, int parity, int max_iter,
+                int restart, double tol, int *iters_out, double *hist_host, cudaError_t *err, precond_fn precond, void *ctx)
+{
+    return shape.precision == 32
+               ? refined_t<float>(g, shape, kind, x, b, mass, parity, max_iter, restart, tol, iters_out, hist_host, err, precond, ctx)
+               : refined_t<double>(g, shape, kind, x, b, mass, parity, max_iter, restart, tol, iters_out, hist_host, err, precond, ctx);
 }
 
 // x = approximate solution of Mhat x = b on `parity` after at most max_iter CGNR iterations (tol = 0: exactly

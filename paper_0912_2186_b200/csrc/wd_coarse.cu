@@ -370,8 +370,12 @@ cudaError_t launch_coarse_build(void *S, void *part, const void *W, const void *
                                 double mass, int precision, int recon, cudaStream_t s)
 {
     if (precision == 32)
-        return recon == 18 ? build_t<float, 18>(S, part, W, links, dims, V, nv, mass, s) : build_t<float, 12>(S, part, W, links, dims, V, nv, mass, s);
-    return recon == 18 ? build_t<double, 18>(S, part, W, links, dims, V, nv, mass, s) : build_t<double, 12>(S, part, W, links, dims, V, nv, mass, s);
+        return recon == 18 ? build_t<float, 18>(S, part, W, links, dims, V, nv, mass, s)
+               : recon == 12 ? build_t<float, 12>(S, part, W, links, dims, V, nv, mass, s)
+                             : build_t<float, 8>(S, part, W, links, dims, V, nv, mass, s);
+    return recon == 18 ? build_t<double, 18>(S, part, W, links, dims, V, nv, mass, s)
+           : recon == 12 ? build_t<double, 12>(S, part, W, links, dims, V, nv, mass, s)
+                         : build_t<double, 8>(S, part, W, links, dims, V, nv, mass, s);
 }
 
 cudaError_t launch_coarse_apply(void *out, const void *in, const void *S, const int dims[4], int nv, int nrhs, int precision,

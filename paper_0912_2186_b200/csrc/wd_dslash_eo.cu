@@ -115,9 +115,11 @@ cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double 
 {
     if (a.precision == 32)
         return a.recon == 18 ? launch_eo_t<float, 18>(a, xin, alpha, beta, parity, dagger, norm_part)
-                             : launch_eo_t<float, 12>(a, xin, alpha, beta, parity, dagger, norm_part);
+               : a.recon == 12 ? launch_eo_t<float, 12>(a, xin, alpha, beta, parity, dagger, norm_part)
+                               : launch_eo_t<float, 8>(a, xin, alpha, beta, parity, dagger, norm_part);
     return a.recon == 18 ? launch_eo_t<double, 18>(a, xin, alpha, beta, parity, dagger, norm_part)
-                         : launch_eo_t<double, 12>(a, xin, alpha, beta, parity, dagger, norm_part);
+           : a.recon == 12 ? launch_eo_t<double, 12>(a, xin, alpha, beta, parity, dagger, norm_part)
+                           : launch_eo_t<double, 8>(a, xin, alpha, beta, parity, dagger, norm_part);
 }
 
 // canonical full-lattice field <-> native half field of one parity (pure data movement)

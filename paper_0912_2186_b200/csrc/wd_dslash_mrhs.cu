@@ -64,6 +64,7 @@ __device__ __forceinline__ void lds_link(const float4 *base, int first0, int str
 #pragma unroll
     for (int i = 0; i < RECON; ++i) u[i] = tmp[LV::skip + i];
     if (RECON == 12) reconstruct_row2(u);
+    if (RECON == 8) reconstruct_from8(u);
 }
 
 __device__ __forceinline__ void shfl12(float (&dst)[12], const float (&src)[12], int src_lane)

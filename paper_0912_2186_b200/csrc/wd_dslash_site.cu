@@ -131,8 +131,9 @@ static cudaError_t launch_site_r(const ApplyArgs &a)
 
 cudaError_t launch_site(const ApplyArgs &a)
 {
-    if (a.precision == 32) return a.recon == 18 ? launch_site_r<float, 18>(a) : launch_site_r<float, 12>(a);
-    return a.recon == 18 ? launch_site_r<double, 18>(a) : launch_site_r<double, 12>(a);
+    if (a.precision == 32)
+        return a.recon == 18 ? launch_site_r<float, 18>(a) : a.recon == 12 ? launch_site_r<float, 12>(a) : launch_site_r<float, 8>(a);
+    return a.recon == 18 ? launch_site_r<double, 18>(a) : a.recon == 12 ? launch_site_r<double, 12>(a) : launch_site_r<double, 8>(a);
 }
 
 } // namespace wd

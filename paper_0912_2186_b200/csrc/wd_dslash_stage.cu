@@ -67,6 +67,7 @@ __device__ __forceinline__ void lds_link_at(const Vec *base, int first0, int str
 #pragma unroll
     for (int i = 0; i < RECON; ++i) u[i] = tmp[LV::skip + i];
     if (RECON == 12) reconstruct_row2(u);
+    if (RECON == 8) reconstruct_from8(u);
 }
 
 template <typename T>
@@ -490,8 +491,10 @@ bool stage_supported(const ApplyArgs &a)
     StageShape s;
     if (a.nrhs < 1 || !stage_shape(a, s)) return false;
     // the tile's staging area must fit the 227 KB of shared memory a CTA can have (fp64 needs twice fp32's)
-    const size_t smem = a.precision == 32 ? (a.recon == 18 ? stage_smem_bytes<float, 18>(a, s) : stage_smem_bytes<float, 12>(a, s))
-                                          : (a.recon == 18 ? stage_smem_bytes<double, 18>(a, s) : stage_smem_bytes<double, 12>(a, s));
+    const size_t smem =
+        a.precision == 32
+            ? (a.recon == 18 ? stage_smem_bytes<float, 18>(a, s) : a.recon == 12 ? stage_smem_bytes<float, 12>(a, s) : stage_smem_bytes<float, 8>(a, s))
+            : (a.recon == 18 ? stage_smem_bytes<double, 18>(a, s) : a.recon == 12 ? stage_smem_bytes<double, 12>(a, s) : stage_smem_bytes<double, 8>(a, s));
     return smem <= 227 * 1024;
 }
 
@@ -506,13 +509,14 @@ cudaError_t launch_stage(const ApplyArgs &a)
     // right-hand side) order, which shares the links through L2, is the faster one (20 RHS on 24^3 x 64: 1.30 against
     // 1.39 ms).  stage_no_mrhs = 0 / 1 forces the choice.
     const bool pow2 = !(a.dims[0] & (a.dims[0] - 1));
-    if (a.precision == 32 && a.nrhs > 1 && !a.dagger && (tn.stage_no_mrhs < 0 ? pow2 : tn.stage_no_mrhs == 0)) {
+    if (a.precision == 32 && a.recon != 8 && a.nrhs > 1 && !a.dagger && (tn.stage_no_mrhs < 0 ? pow2 : tn.stage_no_mrhs == 0)) {
         StageShape s;
         if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
         if (s.nt <= 128) return launch_mrhs(a, s.ty, s.tz); // (a forced bigger tile runs through the single-RHS kernel below)
     }
-    if (a.precision == 32) return a.recon == 18 ? launch_stage_t<float, 18>(a) : launch_stage_t<float, 12>(a);
-    return a.recon == 18 ? launch_stage_t<double, 18>(a) : launch_stage_t<double, 12>(a);
+    if (a.precision == 32)
+        return a.recon == 18 ? launch_stage_t<float, 18>(a) : a.recon == 12 ? launch_stage_t<float, 12>(a) : launch_stage_t<float, 8>(a);
+    return a.recon == 18 ? launch_stage_t<double, 18>(a) : a.recon == 12 ? launch_stage_t<double, 12>(a) : launch_stage_t<double, 8>(a);
 }
 
 } // namespace wd

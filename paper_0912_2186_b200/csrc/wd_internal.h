@@ -16,6 +16,7 @@ struct Tuning {
     int site_slab_mb = -1;          // WD_SITE_SLAB_MB  link slab of the site kernel's multi-RHS block order
     int host_no_pipeline = -1;      // WD_HOST_NO_PIPELINE  1 = one-stream wd_apply_host
     int mrhs_no_tail = -1;          // WD_MRHS_NO_TAIL  1 = no shortened t-chunks in the last wave of the multi-RHS kernel
+    int host_nslab = -1;            // WD_HOST_NSLAB    slabs of the pipelined wd_apply_host (3..32, default 32)
 };
 void tuning_from_env(Tuning &t);
 int tuning_set(Tuning &t, const char *name, int value); // 0 = ok, -1 = unknown name
@@ -48,12 +49,14 @@ struct wd_gauge {
     void *stage_out;     // native out
     size_t stage_bytes;
     // workspace of wd_cgnr_schur (five half fields + reduction scalars), allocated on first use, reused
+    void *rf_ws;         // workspace of the true-residual control around the solvers (three half fields), on first use
+    size_t rf_ws_bytes;
     void *cg_ws;
     size_t cg_ws_bytes;
     double *cg_sc;
     size_t cg_sc_count;
     cudaStream_t pipe_stream[3]; // copy-in, compute, copy-out streams of the pipelined host path
-    cudaEvent_t pipe_event[2 * 16 + 2];
+    cudaEvent_t pipe_event[2 * 32 + 2];
 };
 
 namespace wd {
@@ -100,8 +103,14 @@ int cgnr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, doub
                double tol, int *iters_out, double *hist_host, cudaError_t *err);
 int bicgstab_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter,
                    double tol, int *iters_out, double *hist_host, cudaError_t *err);
+// preconditioner slot of GCR: z = K r, enqueued on `stream` (same type as wd_precond_fn in wd.h)
+typedef int (*precond_fn)(void *ctx, void *z_half_dev, const void *r_half_dev, void *stream);
 int gcr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter, int restart,
-              double tol, int *iters_out, double *hist_host, cudaError_t *err);
+              double tol, int *iters_out, double *hist_host, cudaError_t *err, precond_fn precond = nullptr, void *ctx = nullptr);
+// the public solvers: kind 0 = CGNR, 1 = BiCGstab, 2 = GCR(restart); tol > 0 adds true-residual control (wd_cg.cu)
+int solve_schur(wd_gauge *g, const ApplyArgs &shape, int kind, void *x, const void *b, double mass, int parity, int max_iter,
+                int restart, double tol, int *iters_out, double *hist_host, cudaError_t *err, precond_fn precond = nullptr,
+                void *ctx = nullptr);
 // transfer operators of the multigrid set-up (wd_transfer.cu)
 cudaError_t launch_transfer(int what, void *a, const void *b, const void *c, const int dims[4], long long V, int nv,
                             int precision, cudaStream_t s);
@@ -110,10 +119,14 @@ cudaError_t launch_coarse_build(void *S, void *part, const void *W, const void *
                                 double mass, int precision, int recon, cudaStream_t s);
 cudaError_t launch_coarse_apply(void *out, const void *in, const void *S, const int dims[4], int nv, int nrhs, int precision,
                                 cudaStream_t s);
+// half-precision storage (wd_half.cu): fp32 arithmetic on binary16 fields; canonical side is float32
+cudaError_t launch_half(const ApplyArgs &a);
+cudaError_t launch_spinor_half(void *native, void *canonical, long long V, int nrhs, bool to_native, cudaStream_t s);
+cudaError_t launch_pack_links_half(void *native, const void *canonical, long long V, int recon, cudaStream_t s, int *bad_dev);
 cudaError_t launch_parity_copy(void *native, void *canon, const int dims[4], long long V, int nrhs, int precision,
                                int parity, bool to_native, cudaStream_t s);
 cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon,
-                              cudaStream_t s);
+                              cudaStream_t s, int *bad_dev = nullptr);
 cudaError_t launch_check_temporal_gauge(const void *links, const int dims[4], long long V, int precision, int recon,
                                         int *flag_dev, cudaStream_t s);
 size_t native_link_bytes(long long V, int precision, int recon);

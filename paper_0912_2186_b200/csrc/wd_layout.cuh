@@ -11,7 +11,8 @@
 //       fp64: vector = double2 = reals 2c..2c+1;                                       12 vectors
 //   links, native:   [block b][vector j][lane l]        all FOUR links of a site together:
 //       the site's 4*RECON reals [mu][row][col][re,im] (rows 0,1 only for RECON 12) cut into
-//       16-byte vectors: fp32 r18 18, fp32 r12 12, fp64 r18 36, fp64 r12 24 vectors per site.
+//       16-byte vectors: fp32 r18 18, fp32 r12 12, fp32 r8 8, fp64 r18 36, fp64 r12 24, fp64 r8 16 vectors per site
+//       (RECON 8: the parametrisation of wd_math.cuh:reconstruct_from8).
 //
 // Why blocks: (1) a warp reading vector c of 32 consecutive sites issues ONE contiguous 512-byte
 // request (128 bits per lane, fully coalesced); (2) the distance between two vectors of a site is
@@ -47,6 +48,8 @@ template <> struct LinkLayout<float, 18> { using Vec = float4; static constexpr 
 template <> struct LinkLayout<float, 12> { using Vec = float4; static constexpr int CR = 4, NVEC = 12; };
 template <> struct LinkLayout<double, 18> { using Vec = double2; static constexpr int CR = 2, NVEC = 36; };
 template <> struct LinkLayout<double, 12> { using Vec = double2; static constexpr int CR = 2, NVEC = 24; };
+template <> struct LinkLayout<float, 8> { using Vec = float4; static constexpr int CR = 4, NVEC = 8; };
+template <> struct LinkLayout<double, 8> { using Vec = double2; static constexpr int CR = 2, NVEC = 16; };
 
 __device__ __forceinline__ void unpack(const float4 &v, float *r) { r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w; }
 __device__ __forceinline__ void unpack(const double2 &v, double *r) { r[0] = v.x; r[1] = v.y; }

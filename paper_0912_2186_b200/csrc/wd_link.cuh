@@ -35,6 +35,7 @@ __device__ __forceinline__ void load_link(const T *__restrict__ links, long long
 #pragma unroll
     for (int i = 0; i < RECON; ++i) u[i] = tmp[skip + i];
     if (RECON == 12) reconstruct_row2(u);
+    if (RECON == 8) reconstruct_from8(u);
 }
 
 } // namespace wd

@@ -215,6 +215,43 @@ __device__ __forceinline__ void reconstruct_row2(T (&u)[18])
     }
 }
 
+// Full SU(3) link from 8 stored reals ("stored as 12 or 8 ... floats"; reading R8 in DESIGN.md section 2):
+//   stored  (Re a2, Im a2, Re a3, Im a3, Re b1, Im b1, arg(a1)/pi, arg(c1)/pi)   for rows a, b, c of the link
+//           (the two phases in units of pi, in [-1, 1]: sincospi needs no range reduction by an inexact pi)
+//   |a1| = sqrt(1 - N), N = |a2|^2 + |a3|^2 (row 0 has unit length);  |c1| = sqrt(1 - |a1|^2 - |b1|^2) (so has column 0)
+//   b perpendicular to a and c = conj(a x b) give two linear equations for (b2, b3):
+//       b2 = -(conj(a1) b1 a2 + conj(a3 c1)) / N        b3 = (conj(a2 c1) - a3 conj(a1) b1) / N
+//   c2 = conj(a3 b1 - a1 b3),  c3 = conj(a1 b2 - a2 b1)
+// In place: u[0..7] hold the stored reals on entry.  N = 0 (a2 = a3 = 0, e.g. the unit matrix) cannot be represented;
+// wd_load_gauge refuses such links.  Rounding is amplified by 1/N in b2, b3, c2, c3.
+__device__ __forceinline__ void wd_sincospi(float x, float &s, float &c) { sincospif(x, &s, &c); }
+__device__ __forceinline__ void wd_sincospi(double x, double &s, double &c) { sincospi(x, &s, &c); }
+template <typename T>
+__device__ __forceinline__ void reconstruct_from8(T (&u)[18])
+{
+    const T a2r = u[0], a2i = u[1], a3r = u[2], a3i = u[3], b1r = u[4], b1i = u[5], tha = u[6], thc = u[7];
+    const T N = a2r * a2r + a2i * a2i + a3r * a3r + a3i * a3i;
+    const T inv = (T)1 / N;
+    const T ma1 = sqrt(max((T)0, (T)1 - N));
+    T sa, ca, sc, cc;
+    wd_sincospi(tha, sa, ca);
+    wd_sincospi(thc, sc, cc);
+    const T a1r = ma1 * ca, a1i = ma1 * sa;
+    const T mc1 = sqrt(max((T)0, (T)1 - ma1 * ma1 - (b1r * b1r + b1i * b1i)));
+    const T c1r = mc1 * cc, c1i = mc1 * sc;
+    const T pr = a1r * b1r + a1i * b1i, pi = a1r * b1i - a1i * b1r; // p = conj(a1) b1
+    const T qr = a3r * c1r - a3i * c1i, qi = a3r * c1i + a3i * c1r; // q = a3 c1
+    const T sr = a2r * c1r - a2i * c1i, si = a2r * c1i + a2i * c1r; // s = a2 c1
+    const T b2r = -((pr * a2r - pi * a2i) + qr) * inv, b2i = -((pr * a2i + pi * a2r) - qi) * inv;
+    const T b3r = (sr - (a3r * pr - a3i * pi)) * inv, b3i = (-si - (a3r * pi + a3i * pr)) * inv;
+    // c2 = conj(a3 b1 - a1 b3), c3 = conj(a1 b2 - a2 b1)
+    const T c2r = (a3r * b1r - a3i * b1i) - (a1r * b3r - a1i * b3i), c2i = -((a3r * b1i + a3i * b1r) - (a1r * b3i + a1i * b3r));
+    const T c3r = (a1r * b2r - a1i * b2i) - (a2r * b1r - a2i * b1i), c3i = -((a1r * b2i + a1i * b2r) - (a2r * b1i + a2i * b1r));
+    u[0] = a1r; u[1] = a1i; u[2] = a2r; u[3] = a2i; u[4] = a3r; u[5] = a3i;
+    u[6] = b1r; u[7] = b1i; u[8] = b2r; u[9] = b2i; u[10] = b3r; u[11] = b3i;
+    u[12] = c1r; u[13] = c1i; u[14] = c2r; u[15] = c2i; u[16] = c3r; u[17] = c3i;
+}
+
 // One forward + one backward hop in direction MU accumulated into acc:
 //   acc += (1 - gamma_MU) U_f p_f  +  (1 + gamma_MU) U_b^dag p_b
 template <int MU, typename T>

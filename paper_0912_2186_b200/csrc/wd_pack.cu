@@ -79,8 +79,11 @@ cudaError_t launch_unpack_spinor(void *canonical, const void *native, long long 
 
 // canonical U[mu][site][a][b][re,im] -> native [block][vector][lane], the four links of a site
 // together (wd_layout.cuh); recon 12 keeps rows a = 0,1 of every link.
+// recon 8 stores (Re a2, Im a2, Re a3, Im a3, Re b1, Im b1, arg(a1)/pi, arg(c1)/pi) of the rows a, b, c (wd_math.cuh:
+// reconstruct_from8), the two angles formed in double and rounded once; *bad is set if some link has a2 = a3 = 0
+// (not representable).
 template <typename T, int RECON>
-__global__ void pack_links_kernel(T *__restrict__ dst, const T *__restrict__ src, long long V)
+__global__ void pack_links_kernel(T *__restrict__ dst, const T *__restrict__ src, long long V, int *bad)
 {
     using L = LinkLayout<T, RECON>;
     const long long site = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -90,8 +93,17 @@ __global__ void pack_links_kernel(T *__restrict__ dst, const T *__restrict__ src
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) {
         const T *p = src + ((long long)mu * V + site) * 18;
+        if (RECON == 8) {
+            r[mu * RECON + 0] = p[2]; r[mu * RECON + 1] = p[3]; // a2
+            r[mu * RECON + 2] = p[4]; r[mu * RECON + 3] = p[5]; // a3
+            r[mu * RECON + 4] = p[6]; r[mu * RECON + 5] = p[7]; // b1
+            r[mu * RECON + 6] = (T)(atan2((double)p[1], (double)p[0]) / 3.14159265358979323846);   // arg(a1) / pi
+            r[mu * RECON + 7] = (T)(atan2((double)p[13], (double)p[12]) / 3.14159265358979323846); // arg(c1) / pi
+            if (p[2] == (T)0 && p[3] == (T)0 && p[4] == (T)0 && p[5] == (T)0 && bad) atomicOr(bad, 1);
+        } else {
 #pragma unroll
-        for (int i = 0; i < RECON; ++i) r[mu * RECON + i] = p[i];
+            for (int i = 0; i < RECON; ++i) r[mu * RECON + i] = p[i];
+        }
     }
 #pragma unroll
     for (int j = 0; j < L::NVEC; ++j) {
@@ -103,21 +115,26 @@ __global__ void pack_links_kernel(T *__restrict__ dst, const T *__restrict__ src
 
 size_t native_link_bytes(long long V, int precision, int recon)
 {
-    return (size_t)4 * (size_t)padded_volume(V) * (size_t)recon * (precision == 32 ? 4 : 8);
+    return (size_t)4 * (size_t)padded_volume(V) * (size_t)recon * (precision == 16 ? 2 : precision == 32 ? 4 : 8);
 }
 
-cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon, cudaStream_t s)
+cudaError_t launch_pack_links(void *native, const void *canonical, long long V, int precision, int recon, cudaStream_t s,
+                              int *bad_dev)
 {
     if (V <= 0) return cudaSuccess;
     dim3 grid((unsigned)((V + 127) / 128));
     if (precision == 32 && recon == 18)
-        pack_links_kernel<float, 18><<<grid, 128, 0, s>>>((float *)native, (const float *)canonical, V);
+        pack_links_kernel<float, 18><<<grid, 128, 0, s>>>((float *)native, (const float *)canonical, V, bad_dev);
+    else if (precision == 32 && recon == 12)
+        pack_links_kernel<float, 12><<<grid, 128, 0, s>>>((float *)native, (const float *)canonical, V, bad_dev);
     else if (precision == 32)
-        pack_links_kernel<float, 12><<<grid, 128, 0, s>>>((float *)native, (const float *)canonical, V);
+        pack_links_kernel<float, 8><<<grid, 128, 0, s>>>((float *)native, (const float *)canonical, V, bad_dev);
     else if (recon == 18)
-        pack_links_kernel<double, 18><<<grid, 128, 0, s>>>((double *)native, (const double *)canonical, V);
+        pack_links_kernel<double, 18><<<grid, 128, 0, s>>>((double *)native, (const double *)canonical, V, bad_dev);
+    else if (recon == 12)
+        pack_links_kernel<double, 12><<<grid, 128, 0, s>>>((double *)native, (const double *)canonical, V, bad_dev);
     else
-        pack_links_kernel<double, 12><<<grid, 128, 0, s>>>((double *)native, (const double *)canonical, V);
+        pack_links_kernel<double, 8><<<grid, 128, 0, s>>>((double *)native, (const double *)canonical, V, bad_dev);
     count_launch();
     return cudaGetLastError();
 }

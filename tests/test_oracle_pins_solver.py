@@ -217,3 +217,31 @@ def test_k11_bicgstab_terminates_in_k_steps_on_k_eigenvectors(oracle, k):
     assert len(hist) == k + 1
     assert hist[k] < 1e-9
     assert hist[k - 1] > 1e3 * max(hist[k], 1e-13)
+
+
+def test_k12_preconditioned_gcr_minimises_over_the_preconditioned_krylov_space(oracle):
+    """GCR with a fixed linear preconditioner K: x_k minimises |b - Mhat x| over K K_k(Mhat K, b) =
+    span{K b, K Mhat K b, ...} (right preconditioning); K = 1 reproduces the unpreconditioned solver bit for bit."""
+    dims = (4, 2, 2, 4)
+    U, b = random_fields(dims, 241)
+    mass = -0.1
+    Ur = c2r(U)
+    bm = np.where((parity_mask(dims) == 0)[..., None, None, None], c2r(b[0]), 0.0)
+    Mc = lambda v: r2c(oracle.schur(np.ascontiguousarray(c2r(v)), Ur, dims, mass, 0))
+    a0 = 4.0 + mass
+    K = lambda r: (2.0 / a0) * r - Mc(r) / a0 ** 2           # two terms of the Neumann series of Mhat^-1
+    x0, h0 = wd_solvers.gcr_schur(c2r(b[0]), Ur, dims, mass, 0, niter=6, restart=8)
+    x1, h1 = wd_solvers.gcr_schur(c2r(b[0]), Ur, dims, mass, 0, niter=6, restart=8, precond=lambda r: r.copy())
+    assert np.array_equal(x0, x1) and np.array_equal(h0, h1)
+    k = 5
+    xk, hk = wd_solvers.gcr_schur(c2r(b[0]), Ur, dims, mass, 0, niter=k, restart=8, precond=K)
+    basis = [K(r2c(bm))]
+    for _ in range(k - 1):
+        basis.append(K(Mc(basis[-1])))
+    AK = np.stack([Mc(v).ravel() for v in basis], axis=1)
+    Q, _ = np.linalg.qr(AK)
+    bc = r2c(bm).ravel()
+    best = np.linalg.norm(bc - Q @ (Q.conj().T @ bc)) / np.linalg.norm(bc)
+    assert hk[-1] == pytest.approx(best, rel=1e-7)
+    assert hk[-1] < 0.5 * h0[k]                               # and the preconditioner helps
+    assert np.linalg.norm(bc - Mc(r2c(xk)).ravel()) / np.linalg.norm(bc) == pytest.approx(hk[-1], rel=1e-8)

@@ -1,0 +1,158 @@
+"""-m gpu parity tests of the storage variants: 8-real links and half-precision
+storage, through the C ABI, against the oracle fed with what the storage format actually holds
+(oracle/wd_storage.py, pinned in tests/test_oracle_pins_storage.py).
+
+Tolerances (readings R8 / RH):
+  8 reals   both sides rebuild the link from the SAME eight rounded numbers; the CUDA path does it in the working
+            precision, and rounding in the rebuilt rows is amplified by 1/N, N = |a2|^2 + |a3|^2.  Over a field of
+            Haar or smooth (eps = 0.3) links the rms of 1/N is ~10^2, so the bound is 1e-5 (fp32) / 1e-10 (fp64).
+  half      inputs are the dequantised fields on both sides; the CUDA result is rounded once more to binary16 relative
+            to the site maximum: |error| <= 2^-11 max_site, i.e. <= 2^-11 * sqrt(24) relative L2 in the worst case; 1e-3.
+"""
+import numpy as np
+import pytest
+
+from paper_0912_2186_b200 import binding, fields
+from oracle import wd_storage as ws
+from gpu_util import GpuOp, rel_l2
+
+pytestmark = pytest.mark.gpu
+TOL8 = {32: 1e-5, 64: 1e-10}
+KERNELS = {"auto": 0, "site": 1, "stage": 3}
+
+
+@pytest.mark.parametrize("dims", [(32, 4, 4, 5), (16, 8, 8, 6), (24, 4, 4, 6), (6, 10, 4, 8), (3, 5, 2, 7)])
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("links", ["haar", "smooth"])
+def test_recon8_matches_the_oracle(oracle, dims, precision, links):
+    cfg = fields.Config("r8", dims, precision, links, 8, -0.35, 3, 701)
+    U, psi = fields.make_fields(cfg)
+    U8 = ws.links_from_8(U, precision)                       # what the 8 stored reals say, rebuilt in fp64
+    for kernel in ("site", "stage"):
+        try:
+            op = GpuOp(U, dims, precision, 8, KERNELS[kernel])
+        except binding.WdError as e:
+            assert e.code == -7 and kernel == "stage"        # lattices the staged kernel cannot tile
+            continue
+        for nrhs in (1, 3):
+            got = op.apply(psi[:nrhs], cfg.mass)
+            for r in range(nrhs):
+                want = oracle.apply(psi[r].astype(np.float64), U8, dims, cfg.mass)
+                assert rel_l2(got[r], want) <= TOL8[precision], (kernel, nrhs, r)
+        op.close()
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_recon8_dagger_and_even_odd(oracle, precision):
+    import torch
+    dims = (16, 4, 8, 6)
+    cfg = fields.Config("r8b", dims, precision, "haar", 8, -0.2, 1, 703)
+    U, psi = fields.make_fields(cfg)
+    U8 = ws.links_from_8(U, precision)
+    op = GpuOp(U, dims, precision, 8, KERNELS["stage"])
+    w = op.op
+    canon = torch.from_numpy(psi).cuda()
+    a = torch.empty(w.native_numel(1), dtype=canon.dtype, device="cuda")
+    b = torch.empty_like(a)
+    out = torch.empty_like(canon)
+    w.pack(a, canon, 1)
+    w.apply_dagger(b, a, cfg.mass, 1)
+    w.unpack(out, b, 1)
+    torch.cuda.synchronize()
+    want = oracle.apply(psi[0].astype(np.float64), U8, dims, cfg.mass, sign=+1)
+    assert rel_l2(out.cpu().numpy()[0], want) <= TOL8[precision]
+    # even-odd preconditioned operator with 8-real links
+    n = w.half_numel(1)
+    hi, ho, tmp = (torch.empty(n, dtype=canon.dtype, device="cuda") for _ in range(3))
+    w.pack_parity(hi, canon, 1, 0)
+    w.apply_schur(ho, hi, tmp, cfg.mass, 0, 1)
+    full = torch.zeros_like(canon)
+    w.unpack_parity(full, ho, 1, 0)
+    torch.cuda.synchronize()
+    want = oracle.schur(psi[0].astype(np.float64), U8, dims, cfg.mass, 0)
+    Lx, Ly, Lz, Lt = dims
+    t, z, y, x = np.meshgrid(np.arange(Lt), np.arange(Lz), np.arange(Ly), np.arange(Lx), indexing="ij")
+    even = ((x + y + z + t) % 2 == 0)
+    assert rel_l2(full.cpu().numpy()[0][even], want[even]) <= TOL8[precision]
+    op.close()
+
+
+def test_recon8_refuses_links_it_cannot_hold():
+    dims = (4, 4, 4, 4)
+    U = fields.unit_links(dims).astype(np.float32)
+    with pytest.raises(binding.WdError) as e:
+        GpuOp(U, dims, 32, 8)
+    assert e.value.code == -4
+    cfg = fields.Config("r8c", dims, 32, "haar", 8, 0.1, 1, 705)
+    Uh, _ = fields.make_fields(cfg)
+    op = GpuOp(Uh, dims, 32, 8)
+    with pytest.raises(binding.WdError) as e:
+        op.op.set_temporal_gauge(True)
+    assert e.value.code == -4
+    op.close()
+
+
+# ---------------------------------------------------------------- half-precision storage
+def _half_case(oracle, dims, recon, links, nrhs, dagger=False, seed=711):
+    import torch
+    cfg = fields.Config("half", dims, 32, links, 18, -0.35, nrhs, seed)
+    U, psi = fields.make_fields(cfg)                                    # float32 canonical fields
+    op = binding.WilsonDirac(dims, torch.from_numpy(U).cuda(), 16, recon)
+    assert op.selected_kernel(nrhs) == "site"
+    canon = torch.from_numpy(psi).cuda()
+    n = op.native_numel(nrhs)
+    assert n == nrhs * (-(-fields.volume(dims) // 32) * 32) * 26
+    a = torch.zeros(n, dtype=torch.float16, device="cuda")
+    b = torch.zeros(n, dtype=torch.float16, device="cuda")
+    back = torch.full_like(canon, float("nan"))
+    out = torch.full_like(canon, float("nan"))
+    op.pack(a, canon, nrhs)
+    op.unpack(back, a, nrhs)                                            # what the half field holds
+    (op.apply_dagger if dagger else op.apply)(b, a, cfg.mass, nrhs)
+    op.unpack(out, b, nrhs)
+    torch.cuda.synchronize()
+    op.close()
+    # the stored input is exactly the oracle's quantisation of the same float32 field
+    q, s = ws.quantise_half_spinor(psi)
+    held = ws.dequantise_half_spinor(q, s)
+    assert np.max(np.abs(back.cpu().numpy().astype(np.float64) - held)) <= 1e-6 * np.max(np.abs(held))
+    if recon == 8:
+        Uo = ws.links_from_8(U, 16)
+    else:
+        Uo = ws.quantise_half_links(U if recon == 18 else np.ascontiguousarray(U[..., :2, :, :]))
+    got = out.cpu().numpy().astype(np.float64)
+    for r in range(nrhs):
+        want = oracle.apply(held[r], Uo, dims, cfg.mass, sign=+1 if dagger else -1)
+        assert rel_l2(got[r], want) <= 1e-3, (recon, r, rel_l2(got[r], want))
+        # and it is not the fp32 result in disguise: the error is at the binary16 level
+        assert rel_l2(got[r], want) >= 1e-5
+
+
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (16, 4, 6, 5), (3, 5, 2, 7)])
+@pytest.mark.parametrize("recon", [18, 12, 8])
+def test_half_storage_matches_the_oracle_on_the_dequantised_fields(oracle, dims, recon):
+    _half_case(oracle, dims, recon, "haar", 2)
+
+
+def test_half_storage_dagger_and_smooth_links(oracle):
+    _half_case(oracle, (8, 4, 8, 6), 12, "smooth", 1, dagger=True)
+
+
+def test_half_storage_is_refused_where_it_is_not_implemented():
+    import torch
+    dims = (4, 4, 4, 4)
+    cfg = fields.Config("halfno", dims, 32, "haar", 18, 0.1, 1, 713)
+    U, psi = fields.make_fields(cfg)
+    op = binding.WilsonDirac(dims, torch.from_numpy(U).cuda(), 16, 12)
+    buf = torch.zeros(op.native_numel(1), dtype=torch.float16, device="cuda")
+    buf2 = torch.zeros_like(buf)
+    with pytest.raises(binding.WdError) as e:
+        binding.wd_apply_hop(buf2, buf, op.gauge, dims, 1, 16, 0)
+    assert e.value.code == -3
+    with pytest.raises(binding.WdError) as e:
+        op.set_kernel(3)
+    assert e.value.code == -7
+    with pytest.raises(binding.WdError) as e:
+        op.set_temporal_gauge(True)
+    assert e.value.code == -3
+    op.close()
