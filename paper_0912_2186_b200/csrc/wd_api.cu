@@ -277,8 +277,15 @@ int wd_set_kernel(wd_gauge *gauge, int kernel)
     if (gauge->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_set_kernel: not a live wd_gauge handle");
     if (kernel != WD_KERNEL_AUTO && kernel != WD_KERNEL_SITE && kernel != WD_KERNEL_STAGE)
         return fail(WD_ERR_MISMATCH, "wd_set_kernel: unknown kernel %d", kernel);
-    if (kernel == WD_KERNEL_STAGE && gauge->precision == WD_FP16)
-        return fail(WD_ERR_MISMATCH, "wd_set_kernel: half-precision storage runs through the site-style kernel only");
+    if (kernel == WD_KERNEL_STAGE && gauge->precision == WD_FP16) {
+        wd::ApplyArgs a{};
+        for (int d = 0; d < 4; ++d) a.dims[d] = gauge->dims[d];
+        a.V = gauge->V;
+        if (!wd::half_stage_supported(a))
+            return fail(WD_ERR_MISMATCH, "wd_set_kernel: the staged half-precision kernel does not support this lattice");
+        gauge->kernel = kernel;
+        return WD_OK;
+    }
     if (kernel == WD_KERNEL_STAGE) {
         wd::ApplyArgs a{};
         for (int d = 0; d < 4; ++d) a.dims[d] = gauge->dims[d];
@@ -336,7 +343,8 @@ int wd_unpack_spinor(const wd_lattice *lat, void *canonical_dev, const void *nat
 // members) on every lattice they can tile that has at least one wave of tiles; everything else -> site kernel
 static int auto_kernel(const wd::ApplyArgs &a)
 {
-    if (a.precision == WD_FP16) return WD_KERNEL_SITE; // half-precision storage: the site-style kernel of wd_half.cu
+    if (a.precision == WD_FP16) // half-precision storage: wd_half_stage.cu on large lattices it can tile, else wd_half.cu
+        return (a.V >= (1LL << 18) && wd::half_stage_supported(a)) ? WD_KERNEL_STAGE : WD_KERNEL_SITE;
     const bool big = a.V >= (1LL << 18);
     if (big && wd::stage_supported(a)) return WD_KERNEL_STAGE;
     return WD_KERNEL_SITE;
@@ -372,8 +380,11 @@ static int dispatch_apply(void *out, const void *in, const wd_gauge *g, double m
     a.stream = g->stream;
     a.dagger = dagger;
     cudaError_t e;
-    if (g->precision == WD_FP16)
-        e = wd::launch_half(a);
+    if (g->precision == WD_FP16) {
+        const int k = g->kernel == WD_KERNEL_AUTO ? auto_kernel(a) : g->kernel;
+        if (k == WD_KERNEL_STAGE && !wd::half_stage_supported(a)) return fail(WD_ERR_MISMATCH, "wd_apply: staged kernel cannot take this call");
+        e = k == WD_KERNEL_STAGE ? wd::launch_half_stage(a) : wd::launch_half(a);
+    }
     else if (g->kernel == WD_KERNEL_SITE)
         e = wd::launch_site(a);
     else if (g->kernel == WD_KERNEL_STAGE) {
@@ -446,8 +457,8 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
     // and packed on one stream, D is applied to it (site kernel on the slab's site range) on a second
     // stream as soon as slabs k-1, k, k+1 have arrived, and its result is unpacked and copied out on a
     // third stream, so the host->device and device->host transfers overlap (PCIe is full duplex) ----
-    // (the event arrays of wd_gauge hold 32; more slabs = shorter pipeline fill and drain: measured 32 > 16 > 8)
-    int nslab = g->tune.host_nslab >= 3 ? g->tune.host_nslab : 32;
+    // (the event arrays of wd_gauge hold 32; more slabs = shorter pipeline fill and drain but more launches: measured 16 best)
+    int nslab = g->tune.host_nslab >= 3 ? g->tune.host_nslab : 16;
     if (nslab > 32) nslab = 32;
     if (nslab > Lt) nslab = Lt;
     const bool pipelined = nslab >= 3 && S3 % 128 == 0 && bytes >= (8u << 20) && g->tune.host_no_pipeline <= 0;
@@ -483,7 +494,10 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
         for (int i = 0; i < 3; ++i) cudaStreamWaitEvent(g->pipe_stream[i], ev_start, 0);
         auto t0 = [&](int k) { return (long long)Lt * k / nslab; };
         const size_t row = (size_t)g->V * 24 * w; // bytes of one right-hand side, canonical
-        for (int k = 0; k < nslab; ++k) {
+        // arrival order: the LAST slab first (it is slab 0's backward neighbour), then 0, 1, ..., nslab-2: slab k can be
+        // computed as soon as slab k+1 has arrived, and only two slabs are left to compute when the last one lands
+        for (int i = 0; i < nslab; ++i) {
+            const int k = i == 0 ? nslab - 1 : i - 1;
             const long long s0 = t0(k) * S3, ns = (t0(k + 1) - t0(k)) * S3;
             e = cudaMemcpy2DAsync((char *)g->stage_canon + (size_t)s0 * 24 * w, row,
                                   (const char *)in_canonical_host + (size_t)s0 * 24 * w, row, (size_t)ns * 24 * w, nrhs,
@@ -493,9 +507,7 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
             if (e != cudaSuccess) return bail(e, "wd_apply_host: pack");
             cudaEventRecord(ev_in[k], s_in);
         }
-        // interior slabs in arrival order, then the two that need the wrap-around neighbour
-        for (int i = 0; i < nslab; ++i) {
-            const int k = i < nslab - 2 ? i + 1 : (i == nslab - 2 ? 0 : nslab - 1);
+        for (int k = 0; k < nslab; ++k) {
             const int need[3] = {(k + nslab - 1) % nslab, k, (k + 1) % nslab};
             for (int n : need) cudaStreamWaitEvent(s_cmp, ev_in[n], 0);
             wd::ApplyArgs a = shape_args(g, nrhs);

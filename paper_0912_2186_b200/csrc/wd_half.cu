@@ -61,15 +61,19 @@ __device__ __forceinline__ void load_spinor_h(const uint4 *__restrict__ field, c
     for (int i = 0; i < 24; ++i) p[i] *= s;
 }
 
-// 24 floats -> scale + ratios (reading RH); the same arithmetic as oracle/wd_storage.py:quantise_half_spinor
+// 24 floats -> scale + ratios (reading RH).  EXACT: the ratios are IEEE divisions, the same arithmetic as
+// oracle/wd_storage.py:quantise_half_spinor (wd_pack_spinor: what is stored is bit for bit what the oracle holds);
+// otherwise (kernel epilogues) one reciprocal and 24 products, which may differ by one float ulp before the binary16 rounding.
+template <bool EXACT>
 __device__ __forceinline__ void store_spinor_h(uint4 *__restrict__ field, float *__restrict__ scale, long long site, const float (&p)[24])
 {
     float s = 0.f;
 #pragma unroll
     for (int i = 0; i < 24; ++i) s = fmaxf(s, fabsf(p[i]));
     float r[24];
+    const float rs = s > 0.f ? __frcp_rn(s) : 0.f;
 #pragma unroll
-    for (int i = 0; i < 24; ++i) r[i] = s > 0.f ? __fdiv_rn(p[i], s) : 0.f;
+    for (int i = 0; i < 24; ++i) r[i] = EXACT ? (s > 0.f ? __fdiv_rn(p[i], s) : 0.f) : p[i] * rs;
     uint4 *q = field + (site >> 5) * (3 * BLK) + (site & (BLK - 1));
 #pragma unroll
     for (int c = 0; c < 3; ++c) q[c * BLK] = pack8(&r[8 * c]);
@@ -141,7 +145,7 @@ dslash_half_kernel(uint4 *__restrict__ out, float *__restrict__ out_scale, const
     load_spinor_h(in, in_scale, site, p);
 #pragma unroll
     for (int i = 0; i < 24; ++i) p[i] = fmaf(cdiag, p[i], -0.5f * acc[i]);
-    store_spinor_h(out, out_scale, site, p);
+    store_spinor_h<false>(out, out_scale, site, p);
 }
 
 // canonical float32 [rhs][site][24] <-> native half
@@ -161,7 +165,7 @@ __global__ void spinor_half_kernel(uint4 *native, float *scale, float *canon, lo
             const float4 v = reinterpret_cast<const float4 *>(c)[i];
             p[4 * i] = v.x; p[4 * i + 1] = v.y; p[4 * i + 2] = v.z; p[4 * i + 3] = v.w;
         }
-        store_spinor_h(native, scale, site, p);
+        store_spinor_h<true>(native, scale, site, p);
     } else {
         load_spinor_h(native, scale, site, p);
 #pragma unroll

@@ -16,7 +16,7 @@ struct Tuning {
     int site_slab_mb = -1;          // WD_SITE_SLAB_MB  link slab of the site kernel's multi-RHS block order
     int host_no_pipeline = -1;      // WD_HOST_NO_PIPELINE  1 = one-stream wd_apply_host
     int mrhs_no_tail = -1;          // WD_MRHS_NO_TAIL  1 = no shortened t-chunks in the last wave of the multi-RHS kernel
-    int host_nslab = -1;            // WD_HOST_NSLAB    slabs of the pipelined wd_apply_host (3..32, default 32)
+    int host_nslab = -1;            // WD_HOST_NSLAB    slabs of the pipelined wd_apply_host (3..32, default 16)
 };
 void tuning_from_env(Tuning &t);
 int tuning_set(Tuning &t, const char *name, int value); // 0 = ok, -1 = unknown name
@@ -121,6 +121,8 @@ cudaError_t launch_coarse_apply(void *out, const void *in, const void *S, const 
                                 cudaStream_t s);
 // half-precision storage (wd_half.cu): fp32 arithmetic on binary16 fields; canonical side is float32
 cudaError_t launch_half(const ApplyArgs &a);
+bool half_stage_supported(const ApplyArgs &a); // staged member (wd_half_stage.cu): Lx a power of two, tiles of <= 128 sites
+cudaError_t launch_half_stage(const ApplyArgs &a);
 cudaError_t launch_spinor_half(void *native, void *canonical, long long V, int nrhs, bool to_native, cudaStream_t s);
 cudaError_t launch_pack_links_half(void *native, const void *canonical, long long V, int recon, cudaStream_t s, int *bad_dev);
 cudaError_t launch_parity_copy(void *native, void *canon, const int dims[4], long long V, int nrhs, int precision,

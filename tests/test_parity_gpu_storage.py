@@ -93,12 +93,12 @@ def test_recon8_refuses_links_it_cannot_hold():
 
 
 # ---------------------------------------------------------------- half-precision storage
-def _half_case(oracle, dims, recon, links, nrhs, dagger=False, seed=711):
+def _half_case(oracle, dims, recon, links, nrhs, dagger=False, seed=711, kernel=0):
     import torch
     cfg = fields.Config("half", dims, 32, links, 18, -0.35, nrhs, seed)
     U, psi = fields.make_fields(cfg)                                    # float32 canonical fields
-    op = binding.WilsonDirac(dims, torch.from_numpy(U).cuda(), 16, recon)
-    assert op.selected_kernel(nrhs) == "site"
+    op = binding.WilsonDirac(dims, torch.from_numpy(U).cuda(), 16, recon, kernel=kernel)
+    assert op.selected_kernel(nrhs) == ("stage" if kernel == 3 else "site")
     canon = torch.from_numpy(psi).cuda()
     n = op.native_numel(nrhs)
     assert n == nrhs * (-(-fields.volume(dims) // 32) * 32) * 26
@@ -138,6 +138,42 @@ def test_half_storage_dagger_and_smooth_links(oracle):
     _half_case(oracle, (8, 4, 8, 6), 12, "smooth", 1, dagger=True)
 
 
+@pytest.mark.parametrize("dims", [(32, 4, 4, 5), (16, 8, 8, 6), (8, 4, 12, 7), (4, 8, 8, 3), (32, 6, 10, 4)])
+@pytest.mark.parametrize("recon", [18, 12, 8])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_half_storage_staged_kernel(oracle, dims, recon, dagger):
+    """The staged (cp.async, t-marching) member of the half-precision family: raw binary16 data staged in shared memory,
+    converted at the LDS, result requantised in the epilogue; chunk boundaries and faces as in the fp32 kernel."""
+    _half_case(oracle, dims, recon, "haar", 2, dagger=dagger, kernel=3)
+
+
+def test_half_storage_staged_kernel_is_deterministic(monkeypatch):
+    """Same launch twice: same bits.  Other t-chunk lengths (march restarts at other slices): the same field up to the
+    binary16 rounding of the result (the restart computes the first backward t hop from global memory, a different
+    instruction sequence, so bit equality across chunkings is not promised)."""
+    import torch
+    dims = (16, 8, 8, 12)
+    cfg = fields.Config("halfdet", dims, 32, "smooth", 18, -0.42, 1, 715)
+    U, psi = fields.make_fields(cfg)
+    outs = []
+    for tc in ("16", "16", "1", "5"):
+        monkeypatch.setenv("WD_TILE_TC", tc)
+        op = binding.WilsonDirac(dims, torch.from_numpy(U).cuda(), 16, 12, kernel=3)
+        a = torch.zeros(op.native_numel(1), dtype=torch.float16, device="cuda")
+        b = torch.zeros_like(a)
+        canon = torch.from_numpy(psi).cuda()
+        op.pack(a, canon, 1)
+        op.apply(b, a, cfg.mass, 1)
+        out = torch.empty_like(canon)
+        op.unpack(out, b, 1)
+        torch.cuda.synchronize()
+        outs.append((b.clone(), out.cpu().numpy().astype(np.float64)))
+        op.close()
+    assert torch.equal(outs[0][0].view(torch.int16), outs[1][0].view(torch.int16))
+    for k in (2, 3):
+        assert rel_l2(outs[k][1], outs[0][1]) <= 5e-4
+
+
 def test_half_storage_is_refused_where_it_is_not_implemented():
     import torch
     dims = (4, 4, 4, 4)
@@ -149,9 +185,7 @@ def test_half_storage_is_refused_where_it_is_not_implemented():
     with pytest.raises(binding.WdError) as e:
         binding.wd_apply_hop(buf2, buf, op.gauge, dims, 1, 16, 0)
     assert e.value.code == -3
-    with pytest.raises(binding.WdError) as e:
-        op.set_kernel(3)
-    assert e.value.code == -7
+    op.set_kernel(3)                                    # 4^4 can be tiled by the staged half kernel
     with pytest.raises(binding.WdError) as e:
         op.set_temporal_gauge(True)
     assert e.value.code == -3
