@@ -79,8 +79,8 @@ def test_load_gauge_validates_before_touching_the_device(lib):
     lat = binding.wd_create_lattice((4, 4, 4, 4))
     h = ctypes.c_void_p()
     fake = ctypes.c_void_p(0x1000)
-    assert lib.wd_load_gauge(lat, fake, 16, 18, None, ctypes.byref(h)) == -3
-    assert lib.wd_load_gauge(lat, fake, 32, 8, None, ctypes.byref(h)) == -4
+    assert lib.wd_load_gauge(lat, fake, 24, 18, None, ctypes.byref(h)) == -3   # (16 = half storage, 32, 64 are valid)
+    assert lib.wd_load_gauge(lat, fake, 32, 10, None, ctypes.byref(h)) == -4   # (18, 12, 8 are valid)
     assert lib.wd_load_gauge(lat, None, 32, 18, None, ctypes.byref(h)) == -1
     assert not h.value
     binding.wd_destroy(lat)
