@@ -430,3 +430,42 @@ def test_launch_counter_counts_kernels():
     op.apply(psi, cfg.mass)  # pack + apply + unpack
     assert binding.wd_launch_count() - n0 == 3
     op.close()
+
+
+# ---------------------------------------------------------------- guard bands (compute-sanitizer is closed on this pool)
+@pytest.mark.parametrize("dims,precision,recon,nrhs,kernel", [
+    ((16, 16, 16, 32), 32, 18, 1, "stage"), ((16, 16, 16, 32), 32, 18, 1, "site"), ((4, 4, 4, 4), 64, 18, 1, "auto"),
+    ((16, 8, 8, 6), 32, 12, 5, "stage"), ((24, 4, 4, 6), 32, 18, 4, "stage"), ((16, 8, 8, 6), 64, 18, 3, "stage"),
+    ((32, 4, 4, 5), 32, 8, 2, "stage"), ((6, 10, 4, 9), 32, 18, 3, "site"), ((16, 8, 8, 6), 16, 12, 2, "stage"),
+    ((6, 10, 4, 9), 16, 18, 2, "site")])
+def test_kernels_write_only_their_output(dims, precision, recon, nrhs, kernel):
+    """The output buffer sits between two 64 KB guard bands filled with a bit pattern, the input likewise: after wd_apply
+    and wd_apply_dagger every guard byte is unchanged and every real site of the output has been written.  (Stands in
+    for a memcheck run: compute-sanitizer answers "closed on this pool".)"""
+    import torch
+    from paper_0912_2186_b200 import binding
+    cprec = 32 if precision == 16 else precision
+    cfg = fields.Config("guard", dims, cprec, "haar", recon, -0.3, nrhs, 121)
+    U, psi = fields.make_fields(cfg)
+    op = binding.WilsonDirac(dims, torch.from_numpy(U).cuda(), precision, recon, kernel=KERNELS[kernel])
+    nbytes = binding.wd_spinor_bytes(op.lat, nrhs, precision)
+    G = 65536
+    bufs = []
+    for _ in range(2):
+        raw = torch.full((nbytes + 2 * G,), 0x5A, dtype=torch.uint8, device="cuda")
+        bufs.append(raw)
+    src, dst = bufs[0][G:G + nbytes], bufs[1][G:G + nbytes]
+    canon = torch.from_numpy(psi).cuda()
+    op.pack(src, canon, nrhs)
+    for fn in (op.apply, op.apply_dagger):
+        dst.fill_(0x5A)
+        fn(dst, src, cfg.mass, nrhs)
+        torch.cuda.synchronize()
+        for raw in bufs:
+            assert bool(torch.all(raw[:G] == 0x5A)) and bool(torch.all(raw[G + nbytes:] == 0x5A))
+        out = torch.full_like(canon, float("nan"))
+        op.unpack(out, dst, nrhs)
+        torch.cuda.synchronize()
+        assert bool(torch.isfinite(out).all())
+        assert not bool((out.view(torch.uint8) == 0x5A).all(dim=-1).any())   # no site left at the fill pattern
+    op.close()
