@@ -42,6 +42,31 @@ __device__ __forceinline__ void cpa16(float4 *smem_dst, const float4 *gsrc)
 __device__ __forceinline__ void cpa_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cpa_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
+// ---- bulk-copy (cp.async.bulk + mbarrier) variant of the link staging: the A/B the round-1 review asked for ----
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *b, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect(unsigned long long *b, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *b)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(b))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity)
+{
+    asm volatile("{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n" ::"r"(
+                     smem_u32(b)),
+                 "r"(parity)
+                 : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+
 template <int NV>
 __device__ __forceinline__ void lds_vecs(const float4 *buf, int stride, int slot, float *r)
 {
@@ -67,6 +92,16 @@ __device__ __forceinline__ void lds_link(const float4 *base, int first0, int str
     if (RECON == 8) reconstruct_from8(u);
 }
 
+// link MU of tile site slot s out of the staged links: [vector][slot] (default) or, for the bulk-copy variant,
+// [row of 32 sites][vector][lane]
+template <int MU, int RECON, bool BULK>
+__device__ __forceinline__ void own_link_rd(const float4 *lnk, int nts, int s, float (&u)[18])
+{
+    constexpr int NVEC = LinkLayout<float, RECON>::NVEC;
+    if (BULK) lds_link<MU, RECON>(lnk + (s >> 5) * (NVEC * 32), 0, 32, s & 31, u);
+    else lds_link<MU, RECON>(lnk, 0, nts, s, u);
+}
+
 __device__ __forceinline__ void shfl12(float (&dst)[12], const float (&src)[12], int src_lane)
 {
 #pragma unroll
@@ -90,7 +125,11 @@ template <int RECON> constexpr int mrhs_smem_vecs(int nts, int nrb, int nyb, int
 // XS: x hops by warp shuffles (Lx a power of two); otherwise (e.g. Lx = 24, the paper's 24^3 x 64 volume)
 // x is handled like y and z: neighbour spinor from the slice buffer, neighbour link from the staged links, periodic
 // wrap in the slot arithmetic (the tile always spans the whole x extent).
-template <int RECON, int NRB, int NTS, bool XS>
+// BULK: the link halves are staged by cp.async.bulk (one 512-byte copy per (vector, 32-site row), each issued by one
+// thread, completion through an mbarrier) instead of one 16-byte cp.async per thread and vector; Lx = 32 only (a row of
+// the tile is one layout block).  Selected by the tuning variable mrhs_bulk; measured against the default in
+// profiles/r02_ncu.md section 6.
+template <int RECON, int NRB, int NTS, bool XS, bool BULK = false>
 __global__ void __launch_bounds__(128 * NRB, 1)
 dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const float *__restrict__ links, int Lx, int Ly,
                    int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk, int patch, int tgauge,
@@ -204,13 +243,58 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         else if (NRB == 2 || rr == 1) copy_links(std::integral_constant<int, 1 % NRB>{}, j0, j1, dst, stride, slot, src, src0);
         else copy_links(std::integral_constant<int, 2 % NRB>{}, j0, j1, dst, stride, slot, src, src0);
     };
+    __shared__ unsigned long long mbar[2]; // BULK: completion of the x,y half / the z,t half
+    unsigned ph_xy = 0, ph_zt = 0;
+    if (BULK) {
+        if (tid == 0) {
+            mbar_init(&mbar[0], 1);
+            mbar_init(&mbar[1], 1);
+            asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        }
+        __syncthreads();
+    }
+    // BULK: copy c of a half = (vector j, row r) of the tile's own links, then the face rows.  Row r of the tile
+    // (yy = r % ty, zz = r / ty) is the 32-site layout block of site (0, y, z); its record is NVEC * 512 bytes.
+    const int nrow = nts >> 5, nrow_y = nyb >> 5, nrow_z = nzb >> 5;
+    auto row_block = [&](int yyy, int zzz) { // layout block of the row (y, z) of the lattice, wrapped
+        const int Y = (yyy + Ly) % Ly, Z = (zzz + Lz) % Lz;
+        return ((long long)Lx * (Y + (long long)Ly * Z)) >> 5;
+    };
+    // BULK shared-memory layout of the links: [row][vector][lane] (a row's record is contiguous, as in global memory),
+    // so a half of a row is ONE copy of (j1 - j0) * 512 bytes; face rows likewise.
+    auto bulk_half = [&](unsigned long long *bar, int j0, int j1, const float4 *base_t, int fn, int ffirst, float4 *fdst, int frow,
+                         bool yface) {
+        if (tid == 0) mbar_expect(bar, (unsigned)(nrow * (j1 - j0) + frow * fn) * 512u);
+        if (tid < nrow + frow) {
+            fence_proxy_async(); // earlier generic-proxy reads of these slots (before the barrier) precede the async writes
+            if (tid < nrow) {
+                const int r = tid;
+                const long long blk = row_block(cy * ty + r % ty, cz * tz + r / ty);
+                bulk_g2s(lnk + (r * NVEC + j0) * 32, base_t + (blk * NVEC + j0) * BLK, (unsigned)(j1 - j0) * 512u, bar);
+            } else {
+                const int r = tid - nrow; // face row r: yface: zz = r, yy = 0; zface: yy = r, zz = 0
+                const long long blk = yface ? row_block(cy * ty - 1, cz * tz + r) : row_block(cy * ty + r, cz * tz - 1);
+                bulk_g2s(fdst + r * fn * 32, base_t + (blk * NVEC + ffirst) * BLK, (unsigned)fn * 512u, bar);
+            }
+        }
+    };
     auto stage_XY = [&](long long toff) { // links x,y of the site + the y-face link
+        if (BULK) {
+            bulk_half(&mbar[0], 0, A_END, reinterpret_cast<const float4 *>(links) + (toff >> 5) * (NVEC * BLK), FY::n, FY::first, fly,
+                      nrow_y, true);
+            return;
+        }
         deal_links(0, A_END, lnk, nts, st, lk_own + toff * NVEC, 0);
         if (face_yb) deal_links(0, FY::n, fly, nyb, rank_y, lk_y + toff * NVEC, FY::first);
     };
     // temporal gauge (wd_set_temporal_gauge): U_t(x,t) = 1 for t < Lt-1 -- those links are neither copied nor read
     auto unit_t = [&](int t) { return tgauge && t != Lt - 1; };
     auto stage_ZT = [&](long long toff, int t) { // links z,t of the site + the z-face link
+        if (BULK) {
+            bulk_half(&mbar[1], A_END, unit_t(t) ? FZ::last + 1 : NVEC,
+                      reinterpret_cast<const float4 *>(links) + (toff >> 5) * (NVEC * BLK), FZ::n, FZ::first, flz, nrow_z, false);
+            return;
+        }
         deal_links(A_END, unit_t(t) ? FZ::last + 1 : NVEC, lnk + A_END * nts, nts, st, lk_own + toff * NVEC, A_END);
         if (face_zb) deal_links(0, FZ::n, flz, nzb, rank_z, lk_z + toff * NVEC, FZ::first);
     };
@@ -246,6 +330,10 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         const long long toff_n = (long long)(t + 1 == Lt ? 0 : t + 1) * S3;
         const bool more = (t + 1 < t_end);
         cpa_wait<1>();   // links x,y and the y-face spinor of slice t have landed (own copies)
+        if (BULK) {
+            mbar_wait(&mbar[0], ph_xy);
+            ph_xy ^= 1;
+        }
         __syncthreads(); // (A) ... everybody's; the z,t hops of slice t-1 are over
         stage_ZT(toff, t);
         stage_spinor(plane0 + (cur ^ 1) * plane_sz, sp_own, toff_n);
@@ -259,12 +347,12 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         reconstruct_add<3, +1>(acc, chi_t); // backward t hop, product carried from the previous slice
 
         // ---- x: both hops through warp shuffles (XS), else like y and z ----
-        lds_link<0, RECON>(lnk, 0, nts, st, u);
+        own_link_rd<0, RECON, BULK>(lnk, nts, st, u);
         if (!XS) {
             const int dxf = (x + 1 == Lx ? 1 - Lx : 1), dxb = (x == 0 ? Lx - 1 : -1);
             lds_vecs<6>(pl, nt, tid + dxf, pn);
             hop_forward<0>(acc, u, pn);
-            lds_link<0, RECON>(lnk, 0, nts, st + dxb, u);
+            own_link_rd<0, RECON, BULK>(lnk, nts, st + dxb, u);
             lds_vecs<6>(pl, nt, tid + dxb, pn);
             hop_backward<0>(acc, u, pn);
         } else {
@@ -279,34 +367,40 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
             reconstruct_add<0, +1>(acc, gg);
         }
         // ---- y: forward with the own link, backward with the link of the site below ----
-        lds_link<1, RECON>(lnk, 0, nts, st, u);
+        own_link_rd<1, RECON, BULK>(lnk, nts, st, u);
         if (face_yf) lds_vecs<6>(fy, nt, tid, pn);
         else lds_vecs<6>(pl, nt, tid + Lx, pn);
         hop_forward<1>(acc, u, pn);
         if (face_yb) {
-            lds_link<1, RECON>(fly, FY::first, nyb, rank_y, u);
+            if (BULK) lds_link<1, RECON>(fly + (rank_y >> 5) * (FY::n * 32), FY::first, 32, rank_y & 31, u);
+            else lds_link<1, RECON>(fly, FY::first, nyb, rank_y, u);
             lds_vecs<6>(fy, nt, tid, pn);
         } else {
-            lds_link<1, RECON>(lnk, 0, nts, st - Lx, u);
+            own_link_rd<1, RECON, BULK>(lnk, nts, st - Lx, u);
             lds_vecs<6>(pl, nt, tid - Lx, pn);
         }
         hop_backward<1>(acc, u, pn);
         if (more && (face_yf | face_yb)) stage_spinor(fy, sp_y, toff_n);
         cpa_commit(); // c2
         cpa_wait<1>();   // links z,t of slice t, own spinor of slice t+1, z-face spinor of slice t have landed
+        if (BULK) {
+            mbar_wait(&mbar[1], ph_zt);
+            ph_zt ^= 1;
+        }
         __syncthreads(); // (M) ... everybody's; the x,y hops of slice t are over
         if (more) stage_XY(toff_n);
         cpa_commit(); // c3
         // ---- z ----
-        lds_link<2, RECON>(lnk, 0, nts, st, u);
+        own_link_rd<2, RECON, BULK>(lnk, nts, st, u);
         if (face_zf) lds_vecs<6>(fz, nt, tid, pn);
         else lds_vecs<6>(pl, nt, tid + Lx * ty, pn);
         hop_forward<2>(acc, u, pn);
         if (face_zb) {
-            lds_link<2, RECON>(flz, FZ::first, nzb, rank_z, u);
+            if (BULK) lds_link<2, RECON>(flz + (rank_z >> 5) * (FZ::n * 32), FZ::first, 32, rank_z & 31, u);
+            else lds_link<2, RECON>(flz, FZ::first, nzb, rank_z, u);
             lds_vecs<6>(fz, nt, tid, pn);
         } else {
-            lds_link<2, RECON>(lnk, 0, nts, st - Lx * ty, u);
+            own_link_rd<2, RECON, BULK>(lnk, nts, st - Lx * ty, u);
             lds_vecs<6>(pl, nt, tid - Lx * ty, pn);
         }
         hop_backward<2>(acc, u, pn);
@@ -321,7 +415,7 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
                 reconstruct_add<3, -1>(acc, h);
                 project<3, +1>(psi, chi_t);
             } else {
-                lds_link<3, RECON>(lnk, 0, nts, st, u);
+                own_link_rd<3, RECON, BULK>(lnk, nts, st, u);
                 hop_forward<3>(acc, u, pn);
                 project<3, +1>(psi, h);
                 su3_dag_mul(u, h, chi_t);
@@ -345,10 +439,10 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
 // ---------------------------------------------------------------------------------------------
 namespace {
 
-template <int RECON, int NRB, int NTS, bool XS>
+template <int RECON, int NRB, int NTS, bool XS, bool BULK = false>
 cudaError_t launch_mrhs_n(const ApplyArgs &a, int ty, int tz)
 {
-    auto kern = dslash_mrhs_kernel<RECON, NRB, NTS, XS>;
+    auto kern = dslash_mrhs_kernel<RECON, NRB, NTS, XS, BULK>;
     const int Lx = a.dims[0];
     const int nts = Lx * ty * tz;
     const size_t smem = (size_t)mrhs_smem_vecs<RECON>(nts, NRB, Lx * tz, Lx * ty) * sizeof(float4);
@@ -399,6 +493,8 @@ cudaError_t launch_mrhs_t(const ApplyArgs &a, int ty, int tz)
 {
     const int nts = a.dims[0] * ty * tz;
     if (a.dims[0] & (a.dims[0] - 1)) return nts == 96 ? launch_mrhs_n<RECON, NRB, 96, false>(a, ty, tz) : launch_mrhs_n<RECON, NRB, 0, false>(a, ty, tz);
+    const Tuning &tn = a.tune ? *a.tune : default_tuning();
+    if (nts == 128 && a.dims[0] == 32 && NRB == 3 && tn.mrhs_bulk > 0) return launch_mrhs_n<RECON, NRB, 128, true, true>(a, ty, tz);
     return nts == 128 ? launch_mrhs_n<RECON, NRB, 128, true>(a, ty, tz) : launch_mrhs_n<RECON, NRB, 0, true>(a, ty, tz);
 }
 

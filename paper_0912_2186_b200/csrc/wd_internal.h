@@ -16,6 +16,7 @@ struct Tuning {
     int site_slab_mb = -1;          // WD_SITE_SLAB_MB  link slab of the site kernel's multi-RHS block order
     int host_no_pipeline = -1;      // WD_HOST_NO_PIPELINE  1 = one-stream wd_apply_host
     int mrhs_no_tail = -1;          // WD_MRHS_NO_TAIL  1 = no shortened t-chunks in the last wave of the multi-RHS kernel
+    int mrhs_bulk = -1;             // WD_MRHS_BULK     1 = stage the links of the multi-RHS kernel by cp.async.bulk (A/B variant)
     int host_nslab = -1;            // WD_HOST_NSLAB    slabs of the pipelined wd_apply_host (3..32, default 16)
 };
 void tuning_from_env(Tuning &t);

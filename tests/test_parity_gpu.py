@@ -387,6 +387,29 @@ def test_fp64_multi_rhs_shares_links_through_l2(oracle, dims, nrhs, recon):
     check_config(oracle, cfg, "stage")
 
 
+@pytest.mark.parametrize("recon,tgauge", [(18, False), (12, False), (18, True)])
+def test_multi_rhs_bulk_copy_variant_is_bit_identical(oracle, recon, tgauge):
+    """WD_MRHS_BULK: the link halves staged by cp.async.bulk + mbarrier instead of per-thread cp.async (the A/B variant of
+    profiles/r02_ncu.md section 6): same bits as the default staging, and the oracle's result."""
+    import torch
+    cfg = fields.Config("bulk", (32, 8, 8, 6), 32, "smooth", recon, -0.42, 7, 101)
+    U, psi = fields.make_fields(cfg)
+    if tgauge:
+        U, _ = fields.temporal_gauge(U, 32)
+    op = GpuOp(U, cfg.dims, 32, recon, KERNELS["stage"])
+    if tgauge:
+        op.op.set_temporal_gauge(True)
+    a = op.apply(psi, cfg.mass, return_native=True).clone()
+    op.op.set_tuning("mrhs_bulk", 1)
+    b = op.apply(psi, cfg.mass, return_native=True).clone()
+    got = op.apply(psi, cfg.mass)
+    op.close()
+    assert torch.equal(a, b)
+    want = oracle_apply(oracle, psi, oracle_links(U, recon), cfg.dims, cfg.mass)
+    for r in range(7):
+        assert rel_l2(got[r], want[r]) <= TOL[32]
+
+
 def test_multi_rhs_tail_wave_split_is_bit_identical(oracle):
     """A launch of more work items than SMs whose last wave is partial cuts that wave's items into shorter marches
     (wd_dslash_mrhs.cu); the result is bit-identical to the uncut launch and matches the oracle."""
