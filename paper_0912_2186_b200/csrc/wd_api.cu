@@ -495,8 +495,10 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
         for (int i = 0; i < 3; ++i) cudaStreamWaitEvent(g->pipe_stream[i], ev_start, 0);
         auto t0 = [&](int k) { return (long long)Lt * k / nslab; };
         const size_t row = (size_t)g->V * 24 * w; // bytes of one right-hand side, canonical
-        // arrival order: the LAST slab first (it is slab 0's backward neighbour), then 0, 1, ..., nslab-2: slab k can be
-        // computed as soon as slab k+1 has arrived, and only two slabs are left to compute when the last one lands
+        // Copy streams carry ONLY copies (back to back, nothing between two transfers); pack, apply and unpack all run on
+        // the compute stream.  Arrival order: the LAST slab first (it is slab 0's backward neighbour), then 0, 1, ...,
+        // nslab-2: slab k can be computed as soon as slab k+1 has arrived, and only two slabs are left to compute when
+        // the last one lands.
         for (int i = 0; i < nslab; ++i) {
             const int k = i == 0 ? nslab - 1 : i - 1;
             const long long s0 = t0(k) * S3, ns = (t0(k + 1) - t0(k)) * S3;
@@ -504,13 +506,19 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
                                   (const char *)in_canonical_host + (size_t)s0 * 24 * w, row, (size_t)ns * 24 * w, nrhs,
                                   cudaMemcpyHostToDevice, s_in);
             if (e != cudaSuccess) return bail(e, "wd_apply_host: H2D copy");
-            e = wd::launch_pack_spinor(g->stage_in, g->stage_canon, g->V, nrhs, precision, s_in, s0, ns);
-            if (e != cudaSuccess) return bail(e, "wd_apply_host: pack");
             cudaEventRecord(ev_in[k], s_in);
         }
+        bool packed[32] = {};
         for (int k = 0; k < nslab; ++k) {
             const int need[3] = {(k + nslab - 1) % nslab, k, (k + 1) % nslab};
-            for (int n : need) cudaStreamWaitEvent(s_cmp, ev_in[n], 0);
+            for (int n : need) {
+                if (packed[n]) continue;
+                cudaStreamWaitEvent(s_cmp, ev_in[n], 0);
+                e = wd::launch_pack_spinor(g->stage_in, g->stage_canon, g->V, nrhs, precision, s_cmp, t0(n) * S3,
+                                           (t0(n + 1) - t0(n)) * S3);
+                if (e != cudaSuccess) return bail(e, "wd_apply_host: pack");
+                packed[n] = true;
+            }
             wd::ApplyArgs a = shape_args(g, nrhs);
             a.out = g->stage_out;
             a.in = g->stage_in;
@@ -520,11 +528,11 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
             a.site_begin = t0(k) * S3;
             a.site_end = t0(k + 1) * S3;
             if ((e = wd::launch_site(a)) != cudaSuccess) return bail(e, "wd_apply_host: kernel launch");
-            cudaEventRecord(ev_cmp[k], s_cmp);
-            cudaStreamWaitEvent(s_out, ev_cmp[k], 0);
-            e = wd::launch_unpack_spinor(g->stage_canon_out, g->stage_out, g->V, nrhs, precision, s_out, a.site_begin,
+            e = wd::launch_unpack_spinor(g->stage_canon_out, g->stage_out, g->V, nrhs, precision, s_cmp, a.site_begin,
                                          a.site_end - a.site_begin);
             if (e != cudaSuccess) return bail(e, "wd_apply_host: unpack");
+            cudaEventRecord(ev_cmp[k], s_cmp);
+            cudaStreamWaitEvent(s_out, ev_cmp[k], 0);
             e = cudaMemcpy2DAsync((char *)out_canonical_host + (size_t)a.site_begin * 24 * w, row,
                                   (const char *)g->stage_canon_out + (size_t)a.site_begin * 24 * w, row,
                                   (size_t)(a.site_end - a.site_begin) * 24 * w, nrhs, cudaMemcpyDeviceToHost, s_out);

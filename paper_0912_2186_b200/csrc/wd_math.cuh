@@ -226,18 +226,25 @@ __device__ __forceinline__ void reconstruct_row2(T (&u)[18])
 // wd_load_gauge refuses such links.  Rounding is amplified by 1/N in b2, b3, c2, c3.
 __device__ __forceinline__ void wd_sincospi(float x, float &s, float &c) { sincospif(x, &s, &c); }
 __device__ __forceinline__ void wd_sincospi(double x, double &s, double &c) { sincospi(x, &s, &c); }
+// square root and reciprocal of the rebuild: fp32 takes the 2-ulp hardware approximations (x * rsqrt(x), rcp) -- their error
+// is of the size of the rounding the 1/N amplification already multiplies (tolerance R8) and they save ~25 instructions
+// per link in a kernel that the rebuild makes instruction bound; fp64 is exact
+__device__ __forceinline__ float wd_sqrt0(float x) { return x > 0.f ? x * rsqrtf(x) : 0.f; }
+__device__ __forceinline__ double wd_sqrt0(double x) { return x > 0.0 ? sqrt(x) : 0.0; }
+__device__ __forceinline__ float wd_rcp(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ double wd_rcp(double x) { return 1.0 / x; }
 template <typename T>
 __device__ __forceinline__ void reconstruct_from8(T (&u)[18])
 {
     const T a2r = u[0], a2i = u[1], a3r = u[2], a3i = u[3], b1r = u[4], b1i = u[5], tha = u[6], thc = u[7];
     const T N = a2r * a2r + a2i * a2i + a3r * a3r + a3i * a3i;
-    const T inv = (T)1 / N;
-    const T ma1 = sqrt(max((T)0, (T)1 - N));
+    const T inv = wd_rcp(N);
+    const T ma1 = wd_sqrt0((T)1 - N);
     T sa, ca, sc, cc;
     wd_sincospi(tha, sa, ca);
     wd_sincospi(thc, sc, cc);
     const T a1r = ma1 * ca, a1i = ma1 * sa;
-    const T mc1 = sqrt(max((T)0, (T)1 - ma1 * ma1 - (b1r * b1r + b1i * b1i)));
+    const T mc1 = wd_sqrt0((T)1 - ma1 * ma1 - (b1r * b1r + b1i * b1i));
     const T c1r = mc1 * cc, c1i = mc1 * sc;
     const T pr = a1r * b1r + a1i * b1i, pi = a1r * b1i - a1i * b1r; // p = conj(a1) b1
     const T qr = a3r * c1r - a3i * c1i, qi = a3r * c1i + a3i * c1r; // q = a3 c1
