@@ -54,6 +54,10 @@ def build(force=False, verbose=False):
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_input():
         return LIB
     os.makedirs(OBJDIR, exist_ok=True)
+    keep = {os.path.basename(src)[:-3] for src in sources()}
+    for f in os.listdir(OBJDIR):  # objects of sources that no longer exist
+        if f.split(".")[0] not in keep:
+            os.remove(os.path.join(OBJDIR, f))
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as pool:
         objs = list(pool.map(_compile, sources()))
     cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB, *objs, "-lcudart"]

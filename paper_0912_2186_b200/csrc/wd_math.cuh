@@ -101,7 +101,7 @@ __device__ __forceinline__ void su3_dag_mul(const T (&u)[18], const T (&h)[12], 
 // for 60 % of the kernel's floating-point instructions.  Same products, same summation order per
 // lane as the scalar code above.  Opt-in per translation unit (#define WD_USE_F32X2 before this
 // header): measured on B200 it helps the cp.async-staged kernel, whose limit is issue slots, and
-// slows the latency-bound site and tile kernels (profiles/r01_stage_ncu.md).
+// slows the latency-bound site kernel (profiles/r01_tile_stage_ncu.md).
 #ifdef WD_USE_F32X2
 __device__ __forceinline__ unsigned long long f2_pack(float lo, float hi)
 {
