@@ -508,6 +508,9 @@ def run_wd(args):
         secondary = [
             secondary_leg(binding, torch, dev, stream, local, "c4_32x64_fp32_24rhs", U, 18, 24, 2, 10),
             secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp64", U, 18, 1, 2, 25),
+            # configs 3 and 4 "18 (primary; also report 12)"
+            secondary_leg(binding, torch, dev, stream, local, "c4_32x64_fp32_24rhs", U, 12, 24, 2, 10),
+            secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp64", U, 12, 1, 2, 25),
             # storage variants of the paper's Table 2: 12 and 8 reals per link, half-precision storage
             secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp32", U, 12, 1, 2, 50),
             secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp32", U, 8, 1, 2, 50),
