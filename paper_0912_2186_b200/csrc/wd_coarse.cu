@@ -37,15 +37,6 @@ namespace {
 
 constexpr int TB = 256; // 4^4 sites per block
 
-// block coordinates / lexicographic site of local site `ls` (x fastest) of block b
-struct BlockGeom {
-    int Lx, Ly, Lz, Lt, nbx, nby, nbz, nbt;
-    __host__ __device__ BlockGeom(const int d[4])
-        : Lx(d[0]), Ly(d[1]), Lz(d[2]), Lt(d[3]), nbx(d[0] / 4), nby(d[1] / 4), nbz(d[2] / 4), nbt(d[3] / 4)
-    {
-    }
-};
-
 // g = gamma_MU t (DeGrand-Rossi, wd_math.cuh header): t, g are [spin][colour][re,im]
 template <typename T> __device__ __forceinline__ void gamma_mul(int mu, const T (&t)[24], T (&g)[24])
 {
@@ -101,9 +92,12 @@ coarse_build_kernel(T *__restrict__ S, T *__restrict__ part, const T *__restrict
                     int Ly, int Lz, int Lt, long long V, int nv, T cdiag, int CS)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T *Wb = reinterpret_cast<T *>(smem_raw); // [CS][24][nv]
-    T *Tb = Wb + (size_t)CS * 24 * nv;
-    T *Gb = Tb + (size_t)CS * 24 * nv;
+    // [CS][24][nv] with the site pitch padded by one word: phase 1 writes with lanes = sites (32 different site slots,
+    // same vector), and a pitch of 24 nv words would put all 32 lanes in one bank
+    const int pitch = 24 * nv + 1;
+    T *Wb = reinterpret_cast<T *>(smem_raw);
+    T *Tb = Wb + (size_t)CS * pitch;
+    T *Gb = Tb + (size_t)CS * pitch;
     const int d = blockIdx.x;
     const long long b = blockIdx.y;
     const int n = 2 * nv;
@@ -115,15 +109,20 @@ coarse_build_kernel(T *__restrict__ S, T *__restrict__ part, const T *__restrict
     const long long stride = 24 * padded_volume(V);
     const int tid = threadIdx.x;
 
-    // pairs (alpha, alpha') of this thread: p = tid + 256 * q, q < NP
-    constexpr int NP = 4; // up to 1024 pairs: nv <= 32
-    double acc[NP][2][8]; // [pair][0 = leaves the block, 1 = stays inside][ (s,s') 00, 11 (from t), 01, 10 (from g) : re, im ]
+    // work items of phase 2: (pair of rows alpha = 2 ia, 2 ia + 1; column alpha'), item p = tid + 256 * q, q < NP.  The
+    // hopped vector t, g of column alpha' is read from shared memory once for both rows (the phase is bound by
+    // shared-memory bandwidth: 48 words of t, g per 96 FMAs with one row per thread, 48 per 192 with two).
+    constexpr int NP = 2; // up to 512 items: nv <= 32
+    const int npair = ((nv + 1) / 2) * nv;
+    double acc[NP][2][2][8]; // [item][row 0/1][0 = leaves the block, 1 = stays inside][(s,s') 00, 11 (from t), 01, 10 (from g): re, im]
 #pragma unroll
     for (int q = 0; q < NP; ++q)
 #pragma unroll
-        for (int e = 0; e < 2; ++e)
+        for (int r = 0; r < 2; ++r)
 #pragma unroll
-            for (int i = 0; i < 8; ++i) acc[q][e][i] = 0.0;
+            for (int e = 0; e < 2; ++e)
+#pragma unroll
+                for (int i = 0; i < 8; ++i) acc[q][r][e][i] = 0.0;
 
     for (int c0 = 0; c0 < TB; c0 += CS) {
         __syncthreads(); // the previous chunk's buffers have been consumed
@@ -155,44 +154,53 @@ coarse_build_kernel(T *__restrict__ S, T *__restrict__ part, const T *__restrict
             const int sl = w % CS;
 #pragma unroll
             for (int i = 0; i < 24; ++i) {
-                Wb[((size_t)sl * 24 + i) * nv + a] = own[i];
-                Tb[((size_t)sl * 24 + i) * nv + a] = tt[i];
-                Gb[((size_t)sl * 24 + i) * nv + a] = gg[i];
+                Wb[(size_t)sl * pitch + i * nv + a] = own[i];
+                Tb[(size_t)sl * pitch + i * nv + a] = tt[i];
+                Gb[(size_t)sl * pitch + i * nv + a] = gg[i];
             }
         }
         __syncthreads();
-        // ---- phase 2: (alpha, alpha') pairs ----
+        // ---- phase 2: (two rows alpha, column alpha') items ----
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
             const int p = tid + TB * q;
-            if (p < nv * nv) {
-                const int a = p / nv, ap = p - a * nv;
+            if (p < npair) {
+                const int ia = p / nv, ap = p - ia * nv;
+                const int a0 = 2 * ia, a1 = (2 * ia + 1 < nv) ? 2 * ia + 1 : a0; // (odd nv: the last item redoes row a0, not stored)
                 for (int sl = 0; sl < CS; ++sl) {
                     const int ls = c0 + sl;
                     const int lc = mu == 0 ? (ls & 3) : mu == 1 ? ((ls >> 2) & 3) : mu == 2 ? ((ls >> 4) & 3) : (ls >> 6);
                     const int stays = (d == 0) ? 1 : (fwd ? (lc != 3) : (lc != 0));
-                    const T *wv = Wb + (size_t)sl * 24 * nv + a, *tv = Tb + (size_t)sl * 24 * nv + ap, *gv = Gb + (size_t)sl * 24 * nv + ap;
-                    T dsum[8];
+                    const T *w0 = Wb + (size_t)sl * pitch + a0, *w1 = Wb + (size_t)sl * pitch + a1;
+                    const T *tv = Tb + (size_t)sl * pitch + ap, *gv = Gb + (size_t)sl * pitch + ap;
+                    T ds0[8], ds1[8];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) dsum[i] = (T)0;
+                    for (int i = 0; i < 8; ++i) ds0[i] = ds1[i] = (T)0;
 #pragma unroll
                     for (int s = 0; s < 2; ++s)
 #pragma unroll
                         for (int i = 0; i < 6; ++i) {
                             const int k = s * 12 + 2 * i;
-                            const T wr = wv[(size_t)k * nv], wi = wv[(size_t)(k + 1) * nv];
                             const T tr = tv[(size_t)k * nv], ti = tv[(size_t)(k + 1) * nv];
                             const T gr = gv[(size_t)k * nv], gi = gv[(size_t)(k + 1) * nv];
-                            dsum[2 * s] += wr * tr + wi * ti;     // conj(w) t
-                            dsum[2 * s + 1] += wr * ti - wi * tr;
-                            dsum[4 + 2 * s] += wr * gr + wi * gi; // conj(w) g
-                            dsum[4 + 2 * s + 1] += wr * gi - wi * gr;
+                            const T xr = w0[(size_t)k * nv], xi = w0[(size_t)(k + 1) * nv];
+                            const T yr = w1[(size_t)k * nv], yi = w1[(size_t)(k + 1) * nv];
+                            ds0[2 * s] += xr * tr + xi * ti;     // conj(w) t
+                            ds0[2 * s + 1] += xr * ti - xi * tr;
+                            ds0[4 + 2 * s] += xr * gr + xi * gi; // conj(w) g
+                            ds0[4 + 2 * s + 1] += xr * gi - xi * gr;
+                            ds1[2 * s] += yr * tr + yi * ti;
+                            ds1[2 * s + 1] += yr * ti - yi * tr;
+                            ds1[4 + 2 * s] += yr * gr + yi * gi;
+                            ds1[4 + 2 * s + 1] += yr * gi - yi * gr;
                         }
                     const double m1 = stays ? 1.0 : 0.0, m0 = 1.0 - m1; // (no dynamic index into the register array)
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
-                        acc[q][0][i] = fma(m0, (double)dsum[i], acc[q][0][i]);
-                        acc[q][1][i] = fma(m1, (double)dsum[i], acc[q][1][i]);
+                        acc[q][0][0][i] = fma(m0, (double)ds0[i], acc[q][0][0][i]);
+                        acc[q][0][1][i] = fma(m1, (double)ds0[i], acc[q][0][1][i]);
+                        acc[q][1][0][i] = fma(m0, (double)ds1[i], acc[q][1][0][i]);
+                        acc[q][1][1][i] = fma(m1, (double)ds1[i], acc[q][1][1][i]);
                     }
                 }
             }
@@ -204,22 +212,28 @@ coarse_build_kernel(T *__restrict__ S, T *__restrict__ part, const T *__restrict
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
         const int p = tid + TB * q;
-        if (p < nv * nv) {
-            const int a = p / nv, ap = p - a * nv;
+        if (p < npair) {
+            const int ia = p / nv, ap = p - ia * nv;
 #pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                T *dst = e == 0 ? (d == 0 ? nullptr : S + ((b * 9 + d) * (long long)n * n) * 2)
-                                : part + ((b * 9 + d) * (long long)n * n) * 2;
-                if (!dst) continue;
+            for (int r = 0; r < 2; ++r) {
+                const int a = 2 * ia + r;
+                if (a >= nv) continue;
 #pragma unroll
-                for (int s = 0; s < 2; ++s) {
-                    const int row = s * nv + a;
-                    // (s, s): from t ; (s, 1-s): from g (rows in s, source chirality 1-s)
-                    const long long i0 = (((long long)(s * nv + ap)) * n + row) * 2, i1 = (((long long)((1 - s) * nv + ap)) * n + row) * 2;
-                    dst[i0] = (T)(ct * acc[q][e][2 * s]);
-                    dst[i0 + 1] = (T)(ct * acc[q][e][2 * s + 1]);
-                    dst[i1] = (T)(cg * acc[q][e][4 + 2 * s]);
-                    dst[i1 + 1] = (T)(cg * acc[q][e][4 + 2 * s + 1]);
+                for (int e = 0; e < 2; ++e) {
+                    T *dst = e == 0 ? (d == 0 ? nullptr : S + ((b * 9 + d) * (long long)n * n) * 2)
+                                    : part + ((b * 9 + d) * (long long)n * n) * 2;
+                    if (!dst) continue;
+#pragma unroll
+                    for (int s = 0; s < 2; ++s) {
+                        const int row = s * nv + a;
+                        // (s, s): from t ; (s, 1-s): from g (rows in s, source chirality 1-s)
+                        const long long i0 = (((long long)(s * nv + ap)) * n + row) * 2,
+                                        i1 = (((long long)((1 - s) * nv + ap)) * n + row) * 2;
+                        dst[i0] = (T)(ct * acc[q][r][e][2 * s]);
+                        dst[i0 + 1] = (T)(ct * acc[q][r][e][2 * s + 1]);
+                        dst[i1] = (T)(cg * acc[q][r][e][4 + 2 * s]);
+                        dst[i1 + 1] = (T)(cg * acc[q][r][e][4 + 2 * s + 1]);
+                    }
                 }
             }
         }
@@ -312,23 +326,20 @@ cudaError_t build_t(void *S, void *part, const void *W, const void *links, const
                     cudaStream_t s)
 {
     const long long nblocks = V / TB;
-    if (nblocks < 1 || nblocks > 65535 * 1024LL || nv < 1 || nv > 32) return cudaErrorInvalidConfiguration;
+    if (nblocks < 1 || nv < 1 || nv > 32) return cudaErrorInvalidConfiguration;
     int CS = 32;
-    while (CS > 1 && (size_t)3 * CS * 24 * nv * sizeof(T) > 200 * 1024) CS >>= 1;
-    const size_t smem = (size_t)3 * CS * 24 * nv * sizeof(T);
+    while (CS > 1 && (size_t)3 * CS * (24 * nv + 1) * sizeof(T) > 200 * 1024) CS >>= 1;
+    const size_t smem = (size_t)3 * CS * (24 * nv + 1) * sizeof(T);
     auto kern = coarse_build_kernel<T, RECON>;
     static size_t smem_set[64];
     cudaError_t e = ensure_dynamic_smem((const void *)kern, smem, smem_set);
     if (e != cudaSuccess) return e;
-    // gridDim.y is limited to 65535: fold larger block counts over several launches
+    // gridDim.y is limited to 65535 blocks = 16.7 M sites (checked by wd_build_coarse)
     const int n = 2 * nv;
-    for (long long b0 = 0; b0 < nblocks; b0 += 65535) {
-        const unsigned nb = (unsigned)((nblocks - b0 < 65535) ? nblocks - b0 : 65535);
-        if (b0 != 0) return cudaErrorInvalidConfiguration; // (lattices beyond 65535 blocks = 16.7 M sites: not needed yet)
-        kern<<<dim3(9, nb), TB, smem, s>>>((T *)S, (T *)part, (const T *)W, (const T *)links, dims[0], dims[1], dims[2], dims[3],
-                                          V, nv, (T)(4.0 + mass), CS);
-        count_launch();
-    }
+    if (nblocks > 65535) return cudaErrorInvalidConfiguration;
+    kern<<<dim3(9, (unsigned)nblocks), TB, smem, s>>>((T *)S, (T *)part, (const T *)W, (const T *)links, dims[0], dims[1], dims[2],
+                                                     dims[3], V, nv, (T)(4.0 + mass), CS);
+    count_launch();
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     const long long tot = nblocks * n * n * 2;
     coarse_sum_kernel<T><<<(unsigned)((tot + 255) / 256), 256, 0, s>>>((T *)S, (const T *)part, nblocks, n);
