@@ -325,6 +325,7 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         }
     }
 
+    float psi[24]; // own spinor of the current slice: read from the slice buffer once (as the t+1 neighbour), then carried
     for (int t = t_begin; t < t_end; ++t) {
         const long long toff = (long long)t * S3;
         const long long toff_n = (long long)(t + 1 == Lt ? 0 : t + 1) * S3;
@@ -340,8 +341,8 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         cpa_commit(); // c1
 
         const float4 *pl = plane0 + cur * plane_sz;
-        float acc[24], psi[24], u[18], pn[24];
-        lds_vecs<6>(pl, nt, tid, psi);
+        float acc[24], u[18], pn[24], pnx[24];
+        if (t == t_begin) lds_vecs<6>(pl, nt, tid, psi);
 #pragma unroll
         for (int i = 0; i < 24; ++i) acc[i] = 0.f;
         reconstruct_add<3, +1>(acc, chi_t); // backward t hop, product carried from the previous slice
@@ -409,14 +410,14 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         // ---- t: forward hop now, backward product for the next slice ----
         {
             float h[12];
-            lds_vecs<6>(plane0 + (cur ^ 1) * plane_sz, nt, tid, pn);
+            lds_vecs<6>(plane0 + (cur ^ 1) * plane_sz, nt, tid, pnx);
             if (unit_t(t)) { // U_t(x,t) = 1: projection and reconstruction only
-                project<3, -1>(pn, h);
+                project<3, -1>(pnx, h);
                 reconstruct_add<3, -1>(acc, h);
                 project<3, +1>(psi, chi_t);
             } else {
                 own_link_rd<3, RECON, BULK>(lnk, nts, st, u);
-                hop_forward<3>(acc, u, pn);
+                hop_forward<3>(acc, u, pnx);
                 project<3, +1>(psi, h);
                 su3_dag_mul(u, h, chi_t);
             }
@@ -429,6 +430,8 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
 #pragma unroll
             for (int c = 0; c < 6; ++c) q[c * BLK] = make_float4(psi[4 * c], psi[4 * c + 1], psi[4 * c + 2], psi[4 * c + 3]);
         }
+#pragma unroll
+        for (int i = 0; i < 24; ++i) psi[i] = pnx[i]; // the spinor of slice t+1 is the next step's own spinor
         cur ^= 1;
     }
     cpa_wait<0>();
