@@ -379,11 +379,25 @@ def run_wd_device_inputs(args, torch, binding, cfg, recon, nrhs, dev, local, ker
     for _ in range(max(args.warmup, 3) * aps):
         op.apply(outs[0], ins[0], cfg.mass, nrhs)
     torch.cuda.synchronize()
+    graph = None
+    if args.graph:  # the step captured once in a CUDA graph and replayed: takes the host's launch rate out of the number
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            for i in range(aps):
+                op.apply(outs[i % nbuf], ins[i % nbuf], cfg.mass, nrhs)
+        with torch.cuda.stream(stream):
+            graph.replay()
+        torch.cuda.synchronize()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local) as clocks:
         ev0.record(stream)
-        for i in range(args.steps * aps):
-            op.apply(outs[i % nbuf], ins[i % nbuf], cfg.mass, nrhs)
+        if graph is not None:
+            with torch.cuda.stream(stream):
+                for _ in range(args.steps):
+                    graph.replay()
+        else:
+            for i in range(args.steps * aps):
+                op.apply(outs[i % nbuf], ins[i % nbuf], cfg.mass, nrhs)
         ev1.record(stream)
         torch.cuda.synchronize()
     ms = ev0.elapsed_time(ev1) / (args.steps * aps)
@@ -849,6 +863,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--device-inputs", action="store_true",
                     help="timing-only quick mode for kernel work: device-drawn random links and spinors, no e2e/oracle legs")
+    ap.add_argument("--graph", action="store_true",
+                    help="(with --device-inputs) capture the step of APPLIES wd_apply launches in a CUDA graph and time its replays")
     ap.add_argument("--half", action="store_true", help="(with --device-inputs) half-precision storage, fp32 arithmetic")
     ap.add_argument("--no-secondary", action="store_true",
                     help="skip the short legs for configs[4] (24 RHS) and configs[3] in fp64 that the default run adds")

@@ -349,6 +349,9 @@ class WilsonDirac:
         self.gauge = None
         self.gauge = wd_load_gauge(self.lat, links_canonical_dev, self.precision, self.recon, stream)
         self.volume = wd_lattice_volume(self.lat)
+        self._cdims = _dims(self.dims)          # marshalled once: wd_apply is called in launch-bound loops
+        self._apply = lib().wd_apply
+        self._apply_dagger = lib().wd_apply_dagger
         if kernel != WD_KERNEL_AUTO:
             wd_set_kernel(self.gauge, kernel)
 
@@ -376,7 +379,9 @@ class WilsonDirac:
         return KERNEL_NAMES[wd_selected_kernel(self.gauge, nrhs)]
 
     def apply_dagger(self, out_native_dev, in_native_dev, mass, nrhs=1):
-        wd_apply_dagger(out_native_dev, in_native_dev, self.gauge, mass, self.dims, nrhs, self.precision)
+        rc = self._apply_dagger(_ptr(out_native_dev), _ptr(in_native_dev), self.gauge, mass, self._cdims, nrhs, self.precision)
+        if rc != WD_OK:
+            _check(rc, "wd_apply_dagger")
 
     def native_numel(self, nrhs=1):
         """Elements (float16 / float32 / float64 by precision) of a NATIVE spinor buffer of nrhs fields (the volume is
@@ -384,7 +389,9 @@ class WilsonDirac:
         return wd_spinor_bytes(self.lat, nrhs, self.precision) // {16: 2, 32: 4, 64: 8}[self.precision]
 
     def apply(self, out_native_dev, in_native_dev, mass, nrhs=1):
-        wd_apply(out_native_dev, in_native_dev, self.gauge, mass, self.dims, nrhs, self.precision)
+        rc = self._apply(_ptr(out_native_dev), _ptr(in_native_dev), self.gauge, mass, self._cdims, nrhs, self.precision)
+        if rc != WD_OK:
+            _check(rc, "wd_apply")
 
     # ---- red/black (even-odd) blocks: half fields of one parity ----
     def half_numel(self, nrhs=1):
