@@ -492,3 +492,42 @@ def test_kernels_write_only_their_output(dims, precision, recon, nrhs, kernel):
         assert bool(torch.isfinite(out).all())
         assert not bool((out.view(torch.uint8) == 0x5A).all(dim=-1).any())   # no site left at the fill pattern
     op.close()
+
+
+# ---------------------------------------------------------------- a lattice beyond 2^31 bytes per field: sampled outputs
+def test_large_lattice_sampled_against_the_oracle(oracle):
+    """32 x 48 x 72 x 64 (7.1 M sites: the link field is 2.0 GB, byte offsets beyond 2^31; 864 tile columns):
+    the staged kernel on analytic SU(3) links (cheap to generate: a colour rotation with site-dependent angle and phases)
+    and Gaussian spinors, compared with the oracle on runs of consecutive sites taken at the start, the middle, around a
+    time-slice boundary and at the very end of the lattice."""
+    import torch
+    dims = (32, 48, 72, 64)
+    Lx, Ly, Lz, Lt = dims
+    V = fields.volume(dims)
+    t, z, y, x = np.meshgrid(np.arange(Lt, dtype=np.float32), np.arange(Lz, dtype=np.float32), np.arange(Ly, dtype=np.float32),
+                             np.arange(Lx, dtype=np.float32), indexing="ij", sparse=True)
+    U = np.zeros((4, Lt, Lz, Ly, Lx, 3, 3, 2), dtype=np.float32)
+    for mu in range(4):
+        phi = 0.37 * x + 0.11 * y * (mu + 1) + 0.23 * z + 0.05 * t + 0.7 * mu
+        al = 0.19 * x * y + 0.31 * t + mu
+        be = 0.13 * z * x + 0.29 * y - mu
+        c, s = np.cos(phi), np.sin(phi)
+        U[mu, ..., 0, 0, 0], U[mu, ..., 0, 0, 1] = c * np.cos(al), c * np.sin(al)
+        U[mu, ..., 0, 1, 0], U[mu, ..., 0, 1, 1] = s * np.cos(be), s * np.sin(be)
+        U[mu, ..., 1, 0, 0], U[mu, ..., 1, 0, 1] = -s * np.cos(be), s * np.sin(be)
+        U[mu, ..., 1, 1, 0], U[mu, ..., 1, 1, 1] = c * np.cos(al), -c * np.sin(al)
+        U[mu, ..., 2, 2, 0] = 1.0
+    rng = np.random.default_rng(131)
+    psi = rng.standard_normal((1, Lt, Lz, Ly, Lx, 4, 3, 2), dtype=np.float32)
+    mass = -0.4
+    op = GpuOp(U, dims, 32, 18, KERNELS["auto"])
+    assert op.op.selected_kernel(1) == "stage"
+    got = op.apply(psi, mass)[0].reshape(V, 4, 3, 2)
+    op.close()
+    U64 = U.astype(np.float64)
+    p64 = psi[0].astype(np.float64)
+    S3 = Lx * Ly * Lz
+    for begin in (0, V // 2 - 777, 17 * S3 - 300, V - 600):
+        end = begin + 600
+        want = oracle.apply_range(p64, U64, dims, mass, begin, end)
+        assert rel_l2(got[begin:end], want) <= TOL[32], begin
