@@ -682,7 +682,18 @@ def run_cgnr(args):
         op.pack_parity(b, canon, 1, 0)
     stream.synchronize()
     iters = args.applies_per_step
+    nblk = args.nrhs or 1   # --op cgnr --nrhs N: the block solve (N right-hand sides in lock step, batched operator applies)
+    if nblk > 1:
+        if args.op != "cgnr":
+            raise SystemExit("bench.py: --nrhs with --op is the block CGNR only")
+        with torch.cuda.stream(stream):
+            g = torch.Generator(device=dev).manual_seed(cfg.seed + 1000)
+            b = torch.randn(n * nblk, dtype=tdt, device=dev, generator=g)   # native half fields: any values are valid vectors
+            x = torch.empty_like(b)
+        stream.synchronize()
     solve = {"cgnr": op.cgnr_schur, "bicgstab": op.bicgstab_schur, "gcr": op.gcr_schur}[args.op]
+    if nblk > 1:
+        solve = lambda xx, bb, mass, parity, it: op.cgnr_schur_block(xx, bb, mass, parity, nblk, it)
     # BLAS-1 flops / spinor passes per iteration and even site; matvecs per iteration.  GCR(8): averages over a cycle
     # (3.5 Gram-Schmidt steps of 2 + 6 passes each, plus the copy, the <q,r> dot and the x/r update)
     blas_flops, blas_passes, nmv = {"cgnr": (288, 9, 2), "bicgstab": (672, 19, 2), "gcr": (1150, 38, 1)}[args.op]
@@ -699,15 +710,18 @@ def run_cgnr(args):
         torch.cuda.synchronize()
     ms = ev0.elapsed_time(ev1)
     total_iters = args.steps * iters
-    flops_it = (nmv * (2 * 1320 + 48) + blas_flops) * (V // 2)
-    bytes_it = (V // 2) * (nmv * (2 * 2 * 4 * recon * w + 5 * 24 * w) + blas_passes * 24 * w)
+    flops_it = (nmv * (2 * 1320 + 48) + blas_flops) * (V // 2) * nblk
+    # (block solve: the links are read once per batched launch, the spinor passes scale with the right-hand sides)
+    bytes_it = (V // 2) * (nmv * (2 * 2 * 4 * recon * w + nblk * 5 * 24 * w) + nblk * blas_passes * 24 * w)
+    if nblk > 1:
+        hist = hist[0]
     peak, peak_src = measured_peak()
     achieved = bytes_it * total_iters / (ms * 1e-3) / 1e9
     line = {"metric": "wilson_%s_gflops" % args.op, "value": total_iters * flops_it / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32" if cfg.precision == 32 else "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "op": {"cgnr": "CGNR", "bicgstab": "BiCGstab", "gcr": "GCR(8)"}[args.op] + " on the even-odd preconditioned operator", "dims": list(cfg.dims),
-                       "recon": recon, "mass": cfg.mass, "iterations_per_step": iters,
+                       "recon": recon, "mass": cfg.mass, "iterations_per_step": iters, "nrhs": nblk,
                        "relative_residual_after_step": hist[-1],
                        "l2": "inputs larger than L2 (gauge + five half fields), no flush"},
             "us_per_iteration": ms / total_iters * 1e3, "clocks": clocks.summary(),

@@ -247,6 +247,16 @@ int wd_apply_schur_dagger(void *out_half_dev, const void *in_half_dev, void *tmp
 int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4],
                   int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host);
 
+/* wd_cgnr_schur_block -- the same CGNR for nrhs right-hand sides at once (the set-up and the propagator calculation solve
+ * for many sources with the same links): x and b hold nrhs native half fields, the iterations advance in
+ * lock step, every operator application is ONE batched launch pair in which a block of links serves all right-hand
+ * sides, every right-hand side has its own scalars.  Per right-hand side the arithmetic is that of wd_cgnr_schur with
+ * tol = 0 (bit-identical iterates).  tol > 0 stops when EVERY right-hand side's recursive residual is <= tol * |b_r|
+ * (no true-residual restarts here).  hist_host: HOST, nrhs * (max_iter + 1) doubles, row r = history of right-hand side r.
+ * Workspace 5 * nrhs half fields in the gauge handle. */
+int wd_cgnr_schur_block(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4], int nrhs,
+                        int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host);
+
 /* wd_bicgstab_schur -- BiCGstab (van der Vorst) for Mhat x = b, x_0 = 0: the paper's other solver around the
  * even-odd matvec (Table 2).  Same arguments, execution model and workspace as wd_cgnr_schur;
  * one iteration = two Mhat applications; complex inner products summed deterministically in fp64. */

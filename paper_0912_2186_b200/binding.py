@@ -24,7 +24,7 @@ STATUS_NAMES = {
 SYMBOLS = (
     "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
     "wd_set_kernel", "wd_set_tuning", "wd_set_temporal_gauge", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
-    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_gcr_schur_precond", "wd_coarse_reals", "wd_coarse_stencil_reals", "wd_build_coarse", "wd_apply_coarse",
+    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_gcr_schur_precond", "wd_cgnr_schur_block", "wd_coarse_reals", "wd_coarse_stencil_reals", "wd_build_coarse", "wd_apply_coarse",
     "wd_block_orthonormalise", "wd_restrict", "wd_prolong", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_dagger", "wd_apply_host",
     "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
 )
@@ -273,6 +273,21 @@ def wd_gcr_schur(x_half_dev, b_half_dev, gauge, mass, dims, precision, parity, m
     return it.value, [hist[i] for i in range(it.value + 1)]
 
 
+def wd_cgnr_schur_block(x_half_dev, b_half_dev, gauge, mass, dims, nrhs, precision, parity, max_iter, tol=0.0):
+    """Returns (iterations done, [history of right-hand side r as a list of floats for r < nrhs])."""
+    it = ctypes.c_int(0)
+    hs = int(max_iter) + 1
+    hist = (ctypes.c_double * (int(nrhs) * hs))()
+    fn = lib().wd_cgnr_schur_block
+    fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_double, ctypes.POINTER(ctypes.c_int), ctypes.c_int,
+                   ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.POINTER(ctypes.c_int),
+                   ctypes.POINTER(ctypes.c_double)]
+    fn.restype = ctypes.c_int
+    _check(fn(_ptr(x_half_dev), _ptr(b_half_dev), gauge, float(mass), _dims(dims), int(nrhs), int(precision), int(parity),
+              int(max_iter), float(tol), ctypes.byref(it), hist), "wd_cgnr_schur_block")
+    return it.value, [[hist[r * hs + i] for i in range(it.value + 1)] for r in range(int(nrhs))]
+
+
 PRECOND_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p)
 
 
@@ -424,6 +439,9 @@ class WilsonDirac:
     def gcr_schur(self, x_half_dev, b_half_dev, mass, parity, max_iter, restart=8, tol=0.0):
         return wd_gcr_schur(x_half_dev, b_half_dev, self.gauge, mass, self.dims, self.precision, parity, max_iter, restart,
                             tol)
+
+    def cgnr_schur_block(self, x_half_dev, b_half_dev, mass, parity, nrhs, max_iter, tol=0.0):
+        return wd_cgnr_schur_block(x_half_dev, b_half_dev, self.gauge, mass, self.dims, nrhs, self.precision, parity, max_iter, tol)
 
     def gcr_schur_precond(self, x_half_dev, b_half_dev, mass, parity, max_iter, restart, tol, precond):
         return wd_gcr_schur_precond(x_half_dev, b_half_dev, self.gauge, mass, self.dims, self.precision, parity, max_iter,

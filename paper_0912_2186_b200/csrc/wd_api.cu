@@ -698,6 +698,23 @@ int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, dou
     return WD_OK;
 }
 
+int wd_cgnr_schur_block(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4], int nrhs,
+                        int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host)
+{
+    int rc = check_eo_args("wd_cgnr_schur_block", x_half_dev, b_half_dev, gauge, dims, nrhs, precision, parity);
+    if (rc) return rc;
+    if (max_iter < 0 || tol < 0.0) return fail(WD_ERR_MISMATCH, "wd_cgnr_schur_block: max_iter=%d tol=%g", max_iter, tol);
+    if (4.0 + mass == 0.0) return fail(WD_ERR_MISMATCH, "wd_cgnr_schur_block: 4 + mass = 0");
+    wd::ApplyArgs a = shape_args(gauge, 1);
+    a.links = gauge->links;
+    a.stream = gauge->stream;
+    cudaError_t e = cudaSuccess;
+    if (wd::cgnr_schur_block(gauge, a, x_half_dev, b_half_dev, mass, parity, nrhs, max_iter, tol, iters_out, hist_host, &e))
+        return e == cudaErrorMemoryAllocation ? fail(WD_ERR_ALLOC, "wd_cgnr_schur_block: workspace allocation failed")
+                                              : cuda_fail(e, "wd_cgnr_schur_block");
+    return WD_OK;
+}
+
 int wd_bicgstab_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4],
                       int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host)
 {

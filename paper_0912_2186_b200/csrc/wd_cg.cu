@@ -13,6 +13,7 @@
 // residual history back every CHECK iterations when a tolerance is set.
 #include <cmath>
 #include <cstdio>
+#include <vector>
 #include "wd_internal.h"
 #include "wd_layout.cuh"
 
@@ -81,8 +82,11 @@ template <int NCH> __device__ __forceinline__ bool real_site(long long i, long l
 
 // part[b] = sum over this CTA's grid-stride share of |v|^2
 template <typename Vec, int NCH>
-__global__ void __launch_bounds__(RED_THREADS) norm2_kernel(const Vec *__restrict__ v, long long nvec, long long Vh, double *part)
+__global__ void __launch_bounds__(RED_THREADS) norm2_kernel(const Vec *v, long long nvec, long long Vh, double *part)
 {
+    // blockIdx.y = right-hand side of a block solve (fields nvec apart, partials RED_BLOCKS apart); 0 for one right-hand side
+    v += (long long)blockIdx.y * nvec;
+    part += (long long)blockIdx.y * RED_BLOCKS;
     __shared__ double sh[RED_THREADS / 32];
     double s = 0.0;
     constexpr int UNR = 4;
@@ -103,9 +107,14 @@ __global__ void __launch_bounds__(RED_THREADS) norm2_kernel(const Vec *__restric
 // alpha = zz / ww;  x += alpha p;  r -= alpha w;  rr_part = |r|^2 partials
 template <typename Vec, int NCH>
 __global__ void __launch_bounds__(RED_THREADS)
-update_xr_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict__ p, const Vec *__restrict__ w, long long nvec,
-                 long long Vh, const double *zz_part, const double *ww_part, int npart, double *rr_part)
+update_xr_kernel(Vec *x, Vec *r, const Vec *p, const Vec *w, long long nvec, long long Vh, const double *zz_part,
+                 const double *ww_part, int npart, double *rr_part)
 {
+    {   // blockIdx.y = right-hand side of a block solve
+        const long long rhs = blockIdx.y;
+        x += rhs * nvec; r += rhs * nvec; p += rhs * nvec; w += rhs * nvec;
+        zz_part += rhs * npart; ww_part += rhs * npart; rr_part += rhs * RED_BLOCKS;
+    }
     __shared__ double sh[RED_THREADS / 32];
     const double alpha = safe_div(sum_partials(zz_part, npart), sum_partials(ww_part, npart));
     double s = 0.0;
@@ -136,9 +145,14 @@ update_xr_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict
 // beta = zz_new / zz_old;  p = z + beta p;  hist[k] = sqrt(rr) (block 0)
 template <typename Vec>
 __global__ void __launch_bounds__(RED_THREADS)
-update_p_kernel(Vec *__restrict__ p, const Vec *__restrict__ z, long long nvec, const double *zz_new_part, const double *zz_old_part,
-                int npart, const double *rr_part, double *hist_k)
+update_p_kernel(Vec *p, const Vec *z, long long nvec, const double *zz_new_part, const double *zz_old_part,
+                int npart, const double *rr_part, double *hist_k, long long hist_stride = 0)
 {
+    {   // blockIdx.y = right-hand side of a block solve
+        const long long rhs = blockIdx.y;
+        p += rhs * nvec; z += rhs * nvec;
+        zz_new_part += rhs * npart; zz_old_part += rhs * npart; rr_part += rhs * RED_BLOCKS; hist_k += rhs * hist_stride;
+    }
     const double beta = safe_div(sum_partials(zz_new_part, npart), sum_partials(zz_old_part, npart));
     if (blockIdx.x == 0) { // (block-uniform branch: sum_partials has barriers)
         const double rr = sum_partials(rr_part);
@@ -167,8 +181,10 @@ __global__ void __launch_bounds__(RED_THREADS) zero_kernel(Vec *__restrict__ v, 
     for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) v[i] = Vec{};
 }
 
-__global__ void sqrt_of_sum_kernel(const double *part, double *out) // one CTA of 32 threads
+__global__ void sqrt_of_sum_kernel(const double *part, double *out, long long out_stride = 0) // one CTA of 32 threads per RHS
 {
+    part += (long long)blockIdx.x * RED_BLOCKS;
+    out += (long long)blockIdx.x * out_stride;
     const double t = sum_partials(part);
     if (threadIdx.x == 0) *out = sqrt(t);
 }
@@ -311,33 +327,41 @@ __global__ void bicg_init_kernel(cplxd *scal)
 
 static cudaError_t ensure_workspace(wd_gauge *g, size_t ws_bytes, size_t nsc);
 
+// nrhs right-hand sides advance in lock step (a block solve): every vector kernel gets a right-hand-side dimension
+// (gridDim.y), the operator is applied to all of them in one batched launch (dslash_eo with the right-hand side fastest,
+// so a block of links serves all of them), every right-hand side has its own scalars and history.  Per right-hand side the
+// arithmetic and its order are those of the single solve: the results are bit-identical to nrhs separate calls.
 template <typename T>
 static int cgnr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const void *b_in, double mass, int parity, int max_iter,
-                        double tol, int *iters_out, double *hist_host, cudaError_t *err)
+                        double tol, int *iters_out, double *hist_host, cudaError_t *err, int nrhs = 1)
 {
     using SL = SpinorLayout<T>;
     using Vec = typename SL::Vec;
     constexpr int NCH = SL::NCH;
     constexpr int CHECK = 8; // iterations between convergence checks (the only host synchronisations)
     const long long Vh = shape.V / 2;
-    const long long nvec = padded_volume(Vh) * NCH;
-    const size_t hb = (size_t)nvec * sizeof(Vec);
+    const long long nvec = padded_volume(Vh) * NCH;            // vectors per right-hand side
+    const size_t hb = (size_t)nvec * sizeof(Vec) * (size_t)nrhs; // bytes of one block of nrhs half fields
     cudaStream_t s = shape.stream;
     const double a0 = 4.0 + mass;
+    const long long hs = (long long)max_iter + 1; // history entries per right-hand side
 
     // workspace lives in the gauge handle (a 0.5 GB cudaMalloc / cudaFree per solve costs up to a second)
     // |Mhat p|^2 and |Mhat^dag r|^2 come out of the matvec's epilogue as one partial per CTA of that kernel
     const int npart = (int)((Vh + 127) / 128);
-    const size_t nsc = 3 * (size_t)npart + RED_BLOCKS + (size_t)max_iter + 1; // zz_part[2][npart] | ww_part | rr_part | hist
+    const size_t nsc = (size_t)nrhs * (3 * (size_t)npart + RED_BLOCKS + (size_t)hs); // zz_part[2] | ww_part | rr_part | hist
     if ((*err = ensure_workspace(g, 5 * hb, nsc)) != cudaSuccess) return -1;
     char *ws = (char *)g->cg_ws;
     double *sc = g->cg_sc;
     Vec *r = (Vec *)ws, *p = (Vec *)(ws + hb), *z = (Vec *)(ws + 2 * hb), *w = (Vec *)(ws + 3 * hb), *tmp = (Vec *)(ws + 4 * hb);
     Vec *x = (Vec *)x_out;
-    double *zz_part[2] = {sc, sc + npart}, *ww_part = sc + 2 * (size_t)npart, *rr_part = sc + 3 * (size_t)npart;
-    double *hist = rr_part + RED_BLOCKS;
+    const size_t np_all = (size_t)nrhs * npart;
+    double *zz_part[2] = {sc, sc + np_all}, *ww_part = sc + 2 * np_all, *rr_part = sc + 3 * np_all;
+    double *hist = rr_part + (size_t)nrhs * RED_BLOCKS;
+    const dim3 vgrid(RED_BLOCKS, (unsigned)nrhs);
 
     ApplyArgs a = shape;
+    a.nrhs = nrhs;
     // out = Mhat in  or  Mhat^dagger in;  norm_part receives the per-CTA partials of |out|^2
     auto schur = [&](Vec *out, const Vec *in, bool dagger, double *norm_part) -> cudaError_t {
         a.out = tmp;
@@ -348,45 +372,49 @@ static int cgnr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const 
         a.in = tmp;
         return launch_eo(a, in, a0, 0.5 / a0, parity, dagger, norm_part);
     };
-    auto norm2 = [&](const Vec *v, double *part) {
-        norm2_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(v, nvec, Vh, part);
-        count_launch();
-    };
     int rc = 0, k = 0;
-    double h0 = 0.0;
+    std::vector<double> h0(nrhs, 0.0), hk(nrhs, 0.0);
     auto fail_cuda = [&](cudaError_t e) {
         *err = e;
         rc = -1;
     };
+    // entry `col` of every right-hand side's history -> host
+    auto fetch = [&](std::vector<double> &dst, int col) -> cudaError_t {
+        cudaError_t e = cudaMemcpy2DAsync(dst.data(), sizeof(double), hist + col, (size_t)hs * sizeof(double), sizeof(double), nrhs,
+                                          cudaMemcpyDeviceToHost, s);
+        return e == cudaSuccess ? cudaStreamSynchronize(s) : e;
+    };
     do {
         cudaError_t e;
-        zero_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, nvec);
+        zero_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, nvec * nrhs);
         count_launch();
         if ((e = cudaMemcpyAsync(r, b_in, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
         int cur = 0;
         if ((e = schur(z, r, true, zz_part[cur])) != cudaSuccess) { fail_cuda(e); break; }
         if ((e = cudaMemcpyAsync(p, z, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
-        norm2(r, rr_part);
-        sqrt_of_sum_kernel<<<1, 32, 0, s>>>(rr_part, hist);
+        norm2_kernel<Vec, NCH><<<vgrid, RED_THREADS, 0, s>>>(r, nvec, Vh, rr_part);
+        count_launch();
+        sqrt_of_sum_kernel<<<nrhs, 32, 0, s>>>(rr_part, hist, hs);
         count_launch();
         if (tol > 0.0) {
-            if ((e = cudaMemcpyAsync(&h0, hist, sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
-            if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
-            if (h0 == 0.0) break; // b = 0: x = 0 is the solution
+            if ((e = fetch(h0, 0)) != cudaSuccess) { fail_cuda(e); break; }
+            bool all_zero = true;
+            for (double v : h0) all_zero = all_zero && v == 0.0;
+            if (all_zero) break; // b = 0: x = 0 is the solution
         }
         for (k = 0; k < max_iter; ++k) {
             if ((e = schur(w, p, false, ww_part)) != cudaSuccess) { fail_cuda(e); break; }
-            update_xr_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, r, p, w, nvec, Vh, zz_part[cur], ww_part, npart, rr_part);
+            update_xr_kernel<Vec, NCH><<<vgrid, RED_THREADS, 0, s>>>(x, r, p, w, nvec, Vh, zz_part[cur], ww_part, npart, rr_part);
             count_launch();
             if ((e = schur(z, r, true, zz_part[cur ^ 1])) != cudaSuccess) { fail_cuda(e); break; }
-            update_p_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(p, z, nvec, zz_part[cur ^ 1], zz_part[cur], npart, rr_part, hist + k + 1);
+            update_p_kernel<Vec><<<vgrid, RED_THREADS, 0, s>>>(p, z, nvec, zz_part[cur ^ 1], zz_part[cur], npart, rr_part, hist + k + 1, hs);
             count_launch();
             cur ^= 1;
             if (tol > 0.0 && ((k + 1) % CHECK == 0 || k + 1 == max_iter)) {
-                double hk = 0.0;
-                if ((e = cudaMemcpyAsync(&hk, hist + k + 1, sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
-                if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
-                if (hk <= tol * h0) {
+                if ((e = fetch(hk, k + 1)) != cudaSuccess) { fail_cuda(e); break; }
+                bool done = true;
+                for (int i = 0; i < nrhs; ++i) done = done && hk[i] <= tol * h0[i];
+                if (done) {
                     ++k;
                     break;
                 }
@@ -394,14 +422,18 @@ static int cgnr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const 
         }
         if (rc) break;
         if ((e = cudaGetLastError()) != cudaSuccess) { fail_cuda(e); break; }
-        if (hist_host) {
-            if ((e = cudaMemcpyAsync(hist_host, hist, ((size_t)k + 1) * sizeof(double), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { fail_cuda(e); break; }
+        if (hist_host) { // [rhs][max_iter + 1], entries 0..k of every right-hand side
+            e = cudaMemcpy2DAsync(hist_host, (size_t)hs * sizeof(double), hist, (size_t)hs * sizeof(double), ((size_t)k + 1) * sizeof(double),
+                                  nrhs, cudaMemcpyDeviceToHost, s);
+            if (e != cudaSuccess) { fail_cuda(e); break; }
         }
         if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
-        if (hist_host && hist_host[0] > 0.0) {
-            const double n0 = hist_host[0];
-            for (int i = 0; i <= k; ++i) hist_host[i] /= n0; // relative residual |r_k| / |b|
-        }
+        if (hist_host)
+            for (int i = 0; i < nrhs; ++i) {
+                const double n0 = hist_host[(size_t)i * hs];
+                if (n0 > 0.0)
+                    for (int j = 0; j <= k; ++j) hist_host[(size_t)i * hs + j] /= n0; // relative residual |r_k| / |b|
+            }
     } while (false);
     if (iters_out) *iters_out = k;
     return rc;
@@ -796,6 +828,16 @@ static int refined_t(wd_gauge *g, const ApplyArgs &shape, int kind, void *x_out,
     }
     if (iters_out) *iters_out = total;
     return 0;
+}
+
+// block CGNR: nrhs right-hand sides in lock step, one batched operator application per step (no true-residual restarts:
+// the caller gets the recursive history; wd_cgnr_schur on a single right-hand side has the residual control)
+int cgnr_schur_block(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int nrhs, int max_iter,
+                     double tol, int *iters_out, double *hist_host, cudaError_t *err)
+{
+    return shape.precision == 32
+               ? cgnr_schur_t<float>(g, shape, x, b, mass, parity, max_iter, tol, iters_out, hist_host, err, nrhs)
+               : cgnr_schur_t<double>(g, shape, x, b, mass, parity, max_iter, tol, iters_out, hist_host, err, nrhs);
 }
 
 int solve_schur(wd_gauge *g, const ApplyArgs &shape, int kind, void *x, const void *b, double mass, int parity, int max_iter,

@@ -26,17 +26,21 @@ constexpr int EO_THREADS = 128;
 template <typename T, int RECON, int SGN>
 __global__ void __launch_bounds__(EO_THREADS)
 dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ xin, const T *__restrict__ links,
-                 int Lx, int Ly, int Lz, int Lt, long long Vh, T alpha, T beta, int parity, double *__restrict__ norm_part)
+                 int Lx, int Ly, int Lz, int Lt, long long Vh, T alpha, T beta, int parity, double *__restrict__ norm_part, int nrhs)
 {
+    // gridDim.x = (site blocks) * nrhs with the right-hand side FASTEST: the CTAs resident at any time are all right-hand
+    // sides of a few site blocks, so the links of a block come from HBM once and from L1/L2 for the others
+    const int rhs = (int)(blockIdx.x % (unsigned)nrhs);
+    const long long blk = blockIdx.x / (unsigned)nrhs, nblk = gridDim.x / (unsigned)nrhs;
     // norm_part (may be NULL): per-CTA partial sums of |out|^2 in fp64, fixed order -- lets a solver take the norm of
     // the result without another pass over it (wd_cg.cu)
-    const long long cb_raw = (long long)blockIdx.x * EO_THREADS + threadIdx.x;
+    const long long cb_raw = blk * EO_THREADS + threadIdx.x;
     const bool valid = cb_raw < Vh;
     if (!valid && !norm_part) return;
     const long long cb = valid ? cb_raw : Vh - 1; // (only the last CTA has such threads; they redo a site and drop it)
     const long long Vhp = padded_volume(Vh); // sites per right-hand side of a half field
-    in += (long long)blockIdx.y * 24 * Vhp;
-    out += (long long)blockIdx.y * 24 * Vhp;
+    in += (long long)rhs * 24 * Vhp;
+    out += (long long)rhs * 24 * Vhp;
 
     const int Lxh = Lx / 2;
     long long rem = cb;
@@ -67,7 +71,7 @@ dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restr
     load_link<3, T, RECON>(links, tb, u);   load_spinor(in, tb >> 1, p); hop_backward_s<3, SGN>(acc, u, p);
 
     if (xin) {
-        load_spinor(xin + (long long)blockIdx.y * 24 * Vhp, cb, p);
+        load_spinor(xin + (long long)rhs * 24 * Vhp, cb, p);
 #pragma unroll
         for (int i = 0; i < 24; ++i) acc[i] = fma(alpha, p[i], beta * acc[i]);
     } else {
@@ -88,7 +92,7 @@ dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restr
             double t = 0.0;
 #pragma unroll
             for (int i = 0; i < EO_THREADS / 32; ++i) t += sh[i];
-            norm_part[(long long)blockIdx.y * gridDim.x + blockIdx.x] = t;
+            norm_part[(long long)rhs * nblk + blk] = t;
         }
     }
 }
@@ -99,11 +103,11 @@ static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha
 {
     const long long Vh = a.V / 2;
     const long long nb = (Vh + EO_THREADS - 1) / EO_THREADS;
-    if (nb > 0x7fffffffLL || a.nrhs > 65535) return cudaErrorInvalidConfiguration;
-    dim3 grid((unsigned)nb, (unsigned)a.nrhs);
+    if (nb * a.nrhs > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)(nb * a.nrhs));
     auto kern = dagger ? dslash_eo_kernel<T, RECON, +1> : dslash_eo_kernel<T, RECON, -1>;
     kern<<<grid, EO_THREADS, 0, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)xin, (const T *)a.links, a.dims[0],
-                                             a.dims[1], a.dims[2], a.dims[3], Vh, (T)alpha, (T)beta, parity, norm_part);
+                                             a.dims[1], a.dims[2], a.dims[3], Vh, (T)alpha, (T)beta, parity, norm_part, a.nrhs);
     count_launch();
     return cudaGetLastError();
 }

@@ -104,6 +104,8 @@ int cgnr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, doub
                double tol, int *iters_out, double *hist_host, cudaError_t *err);
 int bicgstab_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter,
                    double tol, int *iters_out, double *hist_host, cudaError_t *err);
+int cgnr_schur_block(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int nrhs, int max_iter,
+                     double tol, int *iters_out, double *hist_host, cudaError_t *err);
 // preconditioner slot of GCR: z = K r, enqueued on `stream` (same type as wd_precond_fn in wd.h)
 typedef int (*precond_fn)(void *ctx, void *z_half_dev, const void *r_half_dev, void *stream);
 int gcr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter, int restart,

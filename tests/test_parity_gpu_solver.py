@@ -270,3 +270,37 @@ def test_zero_right_hand_side_gives_zero_not_nan(solver, tol):
     torch.cuda.synchronize()
     assert torch.all(xh == 0)
     op.close()
+
+
+@pytest.mark.parametrize("precision,recon,tol_x", [(64, 18, 1e-10), (32, 12, 2e-4)])
+def test_block_cgnr_is_the_single_solve_per_right_hand_side(oracle, precision, recon, tol_x):
+    """wd_cgnr_schur_block: nrhs right-hand sides in lock step with batched operator applications.  Each right-hand side's
+    iterate and history are bit-identical to wd_cgnr_schur on it alone, and match the oracle's CGNR."""
+    import torch
+    dims, parity, K, nrhs = (8, 8, 4, 8), 1, 10, 3
+    cfg = fields.Config("blk", dims, precision, "smooth", recon, 0.2, nrhs, 87)
+    U, b = fields.make_fields(cfg)
+    Uo = (U if recon == 18 else np.ascontiguousarray(U[..., :2, :, :])).astype(np.float64)
+    op = GpuOp(U, dims, precision, recon)
+    w = op.op
+    canon = torch.from_numpy(b).cuda()
+    n1 = w.half_numel(1)
+    bh = torch.zeros(nrhs * n1, dtype=canon.dtype, device="cuda")
+    w.pack_parity(bh, canon, nrhs, parity)
+    xh = torch.full_like(bh, float("nan"))
+    iters, hists = w.cgnr_schur_block(xh, bh, cfg.mass, parity, nrhs, K)
+    assert iters == K and len(hists) == nrhs
+    for r in range(nrhs):
+        xs = torch.full((n1,), float("nan"), dtype=canon.dtype, device="cuda")
+        it1, h1 = w.cgnr_schur(xs, bh[r * n1:(r + 1) * n1], cfg.mass, parity, K)
+        torch.cuda.synchronize()
+        assert torch.equal(xs, xh[r * n1:(r + 1) * n1])
+        assert h1 == hists[r]
+        x = from_half(op, xs, b[r:r + 1].shape, parity)[0]
+        want_x, want_hist = wd_solvers.cgnr_schur(b[r].astype(np.float64), Uo, dims, cfg.mass, parity, K)
+        assert rel_l2(x, want_x) <= tol_x
+        assert np.max(np.abs(np.array(hists[r]) / want_hist - 1.0)) <= tol_x * 10
+    # tolerance mode: stops when every right-hand side has converged
+    it2, h2 = w.cgnr_schur_block(xh, bh, cfg.mass, parity, nrhs, 300, tol=1e-5 if precision == 32 else 1e-10)
+    assert it2 < 300 and all(h[-1] <= (1e-5 if precision == 32 else 1e-10) for h in h2)
+    op.close()
