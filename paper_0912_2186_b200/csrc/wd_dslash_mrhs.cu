@@ -27,6 +27,7 @@
 #define WD_USE_F32X2 // packed FFMA2 SU(3) products (wd_math.cuh)
 #include "wd_internal.h"
 #include "wd_layout.cuh"
+#include "wd_async.cuh"
 #include "wd_math.cuh"
 #include "wd_link.cuh"
 
@@ -34,13 +35,6 @@ namespace wd {
 
 namespace {
 
-__device__ __forceinline__ void cpa16(float4 *smem_dst, const float4 *gsrc)
-{
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cpa_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cpa_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 // ---- bulk-copy (cp.async.bulk + mbarrier) variant of the link staging: the A/B the round-1 review asked for ----
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }

@@ -26,6 +26,7 @@
 #define WD_USE_F32X2 // packed FFMA2 SU(3) products (wd_math.cuh)
 #include "wd_internal.h"
 #include "wd_layout.cuh"
+#include "wd_async.cuh"
 #include "wd_math.cuh"
 #include "wd_link.cuh"
 
@@ -33,13 +34,6 @@ namespace wd {
 
 namespace {
 
-__device__ __forceinline__ void cpa16(void *smem_dst, const void *gsrc)
-{
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cpa_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cpa_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 // NV 16-byte vectors [vec][slot stride] -> registers
 template <int NV, typename Vec, typename T>

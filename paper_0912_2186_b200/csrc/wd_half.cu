@@ -16,6 +16,7 @@
 // moves 2 * 52 + 8 * RECON bytes (200 B with 12-real links against 384 B in fp32): the same arithmetic at about half the
 // traffic.  The canonical side of wd_pack_spinor / wd_unpack_spinor / wd_load_gauge is float32 for this precision.
 #include <cuda_fp16.h>
+#include "wd_half.cuh"
 #include "wd_internal.h"
 #include "wd_layout.cuh"
 #include "wd_math.cuh"
@@ -26,25 +27,6 @@ namespace {
 
 constexpr int HT = 128; // threads per CTA
 
-__device__ __forceinline__ void unpack8(const uint4 &v, float *r)
-{
-    const __half2 *h = reinterpret_cast<const __half2 *>(&v);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const float2 f = __half22float2(h[i]);
-        r[2 * i] = f.x;
-        r[2 * i + 1] = f.y;
-    }
-}
-
-__device__ __forceinline__ uint4 pack8(const float *r)
-{
-    uint4 v;
-    __half2 *h = reinterpret_cast<__half2 *>(&v);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) h[i] = __halves2half2(__float2half_rn(r[2 * i]), __float2half_rn(r[2 * i + 1]));
-    return v;
-}
 
 // half spinor of `site` of one right-hand side -> 24 floats (value = scale * ratio)
 __device__ __forceinline__ void load_spinor_h(const uint4 *__restrict__ field, const float *__restrict__ scale, long long site,

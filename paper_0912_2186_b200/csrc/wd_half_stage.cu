@@ -15,8 +15,10 @@
 //   * 400 B of shared memory per site with 12-real links (fp32: 840 B): three CTAs of 128 sites per SM.
 // Lx must be a power of two (4..32); other lattices take the general kernel of wd_half.cu.
 #include <cuda_fp16.h>
+#include "wd_half.cuh"
 #include "wd_internal.h"
 #include "wd_layout.cuh"
+#include "wd_async.cuh"
 #define WD_USE_F32X2
 #include "wd_math.cuh"
 
@@ -24,37 +26,7 @@ namespace wd {
 
 namespace {
 
-__device__ __forceinline__ void cpa16(void *smem_dst, const void *gsrc)
-{
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cpa4(void *smem_dst, const void *gsrc)
-{
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cpa_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cpa_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
-__device__ __forceinline__ void unpack8(const uint4 &v, float *r)
-{
-    const __half2 *h = reinterpret_cast<const __half2 *>(&v);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const float2 f = __half22float2(h[i]);
-        r[2 * i] = f.x;
-        r[2 * i + 1] = f.y;
-    }
-}
-__device__ __forceinline__ uint4 pack8(const float *r)
-{
-    uint4 v;
-    __half2 *h = reinterpret_cast<__half2 *>(&v);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) h[i] = __halves2half2(__float2half_rn(r[2 * i]), __float2half_rn(r[2 * i + 1]));
-    return v;
-}
 
 // staged half spinor [3][stride] + scale -> 24 floats
 __device__ __forceinline__ void lds_spinor(const uint4 *buf, const float *scale, int stride, int slot, float (&p)[24])
