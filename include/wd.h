@@ -187,10 +187,11 @@ int wd_apply_dagger(void *out_native_dev, const void *in_native_dev, const wd_ga
  * wd_apply_host -- the same operation for callers whose data lives in HOST memory, in
  * CANONICAL layout: copies in_canonical_host to the device, packs, applies D, unpacks, copies
  * the result to out_canonical_host and synchronises the gauge's stream before returning.
- * Fields of at least 8 MB on lattices with Lx*Ly*Lz a multiple of 128 and Lt >= 3 are cut into up
- * to 16 slabs of whole time slices and pipelined over three internal streams (copy-in + pack,
- * apply on the slab's site range, unpack + copy-out), so the two PCIe directions overlap; other
- * lattices go through one stream.  Work already enqueued on the gauge's stream is waited for first.
+ * Fields of at least 8 MB on lattices with Lx*Ly*Lz a multiple of 128 and Lt >= 3 are cut into
+ * slabs of whole time slices (16 by default, tuning variable "host_nslab", 3..32) and pipelined
+ * over three internal streams (copies in; pack, apply on a range of time slices, unpack; copies
+ * out), so the two PCIe directions overlap; other lattices go through one stream.  Both paths
+ * give the same bits.  Work already enqueued on the gauge's stream is waited for first.
  * Device staging buffers, streams and events are owned by the gauge handle (created on first use,
  * reused, released by wd_destroy_gauge); not re-entrant for one gauge handle.
  * Pinned host memory gives asynchronous copies; pageable memory works but is slower.

@@ -420,6 +420,15 @@ int wd_apply_dagger(void *out_native_dev, const void *in_native_dev, const wd_ga
     return dispatch_apply(out_native_dev, in_native_dev, gauge, mass, nrhs, 1);
 }
 
+// the same `width` bytes of each of `rows` right-hand sides (pitch `pitch` on both sides); one right-hand side is a plain
+// linear copy
+static cudaError_t copy_rows(char *dst, const char *src, size_t pitch, size_t width, int rows, cudaMemcpyKind kind,
+                             cudaStream_t st)
+{
+    if (rows == 1) return cudaMemcpyAsync(dst, src, width, kind, st);
+    return cudaMemcpy2DAsync(dst, pitch, src, pitch, width, rows, kind, st);
+}
+
 int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_gauge *gauge, double mass,
                   const int dims[4], int nrhs, int precision)
 {
@@ -454,10 +463,9 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
     const int Lt = g->dims[3];
     cudaError_t e;
 
-    // ---- pipelined path: the lattice is cut into up to 32 slabs of whole time slices; slab k is copied in
-    // and packed on one stream, D is applied to it (site kernel on the slab's site range) on a second
-    // stream as soon as slabs k-1, k, k+1 have arrived, and its result is unpacked and copied out on a
-    // third stream, so the host->device and device->host transfers overlap (PCIe is full duplex) ----
+    // ---- pipelined path: the lattice is cut into up to 32 slabs of whole time slices; the slabs are copied in on one
+    // stream; packing, D (site kernel on a range of time slices) and unpacking run on a second as the slabs land; the
+    // results go home on a third, so the host->device and device->host transfers overlap (PCIe is full duplex) ----
     // (the event arrays of wd_gauge hold 32; more slabs = shorter pipeline fill and drain but more launches: measured 16 best)
     int nslab = g->tune.host_nslab >= 3 ? g->tune.host_nslab : 16;
     if (nslab > 32) nslab = 32;
@@ -493,50 +501,85 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
         // everything enqueued on the gauge's stream so far (e.g. the link conversion) comes first
         if ((e = cudaEventRecord(ev_start, s)) != cudaSuccess) return bail(e, "wd_apply_host: event record");
         for (int i = 0; i < 3; ++i) cudaStreamWaitEvent(g->pipe_stream[i], ev_start, 0);
-        auto t0 = [&](int k) { return (long long)Lt * k / nslab; };
+        // Slab boundaries in time slices.  Only one direction of the link is busy until the first result leaves and after
+        // the last slab has landed, so the slabs at either end are thin when Lt allows it (Lt >= 4 nslab, nslab >= 8:
+        // 2, 3 slices at the head; 2, 1, 1 at the tail) and the rest share what is left evenly.
+        long long bnd[33];
+        {
+            for (int k = 0; k <= nslab; ++k) bnd[k] = (long long)Lt * k / nslab;
+            if (Lt >= 4 * nslab && nslab >= 8) {
+                bnd[1] = 2;
+                bnd[2] = 5;
+                bnd[nslab - 1] = Lt - 1;
+                bnd[nslab - 2] = Lt - 2;
+                bnd[nslab - 3] = Lt - 4;
+                const int mid = nslab - 5; // evenly sized slabs 2 .. nslab-4
+                for (int j = 1; j < mid; ++j) bnd[2 + j] = 5 + (Lt - 9) * j / mid;
+            }
+        }
         const size_t row = (size_t)g->V * 24 * w; // bytes of one right-hand side, canonical
         // Copy streams carry ONLY copies (back to back, nothing between two transfers); pack, apply and unpack all run on
-        // the compute stream.  Arrival order: the LAST slab first (it is slab 0's backward neighbour), then 0, 1, ...,
-        // nslab-2: slab k can be computed as soon as slab k+1 has arrived, and only two slabs are left to compute when
-        // the last one lands.
+        // the compute stream.  Arrival order: the LAST slab first (it holds slice 0's backward neighbour), then 0, 1, ...,
+        // nslab-2.  The computed ranges are the slabs shifted back by one slice, so that a range needs nothing beyond the
+        // slab that has just landed:
+        //   after slabs nslab-1 and 0:  [bnd[nslab-1]+1, Lt)  and  [0, bnd[1]-1)
+        //   after slab k = 1..nslab-3:  [bnd[k]-1, bnd[k+1]-1)
+        //   after slab nslab-2 (last):  [bnd[nslab-2]-1, bnd[nslab-1]+1)
+        // and only that last range (the last slab landed plus two slices) is left to compute at the end.  `hold` = the slab
+        // whose arrival releases a range's copy home (see below), -1 = none.
         for (int i = 0; i < nslab; ++i) {
             const int k = i == 0 ? nslab - 1 : i - 1;
-            const long long s0 = t0(k) * S3, ns = (t0(k + 1) - t0(k)) * S3;
-            e = cudaMemcpy2DAsync((char *)g->stage_canon + (size_t)s0 * 24 * w, row,
-                                  (const char *)in_canonical_host + (size_t)s0 * 24 * w, row, (size_t)ns * 24 * w, nrhs,
-                                  cudaMemcpyHostToDevice, s_in);
+            const long long s0 = bnd[k] * S3, ns = (bnd[k + 1] - bnd[k]) * S3;
+            e = copy_rows((char *)g->stage_canon + (size_t)s0 * 24 * w, (const char *)in_canonical_host + (size_t)s0 * 24 * w,
+                          row, (size_t)ns * 24 * w, nrhs, cudaMemcpyHostToDevice, s_in);
             if (e != cudaSuccess) return bail(e, "wd_apply_host: H2D copy");
             cudaEventRecord(ev_in[k], s_in);
         }
-        bool packed[32] = {};
-        for (int k = 0; k < nslab; ++k) {
-            const int need[3] = {(k + nslab - 1) % nslab, k, (k + 1) % nslab};
-            for (int n : need) {
-                if (packed[n]) continue;
-                cudaStreamWaitEvent(s_cmp, ev_in[n], 0);
-                e = wd::launch_pack_spinor(g->stage_in, g->stage_canon, g->V, nrhs, precision, s_cmp, t0(n) * S3,
-                                           (t0(n + 1) - t0(n)) * S3);
-                if (e != cudaSuccess) return bail(e, "wd_apply_host: pack");
-                packed[n] = true;
-            }
+        auto pack_slab = [&](int k) {
+            cudaStreamWaitEvent(s_cmp, ev_in[k], 0);
+            return wd::launch_pack_spinor(g->stage_in, g->stage_canon, g->V, nrhs, precision, s_cmp, bnd[k] * S3,
+                                          (bnd[k + 1] - bnd[k]) * S3);
+        };
+        int n_ev = 0;
+        const char *what = nullptr;
+        // D on the time slices [ta, tb), its result unpacked and sent home
+        auto range = [&](long long ta, long long tb, int hold) {
+            if (tb <= ta) return cudaSuccess;
             wd::ApplyArgs a = shape_args(g, nrhs);
             a.out = g->stage_out;
             a.in = g->stage_in;
             a.links = g->links;
             a.mass = mass;
             a.stream = s_cmp;
-            a.site_begin = t0(k) * S3;
-            a.site_end = t0(k + 1) * S3;
-            if ((e = wd::launch_site(a)) != cudaSuccess) return bail(e, "wd_apply_host: kernel launch");
-            e = wd::launch_unpack_spinor(g->stage_canon_out, g->stage_out, g->V, nrhs, precision, s_cmp, a.site_begin,
-                                         a.site_end - a.site_begin);
-            if (e != cudaSuccess) return bail(e, "wd_apply_host: unpack");
-            cudaEventRecord(ev_cmp[k], s_cmp);
-            cudaStreamWaitEvent(s_out, ev_cmp[k], 0);
-            e = cudaMemcpy2DAsync((char *)out_canonical_host + (size_t)a.site_begin * 24 * w, row,
-                                  (const char *)g->stage_canon_out + (size_t)a.site_begin * 24 * w, row,
-                                  (size_t)(a.site_end - a.site_begin) * 24 * w, nrhs, cudaMemcpyDeviceToHost, s_out);
-            if (e != cudaSuccess) return bail(e, "wd_apply_host: D2H copy");
+            a.site_begin = ta * S3;
+            a.site_end = tb * S3;
+            what = "wd_apply_host: kernel launch";
+            cudaError_t er = wd::launch_site(a);
+            if (er != cudaSuccess) return er;
+            what = "wd_apply_host: unpack";
+            er = wd::launch_unpack_spinor(g->stage_canon_out, g->stage_out, g->V, nrhs, precision, s_cmp, a.site_begin,
+                                          a.site_end - a.site_begin);
+            if (er != cudaSuccess) return er;
+            cudaEventRecord(ev_cmp[n_ev], s_cmp);
+            cudaStreamWaitEvent(s_out, ev_cmp[n_ev], 0);
+            // Measured on B200 (PCIe 5 x16): a host->device copy that STARTS while a device->host copy is in flight loses
+            // about 40 us (16 pieces against one long copy out: 4.89 ms; one piece against 13 out: 4.34 ms for 201 MB
+            // each way), while a copy out may start at any time.  So a result leaves when the NEXT slab has landed: both
+            // directions then start their pieces together and the copy in never starts under a copy out (4.96 -> 4.76 ms)
+            if (hold >= 0) cudaStreamWaitEvent(s_out, ev_in[hold], 0);
+            ++n_ev;
+            what = "wd_apply_host: D2H copy";
+            return copy_rows((char *)out_canonical_host + (size_t)a.site_begin * 24 * w,
+                             (const char *)g->stage_canon_out + (size_t)a.site_begin * 24 * w, row,
+                             (size_t)(a.site_end - a.site_begin) * 24 * w, nrhs, cudaMemcpyDeviceToHost, s_out);
+        };
+        if ((e = pack_slab(nslab - 1)) != cudaSuccess || (e = pack_slab(0)) != cudaSuccess) return bail(e, "wd_apply_host: pack");
+        if ((e = range(0, bnd[1] - 1, 1)) != cudaSuccess) return bail(e, what);
+        if ((e = range(bnd[nslab - 1] + 1, Lt, 1)) != cudaSuccess) return bail(e, what);
+        for (int k = 1; k <= nslab - 2; ++k) {
+            if ((e = pack_slab(k)) != cudaSuccess) return bail(e, "wd_apply_host: pack");
+            const long long tb = k == nslab - 2 ? bnd[nslab - 1] + 1 : bnd[k + 1] - 1;
+            if ((e = range(bnd[k] - 1, tb, k + 1 <= nslab - 2 ? k + 1 : -1)) != cudaSuccess) return bail(e, what);
         }
         if ((e = cudaEventRecord(ev_end, s_out)) != cudaSuccess) return bail(e, "wd_apply_host: event record");
         cudaStreamWaitEvent(s, ev_end, 0);

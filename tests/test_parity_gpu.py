@@ -273,15 +273,21 @@ def test_argument_errors_on_device():
     op.close()
 
 
-@pytest.mark.parametrize("dims,precision,recon,nrhs", [((16, 16, 16, 16), 32, 18, 2), ((32, 16, 16, 5), 64, 12, 2),
-                                                     ((32, 8, 16, 3), 32, 18, 8), ((16, 16, 8, 24), 32, 12, 3)])
-def test_apply_host_pipelined_path(oracle, monkeypatch, dims, precision, recon, nrhs):
+@pytest.mark.parametrize("dims,precision,recon,nrhs,nslab", [
+    ((16, 16, 16, 16), 32, 18, 2, None), ((32, 16, 16, 5), 64, 12, 2, None), ((32, 8, 16, 3), 32, 18, 8, None),
+    ((16, 16, 8, 24), 32, 12, 3, None),
+    # Lt >= 4 nslab: thin slabs at either end of the pipeline (default 16 slabs, then 8, 9, 3 and 32 by the tuning variable)
+    ((16, 16, 8, 64), 32, 18, 1, None), ((16, 16, 8, 64), 32, 12, 2, 8), ((16, 8, 8, 72), 64, 18, 1, 9),
+    ((16, 16, 8, 64), 32, 18, 1, 3), ((16, 16, 8, 64), 32, 18, 1, 32), ((16, 8, 8, 33), 64, 18, 2, 8)])
+def test_apply_host_pipelined_path(oracle, monkeypatch, dims, precision, recon, nrhs, nslab):
     """wd_apply_host on fields large enough for its slab pipeline (H2D / apply / D2H overlapped on three
     streams): same bits as the one-stream host path, and the oracle's result."""
     cfg = fields.Config("hp", dims, precision, "haar", recon, -0.4, nrhs, 53)
     U, psi = fields.make_fields(cfg)
     assert psi.nbytes >= 8 << 20
     op = GpuOp(U, dims, precision, recon, KERNELS["site"])
+    if nslab:
+        op.op.set_tuning("host_nslab", nslab)
     out = np.full_like(psi, np.nan)
     op.op.apply_host(out, psi, cfg.mass, nrhs)
     again = np.full_like(psi, np.nan)
