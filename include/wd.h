@@ -205,6 +205,9 @@ int wd_apply_host(void *out_canonical_host, const void *in_canonical_host, wd_ga
  * Site parity p(x) = (x+y+z+t) mod 2; D = [ (4+m) 1, H_eo ; H_oe, (4+m) 1 ] with H_pq the hopping term of
  * eq. (2.2) from parity q to parity p (factor -1/2 included).  A HALF FIELD holds the V/2 sites of one parity in
  * the blocked native layout over the checkerboard index lex/2; wd_spinor_bytes_parity() is its size.
+ * The first red/black call on a gauge handle (wd_apply_hop, wd_apply_schur*, any solver) allocates and fills, on the
+ * gauge's stream, a parity-ordered copy of the handle's link records (as large as the native links; WD_ERR_ALLOC if
+ * that fails); it is owned by the handle and released by wd_destroy_gauge.
  */
 size_t wd_spinor_bytes_parity(const wd_lattice *lat, int nrhs, int precision);
 

@@ -361,6 +361,7 @@ static wd::ApplyArgs shape_args(const wd_gauge *g, int nrhs)
     a.recon = g->recon;
     a.tgauge = g->tgauge;
     a.tune = &g->tune;
+    a.links_eo = g->links_eo;
     return a;
 }
 
@@ -671,6 +672,24 @@ static int check_eo_args(const char *who, const void *out, const void *in, const
     const size_t hb = half_bytes(g->V, nrhs, precision);
     if (overlap(out, hb, in, hb)) return fail(WD_ERR_ALIAS, "%s: out and in overlap", who);
     if (((uintptr_t)out | (uintptr_t)in) & 15) return fail(WD_ERR_MISMATCH, "%s: buffers must be 16-byte aligned", who);
+    // the red/black kernels read a parity-ordered copy of the link records (wd_dslash_eo.cu); it is made here, on the
+    // gauge's stream, by the first red/black call on the handle (the handle is opaque to the caller: the copy is a cache)
+    if (!g->links_eo) {
+        wd_gauge *gm = const_cast<wd_gauge *>(g);
+        const size_t nb = 2 * wd::eo_links_half_bytes(g->V, g->precision, g->recon);
+        if (cudaMalloc(&gm->links_eo, nb) != cudaSuccess) {
+            gm->links_eo = nullptr;
+            cudaGetLastError();
+            return fail(WD_ERR_ALLOC, "%s: cudaMalloc of %zu bytes for the parity-ordered links failed", who, nb);
+        }
+        cudaError_t e = cudaMemsetAsync(gm->links_eo, 0, nb, g->stream); // padding lanes of the last blocks
+        if (e == cudaSuccess) e = wd::launch_links_to_eo(gm->links_eo, g->links, g->dims, g->V, g->precision, g->recon, g->stream);
+        if (e != cudaSuccess) {
+            cudaFree(gm->links_eo);
+            gm->links_eo = nullptr;
+            return cuda_fail(e, "parity-ordered links");
+        }
+    }
     return WD_OK;
 }
 
@@ -900,6 +919,7 @@ void wd_destroy_gauge(wd_gauge *gauge)
     if (!gauge || gauge->magic != GAUGE_MAGIC) return;
     gauge->magic = 0;
     cudaFree(gauge->links);
+    cudaFree(gauge->links_eo);
     cudaFree(gauge->stage_canon);
     cudaFree(gauge->stage_canon_out);
     cudaFree(gauge->cg_ws);

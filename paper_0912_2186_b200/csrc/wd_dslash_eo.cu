@@ -10,9 +10,12 @@
 //
 // Fields of one parity ("half fields") use the blocked native spinor layout of wd_layout.cuh over the
 // checkerboard index  cb = lex / 2  (lex = x + Lx*(y + Ly*(z + Lz*t)), Lx even), Vh = V/2 sites.  The links
-// are the gauge handle's ordinary full-lattice native links, indexed by lex.  One thread per output site,
-// neighbours straight from global memory (the structure of WD_KERNEL_SITE): every link of the lattice is
-// used exactly once per launch (forward at parity p, daggered at parity q), every input spinor eight times.
+// are a parity-ordered copy of the gauge handle's native link records (wd_gauge::links_eo: the records of the even
+// sites, then those of the odd sites, each half in the blocked layout over cb), made once per gauge handle: with the
+// full-lattice array a warp of one parity touched every other 16-byte lane, i.e. half of every 32-byte sector it
+// pulled through L1.  One thread per output site, neighbours straight from global memory (the structure of
+// WD_KERNEL_SITE): every link of the lattice is used exactly once per launch (forward at parity p, daggered at
+// parity q), every input spinor eight times.
 #include "wd_internal.h"
 #include "wd_layout.cuh"
 #include "wd_math.cuh"
@@ -25,7 +28,8 @@ constexpr int EO_THREADS = 128;
 // SGN = -1: blocks of D; SGN = +1: blocks of gamma5 D gamma5 = D^dagger (all projectors swapped)
 template <typename T, int RECON, int SGN>
 __global__ void __launch_bounds__(EO_THREADS)
-dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ xin, const T *__restrict__ links,
+dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ xin, const T *__restrict__ links_p,
+                 const T *__restrict__ links_q,
                  int Lx, int Ly, int Lz, int Lt, long long Vh, T alpha, T beta, int parity, double *__restrict__ norm_part, int nrhs)
 {
     // gridDim.x = (site blocks) * nrhs with the right-hand side FASTEST: the CTAs resident at any time are all right-hand
@@ -60,15 +64,17 @@ dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restr
 #pragma unroll
     for (int i = 0; i < 24; ++i) acc[i] = (T)0;
     T u[18], p[24];
-    // neighbours have the opposite parity; their half-field index is lex / 2
-    load_link<0, T, RECON>(links, site, u); load_spinor(in, xf >> 1, p); hop_forward_s<0, SGN>(acc, u, p);
-    load_link<0, T, RECON>(links, xb, u);   load_spinor(in, xb >> 1, p); hop_backward_s<0, SGN>(acc, u, p);
-    load_link<1, T, RECON>(links, site, u); load_spinor(in, yf >> 1, p); hop_forward_s<1, SGN>(acc, u, p);
-    load_link<1, T, RECON>(links, yb, u);   load_spinor(in, yb >> 1, p); hop_backward_s<1, SGN>(acc, u, p);
-    load_link<2, T, RECON>(links, site, u); load_spinor(in, zf >> 1, p); hop_forward_s<2, SGN>(acc, u, p);
-    load_link<2, T, RECON>(links, zb, u);   load_spinor(in, zb >> 1, p); hop_backward_s<2, SGN>(acc, u, p);
-    load_link<3, T, RECON>(links, site, u); load_spinor(in, tf >> 1, p); hop_forward_s<3, SGN>(acc, u, p);
-    load_link<3, T, RECON>(links, tb, u);   load_spinor(in, tb >> 1, p); hop_backward_s<3, SGN>(acc, u, p);
+    // neighbours have the opposite parity; their half-field index is lex / 2.  links_p / links_q: link records of the sites
+    // of parity p / 1-p in half-field order, so that a warp's forward links (own sites) and daggered links (neighbour sites)
+    // are 32 consecutive 16-byte lanes like its spinors (with the full-lattice link array they were every other lane)
+    load_link<0, T, RECON>(links_p, cb, u);      load_spinor(in, xf >> 1, p); hop_forward_s<0, SGN>(acc, u, p);
+    load_link<0, T, RECON>(links_q, xb >> 1, u); load_spinor(in, xb >> 1, p); hop_backward_s<0, SGN>(acc, u, p);
+    load_link<1, T, RECON>(links_p, cb, u);      load_spinor(in, yf >> 1, p); hop_forward_s<1, SGN>(acc, u, p);
+    load_link<1, T, RECON>(links_q, yb >> 1, u); load_spinor(in, yb >> 1, p); hop_backward_s<1, SGN>(acc, u, p);
+    load_link<2, T, RECON>(links_p, cb, u);      load_spinor(in, zf >> 1, p); hop_forward_s<2, SGN>(acc, u, p);
+    load_link<2, T, RECON>(links_q, zb >> 1, u); load_spinor(in, zb >> 1, p); hop_backward_s<2, SGN>(acc, u, p);
+    load_link<3, T, RECON>(links_p, cb, u);      load_spinor(in, tf >> 1, p); hop_forward_s<3, SGN>(acc, u, p);
+    load_link<3, T, RECON>(links_q, tb >> 1, u); load_spinor(in, tb >> 1, p); hop_backward_s<3, SGN>(acc, u, p);
 
     if (xin) {
         load_spinor(xin + (long long)rhs * 24 * Vhp, cb, p);
@@ -106,7 +112,11 @@ static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha
     if (nb * a.nrhs > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     dim3 grid((unsigned)(nb * a.nrhs));
     auto kern = dagger ? dslash_eo_kernel<T, RECON, +1> : dslash_eo_kernel<T, RECON, -1>;
-    kern<<<grid, EO_THREADS, 0, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)xin, (const T *)a.links, a.dims[0],
+    if (!a.links_eo) return cudaErrorInvalidValue; // the API builds the parity-ordered links before any red/black launch
+    const char *le = (const char *)a.links_eo;
+    const size_t half = eo_links_half_bytes(a.V, a.precision, a.recon);
+    kern<<<grid, EO_THREADS, 0, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)xin, (const T *)(le + parity * half),
+                                             (const T *)(le + (1 - parity) * half), a.dims[0],
                                              a.dims[1], a.dims[2], a.dims[3], Vh, (T)alpha, (T)beta, parity, norm_part, a.nrhs);
     count_launch();
     return cudaGetLastError();
@@ -124,6 +134,41 @@ cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double 
     return a.recon == 18 ? launch_eo_t<double, 18>(a, xin, alpha, beta, parity, dagger, norm_part)
            : a.recon == 12 ? launch_eo_t<double, 12>(a, xin, alpha, beta, parity, dagger, norm_part)
                            : launch_eo_t<double, 8>(a, xin, alpha, beta, parity, dagger, norm_part);
+}
+
+// ---- parity-ordered link records (pure data movement) ----
+size_t eo_links_half_bytes(long long V, int precision, int recon)
+{
+    const size_t nvec = (size_t)recon * (precision == 32 ? 4 : 8) / 4; // 16-byte vectors per site: four links
+    return (size_t)((V / 2 + BLK - 1) / BLK) * nvec * BLK * 16;
+}
+
+__global__ void links_to_eo_kernel(uint4 *__restrict__ dst, const uint4 *__restrict__ src, int Lx, int Ly, int Lz, long long V,
+                                   int nvec, long long half_vecs)
+{
+    const long long site = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (site >= V) return;
+    long long rem = site;
+    const int x = (int)(rem % Lx); rem /= Lx;
+    const int y = (int)(rem % Ly); rem /= Ly;
+    const int z = (int)(rem % Lz);
+    const long long t = rem / Lz;
+    const int par = (int)((x + y + z + t) & 1);
+    const long long cb = site >> 1;
+    const uint4 *q = src + (site >> 5) * ((long long)nvec * BLK) + (site & (BLK - 1));
+    uint4 *d = dst + par * half_vecs + (cb >> 5) * ((long long)nvec * BLK) + (cb & (BLK - 1));
+    for (int v = 0; v < nvec; ++v) d[(long long)v * BLK] = q[(long long)v * BLK];
+}
+
+cudaError_t launch_links_to_eo(void *links_eo, const void *links, const int dims[4], long long V, int precision, int recon,
+                               cudaStream_t s)
+{
+    const int nvec = recon * (precision == 32 ? 4 : 8) / 4;
+    const long long half_vecs = (long long)(eo_links_half_bytes(V, precision, recon) / 16);
+    links_to_eo_kernel<<<(unsigned)((V + 127) / 128), 128, 0, s>>>((uint4 *)links_eo, (const uint4 *)links, dims[0], dims[1], dims[2],
+                                                                   V, nvec, half_vecs);
+    count_launch();
+    return cudaGetLastError();
 }
 
 // canonical full-lattice field <-> native half field of one parity (pure data movement)

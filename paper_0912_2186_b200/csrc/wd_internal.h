@@ -42,6 +42,8 @@ struct wd_gauge {
     int pipe_ready;   // the three streams and 34 events of the pipelined host path all exist
     void *links;      // native links, device (cudaMalloc)
     size_t links_bytes;
+    void *links_eo;   // the same link records ordered by parity (even sites, then odd sites; record index lex / 2): what the
+                      // red/black kernels read; built from `links` on the first red/black call, NULL until then
     cudaStream_t stream;
     // staging for wd_apply_host (allocated on first use)
     void *stage_canon;   // canonical spinor buffer (input), device
@@ -66,6 +68,7 @@ struct ApplyArgs {
     void *out;
     const void *in;
     const void *links;
+    const void *links_eo;           // red/black kernels: parity-ordered copy of the links (wd_gauge::links_eo)
     int dims[4];
     long long V;
     double mass;
@@ -97,6 +100,10 @@ cudaError_t launch_pack_spinor(void *native, const void *canonical, long long V,
 cudaError_t launch_unpack_spinor(void *canonical, const void *native, long long V, int nrhs, int precision,
                                  cudaStream_t s, long long site0 = 0, long long nsites = -1);
 // red/black blocks (wd_dslash_eo.cu): out_p = alpha * xin_p + beta * hops(in_q); half-field <-> canonical copies
+// parity-ordered link records: record cb of parity p sits at p * eo_links_half_bytes + native position of `cb`
+size_t eo_links_half_bytes(long long V, int precision, int recon);
+cudaError_t launch_links_to_eo(void *links_eo, const void *links, const int dims[4], long long V, int precision, int recon,
+                               cudaStream_t s);
 cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger = false,
                       double *norm_part = nullptr);
 // CGNR for Mhat x = b on one parity (wd_cg.cu); shape carries dims, V, precision, recon, links, stream
