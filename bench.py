@@ -653,8 +653,11 @@ def run_cgnr(args):
     """--op cgnr | bicgstab: the Krylov solvers on the even-odd preconditioned operator (SURVEY.md 8(f) f2;
     PAPER.md:116, Table 2): a step = one solver call of ITER iterations (tol = 0: no host synchronisation inside).
     Per iteration and even site: two operator applications (2 x (2 x 1320 + 48) flops, 2 x Schur-apply bytes) plus
-    the BLAS-1 kernels: CGNR 288 flops / 9 spinor passes (the two norms come out of the matvec epilogue), BiCGstab
-    672 flops / 19 spinor passes, GCR(8) ~1150 flops / 38 passes averaged over a cycle."""
+    the BLAS-1 kernels: CGNR 288 flops / 8 spinor passes (the two norms come out of the matvec epilogue; x += alpha p rides
+    on the p update), BiCGstab
+    672 flops / 15 spinor passes (<rhat, v>, <t, s>, |t|^2 come out of the matvec epilogues, <rhat, r> out of the x / r update), GCR(8) ~1150 flops / 22.25 passes averaged over a cycle
+    (direction j of a cycle: j + 1 passes for its inner products with the earlier q_i, 2j + 5 for the orthogonalisation that
+    also takes <q_j, r> and |q_j|^2, 6 for the x / r update)."""
     import torch
     from paper_0912_2186_b200 import binding, build
     rank, local, world = dist_env()
@@ -695,8 +698,8 @@ def run_cgnr(args):
     if nblk > 1:
         solve = lambda xx, bb, mass, parity, it: op.cgnr_schur_block(xx, bb, mass, parity, nblk, it)
     # BLAS-1 flops / spinor passes per iteration and even site; matvecs per iteration.  GCR(8): averages over a cycle
-    # (3.5 Gram-Schmidt steps of 2 + 6 passes each, plus the copy, the <q,r> dot and the x/r update)
-    blas_flops, blas_passes, nmv = {"cgnr": (288, 9, 2), "bicgstab": (672, 19, 2), "gcr": (1150, 38, 1)}[args.op]
+    # (direction j: 3j + 12 passes for j >= 1, 10 for j = 0)
+    blas_flops, blas_passes, nmv = {"cgnr": (288, 8, 2), "bicgstab": (672, 15, 2), "gcr": (1150, 22.25, 1)}[args.op]
     for _ in range(max(args.warmup, 3)):
         solve(x, b, cfg.mass, 0, iters)
     torch.cuda.synchronize()

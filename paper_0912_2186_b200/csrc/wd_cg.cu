@@ -30,7 +30,19 @@ constexpr int RED_THREADS = 256;
 __device__ __forceinline__ double sum_partials(const double *part, int n = RED_BLOCKS)
 {
     __shared__ double total;
-    if (threadIdx.x < 32) {
+    if (n > 2048) { // the per-CTA partials of a matvec epilogue (thousands): every warp takes a share, same fixed pattern
+        __shared__ double wsum[RED_THREADS / 32];
+        double s = 0.0;
+        for (int i = threadIdx.x; i < n; i += RED_THREADS) s += part[i];
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+        if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = s;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = 0.0;
+            for (int i = 0; i < RED_THREADS / 32; ++i) t += wsum[i];
+            total = t;
+        }
+    } else if (threadIdx.x < 32) {
         double s = 0.0;
         for (int i = threadIdx.x; i < n; i += 32) s += part[i];
         for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
@@ -104,34 +116,33 @@ __global__ void __launch_bounds__(RED_THREADS) norm2_kernel(const Vec *v, long l
     if (threadIdx.x == 0) part[blockIdx.x] = s;
 }
 
-// alpha = zz / ww;  x += alpha p;  r -= alpha w;  rr_part = |r|^2 partials
+// alpha = zz / ww;  r -= alpha w;  rr_part = |r|^2 partials   (x += alpha p is done by update_px_kernel, which reads p anyway)
 template <typename Vec, int NCH>
 __global__ void __launch_bounds__(RED_THREADS)
-update_xr_kernel(Vec *x, Vec *r, const Vec *p, const Vec *w, long long nvec, long long Vh, const double *zz_part,
-                 const double *ww_part, int npart, double *rr_part)
+update_r_kernel(Vec *r, const Vec *w, long long nvec, long long Vh, const double *zz_part, const double *ww_part, int npart,
+                double *rr_part)
 {
     {   // blockIdx.y = right-hand side of a block solve
         const long long rhs = blockIdx.y;
-        x += rhs * nvec; r += rhs * nvec; p += rhs * nvec; w += rhs * nvec;
+        r += rhs * nvec; w += rhs * nvec;
         zz_part += rhs * npart; ww_part += rhs * npart; rr_part += rhs * RED_BLOCKS;
     }
     __shared__ double sh[RED_THREADS / 32];
     const double alpha = safe_div(sum_partials(zz_part, npart), sum_partials(ww_part, npart));
     double s = 0.0;
-    constexpr int UNR = 2; // independent vectors per thread and trip (4 streams x 2 loads in flight; 4 costs occupancy)
+    constexpr int UNR = 4; // independent vectors per thread and trip
     const long long stride = (long long)RED_BLOCKS * RED_THREADS;
     for (long long i0 = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i0 < nvec; i0 += UNR * stride) {
-        Vec pv[UNR], xv[UNR], wv[UNR], rv[UNR];
+        Vec wv[UNR], rv[UNR];
 #pragma unroll
         for (int u = 0; u < UNR; ++u) {
             const long long i = i0 + u * stride;
-            if (i < nvec) { pv[u] = p[i]; xv[u] = x[i]; wv[u] = w[i]; rv[u] = r[i]; }
+            if (i < nvec) { wv[u] = w[i]; rv[u] = r[i]; }
         }
 #pragma unroll
         for (int u = 0; u < UNR; ++u) {
             const long long i = i0 + u * stride;
             if (i < nvec) {
-                x[i] = axpy_vec(alpha, pv[u], xv[u]);
                 const Vec rn = axpy_vec(-alpha, wv[u], rv[u]);
                 r[i] = rn;
                 if (real_site<NCH>(i, Vh)) s += norm2_vec(rn);
@@ -142,35 +153,42 @@ update_xr_kernel(Vec *x, Vec *r, const Vec *p, const Vec *w, long long nvec, lon
     if (threadIdx.x == 0) rr_part[blockIdx.x] = s;
 }
 
-// beta = zz_new / zz_old;  p = z + beta p;  hist[k] = sqrt(rr) (block 0)
+// alpha = zz_old / ww (the step just taken);  x += alpha p;  beta = zz_new / zz_old;  p = z + beta p;
+// hist[k] = sqrt(rr) (block 0)
 template <typename Vec>
 __global__ void __launch_bounds__(RED_THREADS)
-update_p_kernel(Vec *p, const Vec *z, long long nvec, const double *zz_new_part, const double *zz_old_part,
-                int npart, const double *rr_part, double *hist_k, long long hist_stride = 0)
+update_px_kernel(Vec *x, Vec *p, const Vec *z, long long nvec, const double *zz_new_part, const double *zz_old_part,
+                 const double *ww_part, int npart, const double *rr_part, double *hist_k, long long hist_stride = 0)
 {
     {   // blockIdx.y = right-hand side of a block solve
         const long long rhs = blockIdx.y;
-        p += rhs * nvec; z += rhs * nvec;
-        zz_new_part += rhs * npart; zz_old_part += rhs * npart; rr_part += rhs * RED_BLOCKS; hist_k += rhs * hist_stride;
+        x += rhs * nvec; p += rhs * nvec; z += rhs * nvec;
+        zz_new_part += rhs * npart; zz_old_part += rhs * npart; ww_part += rhs * npart; rr_part += rhs * RED_BLOCKS;
+        hist_k += rhs * hist_stride;
     }
-    const double beta = safe_div(sum_partials(zz_new_part, npart), sum_partials(zz_old_part, npart));
+    const double zz_old = sum_partials(zz_old_part, npart);
+    const double alpha = safe_div(zz_old, sum_partials(ww_part, npart));
+    const double beta = safe_div(sum_partials(zz_new_part, npart), zz_old);
     if (blockIdx.x == 0) { // (block-uniform branch: sum_partials has barriers)
         const double rr = sum_partials(rr_part);
         if (threadIdx.x == 0) *hist_k = sqrt(rr);
     }
-    constexpr int UNR = 4;
+    constexpr int UNR = 2; // three streams x 2 loads in flight
     const long long stride = (long long)RED_BLOCKS * RED_THREADS;
     for (long long i0 = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i0 < nvec; i0 += UNR * stride) {
-        Vec pv[UNR], zv[UNR];
+        Vec pv[UNR], zv[UNR], xv[UNR];
 #pragma unroll
         for (int u = 0; u < UNR; ++u) {
             const long long i = i0 + u * stride;
-            if (i < nvec) { pv[u] = p[i]; zv[u] = z[i]; }
+            if (i < nvec) { pv[u] = p[i]; zv[u] = z[i]; xv[u] = x[i]; }
         }
 #pragma unroll
         for (int u = 0; u < UNR; ++u) {
             const long long i = i0 + u * stride;
-            if (i < nvec) p[i] = axpy_vec(beta, pv[u], zv[u]);
+            if (i < nvec) {
+                x[i] = axpy_vec(alpha, pv[u], xv[u]);
+                p[i] = axpy_vec(beta, pv[u], zv[u]);
+            }
         }
     }
 }
@@ -200,11 +218,11 @@ __device__ __forceinline__ cplxd cdiv(cplxd a, cplxd b)
     if (d == 0.0) return {0.0, 0.0}; // breakdown guard (see safe_div)
     return {(a.re * b.re + a.im * b.im) / d, (a.im * b.re - a.re * b.im) / d};
 }
-__device__ __forceinline__ cplxd sum_partials_c(const double *part) // part[0..RED) = re, part[RED..2 RED) = im
+__device__ __forceinline__ cplxd sum_partials_c(const double *part, int n = RED_BLOCKS) // part[0..n) = re, part[n..2n) = im
 {
     cplxd r;
-    r.re = sum_partials(part);
-    r.im = sum_partials(part + RED_BLOCKS);
+    r.re = sum_partials(part, n);
+    r.im = sum_partials(part + n, n);
     return r;
 }
 
@@ -281,9 +299,9 @@ bicg_p_kernel(Vec *__restrict__ p, const Vec *__restrict__ r, const Vec *__restr
 // alpha = rho' / <rhat, v>;  s = r - alpha v  (s overwrites r);  block 0 stores alpha and rho <- rho'
 template <typename Vec>
 __global__ void __launch_bounds__(RED_THREADS)
-bicg_s_kernel(Vec *__restrict__ r, const Vec *__restrict__ v, long long nvec, const double *rv_part, cplxd *scal)
+bicg_s_kernel(Vec *__restrict__ r, const Vec *__restrict__ v, long long nvec, const double *rv_part, int npart, cplxd *scal)
 {
-    const cplxd alpha = cdiv(scal[3], sum_partials_c(rv_part));
+    const cplxd alpha = cdiv(scal[3], sum_partials_c(rv_part, npart)); // <rhat, v> from the epilogue of the matvec that made v
     const cplxd ma = {-alpha.re, -alpha.im};
     for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS)
         r[i] = caxpy_vec(ma, v[i], r[i]);
@@ -293,28 +311,43 @@ bicg_s_kernel(Vec *__restrict__ r, const Vec *__restrict__ v, long long nvec, co
     }
 }
 
-// omega = <t, s> / <t, t>;  x += alpha p + omega s;  r = s - omega t (s lives in r);  |r|^2 partials; block 0 stores omega
+// omega = <t, s> / <t, t>;  x += alpha p + omega s;  r = s - omega t (s lives in r);  |r|^2 partials; block 0 stores omega.
+// st_part = per-CTA partials of <s, t> from the epilogue of the matvec that made t (<t, s> is its conjugate), tt_part those
+// of |t|^2; rho_part receives the partials of <rhat, r> for the next iteration (rhat is read here instead of in a kernel
+// of its own)
 template <typename Vec, int NCH>
 __global__ void __launch_bounds__(RED_THREADS)
-bicg_x_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict__ p, const Vec *__restrict__ t, long long nvec,
-              long long Vh, const double *ts_part, const double *tt_part, cplxd *scal, double *rr_part)
+bicg_x_kernel(Vec *__restrict__ x, Vec *__restrict__ r, const Vec *__restrict__ p, const Vec *__restrict__ t,
+              const Vec *__restrict__ rhat, long long nvec, long long Vh, const double *st_part, const double *tt_part, int npart,
+              cplxd *scal, double *rr_part, double *rho_part)
 {
     __shared__ double sh[RED_THREADS / 32];
-    const cplxd ts = sum_partials_c(ts_part);
-    const double tt = sum_partials(tt_part);
-    const cplxd omega = {safe_div(ts.re, tt), safe_div(ts.im, tt)};
+    const cplxd st = sum_partials_c(st_part, npart);
+    const double tt = sum_partials(tt_part, npart);
+    const cplxd omega = {safe_div(st.re, tt), safe_div(-st.im, tt)};
     const cplxd alpha = scal[1];
     const cplxd mo = {-omega.re, -omega.im};
-    double s2 = 0.0;
+    double s2 = 0.0, re = 0.0, im = 0.0;
     for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) {
         const Vec sv = r[i];
         x[i] = caxpy_vec(omega, sv, caxpy_vec(alpha, p[i], x[i]));
         const Vec rn = caxpy_vec(mo, t[i], sv);
         r[i] = rn;
-        if (real_site<NCH>(i, Vh)) s2 += norm2_vec(rn);
+        if (real_site<NCH>(i, Vh)) {
+            s2 += norm2_vec(rn);
+            cdot_vec(rhat[i], rn, re, im);
+        }
     }
     s2 = block_sum(s2, sh);
-    if (threadIdx.x == 0) rr_part[blockIdx.x] = s2;
+    __syncthreads();
+    re = block_sum(re, sh);
+    __syncthreads();
+    im = block_sum(im, sh);
+    if (threadIdx.x == 0) {
+        rr_part[blockIdx.x] = s2;
+        rho_part[blockIdx.x] = re;
+        rho_part[RED_BLOCKS + blockIdx.x] = im;
+    }
     if (blockIdx.x == 0 && threadIdx.x == 0) scal[2] = omega;
 }
 
@@ -404,10 +437,11 @@ static int cgnr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const 
         }
         for (k = 0; k < max_iter; ++k) {
             if ((e = schur(w, p, false, ww_part)) != cudaSuccess) { fail_cuda(e); break; }
-            update_xr_kernel<Vec, NCH><<<vgrid, RED_THREADS, 0, s>>>(x, r, p, w, nvec, Vh, zz_part[cur], ww_part, npart, rr_part);
+            update_r_kernel<Vec, NCH><<<vgrid, RED_THREADS, 0, s>>>(r, w, nvec, Vh, zz_part[cur], ww_part, npart, rr_part);
             count_launch();
             if ((e = schur(z, r, true, zz_part[cur ^ 1])) != cudaSuccess) { fail_cuda(e); break; }
-            update_p_kernel<Vec><<<vgrid, RED_THREADS, 0, s>>>(p, z, nvec, zz_part[cur ^ 1], zz_part[cur], npart, rr_part, hist + k + 1, hs);
+            update_px_kernel<Vec><<<vgrid, RED_THREADS, 0, s>>>(x, p, z, nvec, zz_part[cur ^ 1], zz_part[cur], ww_part, npart, rr_part,
+                                                                 hist + k + 1, hs);
             count_launch();
             cur ^= 1;
             if (tol > 0.0 && ((k + 1) % CHECK == 0 || k + 1 == max_iter)) {
@@ -473,27 +507,29 @@ static int bicgstab_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, co
     const size_t hb = (size_t)nvec * sizeof(Vec);
     cudaStream_t s = shape.stream;
     const double a0 = 4.0 + mass;
-    const size_t nsc = 8 * (size_t)RED_BLOCKS + 8 + (size_t)max_iter + 1;
+    const int npart = (int)((Vh + 127) / 128); // per-CTA partials of the matvec epilogues
+    const size_t nsc = 3 * (size_t)RED_BLOCKS + 5 * (size_t)npart + 8 + (size_t)max_iter + 1;
     if ((*err = ensure_workspace(g, 6 * hb, nsc)) != cudaSuccess) return -1;
     char *ws = (char *)g->cg_ws;
     Vec *r = (Vec *)ws, *rhat = (Vec *)(ws + hb), *p = (Vec *)(ws + 2 * hb), *v = (Vec *)(ws + 3 * hb), *t = (Vec *)(ws + 4 * hb),
         *tmp = (Vec *)(ws + 5 * hb);
     Vec *x = (Vec *)x_out;
     double *sc = g->cg_sc;
-    double *rho_part = sc, *rv_part = sc + 2 * RED_BLOCKS, *ts_part = sc + 4 * RED_BLOCKS, *tt_part = sc + 6 * RED_BLOCKS,
-           *rr_part = sc + 7 * RED_BLOCKS;
-    cplxd *scal = (cplxd *)(sc + 8 * RED_BLOCKS);
-    double *hist = sc + 8 * RED_BLOCKS + 8;
+    double *rho_part = sc, *rr_part = sc + 2 * RED_BLOCKS, *rv_part = sc + 3 * RED_BLOCKS, *st_part = rv_part + 2 * (size_t)npart,
+           *tt_part = st_part + 2 * (size_t)npart;
+    cplxd *scal = (cplxd *)(tt_part + npart);
+    double *hist = (double *)(scal + 4);
 
     ApplyArgs a = shape;
-    auto schur = [&](Vec *out, const Vec *in) -> cudaError_t {
+    // out = Mhat in; the second launch also leaves the per-CTA partials of <y, out> in dot_part and of |out|^2 in norm_part
+    auto schur = [&](Vec *out, const Vec *in, const Vec *y, double *dot_part, double *norm_part) -> cudaError_t {
         a.out = tmp;
         a.in = in;
         cudaError_t e = launch_eo(a, nullptr, 0.0, -0.5, 1 - parity, false);
         if (e != cudaSuccess) return e;
         a.out = out;
         a.in = tmp;
-        return launch_eo(a, in, a0, 0.5 / a0, parity, false);
+        return launch_eo(a, in, a0, 0.5 / a0, parity, false, norm_part, y, dot_part);
     };
     int rc = 0, k = 0;
     double h0 = 0.0;
@@ -518,18 +554,20 @@ static int bicgstab_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, co
             if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { fail_cuda(e); break; }
             if (h0 == 0.0) break;
         }
+        // rho_0 = <rhat, r_0>; every later rho comes out of bicg_x_kernel, <rhat, v>, <s, t> and |t|^2 out of the matvec
+        // epilogues: 7 launches and 15 spinor passes per iteration (10 and 19 with separate inner-product kernels)
+        cdot_kernel<Vec, NCH, false><<<RED_BLOCKS, RED_THREADS, 0, s>>>(rhat, r, nvec, Vh, rho_part, nullptr);
+        count_launch();
         for (k = 0; k < max_iter; ++k) {
-            cdot_kernel<Vec, NCH, false><<<RED_BLOCKS, RED_THREADS, 0, s>>>(rhat, r, nvec, Vh, rho_part, nullptr);
             bicg_p_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(p, r, v, nvec, rho_part, scal, rr_part, hist + k);
-            count_launch(2);
-            if ((e = schur(v, p)) != cudaSuccess) { fail_cuda(e); break; }
-            cdot_kernel<Vec, NCH, false><<<RED_BLOCKS, RED_THREADS, 0, s>>>(rhat, v, nvec, Vh, rv_part, nullptr);
-            bicg_s_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(r, v, nvec, rv_part, scal);
-            count_launch(2);
-            if ((e = schur(t, r)) != cudaSuccess) { fail_cuda(e); break; }
-            cdot_kernel<Vec, NCH, true><<<RED_BLOCKS, RED_THREADS, 0, s>>>(t, r, nvec, Vh, ts_part, tt_part);
-            bicg_x_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, r, p, t, nvec, Vh, ts_part, tt_part, scal, rr_part);
-            count_launch(2);
+            count_launch();
+            if ((e = schur(v, p, rhat, rv_part, nullptr)) != cudaSuccess) { fail_cuda(e); break; }
+            bicg_s_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(r, v, nvec, rv_part, npart, scal);
+            count_launch();
+            if ((e = schur(t, r, r, st_part, tt_part)) != cudaSuccess) { fail_cuda(e); break; }
+            bicg_x_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, r, p, t, rhat, nvec, Vh, st_part, tt_part, npart, scal, rr_part,
+                                                                      rho_part);
+            count_launch();
             if (tol > 0.0 && ((k + 1) % CHECK == 0 || k + 1 == max_iter)) {
                 double hk = 0.0;
                 sqrt_of_sum_kernel<<<1, 32, 0, s>>>(rr_part, hist + k + 1);
@@ -568,18 +606,87 @@ int bicgstab_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, 
 }
 
 // ---- GCR(m) pieces ----
-// beta = <q_i, q_j> / qq_i;  p_j -= beta p_i;  q_j -= beta q_i
-template <typename Vec>
+constexpr int GCR_GROUP = 8; // earlier directions handled per pass over the new one (GCR(8): all of them)
+
+// part[(2 i + c) * RED_BLOCKS + b] = partials of <q_{i0+i}, q_j> (c = 0 real, 1 imaginary part), i < ni <= GCR_GROUP:
+// q_j is read once for all of them.  q_i = qbase + i * stride
+template <typename Vec, int NCH>
 __global__ void __launch_bounds__(RED_THREADS)
-gcr_orth_kernel(Vec *__restrict__ pj, Vec *__restrict__ qj, const Vec *__restrict__ pi, const Vec *__restrict__ qi, long long nvec,
-                const double *dot_part, const double *qq_i)
+gcr_dots_kernel(const Vec *__restrict__ qbase, long long stride, int i0, int ni, const Vec *__restrict__ qj, long long nvec,
+                long long Vh, double *part)
 {
-    const cplxd d = sum_partials_c(dot_part);
-    const double qq = *qq_i;
-    const cplxd mb = {-safe_div(d.re, qq), -safe_div(d.im, qq)};
-    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < nvec; i += (long long)RED_BLOCKS * RED_THREADS) {
-        pj[i] = caxpy_vec(mb, pi[i], pj[i]);
-        qj[i] = caxpy_vec(mb, qi[i], qj[i]);
+    __shared__ double sh[RED_THREADS / 32];
+    double re[GCR_GROUP], im[GCR_GROUP];
+#pragma unroll
+    for (int i = 0; i < GCR_GROUP; ++i) re[i] = im[i] = 0.0;
+    for (long long k = (long long)blockIdx.x * RED_THREADS + threadIdx.x; k < nvec; k += (long long)RED_BLOCKS * RED_THREADS)
+        if (real_site<NCH>(k, Vh)) {
+            const Vec b = qj[k];
+#pragma unroll
+            for (int i = 0; i < GCR_GROUP; ++i)
+                if (i < ni) cdot_vec(qbase[(i0 + i) * stride + k], b, re[i], im[i]);
+        }
+#pragma unroll
+    for (int i = 0; i < GCR_GROUP; ++i)
+        if (i < ni) { // (ni is uniform: the barriers inside block_sum are reached by every thread)
+            double v = block_sum(re[i], sh);
+            if (threadIdx.x == 0) part[(2 * i) * RED_BLOCKS + blockIdx.x] = v;
+            __syncthreads();
+            v = block_sum(im[i], sh);
+            if (threadIdx.x == 0) part[(2 * i + 1) * RED_BLOCKS + blockIdx.x] = v;
+            __syncthreads();
+        }
+}
+
+// beta_i = <q_i, q_j> / qq_i for the ni directions from i0;  p_j = psrc - sum beta_i p_i;  q_j -= sum beta_i q_i: one pass
+// over p_j and q_j for the whole group.  The inner products were all taken with the q_j that entered the group
+// (classical Gram-Schmidt inside a group; the q_i are mutually orthogonal, so in exact arithmetic this is the modified
+// form the oracle writes out).  psrc may be p_j itself, or r for an unpreconditioned direction (p_j = r needs no copy).
+// FINAL (the last group): also the partials of <q_j, r> and |q_j|^2 of the finished direction.
+template <typename Vec, int NCH, bool FINAL>
+__global__ void __launch_bounds__(RED_THREADS)
+gcr_orth_kernel(Vec *pj, const Vec *psrc, Vec *__restrict__ qj, const Vec *__restrict__ pbase, const Vec *__restrict__ qbase,
+                long long stride, int i0, int ni, long long nvec, long long Vh, const double *part, const double *qq,
+                const Vec *__restrict__ r, double *qr_part, double *qq_part)
+{
+    __shared__ double sh[RED_THREADS / 32];
+    cplxd mb[GCR_GROUP];
+#pragma unroll
+    for (int i = 0; i < GCR_GROUP; ++i) {
+        mb[i] = {0.0, 0.0};
+        if (i < ni) {
+            const cplxd d = sum_partials_c(part + (size_t)(2 * i) * RED_BLOCKS);
+            const double q2 = qq[i0 + i];
+            mb[i] = {-safe_div(d.re, q2), -safe_div(d.im, q2)};
+        }
+    }
+    double re = 0.0, im = 0.0, q2 = 0.0;
+    for (long long k = (long long)blockIdx.x * RED_THREADS + threadIdx.x; k < nvec; k += (long long)RED_BLOCKS * RED_THREADS) {
+        Vec pv = psrc[k], qv = qj[k];
+#pragma unroll
+        for (int i = 0; i < GCR_GROUP; ++i)
+            if (i < ni) {
+                pv = caxpy_vec(mb[i], pbase[(i0 + i) * stride + k], pv);
+                qv = caxpy_vec(mb[i], qbase[(i0 + i) * stride + k], qv);
+            }
+        pj[k] = pv;
+        qj[k] = qv;
+        if (FINAL && real_site<NCH>(k, Vh)) {
+            cdot_vec(qv, r[k], re, im);
+            q2 += norm2_vec(qv);
+        }
+    }
+    if (FINAL) {
+        re = block_sum(re, sh);
+        __syncthreads();
+        im = block_sum(im, sh);
+        __syncthreads();
+        q2 = block_sum(q2, sh);
+        if (threadIdx.x == 0) {
+            qr_part[blockIdx.x] = re;
+            qr_part[RED_BLOCKS + blockIdx.x] = im;
+            qq_part[blockIdx.x] = q2;
+        }
     }
 }
 
@@ -623,7 +730,7 @@ static int gcr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const v
     const size_t hb = (size_t)nvec * sizeof(Vec);
     cudaStream_t s = shape.stream;
     const double a0 = 4.0 + mass;
-    const size_t nsc = 6 * (size_t)RED_BLOCKS + (size_t)restart + (size_t)max_iter + 1;
+    const size_t nsc = (2 * GCR_GROUP + 4) * (size_t)RED_BLOCKS + (size_t)restart + (size_t)max_iter + 1;
     if ((*err = ensure_workspace(g, (size_t)(2 * restart + 2) * hb, nsc)) != cudaSuccess) return -1;
     char *ws = (char *)g->cg_ws;
     Vec *r = (Vec *)ws, *tmp = (Vec *)(ws + hb);
@@ -631,8 +738,8 @@ static int gcr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const v
     auto Q = [&](int j) { return (Vec *)(ws + (size_t)(2 + restart + j) * hb); };
     Vec *x = (Vec *)x_out;
     double *sc = g->cg_sc;
-    double *dot_part = sc, *qr_part = sc + 2 * RED_BLOCKS, *qq_part = sc + 4 * RED_BLOCKS, *rr_part = sc + 5 * RED_BLOCKS;
-    double *qq = sc + 6 * RED_BLOCKS, *hist = qq + restart;
+    double *dot_part = sc, *qr_part = sc + 2 * GCR_GROUP * RED_BLOCKS, *qq_part = qr_part + 2 * RED_BLOCKS, *rr_part = qq_part + RED_BLOCKS;
+    double *qq = rr_part + RED_BLOCKS, *hist = qq + restart;
 
     ApplyArgs a = shape;
     auto schur = [&](Vec *out, const Vec *in) -> cudaError_t {
@@ -664,16 +771,32 @@ static int gcr_schur_t(wd_gauge *g, const ApplyArgs &shape, void *x_out, const v
         }
         for (k = 0; k < max_iter; ++k) {
             const int j = k % restart;
+            // the new direction: K r (written to P(j) by the caller's function) or r itself (copied into P(j) by the
+            // orthogonalisation pass, or by a plain copy when there is nothing to orthogonalise against)
+            const Vec *psrc = r;
             if (precond) {
                 if (precond(ctx, P(j), r, (void *)s) != 0) { fail_cuda(cudaErrorUnknown); break; }
-            } else if ((e = cudaMemcpyAsync(P(j), r, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
-            if ((e = schur(Q(j), P(j))) != cudaSuccess) { fail_cuda(e); break; }
-            for (int i = 0; i < j; ++i) { // modified Gram-Schmidt against the cycle's earlier directions
-                cdot_kernel<Vec, NCH, false><<<RED_BLOCKS, RED_THREADS, 0, s>>>(Q(i), Q(j), nvec, Vh, dot_part, nullptr);
-                gcr_orth_kernel<Vec><<<RED_BLOCKS, RED_THREADS, 0, s>>>(P(j), Q(j), P(i), Q(i), nvec, dot_part, qq + i);
+                psrc = P(j);
+            }
+            if ((e = schur(Q(j), psrc)) != cudaSuccess) { fail_cuda(e); break; }
+            if (j == 0) {
+                if (!precond && (e = cudaMemcpyAsync(P(0), r, hb, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) { fail_cuda(e); break; }
+                cdot_kernel<Vec, NCH, true><<<RED_BLOCKS, RED_THREADS, 0, s>>>(Q(0), r, nvec, Vh, qr_part, qq_part);
+                count_launch();
+            }
+            // Gram-Schmidt against the cycle's earlier directions, GCR_GROUP of them per pass over p_j and q_j; the last
+            // pass also takes <q_j, r> and |q_j|^2
+            for (int i0 = 0; i0 < j; i0 += GCR_GROUP) {
+                const int ni = j - i0 < GCR_GROUP ? j - i0 : GCR_GROUP;
+                gcr_dots_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(Q(0), nvec, i0, ni, Q(j), nvec, Vh, dot_part);
+                if (i0 + ni == j)
+                    gcr_orth_kernel<Vec, NCH, true><<<RED_BLOCKS, RED_THREADS, 0, s>>>(P(j), i0 == 0 ? psrc : P(j), Q(j), P(0), Q(0), nvec, i0, ni,
+                                                                                     nvec, Vh, dot_part, qq, r, qr_part, qq_part);
+                else
+                    gcr_orth_kernel<Vec, NCH, false><<<RED_BLOCKS, RED_THREADS, 0, s>>>(P(j), i0 == 0 ? psrc : P(j), Q(j), P(0), Q(0), nvec, i0, ni,
+                                                                                      nvec, Vh, dot_part, qq, r, qr_part, qq_part);
                 count_launch(2);
             }
-            cdot_kernel<Vec, NCH, true><<<RED_BLOCKS, RED_THREADS, 0, s>>>(Q(j), r, nvec, Vh, qr_part, qq_part);
             gcr_update_kernel<Vec, NCH><<<RED_BLOCKS, RED_THREADS, 0, s>>>(x, r, P(j), Q(j), nvec, Vh, qr_part, qq_part, qq + j, rr_part);
             sqrt_of_sum_kernel<<<1, 32, 0, s>>>(rr_part, hist + k + 1);
             count_launch(3);

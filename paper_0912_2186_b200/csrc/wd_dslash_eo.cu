@@ -30,7 +30,8 @@ template <typename T, int RECON, int SGN>
 __global__ void __launch_bounds__(EO_THREADS)
 dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ xin, const T *__restrict__ links_p,
                  const T *__restrict__ links_q,
-                 int Lx, int Ly, int Lz, int Lt, long long Vh, T alpha, T beta, int parity, double *__restrict__ norm_part, int nrhs)
+                 int Lx, int Ly, int Lz, int Lt, long long Vh, T alpha, T beta, int parity, double *__restrict__ norm_part, int nrhs,
+                 const T *__restrict__ dot_y, double *__restrict__ dot_part)
 {
     // gridDim.x = (site blocks) * nrhs with the right-hand side FASTEST: the CTAs resident at any time are all right-hand
     // sides of a few site blocks, so the links of a block come from HBM once and from L1/L2 for the others
@@ -40,7 +41,7 @@ dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restr
     // the result without another pass over it (wd_cg.cu)
     const long long cb_raw = blk * EO_THREADS + threadIdx.x;
     const bool valid = cb_raw < Vh;
-    if (!valid && !norm_part) return;
+    if (!valid && !norm_part && !dot_part) return;
     const long long cb = valid ? cb_raw : Vh - 1; // (only the last CTA has such threads; they redo a site and drop it)
     const long long Vhp = padded_volume(Vh); // sites per right-hand side of a half field
     in += (long long)rhs * 24 * Vhp;
@@ -101,12 +102,42 @@ dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restr
             norm_part[(long long)rhs * nblk + blk] = t;
         }
     }
+    // dot_part (may be NULL; one right-hand side): per-CTA partials of <y, out> = sum conj(y) out over the sites, real parts in
+    // [0, nblk), imaginary parts in [nblk, 2 nblk) -- the inner products BiCGstab takes with the result of a matvec
+    if (dot_part) {
+        __shared__ double shd[2][EO_THREADS / 32];
+        double re = 0.0, im = 0.0;
+        if (valid) {
+            load_spinor(dot_y, cb, p);
+#pragma unroll
+            for (int i = 0; i < 24; i += 2) {
+                re += (double)p[i] * acc[i] + (double)p[i + 1] * acc[i + 1];
+                im += (double)p[i] * acc[i + 1] - (double)p[i + 1] * acc[i];
+            }
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            re += __shfl_down_sync(0xffffffffu, re, o);
+            im += __shfl_down_sync(0xffffffffu, im, o);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            shd[0][threadIdx.x >> 5] = re;
+            shd[1][threadIdx.x >> 5] = im;
+        }
+        __syncthreads();
+        if (threadIdx.x < 2) {
+            double t = 0.0;
+#pragma unroll
+            for (int i = 0; i < EO_THREADS / 32; ++i) t += shd[threadIdx.x][i];
+            dot_part[threadIdx.x * nblk + blk] = t;
+        }
+    }
 }
 
 template <typename T, int RECON>
 static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger,
-                               double *norm_part)
+                               double *norm_part, const void *dot_y, double *dot_part)
 {
+    if (dot_part && (a.nrhs != 1 || !dot_y)) return cudaErrorInvalidValue;
     const long long Vh = a.V / 2;
     const long long nb = (Vh + EO_THREADS - 1) / EO_THREADS;
     if (nb * a.nrhs > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
@@ -117,23 +148,25 @@ static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha
     const size_t half = eo_links_half_bytes(a.V, a.precision, a.recon);
     kern<<<grid, EO_THREADS, 0, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)xin, (const T *)(le + parity * half),
                                              (const T *)(le + (1 - parity) * half), a.dims[0],
-                                             a.dims[1], a.dims[2], a.dims[3], Vh, (T)alpha, (T)beta, parity, norm_part, a.nrhs);
+                                             a.dims[1], a.dims[2], a.dims[3], Vh, (T)alpha, (T)beta, parity, norm_part, a.nrhs,
+                                             (const T *)dot_y, dot_part);
     count_launch();
     return cudaGetLastError();
 }
 
 // out_p = alpha * xin_p + beta * (sum of the eight projected, link-multiplied hops from parity 1-p); xin may be NULL
 // norm_part: NULL, or ceil(Vh / 128) * nrhs doubles that receive per-CTA partial sums of |out|^2
+// dot_part:  NULL, or 2 * ceil(Vh / 128) doubles that receive per-CTA partial sums of <dot_y, out> (nrhs = 1)
 cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger,
-                      double *norm_part)
+                      double *norm_part, const void *dot_y, double *dot_part)
 {
     if (a.precision == 32)
-        return a.recon == 18 ? launch_eo_t<float, 18>(a, xin, alpha, beta, parity, dagger, norm_part)
-               : a.recon == 12 ? launch_eo_t<float, 12>(a, xin, alpha, beta, parity, dagger, norm_part)
-                               : launch_eo_t<float, 8>(a, xin, alpha, beta, parity, dagger, norm_part);
-    return a.recon == 18 ? launch_eo_t<double, 18>(a, xin, alpha, beta, parity, dagger, norm_part)
-           : a.recon == 12 ? launch_eo_t<double, 12>(a, xin, alpha, beta, parity, dagger, norm_part)
-                           : launch_eo_t<double, 8>(a, xin, alpha, beta, parity, dagger, norm_part);
+        return a.recon == 18 ? launch_eo_t<float, 18>(a, xin, alpha, beta, parity, dagger, norm_part, dot_y, dot_part)
+               : a.recon == 12 ? launch_eo_t<float, 12>(a, xin, alpha, beta, parity, dagger, norm_part, dot_y, dot_part)
+                               : launch_eo_t<float, 8>(a, xin, alpha, beta, parity, dagger, norm_part, dot_y, dot_part);
+    return a.recon == 18 ? launch_eo_t<double, 18>(a, xin, alpha, beta, parity, dagger, norm_part, dot_y, dot_part)
+           : a.recon == 12 ? launch_eo_t<double, 12>(a, xin, alpha, beta, parity, dagger, norm_part, dot_y, dot_part)
+                           : launch_eo_t<double, 8>(a, xin, alpha, beta, parity, dagger, norm_part, dot_y, dot_part);
 }
 
 // ---- parity-ordered link records (pure data movement) ----

@@ -105,7 +105,7 @@ size_t eo_links_half_bytes(long long V, int precision, int recon);
 cudaError_t launch_links_to_eo(void *links_eo, const void *links, const int dims[4], long long V, int precision, int recon,
                                cudaStream_t s);
 cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger = false,
-                      double *norm_part = nullptr);
+                      double *norm_part = nullptr, const void *dot_y = nullptr, double *dot_part = nullptr);
 // CGNR for Mhat x = b on one parity (wd_cg.cu); shape carries dims, V, precision, recon, links, stream
 int cgnr_schur(wd_gauge *g, const ApplyArgs &shape, void *x, const void *b, double mass, int parity, int max_iter,
                double tol, int *iters_out, double *hist_host, cudaError_t *err);
