@@ -140,7 +140,7 @@ def test_bicgstab_converges_to_the_solution(oracle):
 
 @pytest.mark.parametrize("dims,parity", [((4, 4, 4, 4), 0), ((8, 4, 6, 2), 1), ((16, 8, 8, 8), 0)])
 @pytest.mark.parametrize("precision,recon,tol_x", [(64, 18, 1e-10), (64, 12, 1e-10), (32, 18, 2e-4), (32, 12, 2e-4)])
-@pytest.mark.parametrize("restart", [8, 3])
+@pytest.mark.parametrize("restart", [8, 3, 11])  # 11: two groups of the grouped Gram-Schmidt (8 + up to 2)
 def test_gcr_fixed_iterations_match_the_oracle(oracle, dims, parity, precision, recon, tol_x, restart):
     """K = 13 iterations of GCR(restart): more than one restart cycle.  Same derived bounds as CGNR (orthogonal
     projections, well-conditioned system)."""
