@@ -594,21 +594,23 @@ def run_schur(args):
     cfg = fields.CONFIGS[args.workload]
     recon, nrhs = args.recon, cfg.nrhs
     V = fields.volume(cfg.dims)
-    w = 4 if cfg.precision == 32 else 8
-    tdt = torch.float32 if cfg.precision == 32 else torch.float64
+    if args.half and cfg.precision != 32:
+        raise SystemExit("bench.py --op schur --half: half storage has float32 canonical fields; use an fp32 workload")
+    prec = 16 if args.half else cfg.precision  # --half: binary16 storage, fp32 arithmetic (row f4 on the operator of row f1)
+    w = {16: 2, 32: 4, 64: 8}[prec]
+    tdt = {16: torch.float16, 32: torch.float32, 64: torch.float64}[prec]
     U, psi = fields.make_fields(rank_config(cfg, recon, nrhs, rank))
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
         u_dev = torch.from_numpy(U).to(dev)
-        op = binding.WilsonDirac(cfg.dims, u_dev, cfg.precision, recon, stream=stream.cuda_stream)
+        op = binding.WilsonDirac(cfg.dims, u_dev, prec, recon, stream=stream.cuda_stream)
         canon = torch.from_numpy(psi).to(dev)
         n = op.half_numel(nrhs)
         ins = [torch.empty(n, dtype=tdt, device=dev) for _ in range(NBUF)]
         outs = [torch.empty(n, dtype=tdt, device=dev) for _ in range(NBUF)]
         tmp = torch.empty(n, dtype=tdt, device=dev)
-        op.pack_parity(ins[0], canon, nrhs, 0)
-        for b in range(1, NBUF):
-            torch.mul(ins[0], 1.0 + 0.25 * b, out=ins[b])
+        for b in range(NBUF):  # (half storage holds ratios and scales: every input is packed, not scaled in place)
+            op.pack_parity(ins[b], canon * (1.0 + 0.25 * b), nrhs, 0)
     stream.synchronize()
     aps = args.applies_per_step
 
@@ -630,12 +632,14 @@ def run_schur(args):
     ms = ev0.elapsed_time(ev1)
     applies = args.steps * aps
     flops = (2 * 1320 + 48) * (V // 2) * nrhs
-    bytes_per_apply = (V // 2) * (2 * 2 * 4 * recon * w + nrhs * 5 * 24 * w)
+    spinor_b = 52 if prec == 16 else 24 * w  # half storage: 24 binary16 ratios + a float32 scale per site
+    bytes_per_apply = (V // 2) * (2 * 2 * 4 * recon * w + nrhs * 5 * spinor_b)
     peak, peak_src = measured_peak()
     achieved = bytes_per_apply * applies / (ms * 1e-3) / 1e9
     line = {"metric": "wilson_schur_gflops", "value": applies * flops / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if cfg.precision == 32 else "f64", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": {16: "f32 arithmetic on f16 storage", 32: "f32", 64: "f64"}[prec], "data": "synthetic",
             "config": {"workload": cfg.name, "op": "even-odd preconditioned operator (2 launches per apply)",
                        "dims": list(cfg.dims), "recon": recon, "nrhs": nrhs, "mass": cfg.mass, "applies_per_step": aps,
                        "flops_per_even_site": 2 * 1320 + 48,

@@ -67,7 +67,10 @@ typedef enum {
  * and the 24 ratios component / s as binary16 (value = s * ratio) -- 52 bytes per site and right-hand side.  With
  * WD_FP16 the CANONICAL buffers of wd_load_gauge / wd_pack_spinor / wd_unpack_spinor are float32; it is accepted by
  * wd_create_lattice .. wd_spinor_bytes, wd_load_gauge, wd_pack_spinor, wd_unpack_spinor, wd_apply and wd_apply_dagger
- * (one-thread-per-site kernel, any extents, any nrhs); every other entry point answers WD_ERR_PRECISION. */
+ * (one-thread-per-site kernel for any extents and nrhs, staged kernel where the lattice can be tiled), and by the
+ * red/black family wd_spinor_bytes_parity, wd_pack_spinor_parity, wd_unpack_spinor_parity, wd_apply_hop, wd_apply_schur,
+ * wd_apply_schur_dagger (the operator of the paper's "Half" kernel row; the intermediate field of the two launches is a
+ * half-storage field too); every other entry point (solvers, transfer and coarse operators) answers WD_ERR_PRECISION. */
 typedef enum { WD_FP16 = 16, WD_FP32 = 32, WD_FP64 = 64 } wd_precision;
 typedef enum { WD_RECON_18 = 18, WD_RECON_12 = 12, WD_RECON_8 = 8 } wd_recon; /* reals stored per link */
 

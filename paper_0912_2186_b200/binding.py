@@ -410,8 +410,9 @@ class WilsonDirac:
 
     # ---- red/black (even-odd) blocks: half fields of one parity ----
     def half_numel(self, nrhs=1):
-        """Reals in a native HALF field (one parity) of nrhs right-hand sides; 0 if an extent is odd."""
-        return wd_spinor_bytes_parity(self.lat, nrhs, self.precision) // (4 if self.precision == 32 else 8)
+        """Elements (float16 / float32 / float64 by precision) of a native HALF field (one parity) of nrhs right-hand
+        sides; 0 if an extent is odd."""
+        return wd_spinor_bytes_parity(self.lat, nrhs, self.precision) // {16: 2, 32: 4, 64: 8}[self.precision]
 
     def pack_parity(self, native_half_dev, canonical_dev, nrhs, parity, stream=None):
         wd_pack_spinor_parity(self.lat, native_half_dev, canonical_dev, nrhs, self.precision, parity, stream or self.stream)

@@ -67,7 +67,7 @@ int check_apply_args(const void *out, const void *in, const wd_gauge *g, const i
     if (g->magic != GAUGE_MAGIC) return fail(WD_ERR_MISMATCH, "wd_apply: not a live wd_gauge handle");
     if (!valid_storage(precision)) return fail(WD_ERR_PRECISION, "wd_apply: precision %d is not 16, 32 or 64", precision);
     if (precision == WD_FP16 && !allow_half)
-        return fail(WD_ERR_PRECISION, "half-precision storage is taken by wd_apply / wd_apply_dagger only");
+        return fail(WD_ERR_PRECISION, "half-precision storage is taken by wd_apply, wd_apply_dagger, wd_apply_hop and wd_apply_schur* only");
     if (precision != g->precision)
         return fail(WD_ERR_PRECISION, "wd_apply: precision %d but gauge was loaded in %d", precision, g->precision);
     for (int d = 0; d < 4; ++d)
@@ -623,12 +623,13 @@ static bool all_even(const int dims[4])
 
 static size_t half_bytes(long long V, int nrhs, int precision)
 {
+    if (precision == WD_FP16) return (size_t)nrhs * (size_t)wd::padded_volume(V / 2) * 52; // 3 vectors of 8 halves + a float scale
     return (size_t)nrhs * (size_t)wd::padded_volume(V / 2) * 24 * (precision == WD_FP32 ? 4 : 8);
 }
 
 size_t wd_spinor_bytes_parity(const wd_lattice *lat, int nrhs, int precision)
 {
-    if (!lat || lat->magic != LATTICE_MAGIC || nrhs < 1 || !valid_precision(precision) || !all_even(lat->dims)) return 0;
+    if (!lat || lat->magic != LATTICE_MAGIC || nrhs < 1 || !valid_storage(precision) || !all_even(lat->dims)) return 0;
     return half_bytes(lat->V, nrhs, precision);
 }
 
@@ -637,14 +638,16 @@ static int parity_copy(const char *who, const wd_lattice *lat, void *native, voi
 {
     if (!lat || !native || !canon) return fail(WD_ERR_NULL, "%s: NULL argument", who);
     if (lat->magic != LATTICE_MAGIC) return fail(WD_ERR_MISMATCH, "%s: not a live wd_lattice handle", who);
-    if (!valid_precision(precision)) return fail(WD_ERR_PRECISION, "%s: precision %d is not 32 or 64", who, precision);
+    if (!valid_storage(precision)) return fail(WD_ERR_PRECISION, "%s: precision %d is not 16, 32 or 64", who, precision);
     if (nrhs < 1) return fail(WD_ERR_NRHS, "%s: nrhs=%d", who, nrhs);
     if (!all_even(lat->dims)) return fail(WD_ERR_DIMS, "%s: red/black fields need even extents", who);
     if (parity != 0 && parity != 1) return fail(WD_ERR_MISMATCH, "%s: parity %d is not 0 or 1", who, parity);
-    const size_t cbytes = (size_t)nrhs * (size_t)lat->V * 24 * (precision == WD_FP32 ? 4 : 8);
+    const size_t cbytes = (size_t)nrhs * (size_t)lat->V * 24 * canon_real_bytes(precision);
     if (overlap(native, half_bytes(lat->V, nrhs, precision), canon, cbytes)) return fail(WD_ERR_ALIAS, "%s: buffers overlap", who);
-    cudaError_t e = wd::launch_parity_copy(native, canon, lat->dims, lat->V, nrhs, precision, parity, to_native,
-                                           (cudaStream_t)stream);
+    cudaError_t e = precision == WD_FP16
+                        ? wd::launch_parity_copy_half(native, canon, lat->dims, lat->V, nrhs, parity, to_native, (cudaStream_t)stream)
+                        : wd::launch_parity_copy(native, canon, lat->dims, lat->V, nrhs, precision, parity, to_native,
+                                                 (cudaStream_t)stream);
     return e == cudaSuccess ? WD_OK : cuda_fail(e, who);
 }
 
@@ -663,9 +666,9 @@ int wd_unpack_spinor_parity(const wd_lattice *lat, void *canonical_dev, const vo
 }
 
 static int check_eo_args(const char *who, const void *out, const void *in, const wd_gauge *g, const int dims[4], int nrhs,
-                         int precision, int parity)
+                         int precision, int parity, bool allow_half = false)
 {
-    int rc = check_apply_args(out, in, g, dims, nrhs, precision);
+    int rc = check_apply_args(out, in, g, dims, nrhs, precision, allow_half);
     if (rc) return rc;
     if (!all_even(g->dims)) return fail(WD_ERR_DIMS, "%s: red/black blocks need even extents", who);
     if (parity != 0 && parity != 1) return fail(WD_ERR_MISMATCH, "%s: parity %d is not 0 or 1", who, parity);
@@ -696,7 +699,7 @@ static int check_eo_args(const char *who, const void *out, const void *in, const
 int wd_apply_hop(void *out_half_dev, const void *in_half_dev, const wd_gauge *gauge, const int dims[4], int nrhs,
                  int precision, int parity_out)
 {
-    int rc = check_eo_args("wd_apply_hop", out_half_dev, in_half_dev, gauge, dims, nrhs, precision, parity_out);
+    int rc = check_eo_args("wd_apply_hop", out_half_dev, in_half_dev, gauge, dims, nrhs, precision, parity_out, true);
     if (rc) return rc;
     wd::ApplyArgs a = shape_args(gauge, nrhs);
     a.out = out_half_dev;
@@ -710,7 +713,7 @@ int wd_apply_hop(void *out_half_dev, const void *in_half_dev, const wd_gauge *ga
 static int apply_schur(void *out_half_dev, const void *in_half_dev, void *tmp_half_dev, const wd_gauge *gauge, double mass,
                        const int dims[4], int nrhs, int precision, int parity, bool dagger)
 {
-    int rc = check_eo_args("wd_apply_schur", out_half_dev, in_half_dev, gauge, dims, nrhs, precision, parity);
+    int rc = check_eo_args("wd_apply_schur", out_half_dev, in_half_dev, gauge, dims, nrhs, precision, parity, true);
     if (rc) return rc;
     if (!tmp_half_dev) return fail(WD_ERR_NULL, "wd_apply_schur: NULL tmp");
     const size_t hb = half_bytes(gauge->V, nrhs, precision);

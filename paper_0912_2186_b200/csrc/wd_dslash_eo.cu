@@ -160,6 +160,8 @@ static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha
 cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger,
                       double *norm_part, const void *dot_y, double *dot_part)
 {
+    if (a.precision == 16) // half storage: no epilogues (the solvers do not run on it)
+        return norm_part || dot_part ? cudaErrorInvalidValue : launch_eo_half(a, xin, alpha, beta, parity, dagger);
     if (a.precision == 32)
         return a.recon == 18 ? launch_eo_t<float, 18>(a, xin, alpha, beta, parity, dagger, norm_part, dot_y, dot_part)
                : a.recon == 12 ? launch_eo_t<float, 12>(a, xin, alpha, beta, parity, dagger, norm_part, dot_y, dot_part)
@@ -172,7 +174,7 @@ cudaError_t launch_eo(const ApplyArgs &a, const void *xin, double alpha, double 
 // ---- parity-ordered link records (pure data movement) ----
 size_t eo_links_half_bytes(long long V, int precision, int recon)
 {
-    const size_t nvec = (size_t)recon * (precision == 32 ? 4 : 8) / 4; // 16-byte vectors per site: four links
+    const size_t nvec = (size_t)recon * (size_t)(precision / 8) / 4; // 16-byte vectors per site: four links of `recon` reals
     return (size_t)((V / 2 + BLK - 1) / BLK) * nvec * BLK * 16;
 }
 
@@ -196,7 +198,7 @@ __global__ void links_to_eo_kernel(uint4 *__restrict__ dst, const uint4 *__restr
 cudaError_t launch_links_to_eo(void *links_eo, const void *links, const int dims[4], long long V, int precision, int recon,
                                cudaStream_t s)
 {
-    const int nvec = recon * (precision == 32 ? 4 : 8) / 4;
+    const int nvec = recon * (precision / 8) / 4;
     const long long half_vecs = (long long)(eo_links_half_bytes(V, precision, recon) / 16);
     links_to_eo_kernel<<<(unsigned)((V + 127) / 128), 128, 0, s>>>((uint4 *)links_eo, (const uint4 *)links, dims[0], dims[1], dims[2],
                                                                    V, nvec, half_vecs);

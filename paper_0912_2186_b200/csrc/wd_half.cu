@@ -202,7 +202,137 @@ template <int RECON> cudaError_t launch_half_r(const ApplyArgs &a)
     return cudaGetLastError();
 }
 
+// ---- red/black (even-odd) blocks in half storage: the kernel of wd_dslash_eo.cu with half loads and a requantising
+// store.  Half fields of one parity: the layout above over the checkerboard index cb = lex / 2 (Vh = V / 2 sites); links:
+// the parity-ordered copy of the half link records (wd_gauge::links_eo).
+//     out_p = alpha * x_p + beta * sum_mu [ (1-g_mu) U_mu(x) in_q(x+mu) + (1+g_mu) U_mu(x-mu)^dag in_q(x-mu) ]
+constexpr int EH = 128;
+
+template <int RECON, int SGN>
+__global__ void __launch_bounds__(EH)
+dslash_eo_half_kernel(uint4 *__restrict__ out, float *__restrict__ out_scale, const uint4 *__restrict__ in,
+                      const float *__restrict__ in_scale, const uint4 *__restrict__ xin, const float *__restrict__ xin_scale,
+                      const uint4 *__restrict__ links_p, const uint4 *__restrict__ links_q, int Lx, int Ly, int Lz, int Lt,
+                      long long Vh, float alpha, float beta, int parity)
+{
+    const long long cb = (long long)blockIdx.x * EH + threadIdx.x;
+    if (cb >= Vh) return;
+    const long long Vhp = padded_volume(Vh), rhs = blockIdx.y;
+    in += rhs * Vhp * 3;
+    out += rhs * Vhp * 3;
+    in_scale += rhs * Vhp;
+    out_scale += rhs * Vhp;
+    const int Lxh = Lx / 2;
+    long long rem = cb;
+    const int xh = (int)(rem % Lxh); rem /= Lxh;
+    const int y = (int)(rem % Ly); rem /= Ly;
+    const int z = (int)(rem % Lz);
+    const int t = (int)(rem / Lz);
+    const int x = 2 * xh + ((y + z + t + parity) & 1);
+    const long long sy = Lx, sz = (long long)Lx * Ly, st = (long long)Lx * Ly * Lz;
+    const long long site = x + sy * y + sz * z + st * t;
+    const long long xf = site + (x + 1 == Lx ? -(long long)(Lx - 1) : 1), xb = site + (x == 0 ? (long long)(Lx - 1) : -1);
+    const long long yf = site + (y + 1 == Ly ? -(Ly - 1) * sy : sy), yb = site + (y == 0 ? (Ly - 1) * sy : -sy);
+    const long long zf = site + (z + 1 == Lz ? -(Lz - 1) * sz : sz), zb = site + (z == 0 ? (Lz - 1) * sz : -sz);
+    const long long tf = site + (t + 1 == Lt ? -(Lt - 1) * st : st), tb = site + (t == 0 ? (Lt - 1) * st : -st);
+    float acc[24], u[18], p[24];
+#pragma unroll
+    for (int i = 0; i < 24; ++i) acc[i] = 0.f;
+    load_link_h<0, RECON>(links_p, cb, u);      load_spinor_h(in, in_scale, xf >> 1, p); hop_forward_s<0, SGN>(acc, u, p);
+    load_link_h<0, RECON>(links_q, xb >> 1, u); load_spinor_h(in, in_scale, xb >> 1, p); hop_backward_s<0, SGN>(acc, u, p);
+    load_link_h<1, RECON>(links_p, cb, u);      load_spinor_h(in, in_scale, yf >> 1, p); hop_forward_s<1, SGN>(acc, u, p);
+    load_link_h<1, RECON>(links_q, yb >> 1, u); load_spinor_h(in, in_scale, yb >> 1, p); hop_backward_s<1, SGN>(acc, u, p);
+    load_link_h<2, RECON>(links_p, cb, u);      load_spinor_h(in, in_scale, zf >> 1, p); hop_forward_s<2, SGN>(acc, u, p);
+    load_link_h<2, RECON>(links_q, zb >> 1, u); load_spinor_h(in, in_scale, zb >> 1, p); hop_backward_s<2, SGN>(acc, u, p);
+    load_link_h<3, RECON>(links_p, cb, u);      load_spinor_h(in, in_scale, tf >> 1, p); hop_forward_s<3, SGN>(acc, u, p);
+    load_link_h<3, RECON>(links_q, tb >> 1, u); load_spinor_h(in, in_scale, tb >> 1, p); hop_backward_s<3, SGN>(acc, u, p);
+    if (xin) {
+        load_spinor_h(xin + rhs * Vhp * 3, xin_scale + rhs * Vhp, cb, p);
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] = fmaf(alpha, p[i], beta * acc[i]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] = beta * acc[i];
+    }
+    store_spinor_h<false>(out, out_scale, cb, acc);
+}
+
+// canonical float32 full-lattice field <-> native half-storage field of one parity
+template <bool TO_NATIVE>
+__global__ void parity_half_kernel(uint4 *native, float *scale, float *canon, int Lx, int Ly, int Lz, long long V, int parity)
+{
+    const long long Vh = V / 2, Vhp = padded_volume(Vh), rhs = blockIdx.y;
+    const long long cb = (long long)blockIdx.x * EH + threadIdx.x;
+    if (cb >= Vh) return;
+    const int Lxh = Lx / 2;
+    long long rem = cb;
+    const int xh = (int)(rem % Lxh); rem /= Lxh;
+    const int y = (int)(rem % Ly); rem /= Ly;
+    const int z = (int)(rem % Lz);
+    const long long t = rem / Lz;
+    const int x = 2 * xh + (int)((y + z + t + parity) & 1);
+    const long long site = x + (long long)Lx * (y + (long long)Ly * (z + (long long)Lz * t));
+    native += rhs * Vhp * 3;
+    scale += rhs * Vhp;
+    float *c = canon + (rhs * V + site) * 24;
+    float p[24];
+    if (TO_NATIVE) {
+#pragma unroll
+        for (int i = 0; i < 6; ++i) {
+            const float4 v = reinterpret_cast<const float4 *>(c)[i];
+            p[4 * i] = v.x; p[4 * i + 1] = v.y; p[4 * i + 2] = v.z; p[4 * i + 3] = v.w;
+        }
+        store_spinor_h<true>(native, scale, cb, p);
+    } else {
+        load_spinor_h(native, scale, cb, p);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) reinterpret_cast<float4 *>(c)[i] = make_float4(p[4 * i], p[4 * i + 1], p[4 * i + 2], p[4 * i + 3]);
+    }
+}
+
+template <int RECON>
+cudaError_t launch_eo_half_r(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger)
+{
+    const long long Vh = a.V / 2, Vhp = padded_volume(Vh);
+    const long long nb = (Vh + EH - 1) / EH;
+    if (nb > 0x7fffffffLL || a.nrhs > 65535) return cudaErrorInvalidConfiguration;
+    if (!a.links_eo) return cudaErrorInvalidValue;
+    dim3 grid((unsigned)nb, (unsigned)a.nrhs);
+    const size_t sc_off = (size_t)a.nrhs * Vhp * 48; // the scales follow the vectors of all right-hand sides
+    const char *le = (const char *)a.links_eo;
+    const size_t half = eo_links_half_bytes(a.V, 16, a.recon);
+    auto kern = dagger ? dslash_eo_half_kernel<RECON, +1> : dslash_eo_half_kernel<RECON, -1>;
+    kern<<<grid, EH, 0, a.stream>>>((uint4 *)a.out, (float *)((char *)a.out + sc_off), (const uint4 *)a.in,
+                                    (const float *)((const char *)a.in + sc_off), (const uint4 *)xin,
+                                    xin ? (const float *)((const char *)xin + sc_off) : nullptr, (const uint4 *)(le + parity * half),
+                                    (const uint4 *)(le + (1 - parity) * half), a.dims[0], a.dims[1], a.dims[2], a.dims[3], Vh,
+                                    (float)alpha, (float)beta, parity);
+    count_launch();
+    return cudaGetLastError();
+}
+
 } // namespace
+
+cudaError_t launch_eo_half(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger)
+{
+    return a.recon == 18 ? launch_eo_half_r<18>(a, xin, alpha, beta, parity, dagger)
+           : a.recon == 12 ? launch_eo_half_r<12>(a, xin, alpha, beta, parity, dagger)
+                           : launch_eo_half_r<8>(a, xin, alpha, beta, parity, dagger);
+}
+
+cudaError_t launch_parity_copy_half(void *native, void *canon, const int dims[4], long long V, int nrhs, int parity, bool to_native,
+                                    cudaStream_t s)
+{
+    const long long Vh = V / 2;
+    if (Vh <= 0 || nrhs <= 0) return cudaSuccess;
+    if (nrhs > 65535) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)((Vh + EH - 1) / EH), (unsigned)nrhs);
+    float *scale = (float *)((char *)native + (size_t)nrhs * padded_volume(Vh) * 48);
+    if (to_native) parity_half_kernel<true><<<grid, EH, 0, s>>>((uint4 *)native, scale, (float *)canon, dims[0], dims[1], dims[2], V, parity);
+    else parity_half_kernel<false><<<grid, EH, 0, s>>>((uint4 *)native, scale, (float *)canon, dims[0], dims[1], dims[2], V, parity);
+    count_launch();
+    return cudaGetLastError();
+}
 
 cudaError_t launch_half(const ApplyArgs &a)
 {

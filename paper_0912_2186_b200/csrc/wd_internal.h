@@ -100,6 +100,10 @@ cudaError_t launch_pack_spinor(void *native, const void *canonical, long long V,
 cudaError_t launch_unpack_spinor(void *canonical, const void *native, long long V, int nrhs, int precision,
                                  cudaStream_t s, long long site0 = 0, long long nsites = -1);
 // red/black blocks (wd_dslash_eo.cu): out_p = alpha * xin_p + beta * hops(in_q); half-field <-> canonical copies
+// the same in half storage (wd_half.cu): fields of one parity in the half layout over lex / 2; no epilogues
+cudaError_t launch_eo_half(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger);
+cudaError_t launch_parity_copy_half(void *native, void *canon, const int dims[4], long long V, int nrhs, int parity, bool to_native,
+                                    cudaStream_t s);
 // parity-ordered link records: record cb of parity p sits at p * eo_links_half_bytes + native position of `cb`
 size_t eo_links_half_bytes(long long V, int precision, int recon);
 cudaError_t launch_links_to_eo(void *links_eo, const void *links, const int dims[4], long long V, int precision, int recon,

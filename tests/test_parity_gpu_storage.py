@@ -174,16 +174,67 @@ def test_half_storage_staged_kernel_is_deterministic(monkeypatch):
         assert rel_l2(outs[k][1], outs[0][1]) <= 5e-4
 
 
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (16, 4, 6, 2), (4, 2, 2, 6)])
+@pytest.mark.parametrize("recon", [18, 12, 8])
+@pytest.mark.parametrize("parity", [0, 1])
+def test_half_storage_even_odd_blocks(oracle, dims, recon, parity):
+    """wd_apply_hop / wd_apply_schur / wd_apply_schur_dagger on half-storage fields of one parity (the operator of the paper's
+    fastest kernel row): inputs are the dequantised fields on both sides, the result (and, for the Schur
+    operator, the intermediate field) is rounded to binary16 relative to the site maximum -- the bounds of reading RH."""
+    import torch
+    nrhs = 2
+    cfg = fields.Config("halfeo", dims, 32, "haar", 18, 0.3, nrhs, 721)
+    U, psi = fields.make_fields(cfg)
+    w = binding.WilsonDirac(dims, torch.from_numpy(U).cuda(), 16, recon)
+    canon = torch.from_numpy(psi).cuda()
+    n = w.half_numel(nrhs)
+    assert n == nrhs * (-(-(fields.volume(dims) // 2) // 32) * 32) * 26
+    hi, ho, hd, hop, tmp = (torch.zeros(n, dtype=torch.float16, device="cuda") for _ in range(5))
+    w.pack_parity(hi, canon, nrhs, parity)
+    back = torch.zeros_like(canon)
+    w.unpack_parity(back, hi, nrhs, parity)
+    w.apply_schur(ho, hi, tmp, cfg.mass, parity, nrhs)
+    w.apply_schur_dagger(hd, hi, tmp, cfg.mass, parity, nrhs)
+    binding.wd_apply_hop(hop, hi, w.gauge, dims, nrhs, 16, 1 - parity)
+    outs = []
+    for h, par in ((ho, parity), (hd, parity), (hop, 1 - parity)):
+        full = torch.zeros_like(canon)
+        w.unpack_parity(full, h, nrhs, par)
+        outs.append(full.cpu().numpy().astype(np.float64))
+    torch.cuda.synchronize()
+    w.close()
+    Lx, Ly, Lz, Lt = dims
+    t, z, y, x = np.meshgrid(np.arange(Lt), np.arange(Lz), np.arange(Ly), np.arange(Lx), indexing="ij")
+    mine = ((x + y + z + t) % 2 == parity)
+    q, s = ws.quantise_half_spinor(psi)
+    held = ws.dequantise_half_spinor(q, s)
+    got_in = back.cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(got_in[:, mine] - held[:, mine])) <= 1e-6 * np.max(np.abs(held))
+    assert not got_in[:, ~mine].any()
+    if recon == 8:
+        Uo = ws.links_from_8(U, 16)
+    else:
+        Uo = ws.quantise_half_links(U if recon == 18 else np.ascontiguousarray(U[..., :2, :, :]))
+    for r in range(nrhs):
+        src = np.where(mine[..., None, None, None], held[r], 0.0)
+        for got, want, m in ((outs[0][r], oracle.schur(src, Uo, dims, cfg.mass, parity), mine),
+                             (outs[1][r], oracle.schur(src, Uo, dims, cfg.mass, parity, sign=+1), mine),
+                             (outs[2][r], oracle.hop_parity(src, Uo, dims, 1 - parity), ~mine)):
+            err = rel_l2(got[m], want[m])
+            assert 1e-5 <= err <= 1e-3, (recon, r, err)
+            assert not got[~m].any()
+
+
 def test_half_storage_is_refused_where_it_is_not_implemented():
     import torch
     dims = (4, 4, 4, 4)
     cfg = fields.Config("halfno", dims, 32, "haar", 18, 0.1, 1, 713)
     U, psi = fields.make_fields(cfg)
     op = binding.WilsonDirac(dims, torch.from_numpy(U).cuda(), 16, 12)
-    buf = torch.zeros(op.native_numel(1), dtype=torch.float16, device="cuda")
+    buf = torch.zeros(op.half_numel(1), dtype=torch.float16, device="cuda")
     buf2 = torch.zeros_like(buf)
-    with pytest.raises(binding.WdError) as e:
-        binding.wd_apply_hop(buf2, buf, op.gauge, dims, 1, 16, 0)
+    with pytest.raises(binding.WdError) as e:                                  # the solvers run in fp32 / fp64
+        binding.wd_cgnr_schur(buf2, buf, op.gauge, 0.1, dims, 16, 0, 3)
     assert e.value.code == -3
     op.set_kernel(3)                                    # 4^4 can be tiled by the staged half kernel
     with pytest.raises(binding.WdError) as e:
