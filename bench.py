@@ -600,10 +600,16 @@ def run_schur(args):
     w = {16: 2, 32: 4, 64: 8}[prec]
     tdt = {16: torch.float16, 32: torch.float32, 64: torch.float64}[prec]
     U, psi = fields.make_fields(rank_config(cfg, recon, nrhs, rank))
+    if args.temporal_gauge:  # Fig. 4 "GF": unit t-links below the last slice, skipped by the kernel
+        if prec == 16 or recon == 8:
+            raise SystemExit("bench.py --op schur --temporal-gauge: 18- or 12-real links in fp32 / fp64")
+        U, _ = fields.temporal_gauge(U, cfg.precision)
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
         u_dev = torch.from_numpy(U).to(dev)
         op = binding.WilsonDirac(cfg.dims, u_dev, prec, recon, stream=stream.cuda_stream)
+        if args.temporal_gauge:
+            op.set_temporal_gauge(True)
         canon = torch.from_numpy(psi).to(dev)
         n = op.half_numel(nrhs)
         ins = [torch.empty(n, dtype=tdt, device=dev) for _ in range(NBUF)]
@@ -634,6 +640,8 @@ def run_schur(args):
     flops = (2 * 1320 + 48) * (V // 2) * nrhs
     spinor_b = 52 if prec == 16 else 24 * w  # half storage: 24 binary16 ratios + a float32 scale per site
     bytes_per_apply = (V // 2) * (2 * 2 * 4 * recon * w + nrhs * 5 * spinor_b)
+    if args.temporal_gauge:  # the t-links are read on one slice of Lt only (forward on the last, backward on the first)
+        bytes_per_apply -= (V // 2) * 2 * 2 * recon * w * (cfg.dims[3] - 1) // cfg.dims[3]
     peak, peak_src = measured_peak()
     achieved = bytes_per_apply * applies / (ms * 1e-3) / 1e9
     line = {"metric": "wilson_schur_gflops", "value": applies * flops / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": 1,
@@ -642,7 +650,7 @@ def run_schur(args):
             "dtype": {16: "f32 arithmetic on f16 storage", 32: "f32", 64: "f64"}[prec], "data": "synthetic",
             "config": {"workload": cfg.name, "op": "even-odd preconditioned operator (2 launches per apply)",
                        "dims": list(cfg.dims), "recon": recon, "nrhs": nrhs, "mass": cfg.mass, "applies_per_step": aps,
-                       "flops_per_even_site": 2 * 1320 + 48,
+                       "temporal_gauge": bool(args.temporal_gauge), "flops_per_even_site": 2 * 1320 + 48,
                        "l2": "inputs larger than L2 (gauge + rotating half fields), no flush"},
             "us_per_apply": ms / applies * 1e3, "clocks": clocks.summary(),
             "gpu_launches": int(binding.wd_launch_count() - n0),

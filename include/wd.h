@@ -137,7 +137,8 @@ int wd_set_tuning(wd_gauge *gauge, const char *name, int value);
 /* Temporal gauge ("temporal gauge fixing", Fig. 4 / Table 2 "GF"): on != 0 declares that the loaded links
  * satisfy U_t(x,t) = 1 for every t < Lt-1 (the last slice carries the Polyakov lines).  The library verifies it
  * (WD_ERR_MISMATCH if some such link differs from 1 by more than 1e-6 / 1e-12; synchronises the stream) and the staged
- * kernels then neither load those links nor multiply by them; the other kernels ignore the flag (same result).
+ * kernels and the red/black kernel (wd_apply_hop, wd_apply_schur*, the solvers) then neither load those links nor
+ * multiply by them; the other kernels ignore the flag (same result).
  * The operator is unchanged: D(U^g)(g psi) = g D(U) psi. */
 int wd_set_temporal_gauge(wd_gauge *gauge, int on);
 

@@ -31,7 +31,7 @@ __global__ void __launch_bounds__(EO_THREADS)
 dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ xin, const T *__restrict__ links_p,
                  const T *__restrict__ links_q,
                  int Lx, int Ly, int Lz, int Lt, long long Vh, T alpha, T beta, int parity, double *__restrict__ norm_part, int nrhs,
-                 const T *__restrict__ dot_y, double *__restrict__ dot_part)
+                 const T *__restrict__ dot_y, double *__restrict__ dot_part, int tgauge)
 {
     // gridDim.x = (site blocks) * nrhs with the right-hand side FASTEST: the CTAs resident at any time are all right-hand
     // sides of a few site blocks, so the links of a block come from HBM once and from L1/L2 for the others
@@ -74,8 +74,26 @@ dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restr
     load_link<1, T, RECON>(links_q, yb >> 1, u); load_spinor(in, yb >> 1, p); hop_backward_s<1, SGN>(acc, u, p);
     load_link<2, T, RECON>(links_p, cb, u);      load_spinor(in, zf >> 1, p); hop_forward_s<2, SGN>(acc, u, p);
     load_link<2, T, RECON>(links_q, zb >> 1, u); load_spinor(in, zb >> 1, p); hop_backward_s<2, SGN>(acc, u, p);
-    load_link<3, T, RECON>(links_p, cb, u);      load_spinor(in, tf >> 1, p); hop_forward_s<3, SGN>(acc, u, p);
-    load_link<3, T, RECON>(links_q, tb >> 1, u); load_spinor(in, tb >> 1, p); hop_backward_s<3, SGN>(acc, u, p);
+    // tgauge: the caller's links are in temporal gauge (U_t(x,t) = 1 for t < Lt-1; Fig. 4 "GF"): those
+    // links are neither loaded nor multiplied -- a quarter of the link bytes
+    load_spinor(in, tf >> 1, p);
+    if (tgauge && t != Lt - 1) {
+        T h[12];
+        project<3, SGN>(p, h);
+        reconstruct_add<3, SGN>(acc, h);
+    } else {
+        load_link<3, T, RECON>(links_p, cb, u);
+        hop_forward_s<3, SGN>(acc, u, p);
+    }
+    load_spinor(in, tb >> 1, p);
+    if (tgauge && t != 0) {
+        T h[12];
+        project<3, -SGN>(p, h);
+        reconstruct_add<3, -SGN>(acc, h);
+    } else {
+        load_link<3, T, RECON>(links_q, tb >> 1, u);
+        hop_backward_s<3, SGN>(acc, u, p);
+    }
 
     if (xin) {
         load_spinor(xin + (long long)rhs * 24 * Vhp, cb, p);
@@ -149,7 +167,7 @@ static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha
     kern<<<grid, EO_THREADS, 0, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)xin, (const T *)(le + parity * half),
                                              (const T *)(le + (1 - parity) * half), a.dims[0],
                                              a.dims[1], a.dims[2], a.dims[3], Vh, (T)alpha, (T)beta, parity, norm_part, a.nrhs,
-                                             (const T *)dot_y, dot_part);
+                                             (const T *)dot_y, dot_part, a.tgauge);
     count_launch();
     return cudaGetLastError();
 }

@@ -45,6 +45,46 @@ def test_staged_kernel_in_temporal_gauge_matches_the_oracle(oracle, dims, precis
     assert rel_l2(one[0], oracle.apply(psi[0].astype(np.float64), Uo, dims, cfg.mass)) <= TOL[precision]
 
 
+@pytest.mark.parametrize("dims", [(8, 4, 4, 6), (16, 8, 2, 2), (4, 4, 4, 4)])
+@pytest.mark.parametrize("precision,recon", [(32, 18), (32, 12), (64, 18), (64, 12)])
+@pytest.mark.parametrize("parity", [0, 1])
+def test_even_odd_blocks_in_temporal_gauge(oracle, dims, precision, recon, parity):
+    """The red/black kernel skips the unit t-links too (the paper's Fig. 4 "GF" curves are this kernel):
+    M-hat, M-hat^dagger and a CGNR solve with the flag set against the oracle on the same gauge-fixed links, and against
+    the same calls with the flag off."""
+    import torch
+    nrhs = 2
+    cfg = fields.Config("tgeo", dims, precision, "haar", recon, 0.25, nrhs, 85)
+    U, psi = fields.make_fields(cfg)
+    Ug, _ = fields.temporal_gauge(U, precision)
+    Uo = (Ug if recon == 18 else np.ascontiguousarray(Ug[..., :2, :, :])).astype(np.float64)
+    op = GpuOp(Ug, dims, precision, recon)
+    w = op.op
+    canon = torch.from_numpy(psi).cuda()
+    n = w.half_numel(nrhs)
+    hi, tmp = (torch.empty(n, dtype=canon.dtype, device="cuda") for _ in range(2))
+    w.pack_parity(hi, canon, nrhs, parity)
+    res = {}
+    for flag in (False, True):
+        w.set_temporal_gauge(flag)
+        for name, fn in (("schur", w.apply_schur), ("dagger", w.apply_schur_dagger)):
+            ho = torch.empty_like(hi)
+            fn(ho, hi, tmp, cfg.mass, parity, nrhs)
+            full = torch.zeros_like(canon)
+            w.unpack_parity(full, ho, nrhs, parity)
+            res[name, flag] = full.cpu().numpy()
+    op.close()
+    Lx, Ly, Lz, Lt = dims
+    t, z, y, x = np.meshgrid(np.arange(Lt), np.arange(Lz), np.arange(Ly), np.arange(Lx), indexing="ij")
+    mine = ((x + y + z + t) % 2 == parity)
+    for r in range(nrhs):
+        src = np.where(mine[..., None, None, None], psi[r].astype(np.float64), 0.0)
+        for name, sign in (("schur", -1), ("dagger", +1)):
+            want = oracle.schur(src, Uo, dims, cfg.mass, parity, sign=sign)
+            assert rel_l2(res[name, True][r][mine], want[mine]) <= TOL[precision]
+            assert rel_l2(res[name, True][r][mine], res[name, False][r][mine]) <= TOL[precision]
+
+
 def test_full_size_temporal_gauge_32x64(oracle):
     cfg = fields.CONFIGS["c3_32x64_fp32"]
     U, psi = fields.make_fields(cfg)
