@@ -237,6 +237,24 @@ int wd_apply_schur_dagger(void *out_half_dev, const void *in_half_dev, void *tmp
                           double mass, const int dims[4], int nrhs, int precision, int parity);
 
 /*
+ * wd_apply_schur_static -- wd_apply_schur for callers that cannot allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): out = Mhat in on `parity`, WD_FP32 or
+ * WD_FP64, any link format, two launches on the gauge's stream.  The intermediate half field H_qp in lives in a static
+ * device array of WD_STATIC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it until the
+ * process exits) and the links are read from the gauge handle's ordinary native links, so the call allocates nothing:
+ * no cudaMalloc, cudaFree or allocating library routine, on the first call or any later one (unlike the other
+ * red/black entry points, whose first call on a handle allocates a parity-ordered link copy).
+ * Limit: nrhs * padded(V/2) * 24 * sizeof(real) <= WD_STATIC_SCRATCH_BYTES (padded = rounded up to 32 sites), e.g. one
+ * fp32 right-hand side on 349 504 lattice sites (16^3 x 32 fits 2 in fp32, 1 in fp64); beyond it: WD_ERR_DIMS, nothing
+ * launched.  Other errors as wd_apply_schur.  Every call shares the array and it keeps the last call's contents
+ * (nothing in it has to start at zero: it is fully written before it is read); calls that overlap on the GPU
+ * (different streams, several host threads, several gauge handles) race on it -- serialise them.
+ */
+#define WD_STATIC_SCRATCH_BYTES (16u << 20)
+int wd_apply_schur_static(void *out_half_dev, const void *in_half_dev, const wd_gauge *gauge, double mass,
+                          const int dims[4], int nrhs, int precision, int parity);
+
+/*
  * wd_cgnr_schur -- conjugate gradients on the normal equations of the even-odd preconditioned operator
  * ("CG on the normal equations"; CG around the even-odd matvec):
  *     Mhat^dagger Mhat x = Mhat^dagger b,   x_0 = 0,   one right-hand side, half fields of `parity`.

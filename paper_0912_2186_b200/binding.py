@@ -24,7 +24,7 @@ STATUS_NAMES = {
 SYMBOLS = (
     "wd_create_lattice", "wd_lattice_dims", "wd_lattice_volume", "wd_load_gauge", "wd_set_stream",
     "wd_set_kernel", "wd_set_tuning", "wd_set_temporal_gauge", "wd_selected_kernel", "wd_spinor_bytes", "wd_spinor_bytes_parity", "wd_pack_spinor_parity",
-    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_gcr_schur_precond", "wd_cgnr_schur_block", "wd_coarse_reals", "wd_coarse_stencil_reals", "wd_build_coarse", "wd_apply_coarse",
+    "wd_unpack_spinor_parity", "wd_apply_hop", "wd_apply_schur", "wd_apply_schur_dagger", "wd_apply_schur_static", "wd_cgnr_schur", "wd_bicgstab_schur", "wd_gcr_schur", "wd_gcr_schur_precond", "wd_cgnr_schur_block", "wd_coarse_reals", "wd_coarse_stencil_reals", "wd_build_coarse", "wd_apply_coarse",
     "wd_block_orthonormalise", "wd_restrict", "wd_prolong", "wd_pack_spinor", "wd_unpack_spinor", "wd_apply", "wd_apply_dagger", "wd_apply_host",
     "wd_launch_count", "wd_last_error", "wd_destroy_gauge", "wd_destroy",
 )
@@ -72,6 +72,7 @@ def lib():
     L.wd_apply_hop.argtypes = [vp, vp, vp, ip, i, i, i]
     L.wd_apply_schur.argtypes = [vp, vp, vp, vp, d, ip, i, i, i]
     L.wd_apply_schur_dagger.argtypes = [vp, vp, vp, vp, d, ip, i, i, i]
+    L.wd_apply_schur_static.argtypes = [vp, vp, vp, d, ip, i, i, i]
     L.wd_cgnr_schur.argtypes = [vp, vp, vp, d, ip, i, i, i, d, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]
     L.wd_bicgstab_schur.argtypes = L.wd_cgnr_schur.argtypes
     L.wd_gcr_schur.argtypes = [vp, vp, vp, d, ip, i, i, i, i, d, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]
@@ -244,6 +245,15 @@ def wd_apply_schur(out_half_dev, in_half_dev, tmp_half_dev, gauge, mass, dims, n
 def wd_apply_schur_dagger(out_half_dev, in_half_dev, tmp_half_dev, gauge, mass, dims, nrhs, precision, parity):
     _check(lib().wd_apply_schur_dagger(_ptr(out_half_dev), _ptr(in_half_dev), _ptr(tmp_half_dev), gauge, float(mass),
                                        _dims(dims), int(nrhs), int(precision), int(parity)), "wd_apply_schur_dagger")
+
+
+WD_STATIC_SCRATCH_BYTES = 16 << 20  # include/wd.h
+
+
+def wd_apply_schur_static(out_half_dev, in_half_dev, gauge, mass, dims, nrhs, precision, parity):
+    """wd_apply_schur without a caller-supplied intermediate field and without any device allocation (static scratch)."""
+    _check(lib().wd_apply_schur_static(_ptr(out_half_dev), _ptr(in_half_dev), gauge, float(mass), _dims(dims), int(nrhs),
+                                       int(precision), int(parity)), "wd_apply_schur_static")
 
 
 def _solve(name, x_half_dev, b_half_dev, gauge, mass, dims, precision, parity, max_iter, tol):
@@ -426,6 +436,9 @@ class WilsonDirac:
 
     def apply_schur(self, out_half_dev, in_half_dev, tmp_half_dev, mass, parity, nrhs=1):
         wd_apply_schur(out_half_dev, in_half_dev, tmp_half_dev, self.gauge, mass, self.dims, nrhs, self.precision, parity)
+
+    def apply_schur_static(self, out_half_dev, in_half_dev, mass, parity, nrhs=1):
+        wd_apply_schur_static(out_half_dev, in_half_dev, self.gauge, mass, self.dims, nrhs, self.precision, parity)
 
     def apply_schur_dagger(self, out_half_dev, in_half_dev, tmp_half_dev, mass, parity, nrhs=1):
         wd_apply_schur_dagger(out_half_dev, in_half_dev, tmp_half_dev, self.gauge, mass, self.dims, nrhs, self.precision,

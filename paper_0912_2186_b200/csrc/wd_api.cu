@@ -746,6 +746,33 @@ int wd_apply_schur_dagger(void *out_half_dev, const void *in_half_dev, void *tmp
     return apply_schur(out_half_dev, in_half_dev, tmp_half_dev, gauge, mass, dims, nrhs, precision, parity, true);
 }
 
+int wd_apply_schur_static(void *out_half_dev, const void *in_half_dev, const wd_gauge *gauge, double mass, const int dims[4],
+                          int nrhs, int precision, int parity)
+{
+    // (not check_eo_args: that one builds the parity-ordered link copy with cudaMalloc; nothing below allocates)
+    int rc = check_apply_args(out_half_dev, in_half_dev, gauge, dims, nrhs, precision);
+    if (rc) return rc;
+    if (!all_even(gauge->dims)) return fail(WD_ERR_DIMS, "wd_apply_schur_static: red/black blocks need even extents");
+    if (parity != 0 && parity != 1) return fail(WD_ERR_MISMATCH, "wd_apply_schur_static: parity %d is not 0 or 1", parity);
+    const size_t hb = half_bytes(gauge->V, nrhs, precision);
+    if (overlap(out_half_dev, hb, in_half_dev, hb)) return fail(WD_ERR_ALIAS, "wd_apply_schur_static: out and in overlap");
+    if (((uintptr_t)out_half_dev | (uintptr_t)in_half_dev) & 15)
+        return fail(WD_ERR_MISMATCH, "wd_apply_schur_static: buffers must be 16-byte aligned");
+    if (4.0 + mass == 0.0) return fail(WD_ERR_MISMATCH, "wd_apply_schur_static: 4 + mass = 0, the diagonal block is not invertible");
+    wd::ApplyArgs a = shape_args(gauge, nrhs);
+    a.out = out_half_dev;
+    a.in = in_half_dev;
+    a.links = gauge->links;
+    a.mass = mass;
+    a.stream = gauge->stream;
+    const size_t need = wd::schur_static_need(a);
+    if (need > (size_t)WD_STATIC_SCRATCH_BYTES)
+        return fail(WD_ERR_DIMS, "wd_apply_schur_static: the intermediate field needs %zu bytes, the static scratch array holds %zu",
+                    need, (size_t)WD_STATIC_SCRATCH_BYTES);
+    cudaError_t e = wd::launch_schur_static(a, parity);
+    return e == cudaSuccess ? WD_OK : cuda_fail(e, "wd_apply_schur_static");
+}
+
 int wd_cgnr_schur(void *x_half_dev, const void *b_half_dev, wd_gauge *gauge, double mass, const int dims[4],
                   int precision, int parity, int max_iter, double tol, int *iters_out, double *hist_host)
 {

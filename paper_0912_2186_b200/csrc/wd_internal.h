@@ -104,6 +104,9 @@ cudaError_t launch_unpack_spinor(void *canonical, const void *native, long long 
 cudaError_t launch_eo_half(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger);
 cudaError_t launch_parity_copy_half(void *native, void *canon, const int dims[4], long long V, int nrhs, int parity, bool to_native,
                                     cudaStream_t s);
+// wd_noalloc.cu: Mhat with its intermediate field in a static device array (no allocation anywhere)
+size_t schur_static_need(const ApplyArgs &a);
+cudaError_t launch_schur_static(const ApplyArgs &a, int parity);
 // parity-ordered link records: record cb of parity p sits at p * eo_links_half_bytes + native position of `cb`
 size_t eo_links_half_bytes(long long V, int precision, int recon);
 cudaError_t launch_links_to_eo(void *links_eo, const void *links, const int dims[4], long long V, int precision, int recon,
