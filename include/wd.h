@@ -27,6 +27,12 @@
  * There is NO CPU fallback anywhere: without a CUDA device every compute entry point
  * returns WD_ERR_CUDA.
  *
+ * Threads: a wd_lattice may be shared freely (it is immutable).  A wd_gauge handle owns mutable state -- its stream,
+ * tuning, caches built on first use (the parity-ordered links of the red/black entry points, solver workspaces,
+ * staging buffers), also behind entry points that take it as `const wd_gauge *` -- so calls on ONE gauge handle must not
+ * run concurrently on several host threads; different handles are independent (wd_apply_schur_static excepted: all its
+ * calls share one static array).
+ *
  * CANONICAL layouts (what callers, tests and the oracle speak; C order, last index fastest):
  *   spinor  psi[rhs][t][z][y][x][spin 0..3][colour 0..2][re,im]      24 reals per site
  *   links   U  [mu 0..3][t][z][y][x][row a][col b][re,im]            18 reals per link
