@@ -592,7 +592,7 @@ def run_schur(args):
     dev = torch.device("cuda", local)
     torch.cuda.set_device(local)
     cfg = fields.CONFIGS[args.workload]
-    recon, nrhs = args.recon, cfg.nrhs
+    recon, nrhs = args.recon, (args.nrhs or cfg.nrhs)  # --nrhs N: N right-hand sides per batched launch
     V = fields.volume(cfg.dims)
     if args.half and cfg.precision != 32:
         raise SystemExit("bench.py --op schur --half: half storage has float32 canonical fields; use an fp32 workload")

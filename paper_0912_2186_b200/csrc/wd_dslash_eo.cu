@@ -24,6 +24,12 @@
 namespace wd {
 
 constexpr int EO_THREADS = 128;
+#ifndef WD_EO_NR32
+#define WD_EO_NR32 2 // right-hand sides per thread of the multi-RHS member, fp32
+#endif
+#ifndef WD_EO_NR64
+#define WD_EO_NR64 2 // ... fp64
+#endif
 
 // SGN = -1: blocks of D; SGN = +1: blocks of gamma5 D gamma5 = D^dagger (all projectors swapped)
 template <typename T, int RECON, int SGN>
@@ -151,6 +157,119 @@ dslash_eo_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restr
     }
 }
 
+// Several right-hand sides: NR of them per thread, so that a link is loaded (and, for 12- / 8-real links, rebuilt) once for
+// NR hops.  gridDim.x = (site blocks) * (groups of NR right-hand sides), the group FASTEST as above.  Per right-hand side
+// the arithmetic and its order are those of dslash_eo_kernel.  No inner-product epilogue (one right-hand side only).
+template <typename T, int RECON, int SGN, int NR>
+__global__ void __launch_bounds__(EO_THREADS)
+dslash_eo_nr_kernel(T *__restrict__ out, const T *__restrict__ in, const T *__restrict__ xin, const T *__restrict__ links_p,
+                    const T *__restrict__ links_q, int Lx, int Ly, int Lz, int Lt, long long Vh, T alpha, T beta, int parity,
+                    double *__restrict__ norm_part, int nrhs, int tgauge)
+{
+    const unsigned ngroups = (unsigned)((nrhs + NR - 1) / NR);
+    const int rhs0 = (int)(blockIdx.x % ngroups) * NR;
+    const long long blk = blockIdx.x / ngroups, nblk = gridDim.x / ngroups;
+    const long long cb_raw = blk * EO_THREADS + threadIdx.x;
+    const bool valid = cb_raw < Vh;
+    if (!valid && !norm_part) return;
+    const long long cb = valid ? cb_raw : Vh - 1;
+    const long long Vhp = padded_volume(Vh), fs = 24 * Vhp; // reals per right-hand side of a half field
+    in += (long long)rhs0 * fs;
+    out += (long long)rhs0 * fs;
+    const int nr = nrhs - rhs0 < NR ? nrhs - rhs0 : NR; // live right-hand sides of this group (uniform in the CTA)
+
+    const int Lxh = Lx / 2;
+    long long rem = cb;
+    const int xh = (int)(rem % Lxh); rem /= Lxh;
+    const int y = (int)(rem % Ly); rem /= Ly;
+    const int z = (int)(rem % Lz);
+    const int t = (int)(rem / Lz);
+    const int x = 2 * xh + ((y + z + t + parity) & 1);
+    const long long sy = Lx, sz = (long long)Lx * Ly, st = (long long)Lx * Ly * Lz;
+    const long long site = x + sy * y + sz * z + st * t;
+    const long long xf = site + (x + 1 == Lx ? -(long long)(Lx - 1) : 1), xb = site + (x == 0 ? (long long)(Lx - 1) : -1);
+    const long long yf = site + (y + 1 == Ly ? -(Ly - 1) * sy : sy), yb = site + (y == 0 ? (Ly - 1) * sy : -sy);
+    const long long zf = site + (z + 1 == Lz ? -(Lz - 1) * sz : sz), zb = site + (z == 0 ? (Lz - 1) * sz : -sz);
+    const long long tf = site + (t + 1 == Lt ? -(Lt - 1) * st : st), tb = site + (t == 0 ? (Lt - 1) * st : -st);
+
+    T acc[NR][24];
+#pragma unroll
+    for (int r = 0; r < NR; ++r)
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[r][i] = (T)0;
+    T u[18], p[24];
+#define WD_EO_NR_HOP(MU, LINKS, LSITE, NB, FWD)                                                              \
+    load_link<MU, T, RECON>(LINKS, LSITE, u);                                                                \
+    _Pragma("unroll") for (int r = 0; r < NR; ++r) if (r < nr) {                                             \
+        load_spinor(in + r * fs, (NB) >> 1, p);                                                              \
+        if (FWD) hop_forward_s<MU, SGN>(acc[r], u, p);                                                       \
+        else hop_backward_s<MU, SGN>(acc[r], u, p);                                                          \
+    }
+    WD_EO_NR_HOP(0, links_p, cb, xf, true)
+    WD_EO_NR_HOP(0, links_q, xb >> 1, xb, false)
+    WD_EO_NR_HOP(1, links_p, cb, yf, true)
+    WD_EO_NR_HOP(1, links_q, yb >> 1, yb, false)
+    WD_EO_NR_HOP(2, links_p, cb, zf, true)
+    WD_EO_NR_HOP(2, links_q, zb >> 1, zb, false)
+    if (tgauge && t != Lt - 1) { // unit link (temporal gauge): projection and reconstruction only
+#pragma unroll
+        for (int r = 0; r < NR; ++r)
+            if (r < nr) {
+                T h[12];
+                load_spinor(in + r * fs, tf >> 1, p);
+                project<3, SGN>(p, h);
+                reconstruct_add<3, SGN>(acc[r], h);
+            }
+    } else {
+        WD_EO_NR_HOP(3, links_p, cb, tf, true)
+    }
+    if (tgauge && t != 0) {
+#pragma unroll
+        for (int r = 0; r < NR; ++r)
+            if (r < nr) {
+                T h[12];
+                load_spinor(in + r * fs, tb >> 1, p);
+                project<3, -SGN>(p, h);
+                reconstruct_add<3, -SGN>(acc[r], h);
+            }
+    } else {
+        WD_EO_NR_HOP(3, links_q, tb >> 1, tb, false)
+    }
+#undef WD_EO_NR_HOP
+
+    __shared__ double sh[NR][EO_THREADS / 32];
+#pragma unroll
+    for (int r = 0; r < NR; ++r)
+        if (r < nr) {
+            if (xin) {
+                load_spinor(xin + (long long)(rhs0 + r) * fs, cb, p);
+#pragma unroll
+                for (int i = 0; i < 24; ++i) acc[r][i] = fma(alpha, p[i], beta * acc[r][i]);
+            } else {
+#pragma unroll
+                for (int i = 0; i < 24; ++i) acc[r][i] = beta * acc[r][i];
+            }
+            if (valid) store_spinor(out + r * fs, cb, acc[r]);
+            if (norm_part) {
+                double s2 = 0.0;
+                if (valid)
+#pragma unroll
+                    for (int i = 0; i < 24; ++i) s2 += (double)acc[r][i] * acc[r][i];
+                for (int o = 16; o > 0; o >>= 1) s2 += __shfl_down_sync(0xffffffffu, s2, o);
+                if ((threadIdx.x & 31) == 0) sh[r][threadIdx.x >> 5] = s2;
+            }
+        }
+    if (norm_part) {
+        __syncthreads();
+        if (threadIdx.x < nr) {
+            double tt = 0.0;
+#pragma unroll
+            for (int i = 0; i < EO_THREADS / 32; ++i) tt += sh[threadIdx.x][i];
+            norm_part[(long long)(rhs0 + threadIdx.x) * nblk + blk] = tt;
+        }
+    }
+}
+
 template <typename T, int RECON>
 static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha, double beta, int parity, bool dagger,
                                double *norm_part, const void *dot_y, double *dot_part)
@@ -159,6 +278,19 @@ static cudaError_t launch_eo_t(const ApplyArgs &a, const void *xin, double alpha
     const long long Vh = a.V / 2;
     const long long nb = (Vh + EO_THREADS - 1) / EO_THREADS;
     if (nb * a.nrhs > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    if (!a.links_eo) return cudaErrorInvalidValue; // the API builds the parity-ordered links before any red/black launch
+    if (a.nrhs >= 2 && !dot_part) { // several right-hand sides: NR per thread share every link load
+        constexpr int NR = sizeof(T) == 4 ? WD_EO_NR32 : WD_EO_NR64;
+        const long long ng = (a.nrhs + NR - 1) / NR;
+        const char *le = (const char *)a.links_eo;
+        const size_t half = eo_links_half_bytes(a.V, a.precision, a.recon);
+        auto kn = dagger ? dslash_eo_nr_kernel<T, RECON, +1, NR> : dslash_eo_nr_kernel<T, RECON, -1, NR>;
+        kn<<<(unsigned)(nb * ng), EO_THREADS, 0, a.stream>>>((T *)a.out, (const T *)a.in, (const T *)xin, (const T *)(le + parity * half),
+                                                            (const T *)(le + (1 - parity) * half), a.dims[0], a.dims[1], a.dims[2],
+                                                            a.dims[3], Vh, (T)alpha, (T)beta, parity, norm_part, a.nrhs, a.tgauge);
+        count_launch();
+        return cudaGetLastError();
+    }
     dim3 grid((unsigned)(nb * a.nrhs));
     auto kern = dagger ? dslash_eo_kernel<T, RECON, +1> : dslash_eo_kernel<T, RECON, -1>;
     if (!a.links_eo) return cudaErrorInvalidValue; // the API builds the parity-ordered links before any red/black launch
