@@ -21,7 +21,12 @@ One JSON line on stdout (rank 0).  Definitions:
   * secondary  (default run only) two short legs after the headline timing, same launch path, own clocks record:
                configs[4] = 24 right-hand sides (2 steps x 10 applies; roofline.frac against the HBM peak, plus
                frac_of_own_peak against min(HBM bound, FMA-pipe bound at the observed clock)) and configs[3] in fp64
-               (2 steps x 25 applies).  The headline's metric, config and value are unchanged.
+               (2 steps x 25 applies), then the same two with 12-real links and the storage variants of the paper's
+               Table 2 on the headline lattice (12-real, 8-real, half storage).  The headline's metric, config and value
+               are unchanged.
+  * next_rows  (default run only) short legs of the rows built after the hot path, on the headline's lattice and links:
+               the even-odd preconditioned operator (f1), CGNR / BiCGstab / GCR(8) on it (f2; 48 iterations each) and the
+               block CGNR on 12 right-hand sides; each with its own byte model, roofline fraction and clocks record.
   * cpu_baseline  the oracle (oracle/wd_oracle.c, fp64, OpenMP) on this box's host cores, on a
                bounded sample of the same workload.
 Multi-GPU (torchrun): the path has no exchange step on one GPU per lattice; ranks run independent
@@ -301,6 +306,76 @@ def secondary_leg(binding, torch, dev, stream, local, name, U, recon, nrhs, step
             "roofline": roof, "clocks": ck}
 
 
+SOLVER_MODEL = {"cgnr": (288, 8, 2), "bicgstab": (672, 15, 2), "gcr": (1150, 22.25, 1)}  # BLAS-1 flops, spinor passes, matvecs
+
+
+def next_rows_legs(binding, torch, dev, stream, local, name, U, recon):
+    """Short timed legs of the "next" rows on the headline's lattice and links (the operator and the
+    solvers of the paper's Table 2): the even-odd preconditioned operator Mhat, CGNR, BiCGstab and GCR(8)
+    on it, and the 12-right-hand-side block CGNR.  Same byte and flop models as --op schur / cgnr / bicgstab / gcr."""
+    cfg = fields.CONFIGS[name]
+    V, w = fields.volume(cfg.dims), 4
+    peak, peak_src = measured_peak()
+    out = []
+    with torch.cuda.stream(stream):
+        u_dev = torch.from_numpy(fields.round_to(U, 32)).to(dev)
+        op = binding.WilsonDirac(cfg.dims, u_dev, 32, recon, stream=stream.cuda_stream)
+        g = torch.Generator(device=dev).manual_seed(cfg.seed + 2000)
+        n = op.half_numel(1)
+        b = torch.randn(12 * n, dtype=torch.float32, device=dev, generator=g)  # native half fields: any values are vectors
+        x = torch.empty_like(b)
+        tmp = torch.empty(n, dtype=torch.float32, device=dev)
+    stream.synchronize()
+    del u_dev
+
+    def timed(fn, reps):
+        fn()
+        torch.cuda.synchronize()
+        n0 = binding.wd_launch_count()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with ClockSampler(local) as clocks:
+            ev0.record(stream)
+            for _ in range(reps):
+                fn()
+            ev1.record(stream)
+            torch.cuda.synchronize()
+        return ev0.elapsed_time(ev1) / reps, int(binding.wd_launch_count() - n0), clocks.summary()
+
+    def entry(row, what, units, unit_name, ms, flops, nbytes, launches, ck, nrhs=1):
+        achieved = nbytes * units / (ms * 1e-3) / 1e9
+        return {"row": row, "op": what, "workload": name, "recon": recon, "nrhs": nrhs, "dtype": "f32",
+                "value": units * flops / (ms * 1e-3) / 1e9, "unit": UNIT, "us_per_" + unit_name: ms / units * 1e3,
+                "gpu_launches": launches, "clocks": ck,
+                "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                             "peak_source": peak_src, "bytes_per_" + unit_name: nbytes}}
+
+    aps = 20
+
+    def schur():
+        for i in range(aps):
+            op.apply_schur(x[(i % 4) * n:(i % 4 + 1) * n], b[(i % 4) * n:(i % 4 + 1) * n], tmp, cfg.mass, 0, 1)
+
+    ms, nl, ck = timed(schur, 2)
+    out.append(entry("f1", "even-odd preconditioned operator Mhat (2 launches)", aps, "apply", ms,
+                     (2 * 1320 + 48) * (V // 2), (V // 2) * (2 * 2 * 4 * recon * w + 5 * 24 * w), nl, ck))
+    iters = 48
+    for key, label, solve in (("cgnr", "CGNR on Mhat", op.cgnr_schur), ("bicgstab", "BiCGstab on Mhat", op.bicgstab_schur),
+                              ("gcr", "GCR(8) on Mhat", op.gcr_schur)):
+        bf, bp, nmv = SOLVER_MODEL[key]
+        ms, nl, ck = timed(lambda: solve(x[:n], b[:n], cfg.mass, 0, iters), 1)
+        out.append(entry("f2", label, iters, "iteration", ms, (nmv * (2 * 1320 + 48) + bf) * (V // 2),
+                         (V // 2) * (nmv * (2 * 2 * 4 * recon * w + 5 * 24 * w) + bp * 24 * w), nl, ck))
+    bf, bp, nmv = SOLVER_MODEL["cgnr"]
+    ms, nl, ck = timed(lambda: op.cgnr_schur_block(x, b, cfg.mass, 0, 12, 10), 1)
+    out.append(entry("f2 + a'", "block CGNR on Mhat, 12 right-hand sides in lock step", 10, "iteration", ms,
+                     (nmv * (2 * 1320 + 48) + bf) * (V // 2) * 12,
+                     (V // 2) * (nmv * (2 * 2 * 4 * recon * w + 12 * 5 * 24 * w) + 12 * bp * 24 * w), nl, ck, nrhs=12))
+    op.close()
+    del b, x, tmp
+    torch.cuda.empty_cache()
+    return out
+
+
 def pcie_peaks(torch, dev, h_in, h_out):
     """Measured copy rates of THIS box for the e2e roofline: one large cudaMemcpyAsync per direction from / to the pinned
     buffers the e2e leg uses, alone (h2d, d2h) and both at once on two streams (duplex, rate per direction), best of 3,
@@ -515,6 +590,7 @@ def run_wd(args):
     pcie = pcie_peaks(torch, dev, h_in, h_out) if world == 1 else None
 
     secondary = None
+    next_rows = None
     if want_secondary:
         # free the headline's device buffers first (24 RHS need 2 x 2 x 4.8 GB)
         del ins, outs, h_in, h_out
@@ -530,6 +606,7 @@ def run_wd(args):
             secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp32", U, 8, 1, 2, 50),
             secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp32", U, 12, 1, 2, 50, storage=16),
         ]
+        next_rows = next_rows_legs(binding, torch, dev, stream, local, "c3_32x64_fp32", U, 18)
 
     line = None
     if rank == 0:
@@ -568,6 +645,7 @@ def run_wd(args):
             line["cpu_baseline"] = cpu
         if secondary is not None:
             line["secondary"] = secondary
+            line["next_rows"] = next_rows
         print(json.dumps(line), flush=True)
     op.close()
     if world > 1:
