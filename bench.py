@@ -26,7 +26,8 @@ One JSON line on stdout (rank 0).  Definitions:
                are unchanged.
   * next_rows  (default run only) short legs of the rows built after the hot path, on the headline's lattice and links:
                the even-odd preconditioned operator (f1), CGNR / BiCGstab / GCR(8) on it (f2; 48 iterations each) and the
-               block CGNR on 12 right-hand sides; each with its own byte model, roofline fraction and clocks record.
+               block CGNR on 12 right-hand sides, restrict + prolong and the coarse operator apply at N_v = 20 (f3); each
+               with its own byte model, roofline fraction and clocks record.
   * cpu_baseline  the oracle (oracle/wd_oracle.c, fp64, OpenMP) on this box's host cores, on a
                bounded sample of the same workload.
 Multi-GPU (torchrun): the path has no exchange step on one GPU per lattice; ranks run independent
@@ -370,8 +371,50 @@ def next_rows_legs(binding, torch, dev, stream, local, name, U, recon):
     out.append(entry("f2 + a'", "block CGNR on Mhat, 12 right-hand sides in lock step", 10, "iteration", ms,
                      (nmv * (2 * 1320 + 48) + bf) * (V // 2) * 12,
                      (V // 2) * (nmv * (2 * 2 * 4 * recon * w + 12 * 5 * 24 * w) + 12 * bp * 24 * w), nl, ck, nrhs=12))
-    op.close()
     del b, x, tmp
+    torch.cuda.empty_cache()
+    # ---- row f3 (N_v = 20): restrict + prolong, coarse operator build and apply ----
+    nv, nc = 20, 40
+    nb = V // 256
+    with torch.cuda.stream(stream):
+        basis = torch.randn(op.native_numel(nv), dtype=torch.float32, device=dev, generator=g)
+        psi = torch.randn(op.native_numel(1), dtype=torch.float32, device=dev, generator=g)
+        res = torch.empty_like(psi)
+        coarse = torch.empty(binding.wd_coarse_reals(op.lat, nv), dtype=torch.float32, device=dev)
+        binding.wd_block_orthonormalise(op.lat, basis, nv, 32, stream.cuda_stream)
+
+    def transfer():
+        binding.wd_restrict(op.lat, coarse, basis, psi, nv, 32, stream.cuda_stream)
+        binding.wd_prolong(op.lat, res, basis, coarse, nv, 32, stream.cuda_stream)
+
+    ms, nl, ck = timed(transfer, 5)
+    out.append(entry("f3", "restrict + prolong, N_v = 20, 4^4 blocks x 2 chiralities", 1, "step", ms, 2 * nv * V * 12 * 8,
+                     (2 * nv + 2) * V * 24 * w, nl, ck))
+    ns = binding.wd_coarse_stencil_reals(op.lat, nv)
+    with torch.cuda.stream(stream):
+        S = torch.empty(ns, dtype=torch.float32, device=dev)
+        scratch = torch.empty(ns, dtype=torch.float32, device=dev)
+        cin = [torch.randn(nb * nc * 2, dtype=torch.float32, device=dev, generator=g) for _ in range(2)]
+        cout = [torch.empty_like(cin[0]) for _ in range(2)]
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    binding.wd_build_coarse(op.gauge, S, scratch, basis, cfg.mass, cfg.dims, nv, 32)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    build_ms = ev0.elapsed_time(ev1)
+    del scratch, basis, psi, res
+
+    def coarse_apply():
+        for i in range(20):
+            binding.wd_apply_coarse(op.lat, cout[i % 2], cin[i % 2], S, nv, 1, 32, stream.cuda_stream)
+
+    ms, nl, ck = timed(coarse_apply, 3)
+    e = entry("f3", "coarse operator apply, 9-point stencil of (2 N_v)^2 complex blocks, N_v = 20", 20, "apply", ms,
+              nb * 9 * nc * nc * 8, nb * (9 * nc * nc * 2 * w + 2 * nc * 2 * w), nl, ck)
+    e["build_ms_first_call"] = build_ms
+    out.append(e)
+    op.close()
+    del S, cin, cout, coarse
     torch.cuda.empty_cache()
     return out
 
