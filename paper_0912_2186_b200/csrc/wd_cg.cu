@@ -610,8 +610,10 @@ constexpr int GCR_GROUP = 8; // earlier directions handled per pass over the new
 
 // part[(2 i + c) * RED_BLOCKS + b] = partials of <q_{i0+i}, q_j> (c = 0 real, 1 imaginary part), i < ni <= GCR_GROUP:
 // q_j is read once for all of them.  q_i = qbase + i * stride
+// (RED_BLOCKS is 4 CTAs per SM: the register cap keeps all of them resident -- at 80 registers only three fit and the fourth
+// ran as a second, nearly empty wave: 116 us for two passes over the vectors where the plain inner-product kernel takes 37)
 template <typename Vec, int NCH>
-__global__ void __launch_bounds__(RED_THREADS)
+__global__ void __launch_bounds__(RED_THREADS, 4)
 gcr_dots_kernel(const Vec *__restrict__ qbase, long long stride, int i0, int ni, const Vec *__restrict__ qj, long long nvec,
                 long long Vh, double *part)
 {
@@ -644,7 +646,7 @@ gcr_dots_kernel(const Vec *__restrict__ qbase, long long stride, int i0, int ni,
 // form the oracle writes out).  psrc may be p_j itself, or r for an unpreconditioned direction (p_j = r needs no copy).
 // FINAL (the last group): also the partials of <q_j, r> and |q_j|^2 of the finished direction.
 template <typename Vec, int NCH, bool FINAL>
-__global__ void __launch_bounds__(RED_THREADS)
+__global__ void __launch_bounds__(RED_THREADS, 4)
 gcr_orth_kernel(Vec *pj, const Vec *psrc, Vec *__restrict__ qj, const Vec *__restrict__ pbase, const Vec *__restrict__ qbase,
                 long long stride, int i0, int ni, long long nvec, long long Vh, const double *part, const double *qq,
                 const Vec *__restrict__ r, double *qr_part, double *qq_part)
