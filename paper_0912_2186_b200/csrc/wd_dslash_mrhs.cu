@@ -28,6 +28,7 @@
 #include "wd_internal.h"
 #include "wd_layout.cuh"
 #include "wd_async.cuh"
+#include "wd_bulk.cuh"
 #include "wd_math.cuh"
 #include "wd_link.cuh"
 
@@ -36,30 +37,7 @@ namespace wd {
 namespace {
 
 
-// ---- bulk-copy (cp.async.bulk + mbarrier) variant of the link staging: the A/B the round-1 review asked for ----
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long *b, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(b)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect(unsigned long long *b, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *b)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(b))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity)
-{
-    asm volatile("{\n.reg .pred p;\nWAIT_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n" ::"r"(
-                     smem_u32(b)),
-                 "r"(parity)
-                 : "memory");
-}
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+// bulk-copy (cp.async.bulk + mbarrier) variant of the link staging: the A/B the round-1 review asked for; helpers in wd_bulk.cuh
 
 template <int NV>
 __device__ __forceinline__ void lds_vecs(const float4 *buf, int stride, int slot, float *r)
@@ -243,7 +221,7 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         if (tid == 0) {
             mbar_init(&mbar[0], 1);
             mbar_init(&mbar[1], 1);
-            asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+            fence_mbar_init();
         }
         __syncthreads();
     }

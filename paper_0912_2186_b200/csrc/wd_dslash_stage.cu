@@ -492,7 +492,8 @@ bool stage_supported(const ApplyArgs &a)
     return smem <= 227 * 1024;
 }
 
-cudaError_t launch_mrhs(const ApplyArgs &a, int ty, int tz); // wd_dslash_mrhs.cu
+cudaError_t launch_mrhs(const ApplyArgs &a, int ty, int tz);  // wd_dslash_mrhs.cu
+cudaError_t launch_rloop(const ApplyArgs &a, int ty, int tz); // wd_dslash_rloop.cu
 
 cudaError_t launch_stage(const ApplyArgs &a)
 {
@@ -503,6 +504,11 @@ cudaError_t launch_stage(const ApplyArgs &a)
     // right-hand side) order, which shares the links through L2, is the faster one (20 RHS on 24^3 x 64: 1.30 against
     // 1.39 ms).  stage_no_mrhs = 0 / 1 forces the choice.
     const bool pow2 = !(a.dims[0] & (a.dims[0] - 1));
+    if (a.precision == 32 && a.nrhs > 1 && pow2 && tn.mrhs_reg > 0) { // links in registers, loop over the right-hand sides
+        StageShape s;
+        if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
+        if (s.nt <= 128) return launch_rloop(a, s.ty, s.tz);
+    }
     if (a.precision == 32 && a.recon != 8 && a.nrhs > 1 && !a.dagger && (tn.stage_no_mrhs < 0 ? pow2 : tn.stage_no_mrhs == 0)) {
         StageShape s;
         if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
