@@ -303,7 +303,7 @@ dslash_rloop_kernel(float *__restrict__ out, const float *__restrict__ in, const
 // 6 KB x rgrp: rgrp <= 5 for two CTAs per SM.
 constexpr int RING_ROWV = 6 * 32;                    // 16-byte vectors of one row slot
 constexpr int ring_smem_vecs(int rgrp) { return 4 * 4 * RING_ROWV + 2 * 2 * 3 * 128 + 2 * 5 * 64 + rgrp * 3 * 128; }
-constexpr size_t ring_smem_bytes(int rgrp) { return (size_t)ring_smem_vecs(rgrp) * 16 + 16 * 8; }
+constexpr size_t ring_smem_bytes(int rgrp) { return (size_t)ring_smem_vecs(rgrp) * 16 + 17 * 8; }
 
 template <int RECON, int SGN>
 __global__ void __launch_bounds__(128, 2)
@@ -320,7 +320,9 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
     float4 *const exch = smem + 4 * 4 * RING_ROWV;        // [2 buffers][y, z][3][128]
     float4 *const fl = exch + 2 * 2 * 3 * nts;            // [y, z][5][64] face links (18 reals + 2 pad per site)
     float4 *const carry = fl + 2 * 5 * 64;                // [rgrp][3][128]
-    unsigned long long *const mb = reinterpret_cast<unsigned long long *>(carry + rgrp * 3 * nts) + w * 4;
+    unsigned long long *const mb0 = reinterpret_cast<unsigned long long *>(carry + rgrp * 3 * nts);
+    unsigned long long *const mb = mb0 + w * 4; // this warp's four row slots
+    unsigned long long *const xbar = mb0 + 16;  // the CTA's exchange barrier: arrive after the sends, wait before the receives
 
     const int ncy = Ly / ty;
     const int ncol = ncy * (Lz / tz);
@@ -372,9 +374,10 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
     if (lane == 0) {
 #pragma unroll
         for (int s = 0; s < 4; ++s) mbar_init(&mb[s], 1);
+        if (w == 0) mbar_init(xbar, nts);
         fence_mbar_init();
     }
-    __syncwarp();
+    __syncthreads();
     auto slot_off = [&](int t) { return (long long)t * S3 * 6; };
     auto wrap = [&](int t) { return t >= Lt ? t - Lt : t; };
     auto issue = [&](int slot, const float4 *src) { // lane 0 only
@@ -441,11 +444,6 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
             mbar_wait(&mb[OWN], ph);
 #pragma unroll
             for (int c = 0; c < 6; ++c) unpack(ring[OWN * RING_ROWV + c * 32 + lane], &psi[4 * c]);
-            __syncwarp();
-            if (lane == 0 && has_next) {
-                fence_proxy_async();
-                issue(OWN, row_own + noff);
-            }
 #pragma unroll
             for (int i = 0; i < 24; ++i) acc[i] = 0.f;
             // ---- x ----
@@ -475,15 +473,17 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
                 su3_dag_mul(uz, h, chi);
                 sts_half(ez, nts, st, chi);
             }
+            mbar_arrive(xbar); // this thread's half spinors of the pass are in the exchange buffer
             // ---- t ----
             {
                 float pn[24];
                 mbar_wait(&mb[TP], ph);
 #pragma unroll
                 for (int c = 0; c < 6; ++c) unpack(ring[TP * RING_ROWV + c * 32 + lane], &pn[4 * c]);
-                __syncwarp();
+                __syncwarp(); // every lane has read its words of the two slots: refill them for the next pass
                 if (lane == 0 && has_next) {
-                    fence_proxy_async();
+                    fence_proxy_async(); // required (measured: without it a refill can overtake the reads above)
+                    issue(OWN, row_own + noff);
                     issue(TP, row_own + noff_tp);
                 }
                 project<3, SGN>(pn, h);
@@ -502,11 +502,6 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
                 mbar_wait(&mb[FY], ph);
 #pragma unroll
                 for (int c = 0; c < 6; ++c) unpack(ring[FY * RING_ROWV + c * 32 + lane], &pn[4 * c]);
-                __syncwarp();
-                if (lane == 0 && has_next) {
-                    fence_proxy_async();
-                    issue(FY, row_y + noff);
-                }
                 if (yy) {
                     project<1, SGN>(pn, h);
                     su3_mul(uy, h, chi);
@@ -527,7 +522,8 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
                 for (int c = 0; c < 6; ++c) unpack(ring[FZ * RING_ROWV + c * 32 + lane], &pn[4 * c]);
                 __syncwarp();
                 if (lane == 0 && has_next) {
-                    fence_proxy_async();
+                    fence_proxy_async(); // required (measured: without it a refill can overtake the reads above)
+                    issue(FY, row_y + noff);
                     issue(FZ, row_z + noff);
                 }
                 if (zz) {
@@ -543,7 +539,7 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
                     reconstruct_add<2, -SGN>(acc, chi);
                 }
             }
-            __syncthreads(); // the exchange buffer `buf` of this (slice, rhs) is complete
+            mbar_wait(xbar, ph); // everybody's: the exchange buffer `buf` of this (slice, rhs) is complete
             if (yy) {
                 lds_half(ey, nts, st - 32, chi);
                 reconstruct_add<1, -SGN>(acc, chi);
@@ -652,7 +648,7 @@ cudaError_t launch_ring_s(const ApplyArgs &a)
 template <int RECON> cudaError_t launch_rloop_r(const ApplyArgs &a, int ty, int tz)
 {
     const Tuning &tn = a.tune ? *a.tune : default_tuning();
-    if (tn.mrhs_reg >= 2 && a.dims[0] == 32 && ty == 2 && tz == 2)
+    if (tn.mrhs_reg != 1 && a.dims[0] == 32 && ty == 2 && tz == 2) // the ring member wherever it applies
         return a.dagger ? launch_ring_s<RECON, +1>(a) : launch_ring_s<RECON, -1>(a);
     return a.dagger ? launch_rloop_s<RECON, +1>(a, ty, tz) : launch_rloop_s<RECON, -1>(a, ty, tz);
 }

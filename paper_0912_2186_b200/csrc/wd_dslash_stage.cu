@@ -504,7 +504,12 @@ cudaError_t launch_stage(const ApplyArgs &a)
     // right-hand side) order, which shares the links through L2, is the faster one (20 RHS on 24^3 x 64: 1.30 against
     // 1.39 ms).  stage_no_mrhs = 0 / 1 forces the choice.
     const bool pow2 = !(a.dims[0] & (a.dims[0] - 1));
-    if (a.precision == 32 && a.nrhs > 1 && pow2 && tn.mrhs_reg > 0) { // links in registers, loop over the right-hand sides
+    // links in registers, loop over the right-hand sides (wd_dslash_rloop.cu): by measurement (profiles/r02_ncu.md section 10)
+    // the default only for 8-real links on Lx = 32, where the rebuild is paid once per group of right-hand sides instead
+    // of once per right-hand side (24 RHS on 32^3 x 64: 3.94 against 4.19 ms); mrhs_reg = 0 / 1 / 2 forces off / the
+    // plain-load member / the ring member
+    if (a.precision == 32 && a.nrhs > 1 && pow2 &&
+        (tn.mrhs_reg > 0 || (tn.mrhs_reg < 0 && a.recon == 8 && a.dims[0] == 32 && !a.dagger))) {
         StageShape s;
         if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
         if (s.nt <= 128) return launch_rloop(a, s.ty, s.tz);
