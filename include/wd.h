@@ -134,10 +134,10 @@ int wd_set_stream(wd_gauge *gauge, void *stream);
 
 /* Tuning variables of the launchers.  They are read from the environment ONCE, at wd_load_gauge
  * (WD_TILE_SHAPE=ty,tz, WD_TILE_TC, WD_TILE_NCHUNK, WD_TILE_NRB, WD_MRHS_PATCH, WD_STAGE_NO_MRHS, WD_SITE_SLAB_MB,
- * WD_HOST_NO_PIPELINE, WD_MRHS_NO_TAIL, WD_HOST_NSLAB, WD_MRHS_BULK, WD_MRHS_REG, WD_MRHS_RGRP), and stored in the gauge handle; no launch reads the environment.
+ * WD_HOST_NO_PIPELINE, WD_MRHS_NO_TAIL, WD_HOST_NSLAB, WD_MRHS_BULK, WD_MRHS_REG, WD_MRHS_RGRP, WD_STAGE_BULK), and stored in the gauge handle; no launch reads the environment.
  * wd_set_tuning changes one of them afterwards: name is the lower-case variable without the WD_ prefix ("tile_ty",
  * "tile_tz", "tile_tc", "tile_nchunk", "tile_nrb", "mrhs_patch", "stage_no_mrhs", "site_slab_mb", "host_no_pipeline",
- * "mrhs_no_tail", "host_nslab", "mrhs_bulk", "mrhs_reg", "mrhs_rgrp"); value < 0 restores the default.  WD_ERR_MISMATCH for an unknown name.  Host-only. */
+ * "mrhs_no_tail", "host_nslab", "mrhs_bulk", "mrhs_reg", "mrhs_rgrp", "stage_bulk"); value < 0 restores the default.  WD_ERR_MISMATCH for an unknown name.  Host-only. */
 int wd_set_tuning(wd_gauge *gauge, const char *name, int value);
 
 /* Temporal gauge ("temporal gauge fixing", Fig. 4 / Table 2 "GF"): on != 0 declares that the loaded links

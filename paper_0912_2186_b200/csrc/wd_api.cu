@@ -110,6 +110,7 @@ void tuning_from_env(Tuning &t)
     t.mrhs_no_tail = env_int("WD_MRHS_NO_TAIL");
     t.host_nslab = env_int("WD_HOST_NSLAB");
     t.mrhs_bulk = env_int("WD_MRHS_BULK");
+    t.stage_bulk = env_int("WD_STAGE_BULK");
     t.mrhs_reg = env_int("WD_MRHS_REG");
     t.mrhs_rgrp = env_int("WD_MRHS_RGRP");
 }
@@ -122,7 +123,7 @@ int tuning_set(Tuning &t, const char *name, int value)
         {"stage_no_mrhs", &Tuning::stage_no_mrhs}, {"site_slab_mb", &Tuning::site_slab_mb},
         {"host_no_pipeline", &Tuning::host_no_pipeline}, {"mrhs_no_tail", &Tuning::mrhs_no_tail},
         {"host_nslab", &Tuning::host_nslab}, {"mrhs_bulk", &Tuning::mrhs_bulk},
-        {"mrhs_reg", &Tuning::mrhs_reg}, {"mrhs_rgrp", &Tuning::mrhs_rgrp}};
+        {"mrhs_reg", &Tuning::mrhs_reg}, {"stage_bulk", &Tuning::stage_bulk}, {"mrhs_rgrp", &Tuning::mrhs_rgrp}};
     for (auto &e : tab)
         if (!strcmp(name, e.n)) {
             t.*(e.f) = value < 0 ? -1 : value;

@@ -494,6 +494,7 @@ bool stage_supported(const ApplyArgs &a)
 
 cudaError_t launch_mrhs(const ApplyArgs &a, int ty, int tz);  // wd_dslash_mrhs.cu
 cudaError_t launch_rloop(const ApplyArgs &a, int ty, int tz); // wd_dslash_rloop.cu
+cudaError_t launch_stage_bulk(const ApplyArgs &a);             // wd_dslash_stage_bulk.cu
 
 cudaError_t launch_stage(const ApplyArgs &a)
 {
@@ -518,6 +519,11 @@ cudaError_t launch_stage(const ApplyArgs &a)
         StageShape s;
         if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
         if (s.nt <= 128) return launch_mrhs(a, s.ty, s.tz); // (a forced bigger tile runs through the single-RHS kernel below)
+    }
+    if (a.dims[0] == 32 && tn.stage_bulk > 0) { // bulk-copy member: one warp = one x-row = one layout block
+        StageShape s;
+        if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
+        if (s.ty == 2 && s.tz == 2) return launch_stage_bulk(a);
     }
     if (a.precision == 32)
         return a.recon == 18 ? launch_stage_t<float, 18>(a) : a.recon == 12 ? launch_stage_t<float, 12>(a) : launch_stage_t<float, 8>(a);

@@ -18,6 +18,7 @@ struct Tuning {
     int mrhs_no_tail = -1;          // WD_MRHS_NO_TAIL  1 = no shortened t-chunks in the last wave of the multi-RHS kernel
     int mrhs_bulk = -1;             // WD_MRHS_BULK     1 = stage the links of the multi-RHS kernel by cp.async.bulk (A/B variant)
     int host_nslab = -1;            // WD_HOST_NSLAB    slabs of the pipelined wd_apply_host (3..32, default 16)
+    int stage_bulk = -1;            // WD_STAGE_BULK    staged kernel on Lx = 32: 1 = bulk-copy member (wd_dslash_stage_bulk.cu), 0 = per-thread cp.async
     int mrhs_reg = -1;              // WD_MRHS_REG      multi-RHS member with the links in registers (wd_dslash_rloop.cu): 0 = never, 1 = plain-load
                                     //                  member, 2 = ring member (Lx = 32; else plain-load); unset: 8-real links on Lx = 32 only
     int mrhs_rgrp = -1;             // WD_MRHS_RGRP     right-hand sides per group of that member (default: what two CTAs per SM allow)
