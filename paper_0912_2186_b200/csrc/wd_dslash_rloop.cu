@@ -586,7 +586,10 @@ cudaError_t launch_rloop_s(const ApplyArgs &a, int ty, int tz)
     const int budget = 113 * 1024 / 16;
     int rmax = (budget - rloop_smem_vecs(nts, ty, tz, 0)) / (3 * nts);
     if (rmax < 1) return cudaErrorInvalidConfiguration;
-    if (tn.mrhs_rgrp >= 1) rmax = tn.mrhs_rgrp;
+    if (tn.mrhs_rgrp >= 1) { // forced group size, up to what one CTA per SM can hold
+        const int rcap = (227 * 1024 / 16 - rloop_smem_vecs(nts, ty, tz, 0)) / (3 * nts);
+        rmax = tn.mrhs_rgrp < rcap ? tn.mrhs_rgrp : rcap;
+    }
     int ngroups = (a.nrhs + rmax - 1) / rmax;
     const int rgrp = (a.nrhs + ngroups - 1) / ngroups;
     ngroups = (a.nrhs + rgrp - 1) / rgrp;
@@ -619,7 +622,10 @@ cudaError_t launch_ring_s(const ApplyArgs &a)
     auto kern = dslash_rloop_ring_kernel<RECON, SGN>;
     const Tuning &tn = a.tune ? *a.tune : default_tuning();
     int rmax = 5; // two CTAs per SM
-    if (tn.mrhs_rgrp >= 1) rmax = tn.mrhs_rgrp;
+    if (tn.mrhs_rgrp >= 1) { // forced group size, up to what one CTA per SM can hold
+        const int rcap = (int)((227 * 1024 - ring_smem_bytes(0)) / (3 * 128 * 16));
+        rmax = tn.mrhs_rgrp < rcap ? tn.mrhs_rgrp : rcap;
+    }
     int ngroups = (a.nrhs + rmax - 1) / rmax;
     const int rgrp = (a.nrhs + ngroups - 1) / ngroups;
     ngroups = (a.nrhs + rgrp - 1) / rgrp;

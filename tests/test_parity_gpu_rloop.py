@@ -60,7 +60,7 @@ def test_rloop_shapes(oracle, monkeypatch, dims, recon):
 
 
 @pytest.mark.parametrize("nrhs", [2, 3, 7, 12, 20, 24, 29])
-@pytest.mark.parametrize("rgrp", [None, "1", "3", "8"])
+@pytest.mark.parametrize("rgrp", [None, "1", "3", "8", "1000"])
 def test_rloop_groups_and_partial_groups(oracle, monkeypatch, nrhs, rgrp):
     """Group sizes that do and do not divide nrhs (a partial last group simply loops over fewer right-hand sides)."""
     monkeypatch.setenv("WD_MRHS_REG", "1")
@@ -123,7 +123,7 @@ def test_ring_shapes(oracle, monkeypatch, dims, recon):
         run(oracle, fields.Config("ring", dims, 32, "haar", recon, -0.3, nrhs, 67))
 
 
-@pytest.mark.parametrize("rgrp", [None, "1", "3", "5"])
+@pytest.mark.parametrize("rgrp", [None, "1", "3", "5", "1000"])
 @pytest.mark.parametrize("tc", ["1", "2", "5", "100"])
 @pytest.mark.parametrize("patch", ["0", "2"])
 def test_ring_groups_chunks_and_block_orders(oracle, monkeypatch, rgrp, tc, patch):
