@@ -500,6 +500,20 @@ def test_kernels_write_only_their_output(dims, precision, recon, nrhs, kernel):
     op.close()
 
 
+@pytest.mark.parametrize("env,dims,precision,recon,nrhs", [
+    ({"WD_MRHS_REG": "1"}, (16, 8, 8, 6), 32, 18, 5), ({"WD_MRHS_REG": "1"}, (32, 4, 4, 5), 32, 12, 4),
+    ({"WD_MRHS_REG": "2"}, (32, 4, 4, 5), 32, 18, 7), ({"WD_MRHS_REG": "2"}, (32, 8, 4, 3), 32, 8, 3),
+    ({"WD_STAGE_BULK": "1"}, (32, 4, 4, 5), 32, 18, 1), ({"WD_STAGE_BULK": "1"}, (32, 4, 8, 4), 64, 12, 1),
+    ({"WD_STAGE_BULK": "1", "WD_STAGE_NO_MRHS": "1"}, (32, 4, 4, 3), 32, 18, 3)])
+def test_round2_late_members_write_only_their_output(monkeypatch, env, dims, precision, recon, nrhs):
+    """Guard bands around the buffers of the members added late in round 2: the links-in-registers multi-RHS kernels (plain
+    loads, ring of cp.async.bulk row copies) and the bulk-copy member of the single-RHS staged kernel.  A bulk copy that ran
+    past its row, or a prefetch-distance bug turned into a store, would show up here."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    test_kernels_write_only_their_output(dims, precision, recon, nrhs, "stage")
+
+
 # ---------------------------------------------------------------- a lattice beyond 2^31 bytes per field: sampled outputs
 def test_large_lattice_sampled_against_the_oracle(oracle):
     """32 x 48 x 72 x 64 (7.1 M sites: the link field is 2.0 GB, byte offsets beyond 2^31; 864 tile columns):
