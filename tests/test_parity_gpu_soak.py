@@ -11,7 +11,10 @@ pytestmark = pytest.mark.gpu
 
 SHAPES = [(32, 6, 4, 3), (32, 10, 2, 2), (16, 12, 6, 5), (8, 16, 4, 9), (4, 8, 24, 2), (32, 4, 12, 7), (24, 8, 2, 4),
           (12, 8, 4, 6), (16, 2, 2, 17), (32, 2, 6, 1), (32, 12, 12, 3)]
-ENVS = [{}, {"WD_TILE_TC": "1"}, {"WD_TILE_TC": "3", "WD_TILE_NRB": "2"}, {"WD_MRHS_PATCH": "0", "WD_TILE_SHAPE": "2,2"}]
+ENVS = [{}, {"WD_TILE_TC": "1"}, {"WD_TILE_TC": "3", "WD_TILE_NRB": "2"}, {"WD_MRHS_PATCH": "0", "WD_TILE_SHAPE": "2,2"},
+        # the members added late in round 2 (they apply where Lx is a power of two / Lx = 32 and fall through elsewhere)
+        {"WD_MRHS_REG": "1", "WD_MRHS_RGRP": "3"}, {"WD_MRHS_REG": "2", "WD_TILE_TC": "2"}, {"WD_STAGE_BULK": "1"},
+        {"WD_STAGE_BULK": "1", "WD_STAGE_NO_MRHS": "1", "WD_TILE_TC": "3"}]
 
 
 @pytest.mark.parametrize("dims", SHAPES)
