@@ -303,7 +303,7 @@ def secondary_leg(binding, torch, dev, stream, local, name, U, recon, nrhs, step
             "recon": recon, "dtype": {16: "f32 arithmetic on f16 storage", 32: "f32", 64: "f64"}[prec],
             "bytes_per_site": compulsory_bytes_per_site(prec, recon, nrhs), "us_per_apply": ms * 1e3,
             "steps": steps, "applies_per_step": aps, "gpu_launches": int(launches),
-            "data": "synthetic: headline links recipe (smooth, eps=0.3), device-drawn Gaussian spinors",
+            "data": "synthetic: " + ("headline links recipe (smooth, eps=0.3)" if cfg.links == "smooth" else "the workload's links recipe (" + cfg.links + ")") + ", device-drawn Gaussian spinors",
             "roofline": roof, "clocks": ck}
 
 
@@ -649,6 +649,14 @@ def run_wd(args):
             secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp32", U, 8, 1, 2, 50),
             secondary_leg(binding, torch, dev, stream, local, "c3_32x64_fp32", U, 12, 1, 2, 50, storage=16),
         ]
+        # configs[2] (24^3 x 64, 12-real links: Lx not a power of two) and the paper's own set-up shape on it: N_v = 20
+        # right-hand sides on a 24^3 x 64 volume
+        U2, _ = fields.make_fields(fields.CONFIGS["c2_24x64_fp32_r12"], nrhs=1)
+        secondary += [
+            secondary_leg(binding, torch, dev, stream, local, "c2_24x64_fp32_r12", U2, 12, 1, 2, 50),
+            secondary_leg(binding, torch, dev, stream, local, "c2_24x64_fp32_r12", U2, 12, 20, 2, 10),
+        ]
+        del U2
         next_rows = next_rows_legs(binding, torch, dev, stream, local, "c3_32x64_fp32", U, 18)
 
     line = None
