@@ -480,7 +480,24 @@ cudaError_t launch_mrhs_r(const ApplyArgs &a, int ty, int tz)
     const Tuning &tn = a.tune ? *a.tune : default_tuning();
     int nrb = a.nrhs >= 3 ? 3 : a.nrhs;
     if (tn.tile_nrb >= 1 && tn.tile_nrb <= 3) nrb = tn.tile_nrb;
-    if (nrb >= 3) return launch_mrhs_t<RECON, 3>(a, ty, tz);
+    if (nrb >= 3) {
+        // A partial last group of three computes duplicates that are thrown away (4 right-hand sides cost what 6 do).
+        // Measured on 32^3 x 64 (profiles/r02_ncu.md section 12): it pays to give the remainder its own launch when it is a
+        // single right-hand side (the single-RHS staged kernel) or a pair behind at least two full groups (groups of two).
+        const int rem = a.nrhs % 3;
+        if (tn.tile_nrb < 0 && a.nrhs > 3 && (rem == 1 || (rem == 2 && a.nrhs >= 8))) {
+            ApplyArgs m = a, r = a;
+            m.nrhs = a.nrhs - rem;
+            cudaError_t e = launch_mrhs_t<RECON, 3>(m, ty, tz);
+            if (e != cudaSuccess) return e;
+            const size_t field = (size_t)24 * padded_volume(a.V) * sizeof(float); // one right-hand side (fp32)
+            r.in = (const char *)a.in + field * m.nrhs;
+            r.out = (char *)a.out + field * m.nrhs;
+            r.nrhs = rem;
+            return rem == 1 ? launch_stage(r) : launch_mrhs_t<RECON, 2>(r, ty, tz);
+        }
+        return launch_mrhs_t<RECON, 3>(a, ty, tz);
+    }
     if (nrb == 2) return launch_mrhs_t<RECON, 2>(a, ty, tz);
     return launch_mrhs_t<RECON, 1>(a, ty, tz);
 }
