@@ -101,7 +101,7 @@ template <int RECON> constexpr int mrhs_smem_vecs(int nts, int nrb, int nyb, int
 // thread, completion through an mbarrier) instead of one 16-byte cp.async per thread and vector; Lx = 32 only (a row of
 // the tile is one layout block).  Selected by the tuning variable mrhs_bulk; measured against the default in
 // profiles/r02_ncu.md section 6.
-template <int RECON, int NRB, int NTS, bool XS, bool BULK = false>
+template <int RECON, int NRB, int NTS, bool XS, bool BULK = false, int SGN = -1>
 __global__ void __launch_bounds__(128 * NRB, 1)
 dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const float *__restrict__ links, int Lx, int Ly,
                    int Lz, int Lt, int ty, int tz, long long V, float cdiag, int nrhs, int nchunk, int patch, int tgauge,
@@ -287,7 +287,7 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         const long long site_tb = s3 + (long long)tb * S3;
         float u[18], p[24], h[12];
         load_spinor(in, site_tb, p);
-        project<3, +1>(p, h);
+        project<3, -SGN>(p, h);
         if (unit_t(tb)) {
 #pragma unroll
             for (int i = 0; i < 12; ++i) chi_t[i] = h[i];
@@ -317,33 +317,33 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         if (t == t_begin) lds_vecs<6>(pl, nt, tid, psi);
 #pragma unroll
         for (int i = 0; i < 24; ++i) acc[i] = 0.f;
-        reconstruct_add<3, +1>(acc, chi_t); // backward t hop, product carried from the previous slice
+        reconstruct_add<3, -SGN>(acc, chi_t); // backward t hop, product carried from the previous slice
 
         // ---- x: both hops through warp shuffles (XS), else like y and z ----
         own_link_rd<0, RECON, BULK>(lnk, nts, st, u);
         if (!XS) {
             const int dxf = (x + 1 == Lx ? 1 - Lx : 1), dxb = (x == 0 ? Lx - 1 : -1);
             lds_vecs<6>(pl, nt, tid + dxf, pn);
-            hop_forward<0>(acc, u, pn);
+            hop_forward_s<0, SGN>(acc, u, pn);
             own_link_rd<0, RECON, BULK>(lnk, nts, st + dxb, u);
             lds_vecs<6>(pl, nt, tid + dxb, pn);
-            hop_backward<0>(acc, u, pn);
+            hop_backward_s<0, SGN>(acc, u, pn);
         } else {
             float h[12], gg[12], chi[12];
-            project<0, -1>(psi, h);
+            project<0, SGN>(psi, h);
             shfl12(gg, h, lane_r); // P-_x psi(x+1)
             su3_mul(u, gg, chi);
-            reconstruct_add<0, -1>(acc, chi);
-            project<0, +1>(psi, h);
+            reconstruct_add<0, SGN>(acc, chi);
+            project<0, -SGN>(psi, h);
             su3_dag_mul(u, h, chi); // U_x(x)^dag P+_x psi(x): belongs to x+1
             shfl12(gg, chi, lane_l);
-            reconstruct_add<0, +1>(acc, gg);
+            reconstruct_add<0, -SGN>(acc, gg);
         }
         // ---- y: forward with the own link, backward with the link of the site below ----
         own_link_rd<1, RECON, BULK>(lnk, nts, st, u);
         if (face_yf) lds_vecs<6>(fy, nt, tid, pn);
         else lds_vecs<6>(pl, nt, tid + Lx, pn);
-        hop_forward<1>(acc, u, pn);
+        hop_forward_s<1, SGN>(acc, u, pn);
         if (face_yb) {
             if (BULK) lds_link<1, RECON>(fly + (rank_y >> 5) * (FY::n * 32), FY::first, 32, rank_y & 31, u);
             else lds_link<1, RECON>(fly, FY::first, nyb, rank_y, u);
@@ -352,7 +352,7 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
             own_link_rd<1, RECON, BULK>(lnk, nts, st - Lx, u);
             lds_vecs<6>(pl, nt, tid - Lx, pn);
         }
-        hop_backward<1>(acc, u, pn);
+        hop_backward_s<1, SGN>(acc, u, pn);
         if (more && (face_yf | face_yb)) stage_spinor(fy, sp_y, toff_n);
         cpa_commit(); // c2
         cpa_wait<1>();   // links z,t of slice t, own spinor of slice t+1, z-face spinor of slice t have landed
@@ -367,7 +367,7 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
         own_link_rd<2, RECON, BULK>(lnk, nts, st, u);
         if (face_zf) lds_vecs<6>(fz, nt, tid, pn);
         else lds_vecs<6>(pl, nt, tid + Lx * ty, pn);
-        hop_forward<2>(acc, u, pn);
+        hop_forward_s<2, SGN>(acc, u, pn);
         if (face_zb) {
             if (BULK) lds_link<2, RECON>(flz + (rank_z >> 5) * (FZ::n * 32), FZ::first, 32, rank_z & 31, u);
             else lds_link<2, RECON>(flz, FZ::first, nzb, rank_z, u);
@@ -376,7 +376,7 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
             own_link_rd<2, RECON, BULK>(lnk, nts, st - Lx * ty, u);
             lds_vecs<6>(pl, nt, tid - Lx * ty, pn);
         }
-        hop_backward<2>(acc, u, pn);
+        hop_backward_s<2, SGN>(acc, u, pn);
         if (more && (face_zf | face_zb)) stage_spinor(fz, sp_z, toff_n);
         cpa_commit(); // c4
         // ---- t: forward hop now, backward product for the next slice ----
@@ -384,13 +384,13 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
             float h[12];
             lds_vecs<6>(plane0 + (cur ^ 1) * plane_sz, nt, tid, pnx);
             if (unit_t(t)) { // U_t(x,t) = 1: projection and reconstruction only
-                project<3, -1>(pnx, h);
-                reconstruct_add<3, -1>(acc, h);
-                project<3, +1>(psi, chi_t);
+                project<3, SGN>(pnx, h);
+                reconstruct_add<3, SGN>(acc, h);
+                project<3, -SGN>(psi, chi_t);
             } else {
                 own_link_rd<3, RECON, BULK>(lnk, nts, st, u);
-                hop_forward<3>(acc, u, pnx);
-                project<3, +1>(psi, h);
+                hop_forward_s<3, SGN>(acc, u, pnx);
+                project<3, -SGN>(psi, h);
                 su3_dag_mul(u, h, chi_t);
             }
         }
@@ -414,10 +414,10 @@ dslash_mrhs_kernel(float *__restrict__ out, const float *__restrict__ in, const 
 // ---------------------------------------------------------------------------------------------
 namespace {
 
-template <int RECON, int NRB, int NTS, bool XS, bool BULK = false>
+template <int RECON, int NRB, int NTS, bool XS, bool BULK = false, int SGN = -1>
 cudaError_t launch_mrhs_n(const ApplyArgs &a, int ty, int tz)
 {
-    auto kern = dslash_mrhs_kernel<RECON, NRB, NTS, XS, BULK>;
+    auto kern = dslash_mrhs_kernel<RECON, NRB, NTS, XS, BULK, SGN>;
     const int Lx = a.dims[0];
     const int nts = Lx * ty * tz;
     const size_t smem = (size_t)mrhs_smem_vecs<RECON>(nts, NRB, Lx * tz, Lx * ty) * sizeof(float4);
@@ -467,9 +467,12 @@ template <int RECON, int NRB>
 cudaError_t launch_mrhs_t(const ApplyArgs &a, int ty, int tz)
 {
     const int nts = a.dims[0] * ty * tz;
+    if ((a.dims[0] & (a.dims[0] - 1)) && a.dagger) return cudaErrorInvalidConfiguration;
     if (a.dims[0] & (a.dims[0] - 1)) return nts == 96 ? launch_mrhs_n<RECON, NRB, 96, false>(a, ty, tz) : launch_mrhs_n<RECON, NRB, 0, false>(a, ty, tz);
     const Tuning &tn = a.tune ? *a.tune : default_tuning();
     if (nts == 128 && a.dims[0] == 32 && NRB == 3 && tn.mrhs_bulk > 0) return launch_mrhs_n<RECON, NRB, 128, true, true>(a, ty, tz);
+    // D^dagger = gamma5 D gamma5 (projector signs swapped): the default tile of a power-of-two Lx
+    if (a.dagger) return nts == 128 ? launch_mrhs_n<RECON, NRB, 128, true, false, +1>(a, ty, tz) : cudaErrorInvalidConfiguration;
     return nts == 128 ? launch_mrhs_n<RECON, NRB, 128, true>(a, ty, tz) : launch_mrhs_n<RECON, NRB, 0, true>(a, ty, tz);
 }
 

@@ -515,10 +515,11 @@ cudaError_t launch_stage(const ApplyArgs &a)
         if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
         if (s.nt <= 128) return launch_rloop(a, s.ty, s.tz);
     }
-    if (a.precision == 32 && a.recon != 8 && a.nrhs > 1 && !a.dagger && (tn.stage_no_mrhs < 0 ? pow2 : tn.stage_no_mrhs == 0)) {
+    if (a.precision == 32 && a.recon != 8 && a.nrhs > 1 && (tn.stage_no_mrhs < 0 ? pow2 : tn.stage_no_mrhs == 0)) {
         StageShape s;
         if (!stage_shape(a, s)) return cudaErrorInvalidConfiguration;
-        if (s.nt <= 128) return launch_mrhs(a, s.ty, s.tz); // (a forced bigger tile runs through the single-RHS kernel below)
+        // (D^dagger: the multi-RHS kernel has its sign-swapped member for the default 128-site tile of a power-of-two Lx)
+        if (s.nt <= 128 && (!a.dagger || (pow2 && s.nt == 128))) return launch_mrhs(a, s.ty, s.tz); // (a forced bigger tile runs through the single-RHS kernel below)
     }
     if (a.dims[0] == 32 && tn.stage_bulk > 0) { // bulk-copy member: one warp = one x-row = one layout block
         StageShape s;

@@ -345,11 +345,12 @@ def test_apply_dagger_matches_the_oracle_and_gamma5_hermiticity(oracle, dims, pr
 # ---------------------------------------------------------------- round 2: dagger / Lx = 24 / fp64 members of the staged family
 @pytest.mark.parametrize("dims", [(32, 4, 4, 5), (16, 8, 8, 6), (8, 4, 12, 6), (4, 4, 4, 4), (24, 4, 4, 6), (12, 8, 4, 3)])
 @pytest.mark.parametrize("precision,recon", [(64, 18), (32, 18), (32, 12), (64, 12)])
-@pytest.mark.parametrize("nrhs", [1, 3])
+@pytest.mark.parametrize("nrhs", [1, 3, 4, 8])
 def test_staged_dagger_matches_the_oracle(oracle, dims, precision, recon, nrhs):
     """wd_apply_dagger through the STAGED kernel (templated on the projector sign): D^dagger = gamma5 D gamma5
-     against the oracle's sign=+1 operator; several right-hand sides go through the single-RHS member in
-    the (patch, column, right-hand side) block order."""
+     against the oracle's sign=+1 operator; several right-hand sides go through the sign-swapped member of
+    the multi-RHS kernel (fp32, 128-site tiles of a power-of-two Lx; 4 = a full group + a single-RHS launch, 8 = two groups
+    + a pair) and otherwise through the single-RHS member in the (patch, column, right-hand side) block order."""
     import torch
     cfg = fields.Config("sdag", dims, precision, "haar", recon, -0.3, nrhs, 93)
     U, psi = fields.make_fields(cfg)
