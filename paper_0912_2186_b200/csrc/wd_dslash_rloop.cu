@@ -22,6 +22,12 @@
 // patch march through the same slices together and the links reach the later groups from L2.
 // The HBM streams (the spinor rows of the next slice, the link records of the next slice) are requested ahead of time by
 // one lane per warp with cp.async.bulk.prefetch.L2, so that the loads that need them are L2 hits.
+//
+// Measured (24 right-hand sides on 32^3 x 64, fp32, 18-real links; profiles/r02_ncu.md section 10): the LSU work per (site, rhs)
+// falls as planned (LSU pipe 68 % -> 50 % busy), but 206-236 registers per thread leave 8 warps per SM and the FMA pipe reaches
+// 40 % (ring member) / 31 % (plain loads): 3.6 / 4.4 ms against 3.1 ms for the 12-warp shared-memory member.  Selected by the
+// tuning variable mrhs_reg; the default route only for 8-real links with several right-hand sides on Lx = 32 (3.94 against
+// 4.19 ms: the rebuild is paid once per group).
 #include <cstdio>
 #include <cstdlib>
 #define WD_USE_F32X2 // packed FFMA2 SU(3) products (wd_math.cuh)
