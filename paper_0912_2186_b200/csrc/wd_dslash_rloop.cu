@@ -308,10 +308,12 @@ dslash_rloop_kernel(float *__restrict__ out, const float *__restrict__ in, const
 // Shared memory per CTA: ring 4 warps x 4 slots x 3 KB = 48 KB, exchange 24 KB, face links 10 KB, carried t products
 // 6 KB x rgrp: rgrp <= 5 for two CTAs per SM.
 constexpr int RING_ROWV = 6 * 32;                    // 16-byte vectors of one row slot
-constexpr int ring_smem_vecs(int rgrp) { return 4 * 4 * RING_ROWV + 2 * 2 * 3 * 128 + 2 * 5 * 64 + rgrp * 3 * 128; }
-constexpr size_t ring_smem_bytes(int rgrp) { return (size_t)ring_smem_vecs(rgrp) * 16 + 17 * 8; }
+// UNI ("uniform roles"): every thread also holds U_y, U_z of the sites below it in registers and does its own backward hops, so
+// that the four warps of a tile do the same number of SU(3) products per pass and no face links sit in shared memory
+constexpr int ring_smem_vecs(int rgrp, bool uni) { return 4 * 4 * RING_ROWV + 2 * 2 * 3 * 128 + (uni ? 0 : 2 * 5 * 64) + rgrp * 3 * 128; }
+constexpr size_t ring_smem_bytes(int rgrp, bool uni) { return (size_t)ring_smem_vecs(rgrp, uni) * 16 + 17 * 8; }
 
-template <int RECON, int SGN>
+template <int RECON, int SGN, bool UNI>
 __global__ void __launch_bounds__(128, 2)
 dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, const float *__restrict__ links, int Ly, int Lz, int Lt,
                          long long V, float cdiag, int nrhs, int rgrp, int nchunk, int patch)
@@ -325,7 +327,7 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
     float4 *const ring = smem + w * 4 * RING_ROWV;        // this warp's four row slots
     float4 *const exch = smem + 4 * 4 * RING_ROWV;        // [2 buffers][y, z][3][128]
     float4 *const fl = exch + 2 * 2 * 3 * nts;            // [y, z][5][64] face links (18 reals + 2 pad per site)
-    float4 *const carry = fl + 2 * 5 * 64;                // [rgrp][3][128]
+    float4 *const carry = fl + (UNI ? 0 : 2 * 5 * 64);    // [rgrp][3][128]
     unsigned long long *const mb0 = reinterpret_cast<unsigned long long *>(carry + rgrp * 3 * nts);
     unsigned long long *const mb = mb0 + w * 4; // this warp's four row slots
     unsigned long long *const xbar = mb0 + 16;  // the CTA's exchange barrier: arrive after the sends, wait before the receives
@@ -419,14 +421,19 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
         load_link<1, float, RECON>(links, s3 + toff, uy);
         load_link<2, float, RECON>(links, s3 + toff, uz);
         load_link<3, float, RECON>(links, s3 + toff, ut);
-        if (!yy) { // U_y of the out-of-tile site below: rebuilt once, read back per right-hand side
+        float uyb[18], uzb[18]; // UNI: U_y, U_z of the sites below (in the tile or not)
+        if (UNI) {
+            load_link<1, float, RECON>(links, (yy ? s3 - Lx : s3_y) + toff, uyb);
+            load_link<2, float, RECON>(links, (zz ? s3 - (long long)Lx * Ly : s3_z) + toff, uzb);
+        }
+        if (!UNI && !yy) { // U_y of the out-of-tile site below: rebuilt once, read back per right-hand side
             float uf[18];
             load_link<1, float, RECON>(links, s3_y + toff, uf);
 #pragma unroll
             for (int c = 0; c < 5; ++c)
                 fl[c * 64 + fl_y] = make_float4(uf[4 * c], uf[4 * c + 1], c < 4 ? uf[4 * c + 2] : 0.f, c < 4 ? uf[4 * c + 3] : 0.f);
         }
-        if (!zz) {
+        if (!UNI && !zz) {
             float uf[18];
             load_link<2, float, RECON>(links, s3_z + toff, uf);
 #pragma unroll
@@ -466,6 +473,9 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
             if (yy) { // the site below is in the tile: P psi for its forward hop
                 project<1, SGN>(psi, h);
                 sts_half(ey, nts, st, h);
+            } else if (UNI) { // the site above is in the tile: P psi for its backward hop (it holds this site's link)
+                project<1, -SGN>(psi, h);
+                sts_half(ey, nts, st, h);
             } else {  // the site above is in the tile: U_y^dag P psi for its backward hop
                 project<1, -SGN>(psi, h);
                 su3_dag_mul(uy, h, chi);
@@ -473,6 +483,9 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
             }
             if (zz) {
                 project<2, SGN>(psi, h);
+                sts_half(ez, nts, st, h);
+            } else if (UNI) {
+                project<2, -SGN>(psi, h);
                 sts_half(ez, nts, st, h);
             } else {
                 project<2, -SGN>(psi, h);
@@ -512,6 +525,10 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
                     project<1, SGN>(pn, h);
                     su3_mul(uy, h, chi);
                     reconstruct_add<1, SGN>(acc, chi);
+                } else if (UNI) {
+                    project<1, -SGN>(pn, h);
+                    su3_dag_mul(uyb, h, chi);
+                    reconstruct_add<1, -SGN>(acc, chi);
                 } else {
                     float uf[20];
 #pragma unroll
@@ -536,6 +553,10 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
                     project<2, SGN>(pn, h);
                     su3_mul(uz, h, chi);
                     reconstruct_add<2, SGN>(acc, chi);
+                } else if (UNI) {
+                    project<2, -SGN>(pn, h);
+                    su3_dag_mul(uzb, h, chi);
+                    reconstruct_add<2, -SGN>(acc, chi);
                 } else {
                     float uf[20];
 #pragma unroll
@@ -546,7 +567,11 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
                 }
             }
             mbar_wait(xbar, ph); // everybody's: the exchange buffer `buf` of this (slice, rhs) is complete
-            if (yy) {
+            if (yy && UNI) {
+                lds_half(ey, nts, st - 32, h);
+                su3_dag_mul(uyb, h, chi);
+                reconstruct_add<1, -SGN>(acc, chi);
+            } else if (yy) {
                 lds_half(ey, nts, st - 32, chi);
                 reconstruct_add<1, -SGN>(acc, chi);
             } else {
@@ -554,7 +579,11 @@ dslash_rloop_ring_kernel(float *__restrict__ out, const float *__restrict__ in, 
                 su3_mul(uy, h, chi);
                 reconstruct_add<1, SGN>(acc, chi);
             }
-            if (zz) {
+            if (zz && UNI) {
+                lds_half(ez, nts, st - 64, h);
+                su3_dag_mul(uzb, h, chi);
+                reconstruct_add<2, -SGN>(acc, chi);
+            } else if (zz) {
                 lds_half(ez, nts, st - 64, chi);
                 reconstruct_add<2, -SGN>(acc, chi);
             } else {
@@ -622,20 +651,20 @@ cudaError_t launch_rloop_s(const ApplyArgs &a, int ty, int tz)
     return cudaGetLastError();
 }
 
-template <int RECON, int SGN>
+template <int RECON, int SGN, bool UNI>
 cudaError_t launch_ring_s(const ApplyArgs &a)
 {
-    auto kern = dslash_rloop_ring_kernel<RECON, SGN>;
+    auto kern = dslash_rloop_ring_kernel<RECON, SGN, UNI>;
     const Tuning &tn = a.tune ? *a.tune : default_tuning();
-    int rmax = 5; // two CTAs per SM
+    int rmax = UNI ? 6 : 5; // two CTAs per SM
     if (tn.mrhs_rgrp >= 1) { // forced group size, up to what one CTA per SM can hold
-        const int rcap = (int)((227 * 1024 - ring_smem_bytes(0)) / (3 * 128 * 16));
+        const int rcap = (int)((227 * 1024 - ring_smem_bytes(0, UNI)) / (3 * 128 * 16));
         rmax = tn.mrhs_rgrp < rcap ? tn.mrhs_rgrp : rcap;
     }
     int ngroups = (a.nrhs + rmax - 1) / rmax;
     const int rgrp = (a.nrhs + ngroups - 1) / ngroups;
     ngroups = (a.nrhs + rgrp - 1) / rgrp;
-    const size_t smem = ring_smem_bytes(rgrp);
+    const size_t smem = ring_smem_bytes(rgrp, UNI);
     if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
     static size_t smem_set[64];
     cudaError_t e = ensure_dynamic_smem((const void *)kern, smem, smem_set);
@@ -661,7 +690,10 @@ template <int RECON> cudaError_t launch_rloop_r(const ApplyArgs &a, int ty, int 
 {
     const Tuning &tn = a.tune ? *a.tune : default_tuning();
     if (tn.mrhs_reg != 1 && a.dims[0] == 32 && ty == 2 && tz == 2) // the ring member wherever it applies
-        return a.dagger ? launch_ring_s<RECON, +1>(a) : launch_ring_s<RECON, -1>(a);
+    {
+        if (tn.mrhs_reg == 3 || tn.mrhs_reg < 0) return a.dagger ? launch_ring_s<RECON, +1, true>(a) : launch_ring_s<RECON, -1, true>(a);
+        return a.dagger ? launch_ring_s<RECON, +1, false>(a) : launch_ring_s<RECON, -1, false>(a);
+    }
     return a.dagger ? launch_rloop_s<RECON, +1>(a, ty, tz) : launch_rloop_s<RECON, -1>(a, ty, tz);
 }
 

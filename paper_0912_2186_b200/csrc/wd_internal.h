@@ -20,7 +20,8 @@ struct Tuning {
     int host_nslab = -1;            // WD_HOST_NSLAB    slabs of the pipelined wd_apply_host (3..32, default 16)
     int stage_bulk = -1;            // WD_STAGE_BULK    staged kernel on Lx = 32: 1 = bulk-copy member (wd_dslash_stage_bulk.cu), 0 = per-thread cp.async
     int mrhs_reg = -1;              // WD_MRHS_REG      multi-RHS member with the links in registers (wd_dslash_rloop.cu): 0 = never, 1 = plain-load
-                                    //                  member, 2 = ring member (Lx = 32; else plain-load); unset: 8-real links on Lx = 32 only
+                                    //                  member, 2 = ring member (Lx = 32; else plain-load), 3 = ring member with uniform roles;
+                                    //                  unset: 8-real links on Lx = 32 only (uniform-role ring)
     int mrhs_rgrp = -1;             // WD_MRHS_RGRP     right-hand sides per group of that member (default: what two CTAs per SM allow)
 };
 void tuning_from_env(Tuning &t);

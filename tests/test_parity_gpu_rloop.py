@@ -115,10 +115,12 @@ def test_rloop_deterministic(monkeypatch):
 
 
 # ---------------------------------------------------------------- the ring member (Lx = 32: warp-private cp.async.bulk row slots)
+# reg = "2": in-tile backward products formed at the source site; "3": uniform roles (every thread holds the links below it)
 @pytest.mark.parametrize("dims", [(32, 4, 4, 4), (32, 8, 8, 3), (32, 2, 2, 2), (32, 6, 10, 4), (32, 4, 2, 1)])
 @pytest.mark.parametrize("recon", [18, 12, 8])
-def test_ring_shapes(oracle, monkeypatch, dims, recon):
-    monkeypatch.setenv("WD_MRHS_REG", "2")
+@pytest.mark.parametrize("reg", ["2", "3"])
+def test_ring_shapes(oracle, monkeypatch, dims, recon, reg):
+    monkeypatch.setenv("WD_MRHS_REG", reg)
     for nrhs in (2, 7):
         run(oracle, fields.Config("ring", dims, 32, "haar", recon, -0.3, nrhs, 67))
 
@@ -126,8 +128,9 @@ def test_ring_shapes(oracle, monkeypatch, dims, recon):
 @pytest.mark.parametrize("rgrp", [None, "1", "3", "5", "1000"])
 @pytest.mark.parametrize("tc", ["1", "2", "5", "100"])
 @pytest.mark.parametrize("patch", ["0", "2"])
-def test_ring_groups_chunks_and_block_orders(oracle, monkeypatch, rgrp, tc, patch):
-    monkeypatch.setenv("WD_MRHS_REG", "2")
+@pytest.mark.parametrize("reg", ["2", "3"])
+def test_ring_groups_chunks_and_block_orders(oracle, monkeypatch, rgrp, tc, patch, reg):
+    monkeypatch.setenv("WD_MRHS_REG", reg)
     monkeypatch.setenv("WD_TILE_TC", tc)
     monkeypatch.setenv("WD_MRHS_PATCH", patch)
     if rgrp:
@@ -136,19 +139,22 @@ def test_ring_groups_chunks_and_block_orders(oracle, monkeypatch, rgrp, tc, patc
 
 
 @pytest.mark.parametrize("recon", [18, 12, 8])
-def test_ring_dagger(oracle, monkeypatch, recon):
-    monkeypatch.setenv("WD_MRHS_REG", "2")
+@pytest.mark.parametrize("reg", ["2", "3"])
+def test_ring_dagger(oracle, monkeypatch, recon, reg):
+    monkeypatch.setenv("WD_MRHS_REG", reg)
     run(oracle, fields.Config("ringd", (32, 4, 4, 6), 32, "haar", recon, -0.2, 4, 73), dagger=True)
 
 
-def test_ring_config4_full_size(oracle, monkeypatch):
-    monkeypatch.setenv("WD_MRHS_REG", "2")
+@pytest.mark.parametrize("reg", ["2", "3"])
+def test_ring_config4_full_size(oracle, monkeypatch, reg):
+    monkeypatch.setenv("WD_MRHS_REG", reg)
     run(oracle, fields.CONFIGS["c4_32x64_fp32_24rhs"])
 
 
-def test_ring_deterministic(monkeypatch):
+@pytest.mark.parametrize("reg", ["2", "3"])
+def test_ring_deterministic(monkeypatch, reg):
     import torch
-    monkeypatch.setenv("WD_MRHS_REG", "2")
+    monkeypatch.setenv("WD_MRHS_REG", reg)
     cfg = fields.Config("ringdet", (32, 8, 8, 8), 32, "smooth", 18, -0.42, 6, 79)
     U, psi = fields.make_fields(cfg)
     op = GpuOp(U, cfg.dims, 32, 18, STAGE)
