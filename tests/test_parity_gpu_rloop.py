@@ -89,10 +89,67 @@ def test_rloop_dagger(oracle, monkeypatch, recon):
     run(oracle, fields.Config("rloopd", (32, 4, 4, 6), 32, "haar", recon, -0.2, 4, 53), dagger=True)
 
 
-def test_rloop_config4_full_size(oracle, monkeypatch):
-    """BASELINE.json:configs[4] (32^3 x 64, 24 right-hand sides) in the launch configuration bench.py times."""
-    monkeypatch.setenv("WD_MRHS_REG", "1")
-    run(oracle, fields.CONFIGS["c4_32x64_fp32_24rhs"])
+@pytest.fixture(scope="module")
+def config4_reference():
+    """configs[4] inputs (seeded, fields.make_fields) packed on the device once for the three full-size tests below, and the
+    result of the default multi-RHS member on them (tests/test_parity_gpu.py checks that member against the oracle on all 24
+    right-hand sides)."""
+    import os
+    import torch
+    cfg = fields.CONFIGS["c4_32x64_fp32_24rhs"]
+    U, psi = fields.make_fields(cfg)
+    old = os.environ.get("WD_MRHS_REG")
+    os.environ["WD_MRHS_REG"] = "0"
+    try:
+        op = GpuOp(U, cfg.dims, 32, cfg.recon, STAGE)
+    finally:
+        if old is None:
+            del os.environ["WD_MRHS_REG"]
+        else:
+            os.environ["WD_MRHS_REG"] = old
+    w = op.op
+    canon = torch.from_numpy(psi).cuda()
+    native_in = torch.full((w.native_numel(cfg.nrhs),), float("nan"), dtype=canon.dtype, device="cuda")
+    ref = torch.full_like(native_in, float("nan"))
+    w.pack(native_in, canon, cfg.nrhs)
+    w.apply(ref, native_in, cfg.mass, cfg.nrhs)
+    torch.cuda.synchronize()
+    del canon
+    op.close()
+    yield cfg, U, psi, native_in, ref
+    del native_in, ref
+    torch.cuda.empty_cache()
+
+
+def full_size_config4(oracle, monkeypatch, reg, reference):
+    """BASELINE.json:configs[4] (32^3 x 64, 24 right-hand sides) in the launch configuration bench.py times: all 24 right-hand
+    sides against the default multi-RHS member (compared on the device, in the native layout), and right-hand sides 0, 5, 11,
+    12, 23 (first / last of a group for every group size in use) element by element against the oracle."""
+    import torch
+    cfg, U, psi, native_in, ref = reference
+    monkeypatch.setenv("WD_MRHS_REG", reg)
+    op = GpuOp(U, cfg.dims, 32, cfg.recon, STAGE)
+    w = op.op
+    got = torch.full_like(native_in, float("nan"))
+    w.apply(got, native_in, cfg.mass, cfg.nrhs)
+    n1 = w.native_numel(1)
+    for r in range(cfg.nrhs):
+        g, f = got[r * n1:(r + 1) * n1].double(), ref[r * n1:(r + 1) * n1].double()
+        live = torch.isfinite(f)                       # pad sites of the native layout are never written
+        assert bool(torch.isfinite(g[live]).all())
+        assert float(torch.linalg.vector_norm(g[live] - f[live]) / torch.linalg.vector_norm(f[live])) <= TOL[32], r
+    Lx, Ly, Lz, Lt = cfg.dims
+    canon = torch.full((cfg.nrhs, Lt, Lz, Ly, Lx, 4, 3, 2), float("nan"), dtype=got.dtype, device="cuda")
+    w.unpack(canon, got, cfg.nrhs)
+    torch.cuda.synchronize()
+    op.close()
+    U64 = U.astype(np.float64)
+    for r in (0, 5, 11, 12, 23):
+        assert rel_l2(canon[r].cpu().numpy(), oracle.apply(psi[r].astype(np.float64), U64, cfg.dims, cfg.mass)) <= TOL[32], r
+
+
+def test_rloop_config4_full_size(oracle, monkeypatch, config4_reference):
+    full_size_config4(oracle, monkeypatch, "1", config4_reference)
 
 
 def test_rloop_nv20_on_the_paper_volume_shape(oracle, monkeypatch):
@@ -146,9 +203,8 @@ def test_ring_dagger(oracle, monkeypatch, recon, reg):
 
 
 @pytest.mark.parametrize("reg", ["2", "3"])
-def test_ring_config4_full_size(oracle, monkeypatch, reg):
-    monkeypatch.setenv("WD_MRHS_REG", reg)
-    run(oracle, fields.CONFIGS["c4_32x64_fp32_24rhs"])
+def test_ring_config4_full_size(oracle, monkeypatch, config4_reference, reg):
+    full_size_config4(oracle, monkeypatch, reg, config4_reference)
 
 
 @pytest.mark.parametrize("reg", ["2", "3"])
